@@ -1,0 +1,7 @@
+"""FP64 CPU oracle for the CPRA loop -- TEST INFRASTRUCTURE (see cpra_oracle.c header).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It shares no code with paper_2402_05283_b200/ and never imports it."""
+from .cpra_oracle import Oracle, build_oracle, dft2_naive, fft2, hio, mix, modulus
+
+__all__ = ["Oracle", "build_oracle", "dft2_naive", "fft2", "hio", "mix", "modulus"]

@@ -1,0 +1,559 @@
+/*
+ * oracle/cpra_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, obviously-correct CPU implementation of the CPRA iteration loop
+ * (arXiv 2402.05283, "Real time 3D coherent X-ray diffraction imaging"), written from
+ * /root/reference/PAPER.md (cited as P:<line>) and the readings listed in DESIGN.md.
+ * It is the parity oracle for the CUDA path and shares NO code with it.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load it.
+ *
+ * Precision: every real number is `real` = double (liboracle.so).  The same source compiled with
+ * -DORACLE_REAL=float (liboracle_f32.so) is used ONLY to show how far an fp32 state drifts from
+ * the fp64 one over 20 iterations ("hard parts"); it is never the reference.
+ *
+ * What is computed, in the paper's order (one call oracle_iterate(k, beta) repeats k times):
+ *   1. carousel mix, Eq. (4):  ghat_n = sum_{j=-K..K} alpha_|j| g_{(n+j) mod Np}
+ *      (Jacobi: all right-hand sides from the state before the step; fires iff t mod n_ei == 0)
+ *   2. forward 2D FT, Eq. (3):     G_n = F[ghat_n]      (e^{-2 pi i ...}, unnormalised)
+ *   3. error:                      num_n = sum_{M=1} (|G_n| - A_n)^2, E_n = sqrt(num_n/den_n)
+ *   4. Fourier-modulus constraint, P:13, P:25, P:98:
+ *                                        measured: G' = A G/|G| (G' = A if |G| = 0); masked: G' = G
+ *   5. inverse 2D FT:              g'_n = F^-1[G'_n]    (e^{+2 pi i ...} / N^2)
+ *   6. support / HIO, P:98 ref [22], P:104 (beta):
+ *                                        S=1: g_n <- g'_n ;  S=0: g_n <- ghat_n - beta g'_n
+ *   7. t <- t + 1
+ * plus the one-shot Fourier-slice assembly of Step D's first sentence; the
+ * interpolation scheme is the polar bilinear gather of DESIGN.md (the paper only says
+ * "interpolate"): PARITY UNPINNED for the interpolation error itself.
+ *
+ * Pins (tests/test_oracle_*.py): brute-force O(N^4) DFT below (separate code path), numpy.fft,
+ * Parseval, shift theorem, Fourier-slice identity, idempotence of the two projections, closed-form
+ * HIO decay, circulant eigenvalues of the mix, fixed point of the true object, error closed forms.
+ * Full multi-iteration trajectories have no external pin: PARITY UNPINNED beyond those invariants.
+ *
+ * Layout: images row-major [n][y][x], x fastest; complex = interleaved (re, im).  All I/O arrays of
+ * this library are double / interleaved double regardless of `real`.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifndef ORACLE_REAL
+#define ORACLE_REAL double
+#endif
+typedef ORACLE_REAL real;
+typedef struct { real re, im; } cplx;
+
+#define ORACLE_OK 0
+#define ORACLE_ERR_INVALID_ARG (-1)
+#define ORACLE_ERR_UNSUPPORTED_SIZE (-2)
+#define ORACLE_ERR_NOT_READY (-3)
+
+static const double PI = 3.14159265358979323846264338327950288;
+
+/* ------------------------------------------------------------------------------------------ */
+/* Fourier transforms                                                                          */
+/* ------------------------------------------------------------------------------------------ */
+
+/* Textbook iterative radix-2 decimation-in-time FFT, in place, N a power of two.
+ * tw[m] = e^{sign 2 pi i m / N}, m = 0..N/2-1 (computed in double by twiddle_table, rounded once).
+ * sign = -1: X[k] = sum_x x[x] e^{-2 pi i k x / N};  sign = +1: e^{+...}; never scaled here. */
+static void fft1d(cplx* a, int N, const cplx* tw)
+{
+    /* bit-reversal permutation */
+    for (int i = 1, j = 0; i < N; ++i) {
+        int bit = N >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) { cplx t = a[i]; a[i] = a[j]; a[j] = t; }
+    }
+    for (int len = 2; len <= N; len <<= 1) {
+        const int half = len >> 1, step = N / len;
+        for (int i = 0; i < N; i += len) {
+            for (int k = 0; k < half; ++k) {
+                const real wr = tw[k * step].re, wi = tw[k * step].im;   /* e^{sign 2 pi i k/len} */
+                const cplx u = a[i + k], v = a[i + k + half];
+                const real tr = v.re * wr - v.im * wi;
+                const real ti = v.re * wi + v.im * wr;
+                a[i + k].re = u.re + tr;        a[i + k].im = u.im + ti;
+                a[i + k + half].re = u.re - tr; a[i + k + half].im = u.im - ti;
+            }
+        }
+    }
+}
+
+static cplx* twiddle_table(int N, int sign)
+{
+    cplx* tw = (cplx*)malloc(sizeof(cplx) * (size_t)(N / 2 + 1));
+    for (int m = 0; m < N / 2; ++m) {
+        const double ang = sign * 2.0 * PI * (double)m / (double)N;
+        tw[m].re = (real)cos(ang); tw[m].im = (real)sin(ang);
+    }
+    return tw;
+}
+
+/* 2D transform of one N x N image, in place: all rows, then all columns (Eq. (3) is a
+ * separable double sum).  sign=+1 additionally divides by N^2 (P:19 inverse FT; reading A10). */
+static void fft2d(cplx* img, int N, int sign)
+{
+    cplx* col = (cplx*)malloc(sizeof(cplx) * (size_t)N);
+    cplx* tw = twiddle_table(N, sign);
+    for (int y = 0; y < N; ++y) fft1d(img + (size_t)y * N, N, tw);
+    for (int x = 0; x < N; ++x) {
+        for (int y = 0; y < N; ++y) col[y] = img[(size_t)y * N + x];
+        fft1d(col, N, tw);
+        for (int y = 0; y < N; ++y) img[(size_t)y * N + x] = col[y];
+    }
+    free(col); free(tw);
+    if (sign > 0) {
+        const real s = (real)(1.0 / ((double)N * (double)N));
+        for (size_t i = 0; i < (size_t)N * N; ++i) { img[i].re *= s; img[i].im *= s; }
+    }
+}
+
+/* Brute-force definition, O(N^4), its own code path (no FFT, no shared twiddle logic), always in
+ * double: out[ky][kx] = sum_{y,x} in[y][x] e^{sign 2 pi i (ky y + kx x)/N}  (/N^2 if sign=+1). */
+int oracle_dft2_naive(const double* in, double* out, int N, int sign)
+{
+    if (!in || !out || N < 1 || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    for (int ky = 0; ky < N; ++ky)
+        for (int kx = 0; kx < N; ++kx) {
+            double sr = 0.0, si = 0.0;
+            for (int y = 0; y < N; ++y)
+                for (int x = 0; x < N; ++x) {
+                    const long m = ((long)ky * y + (long)kx * x) % N;
+                    const double ang = sign * 2.0 * PI * (double)m / (double)N;
+                    const double c = cos(ang), s = sin(ang);
+                    const double ar = in[2 * ((size_t)y * N + x)], ai = in[2 * ((size_t)y * N + x) + 1];
+                    sr += ar * c - ai * s;
+                    si += ar * s + ai * c;
+                }
+            if (sign > 0) { sr /= (double)N * N; si /= (double)N * N; }
+            out[2 * ((size_t)ky * N + kx)] = sr;
+            out[2 * ((size_t)ky * N + kx) + 1] = si;
+        }
+    return ORACLE_OK;
+}
+
+static int is_pow2(int N) { return N > 0 && (N & (N - 1)) == 0; }
+
+/* Exported FFT of a stack of `count` images (double I/O), the routine the loop itself uses. */
+int oracle_fft2(const double* in, double* out, int N, int count, int sign)
+{
+    if (!in || !out || !is_pow2(N) || count < 0 || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N;
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int n = 0; n < count; ++n) {
+        cplx* buf = (cplx*)malloc(sizeof(cplx) * px);
+        for (size_t i = 0; i < px; ++i) {
+            buf[i].re = (real)in[2 * (n * px + i)];
+            buf[i].im = (real)in[2 * (n * px + i) + 1];
+        }
+        fft2d(buf, N, sign);
+        for (size_t i = 0; i < px; ++i) {
+            out[2 * (n * px + i)] = (double)buf[i].re;
+            out[2 * (n * px + i) + 1] = (double)buf[i].im;
+        }
+        free(buf);
+    }
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* The three pointwise operators, as the loop uses them                                        */
+/* ------------------------------------------------------------------------------------------ */
+
+/* Eq. (4), reading A1 (weights on n+-1, n+-2, ...; periodic in n) and A4 (Jacobi):
+ * out_n = sum_{j=-K}^{K} alpha_|j| in_{(n+j) mod Np}.  in and out must not alias. */
+static void mix_stack(const cplx* in, cplx* out, int Np, size_t px, int K, const real* alpha)
+{
+    #pragma omp parallel for schedule(static)
+    for (int n = 0; n < Np; ++n) {
+        cplx* o = out + (size_t)n * px;
+        for (size_t i = 0; i < px; ++i) { o[i].re = 0; o[i].im = 0; }
+        for (int j = -K; j <= K; ++j) {
+            const int m = ((n + j) % Np + Np) % Np;
+            const real a = alpha[j < 0 ? -j : j];
+            const cplx* s = in + (size_t)m * px;
+            for (size_t i = 0; i < px; ++i) { o[i].re += a * s[i].re; o[i].im += a * s[i].im; }
+        }
+    }
+}
+
+/* Fourier-modulus constraint on one image in native order (only |E|^2 = I is
+ * measured; beamstop pixels are unmeasured).  Readings A12 (masked: G' = G) and A13
+ * (|G| = 0: phase 0).  Returns num = sum_{M=1} (|G| - A)^2 of the INPUT G (error, reading A9). */
+static double modulus_image(cplx* G, const real* A, const unsigned char* M, size_t px)
+{
+    double num = 0.0;
+    for (size_t i = 0; i < px; ++i) {
+        if (!M[i]) continue;
+        const real mag = (real)sqrt((double)(G[i].re * G[i].re + G[i].im * G[i].im));
+        const real d = mag - A[i];
+        num += (double)(d * d);
+        if (mag > 0) {
+            const real s = A[i] / mag;
+            G[i].re *= s; G[i].im *= s;
+        } else {
+            G[i].re = A[i]; G[i].im = 0;
+        }
+    }
+    return num;
+}
+
+/* Support / HIO update on one image (Fienup's hybrid input-output, P:98 ref [22]; beta P:104;
+ * readings A6, A7: fixed support, no positivity, complex componentwise):
+ *   S=1: g <- g' ;  S=0: g <- ghat - beta g'.   ghat is overwritten with the new g. */
+static void hio_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px, real beta)
+{
+    for (size_t i = 0; i < px; ++i) {
+        if (S[i]) { ghat[i] = gp[i]; }
+        else { ghat[i].re -= beta * gp[i].re; ghat[i].im -= beta * gp[i].im; }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Plan / state                                                                                */
+/* ------------------------------------------------------------------------------------------ */
+typedef struct oracle_plan_s {
+    int N, Np;
+    size_t px;
+    real* A;              /* [Np][N][N] sqrt(max(I,0)), native (unshifted) order */
+    unsigned char* M;     /* [Np][N][N] 1 = measured, native order */
+    unsigned char* S;     /* [Np][N][N] 1 = inside the support */
+    double* den;          /* [Np] sum_{M=1} I */
+    double* angles;       /* [Np] */
+    cplx* g;              /* state */
+    cplx* tmp;            /* mixed copy ghat */
+    int K; real alpha[64]; int n_ei;
+    long t;
+    double* E; double Eglobal;
+    int have_data, have_support, have_estimate, have_error;
+} oracle_plan_s;
+typedef oracle_plan_s* oracle_plan_t;
+
+int oracle_plan(oracle_plan_t* out, int N, int Np)
+{
+    if (!out) return ORACLE_ERR_INVALID_ARG;
+    if (!is_pow2(N) || N < 2 || N > 4096 || Np < 1) return ORACLE_ERR_UNSUPPORTED_SIZE;
+    oracle_plan_t p = (oracle_plan_t)calloc(1, sizeof(*p));
+    p->N = N; p->Np = Np; p->px = (size_t)N * N;
+    const size_t tot = p->px * (size_t)Np;
+    p->A = (real*)calloc(tot, sizeof(real));
+    p->M = (unsigned char*)calloc(tot, 1);
+    p->S = (unsigned char*)calloc(tot, 1);
+    p->den = (double*)calloc((size_t)Np, sizeof(double));
+    p->angles = (double*)calloc((size_t)Np, sizeof(double));
+    p->g = (cplx*)calloc(tot, sizeof(cplx));
+    p->tmp = (cplx*)calloc(tot, sizeof(cplx));
+    p->E = (double*)calloc((size_t)Np, sizeof(double));
+    /* reading A2: the paper's example weights */
+    p->K = 1; p->alpha[0] = (real)0.6; p->alpha[1] = (real)0.2; p->n_ei = 1;
+    *out = p;
+    return ORACLE_OK;
+}
+
+int oracle_destroy(oracle_plan_t p)
+{
+    if (!p) return ORACLE_ERR_INVALID_ARG;
+    free(p->A); free(p->M); free(p->S); free(p->den); free(p->angles);
+    free(p->g); free(p->tmp); free(p->E); free(p);
+    return ORACLE_OK;
+}
+
+/* I: [Np][N][N] detector-centred (DC at index N/2); mask likewise, NULL = all measured.
+ * A = sqrt(max(I,0)) (reading A14), moved to native order (ifftshift, reading A11);
+ * den_n = sum_{M=1} I_n (clamped I). */
+int oracle_set_data(oracle_plan_t p, const double* I, const unsigned char* mask, const double* angles)
+{
+    if (!p || !I) return ORACLE_ERR_INVALID_ARG;
+    const int N = p->N, h = N / 2;
+    for (int n = 0; n < p->Np; ++n) {
+        double den = 0.0;
+        for (int y = 0; y < N; ++y)
+            for (int x = 0; x < N; ++x) {
+                const size_t src = (size_t)n * p->px + (size_t)y * N + x;              /* centred */
+                const size_t dst = (size_t)n * p->px + (size_t)((y + h) % N) * N + ((x + h) % N);
+                const double v = I[src] > 0.0 ? I[src] : 0.0;
+                const unsigned char m = mask ? (mask[src] ? 1 : 0) : 1;
+                p->A[dst] = (real)sqrt(v);
+                p->M[dst] = m;
+                if (m) den += v;
+            }
+        p->den[n] = den;
+        p->angles[n] = angles ? angles[n] : 0.0;
+    }
+    p->have_data = 1;
+    return ORACLE_OK;
+}
+
+int oracle_set_support(oracle_plan_t p, const unsigned char* S)
+{
+    if (!p || !S) return ORACLE_ERR_INVALID_ARG;
+    const size_t tot = p->px * (size_t)p->Np;
+    for (size_t i = 0; i < tot; ++i) p->S[i] = S[i] ? 1 : 0;
+    p->have_support = 1;
+    return ORACLE_OK;
+}
+
+int oracle_set_carousel(oracle_plan_t p, int K, const double* alpha, int n_ei)
+{
+    if (!p || !alpha || K < 0 || K > 63 || 2 * K + 1 > p->Np || n_ei < 1) return ORACLE_ERR_INVALID_ARG;
+    p->K = K;
+    for (int j = 0; j <= K; ++j) p->alpha[j] = (real)alpha[j];    /* reading A2: not renormalised */
+    p->n_ei = n_ei;
+    return ORACLE_OK;
+}
+
+/* g0: interleaved complex double [Np][N][N]; resets t = 0. */
+int oracle_set_estimate(oracle_plan_t p, const double* g0)
+{
+    if (!p || !g0) return ORACLE_ERR_INVALID_ARG;
+    const size_t tot = p->px * (size_t)p->Np;
+    for (size_t i = 0; i < tot; ++i) { p->g[i].re = (real)g0[2 * i]; p->g[i].im = (real)g0[2 * i + 1]; }
+    p->t = 0; p->have_estimate = 1; p->have_error = 0;
+    return ORACLE_OK;
+}
+
+int oracle_set_iteration(oracle_plan_t p, long t) { if (!p || t < 0) return ORACLE_ERR_INVALID_ARG; p->t = t; return ORACLE_OK; }
+long oracle_get_iteration(oracle_plan_t p) { return p ? p->t : -1; }
+
+int oracle_iterate(oracle_plan_t p, int k, double beta_d)
+{
+    if (!p || k < 0 || !isfinite(beta_d)) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_data || !p->have_support || !p->have_estimate) return ORACLE_ERR_NOT_READY;
+    const real beta = (real)beta_d;
+    const size_t px = p->px;
+    const int N = p->N, Np = p->Np;
+    for (int it = 0; it < k; ++it) {
+        /* 1. mix (Eq. (4)) at the start of an episode; otherwise ghat = g */
+        const int do_mix = (p->t % p->n_ei) == 0;
+        if (do_mix) {
+            mix_stack(p->g, p->tmp, Np, px, p->K, p->alpha);
+            cplx* sw = p->g; p->g = p->tmp; p->tmp = sw;            /* p->g now holds ghat */
+        }
+        double numtot = 0.0, dentot = 0.0;
+        #pragma omp parallel for schedule(dynamic, 1) reduction(+:numtot, dentot)
+        for (int n = 0; n < Np; ++n) {
+            cplx* ghat = p->g + (size_t)n * px;
+            cplx* G = (cplx*)malloc(sizeof(cplx) * px);
+            memcpy(G, ghat, sizeof(cplx) * px);
+            fft2d(G, N, -1);                                                     /* 2 */
+            const double num = modulus_image(G, p->A + (size_t)n * px, p->M + (size_t)n * px, px); /* 3, 4 */
+            fft2d(G, N, +1);                                                     /* 5 */
+            hio_image(ghat, G, p->S + (size_t)n * px, px, beta);                 /* 6 */
+            free(G);
+            p->E[n] = p->den[n] > 0.0 ? sqrt(num / p->den[n]) : 0.0;
+            numtot += num; dentot += p->den[n];
+        }
+        p->Eglobal = dentot > 0.0 ? sqrt(numtot / dentot) : 0.0;
+        p->have_error = 1;
+        p->t += 1;                                                               /* 7 */
+    }
+    return ORACLE_OK;
+}
+
+int oracle_get_error(oracle_plan_t p, double* E, double* Eglobal)
+{
+    if (!p) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_error) return ORACLE_ERR_NOT_READY;
+    if (E) memcpy(E, p->E, sizeof(double) * (size_t)p->Np);
+    if (Eglobal) *Eglobal = p->Eglobal;
+    return ORACLE_OK;
+}
+
+/* which = 0: the iterate g; which = 1: S.g (the estimate restricted to the support). */
+int oracle_get_projections(oracle_plan_t p, int which, double* out)
+{
+    if (!p || !out || (which != 0 && which != 1)) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_estimate) return ORACLE_ERR_NOT_READY;
+    const size_t tot = p->px * (size_t)p->Np;
+    for (size_t i = 0; i < tot; ++i) {
+        const int keep = which == 0 || p->S[i];
+        out[2 * i] = keep ? (double)p->g[i].re : 0.0;
+        out[2 * i + 1] = keep ? (double)p->g[i].im : 0.0;
+    }
+    return ORACLE_OK;
+}
+
+/* Stand-alone entry points for the pins: the very functions the loop calls. */
+int oracle_mix(const double* in, double* out, int N, int Np, int K, const double* alpha)
+{
+    if (!in || !out || !alpha || K < 0 || K > 63 || 2 * K + 1 > Np) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N, tot = px * Np;
+    cplx* a = (cplx*)malloc(sizeof(cplx) * tot); cplx* b = (cplx*)malloc(sizeof(cplx) * tot);
+    real al[64];
+    for (int j = 0; j <= K; ++j) al[j] = (real)alpha[j];
+    for (size_t i = 0; i < tot; ++i) { a[i].re = (real)in[2 * i]; a[i].im = (real)in[2 * i + 1]; }
+    mix_stack(a, b, Np, px, K, al);
+    for (size_t i = 0; i < tot; ++i) { out[2 * i] = b[i].re; out[2 * i + 1] = b[i].im; }
+    free(a); free(b);
+    return ORACLE_OK;
+}
+
+/* G (native order, interleaved double, in place), A and M native order; returns num via *num. */
+int oracle_modulus(double* G, const double* A, const unsigned char* M, int N, double* num)
+{
+    if (!G || !A || !M) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N;
+    cplx* g = (cplx*)malloc(sizeof(cplx) * px); real* a = (real*)malloc(sizeof(real) * px);
+    for (size_t i = 0; i < px; ++i) { g[i].re = (real)G[2 * i]; g[i].im = (real)G[2 * i + 1]; a[i] = (real)A[i]; }
+    const double s = modulus_image(g, a, M, px);
+    for (size_t i = 0; i < px; ++i) { G[2 * i] = g[i].re; G[2 * i + 1] = g[i].im; }
+    if (num) *num = s;
+    free(g); free(a);
+    return ORACLE_OK;
+}
+
+/* ghat (in place -> new g), gp = g', S. */
+int oracle_hio(double* ghat, const double* gp, const unsigned char* S, int N, double beta)
+{
+    if (!ghat || !gp || !S) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N;
+    cplx* a = (cplx*)malloc(sizeof(cplx) * px); cplx* b = (cplx*)malloc(sizeof(cplx) * px);
+    for (size_t i = 0; i < px; ++i) {
+        a[i].re = (real)ghat[2 * i]; a[i].im = (real)ghat[2 * i + 1];
+        b[i].re = (real)gp[2 * i]; b[i].im = (real)gp[2 * i + 1];
+    }
+    hio_image(a, b, S, px, (real)beta);
+    for (size_t i = 0; i < px; ++i) { ghat[2 * i] = a[i].re; ghat[2 * i + 1] = a[i].im; }
+    free(a); free(b);
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Fourier-slice assembly (first sentence of Step D; Fourier slice theorem P:35-44)      */
+/* ------------------------------------------------------------------------------------------ */
+/*
+ * Geometry (reading A18): rotation about z, arrays O[z][y][x], P_n[z][u],
+ *   x = u cos(th) - s sin(th), y = u sin(th) + s cos(th)  =>
+ *   F2[P_n](kz, ku) = F3[O](kz, ky = ku sin(th_n), kx = ku cos(th_n)).
+ * Steps (reading A17 -- the paper only says "interpolate"):
+ *  (i)   E_n = F2[S_n g_n]; multiply by (-1)^(kz+ku): moves the real-space origin to the centre
+ *        pixel (N/2, N/2), so that the spectrum of a centred object is smooth.
+ *  (ii)  every slice is two rays from the origin: direction th_n (ku >= 0) and th_n + pi
+ *        (ku <= 0).  Sort the 2 Np directions on [0, 2 pi); directions closer than 1e-9 rad are
+ *        one ray whose samples are the mean of the contributors.
+ *  (iii) voxel (kz,ky,kx), signed integer frequencies in [-N/2, N/2): rho = sqrt(kx^2+ky^2),
+ *        phi = atan2(ky,kx) mod 2 pi.  rho > N/2-1: value 0, weight 0.  rho = 0: mean of all
+ *        slices' DC sample at that kz.  Otherwise bilinear in (phi, rho) between the two rays
+ *        bracketing phi (periodic) and the radial samples floor(rho), floor(rho)+1; weight 1.
+ *  (iv)  multiply by (-1)^(kx+ky+kz), store at native indices (k mod N): comparable to fftn(O)
+ *        of an object centred at (N/2,N/2,N/2).
+ * vol: interleaved complex double [N][N][N] (kz,ky,kx); weight: [N][N][N] double or NULL.
+ */
+typedef struct { double phi; int n; int neg; } ray_t;
+static int ray_cmp(const void* a, const void* b)
+{
+    const ray_t* x = (const ray_t*)a; const ray_t* y = (const ray_t*)b;
+    if (x->phi < y->phi) return -1;
+    if (x->phi > y->phi) return 1;
+    return (x->n > y->n) - (x->n < y->n);
+}
+
+int oracle_assemble_3d(oracle_plan_t p, double* vol, double* weight)
+{
+    if (!p || !vol) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_estimate || !p->have_support || !p->have_data) return ORACLE_ERR_NOT_READY;
+    const int N = p->N, Np = p->Np, h = N / 2;
+    const size_t px = p->px;
+
+    /* (i) spectra of the supported estimates, origin moved to the centre pixel */
+    cplx* E = (cplx*)malloc(sizeof(cplx) * px * (size_t)Np);
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int n = 0; n < Np; ++n) {
+        cplx* e = E + (size_t)n * px;
+        for (size_t i = 0; i < px; ++i) {
+            const size_t gi = (size_t)n * px + i;
+            if (p->S[gi]) e[i] = p->g[gi]; else { e[i].re = 0; e[i].im = 0; }
+        }
+        fft2d(e, N, -1);
+        for (int kz = 0; kz < N; ++kz)
+            for (int ku = 0; ku < N; ++ku)
+                if ((kz + ku) & 1) { e[(size_t)kz * N + ku].re = -e[(size_t)kz * N + ku].re;
+                                     e[(size_t)kz * N + ku].im = -e[(size_t)kz * N + ku].im; }
+    }
+
+    /* (ii) rays: sorted unique directions, each with its contributors [start, start+count) */
+    const int R2 = 2 * Np;
+    ray_t* rays = (ray_t*)malloc(sizeof(ray_t) * (size_t)R2);
+    for (int n = 0; n < Np; ++n)
+        for (int neg = 0; neg < 2; ++neg) {
+            double ph = fmod(p->angles[n] + (neg ? PI : 0.0), 2.0 * PI);
+            if (ph < 0.0) ph += 2.0 * PI;
+            if (ph >= 2.0 * PI - 1e-9) ph = 0.0;          /* 2 pi is the direction 0 */
+            rays[2 * n + neg].phi = ph; rays[2 * n + neg].n = n; rays[2 * n + neg].neg = neg;
+        }
+    qsort(rays, (size_t)R2, sizeof(ray_t), ray_cmp);
+    int* ustart = (int*)malloc(sizeof(int) * (size_t)(R2 + 1));
+    double* uphi = (double*)malloc(sizeof(double) * (size_t)R2);
+    int U = 0;
+    for (int i = 0; i < R2; ++i) {
+        if (U == 0 || rays[i].phi - uphi[U - 1] > 1e-9) { ustart[U] = i; uphi[U] = rays[i].phi; ++U; }
+    }
+    ustart[U] = R2;
+
+    /* (iii)+(iv) gather */
+    #pragma omp parallel for schedule(static)
+    for (int iz = 0; iz < N; ++iz) {
+        const int kz = iz < h ? iz : iz - N;
+        for (int iy = 0; iy < N; ++iy) {
+            const int ky = iy < h ? iy : iy - N;
+            for (int ix = 0; ix < N; ++ix) {
+                const int kx = ix < h ? ix : ix - N;
+                const size_t o = ((size_t)iz * N + iy) * N + ix;
+                const double rho = sqrt((double)kx * kx + (double)ky * ky);
+                double vr = 0.0, vi = 0.0, w = 0.0;
+                if (rho == 0.0) {
+                    for (int n = 0; n < Np; ++n) { vr += E[(size_t)n * px + (size_t)iz * N].re; vi += E[(size_t)n * px + (size_t)iz * N].im; }
+                    vr /= Np; vi /= Np; w = 1.0;
+                } else if (rho <= (double)(h - 1)) {
+                    double phi = atan2((double)ky, (double)kx);
+                    if (phi < 0.0) phi += 2.0 * PI;
+                    /* bracket: largest a with uphi[a] <= phi (periodic) */
+                    int a = -1;
+                    for (int lo = 0, hi = U - 1; lo <= hi;) {
+                        const int mid = (lo + hi) / 2;
+                        if (uphi[mid] <= phi) { a = mid; lo = mid + 1; } else hi = mid - 1;
+                    }
+                    double pa, pb; int b;
+                    if (a < 0) { a = U - 1; pa = uphi[a] - 2.0 * PI; } else pa = uphi[a];
+                    b = a + 1;
+                    if (b >= U) { b = 0; pb = uphi[0] + 2.0 * PI; } else pb = uphi[b];
+                    const double wp = (pb > pa) ? (phi - pa) / (pb - pa) : 0.0;
+                    const int r0 = (int)floor(rho);
+                    const double wr = rho - (double)r0;
+                    const int ur[2] = { a, b };
+                    const double wphi[2] = { 1.0 - wp, wp };
+                    for (int q = 0; q < 2; ++q) {
+                        if (wphi[q] == 0.0) continue;
+                        const int u = ur[q];
+                        const int cnt = ustart[u + 1] - ustart[u];
+                        for (int rr = 0; rr < 2; ++rr) {
+                            const double wrr = rr ? wr : 1.0 - wr;
+                            if (wrr == 0.0) continue;
+                            const int r = r0 + rr;
+                            double sr = 0.0, si = 0.0;
+                            for (int c = ustart[u]; c < ustart[u + 1]; ++c) {
+                                const int ku = rays[c].neg ? -r : r;
+                                const int iu = ((ku % N) + N) % N;
+                                const cplx e = E[(size_t)rays[c].n * px + (size_t)iz * N + iu];
+                                sr += e.re; si += e.im;
+                            }
+                            vr += wphi[q] * wrr * sr / cnt;
+                            vi += wphi[q] * wrr * si / cnt;
+                        }
+                    }
+                    w = 1.0;
+                }
+                if ((kx + ky + kz) & 1) { vr = -vr; vi = -vi; }
+                vol[2 * o] = vr; vol[2 * o + 1] = vi;
+                if (weight) weight[o] = w;
+            }
+        }
+    }
+    free(E); free(rays); free(ustart); free(uphi);
+    return ORACLE_OK;
+}
+
+const char* oracle_real_name(void) { return sizeof(real) == 8 ? "f64" : "f32"; }

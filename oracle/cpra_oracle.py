@@ -1,0 +1,190 @@
+"""ctypes binding of oracle/cpra_oracle.c -- TEST INFRASTRUCTURE (see the C file's header).
+
+`Oracle(N, Np)` mirrors the product's C ABI (cpra_plan / set_data / set_support / set_carousel /
+set_estimate / iterate / get_error / get_projections / assemble_3d) with host numpy arrays, FP64
+internally.  `Oracle(..., precision="f32")` loads the float build of the same source, used only to
+report the drift of an fp32 state next to the GPU's; it is never the reference.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBS = {}
+
+
+def build_oracle(force: bool = False) -> dict:
+    """gcc-compile cpra_oracle.c into liboracle.so (double) and liboracle_f32.so (float)."""
+    src = os.path.join(_HERE, "cpra_oracle.c")
+    outs = {}
+    for prec, define in (("f64", "double"), ("f32", "float")):
+        out = os.path.join(_HERE, "liboracle.so" if prec == "f64" else "liboracle_f32.so")
+        if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
+            subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c99",
+                                   f"-DORACLE_REAL={define}", "-o", out, src, "-lm"])
+        outs[prec] = out
+    return outs
+
+
+def _lib(precision: str = "f64"):
+    if precision not in _LIBS:
+        lib = ctypes.CDLL(build_oracle()[precision])
+        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        lib.oracle_plan.argtypes = [ctypes.POINTER(vp), ci, ci]
+        lib.oracle_destroy.argtypes = [vp]
+        lib.oracle_set_data.argtypes = [vp, vp, vp, vp]
+        lib.oracle_set_support.argtypes = [vp, vp]
+        lib.oracle_set_carousel.argtypes = [vp, ci, vp, ci]
+        lib.oracle_set_estimate.argtypes = [vp, vp]
+        lib.oracle_set_iteration.argtypes = [vp, ctypes.c_long]
+        lib.oracle_get_iteration.argtypes = [vp]
+        lib.oracle_get_iteration.restype = ctypes.c_long
+        lib.oracle_iterate.argtypes = [vp, ci, cd]
+        lib.oracle_get_error.argtypes = [vp, vp, vp]
+        lib.oracle_get_projections.argtypes = [vp, ci, vp]
+        lib.oracle_assemble_3d.argtypes = [vp, vp, vp]
+        lib.oracle_fft2.argtypes = [vp, vp, ci, ci, ci]
+        lib.oracle_dft2_naive.argtypes = [vp, vp, ci, ci]
+        lib.oracle_mix.argtypes = [vp, vp, ci, ci, ci, vp]
+        lib.oracle_modulus.argtypes = [vp, vp, vp, ci, vp]
+        lib.oracle_hio.argtypes = [vp, vp, vp, ci, cd]
+        lib.oracle_real_name.restype = ctypes.c_char_p
+        _LIBS[precision] = lib
+    return _LIBS[precision]
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code, what):
+        super().__init__(f"{what} returned {code}")
+        self.code = code
+
+
+def _chk(code, what):
+    if code != 0:
+        raise OracleError(code, what)
+
+
+def _c128(a):
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def fft2(stack, sign=-1, precision="f64"):
+    """Radix-2 2D FFT of an image or a stack [count,N,N] (sign=-1 forward, +1 inverse/N^2)."""
+    a = _c128(stack)
+    N = a.shape[-1]
+    out = np.empty_like(a)
+    _chk(_lib(precision).oracle_fft2(a.ctypes.data, out.ctypes.data, N, a.size // (N * N), sign), "oracle_fft2")
+    return out
+
+
+def dft2_naive(img, sign=-1):
+    a = _c128(img)
+    out = np.empty_like(a)
+    _chk(_lib().oracle_dft2_naive(a.ctypes.data, out.ctypes.data, a.shape[-1], sign), "oracle_dft2_naive")
+    return out
+
+
+def mix(stack, alpha, precision="f64"):
+    a = _c128(stack)
+    Np, N = a.shape[0], a.shape[-1]
+    al = np.ascontiguousarray(alpha, dtype=np.float64)
+    out = np.empty_like(a)
+    _chk(_lib(precision).oracle_mix(a.ctypes.data, out.ctypes.data, N, Np, len(al) - 1, al.ctypes.data), "oracle_mix")
+    return out
+
+
+def modulus(G, A, M, precision="f64"):
+    """Fourier-modulus constraint on one native-order image.  Returns (G', num)."""
+    g = _c128(G).copy()
+    a = np.ascontiguousarray(A, dtype=np.float64)
+    m = np.ascontiguousarray(M, dtype=np.uint8)
+    num = ctypes.c_double(0.0)
+    _chk(_lib(precision).oracle_modulus(g.ctypes.data, a.ctypes.data, m.ctypes.data, g.shape[-1],
+                                        ctypes.addressof(num)), "oracle_modulus")
+    return g, num.value
+
+
+def hio(ghat, gp, S, beta, precision="f64"):
+    a = _c128(ghat).copy()
+    b = _c128(gp)
+    s = np.ascontiguousarray(S, dtype=np.uint8)
+    _chk(_lib(precision).oracle_hio(a.ctypes.data, b.ctypes.data, s.ctypes.data, a.shape[-1], float(beta)), "oracle_hio")
+    return a
+
+
+class Oracle:
+    """The CPRA loop on the host in FP64 (or fp32 with precision='f32'; drift display only)."""
+
+    def __init__(self, N: int, Np: int, precision: str = "f64"):
+        self._l = _lib(precision)
+        self.N, self.Np = int(N), int(Np)
+        h = ctypes.c_void_p()
+        _chk(self._l.oracle_plan(ctypes.byref(h), self.N, self.Np), "oracle_plan")
+        self._h = h
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._l.oracle_destroy(self._h)
+            self._h = None
+
+    def set_data(self, intensity, mask=None, angles=None):
+        I = np.ascontiguousarray(intensity, dtype=np.float64)
+        assert I.shape == (self.Np, self.N, self.N)
+        m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+        a = None if angles is None else np.ascontiguousarray(angles, dtype=np.float64)
+        _chk(self._l.oracle_set_data(self._h, I.ctypes.data, None if m is None else m.ctypes.data,
+                                     None if a is None else a.ctypes.data), "oracle_set_data")
+
+    def set_support(self, support):
+        s = np.ascontiguousarray(support, dtype=np.uint8)
+        assert s.shape == (self.Np, self.N, self.N)
+        _chk(self._l.oracle_set_support(self._h, s.ctypes.data), "oracle_set_support")
+
+    def set_carousel(self, alpha, n_ei=1):
+        al = np.ascontiguousarray(alpha, dtype=np.float64)
+        _chk(self._l.oracle_set_carousel(self._h, len(al) - 1, al.ctypes.data, int(n_ei)), "oracle_set_carousel")
+
+    def set_estimate(self, g0):
+        g = _c128(g0)
+        assert g.shape == (self.Np, self.N, self.N)
+        _chk(self._l.oracle_set_estimate(self._h, g.ctypes.data), "oracle_set_estimate")
+
+    def set_iteration(self, t):
+        _chk(self._l.oracle_set_iteration(self._h, int(t)), "oracle_set_iteration")
+
+    @property
+    def iteration(self):
+        return int(self._l.oracle_get_iteration(self._h))
+
+    def iterate(self, k, beta=0.9):
+        _chk(self._l.oracle_iterate(self._h, int(k), float(beta)), "oracle_iterate")
+
+    def get_error(self):
+        E = np.empty(self.Np, dtype=np.float64)
+        Eg = ctypes.c_double(0.0)
+        _chk(self._l.oracle_get_error(self._h, E.ctypes.data, ctypes.addressof(Eg)), "oracle_get_error")
+        return E, Eg.value
+
+    def get_projections(self, which=0):
+        out = np.empty((self.Np, self.N, self.N), dtype=np.complex128)
+        _chk(self._l.oracle_get_projections(self._h, int(which), out.ctypes.data), "oracle_get_projections")
+        return out
+
+    def assemble_3d(self, want_weight=True):
+        vol = np.empty((self.N,) * 3, dtype=np.complex128)
+        w = np.empty((self.N,) * 3, dtype=np.float64) if want_weight else None
+        _chk(self._l.oracle_assemble_3d(self._h, vol.ctypes.data, None if w is None else w.ctypes.data),
+             "oracle_assemble_3d")
+        return (vol, w) if want_weight else vol
+
+    def load(self, problem, alpha=(0.6, 0.2), n_ei=1):
+        """Convenience: feed a cpra_inputs.Problem."""
+        self.set_data(problem.intensity, problem.mask, problem.angles)
+        self.set_support(problem.support)
+        self.set_carousel(alpha, n_ei)
+        self.set_estimate(problem.estimate)
+        return self
