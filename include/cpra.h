@@ -1,0 +1,204 @@
+/*
+ * cpra.h -- C ABI of the B200-native CPRA iteration loop (libcpra.so).
+ *
+ * The library runs the data-parallel hot path of the carousel phase retrieval algorithm of
+ * "Real time 3D coherent X-ray diffraction imaging" (arXiv 2402.05283): all N_p two-dimensional
+ * projection reconstructions advance together, one iteration being
+ *     carousel mix (Eq. (4))  ->  forward 2D FT  ->  error + Fourier-modulus constraint
+ *                             ->  inverse 2D FT  ->  support / HIO update,
+ * plus a one-shot Fourier-slice assembly of the retrieved projections into the N^3 spectrum.
+ * Citations "P:<line>" are lines of the paper text; "A<k>" are the readings
+ * of ambiguous passages listed in DESIGN.md.
+ *
+ * Conventions
+ *   - n = 0..Np-1 projections (the paper counts from 1); pixel (y, x), row-major, x fastest;
+ *     complex = interleaved (re, im) fp32; N a power of two in [16, 1024].
+ *   - Pointer names: d_* = DEVICE pointers (the caller's allocator, e.g. torch data_ptr());
+ *     h_* = HOST pointers.  The library never allocates device memory: every internal buffer lives
+ *     in the workspace the caller binds (cpra_workspace_bytes / cpra_bind_workspace).
+ *   - Ownership: the caller owns every buffer it passes.  set_* calls copy / precompute into the
+ *     workspace; the caller's buffer may be reused as soon as the plan's stream has passed the call.
+ *   - Asynchrony: every call only enqueues work on the plan's CUDA stream (no host sync, no D2H),
+ *     except cpra_reconstruct_host, which synchronises the stream before it returns.
+ *   - Errors: every call returns CPRA_OK (0) or a negative code; nothing throws, aborts or prints.
+ *     Errors detectable at enqueue time are returned at once; a kernel fault surfaces as
+ *     CPRA_ERR_CUDA from a later call.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns CPRA_ERR_CUDA.
+ */
+#ifndef CPRA_H
+#define CPRA_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cpra_plan_s* cpra_plan_t; /* opaque */
+
+enum {
+    CPRA_OK = 0,
+    CPRA_ERR_INVALID_ARG = -1,      /* NULL pointer, k < 0, bad K / n_ei / beta, bad `which` */
+    CPRA_ERR_UNSUPPORTED_SIZE = -2, /* N not a power of two in [16, 1024], or Np < 1 */
+    CPRA_ERR_NOT_READY = -3,        /* call made before the state it needs exists */
+    CPRA_ERR_WORKSPACE = -4,        /* workspace missing, too small or misaligned */
+    CPRA_ERR_CUDA = -5,             /* a CUDA runtime call or an earlier kernel failed */
+    CPRA_ERR_INVALID_VALUE = -6     /* reserved (input value checks; not performed) */
+};
+
+/* Largest half-width K of the carousel weights accepted by cpra_set_carousel. */
+#define CPRA_MAX_K 8
+
+/* `which` of cpra_get_projections */
+#define CPRA_ITERATE 0   /* the iterate g_n */
+#define CPRA_SUPPORTED 1 /* S_n * g_n */
+
+/* plan flags */
+#define CPRA_FLAG_DEFAULT 0u
+#define CPRA_FLAG_FORCE_MULTIPASS 1u /* never use the one-CTA-per-image shared-memory kernel (N <= 128) */
+#define CPRA_FLAG_NO_CHUNKING 2u     /* run every pass over all Np images (no L2-resident chunking) */
+
+/*
+ * Create a plan for Np projections of N x N pixels ("a scattered intensity map ... of N x N
+ * pixels is collected" for each of the N_p angles).  `cuda_stream` is a cudaStream_t (NULL = the
+ * legacy default stream); all later work of this plan is enqueued on it.  Host-only: no device work.
+ * Defaults: carousel weights alpha = (0.6, 0.2), K = 1, n_ei = 1 (K = 0, alpha_0 = 1 if Np < 3).
+ * Errors: INVALID_ARG (out NULL), UNSUPPORTED_SIZE.
+ */
+int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream);
+
+/* Bytes of device workspace this plan needs (a multiple of 256).  Host-only. */
+int cpra_workspace_bytes(cpra_plan_t plan, size_t* bytes);
+
+/*
+ * Hand the plan its device workspace: `bytes` >= cpra_workspace_bytes, d_ws 256-byte aligned.  The
+ * caller keeps ownership and must keep it alive until cpra_destroy.  Uploads the twiddle table.
+ * Errors: INVALID_ARG, WORKSPACE (too small / misaligned), CUDA.
+ */
+int cpra_bind_workspace(cpra_plan_t plan, void* d_ws, size_t bytes);
+
+/*
+ * The measured data (I_n = |E_n|^2 for each angle; a beamstop leaves the central
+ * pixels unmeasured).
+ *   d_I      [Np][N][N] fp32 intensities, detector-centred (zero frequency at index (N/2, N/2)).
+ *   d_mask   [Np][N][N] u8, 1 = measured, 0 = unmeasured (left free by the modulus constraint,
+ *            A12); NULL = everything measured.
+ *   h_angles [Np] doubles on the HOST, rotation angle theta_n about z in radians; used only
+ *            by cpra_assemble_3d; NULL = all zero.
+ * Precomputes A = sqrt(max(I, 0)) (A14) in the library's internal frequency order with the mask
+ * folded in, and den_n = sum over measured pixels of I_n (the error normalisation, A9).
+ * Errors: INVALID_ARG (d_I NULL), WORKSPACE (not bound), CUDA.
+ */
+int cpra_set_data(cpra_plan_t plan, const float* d_I, const unsigned char* d_mask, const double* h_angles);
+
+/*
+ * The real-space constraint ("space constraints"): d_S [Np][N][N] u8, non-zero = inside
+ * the support of projection n.  Stored bit-packed.  Errors: INVALID_ARG, WORKSPACE, CUDA.
+ */
+int cpra_set_support(cpra_plan_t plan, const unsigned char* d_S);
+
+/*
+ * Carousel coupling, Eq. (4) (readings A1-A4): at the start of iteration t, iff
+ * t mod n_ei == 0,   ghat_n = sum_{j=-K..K} alpha_|j| g_{(n+j) mod Np}   (Jacobi, periodic in n);
+ * otherwise ghat_n = g_n.  h_alpha: K+1 doubles on the HOST (alpha_0 .. alpha_K), used as given
+ * (not renormalised).  K = 0 with alpha_0 = 1 switches the coupling off.
+ * Errors: INVALID_ARG (NULL, K < 0, K > CPRA_MAX_K, 2K+1 > Np, n_ei < 1).
+ */
+int cpra_set_carousel(cpra_plan_t plan, int K, const double* h_alpha, int n_ei);
+
+/*
+ * The starting estimate ("random initial guess"; A15): d_g0 interleaved complex fp32
+ * [Np][N][N], objects centred at pixel (N/2, N/2).  Resets the iteration counter t to 0.
+ * Errors: INVALID_ARG, WORKSPACE, CUDA.
+ */
+int cpra_set_estimate(cpra_plan_t plan, const float* d_g0);
+
+/* Iteration counter t (iterations since cpra_set_estimate); settable for exact resume with n_ei > 1. */
+int cpra_get_iteration(cpra_plan_t plan, long* t);
+int cpra_set_iteration(cpra_plan_t plan, long t);
+
+/*
+ * Run k iterations of the loop (Step B of the paper, all Np projections at once) with
+ * HIO feedback beta (P:98 ref [22]).  One iteration, in the paper's order:
+ *   1. ghat = mix(g) as set by cpra_set_carousel                       (Eq. (4))
+ *   2. G_n  = F[ghat_n], forward 2D FT, e^{-2 pi i ...}, unnormalised  (Eq. (3), A10)
+ *   3. num_n = sum_{measured} (|G_n| - A_n)^2                          (A9)
+ *   4. measured: G'_n = A_n G_n/|G_n| (G'_n = A_n where |G_n| = 0, A13); unmeasured: G'_n = G_n
+ *   5. g'_n = F^-1[G'_n], e^{+2 pi i ...} / N^2
+ *   6. S_n = 1: g_n <- g'_n;  S_n = 0: g_n <- ghat_n - beta g'_n       (HIO, complex, A6/A7)
+ *   7. t <- t + 1
+ * k = 0 is a valid no-op.  iterate(k1) followed by iterate(k2) equals iterate(k1 + k2) bit for bit.
+ * Errors: INVALID_ARG (k < 0, beta not finite), NOT_READY (data, support or estimate missing),
+ * WORKSPACE, CUDA.
+ */
+int cpra_iterate(cpra_plan_t plan, int k, float beta);
+
+/*
+ * Reconstruction error of the LAST iteration run (evaluated on its input, before the modulus
+ * step; A9): d_E [Np] fp32, E_n = sqrt(num_n / den_n) (0 where den_n = 0); d_Eglobal [1] fp32,
+ * sqrt(sum_n num_n / sum_n den_n).  Either pointer may be NULL.  Device-side reduction, fixed
+ * summation order (deterministic).  Errors: NOT_READY (no iteration run yet), CUDA.
+ */
+int cpra_get_error(cpra_plan_t plan, float* d_E, float* d_Eglobal);
+
+/*
+ * The projected objects O'_n: d_out interleaved complex fp32 [Np][N][N];
+ * which = CPRA_ITERATE: g_n; which = CPRA_SUPPORTED: S_n g_n.
+ * Errors: INVALID_ARG, NOT_READY (no estimate; SUPPORTED also needs the support), CUDA.
+ */
+int cpra_get_projections(cpra_plan_t plan, int which, float* d_out);
+
+/*
+ * Fourier-slice assembly (first sentence of Step D; Fourier slice theorem P:35-44):
+ * E_n = F[S_n g_n] are placed as central slices of the 3D spectrum (rotation about z by
+ * theta_n: F2[P_n](kz, ku) = F3[O](kz, ky = ku sin theta_n, kx = ku cos theta_n)) and every voxel
+ * is interpolated bilinearly in (angle, radius) between the two bracketing slices (A17; the paper
+ * only says "interpolate").  d_vol: interleaved complex fp32 [N][N][N] (kz, ky, kx), native FFT
+ * order, comparable with the 3D FT of an object centred at (N/2, N/2, N/2); voxels with
+ * sqrt(kx^2+ky^2) > N/2-1 are zero.  d_weight: fp32 [N][N][N], 1 where a value was written, 0
+ * elsewhere; may be NULL.  One-shot, outside the timed loop.
+ * Errors: INVALID_ARG, NOT_READY (data, support or estimate missing), CUDA.
+ */
+int cpra_assemble_3d(cpra_plan_t plan, float* d_vol, float* d_weight);
+
+/*
+ * Diagnostic: the library's own 2D FFT of a stack, natural order in and out.  d_in, d_out:
+ * interleaved complex fp32 [Np][N][N]; sign = -1 forward (unnormalised), +1 inverse (/N^2).
+ * Uses the same kernels as the loop (row pass, column pass); overwrites the FFT scratch only.
+ * Errors: INVALID_ARG, WORKSPACE, CUDA.
+ */
+int cpra_fft2(cpra_plan_t plan, const float* d_in, float* d_out, int sign);
+
+/*
+ * End-to-end convenience with HOST buffers (pinned memory recommended): uploads the inputs,
+ * runs k iterations, downloads the result and synchronises the plan's stream.
+ *   h_I [Np][N][N] fp32, h_mask [Np][N][N] u8 or NULL, h_angles [Np] or NULL, h_S [Np][N][N] u8,
+ *   h_g0 [Np][N][N] complex fp32  ->  h_out [Np][N][N] complex fp32 (the iterate; may be NULL),
+ *   h_E [Np] fp32 or NULL, h_Eglobal [1] fp32 or NULL.
+ * d_stage: DEVICE staging buffer of at least cpra_host_staging_bytes (caller-owned, 256-aligned).
+ * Errors: as the calls it is made of.
+ */
+int cpra_host_staging_bytes(cpra_plan_t plan, size_t* bytes);
+int cpra_reconstruct_host(cpra_plan_t plan, void* d_stage, size_t stage_bytes,
+                          const float* h_I, const unsigned char* h_mask, const double* h_angles,
+                          const unsigned char* h_S, const float* h_g0, int k, float beta,
+                          float* h_out, float* h_E, float* h_Eglobal);
+
+/* Tuning knob: process the Np images in chunks of `images` (K1, K2, K3 per chunk) so that a chunk's
+ * intermediate spectrum stays in the 126 MB L2 between the three passes; 0 = one chunk (all images).
+ * Results are bit-identical for every chunk size.  Errors: INVALID_ARG. */
+int cpra_set_chunk(cpra_plan_t plan, int images);
+
+/* Number of kernels this plan has launched since it was created (for bench.py's gpu_launches). */
+int cpra_launch_count(cpra_plan_t plan, long* count);
+
+/* Free the plan (host memory only; the workspace stays the caller's). */
+int cpra_destroy(cpra_plan_t plan);
+
+/* Static, never NULL. */
+const char* cpra_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CPRA_H */

@@ -1,0 +1,260 @@
+"""Thin ctypes binding of libcpra.so (include/cpra.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI.  PyTorch is used for device
+memory and streams only.  Nothing here falls back to the CPU: if the library cannot be loaded, or
+a call fails, a `CpraError` is raised."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+CPRA_OK = 0
+ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_READY, ERR_WORKSPACE, ERR_CUDA, ERR_INVALID_VALUE = -1, -2, -3, -4, -5, -6
+ITERATE, SUPPORTED = 0, 1
+FLAG_DEFAULT, FLAG_FORCE_MULTIPASS, FLAG_NO_CHUNKING = 0, 1, 2
+MAX_K = 8
+
+_vp, _ci, _cf, _cl, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_long, ctypes.c_size_t
+
+# name -> (restype, argtypes): every symbol include/cpra.h declares
+SIGNATURES = {
+    "cpra_plan": (_ci, [ctypes.POINTER(_vp), _ci, _ci, ctypes.c_uint, _vp]),
+    "cpra_workspace_bytes": (_ci, [_vp, ctypes.POINTER(_sz)]),
+    "cpra_bind_workspace": (_ci, [_vp, _vp, _sz]),
+    "cpra_set_data": (_ci, [_vp, _vp, _vp, _vp]),
+    "cpra_set_support": (_ci, [_vp, _vp]),
+    "cpra_set_carousel": (_ci, [_vp, _ci, _vp, _ci]),
+    "cpra_set_estimate": (_ci, [_vp, _vp]),
+    "cpra_get_iteration": (_ci, [_vp, ctypes.POINTER(_cl)]),
+    "cpra_set_iteration": (_ci, [_vp, _cl]),
+    "cpra_iterate": (_ci, [_vp, _ci, _cf]),
+    "cpra_get_error": (_ci, [_vp, _vp, _vp]),
+    "cpra_get_projections": (_ci, [_vp, _ci, _vp]),
+    "cpra_assemble_3d": (_ci, [_vp, _vp, _vp]),
+    "cpra_fft2": (_ci, [_vp, _vp, _vp, _ci]),
+    "cpra_host_staging_bytes": (_ci, [_vp, ctypes.POINTER(_sz)]),
+    "cpra_reconstruct_host": (_ci, [_vp, _vp, _sz, _vp, _vp, _vp, _vp, _vp, _ci, _cf, _vp, _vp, _vp]),
+    "cpra_set_chunk": (_ci, [_vp, _ci]),
+    "cpra_launch_count": (_ci, [_vp, ctypes.POINTER(_cl)]),
+    "cpra_destroy": (_ci, [_vp]),
+    "cpra_status_string": (ctypes.c_char_p, [_ci]),
+}
+
+_LIB = None
+
+
+class CpraError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        self.code = int(code)
+        name = lib().cpra_status_string(self.code).decode() if _LIB is not None else str(code)
+        super().__init__(f"{what} failed: {name} ({self.code})")
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib() -> ctypes.CDLL:
+    """Load libcpra.so (building it first if the sources are newer).  Raises if unavailable."""
+    global _LIB
+    if _LIB is None:
+        path = _build.build()
+        if not os.path.exists(path):
+            raise OSError(f"{path} is missing and could not be built; there is no fallback path")
+        L = ctypes.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)      # AttributeError if the symbol is not exported
+            fn.restype, fn.argtypes = res, args
+        _LIB = L
+    return _LIB
+
+
+def _chk(code: int, what: str) -> None:
+    if code != CPRA_OK:
+        raise CpraError(code, what)
+
+
+def _dptr(t, dtype, nelem=None):
+    """Device pointer of a contiguous CUDA torch tensor (checked)."""
+    import torch
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
+        raise TypeError("expected a contiguous CUDA torch tensor")
+    if t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    if nelem is not None and t.numel() != nelem:
+        raise ValueError(f"expected {nelem} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+class Plan:
+    """One CPRA problem: N x N pixels, Np projections, on the current CUDA device and stream.
+
+    Mirrors the C ABI one to one: set_data / set_support / set_carousel / set_estimate / iterate /
+    get_error / get_projections / assemble_3d (+ fft2, reconstruct_host).  Tensors are torch CUDA
+    tensors owned by the caller; complex arrays are torch.complex64."""
+
+    def __init__(self, N: int, Np: int, flags: int = FLAG_DEFAULT, stream=None, device=None):
+        import torch
+        self._l = lib()
+        self.N, self.Np = int(N), int(Np)
+        self._h = _vp()
+        self._ws = None
+        if not torch.cuda.is_available():
+            # validate the sizes first so that argument errors are reported as such
+            _chk(self._l.cpra_plan(ctypes.byref(self._h), self.N, self.Np, flags, None), "cpra_plan")
+            self.close()
+            raise CpraError(ERR_CUDA, "cpra_plan (no CUDA device; there is no CPU fallback)")
+        self.device = torch.device(device if device is not None else f"cuda:{torch.cuda.current_device()}")
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        _chk(self._l.cpra_plan(ctypes.byref(self._h), self.N, self.Np, flags, _vp(self.stream.cuda_stream)), "cpra_plan")
+        nbytes = _sz()
+        _chk(self._l.cpra_workspace_bytes(self._h, ctypes.byref(nbytes)), "cpra_workspace_bytes")
+        self.workspace_bytes = int(nbytes.value)
+        self._ws = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
+        _chk(self._l.cpra_bind_workspace(self._h, _vp(self._ws.data_ptr()), self.workspace_bytes), "cpra_bind_workspace")
+        self._stage = None
+        self._px = self.Np * self.N * self.N
+
+    # -- lifetime ---------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._l.cpra_destroy(self._h)
+            self._h = _vp()
+        self._ws = None
+        self._stage = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C ABI, one method per call ------------------------------------------------------------
+    def set_data(self, intensity, mask=None, angles=None):
+        import torch
+        a = None
+        if angles is not None:
+            a = np.ascontiguousarray(np.asarray(angles, dtype=np.float64))
+            if a.shape != (self.Np,):
+                raise ValueError("angles must have Np entries")
+        _chk(self._l.cpra_set_data(self._h, _dptr(intensity, torch.float32, self._px),
+                                   _dptr(mask, torch.uint8, self._px),
+                                   None if a is None else a.ctypes.data), "cpra_set_data")
+
+    def set_support(self, support):
+        import torch
+        _chk(self._l.cpra_set_support(self._h, _dptr(support, torch.uint8, self._px)), "cpra_set_support")
+
+    def set_carousel(self, alpha, n_ei=1):
+        al = np.ascontiguousarray(np.asarray(alpha, dtype=np.float64))
+        _chk(self._l.cpra_set_carousel(self._h, len(al) - 1, al.ctypes.data, int(n_ei)), "cpra_set_carousel")
+
+    def set_estimate(self, g0):
+        import torch
+        _chk(self._l.cpra_set_estimate(self._h, _dptr(g0, torch.complex64, self._px)), "cpra_set_estimate")
+
+    @property
+    def iteration(self) -> int:
+        t = _cl()
+        _chk(self._l.cpra_get_iteration(self._h, ctypes.byref(t)), "cpra_get_iteration")
+        return int(t.value)
+
+    @iteration.setter
+    def iteration(self, t: int):
+        _chk(self._l.cpra_set_iteration(self._h, int(t)), "cpra_set_iteration")
+
+    def set_chunk(self, images: int):
+        _chk(self._l.cpra_set_chunk(self._h, int(images)), "cpra_set_chunk")
+
+    def iterate(self, k: int, beta: float = 0.9):
+        _chk(self._l.cpra_iterate(self._h, int(k), float(beta)), "cpra_iterate")
+
+    def get_error(self):
+        """(E[Np], E_global[1]) as CUDA float32 tensors (no host sync)."""
+        import torch
+        E = torch.empty(self.Np, dtype=torch.float32, device=self.device)
+        Eg = torch.empty(1, dtype=torch.float32, device=self.device)
+        _chk(self._l.cpra_get_error(self._h, E.data_ptr(), Eg.data_ptr()), "cpra_get_error")
+        return E, Eg
+
+    def get_projections(self, which: int = ITERATE, out=None):
+        import torch
+        if out is None:
+            out = torch.empty((self.Np, self.N, self.N), dtype=torch.complex64, device=self.device)
+        _chk(self._l.cpra_get_projections(self._h, int(which), _dptr(out, torch.complex64, self._px)), "cpra_get_projections")
+        return out
+
+    def assemble_3d(self, want_weight: bool = True):
+        import torch
+        vol = torch.empty((self.N,) * 3, dtype=torch.complex64, device=self.device)
+        w = torch.empty((self.N,) * 3, dtype=torch.float32, device=self.device) if want_weight else None
+        _chk(self._l.cpra_assemble_3d(self._h, vol.data_ptr(), None if w is None else w.data_ptr()), "cpra_assemble_3d")
+        return (vol, w) if want_weight else vol
+
+    def fft2(self, stack, sign: int = -1):
+        import torch
+        out = torch.empty_like(stack)
+        _chk(self._l.cpra_fft2(self._h, _dptr(stack, torch.complex64, self._px), out.data_ptr(), int(sign)), "cpra_fft2")
+        return out
+
+    @property
+    def launch_count(self) -> int:
+        c = _cl()
+        _chk(self._l.cpra_launch_count(self._h, ctypes.byref(c)), "cpra_launch_count")
+        return int(c.value)
+
+    # -- host-buffer end-to-end call ---------------------------------------------------------------
+    def host_staging_bytes(self) -> int:
+        b = _sz()
+        _chk(self._l.cpra_host_staging_bytes(self._h, ctypes.byref(b)), "cpra_host_staging_bytes")
+        return int(b.value)
+
+    def reconstruct_host(self, intensity, mask, angles, support, g0, k, beta=0.9, out=None, want_error=True):
+        """Host (CPU, ideally pinned) torch tensors or numpy arrays in, host arrays out.
+        Returns (projections complex64 [Np,N,N] host, E[Np] host, E_global float)."""
+        import torch
+
+        def hptr(x, dtype, n):
+            if x is None:
+                return None, None
+            t = torch.as_tensor(x)
+            if t.is_cuda or not t.is_contiguous() or t.dtype != dtype or t.numel() != n:
+                raise TypeError("expected a contiguous host tensor of the right dtype and size")
+            return t, t.data_ptr()
+
+        if self._stage is None:
+            self._stage = torch.empty(self.host_staging_bytes(), dtype=torch.uint8, device=self.device)
+        keep = []
+        tI, pI = hptr(intensity, torch.float32, self._px); keep.append(tI)
+        tM, pM = hptr(mask, torch.uint8, self._px); keep.append(tM)
+        tS, pS = hptr(support, torch.uint8, self._px); keep.append(tS)
+        tG, pG = hptr(g0, torch.complex64, self._px); keep.append(tG)
+        a = None if angles is None else np.ascontiguousarray(np.asarray(angles, dtype=np.float64))
+        if out is None:
+            out = torch.empty((self.Np, self.N, self.N), dtype=torch.complex64).pin_memory()
+        E = torch.empty(self.Np + 1, dtype=torch.float32).pin_memory() if want_error else None
+        _chk(self._l.cpra_reconstruct_host(
+            self._h, self._stage.data_ptr(), self._stage.numel(), pI, pM,
+            None if a is None else a.ctypes.data, pS, pG, int(k), float(beta), out.data_ptr(),
+            None if E is None else E.data_ptr(),
+            None if E is None else E.data_ptr() + 4 * self.Np), "cpra_reconstruct_host")
+        if E is None:
+            return out, None, None
+        return out, E[:self.Np], float(E[self.Np])
+
+    # -- convenience --------------------------------------------------------------------------------
+    def load(self, problem, alpha=(0.6, 0.2), n_ei=1):
+        """Upload a cpra_inputs.Problem (numpy) and set everything."""
+        import torch
+        dev = self.device
+        self.set_data(torch.from_numpy(problem.intensity).to(dev), torch.from_numpy(problem.mask).to(dev), problem.angles)
+        self.set_support(torch.from_numpy(problem.support).to(dev))
+        self.set_carousel(alpha, n_ei)
+        self.set_estimate(torch.from_numpy(problem.estimate).to(dev))
+        return self

@@ -1,0 +1,548 @@
+// cpra_api.cu -- the C ABI of libcpra.so (include/cpra.h): plan, workspace, launch logic.
+// Host code only decides what to enqueue; every step of the path runs in the kernels of
+// cpra_kernels.cuh.  There is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/cpra.h"
+#include "cpra_kernels.cuh"
+
+using namespace cpra;
+
+struct cpra_plan_s {
+    int N = 0, Np = 0;
+    unsigned flags = 0;
+    cudaStream_t stream = nullptr;
+    Geo geo{};
+    // workspace carve-up
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    float2* tw = nullptr;
+    float* A = nullptr;
+    uint16_t* S16 = nullptr;
+    float2* st[2] = {nullptr, nullptr};
+    float2* scr = nullptr;
+    double* partial = nullptr;
+    double* den = nullptr;
+    double* uphi = nullptr;
+    int* ustart = nullptr;
+    int* rays = nullptr;
+    int cur = 0;
+    // parameters / state
+    int K = 1;
+    float alpha[MAXK + 1] = {0};
+    int n_ei = 1;
+    long t = 0;
+    bool have_data = false, have_support = false, have_estimate = false, have_error = false;
+    bool attrs_set = false;
+    std::vector<double> angles;
+    std::vector<float2> h_tw;
+    std::vector<double> h_uphi;
+    std::vector<int> h_ustart, h_rays;
+    long launches = 0;
+    int chunk = 0;  // images per L2-resident chunk; 0 = all
+};
+
+namespace {
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Carve {
+    size_t off = 0;
+    size_t take(size_t bytes) { const size_t o = off; off = align256(off + bytes); return o; }
+};
+
+struct Layout {
+    size_t tw, A, S16, st0, st1, scr, partial, den, uphi, ustart, rays, total;
+};
+
+Layout layout_of(int N, int Np)
+{
+    const size_t px = (size_t)Np * N * N;
+    Carve c;
+    Layout L;
+    L.tw = c.take(sizeof(float2) * N);
+    L.A = c.take(sizeof(float) * px);
+    L.S16 = c.take(px / 8);
+    L.st0 = c.take(sizeof(float2) * px);
+    L.st1 = c.take(sizeof(float2) * px);
+    L.scr = c.take(sizeof(float2) * px);
+    L.partial = c.take(sizeof(double) * (size_t)Np * (N / TB));
+    L.den = c.take(sizeof(double) * Np);
+    L.uphi = c.take(sizeof(double) * 2 * Np);
+    L.ustart = c.take(sizeof(int) * (2 * (size_t)Np + 1));
+    L.rays = c.take(sizeof(int) * 2 * (size_t)Np);
+    L.total = c.off;
+    return L;
+}
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+template <int N> constexpr int threads_for() { return N <= 32 ? 64 : N <= 128 ? 128 : N <= 512 ? 256 : 512; }
+
+#define CPRA_DISPATCH_N(N_, ...)                                                     \
+    switch (N_) {                                                                    \
+        case 16:   { constexpr int NN = 16;   __VA_ARGS__; break; }                  \
+        case 32:   { constexpr int NN = 32;   __VA_ARGS__; break; }                  \
+        case 64:   { constexpr int NN = 64;   __VA_ARGS__; break; }                  \
+        case 128:  { constexpr int NN = 128;  __VA_ARGS__; break; }                  \
+        case 256:  { constexpr int NN = 256;  __VA_ARGS__; break; }                  \
+        case 512:  { constexpr int NN = 512;  __VA_ARGS__; break; }                  \
+        case 1024: { constexpr int NN = 1024; __VA_ARGS__; break; }                  \
+        default: return CPRA_ERR_UNSUPPORTED_SIZE;                                   \
+    }
+
+template <class F>
+cudaError_t allow_smem(F* f, int bytes)
+{
+    return cudaFuncSetAttribute(reinterpret_cast<const void*>(f), cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+template <int N>
+int set_attrs()
+{
+    constexpr int NT = threads_for<N>();
+    cudaError_t e = cudaSuccess;
+    auto acc = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    acc(allow_smem(k_row_fwd<N, NT, MIX_NONE>, row_smem_bytes<N>()));
+    acc(allow_smem(k_row_fwd<N, NT, MIX_K1>, row_smem_bytes<N>()));
+    acc(allow_smem(k_row_fwd<N, NT, MIX_GEN>, row_smem_bytes<N>()));
+    acc(allow_smem(k_row_fwd<N, NT, MIX_MASK>, row_smem_bytes<N>()));
+    acc(allow_smem(k_col<N, NT, COL_FULL>, col_smem_bytes<N>()));
+    acc(allow_smem(k_col<N, NT, COL_FWD>, col_smem_bytes<N>()));
+    acc(allow_smem(k_col<N, NT, COL_INV>, col_smem_bytes<N>()));
+    acc(allow_smem(k_row_inv<N, NT, ROWINV_PLAIN, MIX_NONE>, row_smem_bytes<N>()));
+    acc(allow_smem(k_row_inv<N, NT, ROWINV_HIO, MIX_NONE>, row_smem_bytes<N>()));
+    acc(allow_smem(k_row_inv<N, NT, ROWINV_HIO, MIX_K1>, row_smem_bytes<N>()));
+    acc(allow_smem(k_row_inv<N, NT, ROWINV_HIO, MIX_GEN>, row_smem_bytes<N>()));
+    return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+}
+
+MixParams mix_params(const cpra_plan_s* p)
+{
+    MixParams mp;
+    mp.K = p->K;
+    for (int j = 0; j <= MAXK; ++j) mp.a[j] = j <= p->K ? p->alpha[j] : 0.f;
+    return mp;
+}
+
+int check_launch(cpra_plan_s* p, int n = 1)
+{
+    p->launches += n;
+    return cudaGetLastError() == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+}
+
+// mix mode of one iteration: does the carousel fire, and which kernel variant serves it
+int mix_mode(const cpra_plan_s* p, bool fires)
+{
+    if (!fires) return MIX_NONE;
+    if (p->K == 0) return p->alpha[0] == 1.0f ? MIX_NONE : MIX_GEN;
+    return p->K == 1 ? MIX_K1 : MIX_GEN;
+}
+
+template <int N>
+int launch_row_fwd(cpra_plan_s* p, const float2* cur, int mode, int n0, int nimg)
+{
+    constexpr int NT = threads_for<N>();
+    const dim3 grid((unsigned)nimg * (N / TB));
+    const int smem = row_smem_bytes<N>();
+    const MixParams mp = mix_params(p);
+#define ROWFWD(M) k_row_fwd<N, NT, M><<<grid, NT, smem, p->stream>>>(cur, p->scr, p->tw, p->S16, mp, p->Np, n0, nimg)
+    switch (mode) {
+        case MIX_NONE: ROWFWD(MIX_NONE); break;
+        case MIX_K1: ROWFWD(MIX_K1); break;
+        case MIX_GEN: ROWFWD(MIX_GEN); break;
+        default: ROWFWD(MIX_MASK); break;
+    }
+#undef ROWFWD
+    return check_launch(p);
+}
+
+template <int N>
+int launch_col(cpra_plan_s* p, int mode, int n0, int nimg, float scale)
+{
+    constexpr int NT = threads_for<N>();
+    const dim3 grid((unsigned)nimg * (N / TB));
+    const int smem = col_smem_bytes<N>();
+    switch (mode) {
+        case COL_FULL: k_col<N, NT, COL_FULL><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
+        case COL_FWD: k_col<N, NT, COL_FWD><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
+        default: k_col<N, NT, COL_INV><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
+    }
+    return check_launch(p);
+}
+
+template <int N>
+int launch_row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg)
+{
+    constexpr int NT = threads_for<N>();
+    const dim3 grid((unsigned)nimg * (N / TB));
+    const int smem = row_smem_bytes<N>();
+    const MixParams mp = mix_params(p);
+#define ROWINV(H, M) k_row_inv<N, NT, H, M><<<grid, NT, smem, p->stream>>>(p->scr, cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg)
+    if (!hio) ROWINV(ROWINV_PLAIN, MIX_NONE);
+    else if (mode == MIX_NONE) ROWINV(ROWINV_HIO, MIX_NONE);
+    else if (mode == MIX_K1) ROWINV(ROWINV_HIO, MIX_K1);
+    else ROWINV(ROWINV_HIO, MIX_GEN);
+#undef ROWINV
+    return check_launch(p);
+}
+
+int ready(const cpra_plan_s* p) { return p->ws ? CPRA_OK : CPRA_ERR_WORKSPACE; }
+
+unsigned blocks_for(size_t total, int nt) { return (unsigned)((total + nt - 1) / nt); }
+
+// sorted unique ray directions of the assembly (step (ii))
+void build_rays(cpra_plan_s* p)
+{
+    const double PI = 3.14159265358979323846264338327950288;
+    struct Ray { double phi; int n, neg; };
+    std::vector<Ray> rays;
+    rays.reserve(2 * (size_t)p->Np);
+    for (int n = 0; n < p->Np; ++n)
+        for (int neg = 0; neg < 2; ++neg) {
+            double ph = std::fmod(p->angles[n] + (neg ? PI : 0.0), 2.0 * PI);
+            if (ph < 0.0) ph += 2.0 * PI;
+            if (ph >= 2.0 * PI - 1e-9) ph = 0.0;
+            rays.push_back({ph, n, neg});
+        }
+    std::sort(rays.begin(), rays.end(), [](const Ray& a, const Ray& b) { return a.phi < b.phi || (a.phi == b.phi && a.n < b.n); });
+    p->h_uphi.clear(); p->h_ustart.clear(); p->h_rays.clear();
+    for (size_t i = 0; i < rays.size(); ++i) {
+        if (p->h_uphi.empty() || rays[i].phi - p->h_uphi.back() > 1e-9) {
+            p->h_ustart.push_back((int)i);
+            p->h_uphi.push_back(rays[i].phi);
+        }
+        p->h_rays.push_back(rays[i].n | (rays[i].neg << 30));
+    }
+    p->h_ustart.push_back((int)rays.size());
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* cpra_status_string(int s)
+{
+    switch (s) {
+        case CPRA_OK: return "CPRA_OK";
+        case CPRA_ERR_INVALID_ARG: return "CPRA_ERR_INVALID_ARG";
+        case CPRA_ERR_UNSUPPORTED_SIZE: return "CPRA_ERR_UNSUPPORTED_SIZE";
+        case CPRA_ERR_NOT_READY: return "CPRA_ERR_NOT_READY";
+        case CPRA_ERR_WORKSPACE: return "CPRA_ERR_WORKSPACE";
+        case CPRA_ERR_CUDA: return "CPRA_ERR_CUDA";
+        case CPRA_ERR_INVALID_VALUE: return "CPRA_ERR_INVALID_VALUE";
+        default: return "CPRA_ERR_UNKNOWN";
+    }
+}
+
+int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream)
+{
+    if (!out) return CPRA_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!is_pow2(N) || N < 16 || N > 1024 || Np < 1 || Np >= (1 << 30)) return CPRA_ERR_UNSUPPORTED_SIZE;
+    cpra_plan_s* p = new (std::nothrow) cpra_plan_s;
+    if (!p) return CPRA_ERR_INVALID_ARG;
+    p->N = N; p->Np = Np; p->flags = flags;
+    p->stream = (cudaStream_t)cuda_stream;
+    int R0 = 1, R1 = 1, R2 = 1, RL = 1;
+    { auto f = [&]() -> int { CPRA_DISPATCH_N(N, R0 = Radix<NN>::R0; R1 = Radix<NN>::R1; R2 = Radix<NN>::R2; RL = last_radix<NN>()); return 0; }; f(); }
+    p->geo = Geo{N, Np, R0, R1, R2, RL};
+    // reading A2: the paper's example weights
+    if (Np >= 3) { p->K = 1; p->alpha[0] = 0.6f; p->alpha[1] = 0.2f; }
+    else { p->K = 0; p->alpha[0] = 1.0f; }
+    p->n_ei = 1;
+    p->angles.assign(Np, 0.0);
+    // twiddles exp(-2 pi i m / N), computed in double and rounded once
+    p->h_tw.resize(N);
+    const double PI = 3.14159265358979323846264338327950288;
+    for (int m = 0; m < N; ++m) {
+        const double a = -2.0 * PI * (double)m / (double)N;
+        p->h_tw[m] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    if (const char* e = std::getenv("CPRA_CHUNK")) p->chunk = std::max(0, std::atoi(e));
+    *out = p;
+    return CPRA_OK;
+}
+
+int cpra_destroy(cpra_plan_t p)
+{
+    if (!p) return CPRA_ERR_INVALID_ARG;
+    delete p;
+    return CPRA_OK;
+}
+
+int cpra_workspace_bytes(cpra_plan_t p, size_t* bytes)
+{
+    if (!p || !bytes) return CPRA_ERR_INVALID_ARG;
+    *bytes = layout_of(p->N, p->Np).total;
+    return CPRA_OK;
+}
+
+int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
+{
+    if (!p || !d_ws) return CPRA_ERR_INVALID_ARG;
+    const Layout L = layout_of(p->N, p->Np);
+    if (bytes < L.total || ((uintptr_t)d_ws & 255)) return CPRA_ERR_WORKSPACE;
+    char* w = (char*)d_ws;
+    p->ws = w; p->ws_bytes = bytes;
+    p->tw = (float2*)(w + L.tw);
+    p->A = (float*)(w + L.A);
+    p->S16 = (uint16_t*)(w + L.S16);
+    p->st[0] = (float2*)(w + L.st0);
+    p->st[1] = (float2*)(w + L.st1);
+    p->scr = (float2*)(w + L.scr);
+    p->partial = (double*)(w + L.partial);
+    p->den = (double*)(w + L.den);
+    p->uphi = (double*)(w + L.uphi);
+    p->ustart = (int*)(w + L.ustart);
+    p->rays = (int*)(w + L.rays);
+    p->cur = 0;
+    p->have_data = p->have_support = p->have_estimate = p->have_error = false;
+    if (!p->attrs_set) {
+        int rc = CPRA_OK;
+        { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = set_attrs<NN>()); return 0; }; f(); }
+        if (rc != CPRA_OK) { p->ws = nullptr; return rc; }
+        p->attrs_set = true;
+    }
+    if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float2) * p->N, cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
+        p->ws = nullptr;
+        return CPRA_ERR_CUDA;
+    }
+    return CPRA_OK;
+}
+
+int cpra_set_data(cpra_plan_t p, const float* d_I, const unsigned char* d_mask, const double* h_angles)
+{
+    if (!p || !d_I) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    for (int n = 0; n < p->Np; ++n) p->angles[n] = h_angles ? h_angles[n] : 0.0;
+    k_set_data<<<p->Np, 256, 0, p->stream>>>(d_I, d_mask, p->A, p->den, p->geo);
+    if (int rc = check_launch(p)) return rc;
+    p->have_data = true;
+    p->have_error = false;
+    return CPRA_OK;
+}
+
+int cpra_set_support(cpra_plan_t p, const unsigned char* d_S)
+{
+    if (!p || !d_S) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    const size_t total16 = (size_t)p->Np * p->N * p->N / TB;
+    k_pack_support<<<blocks_for(total16, 256), 256, 0, p->stream>>>(d_S, p->S16, p->N, total16);
+    if (int rc = check_launch(p)) return rc;
+    p->have_support = true;
+    return CPRA_OK;
+}
+
+int cpra_set_carousel(cpra_plan_t p, int K, const double* h_alpha, int n_ei)
+{
+    if (!p || !h_alpha || K < 0 || K > CPRA_MAX_K || 2 * K + 1 > p->Np || n_ei < 1) return CPRA_ERR_INVALID_ARG;
+    for (int j = 0; j <= K; ++j)
+        if (!std::isfinite(h_alpha[j])) return CPRA_ERR_INVALID_ARG;
+    p->K = K;
+    for (int j = 0; j <= MAXK; ++j) p->alpha[j] = j <= K ? (float)h_alpha[j] : 0.f;
+    p->n_ei = n_ei;
+    return CPRA_OK;
+}
+
+int cpra_set_estimate(cpra_plan_t p, const float* d_g0)
+{
+    if (!p || !d_g0) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, p->st[p->cur], p->N, total);
+    if (int rc = check_launch(p)) return rc;
+    p->t = 0;
+    p->have_estimate = true;
+    p->have_error = false;
+    return CPRA_OK;
+}
+
+int cpra_get_iteration(cpra_plan_t p, long* t)
+{
+    if (!p || !t) return CPRA_ERR_INVALID_ARG;
+    *t = p->t;
+    return CPRA_OK;
+}
+
+int cpra_set_iteration(cpra_plan_t p, long t)
+{
+    if (!p || t < 0) return CPRA_ERR_INVALID_ARG;
+    p->t = t;
+    return CPRA_OK;
+}
+
+int cpra_set_chunk(cpra_plan_t p, int images)
+{
+    if (!p || images < 0) return CPRA_ERR_INVALID_ARG;
+    p->chunk = images;
+    return CPRA_OK;
+}
+
+int cpra_iterate(cpra_plan_t p, int k, float beta)
+{
+    if (!p || k < 0 || !std::isfinite(beta)) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_data || !p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
+    const float scale = 1.0f / ((float)p->N * (float)p->N);
+    const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
+    for (int it = 0; it < k; ++it) {
+        const int mode = mix_mode(p, (p->t % p->n_ei) == 0);
+        const float2* cur = p->st[p->cur];
+        float2* nxt = p->st[p->cur ^ 1];
+        for (int n0 = 0; n0 < p->Np; n0 += chunk) {
+            const int nimg = std::min(chunk, p->Np - n0);
+            int rc = CPRA_OK;
+            { auto f = [&]() -> int {
+                CPRA_DISPATCH_N(p->N,
+                    rc = launch_row_fwd<NN>(p, cur, mode, n0, nimg);
+                    if (rc == CPRA_OK) rc = launch_col<NN>(p, COL_FULL, n0, nimg, scale);
+                    if (rc == CPRA_OK) rc = launch_row_inv<NN>(p, cur, nxt, true, mode, beta, 1.0f, n0, nimg));
+                return 0; }; f(); }
+            if (rc != CPRA_OK) return rc;
+        }
+        p->cur ^= 1;
+        p->t += 1;
+        p->have_error = true;
+    }
+    return CPRA_OK;
+}
+
+int cpra_get_error(cpra_plan_t p, float* d_E, float* d_Eglobal)
+{
+    if (!p) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_error) return CPRA_ERR_NOT_READY;
+    if (!d_E && !d_Eglobal) return CPRA_OK;
+    k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, d_E, d_Eglobal, p->Np, p->N / TB);
+    return check_launch(p);
+}
+
+int cpra_get_projections(cpra_plan_t p, int which, float* d_out)
+{
+    if (!p || !d_out || (which != CPRA_ITERATE && which != CPRA_SUPPORTED)) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_estimate || (which == CPRA_SUPPORTED && !p->have_support)) return CPRA_ERR_NOT_READY;
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    k_unpack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>(p->st[p->cur], p->S16, (float2*)d_out, p->N, total, which == CPRA_SUPPORTED);
+    return check_launch(p);
+}
+
+int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
+{
+    if (!p || !d_in || !d_out || (sign != 1 && sign != -1)) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    float2* tmp = p->st[p->cur ^ 1];
+    const unsigned nb = blocks_for(total, 256);
+    int rc = CPRA_OK;
+    if (sign < 0) {
+        k_pack_state<<<nb, 256, 0, p->stream>>>((const float2*)d_in, tmp, p->N, total);
+        if ((rc = check_launch(p))) return rc;
+        { auto f = [&]() -> int {
+            CPRA_DISPATCH_N(p->N,
+                rc = launch_row_fwd<NN>(p, tmp, MIX_NONE, 0, p->Np);
+                if (rc == CPRA_OK) rc = launch_col<NN>(p, COL_FWD, 0, p->Np, 1.0f));
+            return 0; }; f(); }
+        if (rc) return rc;
+        k_unpack_spectrum<<<nb, 256, 0, p->stream>>>(p->scr, (float2*)d_out, p->geo, total);
+        return check_launch(p);
+    }
+    k_pack_spectrum<<<nb, 256, 0, p->stream>>>((const float2*)d_in, p->scr, p->geo, total);
+    if ((rc = check_launch(p))) return rc;
+    const float scale = 1.0f / ((float)p->N * (float)p->N);
+    { auto f = [&]() -> int {
+        CPRA_DISPATCH_N(p->N,
+            rc = launch_col<NN>(p, COL_INV, 0, p->Np, 1.0f);
+            if (rc == CPRA_OK) rc = launch_row_inv<NN>(p, tmp, tmp, false, MIX_NONE, 0.f, scale, 0, p->Np));
+        return 0; }; f(); }
+    if (rc) return rc;
+    k_unpack_state<<<nb, 256, 0, p->stream>>>(tmp, p->S16, (float2*)d_out, p->N, total, 0);
+    return check_launch(p);
+}
+
+int cpra_assemble_3d(cpra_plan_t p, float* d_vol, float* d_weight)
+{
+    if (!p || !d_vol) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_data || !p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
+    build_rays(p);
+    const int U = (int)p->h_uphi.size();
+    if (cudaMemcpyAsync(p->uphi, p->h_uphi.data(), sizeof(double) * U, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+        cudaMemcpyAsync(p->ustart, p->h_ustart.data(), sizeof(int) * (U + 1), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+        cudaMemcpyAsync(p->rays, p->h_rays.data(), sizeof(int) * p->h_rays.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess)
+        return CPRA_ERR_CUDA;
+    // (i) E_n = F[S_n g_n] into the scratch
+    int rc = CPRA_OK;
+    { auto f = [&]() -> int {
+        CPRA_DISPATCH_N(p->N,
+            rc = launch_row_fwd<NN>(p, p->st[p->cur], MIX_MASK, 0, p->Np);
+            if (rc == CPRA_OK) rc = launch_col<NN>(p, COL_FWD, 0, p->Np, 1.0f));
+        return 0; }; f(); }
+    if (rc) return rc;
+    // (ii)-(iv) gather
+    const int N = p->N;
+    const int zsplit = std::max(1, std::min(N, 4096 / std::max(1, (N * N) / 256)));
+    const int zper = (N + zsplit - 1) / zsplit;
+    const dim3 grid(blocks_for((size_t)N * N, 128), (unsigned)((N + zper - 1) / zper));
+    k_assemble<<<grid, 128, 0, p->stream>>>(p->scr, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
+    return check_launch(p);
+}
+
+int cpra_host_staging_bytes(cpra_plan_t p, size_t* bytes)
+{
+    if (!p || !bytes) return CPRA_ERR_INVALID_ARG;
+    const size_t px = (size_t)p->Np * p->N * p->N;
+    *bytes = align256(px * 8) + align256(px * 4) + 2 * align256(px) + align256(sizeof(float) * (p->Np + 1));
+    return CPRA_OK;
+}
+
+int cpra_reconstruct_host(cpra_plan_t p, void* d_stage, size_t stage_bytes, const float* h_I,
+                          const unsigned char* h_mask, const double* h_angles, const unsigned char* h_S,
+                          const float* h_g0, int k, float beta, float* h_out, float* h_E, float* h_Eglobal)
+{
+    if (!p || !d_stage || !h_I || !h_S || !h_g0 || k < 0) return CPRA_ERR_INVALID_ARG;
+    size_t need = 0;
+    cpra_host_staging_bytes(p, &need);
+    if (stage_bytes < need || ((uintptr_t)d_stage & 255)) return CPRA_ERR_WORKSPACE;
+    if (int rc = ready(p)) return rc;
+    const size_t px = (size_t)p->Np * p->N * p->N;
+    char* s = (char*)d_stage;
+    float* d_g = (float*)s;                          s += align256(px * 8);
+    float* d_I = (float*)s;                          s += align256(px * 4);
+    unsigned char* d_M = (unsigned char*)s;          s += align256(px);
+    unsigned char* d_S = (unsigned char*)s;          s += align256(px);
+    float* d_E = (float*)s;
+    auto H2D = [&](void* d, const void* h, size_t b) { return cudaMemcpyAsync(d, h, b, cudaMemcpyHostToDevice, p->stream) == cudaSuccess; };
+    auto D2H = [&](void* h, const void* d, size_t b) { return cudaMemcpyAsync(h, d, b, cudaMemcpyDeviceToHost, p->stream) == cudaSuccess; };
+    if (!H2D(d_I, h_I, px * 4) || (h_mask && !H2D(d_M, h_mask, px)) || !H2D(d_S, h_S, px) || !H2D(d_g, h_g0, px * 8)) return CPRA_ERR_CUDA;
+    int rc;
+    if ((rc = cpra_set_data(p, d_I, h_mask ? d_M : nullptr, h_angles))) return rc;
+    if ((rc = cpra_set_support(p, d_S))) return rc;
+    if ((rc = cpra_set_estimate(p, d_g))) return rc;
+    if ((rc = cpra_iterate(p, k, beta))) return rc;
+    if (h_out) {
+        if ((rc = cpra_get_projections(p, CPRA_ITERATE, d_g))) return rc;
+        if (!D2H(h_out, d_g, px * 8)) return CPRA_ERR_CUDA;
+    }
+    if ((h_E || h_Eglobal) && k > 0) {
+        if ((rc = cpra_get_error(p, d_E, d_E + p->Np))) return rc;
+        if (h_E && !D2H(h_E, d_E, sizeof(float) * p->Np)) return CPRA_ERR_CUDA;
+        if (h_Eglobal && !D2H(h_Eglobal, d_E + p->Np, sizeof(float))) return CPRA_ERR_CUDA;
+    }
+    return cudaStreamSynchronize(p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+}
+
+int cpra_launch_count(cpra_plan_t p, long* count)
+{
+    if (!p || !count) return CPRA_ERR_INVALID_ARG;
+    *count = p->launches;
+    return CPRA_OK;
+}
+
+}  // extern "C"
