@@ -259,6 +259,21 @@ def angles_for(config: int, Np: int) -> np.ndarray:
     return np.deg2rad(CONFIGS[config]["range_deg"]) * np.arange(Np, dtype=np.float64) / Np
 
 
+def random_phase_estimate(intensity_c: np.ndarray, mask: np.ndarray, rng) -> np.ndarray:
+    """Random-phase start ("random initial guess"):
+    g0_n = F^-1[M_n sqrt(I_n) e^{i phi}], phi ~ U[0, 2 pi) iid per pixel.  `rng`: a numpy Generator
+    or an integer seed (one restart of PAPER.md:64's N_r random restarts per seed)."""
+    if not isinstance(rng, np.random.Generator):
+        rng = np.random.default_rng(np.random.SeedSequence([SEED_BASE, 9, int(rng)]))
+    Np, N = intensity_c.shape[0], intensity_c.shape[-1]
+    est = np.empty((Np, N, N), dtype=np.complex64)
+    for n in range(Np):
+        A_native = np.fft.ifftshift(np.sqrt(np.maximum(intensity_c[n].astype(np.float64), 0.0)) * mask[n])
+        phi = rng.uniform(0.0, 2.0 * math.pi, size=(N, N))
+        est[n] = np.fft.ifft2(A_native * np.exp(1j * phi)).astype(np.complex64)
+    return est
+
+
 def make_problem(config: int, Np: Optional[int] = None, N: Optional[int] = None,
                  seed_offset: int = 0, keep_object: bool = False,
                  noise: bool = True) -> Problem:
@@ -300,12 +315,7 @@ def make_problem(config: int, Np: Optional[int] = None, N: Optional[int] = None,
         sup = a > 0.2 * a.max(axis=(-2, -1), keepdims=True)
     support = _dilate(sup, cfg["support_r"]).astype(np.uint8)
 
-    # random-phase start: g0 = F^-1[M A e^{i phi}], phi ~ U[0, 2 pi)
-    A_native = np.fft.ifftshift(np.sqrt(np.maximum(I_c.astype(np.float64), 0.0)) * mask, axes=(-2, -1))
-    est = np.empty((Np, N, N), dtype=np.complex64)
-    for n in range(Np):
-        phi = rng_phase.uniform(0.0, 2.0 * math.pi, size=(N, N))
-        est[n] = np.fft.ifft2(A_native[n] * np.exp(1j * phi)).astype(np.complex64)
+    est = random_phase_estimate(I_c, mask, rng_phase)
 
     return Problem(config=config, N=N, Np=Np, angles=angles,
                    intensity=np.ascontiguousarray(I_c), mask=np.ascontiguousarray(mask),

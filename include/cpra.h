@@ -189,6 +189,21 @@ int cpra_reconstruct_host(cpra_plan_t plan, void* d_stage, size_t stage_bytes,
  * Results are bit-identical for every chunk size.  Errors: INVALID_ARG. */
 int cpra_set_chunk(cpra_plan_t plan, int images);
 
+/*
+ * Per-kernel timing for the roofline report (bench.py): while enabled, every kernel launch of
+ * cpra_iterate is bracketed by CUDA events on the plan's stream, summed per kernel class.
+ * cpra_profile_read synchronises the stream, writes the accumulated milliseconds and launch counts
+ * (HOST arrays of CPRA_PROFILE_CLASSES entries) and resets them.  Not for use inside a timed
+ * throughput measurement: the event records sit between the launches.
+ * Errors: INVALID_ARG, CUDA.
+ */
+#define CPRA_PROFILE_ROW_FWD 0 /* mix + forward row FFT */
+#define CPRA_PROFILE_COL 1     /* forward column FFT + error + modulus + inverse column FFT */
+#define CPRA_PROFILE_ROW_INV 2 /* inverse row FFT + support / HIO */
+#define CPRA_PROFILE_CLASSES 3
+int cpra_profile(cpra_plan_t plan, int enable);
+int cpra_profile_read(cpra_plan_t plan, double* h_ms, long* h_launches);
+
 /* Number of kernels this plan has launched since it was created (for bench.py's gpu_launches). */
 int cpra_launch_count(cpra_plan_t plan, long* count);
 

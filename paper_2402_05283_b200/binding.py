@@ -17,6 +17,8 @@ ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_READY, ERR_WORKSPACE, ERR_CUDA, E
 ITERATE, SUPPORTED = 0, 1
 FLAG_DEFAULT, FLAG_FORCE_MULTIPASS, FLAG_NO_CHUNKING = 0, 1, 2
 MAX_K = 8
+PROFILE_CLASSES = 3
+PROFILE_NAMES = ("row_fwd", "col", "row_inv")
 
 _vp, _ci, _cf, _cl, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_long, ctypes.c_size_t
 
@@ -39,6 +41,8 @@ SIGNATURES = {
     "cpra_host_staging_bytes": (_ci, [_vp, ctypes.POINTER(_sz)]),
     "cpra_reconstruct_host": (_ci, [_vp, _vp, _sz, _vp, _vp, _vp, _vp, _vp, _ci, _cf, _vp, _vp, _vp]),
     "cpra_set_chunk": (_ci, [_vp, _ci]),
+    "cpra_profile": (_ci, [_vp, _ci]),
+    "cpra_profile_read": (_ci, [_vp, _vp, _vp]),
     "cpra_launch_count": (_ci, [_vp, ctypes.POINTER(_cl)]),
     "cpra_destroy": (_ci, [_vp]),
     "cpra_status_string": (ctypes.c_char_p, [_ci]),
@@ -202,6 +206,16 @@ class Plan:
         out = torch.empty_like(stack)
         _chk(self._l.cpra_fft2(self._h, _dptr(stack, torch.complex64, self._px), out.data_ptr(), int(sign)), "cpra_fft2")
         return out
+
+    def profile(self, enable: bool):
+        _chk(self._l.cpra_profile(self._h, int(bool(enable))), "cpra_profile")
+
+    def profile_read(self):
+        """{class name: (milliseconds, launches)} accumulated since the last read (synchronises)."""
+        ms = (ctypes.c_double * PROFILE_CLASSES)()
+        cnt = (_cl * PROFILE_CLASSES)()
+        _chk(self._l.cpra_profile_read(self._h, ms, cnt), "cpra_profile_read")
+        return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(PROFILE_NAMES)}
 
     @property
     def launch_count(self) -> int:

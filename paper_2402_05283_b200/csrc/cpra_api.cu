@@ -45,6 +45,12 @@ struct cpra_plan_s {
     std::vector<int> h_ustart, h_rays;
     long launches = 0;
     int chunk = 0;  // images per L2-resident chunk; 0 = all
+    // per-kernel-class timing (cpra_profile): event pairs around every launch of the loop
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev;      // 2 * PROF_PAIRS events, created on first use
+    std::vector<int> ev_cls;          // class of each recorded pair
+    double prof_ms[CPRA_PROFILE_CLASSES] = {0};
+    long prof_n[CPRA_PROFILE_CLASSES] = {0};
 };
 
 namespace {
@@ -130,6 +136,42 @@ MixParams mix_params(const cpra_plan_s* p)
     return mp;
 }
 
+constexpr int PROF_PAIRS = 2048;
+
+// fold the recorded event pairs into the per-class sums (synchronises the stream)
+int prof_drain(cpra_plan_s* p)
+{
+    if (p->ev_cls.empty()) return CPRA_OK;
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    for (size_t i = 0; i < p->ev_cls.size(); ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p->ev[2 * i], p->ev[2 * i + 1]) != cudaSuccess) return CPRA_ERR_CUDA;
+        p->prof_ms[p->ev_cls[i]] += (double)ms;
+        p->prof_n[p->ev_cls[i]] += 1;
+    }
+    p->ev_cls.clear();
+    return CPRA_OK;
+}
+
+struct ProfScope {
+    cpra_plan_s* p;
+    bool on;
+    size_t slot = 0;
+    ProfScope(cpra_plan_s* p_, int cls) : p(p_), on(p_->profiling)
+    {
+        if (!on) return;
+        if (p->ev.empty()) {
+            p->ev.resize(2 * PROF_PAIRS);
+            for (auto& e : p->ev) cudaEventCreate(&e);
+        }
+        if (p->ev_cls.size() == PROF_PAIRS) prof_drain(p);
+        slot = p->ev_cls.size();
+        p->ev_cls.push_back(cls);
+        cudaEventRecord(p->ev[2 * slot], p->stream);
+    }
+    ~ProfScope() { if (on) cudaEventRecord(p->ev[2 * slot + 1], p->stream); }
+};
+
 int check_launch(cpra_plan_s* p, int n = 1)
 {
     p->launches += n;
@@ -151,6 +193,7 @@ int launch_row_fwd(cpra_plan_s* p, const float2* cur, int mode, int n0, int nimg
     const dim3 grid((unsigned)nimg * (N / TB));
     const int smem = row_smem_bytes<N>();
     const MixParams mp = mix_params(p);
+    ProfScope prof(p, CPRA_PROFILE_ROW_FWD);
 #define ROWFWD(M) k_row_fwd<N, NT, M><<<grid, NT, smem, p->stream>>>(cur, p->scr, p->tw, p->S16, mp, p->Np, n0, nimg)
     switch (mode) {
         case MIX_NONE: ROWFWD(MIX_NONE); break;
@@ -168,6 +211,7 @@ int launch_col(cpra_plan_s* p, int mode, int n0, int nimg, float scale)
     constexpr int NT = threads_for<N>();
     const dim3 grid((unsigned)nimg * (N / TB));
     const int smem = col_smem_bytes<N>();
+    ProfScope prof(p, CPRA_PROFILE_COL);
     switch (mode) {
         case COL_FULL: k_col<N, NT, COL_FULL><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
         case COL_FWD: k_col<N, NT, COL_FWD><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
@@ -183,6 +227,7 @@ int launch_row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, bool hio, int
     const dim3 grid((unsigned)nimg * (N / TB));
     const int smem = row_smem_bytes<N>();
     const MixParams mp = mix_params(p);
+    ProfScope prof(p, CPRA_PROFILE_ROW_INV);
 #define ROWINV(H, M) k_row_inv<N, NT, H, M><<<grid, NT, smem, p->stream>>>(p->scr, cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg)
     if (!hio) ROWINV(ROWINV_PLAIN, MIX_NONE);
     else if (mode == MIX_NONE) ROWINV(ROWINV_HIO, MIX_NONE);
@@ -272,6 +317,7 @@ int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream
 int cpra_destroy(cpra_plan_t p)
 {
     if (!p) return CPRA_ERR_INVALID_ARG;
+    for (auto& e : p->ev) cudaEventDestroy(e);
     delete p;
     return CPRA_OK;
 }
@@ -536,6 +582,25 @@ int cpra_reconstruct_host(cpra_plan_t p, void* d_stage, size_t stage_bytes, cons
         if (h_Eglobal && !D2H(h_Eglobal, d_E + p->Np, sizeof(float))) return CPRA_ERR_CUDA;
     }
     return cudaStreamSynchronize(p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+}
+
+int cpra_profile(cpra_plan_t p, int enable)
+{
+    if (!p) return CPRA_ERR_INVALID_ARG;
+    if (!enable && p->profiling) { if (int rc = prof_drain(p)) return rc; }
+    p->profiling = enable != 0;
+    return CPRA_OK;
+}
+
+int cpra_profile_read(cpra_plan_t p, double* h_ms, long* h_launches)
+{
+    if (!p || !h_ms || !h_launches) return CPRA_ERR_INVALID_ARG;
+    if (int rc = prof_drain(p)) return rc;
+    for (int c = 0; c < CPRA_PROFILE_CLASSES; ++c) {
+        h_ms[c] = p->prof_ms[c]; h_launches[c] = p->prof_n[c];
+        p->prof_ms[c] = 0.0; p->prof_n[c] = 0;
+    }
+    return CPRA_OK;
 }
 
 int cpra_launch_count(cpra_plan_t p, long* count)

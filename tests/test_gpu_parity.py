@@ -1,0 +1,341 @@
+"""Parity of the CUDA path (through the C ABI) with the FP64 oracle, element by element, on the
+same seeded inputs.  Tolerances are north_star's (BASELINE.json): one applied iteration
+relative L2 <= 1e-5; a 20-iteration run relative L2 <= 1e-3 with the Fourier error metric within
+1e-4 relative.  Integer / byte outputs (the assembly weight) are compared bit-exactly.
+
+Run on the B200 box:  python -m pytest tests -m gpu -x -q"""
+import numpy as np
+import pytest
+
+import cpra_inputs
+from conftest import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_1 = 1e-5      # one applied iteration
+TOL_20 = 1e-3     # 20 iterations
+TOL_E = 1e-4      # error metric, relative
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "the gpu-marked tests need a CUDA device"
+    return torch
+
+
+def _gpu(problem, alpha=(0.6, 0.2), n_ei=1, flags=0):
+    import paper_2402_05283_b200 as cpra
+    return cpra.Plan(problem.N, problem.Np, flags=flags).load(problem, alpha, n_ei)
+
+
+def _oracle(problem, alpha=(0.6, 0.2), n_ei=1, precision="f64"):
+    from oracle import Oracle
+    return Oracle(problem.N, problem.Np, precision).load(problem, alpha, n_ei)
+
+
+def _get(plan, which=0):
+    return plan.get_projections(which).cpu().numpy()
+
+
+def _errors(plan):
+    E, Eg = plan.get_error()
+    return E.cpu().numpy().astype(np.float64), float(Eg.cpu()[0])
+
+
+# ------------------------------------------------------------------------------------------------
+# the library's own FFT (the kernels of the loop) against numpy's, every supported N
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [16, 32, 64, 128, 256, 512, 1024])
+def test_fft2_all_sizes(torch_cuda, N):
+    import paper_2402_05283_b200 as cpra
+    Np = 3
+    rng = np.random.default_rng(N)
+    x = (rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))).astype(np.complex64)
+    plan = cpra.Plan(N, Np)
+    d = torch_cuda.from_numpy(x).cuda()
+    F = plan.fft2(d, -1).cpu().numpy()
+    ref = np.fft.fft2(x.astype(np.complex128))
+    assert rel_l2(F, ref) < 2e-6, rel_l2(F, ref)
+    B = plan.fft2(torch_cuda.from_numpy(F).cuda(), +1).cpu().numpy()
+    assert rel_l2(B, x) < 3e-6
+    # a delta at (y0, x0) pins the index order and the sign of the exponent
+    dl = np.zeros((Np, N, N), np.complex64)
+    dl[:, 3, 5] = 1.0
+    Fd = plan.fft2(torch_cuda.from_numpy(dl).cuda(), -1).cpu().numpy()
+    ky, kx = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    assert np.abs(Fd[1] - np.exp(-2j * np.pi * (3 * ky + 5 * kx) / N)).max() < 1e-5
+
+
+# ------------------------------------------------------------------------------------------------
+# single applied iteration, from t = 0 and from oracle states at t = 10 and t = 19
+# ------------------------------------------------------------------------------------------------
+CASES = [
+    # (config, Np, N)  -- N = None: the config's own size; Np reduced so the oracle finishes in seconds
+    (1, 32, None),
+    (2, 12, None),
+    (3, 6, None),
+    (4, 4, None),
+    (5, 3, None),
+]
+
+
+@pytest.fixture(scope="module")
+def problems():
+    cache = {}
+
+    def get(cfg, Np, N=None):
+        key = (cfg, Np, N)
+        if key not in cache:
+            cache[key] = cpra_inputs.make_problem(cfg, Np=Np, N=N)
+        return cache[key]
+    return get
+
+
+@pytest.mark.parametrize("cfg,Np,N", CASES)
+def test_single_iteration(torch_cuda, problems, cfg, Np, N):
+    p = problems(cfg, Np, N)
+    o = _oracle(p)
+    g = _gpu(p)
+    o.iterate(1, p.beta)
+    g.iterate(1, p.beta)
+    r = rel_l2(_get(g), o.get_projections(0))
+    assert r <= TOL_1, r
+    E, Eg = _errors(g)
+    Eo, Ego = o.get_error()
+    assert abs(Eg - Ego) <= TOL_E * Ego and np.abs(E - Eo).max() <= TOL_E * Eo.max()
+    assert rel_l2(_get(g, 1), o.get_projections(1)) <= TOL_1
+
+
+@pytest.mark.parametrize("cfg,Np,N", CASES[:3])
+def test_single_iteration_from_later_oracle_states(torch_cuda, problems, cfg, Np, N):
+    """Isolates the per-step error from the drift: load the oracle's state at t = 10 and t = 19
+    (rounded to fp32 on both sides) and apply one iteration."""
+    from oracle import Oracle
+    p = problems(cfg, Np, N)
+    o = _oracle(p)
+    g = _gpu(p)
+    done = 0
+    for t in (10, 19):
+        o.iterate(t - done, p.beta)
+        done = t
+        state = o.get_projections(0).astype(np.complex64)
+        o2 = Oracle(p.N, p.Np).load(p)
+        o2.set_estimate(state)
+        o2.set_iteration(t)
+        o2.iterate(1, p.beta)
+        g.set_estimate(torch_cuda.from_numpy(state).cuda())
+        g.iteration = t
+        g.iterate(1, p.beta)
+        r = rel_l2(_get(g), o2.get_projections(0))
+        assert r <= TOL_1, (t, r)
+
+
+# ------------------------------------------------------------------------------------------------
+# 20 iterations: iterate, E(t) for every t, n_ei = 1 and 2; float-oracle drift printed beside it
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_ei", [1, 2])
+@pytest.mark.parametrize("cfg,Np,N", CASES)
+def test_twenty_iterations(torch_cuda, problems, cfg, Np, N, n_ei):
+    p = problems(cfg, Np, N)
+    o = _oracle(p, n_ei=n_ei)
+    f = _oracle(p, n_ei=n_ei, precision="f32")
+    g = _gpu(p, n_ei=n_ei)
+    for t in range(20):
+        o.iterate(1, p.beta)
+        g.iterate(1, p.beta)
+        _, Eg = _errors(g)
+        _, Ego = o.get_error()
+        assert abs(Eg - Ego) <= TOL_E * Ego, (t, Eg, Ego)
+    f.iterate(20, p.beta)
+    ref = o.get_projections(0)
+    r = rel_l2(_get(g), ref)
+    rs = rel_l2(_get(g, 1), o.get_projections(1))
+    rf = rel_l2(f.get_projections(0), ref)
+    print(f"\nconfig {cfg} Np={Np} n_ei={n_ei}: relL2@20 ITERATE gpu={r:.3e} float-oracle={rf:.3e} SUPPORTED gpu={rs:.3e}")
+    assert r <= TOL_20, (r, rf)
+    assert rs <= TOL_20, rs
+
+
+def test_tiny_full_run(torch_cuda, problems):
+    """Config 1 as BASELINE.json states it: 50 iterations, beta = 0.9.  The error metric of every
+    iteration agrees; the iterate is reported (the map amplifies differences ~1.5x per iteration)."""
+    p = problems(1, 32)
+    o, g = _oracle(p), _gpu(p)
+    for t in range(p.iters):
+        o.iterate(1, p.beta)
+        g.iterate(1, p.beta)
+        if t % 10 == 9:
+            _, Eg = _errors(g)
+            _, Ego = o.get_error()
+            assert abs(Eg - Ego) <= 5e-3 * Ego, (t, Eg, Ego)
+    print(f"\ntiny 50 it: relL2={rel_l2(_get(g), o.get_projections(0)):.3e}")
+
+
+# ------------------------------------------------------------------------------------------------
+# carousel variants and degenerate stacks
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("alpha,n_ei", [((1.0,), 1), ((0.5, 0.2, 0.05), 1), ((0.4, 0.15, 0.1, 0.05), 3), ((0.7, 0.15), 10)])
+def test_carousel_variants(torch_cuda, alpha, n_ei):
+    p = cpra_inputs.random_stack(64, 9, seed=3, beamstop=3)
+    o, g = _oracle(p, alpha, n_ei), _gpu(p, alpha, n_ei)
+    o.iterate(4, 0.9)
+    g.iterate(4, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 4 * TOL_1
+    _, Eg = _errors(g)
+    assert abs(Eg - o.get_error()[1]) <= TOL_E * o.get_error()[1]
+
+
+@pytest.mark.parametrize("N,Np", [(16, 1), (16, 2), (32, 3), (64, 1), (128, 5), (256, 2), (512, 1), (1024, 1)])
+def test_small_and_ragged_stacks(torch_cuda, N, Np):
+    """Np = 1 and 2 (no room for K = 1: default falls back to no coupling), Np = 3 (every image is
+    every other's neighbour), every supported N."""
+    p = cpra_inputs.random_stack(N, Np, seed=N + Np, beamstop=3 if N > 16 else 0)
+    alpha = (0.6, 0.2) if Np >= 3 else (1.0,)
+    o, g = _oracle(p, alpha), _gpu(p, alpha)
+    o.iterate(2, 0.9)
+    g.iterate(2, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 2 * TOL_1
+    E, Eg = _errors(g)
+    Eo, Ego = o.get_error()
+    assert np.abs(E - Eo).max() <= TOL_E * Eo.max() and abs(Eg - Ego) <= TOL_E * Ego
+
+
+def test_degenerate_values(torch_cuda):
+    """|G| = 0 everywhere (zero estimate: phase 0, reading A13), negative intensities (A = 0,
+    reading A14), everything masked, empty and full supports."""
+    import paper_2402_05283_b200 as cpra
+    from oracle import Oracle
+    N, Np = 32, 4
+    base = cpra_inputs.random_stack(N, Np, seed=11)
+    variants = []
+    z = cpra_inputs.random_stack(N, Np, seed=11); z.estimate[:] = 0; variants.append(("zero estimate", z))
+    ng = cpra_inputs.random_stack(N, Np, seed=11); ng.intensity[:, ::2] *= -1; variants.append(("negative I", ng))
+    am = cpra_inputs.random_stack(N, Np, seed=11); am.mask[:] = 0; variants.append(("all masked", am))
+    es = cpra_inputs.random_stack(N, Np, seed=11); es.support[:] = 0; variants.append(("empty support", es))
+    fs = cpra_inputs.random_stack(N, Np, seed=11); fs.support[:] = 1; variants.append(("full support", fs))
+    for name, p in variants:
+        o, g = _oracle(p), _gpu(p)
+        o.iterate(2, 0.9)
+        g.iterate(2, 0.9)
+        ref = o.get_projections(0)
+        out = _get(g)
+        assert np.isfinite(out.view(np.float32)).all(), name
+        assert np.linalg.norm(out - ref) <= 2 * TOL_1 * max(np.linalg.norm(ref), 1e-30) + 1e-30, name
+        E, Eg = _errors(g)
+        Eo, Ego = o.get_error()
+        assert np.abs(E - Eo).max() <= TOL_E * max(Eo.max(), 1e-30) + 1e-12, (name, E, Eo)
+    assert base is not None
+
+
+# ------------------------------------------------------------------------------------------------
+# API properties (SURVEY.md 8(c) "pins": API)
+# ------------------------------------------------------------------------------------------------
+def test_iterate_splits_are_bit_identical_and_state_round_trips(torch_cuda):
+    p = cpra_inputs.random_stack(128, 7, seed=5, beamstop=5)
+    a = _gpu(p, n_ei=2); a.iterate(7, 0.9)
+    b = _gpu(p, n_ei=2); b.iterate(3, 0.9); b.iterate(0, 0.9); b.iterate(4, 0.9)
+    ga, gb = _get(a), _get(b)
+    assert np.array_equal(ga.view(np.uint32), gb.view(np.uint32))
+    assert a.iteration == b.iteration == 7
+    # checkpoint / resume: get -> set (+ iteration counter) reproduces the run exactly
+    c = _gpu(p, n_ei=2); c.iterate(3, 0.9)
+    state = c.get_projections(0)
+    d = _gpu(p, n_ei=2); d.set_estimate(state); d.iteration = 3; d.iterate(4, 0.9)
+    assert np.array_equal(_get(d).view(np.uint32), ga.view(np.uint32))
+    Ea, Ega = _errors(a)
+    Ed, Egd = _errors(d)
+    assert np.array_equal(Ea, Ed) and Ega == Egd
+
+
+def test_chunking_and_multipass_flags_do_not_change_results(torch_cuda):
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(64, 10, seed=8, beamstop=3)
+    ref = _gpu(p); ref.iterate(3, 0.9)
+    r = _get(ref)
+    for chunk in (1, 3, 4, 10, 64):
+        q = _gpu(p); q.set_chunk(chunk); q.iterate(3, 0.9)
+        assert np.array_equal(_get(q).view(np.uint32), r.view(np.uint32)), chunk
+    q = _gpu(p, flags=cpra.FLAG_FORCE_MULTIPASS | cpra.FLAG_NO_CHUNKING); q.iterate(3, 0.9)
+    assert rel_l2(_get(q), r) <= TOL_1
+
+
+def test_not_ready_and_argument_errors(torch_cuda):
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(32, 4, seed=1)
+    plan = cpra.Plan(32, 4)
+    with pytest.raises(cpra.CpraError) as e:
+        plan.iterate(1)
+    assert e.value.code == cpra.ERR_NOT_READY
+    plan.set_data(torch_cuda.from_numpy(p.intensity).cuda())
+    plan.set_support(torch_cuda.from_numpy(p.support).cuda())
+    with pytest.raises(cpra.CpraError) as e:
+        plan.iterate(1)
+    assert e.value.code == cpra.ERR_NOT_READY
+    with pytest.raises(cpra.CpraError) as e:
+        plan.get_error()
+    assert e.value.code == cpra.ERR_NOT_READY
+    plan.set_estimate(torch_cuda.from_numpy(p.estimate).cuda())
+    plan.iterate(0)                                                     # valid no-op
+    assert np.array_equal(_get(plan), p.estimate)
+    with pytest.raises(cpra.CpraError) as e:
+        plan.iterate(-1)
+    assert e.value.code == cpra.ERR_INVALID_ARG
+    with pytest.raises(cpra.CpraError) as e:
+        plan.set_carousel([0.2, 0.2, 0.2], 1)                           # 2K+1 > Np
+    assert e.value.code == cpra.ERR_INVALID_ARG
+    n0 = plan.launch_count
+    plan.iterate(2)
+    assert plan.launch_count > n0
+
+
+def test_reconstruct_host_equals_device_calls(torch_cuda):
+    p = cpra_inputs.random_stack(64, 6, seed=9, beamstop=3)
+    g = _gpu(p); g.iterate(5, 0.9)
+    E, Eg = _errors(g)
+    import paper_2402_05283_b200 as cpra
+    h = cpra.Plan(64, 6)
+    out, Eh, Egh = h.reconstruct_host(p.intensity, p.mask, p.angles, p.support, p.estimate, 5, 0.9)
+    assert np.array_equal(out.numpy().view(np.uint32), _get(g).view(np.uint32))
+    assert np.array_equal(Eh.numpy().astype(np.float64), E) and Egh == Eg
+
+
+# ------------------------------------------------------------------------------------------------
+# Fourier-slice assembly (A7)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,Np,N", [(1, 32, None), (2, 10, 64), (4, 12, 64)])
+def test_assembly_parity(torch_cuda, problems, cfg, Np, N):
+    p = problems(cfg, Np, N)
+    o, g = _oracle(p), _gpu(p)
+    o.iterate(3, p.beta)
+    g.iterate(3, p.beta)
+    vo, wo = o.assemble_3d()
+    vg, wg = g.assemble_3d()
+    assert np.array_equal(wg.cpu().numpy().astype(np.float64), wo)              # exact: which voxels are filled
+    assert rel_l2(vg.cpu().numpy(), vo) <= 3 * TOL_1
+    # the loop state is untouched by the assembly
+    o.iterate(1, p.beta); g.iterate(1, p.beta)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 2 * TOL_1
+
+
+def test_assembly_exact_grid_lines(torch_cuda):
+    """theta = 0 and 90 degrees land on grid lines: with the true projections as the estimate
+    those voxels equal the 3D FT of the object (Fourier slice theorem)."""
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.make_problem(1, Np=4, keep_object=True, noise=False)       # angles 0, 45, 90, 135
+    N = p.N
+    plan = cpra.Plan(N, p.Np)
+    plan.set_data(torch_cuda.from_numpy(p.intensity).cuda(), None, p.angles)
+    plan.set_support(torch_cuda.ones((p.Np, N, N), dtype=torch_cuda.uint8, device="cuda"))
+    plan.set_estimate(torch_cuda.from_numpy(p.projections.astype(np.complex64)).cuda())
+    vol, w = plan.assemble_3d()
+    vol = vol.cpu().numpy()
+    pad = np.zeros((N, N, N))
+    o = (N - p.obj.shape[0]) // 2
+    pad[o:o + p.obj.shape[0], o:o + p.obj.shape[0], o:o + p.obj.shape[0]] = p.obj
+    F3 = np.fft.fftn(pad)
+    h = N // 2
+    for kz in (0, 1, 5, N - 3):
+        for k in (1, 2, 7, h - 1):
+            for idx in ((kz, 0, k), (kz, 0, N - k), (kz, k, 0), (kz, N - k, 0)):
+                assert abs(vol[idx] - F3[idx]) <= 2e-5 * np.abs(F3).max(), idx
