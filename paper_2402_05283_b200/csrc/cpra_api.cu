@@ -9,7 +9,7 @@
 #include <vector>
 
 #include "../../include/cpra.h"
-#include "cpra_kernels.cuh"
+#include "cpra_layout.cuh"
 
 using namespace cpra;
 
@@ -21,11 +21,11 @@ struct cpra_plan_s {
     // workspace carve-up
     char* ws = nullptr;
     size_t ws_bytes = 0;
-    float2* tw = nullptr;
+    float4* tw = nullptr;
     float* A = nullptr;
     uint16_t* S16 = nullptr;
-    float2* st[2] = {nullptr, nullptr};
-    float2* scr = nullptr;
+    float4* st[2] = {nullptr, nullptr};
+    float4* scr = nullptr;
     double* partial = nullptr;
     double* den = nullptr;
     double* uphi = nullptr;
@@ -40,7 +40,7 @@ struct cpra_plan_s {
     bool have_data = false, have_support = false, have_estimate = false, have_error = false;
     bool attrs_set = false;
     std::vector<double> angles;
-    std::vector<float2> h_tw;
+    std::vector<float4> h_tw;
     std::vector<double> h_uphi;
     std::vector<int> h_ustart, h_rays;
     long launches = 0;
@@ -71,7 +71,7 @@ Layout layout_of(int N, int Np)
     const size_t px = (size_t)Np * N * N;
     Carve c;
     Layout L;
-    L.tw = c.take(sizeof(float2) * N);
+    L.tw = c.take(sizeof(float4) * 1024);   // >= tw_quads<N>() for every N
     L.A = c.take(sizeof(float) * px);
     L.S16 = c.take(px / 8);
     L.st0 = c.take(sizeof(float2) * px);
@@ -88,7 +88,27 @@ Layout layout_of(int N, int Np)
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
-template <int N> constexpr int threads_for() { return N <= 32 ? 64 : N <= 128 ? 128 : N <= 512 ? 256 : 512; }
+// per-stage twiddle tables of cpra_fft.cuh: quads [wr, wr, wi, wi], w = exp(-2 pi i n2 r / L),
+// computed in double and rounded once
+template <int N>
+void build_twiddles(std::vector<float4>& t)
+{
+    using RX = Radix<N>;
+    const double PI = 3.14159265358979323846264338327950288;
+    t.clear();
+    auto stage = [&](int L, int R) {
+        const int M = L / R;
+        for (int n2 = 0; n2 < M; ++n2)
+            for (int r = 1; r < R; ++r) {
+                const double a = -2.0 * PI * (double)(n2 * r) / (double)L;
+                const float wr = (float)std::cos(a), wi = (float)std::sin(a);
+                t.push_back(make_float4(wr, wr, wi, wi));
+            }
+    };
+    stage(N, RX::R0);
+    if (RX::S == 3) stage(N / RX::R0, RX::R1);
+    t.resize(1024, make_float4(0.f, 0.f, 0.f, 0.f));
+}
 
 #define CPRA_DISPATCH_N(N_, ...)                                                     \
     switch (N_) {                                                                    \
@@ -111,20 +131,21 @@ cudaError_t allow_smem(F* f, int bytes)
 template <int N>
 int set_attrs()
 {
-    constexpr int NT = threads_for<N>();
+    static_assert(tw_quads<N>() <= 1024, "twiddle region of the workspace too small");
     cudaError_t e = cudaSuccess;
     auto acc = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-    acc(allow_smem(k_row_fwd<N, NT, MIX_NONE>, row_smem_bytes<N>()));
-    acc(allow_smem(k_row_fwd<N, NT, MIX_K1>, row_smem_bytes<N>()));
-    acc(allow_smem(k_row_fwd<N, NT, MIX_GEN>, row_smem_bytes<N>()));
-    acc(allow_smem(k_row_fwd<N, NT, MIX_MASK>, row_smem_bytes<N>()));
-    acc(allow_smem(k_col<N, NT, COL_FULL>, col_smem_bytes<N>()));
-    acc(allow_smem(k_col<N, NT, COL_FWD>, col_smem_bytes<N>()));
-    acc(allow_smem(k_col<N, NT, COL_INV>, col_smem_bytes<N>()));
-    acc(allow_smem(k_row_inv<N, NT, ROWINV_PLAIN, MIX_NONE>, row_smem_bytes<N>()));
-    acc(allow_smem(k_row_inv<N, NT, ROWINV_HIO, MIX_NONE>, row_smem_bytes<N>()));
-    acc(allow_smem(k_row_inv<N, NT, ROWINV_HIO, MIX_K1>, row_smem_bytes<N>()));
-    acc(allow_smem(k_row_inv<N, NT, ROWINV_HIO, MIX_GEN>, row_smem_bytes<N>()));
+    constexpr int SM = smem_bytes<N>();
+    acc(allow_smem(k_row_fwd<N, MIX_NONE>, SM));
+    acc(allow_smem(k_row_fwd<N, MIX_K1>, SM));
+    acc(allow_smem(k_row_fwd<N, MIX_GEN>, SM));
+    acc(allow_smem(k_row_fwd<N, MIX_MASK>, SM));
+    acc(allow_smem(k_col<N, COL_FULL>, SM));
+    acc(allow_smem(k_col<N, COL_FWD>, SM));
+    acc(allow_smem(k_col<N, COL_INV>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_PLAIN, MIX_NONE>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_NONE>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_K1>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_GEN>, SM));
     return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
 }
 
@@ -187,14 +208,14 @@ int mix_mode(const cpra_plan_s* p, bool fires)
 }
 
 template <int N>
-int launch_row_fwd(cpra_plan_s* p, const float2* cur, int mode, int n0, int nimg)
+int launch_row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg)
 {
-    constexpr int NT = threads_for<N>();
+    constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / TB));
-    const int smem = row_smem_bytes<N>();
+    const int smem = smem_bytes<N>();
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_FWD);
-#define ROWFWD(M) k_row_fwd<N, NT, M><<<grid, NT, smem, p->stream>>>(cur, p->scr, p->tw, p->S16, mp, p->Np, n0, nimg)
+#define ROWFWD(M) k_row_fwd<N, M><<<grid, NT, smem, p->stream>>>(cur, p->scr, p->tw, p->S16, mp, p->Np, n0, nimg)
     switch (mode) {
         case MIX_NONE: ROWFWD(MIX_NONE); break;
         case MIX_K1: ROWFWD(MIX_K1); break;
@@ -208,27 +229,27 @@ int launch_row_fwd(cpra_plan_s* p, const float2* cur, int mode, int n0, int nimg
 template <int N>
 int launch_col(cpra_plan_s* p, int mode, int n0, int nimg, float scale)
 {
-    constexpr int NT = threads_for<N>();
+    constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / TB));
-    const int smem = col_smem_bytes<N>();
+    const int smem = smem_bytes<N>();
     ProfScope prof(p, CPRA_PROFILE_COL);
     switch (mode) {
-        case COL_FULL: k_col<N, NT, COL_FULL><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
-        case COL_FWD: k_col<N, NT, COL_FWD><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
-        default: k_col<N, NT, COL_INV><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
+        case COL_FULL: k_col<N, COL_FULL><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
+        case COL_FWD: k_col<N, COL_FWD><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
+        default: k_col<N, COL_INV><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
     }
     return check_launch(p);
 }
 
 template <int N>
-int launch_row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg)
+int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg)
 {
-    constexpr int NT = threads_for<N>();
+    constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / TB));
-    const int smem = row_smem_bytes<N>();
+    const int smem = smem_bytes<N>();
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_INV);
-#define ROWINV(H, M) k_row_inv<N, NT, H, M><<<grid, NT, smem, p->stream>>>(p->scr, cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg)
+#define ROWINV(H, M) k_row_inv<N, H, M><<<grid, NT, smem, p->stream>>>(p->scr, cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg)
     if (!hio) ROWINV(ROWINV_PLAIN, MIX_NONE);
     else if (mode == MIX_NONE) ROWINV(ROWINV_HIO, MIX_NONE);
     else if (mode == MIX_K1) ROWINV(ROWINV_HIO, MIX_K1);
@@ -302,13 +323,7 @@ int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream
     else { p->K = 0; p->alpha[0] = 1.0f; }
     p->n_ei = 1;
     p->angles.assign(Np, 0.0);
-    // twiddles exp(-2 pi i m / N), computed in double and rounded once
-    p->h_tw.resize(N);
-    const double PI = 3.14159265358979323846264338327950288;
-    for (int m = 0; m < N; ++m) {
-        const double a = -2.0 * PI * (double)m / (double)N;
-        p->h_tw[m] = make_float2((float)std::cos(a), (float)std::sin(a));
-    }
+    { auto f = [&]() -> int { CPRA_DISPATCH_N(N, build_twiddles<NN>(p->h_tw)); return 0; }; f(); }
     if (const char* e = std::getenv("CPRA_CHUNK")) p->chunk = std::max(0, std::atoi(e));
     *out = p;
     return CPRA_OK;
@@ -336,12 +351,12 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
     if (bytes < L.total || ((uintptr_t)d_ws & 255)) return CPRA_ERR_WORKSPACE;
     char* w = (char*)d_ws;
     p->ws = w; p->ws_bytes = bytes;
-    p->tw = (float2*)(w + L.tw);
+    p->tw = (float4*)(w + L.tw);
     p->A = (float*)(w + L.A);
     p->S16 = (uint16_t*)(w + L.S16);
-    p->st[0] = (float2*)(w + L.st0);
-    p->st[1] = (float2*)(w + L.st1);
-    p->scr = (float2*)(w + L.scr);
+    p->st[0] = (float4*)(w + L.st0);
+    p->st[1] = (float4*)(w + L.st1);
+    p->scr = (float4*)(w + L.scr);
     p->partial = (double*)(w + L.partial);
     p->den = (double*)(w + L.den);
     p->uphi = (double*)(w + L.uphi);
@@ -355,7 +370,7 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
         if (rc != CPRA_OK) { p->ws = nullptr; return rc; }
         p->attrs_set = true;
     }
-    if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float2) * p->N, cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
+    if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float4) * p->h_tw.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
         p->ws = nullptr;
         return CPRA_ERR_CUDA;
     }
@@ -401,7 +416,7 @@ int cpra_set_estimate(cpra_plan_t p, const float* d_g0)
     if (!p || !d_g0) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     const size_t total = (size_t)p->Np * p->N * p->N;
-    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, p->st[p->cur], p->N, total);
+    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, (float*)p->st[p->cur], p->N, total);
     if (int rc = check_launch(p)) return rc;
     p->t = 0;
     p->have_estimate = true;
@@ -439,8 +454,8 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
     for (int it = 0; it < k; ++it) {
         const int mode = mix_mode(p, (p->t % p->n_ei) == 0);
-        const float2* cur = p->st[p->cur];
-        float2* nxt = p->st[p->cur ^ 1];
+        const float4* cur = p->st[p->cur];
+        float4* nxt = p->st[p->cur ^ 1];
         for (int n0 = 0; n0 < p->Np; n0 += chunk) {
             const int nimg = std::min(chunk, p->Np - n0);
             int rc = CPRA_OK;
@@ -475,7 +490,7 @@ int cpra_get_projections(cpra_plan_t p, int which, float* d_out)
     if (int rc = ready(p)) return rc;
     if (!p->have_estimate || (which == CPRA_SUPPORTED && !p->have_support)) return CPRA_ERR_NOT_READY;
     const size_t total = (size_t)p->Np * p->N * p->N;
-    k_unpack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>(p->st[p->cur], p->S16, (float2*)d_out, p->N, total, which == CPRA_SUPPORTED);
+    k_unpack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->st[p->cur], p->S16, (float2*)d_out, p->N, total, which == CPRA_SUPPORTED);
     return check_launch(p);
 }
 
@@ -484,11 +499,11 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
     if (!p || !d_in || !d_out || (sign != 1 && sign != -1)) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     const size_t total = (size_t)p->Np * p->N * p->N;
-    float2* tmp = p->st[p->cur ^ 1];
+    float4* tmp = p->st[p->cur ^ 1];
     const unsigned nb = blocks_for(total, 256);
     int rc = CPRA_OK;
     if (sign < 0) {
-        k_pack_state<<<nb, 256, 0, p->stream>>>((const float2*)d_in, tmp, p->N, total);
+        k_pack_state<<<nb, 256, 0, p->stream>>>((const float2*)d_in, (float*)tmp, p->N, total);
         if ((rc = check_launch(p))) return rc;
         { auto f = [&]() -> int {
             CPRA_DISPATCH_N(p->N,
@@ -496,10 +511,10 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
                 if (rc == CPRA_OK) rc = launch_col<NN>(p, COL_FWD, 0, p->Np, 1.0f));
             return 0; }; f(); }
         if (rc) return rc;
-        k_unpack_spectrum<<<nb, 256, 0, p->stream>>>(p->scr, (float2*)d_out, p->geo, total);
+        k_unpack_spectrum<<<nb, 256, 0, p->stream>>>((const float*)p->scr, (float2*)d_out, p->geo, total);
         return check_launch(p);
     }
-    k_pack_spectrum<<<nb, 256, 0, p->stream>>>((const float2*)d_in, p->scr, p->geo, total);
+    k_pack_spectrum<<<nb, 256, 0, p->stream>>>((const float2*)d_in, (float*)p->scr, p->geo, total);
     if ((rc = check_launch(p))) return rc;
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     { auto f = [&]() -> int {
@@ -508,7 +523,7 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
             if (rc == CPRA_OK) rc = launch_row_inv<NN>(p, tmp, tmp, false, MIX_NONE, 0.f, scale, 0, p->Np));
         return 0; }; f(); }
     if (rc) return rc;
-    k_unpack_state<<<nb, 256, 0, p->stream>>>(tmp, p->S16, (float2*)d_out, p->N, total, 0);
+    k_unpack_state<<<nb, 256, 0, p->stream>>>((const float*)tmp, p->S16, (float2*)d_out, p->N, total, 0);
     return check_launch(p);
 }
 
@@ -536,7 +551,7 @@ int cpra_assemble_3d(cpra_plan_t p, float* d_vol, float* d_weight)
     const int zsplit = std::max(1, std::min(N, 4096 / std::max(1, (N * N) / 256)));
     const int zper = (N + zsplit - 1) / zsplit;
     const dim3 grid(blocks_for((size_t)N * N, 128), (unsigned)((N + zper - 1) / zper));
-    k_assemble<<<grid, 128, 0, p->stream>>>(p->scr, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
+    k_assemble<<<grid, 128, 0, p->stream>>>((const float*)p->scr, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
     return check_launch(p);
 }
 

@@ -1,36 +1,45 @@
-// cpra_fft.cuh -- register/shared-memory FFT building blocks of the CPRA loop (sm_100a, complex fp32).
+// cpra_fft.cuh -- register / shared-memory FFT building blocks of the CPRA loop (sm_100a, complex fp32).
 //
 // The 2D FTs of the "conventional 2D CXDI" iteration (the N^2 log N term of
 // PAPER.md:74) are done as 1D FFTs of length N along the SLOW index of a [N][16] tile whose fast
 // index is a batch of 16 independent transforms (16 rows for the row pass, 16 columns for the
-// column pass).  A warp's lanes run along the batch index, so every shared-memory access of every
-// stage is 16 consecutive float2 = 128 B per half-warp: bank-conflict free for any stride pattern.
+// column pass).
+//
+// Packed arithmetic: a thread owns a PAIR of batch members (a, b) and keeps them as
+//     c2 = { re = (re_a, re_b), im = (im_a, im_b) }
+// so that every add / multiply / fma of the butterflies is one sm_100 packed instruction
+// (FADD2 / FMUL2 / FFMA2: two fp32 results per issue slot, negation and broadcast immediates free).
+// The same 16 bytes [re_a, re_b, im_a, im_b] ("quad") are the unit of every shared-memory and
+// global-memory layout of the loop: a position of the tile is 8 quads = 128 B, a quarter-warp of
+// LDS.128 / STS.128 reads one whole position, so every stage is bank-conflict free for any stride.
 //
 // Forward: in-place decimation-in-frequency, radices R0, R1[, R2] (first stage has stride N/R0),
 //          natural order in, digit-reversed order out:  X[k] ends at position pos(k),
 //          k = k0 + R0 (k1 + R1 k2)  ->  pos = k2 + R2 (k1 + R1 k0).
 // Inverse: the mirror image (decimation-in-time), digit-reversed in, natural out.
-// Each butterfly reads and writes the SAME R positions, so a stage needs one barrier, any number of
-// butterflies per thread, and the last forward stage / pointwise step / first inverse stage fuse in
-// registers.  The pointwise steps of the loop never need natural frequency order: sqrt(I) is stored
-// once in the permuted order (cpra_set_data).
+// Each butterfly reads and writes the SAME R positions, so a stage needs one barrier and the last
+// forward stage / pointwise step / first inverse stage fuse in registers.  The pointwise steps of
+// the loop never need natural frequency order: sqrt(I) is stored once in the permuted order.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace cpra {
 
-constexpr int TB = 16;  // tile width = batch of transforms = lanes of a half-warp
+constexpr int TB = 16;     // tile width = batch of transforms
+constexpr int NPAIR = 8;   // batch pairs = quads per position
 
 // ---- stage plan ------------------------------------------------------------------------------
+// NT = threads per CTA, chosen so that the last stage has NPAIR * N / RL = B * NT butterflies with
+// B in {1, 2}: the transposing stage of the row kernels keeps all of them in registers.
 template <int N> struct Radix;
-template <> struct Radix<16>   { static constexpr int S = 2, R0 = 4,  R1 = 4,  R2 = 1; };
-template <> struct Radix<32>   { static constexpr int S = 2, R0 = 8,  R1 = 4,  R2 = 1; };
-template <> struct Radix<64>   { static constexpr int S = 2, R0 = 8,  R1 = 8,  R2 = 1; };
-template <> struct Radix<128>  { static constexpr int S = 2, R0 = 16, R1 = 8,  R2 = 1; };
-template <> struct Radix<256>  { static constexpr int S = 2, R0 = 16, R1 = 16, R2 = 1; };
-template <> struct Radix<512>  { static constexpr int S = 3, R0 = 8,  R1 = 8,  R2 = 8; };
-template <> struct Radix<1024> { static constexpr int S = 3, R0 = 16, R1 = 8,  R2 = 8; };
+template <> struct Radix<16>   { static constexpr int S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32;  };
+template <> struct Radix<32>   { static constexpr int S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64;  };
+template <> struct Radix<64>   { static constexpr int S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64;  };
+template <> struct Radix<128>  { static constexpr int S = 2, R0 = 16, R1 = 8,  R2 = 1, NT = 128; };
+template <> struct Radix<256>  { static constexpr int S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128; };
+template <> struct Radix<512>  { static constexpr int S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256; };
+template <> struct Radix<1024> { static constexpr int S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 512; };
 
 template <int N> __host__ __device__ constexpr int last_radix() { return Radix<N>::S == 3 ? Radix<N>::R2 : Radix<N>::R1; }
 
@@ -41,125 +50,204 @@ __host__ __device__ __forceinline__ int fft_pos(int k, int R0, int R1, int R2)
     return k2 + R2 * (k1 + R1 * k0);
 }
 
-// ---- complex helpers -------------------------------------------------------------------------
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-// a * w
-__device__ __forceinline__ float2 cmul(float2 a, float2 w)
+// ---- twiddle tables ----------------------------------------------------------------------------
+// One table per stage with M = L / R > 1, entry (n2, r) for r = 1 .. R-1 at quad index
+// n2 (R - 1) + (r - 1):  [wr, wr, wi, wi],  w = exp(-2 pi i n2 r / L)  (computed in double, rounded
+// once, on the host).  Stage 0 (L = N) first, then stage 1 (L = N / R0) if the plan has 3 stages.
+template <int N> __host__ __device__ constexpr int tw_quads_stage0() { return (N / Radix<N>::R0) * (Radix<N>::R0 - 1); }
+template <int N> __host__ __device__ constexpr int tw_quads_stage1()
 {
-    return make_float2(fmaf(a.x, w.x, -a.y * w.y), fmaf(a.x, w.y, a.y * w.x));
+    return Radix<N>::S == 3 ? (N / (Radix<N>::R0 * Radix<N>::R1)) * (Radix<N>::R1 - 1) : 0;
+}
+template <int N> __host__ __device__ constexpr int tw_quads() { return tw_quads_stage0<N>() + tw_quads_stage1<N>(); }
+
+// ---- packed helpers ----------------------------------------------------------------------------
+struct c2 {
+    float2 re, im;
+};
+
+__device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 padd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 psub(float2 a, float2 b) { return __fadd2_rn(a, neg2(b)); }
+__device__ __forceinline__ float2 pmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+
+__device__ __forceinline__ c2 from_quad(float4 q) { return c2{make_float2(q.x, q.y), make_float2(q.z, q.w)}; }
+__device__ __forceinline__ float4 to_quad(c2 v) { return make_float4(v.re.x, v.re.y, v.im.x, v.im.y); }
+
+__device__ __forceinline__ c2 cadd(c2 a, c2 b) { return c2{padd(a.re, b.re), padd(a.im, b.im)}; }
+__device__ __forceinline__ c2 csub(c2 a, c2 b) { return c2{psub(a.re, b.re), psub(a.im, b.im)}; }
+// a * w, w = (wr, wi) broadcast pairs
+__device__ __forceinline__ c2 cmul(c2 a, float2 wr, float2 wi)
+{
+    return c2{pfma(a.re, wr, neg2(pmul(a.im, wi))), pfma(a.re, wi, pmul(a.im, wr))};
 }
 // a * conj(w)
-__device__ __forceinline__ float2 cmulc(float2 a, float2 w)
+__device__ __forceinline__ c2 cmulc(c2 a, float2 wr, float2 wi)
 {
-    return make_float2(fmaf(a.x, w.x, a.y * w.y), fmaf(a.y, w.x, -a.x * w.y));
+    return c2{pfma(a.re, wr, pmul(a.im, wi)), pfma(a.im, wr, neg2(pmul(a.re, wi)))};
 }
 
-// a * exp(-+ 2 pi i q / 16)  (- forward, + inverse); q is a compile-time constant after unrolling
+// lo = e + W o, hi = e - W o with W = exp(-+ 2 pi i q / 16)  (- forward, + inverse); q is a
+// compile-time constant after unrolling
 template <bool INV>
-__device__ __forceinline__ float2 mul_w16(float2 a, int q)
+__device__ __forceinline__ void tw_addsub(c2 e, c2 o, int q, c2& lo, c2& hi)
 {
     constexpr float H = 0.70710678118654752440f;
     constexpr float C1 = 0.92387953251128675613f, S1 = 0.38268343236508977173f;
-    switch (q) {
-        case 0: return a;
-        case 4: return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
-        case 2: return INV ? make_float2((a.x - a.y) * H, (a.x + a.y) * H) : make_float2((a.x + a.y) * H, (a.y - a.x) * H);
-        case 6: return INV ? make_float2((-a.x - a.y) * H, (a.x - a.y) * H) : make_float2((a.y - a.x) * H, (-a.x - a.y) * H);
-        default: {
-            // q = 1, 3, 5, 7: c = cos(2 pi q/16), s = sin(2 pi q/16)
-            const float c = (q == 1) ? C1 : (q == 3) ? S1 : (q == 5) ? -S1 : -C1;
-            const float s = (q == 1 || q == 7) ? S1 : C1;
-            return INV ? make_float2(fmaf(a.x, c, -a.y * s), fmaf(a.y, c, a.x * s))
-                       : make_float2(fmaf(a.x, c, a.y * s), fmaf(a.y, c, -a.x * s));
-        }
+    if (q == 0) {
+        lo = cadd(e, o);
+        hi = csub(e, o);
+    } else if (q == 4) {
+        // forward W = -i: W o = (o.im, -o.re);  inverse W = +i: W o = (-o.im, o.re)
+        const c2 p{padd(e.re, o.im), psub(e.im, o.re)};
+        const c2 m{psub(e.re, o.im), padd(e.im, o.re)};
+        lo = INV ? m : p;
+        hi = INV ? p : m;
+    } else if (q == 2 || q == 6) {
+        // q = 2: W = (1 -+ i) H;  q = 6: W = (-1 -+ i) H
+        const float2 s = padd(o.re, o.im), d = psub(o.im, o.re);   // o.re + o.im, o.im - o.re
+        float2 tr, ti;   // W o = H (tr, ti)
+        if (q == 2) { tr = INV ? neg2(d) : s;  ti = INV ? s : d; }
+        else        { tr = INV ? neg2(s) : d;  ti = INV ? neg2(d) : neg2(s); }
+        lo = c2{pfma(tr, bc(H), e.re), pfma(ti, bc(H), e.im)};
+        hi = c2{pfma(tr, bc(-H), e.re), pfma(ti, bc(-H), e.im)};
+    } else {
+        // q = 1, 3, 5, 7: W = c -+ i s with c = cos(2 pi q / 16), s = sin(2 pi q / 16)
+        const float c = (q == 1) ? C1 : (q == 3) ? S1 : (q == 5) ? -S1 : -C1;
+        const float s0 = (q == 1 || q == 7) ? S1 : C1;
+        const float s = INV ? -s0 : s0;
+        // W o = (o.re c + o.im s, o.im c - o.re s)
+        const float2 tr = pfma(o.re, bc(c), pmul(o.im, bc(s)));
+        const float2 ti = pfma(o.im, bc(c), neg2(pmul(o.re, bc(s))));
+        lo = c2{padd(e.re, tr), padd(e.im, ti)};
+        hi = c2{psub(e.re, tr), psub(e.im, ti)};
     }
 }
 
 // ---- radix-R DFT in registers, natural order in and out ----------------------------------------
 template <int R, bool INV>
-__device__ __forceinline__ void dft(float2 (&v)[R])
+__device__ __forceinline__ void dft(c2 (&v)[R])
 {
     if constexpr (R == 2) {
-        const float2 a = v[0];
+        const c2 a = v[0];
         v[0] = cadd(a, v[1]);
         v[1] = csub(a, v[1]);
-    } else if constexpr (R == 4) {
-        const float2 t0 = cadd(v[0], v[2]), t1 = csub(v[0], v[2]);
-        const float2 t2 = cadd(v[1], v[3]), t3 = csub(v[1], v[3]);
-        const float2 t3r = INV ? make_float2(-t3.y, t3.x) : make_float2(t3.y, -t3.x);
-        v[0] = cadd(t0, t2); v[2] = csub(t0, t2);
-        v[1] = cadd(t1, t3r); v[3] = csub(t1, t3r);
     } else {
-        float2 e[R / 2], o[R / 2];
+        c2 e[R / 2], o[R / 2];
 #pragma unroll
         for (int k = 0; k < R / 2; ++k) { e[k] = v[2 * k]; o[k] = v[2 * k + 1]; }
         dft<R / 2, INV>(e);
         dft<R / 2, INV>(o);
 #pragma unroll
-        for (int k = 0; k < R / 2; ++k) {
-            const float2 t = mul_w16<INV>(o[k], k * (16 / R));
-            v[k] = cadd(e[k], t);
-            v[k + R / 2] = csub(e[k], t);
-        }
+        for (int k = 0; k < R / 2; ++k) tw_addsub<INV>(e[k], o[k], k * (16 / R), v[k], v[k + R / 2]);
     }
 }
 
-// ---- one in-place stage over a [N][TB] tile ------------------------------------------------------
+// twiddle the R values of a butterfly: forward after the DFT (times w), inverse before it (times
+// conj w); tws = this stage's table in shared memory, n2 = the butterfly's index inside its block
+template <int R, bool INV>
+__device__ __forceinline__ void twiddle(c2 (&v)[R], const float4* __restrict__ tws, int n2)
+{
+    const float4* __restrict__ t = tws + n2 * (R - 1);
+#pragma unroll
+    for (int r = 1; r < R; ++r) {
+        const float4 w = t[r - 1];
+        const float2 wr = make_float2(w.x, w.y), wi = make_float2(w.z, w.w);
+        v[r] = INV ? cmulc(v[r], wr, wi) : cmul(v[r], wr, wi);
+    }
+}
+
+// ---- one in-place stage over a [N][NPAIR] tile of quads -------------------------------------------
 // Sub-transform length L, radix R, M = L/R: butterfly (blk, n2) touches positions blk L + n2 + M r.
-// tw[m] = exp(-2 pi i m / N) (shared memory).  ld(pos, b) / st(pos, b, value) move one element.
-// Forward: butterfly, then outputs r >= 1 times w_L^{n2 r}.  Inverse: inputs times conj first.
+// ld(pos, j) / st(pos, j, value) move one quad of batch pair j.
 template <int N, int R, int L, bool INV, int NT, int UNROLL, class LD, class ST>
-__device__ __forceinline__ void fft_stage(const float2* __restrict__ tw, LD ld, ST st)
+__device__ __forceinline__ void fft_stage(const float4* __restrict__ tws, LD ld, ST st)
 {
     constexpr int M = L / R;
-    constexpr int NBF = TB * (N / R);
+    constexpr int NBF = NPAIR * (N / R);
     constexpr int ITERS = (NBF + NT - 1) / NT;
 #pragma unroll UNROLL
     for (int it = 0; it < ITERS; ++it) {
         const int bf = (int)threadIdx.x + it * NT;
         if ((NBF % NT) != 0 && bf >= NBF) break;
-        const int b = bf % TB, q = bf / TB;
+        const int j = bf % NPAIR, q = bf / NPAIR;
         const int blk = q / M, n2 = q % M;
         const int base = blk * L + n2;
-        float2 v[R];
+        c2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = ld(base + M * r, b);
-        if (INV && M > 1) {
-#pragma unroll
-            for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], tw[n2 * r * (N / L)]);
-        }
+        for (int r = 0; r < R; ++r) v[r] = ld(base + M * r, j);
+        if constexpr (INV && M > 1) twiddle<R, true>(v, tws, n2);
         dft<R, INV>(v);
-        if (!INV && M > 1) {
+        if constexpr (!INV && M > 1) twiddle<R, false>(v, tws, n2);
 #pragma unroll
-            for (int r = 1; r < R; ++r) v[r] = cmul(v[r], tw[n2 * r * (N / L)]);
-        }
-#pragma unroll
-        for (int r = 0; r < R; ++r) st(base + M * r, b, v[r]);
+        for (int r = 0; r < R; ++r) st(base + M * r, j, v[r]);
     }
 }
 
 // Last forward stage (L = R, contiguous positions R q + r) + pointwise step + first inverse stage,
-// fused in registers.  pw(v, q, b) edits the R values in place.
+// fused in registers.  pw(v, q, j) edits the R values in place.
 template <int N, int R, int NT, int UNROLL, class LD, class PW, class ST>
 __device__ __forceinline__ void fft_stage_mid(LD ld, PW pw, ST st)
 {
-    constexpr int NBF = TB * (N / R);
+    constexpr int NBF = NPAIR * (N / R);
     constexpr int ITERS = (NBF + NT - 1) / NT;
 #pragma unroll UNROLL
     for (int it = 0; it < ITERS; ++it) {
         const int bf = (int)threadIdx.x + it * NT;
         if ((NBF % NT) != 0 && bf >= NBF) break;
-        const int b = bf % TB, q = bf / TB;
-        float2 v[R];
+        const int j = bf % NPAIR, q = bf / NPAIR;
+        c2 v[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[r] = ld(q * R + r, b);
+        for (int r = 0; r < R; ++r) v[r] = ld(q * R + r, j);
         dft<R, false>(v);
-        pw(v, q, b);
+        pw(v, q, j);
         dft<R, true>(v);
 #pragma unroll
-        for (int r = 0; r < R; ++r) st(q * R + r, b, v[r]);
+        for (int r = 0; r < R; ++r) st(q * R + r, j, v[r]);
     }
 }
+
+// ---- asynchronous bulk copies (TMA 1D; SASS: UBLKCP) and their mbarrier -----------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared, completion counted in bytes on the mbarrier; 16 B aligned, bytes % 16 == 0
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// shared -> global (bulk async group)
+__device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// make generic-proxy shared-memory writes visible to the async proxy (before a bulk store)
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 }  // namespace cpra

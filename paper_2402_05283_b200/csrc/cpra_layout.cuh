@@ -1,0 +1,222 @@
+// cpra_layout.cuh -- one-off kernels of the CPRA library (not on the timed path): conversions between
+// the caller's natural [n][y][x] arrays and the internal tiled layouts of cpra_kernels.cuh, the
+// error finalisation, and the Fourier-slice assembly.
+#pragma once
+#include "cpra_kernels.cuh"
+
+namespace cpra {
+
+struct Geo {
+    int N, Np, R0, R1, R2, RL;
+};
+// float index of the real part of element (n, y, x) of the row-tiled state; the imaginary part is 2
+// floats further (quad = [re_a, re_b, im_a, im_b])
+__device__ __forceinline__ size_t st_idx(int N, int n, int y, int x)
+{
+    return (((size_t)n * (N / TB) + (y / TB)) * N + x) * 32 + ((y % TB) / 2) * 4 + (y & 1);
+}
+// the same for element (n, py, px) of the column-tiled scratch
+__device__ __forceinline__ size_t sc_idx(int N, int n, int py, int px)
+{
+    return (((size_t)n * (N / TB) + (px / TB)) * N + py) * 32 + sw((px % TB) / 2, py) * 4 + (px & 1);
+}
+__device__ __forceinline__ size_t a_idx(int N, int RL, int n, int py, int px)
+{
+    return ((((size_t)n * (N / TB) + (px / TB)) * (N / RL) + (py / RL)) * NPAIR + (px % TB) / 2) * (2 * RL) + (py % RL) * 2 + (px & 1);
+}
+__device__ __forceinline__ float2 ld_c(const float* __restrict__ a, size_t i) { return make_float2(a[i], a[i + 2]); }
+__device__ __forceinline__ void st_c(float* __restrict__ a, size_t i, float2 v) { a[i] = v.x; a[i + 2] = v.y; }
+
+// A0: A = sqrt(max(I, 0)) (A14), mask folded in as A = -1, detector-centred ->
+// native (ifftshift, A11) -> the permuted order of the FFT kernels; den_n = sum_{M=1} max(I, 0).
+__global__ void k_set_data(const float* __restrict__ I, const unsigned char* __restrict__ mask,
+                           float* __restrict__ Aperm, double* __restrict__ den, Geo g)
+{
+    const int n = blockIdx.x, N = g.N, h = N / 2;
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < N * N; i += blockDim.x) {
+        const int yc = i / N, xc = i % N;
+        const size_t src = (size_t)n * N * N + i;
+        const float v = fmaxf(I[src], 0.f);
+        const bool m = mask ? (mask[src] != 0) : true;
+        const int ky = (yc + h) % N, kx = (xc + h) % N;
+        Aperm[a_idx(N, g.RL, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2))] = m ? sqrtf(v) : -1.f;
+        if (m) acc += (double)v;
+    }
+    __shared__ double red[32];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < (int)blockDim.x / 32; ++w) s += red[w];
+        den[n] = s;
+    }
+}
+
+// support u8 [n][y][x] -> bit-packed [n][rt][x] u16
+__global__ void k_pack_support(const unsigned char* __restrict__ S, uint16_t* __restrict__ S16, int N, size_t total16)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;  // index into S16
+    if (i >= total16) return;
+    const int x = (int)(i % N);
+    const size_t nr = i / N;  // n * NRT + rt
+    const int rt = (int)(nr % (N / TB));
+    const size_t n = nr / (N / TB);
+    unsigned bits = 0;
+    for (int b = 0; b < TB; ++b)
+        if (S[(n * N + (size_t)(rt * TB + b)) * N + x]) bits |= 1u << b;
+    S16[i] = (uint16_t)bits;
+}
+
+// natural [n][y][x] <-> row-tiled state; `masked` multiplies by the support.  One thread per
+// element, indexed in natural order.
+__global__ void k_pack_state(const float2* __restrict__ in, float* __restrict__ st, int N, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+    st_c(st, st_idx(N, n, y, x), in[i]);
+}
+__global__ void k_unpack_state(const float* __restrict__ st, const uint16_t* __restrict__ S16,
+                               float2* __restrict__ out, int N, size_t total, int masked)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+    float2 v = ld_c(st, st_idx(N, n, y, x));
+    if (masked && !((S16[((size_t)n * (N / TB) + y / TB) * N + x] >> (y % TB)) & 1)) v = make_float2(0.f, 0.f);
+    out[i] = v;
+}
+// natural-order spectrum [n][ky][kx] <-> column-tiled permuted scratch
+__global__ void k_unpack_spectrum(const float* __restrict__ scr, float2* __restrict__ out, Geo g, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = g.N;
+    const int kx = (int)(i % N), ky = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+    out[i] = ld_c(scr, sc_idx(N, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)));
+}
+__global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict__ scr, Geo g, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = g.N;
+    const int kx = (int)(i % N), ky = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+    st_c(scr, sc_idx(N, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)), in[i]);
+}
+
+// A3: E_n = sqrt(num_n / den_n), E = sqrt(sum num / sum den); one block, fixed order.
+__global__ void k_finalize_error(const double* __restrict__ partial, const double* __restrict__ den,
+                                 float* __restrict__ E, float* __restrict__ Eg, int Np, int NCT)
+{
+    double num = 0.0, dd = 0.0;
+    for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+        double s = 0.0;
+        for (int c = 0; c < NCT; ++c) s += partial[(size_t)n * NCT + c];
+        const double d = den[n];
+        if (E) E[n] = d > 0.0 ? (float)sqrt(s / d) : 0.f;
+        num += s; dd += d;
+    }
+    __shared__ double rn[32], rd[32];
+    for (int o = 16; o > 0; o >>= 1) {
+        num += __shfl_xor_sync(0xffffffffu, num, o);
+        dd += __shfl_xor_sync(0xffffffffu, dd, o);
+    }
+    if ((threadIdx.x & 31) == 0) { rn[threadIdx.x >> 5] = num; rd[threadIdx.x >> 5] = dd; }
+    __syncthreads();
+    if (threadIdx.x == 0 && Eg) {
+        double a = 0.0, b = 0.0;
+        for (int w = 0; w < (int)blockDim.x / 32; ++w) { a += rn[w]; b += rd[w]; }
+        *Eg = b > 0.0 ? (float)sqrt(a / b) : 0.f;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A7: Fourier-slice assembly (slice theorem PAPER.md:35-44; reading A17).
+// scr holds E_n = F[S_n g_n] in the permuted column-tiled layout.  One thread per (ky, kx) computes
+// the polar geometry in fp64 once, then walks kz.
+//   uphi[U]      sorted unique ray directions in [0, 2 pi)
+//   ustart[U+1]  contributors of unique ray u are rays[ustart[u] .. ustart[u+1])
+//   rays[]       n | (neg << 30): the slice and whether the ray is its ku <= 0 half
+// ------------------------------------------------------------------------------------------------
+__global__ void k_assemble(const float* __restrict__ scr, float2* __restrict__ vol, float* __restrict__ wgt,
+                           const double* __restrict__ uphi, const int* __restrict__ ustart,
+                           const int* __restrict__ rays, int U, Geo g, int zper)
+{
+    const int N = g.N, Np = g.Np, h = N / 2;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N * N) return;
+    const int ix = i % N, iy = i / N;
+    const int kx = ix < h ? ix : ix - N, ky = iy < h ? iy : iy - N;
+    const double PI = 3.14159265358979323846264338327950288;
+    const double rho = sqrt((double)kx * kx + (double)ky * ky);
+    int mode = 0;  // 0: outside, 1: axis (rho = 0), 2: interpolate
+    int ur[2] = {0, 0}, r0 = 0;
+    double wphi[2] = {0.0, 0.0}, wr = 0.0;
+    if (rho == 0.0) mode = 1;
+    else if (rho <= (double)(h - 1)) {
+        mode = 2;
+        double phi = atan2((double)ky, (double)kx);
+        if (phi < 0.0) phi += 2.0 * PI;
+        int a = -1;
+        for (int lo = 0, hi = U - 1; lo <= hi;) {
+            const int mid = (lo + hi) / 2;
+            if (uphi[mid] <= phi) { a = mid; lo = mid + 1; } else hi = mid - 1;
+        }
+        double pa, pb; int b;
+        if (a < 0) { a = U - 1; pa = uphi[a] - 2.0 * PI; } else pa = uphi[a];
+        b = a + 1;
+        if (b >= U) { b = 0; pb = uphi[0] + 2.0 * PI; } else pb = uphi[b];
+        const double wp = (pb > pa) ? (phi - pa) / (pb - pa) : 0.0;
+        r0 = (int)floor(rho);
+        wr = rho - (double)r0;
+        ur[0] = a; ur[1] = b; wphi[0] = 1.0 - wp; wphi[1] = wp;
+    }
+    const int z0 = blockIdx.y * zper, z1 = min(N, z0 + zper);
+    for (int iz = z0; iz < z1; ++iz) {
+        const int kz = iz < h ? iz : iz - N;
+        const int pz = fft_pos(iz, g.R0, g.R1, g.R2);
+        double vr = 0.0, vi = 0.0;
+        float w = 0.f;
+        if (mode == 1) {
+            const int pu = fft_pos(0, g.R0, g.R1, g.R2);
+            for (int n = 0; n < Np; ++n) {
+                const float2 e = ld_c(scr, sc_idx(N, n, pz, pu));
+                const double sg = (iz & 1) ? -1.0 : 1.0;
+                vr += sg * e.x; vi += sg * e.y;
+            }
+            vr /= Np; vi /= Np; w = 1.f;
+        } else if (mode == 2) {
+            for (int q = 0; q < 2; ++q) {
+                if (wphi[q] == 0.0) continue;
+                const int u = ur[q];
+                const int c0 = ustart[u], c1 = ustart[u + 1];
+                for (int rr = 0; rr < 2; ++rr) {
+                    const double wrr = rr ? wr : 1.0 - wr;
+                    if (wrr == 0.0) continue;
+                    const int r = r0 + rr;
+                    double sr = 0.0, si = 0.0;
+                    for (int c = c0; c < c1; ++c) {
+                        const int code = rays[c];
+                        const int n = code & 0x3fffffff;
+                        const int ku = (code >> 30) ? -r : r;
+                        const int iu = ((ku % N) + N) % N;
+                        const float2 e = ld_c(scr, sc_idx(N, n, pz, fft_pos(iu, g.R0, g.R1, g.R2)));
+                        const double sg = ((iz + iu) & 1) ? -1.0 : 1.0;   // origin -> centre pixel
+                        sr += sg * e.x; si += sg * e.y;
+                    }
+                    vr += wphi[q] * wrr * sr / (c1 - c0);
+                    vi += wphi[q] * wrr * si / (c1 - c0);
+                }
+            }
+            w = 1.f;
+        }
+        if ((kx + ky + kz) & 1) { vr = -vr; vi = -vi; }
+        const size_t o = ((size_t)iz * N + iy) * N + ix;
+        vol[o] = make_float2((float)vr, (float)vi);
+        if (wgt) wgt[o] = w;
+    }
+}
+
+}  // namespace cpra
