@@ -31,15 +31,16 @@ constexpr int NPAIR = 8;   // batch pairs = quads per position
 
 // ---- stage plan ------------------------------------------------------------------------------
 // NT = threads per CTA, chosen so that the last stage has NPAIR * N / RL = B * NT butterflies with
-// B in {1, 2}: the transposing stage of the row kernels keeps all of them in registers.
+// B in {1, 2}: the transposing stage of the row kernels keeps all of them in registers.  MINB = CTAs
+// per SM the register allocation is held to (shared memory allows that many).
 template <int N> struct Radix;
-template <> struct Radix<16>   { static constexpr int S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32;  };
-template <> struct Radix<32>   { static constexpr int S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64;  };
-template <> struct Radix<64>   { static constexpr int S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64;  };
-template <> struct Radix<128>  { static constexpr int S = 2, R0 = 16, R1 = 8,  R2 = 1, NT = 128; };
-template <> struct Radix<256>  { static constexpr int S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128; };
-template <> struct Radix<512>  { static constexpr int S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256; };
-template <> struct Radix<1024> { static constexpr int S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 512; };
+template <> struct Radix<16>   { static constexpr int S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32,  MINB = 8; };
+template <> struct Radix<32>   { static constexpr int S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64,  MINB = 8; };
+template <> struct Radix<64>   { static constexpr int S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64,  MINB = 8; };
+template <> struct Radix<128>  { static constexpr int S = 2, R0 = 16, R1 = 8,  R2 = 1, NT = 128, MINB = 4; };
+template <> struct Radix<256>  { static constexpr int S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128, MINB = 4; };
+template <> struct Radix<512>  { static constexpr int S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256, MINB = 3; };
+template <> struct Radix<1024> { static constexpr int S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 512, MINB = 1; };
 
 template <int N> __host__ __device__ constexpr int last_radix() { return Radix<N>::S == 3 ? Radix<N>::R2 : Radix<N>::R1; }
 
@@ -75,6 +76,14 @@ __device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return __
 
 __device__ __forceinline__ c2 from_quad(float4 q) { return c2{make_float2(q.x, q.y), make_float2(q.z, q.w)}; }
 __device__ __forceinline__ float4 to_quad(c2 v) { return make_float4(v.re.x, v.re.y, v.im.x, v.im.y); }
+// store one quad to shared memory as two 64-bit halves: the packed results live in separate
+// register pairs, and a 128-bit store would first have to gather them into four consecutive registers
+__device__ __forceinline__ void st_quad(float4* q, c2 v)
+{
+    const uint32_t a = (uint32_t)__cvta_generic_to_shared(q);
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.re.x), "f"(v.re.y) : "memory");
+    asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(a), "f"(v.im.x), "f"(v.im.y) : "memory");
+}
 
 __device__ __forceinline__ c2 cadd(c2 a, c2 b) { return c2{padd(a.re, b.re), padd(a.im, b.im)}; }
 __device__ __forceinline__ c2 csub(c2 a, c2 b) { return c2{psub(a.re, b.re), psub(a.im, b.im)}; }

@@ -128,7 +128,7 @@ __device__ __forceinline__ void load_transposed(const float4* __restrict__ tile,
 // n-1, n+1 are read with 128-bit loads inside the first stage.
 // ------------------------------------------------------------------------------------------------
 template <int N, int MODE>
-__global__ void __launch_bounds__(Radix<N>::NT)
+__global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
 k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4* __restrict__ twg,
           const uint16_t* __restrict__ S16, MixParams mp, int Np, int n0, int nimg)
 {
@@ -165,7 +165,7 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4
         return v;
     };
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NPAIR + j]); };
-    auto st_s = [&](int p, int j, c2 v) { tile[p * NPAIR + j] = to_quad(v); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NPAIR + j, v); };
 
     fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_first, st_s);
     __syncthreads();
@@ -203,31 +203,45 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4
 // A < 0 marks an unmeasured pixel (beamstop): left free.  `scale` (= 1/N^2, a power
 // of two) is folded into the constraint.  partial[n][ct] = sum over the tile of (|G| - A)^2.
 // ------------------------------------------------------------------------------------------------
-// one pixel of the constraint: returns the factor G' = s G (or sets `zero`: G' = s (1, 0))
-__device__ __forceinline__ float modulus_factor(float m2, float a, float scale, float& acc, bool& zero)
+// The error metric and the constraint on a pair of pixels, branch-free.  v = G (two pixels), a = A
+// of the two pixels (A < 0: unmeasured).  Returns with v = G' / N^2 and acc += (|G| - A)^2 over the
+// measured ones.  |G|^2 below the smallest normal number counts as |G| = 0: phase 0, G' = A
+// (reading A13; rsqrt.approx.ftz would return +inf there).
+__device__ __forceinline__ float rsqrt_ftz(float x)
 {
-    zero = false;
-    float s = scale;                           // unmeasured: G' = G
-    if (a >= 0.f) {                            // measured
-        float rs = rsqrtf(m2);                 // + one Newton step: ~1 ulp
-        const float h = 0.5f * m2 * rs;
-        rs = fmaf(rs, fmaf(-h, rs, 0.5f), rs);
-        const float mag = m2 * rs;
-        if (m2 > 0.f) {
-            const float d = mag - a;
-            acc = fmaf(d, d, acc);
-            s = a * rs * scale;                // G' = A G / |G|
-        } else {                               // |G| = 0: phase 0 (reading A13)
-            acc = fmaf(a, a, acc);
-            zero = true;
-            s = a * scale;
-        }
-    }
-    return s;
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ void modulus_pair(c2& v, float2 a, float scale, float2& acc)
+{
+    const float2 m2 = pfma(v.re, v.re, pmul(v.im, v.im));
+    const bool p0 = m2.x >= 1.17549435e-38f, p1 = m2.y >= 1.17549435e-38f;   // |G| > 0
+    const bool k0 = a.x >= 0.f, k1 = a.y >= 0.f;                              // measured
+    float2 rs = make_float2(rsqrt_ftz(m2.x), rsqrt_ftz(m2.y));
+    const float2 h = pmul(pmul(m2, bc(0.5f)), rs);                            // one Newton step: ~1 ulp
+    rs = pfma(rs, pfma(neg2(h), rs, bc(0.5f)), rs);
+    rs.x = p0 ? rs.x : 1.f;
+    rs.y = p1 ? rs.y : 1.f;
+    v.re.x = p0 ? v.re.x : 1.f;                                               // |G| = 0: G / |G| := (1, 0)
+    v.re.y = p1 ? v.re.y : 1.f;
+    const float2 mag = pmul(make_float2(p0 ? m2.x : 0.f, p1 ? m2.y : 0.f), rs);
+    float2 d = psub(mag, a);
+    d.x = k0 ? d.x : 0.f;
+    d.y = k1 ? d.y : 0.f;
+    acc = pfma(d, d, acc);
+    float2 f = pmul(pmul(a, rs), bc(scale));                                   // G' = A G / |G|
+    f.x = k0 ? f.x : scale;                                                    // unmeasured: G' = G
+    f.y = k1 ? f.y : scale;
+    // an unmeasured pixel with |G| = 0 stays 0 (v.re was set to 1 above)
+    v.re.x = (k0 || p0) ? v.re.x : 0.f;
+    v.re.y = (k1 || p1) ? v.re.y : 0.f;
+    v.re = pmul(v.re, f);
+    v.im = pmul(v.im, f);
 }
 
 template <int N, int MODE>
-__global__ void __launch_bounds__(Radix<N>::NT)
+__global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
 k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* __restrict__ twg,
       double* __restrict__ partial, int n0, float scale)
 {
@@ -250,7 +264,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* _
     mbar_wait(s.bar, 0);
 
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NPAIR + sw(j, p)]); };
-    auto st_s = [&](int p, int j, c2 v) { tile[p * NPAIR + sw(j, p)] = to_quad(v); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NPAIR + sw(j, p), v); };
 
     if constexpr (MODE == COL_FULL || MODE == COL_FWD) {
         fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_s, st_s);
@@ -265,7 +279,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* _
     }
     if constexpr (MODE == COL_FULL) {
         const float* __restrict__ At = Aperm + ((size_t)n * NCT + ct) * N * TB;
-        float acc = 0.f;
+        float2 acc2 = make_float2(0.f, 0.f);
         auto pw = [&](c2 (&v)[RL], int q, int j) {
             const float4* __restrict__ a4 = reinterpret_cast<const float4*>(At + (size_t)(q * NPAIR + j) * (2 * RL));
             float2 a[RL];
@@ -276,19 +290,10 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* _
                 a[2 * r + 1] = make_float2(t.z, t.w);
             }
 #pragma unroll
-            for (int r = 0; r < RL; ++r) {
-                const float2 m2 = pfma(v[r].re, v[r].re, pmul(v[r].im, v[r].im));
-                bool z0, z1;
-                float2 f;
-                f.x = modulus_factor(m2.x, a[r].x, scale, acc, z0);
-                f.y = modulus_factor(m2.y, a[r].y, scale, acc, z1);
-                if (z0) { v[r].re.x = 1.f; v[r].im.x = 0.f; }
-                if (z1) { v[r].re.y = 1.f; v[r].im.y = 0.f; }
-                v[r].re = pmul(v[r].re, f);
-                v[r].im = pmul(v[r].im, f);
-            }
+            for (int r = 0; r < RL; ++r) modulus_pair(v[r], a[r], scale, acc2);
         };
         fft_stage_mid<N, RL, NT, 1>(ld_s, pw, st_s);
+        float acc = acc2.x + acc2.y;
         // block reduction of the error numerator (fixed order: deterministic)
         __shared__ float red[32];
 #pragma unroll
@@ -329,7 +334,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* _
 // transposes them into the row layout; the new state tile leaves by one bulk copy.
 // ------------------------------------------------------------------------------------------------
 template <int N, int MODE, int MIXMODE>
-__global__ void __launch_bounds__(Radix<N>::NT)
+__global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
 k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4* __restrict__ nxt,
           const float4* __restrict__ twg, const uint16_t* __restrict__ S16, MixParams mp, float beta,
           float scale, int Np, int n0, int nimg)
@@ -361,7 +366,7 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
     mbar_wait(s.bar, 0);
 
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NPAIR + j]); };
-    auto st_s = [&](int p, int j, c2 v) { tile[p * NPAIR + j] = to_quad(v); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NPAIR + j, v); };
 
     // first inverse stage (contiguous positions, no twiddles), reading the scratch layout
     {
