@@ -200,7 +200,8 @@ int cpra_set_chunk(cpra_plan_t plan, int images);
 #define CPRA_PROFILE_ROW_FWD 0 /* mix + forward row FFT */
 #define CPRA_PROFILE_COL 1     /* forward column FFT + error + modulus + inverse column FFT */
 #define CPRA_PROFILE_ROW_INV 2 /* inverse row FFT + support / HIO */
-#define CPRA_PROFILE_CLASSES 3
+#define CPRA_PROFILE_IMAGE 3   /* N <= 128: the whole iteration of a projection in one kernel */
+#define CPRA_PROFILE_CLASSES 4
 int cpra_profile(cpra_plan_t plan, int enable);
 int cpra_profile_read(cpra_plan_t plan, double* h_ms, long* h_launches);
 

@@ -10,6 +10,7 @@
 
 #include "../../include/cpra.h"
 #include "cpra_layout.cuh"
+#include "cpra_image.cuh"
 
 using namespace cpra;
 
@@ -146,6 +147,12 @@ int set_attrs()
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_NONE>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_K1>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_GEN>, SM));
+    if constexpr (N <= 128) {
+        constexpr int ISM = image_smem_bytes<N>();
+        acc(allow_smem(k_image<N, MIX_NONE>, ISM));
+        acc(allow_smem(k_image<N, MIX_K1>, ISM));
+        acc(allow_smem(k_image<N, MIX_GEN>, ISM));
+    }
     return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
 }
 
@@ -256,6 +263,26 @@ int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int
     else ROWINV(ROWINV_HIO, MIX_GEN);
 #undef ROWINV
     return check_launch(p);
+}
+
+// the whole iteration of every projection in one launch (N <= 128, cpra_image.cuh)
+template <int N>
+int launch_image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale)
+{
+    if constexpr (N <= 128) {
+        constexpr int NT = image_threads<N>(), ISM = image_smem_bytes<N>();
+        const dim3 grid((unsigned)p->Np);
+        const MixParams mp = mix_params(p);
+        ProfScope prof(p, CPRA_PROFILE_IMAGE);
+#define IMG(M) k_image<N, M><<<grid, NT, ISM, p->stream>>>(cur, nxt, p->A, p->tw, p->S16, p->partial, mp, beta, scale, p->Np, 0)
+        if (mode == MIX_NONE) IMG(MIX_NONE);
+        else if (mode == MIX_K1) IMG(MIX_K1);
+        else IMG(MIX_GEN);
+#undef IMG
+        return check_launch(p);
+    } else {
+        return CPRA_ERR_UNSUPPORTED_SIZE;
+    }
 }
 
 int ready(const cpra_plan_s* p) { return p->ws ? CPRA_OK : CPRA_ERR_WORKSPACE; }
@@ -456,6 +483,15 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
         const int mode = mix_mode(p, (p->t % p->n_ei) == 0);
         const float4* cur = p->st[p->cur];
         float4* nxt = p->st[p->cur ^ 1];
+        if (p->N <= 128 && !(p->flags & CPRA_FLAG_FORCE_MULTIPASS)) {
+            int rc = CPRA_OK;
+            { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = launch_image<NN>(p, cur, nxt, mode, beta, scale)); return 0; }; f(); }
+            if (rc != CPRA_OK) return rc;
+            p->cur ^= 1;
+            p->t += 1;
+            p->have_error = true;
+            continue;
+        }
         for (int n0 = 0; n0 < p->Np; n0 += chunk) {
             const int nimg = std::min(chunk, p->Np - n0);
             int rc = CPRA_OK;

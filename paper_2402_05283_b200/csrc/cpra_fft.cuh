@@ -32,15 +32,17 @@ constexpr int NPAIR = 8;   // batch pairs = quads per position
 // ---- stage plan ------------------------------------------------------------------------------
 // NT = threads per CTA, chosen so that the last stage has NPAIR * N / RL = B * NT butterflies with
 // B in {1, 2}: the transposing stage of the row kernels keeps all of them in registers.  MINB = CTAs
-// per SM the register allocation is held to (shared memory allows that many).
+// per SM the register allocation is held to (shared memory allows that many).  PF: k_row_fwd
+// requests the neighbours' share of the mix for all its first-stage butterflies before it waits for its
+// own tile (MINBF = its CTAs per SM: the prefetch needs 2 x 32 more registers).
 template <int N> struct Radix;
-template <> struct Radix<16>   { static constexpr int S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32,  MINB = 8; };
-template <> struct Radix<32>   { static constexpr int S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64,  MINB = 8; };
-template <> struct Radix<64>   { static constexpr int S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64,  MINB = 8; };
-template <> struct Radix<128>  { static constexpr int S = 2, R0 = 16, R1 = 8,  R2 = 1, NT = 128, MINB = 4; };
-template <> struct Radix<256>  { static constexpr int S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128, MINB = 4; };
-template <> struct Radix<512>  { static constexpr int S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256, MINB = 3; };
-template <> struct Radix<1024> { static constexpr int S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 512, MINB = 1; };
+template <> struct Radix<16>   { static constexpr int S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<32>   { static constexpr int S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<64>   { static constexpr int S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<128>  { static constexpr int S = 2, R0 = 8,  R1 = 16, R2 = 1, NT = 64,  MINB = 6; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<256>  { static constexpr int S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128, MINB = 4; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<512>  { static constexpr int S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256, MINB = 3; static constexpr bool PF = true; static constexpr int MINBF = 2; };
+template <> struct Radix<1024> { static constexpr int S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 512, MINB = 1; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 
 template <int N> __host__ __device__ constexpr int last_radix() { return Radix<N>::S == 3 ? Radix<N>::R2 : Radix<N>::R1; }
 

@@ -54,6 +54,38 @@ struct MixLoader {
         cm = cur + (size_t)(n_ == 0 ? Np_ - 1 : n_ - 1) * istride_;
         cp = cur + (size_t)(n_ == Np_ - 1 ? 0 : n_ + 1) * istride_;
     }
+    // the neighbours' share of the mix at quad q: sum_k a_k (g_{n-k} + g_{n+k}), and its combination
+    // with the own quad: a_0 own + nb
+    __device__ __forceinline__ c2 nbsum(size_t q) const
+    {
+        if constexpr (MODE == MIX_K1) {
+            const c2 m = from_quad(__ldg(cm + q)), p = from_quad(__ldg(cp + q));
+            const float2 a1 = bc(mp.a[1]);
+            return c2{pmul(a1, padd(m.re, p.re)), pmul(a1, padd(m.im, p.im))};
+        } else if constexpr (MODE == MIX_GEN) {
+            c2 acc{make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+            for (int k = 1; k <= mp.K; ++k) {
+                int nm = n - k; if (nm < 0) nm += Np;
+                int np = n + k; if (np >= Np) np -= Np;
+                const c2 m = from_quad(__ldg(base + (size_t)nm * istride + q));
+                const c2 p = from_quad(__ldg(base + (size_t)np * istride + q));
+                acc.re = pfma(bc(mp.a[k]), padd(m.re, p.re), acc.re);
+                acc.im = pfma(bc(mp.a[k]), padd(m.im, p.im), acc.im);
+            }
+            return acc;
+        } else {
+            return c2{make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        }
+    }
+    __device__ __forceinline__ c2 combine(c2 own, c2 nb) const
+    {
+        if constexpr (MODE == MIX_K1 || MODE == MIX_GEN) {
+            const float2 a0 = bc(mp.a[0]);
+            return c2{pfma(a0, own.re, nb.re), pfma(a0, own.im, nb.im)};
+        } else {
+            return own;
+        }
+    }
     __device__ __forceinline__ c2 operator()(c2 own, size_t q) const
     {
         if constexpr (MODE == MIX_NONE || MODE == MIX_MASK) {
@@ -128,7 +160,7 @@ __device__ __forceinline__ void load_transposed(const float4* __restrict__ tile,
 // n-1, n+1 are read with 128-bit loads inside the first stage.
 // ------------------------------------------------------------------------------------------------
 template <int N, int MODE>
-__global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
+__global__ void __launch_bounds__(Radix<N>::NT, (Radix<N>::PF && (MODE == MIX_K1 || MODE == MIX_GEN)) ? Radix<N>::MINBF : Radix<N>::MINB)
 k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4* __restrict__ twg,
           const uint16_t* __restrict__ S16, MixParams mp, int Np, int n0, int nimg)
 {
@@ -136,6 +168,8 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4
     constexpr int NT = RX::NT, NRT = N / TB, NCT = N / TB, RL = last_radix<N>();
     constexpr int B = NPAIR * (N / RL) / NT;   // butterflies per thread in the last stage
     static_assert(B * NT == NPAIR * (N / RL) && B >= 1, "last stage must fill the CTA exactly");
+    constexpr int R0 = RX::R0, M0 = N / R0, NBF0 = NPAIR * M0, IT0 = (NBF0 + NT - 1) / NT;
+    constexpr bool PFMIX = RX::PF && (MODE == MIX_K1 || MODE == MIX_GEN);
     extern __shared__ __align__(128) float4 sm[];
     const Smem<N> s(sm);
     float4* __restrict__ tile = s.tile;
@@ -153,7 +187,7 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4
     }
     const MixLoader<MODE> mix(cur, istride, n, Np, mp);
     const uint16_t* __restrict__ Srow = S16 + ((size_t)n * NRT + rt) * N;
-    mbar_wait(s.bar, 0);
+    if constexpr (!PFMIX) mbar_wait(s.bar, 0);
 
     auto ld_first = [&](int x, int j) -> c2 {
         c2 v = mix(from_quad(tile[x * NPAIR + j]), toff + (size_t)x * NPAIR + j);
@@ -167,7 +201,35 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NPAIR + j]); };
     auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NPAIR + j, v); };
 
-    fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_first, st_s);
+    if constexpr (PFMIX) {
+        // the neighbours' share of every first-stage butterfly of this thread is requested before
+        // the own tile is waited for
+        c2 nbv[IT0][R0];
+#pragma unroll
+        for (int it = 0; it < IT0; ++it) {
+            const int bf = (int)threadIdx.x + it * NT, j = bf % NPAIR, q = bf / NPAIR;
+            if (bf < NBF0) {
+#pragma unroll
+                for (int r = 0; r < R0; ++r) nbv[it][r] = mix.nbsum(toff + (size_t)(q + M0 * r) * NPAIR + j);
+            }
+        }
+        mbar_wait(s.bar, 0);
+#pragma unroll
+        for (int it = 0; it < IT0; ++it) {
+            const int bf = (int)threadIdx.x + it * NT, j = bf % NPAIR, q = bf / NPAIR;
+            if (bf < NBF0) {
+                c2 v[R0];
+#pragma unroll
+                for (int r = 0; r < R0; ++r) v[r] = mix.combine(ld_s(q + M0 * r, j), nbv[it][r]);
+                dft<R0, false>(v);
+                twiddle<R0, false>(v, s.tw0, q);
+#pragma unroll
+                for (int r = 0; r < R0; ++r) st_s(q + M0 * r, j, v[r]);
+            }
+        }
+    } else {
+        fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_first, st_s);
+    }
     __syncthreads();
     if constexpr (RX::S == 3) {
         fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);

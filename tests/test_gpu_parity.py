@@ -313,6 +313,24 @@ def test_chunking_and_multipass_flags_do_not_change_results(torch_cuda):
     assert rel_l2(_get(q), r) <= TOL_1
 
 
+@pytest.mark.parametrize("N", [16, 32, 64, 128])
+def test_multipass_kernels_at_small_N(torch_cuda, N):
+    """N <= 128 runs the whole-image kernel by default; FLAG_FORCE_MULTIPASS sends the same sizes
+    through the three tile kernels.  Both against the oracle."""
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(N, 5, seed=40 + N, beamstop=3 if N > 16 else 0)
+    o = _oracle(p)
+    o.iterate(2, 0.9)
+    ref = o.get_projections(0)
+    for flags in (0, cpra.FLAG_FORCE_MULTIPASS):
+        g = _gpu(p, flags=flags)
+        g.iterate(2, 0.9)
+        assert rel_l2(_get(g), ref) <= 2 * TOL_1, flags
+        E, Eg = _errors(g)
+        Eo, Ego = o.get_error()
+        assert np.abs(E - Eo).max() <= TOL_E * Eo.max() and abs(Eg - Ego) <= TOL_E * Ego, flags
+
+
 def test_not_ready_and_argument_errors(torch_cuda):
     import paper_2402_05283_b200 as cpra
     p = cpra_inputs.random_stack(32, 4, seed=1)
