@@ -22,7 +22,7 @@ struct cpra_plan_s {
     // workspace carve-up
     char* ws = nullptr;
     size_t ws_bytes = 0;
-    float4* tw = nullptr;
+    float2* tw = nullptr;
     float* A = nullptr;
     uint16_t* S16 = nullptr;
     float4* st[2] = {nullptr, nullptr};
@@ -41,7 +41,7 @@ struct cpra_plan_s {
     bool have_data = false, have_support = false, have_estimate = false, have_error = false;
     bool attrs_set = false;
     std::vector<double> angles;
-    std::vector<float4> h_tw;
+    std::vector<float2> h_tw;
     std::vector<double> h_uphi;
     std::vector<int> h_ustart, h_rays;
     long launches = 0;
@@ -72,7 +72,7 @@ Layout layout_of(int N, int Np)
     const size_t px = (size_t)Np * N * N;
     Carve c;
     Layout L;
-    L.tw = c.take(sizeof(float4) * 1024);   // >= tw_quads<N>() for every N
+    L.tw = c.take(sizeof(float2) * 1024);   // >= tw_count<N>() for every N
     L.A = c.take(sizeof(float) * px);
     L.S16 = c.take(px / 8);
     L.st0 = c.take(sizeof(float2) * px);
@@ -89,10 +89,10 @@ Layout layout_of(int N, int Np)
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
-// per-stage twiddle tables of cpra_fft.cuh: quads [wr, wr, wi, wi], w = exp(-2 pi i n2 r / L),
-// computed in double and rounded once
+// per-stage twiddle tables of cpra_fft.cuh: (wr, wi), w = exp(-2 pi i n2 r / L), computed in double
+// and rounded once
 template <int N>
-void build_twiddles(std::vector<float4>& t)
+void build_twiddles(std::vector<float2>& t)
 {
     using RX = Radix<N>;
     const double PI = 3.14159265358979323846264338327950288;
@@ -102,13 +102,12 @@ void build_twiddles(std::vector<float4>& t)
         for (int n2 = 0; n2 < M; ++n2)
             for (int r = 1; r < R; ++r) {
                 const double a = -2.0 * PI * (double)(n2 * r) / (double)L;
-                const float wr = (float)std::cos(a), wi = (float)std::sin(a);
-                t.push_back(make_float4(wr, wr, wi, wi));
+                t.push_back(make_float2((float)std::cos(a), (float)std::sin(a)));
             }
     };
     stage(N, RX::R0);
     if (RX::S == 3) stage(N / RX::R0, RX::R1);
-    t.resize(1024, make_float4(0.f, 0.f, 0.f, 0.f));
+    t.resize(1024, make_float2(0.f, 0.f));
 }
 
 #define CPRA_DISPATCH_N(N_, ...)                                                     \
@@ -132,7 +131,7 @@ cudaError_t allow_smem(F* f, int bytes)
 template <int N>
 int set_attrs()
 {
-    static_assert(tw_quads<N>() <= 1024, "twiddle region of the workspace too small");
+    static_assert(tw_count<N>() <= 1024, "twiddle region of the workspace too small");
     cudaError_t e = cudaSuccess;
     auto acc = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     constexpr int SM = smem_bytes<N>();
@@ -378,7 +377,7 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
     if (bytes < L.total || ((uintptr_t)d_ws & 255)) return CPRA_ERR_WORKSPACE;
     char* w = (char*)d_ws;
     p->ws = w; p->ws_bytes = bytes;
-    p->tw = (float4*)(w + L.tw);
+    p->tw = (float2*)(w + L.tw);
     p->A = (float*)(w + L.A);
     p->S16 = (uint16_t*)(w + L.S16);
     p->st[0] = (float4*)(w + L.st0);
@@ -397,7 +396,7 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
         if (rc != CPRA_OK) { p->ws = nullptr; return rc; }
         p->attrs_set = true;
     }
-    if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float4) * p->h_tw.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
+    if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float2) * p->h_tw.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
         p->ws = nullptr;
         return CPRA_ERR_CUDA;
     }

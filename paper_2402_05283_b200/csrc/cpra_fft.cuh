@@ -54,15 +54,17 @@ __host__ __device__ __forceinline__ int fft_pos(int k, int R0, int R1, int R2)
 }
 
 // ---- twiddle tables ----------------------------------------------------------------------------
-// One table per stage with M = L / R > 1, entry (n2, r) for r = 1 .. R-1 at quad index
-// n2 (R - 1) + (r - 1):  [wr, wr, wi, wi],  w = exp(-2 pi i n2 r / L)  (computed in double, rounded
-// once, on the host).  Stage 0 (L = N) first, then stage 1 (L = N / R0) if the plan has 3 stages.
-template <int N> __host__ __device__ constexpr int tw_quads_stage0() { return (N / Radix<N>::R0) * (Radix<N>::R0 - 1); }
-template <int N> __host__ __device__ constexpr int tw_quads_stage1()
+// One table per stage with M = L / R > 1, entry (n2, r) for r = 1 .. R-1 at index
+// n2 (R - 1) + (r - 1):  (wr, wi),  w = exp(-2 pi i n2 r / L)  (computed in double, rounded once, on
+// the host).  Stage 0 (L = N) first, then stage 1 (L = N / R0) if the plan has 3 stages.  A twiddle
+// is one 64-bit shared-memory load; the packed instructions take wr and wi as scalar operands that
+// the hardware broadcasts to both halves (SASS "R12.F32"), so no duplicated copy is stored or built.
+template <int N> __host__ __device__ constexpr int tw_count_stage0() { return (N / Radix<N>::R0) * (Radix<N>::R0 - 1); }
+template <int N> __host__ __device__ constexpr int tw_count_stage1()
 {
     return Radix<N>::S == 3 ? (N / (Radix<N>::R0 * Radix<N>::R1)) * (Radix<N>::R1 - 1) : 0;
 }
-template <int N> __host__ __device__ constexpr int tw_quads() { return tw_quads_stage0<N>() + tw_quads_stage1<N>(); }
+template <int N> __host__ __device__ constexpr int tw_count() { return tw_count_stage0<N>() + tw_count_stage1<N>(); }
 
 // ---- packed helpers ----------------------------------------------------------------------------
 struct c2 {
@@ -159,14 +161,13 @@ __device__ __forceinline__ void dft(c2 (&v)[R])
 // twiddle the R values of a butterfly: forward after the DFT (times w), inverse before it (times
 // conj w); tws = this stage's table in shared memory, n2 = the butterfly's index inside its block
 template <int R, bool INV>
-__device__ __forceinline__ void twiddle(c2 (&v)[R], const float4* __restrict__ tws, int n2)
+__device__ __forceinline__ void twiddle(c2 (&v)[R], const float2* __restrict__ tws, int n2)
 {
-    const float4* __restrict__ t = tws + n2 * (R - 1);
+    const float2* __restrict__ t = tws + n2 * (R - 1);
 #pragma unroll
     for (int r = 1; r < R; ++r) {
-        const float4 w = t[r - 1];
-        const float2 wr = make_float2(w.x, w.y), wi = make_float2(w.z, w.w);
-        v[r] = INV ? cmulc(v[r], wr, wi) : cmul(v[r], wr, wi);
+        const float2 w = t[r - 1];
+        v[r] = INV ? cmulc(v[r], bc(w.x), bc(w.y)) : cmul(v[r], bc(w.x), bc(w.y));
     }
 }
 
@@ -174,7 +175,7 @@ __device__ __forceinline__ void twiddle(c2 (&v)[R], const float4* __restrict__ t
 // Sub-transform length L, radix R, M = L/R: butterfly (blk, n2) touches positions blk L + n2 + M r.
 // ld(pos, j) / st(pos, j, value) move one quad of batch pair j.
 template <int N, int R, int L, bool INV, int NT, int UNROLL, class LD, class ST>
-__device__ __forceinline__ void fft_stage(const float4* __restrict__ tws, LD ld, ST st)
+__device__ __forceinline__ void fft_stage(const float2* __restrict__ tws, LD ld, ST st)
 {
     constexpr int M = L / R;
     constexpr int NBF = NPAIR * (N / R);

@@ -21,7 +21,7 @@ template <int N> __host__ __device__ constexpr int image_smem_bytes() { return i
 
 // one in-place stage over all N/16 tiles of the image; ld(t, pos, j) / st(t, pos, j, v)
 template <int N, int R, int L, bool INV, int NT, class LD, class ST>
-__device__ __forceinline__ void image_stage(const float4* __restrict__ tws, LD ld, ST st)
+__device__ __forceinline__ void image_stage(const float2* __restrict__ tws, LD ld, ST st)
 {
     constexpr int M = L / R;
     constexpr int NBFT = NPAIR * (N / R), NBF = NBFT * (N / TB);
@@ -80,7 +80,7 @@ __device__ __forceinline__ void load_transposed_img(const float4* __restrict__ i
 template <int N, int MIXMODE>
 __global__ void __launch_bounds__(image_threads<N>())
 k_image(const float4* __restrict__ cur, float4* __restrict__ nxt, const float* __restrict__ Aperm,
-        const float4* __restrict__ twg, const uint16_t* __restrict__ S16, double* __restrict__ partial,
+        const float2* __restrict__ twg, const uint16_t* __restrict__ S16, double* __restrict__ partial,
         MixParams mp, float beta, float scale, int Np, int n0)
 {
     using RX = Radix<N>;
@@ -89,8 +89,8 @@ k_image(const float4* __restrict__ cur, float4* __restrict__ nxt, const float* _
     constexpr int NBFL = NPAIR * (N / RL);   // last-stage butterflies per tile; NT = NRT * NBFL
     extern __shared__ __align__(128) float4 sm[];
     float4* __restrict__ img = sm;
-    const float4* __restrict__ tw0 = sm + image_quads<N>();
-    uint64_t* bar = reinterpret_cast<uint64_t*>(sm + image_quads<N>() + tw_quads<N>());
+    const float2* __restrict__ tw0 = reinterpret_cast<const float2*>(sm + image_quads<N>());
+    uint64_t* bar = reinterpret_cast<uint64_t*>(const_cast<float2*>(tw0) + tw_count<N>());
     float* red = reinterpret_cast<float*>(bar + 2);
     const int n = n0 + (int)blockIdx.x;
     const size_t istride = image_quads<N>();
@@ -100,7 +100,7 @@ k_image(const float4* __restrict__ cur, float4* __restrict__ nxt, const float* _
     if (threadIdx.x == 0) {
         mbar_expect_tx(bar, image_bytes<N>() + tw_bytes<N>());
         bulk_load(img, cur + (size_t)n * istride, image_bytes<N>(), bar);
-        bulk_load(const_cast<float4*>(tw0), twg, tw_bytes<N>(), bar);
+        bulk_load(const_cast<float2*>(tw0), twg, tw_bytes<N>(), bar);
     }
     const MixLoader<MIXMODE> mix(cur, istride, n, Np, mp);
     mbar_wait(bar, 0);

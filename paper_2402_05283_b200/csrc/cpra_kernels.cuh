@@ -30,7 +30,7 @@ enum { ROWINV_HIO = 0, ROWINV_PLAIN = 1 };
 
 template <int N> __host__ __device__ constexpr int tile_quads() { return N * NPAIR; }
 template <int N> __host__ __device__ constexpr int tile_bytes() { return N * NPAIR * 16; }
-template <int N> __host__ __device__ constexpr int tw_bytes() { return tw_quads<N>() * 16; }
+template <int N> __host__ __device__ constexpr int tw_bytes() { return tw_count<N>() * 8; }
 // tile + twiddle tables + mbarrier
 template <int N> __host__ __device__ constexpr int smem_bytes() { return tile_bytes<N>() + tw_bytes<N>() + 16; }
 
@@ -113,12 +113,12 @@ struct MixLoader {
 template <int N>
 struct Smem {
     float4* tile;
-    const float4* tw0;
-    const float4* tw1;
+    const float2* tw0;
+    const float2* tw1;
     uint64_t* bar;
     __device__ __forceinline__ explicit Smem(float4* sm)
-        : tile(sm), tw0(sm + tile_quads<N>()), tw1(sm + tile_quads<N>() + tw_quads_stage0<N>()),
-          bar(reinterpret_cast<uint64_t*>(sm + tile_quads<N>() + tw_quads<N>())) {}
+        : tile(sm), tw0(reinterpret_cast<const float2*>(sm + tile_quads<N>())), tw1(tw0 + tw_count_stage0<N>()),
+          bar(reinterpret_cast<uint64_t*>(const_cast<float2*>(tw0) + tw_count<N>())) {}
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -161,7 +161,7 @@ __device__ __forceinline__ void load_transposed(const float4* __restrict__ tile,
 // ------------------------------------------------------------------------------------------------
 template <int N, int MODE>
 __global__ void __launch_bounds__(Radix<N>::NT, (Radix<N>::PF && (MODE == MIX_K1 || MODE == MIX_GEN)) ? Radix<N>::MINBF : Radix<N>::MINB)
-k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4* __restrict__ twg,
+k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2* __restrict__ twg,
           const uint16_t* __restrict__ S16, MixParams mp, int Np, int n0, int nimg)
 {
     using RX = Radix<N>;
@@ -183,7 +183,7 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float4
     if (threadIdx.x == 0) {
         mbar_expect_tx(s.bar, tile_bytes<N>() + tw_bytes<N>());
         bulk_load(tile, cur + (size_t)n * istride + toff, tile_bytes<N>(), s.bar);
-        bulk_load(const_cast<float4*>(s.tw0), twg, tw_bytes<N>(), s.bar);
+        bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
     }
     const MixLoader<MODE> mix(cur, istride, n, Np, mp);
     const uint16_t* __restrict__ Srow = S16 + ((size_t)n * NRT + rt) * N;
@@ -304,7 +304,7 @@ __device__ __forceinline__ void modulus_pair(c2& v, float2 a, float scale, float
 
 template <int N, int MODE>
 __global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
-k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* __restrict__ twg,
+k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* __restrict__ twg,
       double* __restrict__ partial, int n0, float scale)
 {
     using RX = Radix<N>;
@@ -321,7 +321,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* _
     if (threadIdx.x == 0) {
         mbar_expect_tx(s.bar, tile_bytes<N>() + tw_bytes<N>());
         bulk_load(tile, g, tile_bytes<N>(), s.bar);
-        bulk_load(const_cast<float4*>(s.tw0), twg, tw_bytes<N>(), s.bar);
+        bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
     }
     mbar_wait(s.bar, 0);
 
@@ -398,7 +398,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float4* _
 template <int N, int MODE, int MIXMODE>
 __global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
 k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4* __restrict__ nxt,
-          const float4* __restrict__ twg, const uint16_t* __restrict__ S16, MixParams mp, float beta,
+          const float2* __restrict__ twg, const uint16_t* __restrict__ S16, MixParams mp, float beta,
           float scale, int Np, int n0, int nimg)
 {
     using RX = Radix<N>;
@@ -416,7 +416,7 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
     __syncthreads();
     if (threadIdx.x == 0) {
         mbar_expect_tx(s.bar, tile_bytes<N>() + tw_bytes<N>());
-        bulk_load(const_cast<float4*>(s.tw0), twg, tw_bytes<N>(), s.bar);
+        bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
     }
     __syncwarp();
     {
