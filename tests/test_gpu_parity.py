@@ -226,6 +226,35 @@ def test_tiny_full_run(torch_cuda, problems):
 
 
 # ------------------------------------------------------------------------------------------------
+# full BASELINE.json sizes, in the launch configuration bench.py times, on sampled projections
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_full_size_sampled_projections(torch_cuda, cfg):
+    """Two iterations of the whole workload (config 4 = the headline: N = 512, N_p = 360) on the
+    GPU.  With K = 1 projection n after two iterations depends on projections n-2 .. n+2 only, so the
+    oracle run on that 5-stack (its wrap-around touches only the two outer members, whose second
+    iteration is not used) reproduces projection n exactly: checked for n at the seam and inside."""
+    import dataclasses
+    from oracle import Oracle
+    p = cpra_inputs.make_problem(cfg)
+    g = _gpu(p)
+    g.iterate(2, p.beta)
+    out = _get(g)
+    E, _ = _errors(g)
+    for n in (0, 1, p.Np // 2, p.Np - 1):
+        idx = [(n + d) % p.Np for d in (-2, -1, 0, 1, 2)]
+        sub = dataclasses.replace(p, Np=5, angles=p.angles[idx], intensity=np.ascontiguousarray(p.intensity[idx]),
+                                  mask=np.ascontiguousarray(p.mask[idx]), support=np.ascontiguousarray(p.support[idx]),
+                                  estimate=np.ascontiguousarray(p.estimate[idx]), projections=p.projections[idx])
+        o = Oracle(p.N, 5).load(sub)
+        o.iterate(2, p.beta)
+        ref = o.get_projections(0)[2]
+        assert rel_l2(out[n], ref) <= 3 * TOL_1, (n, rel_l2(out[n], ref))
+        Eo, _ = o.get_error()
+        assert abs(E[n] - Eo[2]) <= TOL_E * Eo[2], (n, E[n], Eo[2])
+
+
+# ------------------------------------------------------------------------------------------------
 # carousel variants and degenerate stacks
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("alpha,n_ei", [((1.0,), 1), ((0.5, 0.2, 0.05), 1), ((0.4, 0.15, 0.1, 0.05), 3), ((0.7, 0.15), 10)])
