@@ -31,8 +31,8 @@ enum { ROWINV_HIO = 0, ROWINV_PLAIN = 1 };
 template <int N> __host__ __device__ constexpr int tile_quads() { return N * NPAIR; }
 template <int N> __host__ __device__ constexpr int tile_bytes() { return N * NPAIR * 16; }
 template <int N> __host__ __device__ constexpr int tw_bytes() { return tw_count<N>() * 8; }
-// tile + twiddle tables + mbarrier
-template <int N> __host__ __device__ constexpr int smem_bytes() { return tile_bytes<N>() + tw_bytes<N>() + 16; }
+// tile + twiddle tables + mbarrier + the tile's support words (k_row_inv)
+template <int N> __host__ __device__ constexpr int smem_bytes() { return tile_bytes<N>() + tw_bytes<N>() + 16 + 2 * N; }
 
 // slot of column pair j at row py of a scratch tile
 __host__ __device__ __forceinline__ int sw(int j, int py) { return j ^ ((py >> 1) & 7); }
@@ -116,9 +116,11 @@ struct Smem {
     const float2* tw0;
     const float2* tw1;
     uint64_t* bar;
+    uint16_t* sup;   // [N] support words of the tile
     __device__ __forceinline__ explicit Smem(float4* sm)
         : tile(sm), tw0(reinterpret_cast<const float2*>(sm + tile_quads<N>())), tw1(tw0 + tw_count_stage0<N>()),
-          bar(reinterpret_cast<uint64_t*>(const_cast<float2*>(tw0) + tw_count<N>())) {}
+          bar(reinterpret_cast<uint64_t*>(const_cast<float2*>(tw0) + tw_count<N>())),
+          sup(reinterpret_cast<uint16_t*>(bar + 2)) {}
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -415,8 +417,9 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
     if (threadIdx.x == 0) mbar_init(s.bar, 1);
     __syncthreads();
     if (threadIdx.x == 0) {
-        mbar_expect_tx(s.bar, tile_bytes<N>() + tw_bytes<N>());
+        mbar_expect_tx(s.bar, tile_bytes<N>() + tw_bytes<N>() + (MODE == ROWINV_HIO ? 2 * N : 0));
         bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
+        if constexpr (MODE == ROWINV_HIO) bulk_load(s.sup, S16 + ((size_t)n * NRT + rt) * N, 2 * N, s.bar);
     }
     __syncwarp();
     {
@@ -465,12 +468,11 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
     } else {
         const MixLoader<MIXMODE> mix(cur, istride, n, Np, mp);
         const float4* __restrict__ own = cur + (size_t)n * istride + toff;
-        const uint16_t* __restrict__ Srow = S16 + ((size_t)n * NRT + rt) * N;
         const float2 nb = bc(-beta);
 #pragma unroll 4
         for (int i = threadIdx.x; i < tile_quads<N>(); i += NT) {
             const int x = i / NPAIR, j = i % NPAIR;
-            const unsigned bits = (unsigned)Srow[x] >> (2 * j);
+            const unsigned bits = (unsigned)s.sup[x] >> (2 * j);
             const c2 gh = mix(from_quad(__ldg(own + i)), toff + (size_t)i);
             const c2 gp = from_quad(tile[i]);
             const float2 ore = pfma(nb, gp.re, gh.re), oim = pfma(nb, gp.im, gh.im);
