@@ -78,7 +78,7 @@ Layout layout_of(int N, int Np)
     L.st0 = c.take(sizeof(float2) * px);
     L.st1 = c.take(sizeof(float2) * px);
     L.scr = c.take(sizeof(float2) * px);
-    L.partial = c.take(sizeof(double) * (size_t)Np * (N / TB));
+    L.partial = c.take(sizeof(double) * (size_t)Np * (N / 8));   // >= N / Radix<N>::TB tiles per image
     L.den = c.take(sizeof(double) * Np);
     L.uphi = c.take(sizeof(double) * 2 * Np);
     L.ustart = c.take(sizeof(int) * (2 * (size_t)Np + 1));
@@ -217,7 +217,7 @@ template <int N>
 int launch_row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg)
 {
     constexpr int NT = Radix<N>::NT;
-    const dim3 grid((unsigned)nimg * (N / TB));
+    const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
     const int smem = smem_bytes<N>();
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_FWD);
@@ -236,7 +236,7 @@ template <int N>
 int launch_col(cpra_plan_s* p, int mode, int n0, int nimg, float scale)
 {
     constexpr int NT = Radix<N>::NT;
-    const dim3 grid((unsigned)nimg * (N / TB));
+    const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
     const int smem = smem_bytes<N>();
     ProfScope prof(p, CPRA_PROFILE_COL);
     switch (mode) {
@@ -251,7 +251,7 @@ template <int N>
 int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg)
 {
     constexpr int NT = Radix<N>::NT;
-    const dim3 grid((unsigned)nimg * (N / TB));
+    const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
     const int smem = smem_bytes<N>();
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_INV);
@@ -341,9 +341,9 @@ int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream
     if (!p) return CPRA_ERR_INVALID_ARG;
     p->N = N; p->Np = Np; p->flags = flags;
     p->stream = (cudaStream_t)cuda_stream;
-    int R0 = 1, R1 = 1, R2 = 1, RL = 1;
-    { auto f = [&]() -> int { CPRA_DISPATCH_N(N, R0 = Radix<NN>::R0; R1 = Radix<NN>::R1; R2 = Radix<NN>::R2; RL = last_radix<NN>()); return 0; }; f(); }
-    p->geo = Geo{N, Np, R0, R1, R2, RL};
+    int R0 = 1, R1 = 1, R2 = 1, RL = 1, TBN = 16;
+    { auto f = [&]() -> int { CPRA_DISPATCH_N(N, R0 = Radix<NN>::R0; R1 = Radix<NN>::R1; R2 = Radix<NN>::R2; RL = last_radix<NN>(); TBN = tile_batch<NN>()); return 0; }; f(); }
+    p->geo = Geo{N, Np, R0, R1, R2, RL, TBN};
     // reading A2: the paper's example weights
     if (Np >= 3) { p->K = 1; p->alpha[0] = 0.6f; p->alpha[1] = 0.2f; }
     else { p->K = 0; p->alpha[0] = 1.0f; }
@@ -442,7 +442,7 @@ int cpra_set_estimate(cpra_plan_t p, const float* d_g0)
     if (!p || !d_g0) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     const size_t total = (size_t)p->Np * p->N * p->N;
-    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, (float*)p->st[p->cur], p->N, total);
+    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, (float*)p->st[p->cur], p->geo, total);
     if (int rc = check_launch(p)) return rc;
     p->t = 0;
     p->have_estimate = true;
@@ -515,7 +515,7 @@ int cpra_get_error(cpra_plan_t p, float* d_E, float* d_Eglobal)
     if (int rc = ready(p)) return rc;
     if (!p->have_error) return CPRA_ERR_NOT_READY;
     if (!d_E && !d_Eglobal) return CPRA_OK;
-    k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, d_E, d_Eglobal, p->Np, p->N / TB);
+    k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, d_E, d_Eglobal, p->Np, p->N / p->geo.TB);
     return check_launch(p);
 }
 
@@ -525,7 +525,7 @@ int cpra_get_projections(cpra_plan_t p, int which, float* d_out)
     if (int rc = ready(p)) return rc;
     if (!p->have_estimate || (which == CPRA_SUPPORTED && !p->have_support)) return CPRA_ERR_NOT_READY;
     const size_t total = (size_t)p->Np * p->N * p->N;
-    k_unpack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->st[p->cur], p->S16, (float2*)d_out, p->N, total, which == CPRA_SUPPORTED);
+    k_unpack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->st[p->cur], p->S16, (float2*)d_out, p->geo, total, which == CPRA_SUPPORTED);
     return check_launch(p);
 }
 
@@ -538,7 +538,7 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
     const unsigned nb = blocks_for(total, 256);
     int rc = CPRA_OK;
     if (sign < 0) {
-        k_pack_state<<<nb, 256, 0, p->stream>>>((const float2*)d_in, (float*)tmp, p->N, total);
+        k_pack_state<<<nb, 256, 0, p->stream>>>((const float2*)d_in, (float*)tmp, p->geo, total);
         if ((rc = check_launch(p))) return rc;
         { auto f = [&]() -> int {
             CPRA_DISPATCH_N(p->N,
@@ -558,7 +558,7 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
             if (rc == CPRA_OK) rc = launch_row_inv<NN>(p, tmp, tmp, false, MIX_NONE, 0.f, scale, 0, p->Np));
         return 0; }; f(); }
     if (rc) return rc;
-    k_unpack_state<<<nb, 256, 0, p->stream>>>((const float*)tmp, p->S16, (float2*)d_out, p->N, total, 0);
+    k_unpack_state<<<nb, 256, 0, p->stream>>>((const float*)tmp, p->S16, (float2*)d_out, p->geo, total, 0);
     return check_launch(p);
 }
 

@@ -26,8 +26,8 @@
 
 namespace cpra {
 
-constexpr int TB = 16;     // tile width = batch of transforms
-constexpr int NPAIR = 8;   // batch pairs = quads per position
+constexpr int TB = 16;     // tile width = batch of transforms (Radix<N>::TB: 8 at N = 1024, so that a tile is 64 KiB)
+constexpr int NPAIR = 8;   // batch pairs = quads per position (Radix<N>::TB / 2)
 
 // ---- stage plan ------------------------------------------------------------------------------
 // NT = threads per CTA, chosen so that the last stage has NPAIR * N / RL = B * NT butterflies with
@@ -36,14 +36,16 @@ constexpr int NPAIR = 8;   // batch pairs = quads per position
 // requests the neighbours' share of the mix for all its first-stage butterflies before it waits for its
 // own tile (MINBF = its CTAs per SM: the prefetch needs 2 x 32 more registers).
 template <int N> struct Radix;
-template <> struct Radix<16>   { static constexpr int S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
-template <> struct Radix<32>   { static constexpr int S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
-template <> struct Radix<64>   { static constexpr int S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
-template <> struct Radix<128>  { static constexpr int S = 2, R0 = 8,  R1 = 16, R2 = 1, NT = 64,  MINB = 6; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
-template <> struct Radix<256>  { static constexpr int S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128, MINB = 4; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
-template <> struct Radix<512>  { static constexpr int S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256, MINB = 3; static constexpr bool PF = true; static constexpr int MINBF = 2; };
-template <> struct Radix<1024> { static constexpr int S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 512, MINB = 1; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<16>   { static constexpr int TB = 16, S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<32>   { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<64>   { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<128>  { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 16, R2 = 1, NT = 64,  MINB = 6; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<256>  { static constexpr int TB = 16, S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128, MINB = 4; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<512>  { static constexpr int TB = 16, S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256, MINB = 3; static constexpr bool PF = true; static constexpr int MINBF = 2; };
+template <> struct Radix<1024> { static constexpr int TB = 8, S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 256, MINB = 2; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 
+template <int N> __host__ __device__ constexpr int tile_batch() { return Radix<N>::TB; }
+template <int N> __host__ __device__ constexpr int tile_pairs() { return Radix<N>::TB / 2; }
 template <int N> __host__ __device__ constexpr int last_radix() { return Radix<N>::S == 3 ? Radix<N>::R2 : Radix<N>::R1; }
 
 // position of frequency k after the forward transform (runtime radices: used by layout kernels)
@@ -177,14 +179,14 @@ __device__ __forceinline__ void twiddle(c2 (&v)[R], const float2* __restrict__ t
 template <int N, int R, int L, bool INV, int NT, int UNROLL, class LD, class ST>
 __device__ __forceinline__ void fft_stage(const float2* __restrict__ tws, LD ld, ST st)
 {
-    constexpr int M = L / R;
-    constexpr int NBF = NPAIR * (N / R);
+    constexpr int M = L / R, NP = tile_pairs<N>();
+    constexpr int NBF = NP * (N / R);
     constexpr int ITERS = (NBF + NT - 1) / NT;
 #pragma unroll UNROLL
     for (int it = 0; it < ITERS; ++it) {
         const int bf = (int)threadIdx.x + it * NT;
         if ((NBF % NT) != 0 && bf >= NBF) break;
-        const int j = bf % NPAIR, q = bf / NPAIR;
+        const int j = bf % NP, q = bf / NP;
         const int blk = q / M, n2 = q % M;
         const int base = blk * L + n2;
         c2 v[R];
@@ -203,13 +205,14 @@ __device__ __forceinline__ void fft_stage(const float2* __restrict__ tws, LD ld,
 template <int N, int R, int NT, int UNROLL, class LD, class PW, class ST>
 __device__ __forceinline__ void fft_stage_mid(LD ld, PW pw, ST st)
 {
-    constexpr int NBF = NPAIR * (N / R);
+    constexpr int NP = tile_pairs<N>();
+    constexpr int NBF = NP * (N / R);
     constexpr int ITERS = (NBF + NT - 1) / NT;
 #pragma unroll UNROLL
     for (int it = 0; it < ITERS; ++it) {
         const int bf = (int)threadIdx.x + it * NT;
         if ((NBF % NT) != 0 && bf >= NBF) break;
-        const int j = bf % NPAIR, q = bf / NPAIR;
+        const int j = bf % NP, q = bf / NP;
         c2 v[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) v[r] = ld(q * R + r, j);

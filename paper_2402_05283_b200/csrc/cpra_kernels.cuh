@@ -28,14 +28,26 @@ enum { MIX_NONE = 0, MIX_K1 = 1, MIX_GEN = 2, MIX_MASK = 3 };
 enum { COL_FULL = 0, COL_FWD = 1, COL_INV = 2 };
 enum { ROWINV_HIO = 0, ROWINV_PLAIN = 1 };
 
-template <int N> __host__ __device__ constexpr int tile_quads() { return N * NPAIR; }
-template <int N> __host__ __device__ constexpr int tile_bytes() { return N * NPAIR * 16; }
+template <int N> __host__ __device__ constexpr int tile_quads() { return N * tile_pairs<N>(); }
+template <int N> __host__ __device__ constexpr int tile_bytes() { return N * tile_pairs<N>() * 16; }
 template <int N> __host__ __device__ constexpr int tw_bytes() { return tw_count<N>() * 8; }
 // tile + twiddle tables + mbarrier + the tile's support words (k_row_inv)
 template <int N> __host__ __device__ constexpr int smem_bytes() { return tile_bytes<N>() + tw_bytes<N>() + 16 + 2 * N; }
 
-// slot of column pair j at row py of a scratch tile
-__host__ __device__ __forceinline__ int sw(int j, int py) { return j ^ ((py >> 1) & 7); }
+// slot of column pair j at row py of a scratch tile with np pairs per position
+__host__ __device__ __forceinline__ int sw(int j, int py, int np = NPAIR) { return j ^ ((py >> 1) & (np - 1)); }
+// Physical place of logical position p of a tile.  With 16 transforms per tile a position is 128 B
+// and any two positions are conflict-free.  With 8 (N = 1024) a position is 64 B = half of the bank
+// window and a quarter-warp touches two positions (two butterflies): they must differ in parity.
+// They do in every stage with stride > 1 (consecutive n2); in the stage with contiguous positions
+// (radix 8) they are 8 apart, so odd 8-blocks swap their even and odd positions.  HBM tiles have the
+// same order (they are bulk-copied verbatim).
+__host__ __device__ __forceinline__ int ppos(int p, int tb) { return tb == 16 ? p : p ^ ((p >> 3) & 1); }
+template <int N> __host__ __device__ __forceinline__ int ppos(int p)
+{
+    static_assert(tile_batch<N>() == 16 || last_radix<N>() == 8, "8-wide tiles: the contiguous stage must be radix 8");
+    return ppos(p, tile_batch<N>());
+}
 
 // The carousel mix of Eq. (4) evaluated at one quad: `q` = quad offset inside an
 // image (same for every n), `istride` = quads per image.  `own` = the quad of image n itself.
@@ -130,26 +142,33 @@ struct Smem {
 // 2 x RL/2 quads (one per row and column pair) inside the 16 x 16 block ct = RL q / 16, which
 // occupies the same 2 KiB of shared memory: position (16 ct + row) , slot jc ^ j.
 // ------------------------------------------------------------------------------------------------
-template <int RL>
-__device__ __forceinline__ void store_transposed(float4* __restrict__ tile, const c2 (&v)[RL], int q, int j)
+// `rt` = the row tile: inside its 8-row block the rows sit in the physical order of the column tile,
+// ppos(TB rt + r) = TB rt + (r ^ flip).  (With 8-wide tiles the two butterflies of a quarter-warp hit
+// the same half of the bank window here: a 2-way conflict on these 2 of the kernel's accesses.)
+template <int N>
+__device__ __forceinline__ void store_transposed(float4* __restrict__ tile, const c2 (&v)[last_radix<N>()], int q, int j, int rt)
 {
-    const int p0 = q * RL, ct = p0 / TB, jc0 = (p0 % TB) / 2;
+    constexpr int RL = last_radix<N>(), TBN = tile_batch<N>(), NP = tile_pairs<N>();
+    const int p0 = q * RL, ct = p0 / TBN, jc0 = (p0 % TBN) / 2;
+    const int r0 = ppos<N>(TBN * rt + 2 * j) % TBN, r1 = ppos<N>(TBN * rt + 2 * j + 1) % TBN;
 #pragma unroll
     for (int i = 0; i < RL / 2; ++i) {
         const int slot = (jc0 + i) ^ j;
-        tile[(ct * TB + 2 * j) * NPAIR + slot] = make_float4(v[2 * i].re.x, v[2 * i + 1].re.x, v[2 * i].im.x, v[2 * i + 1].im.x);
-        tile[(ct * TB + 2 * j + 1) * NPAIR + slot] = make_float4(v[2 * i].re.y, v[2 * i + 1].re.y, v[2 * i].im.y, v[2 * i + 1].im.y);
+        tile[(ct * TBN + r0) * NP + slot] = make_float4(v[2 * i].re.x, v[2 * i + 1].re.x, v[2 * i].im.x, v[2 * i + 1].im.x);
+        tile[(ct * TBN + r1) * NP + slot] = make_float4(v[2 * i].re.y, v[2 * i + 1].re.y, v[2 * i].im.y, v[2 * i + 1].im.y);
     }
 }
-template <int RL>
-__device__ __forceinline__ void load_transposed(const float4* __restrict__ tile, c2 (&v)[RL], int q, int j)
+template <int N>
+__device__ __forceinline__ void load_transposed(const float4* __restrict__ tile, c2 (&v)[last_radix<N>()], int q, int j, int rt)
 {
-    const int p0 = q * RL, ct = p0 / TB, jc0 = (p0 % TB) / 2;
+    constexpr int RL = last_radix<N>(), TBN = tile_batch<N>(), NP = tile_pairs<N>();
+    const int p0 = q * RL, ct = p0 / TBN, jc0 = (p0 % TBN) / 2;
+    const int r0 = ppos<N>(TBN * rt + 2 * j) % TBN, r1 = ppos<N>(TBN * rt + 2 * j + 1) % TBN;
 #pragma unroll
     for (int i = 0; i < RL / 2; ++i) {
         const int slot = (jc0 + i) ^ j;
-        const float4 a = tile[(ct * TB + 2 * j) * NPAIR + slot];
-        const float4 b = tile[(ct * TB + 2 * j + 1) * NPAIR + slot];
+        const float4 a = tile[(ct * TBN + r0) * NP + slot];
+        const float4 b = tile[(ct * TBN + r1) * NP + slot];
         v[2 * i] = c2{make_float2(a.x, b.x), make_float2(a.z, b.z)};
         v[2 * i + 1] = c2{make_float2(a.y, b.y), make_float2(a.w, b.w)};
     }
@@ -167,10 +186,11 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
           const uint16_t* __restrict__ S16, MixParams mp, int Np, int n0, int nimg)
 {
     using RX = Radix<N>;
-    constexpr int NT = RX::NT, NRT = N / TB, NCT = N / TB, RL = last_radix<N>();
-    constexpr int B = NPAIR * (N / RL) / NT;   // butterflies per thread in the last stage
-    static_assert(B * NT == NPAIR * (N / RL) && B >= 1, "last stage must fill the CTA exactly");
-    constexpr int R0 = RX::R0, M0 = N / R0, NBF0 = NPAIR * M0, IT0 = (NBF0 + NT - 1) / NT;
+    constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>();
+    constexpr int NT = RX::NT, NRT = N / TBN, NCT = N / TBN, RL = last_radix<N>();
+    constexpr int B = NP * (N / RL) / NT;   // butterflies per thread in the last stage
+    static_assert(B * NT == NP * (N / RL) && B >= 1, "last stage must fill the CTA exactly");
+    constexpr int R0 = RX::R0, M0 = N / R0, NBF0 = NP * M0, IT0 = (NBF0 + NT - 1) / NT;
     constexpr bool PFMIX = RX::PF && (MODE == MIX_K1 || MODE == MIX_GEN);
     extern __shared__ __align__(128) float4 sm[];
     const Smem<N> s(sm);
@@ -188,20 +208,22 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
         bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
     }
     const MixLoader<MODE> mix(cur, istride, n, Np, mp);
-    const uint16_t* __restrict__ Srow = S16 + ((size_t)n * NRT + rt) * N;
+    const uint16_t* __restrict__ Srow = S16 + ((size_t)n * (N / 16) + (rt * TBN) / 16) * N;   // 16-row words
+    const int sshift = (rt * TBN) % 16;
+    auto tq = [&](int p, int j) -> int { return ppos<N>(p) * NP + j; };   // quad of (position, pair) in a state tile
     if constexpr (!PFMIX) mbar_wait(s.bar, 0);
 
     auto ld_first = [&](int x, int j) -> c2 {
-        c2 v = mix(from_quad(tile[x * NPAIR + j]), toff + (size_t)x * NPAIR + j);
+        c2 v = mix(from_quad(tile[tq(x, j)]), toff + (size_t)tq(x, j));
         if constexpr (MODE == MIX_MASK) {
-            const unsigned bits = (unsigned)Srow[x] >> (2 * j);
+            const unsigned bits = (unsigned)Srow[x] >> (sshift + 2 * j);
             if (!(bits & 1)) { v.re.x = 0.f; v.im.x = 0.f; }
             if (!(bits & 2)) { v.re.y = 0.f; v.im.y = 0.f; }
         }
         return v;
     };
-    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NPAIR + j]); };
-    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NPAIR + j, v); };
+    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[tq(p, j)]); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + tq(p, j), v); };
 
     if constexpr (PFMIX) {
         // the neighbours' share of every first-stage butterfly of this thread is requested before
@@ -209,16 +231,16 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
         c2 nbv[IT0][R0];
 #pragma unroll
         for (int it = 0; it < IT0; ++it) {
-            const int bf = (int)threadIdx.x + it * NT, j = bf % NPAIR, q = bf / NPAIR;
+            const int bf = (int)threadIdx.x + it * NT, j = bf % NP, q = bf / NP;
             if (bf < NBF0) {
 #pragma unroll
-                for (int r = 0; r < R0; ++r) nbv[it][r] = mix.nbsum(toff + (size_t)(q + M0 * r) * NPAIR + j);
+                for (int r = 0; r < R0; ++r) nbv[it][r] = mix.nbsum(toff + (size_t)tq(q + M0 * r, j));
             }
         }
         mbar_wait(s.bar, 0);
 #pragma unroll
         for (int it = 0; it < IT0; ++it) {
-            const int bf = (int)threadIdx.x + it * NT, j = bf % NPAIR, q = bf / NPAIR;
+            const int bf = (int)threadIdx.x + it * NT, j = bf % NP, q = bf / NP;
             if (bf < NBF0) {
                 c2 v[R0];
 #pragma unroll
@@ -241,7 +263,7 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
     c2 v[B][RL];
 #pragma unroll
     for (int b = 0; b < B; ++b) {
-        const int bf = (int)threadIdx.x + b * NT, j = bf % NPAIR, q = bf / NPAIR;
+        const int bf = (int)threadIdx.x + b * NT, j = bf % NP, q = bf / NP;
 #pragma unroll
         for (int r = 0; r < RL; ++r) v[b][r] = ld_s(q * RL + r, j);
         dft<RL, false>(v[b]);
@@ -250,14 +272,14 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
 #pragma unroll
     for (int b = 0; b < B; ++b) {
         const int bf = (int)threadIdx.x + b * NT;
-        store_transposed<RL>(tile, v[b], bf / NPAIR, bf % NPAIR);
+        store_transposed<N>(tile, v[b], bf / NP, bf % NP, rt);
     }
     fence_async_smem();
     __syncthreads();
-    // block ct of the tile -> scratch[n][ct][16 rt .. 16 rt + 15]: 2 KiB each
-    float4* __restrict__ dst = scr + (size_t)n * istride + (size_t)rt * TB * NPAIR;
+    // block ct of the tile -> rows [TBN rt, TBN rt + TBN) of scratch tile (n, ct): TBN x TBN x 8 bytes each
+    float4* __restrict__ dst = scr + (size_t)n * istride + (size_t)rt * TBN * NP;
     for (int ct = threadIdx.x; ct < NCT; ct += NT)
-        bulk_store(dst + (size_t)ct * tile_quads<N>(), tile + ct * TB * NPAIR, TB * NPAIR * 16);
+        bulk_store(dst + (size_t)ct * tile_quads<N>(), tile + ct * TBN * NP, TBN * NP * 16);
     if (threadIdx.x < NCT) { bulk_commit(); bulk_wait_read0(); }
 }
 
@@ -310,7 +332,8 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
       double* __restrict__ partial, int n0, float scale)
 {
     using RX = Radix<N>;
-    constexpr int NT = RX::NT, NCT = N / TB, RL = last_radix<N>();
+    constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>();
+    constexpr int NT = RX::NT, NCT = N / TBN, RL = last_radix<N>();
     extern __shared__ __align__(128) float4 sm[];
     const Smem<N> s(sm);
     float4* __restrict__ tile = s.tile;
@@ -327,8 +350,8 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
     }
     mbar_wait(s.bar, 0);
 
-    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NPAIR + sw(j, p)]); };
-    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NPAIR + sw(j, p), v); };
+    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[ppos<N>(p) * NP + sw(j, p, NP)]); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + ppos<N>(p) * NP + sw(j, p, NP), v); };
 
     if constexpr (MODE == COL_FULL || MODE == COL_FWD) {
         fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_s, st_s);
@@ -342,10 +365,10 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
         fft_stage<N, RL, RL, false, NT, 1>(s.tw0, ld_s, st_s);
     }
     if constexpr (MODE == COL_FULL) {
-        const float* __restrict__ At = Aperm + ((size_t)n * NCT + ct) * N * TB;
+        const float* __restrict__ At = Aperm + ((size_t)n * NCT + ct) * N * TBN;
         float2 acc2 = make_float2(0.f, 0.f);
         auto pw = [&](c2 (&v)[RL], int q, int j) {
-            const float4* __restrict__ a4 = reinterpret_cast<const float4*>(At + (size_t)(q * NPAIR + j) * (2 * RL));
+            const float4* __restrict__ a4 = reinterpret_cast<const float4*>(At + (size_t)(q * NP + j) * (2 * RL));
             float2 a[RL];
 #pragma unroll
             for (int r = 0; r < RL / 2; ++r) {
@@ -404,8 +427,9 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
           float scale, int Np, int n0, int nimg)
 {
     using RX = Radix<N>;
-    constexpr int NT = RX::NT, NRT = N / TB, NCT = N / TB, RL = last_radix<N>();
-    constexpr int B = NPAIR * (N / RL) / NT;
+    constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>();
+    constexpr int NT = RX::NT, NRT = N / TBN, NCT = N / TBN, RL = last_radix<N>();
+    constexpr int B = NP * (N / RL) / NT;
     extern __shared__ __align__(128) float4 sm[];
     const Smem<N> s(sm);
     float4* __restrict__ tile = s.tile;
@@ -419,19 +443,19 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
     if (threadIdx.x == 0) {
         mbar_expect_tx(s.bar, tile_bytes<N>() + tw_bytes<N>() + (MODE == ROWINV_HIO ? 2 * N : 0));
         bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
-        if constexpr (MODE == ROWINV_HIO) bulk_load(s.sup, S16 + ((size_t)n * NRT + rt) * N, 2 * N, s.bar);
+        if constexpr (MODE == ROWINV_HIO) bulk_load(s.sup, S16 + ((size_t)n * (N / 16) + (rt * TBN) / 16) * N, 2 * N, s.bar);
     }
     __syncwarp();
     {
-        const float4* __restrict__ src = scr + (size_t)n * istride + (size_t)rt * TB * NPAIR;
+        const float4* __restrict__ src = scr + (size_t)n * istride + (size_t)rt * TBN * NP;
         if (threadIdx.x < 32)
             for (int ct = threadIdx.x; ct < NCT; ct += 32)
-                bulk_load(tile + ct * TB * NPAIR, src + (size_t)ct * tile_quads<N>(), TB * NPAIR * 16, s.bar);
+                bulk_load(tile + ct * TBN * NP, src + (size_t)ct * tile_quads<N>(), TBN * NP * 16, s.bar);
     }
     mbar_wait(s.bar, 0);
 
-    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NPAIR + j]); };
-    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NPAIR + j, v); };
+    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[ppos<N>(p) * NP + j]); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + ppos<N>(p) * NP + j, v); };
 
     // first inverse stage (contiguous positions, no twiddles), reading the scratch layout
     {
@@ -439,13 +463,13 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
 #pragma unroll
         for (int b = 0; b < B; ++b) {
             const int bf = (int)threadIdx.x + b * NT;
-            load_transposed<RL>(tile, v[b], bf / NPAIR, bf % NPAIR);
+            load_transposed<N>(tile, v[b], bf / NP, bf % NP, rt);
             dft<RL, true>(v[b]);
         }
         __syncthreads();
 #pragma unroll
         for (int b = 0; b < B; ++b) {
-            const int bf = (int)threadIdx.x + b * NT, j = bf % NPAIR, q = bf / NPAIR;
+            const int bf = (int)threadIdx.x + b * NT, j = bf % NP, q = bf / NP;
 #pragma unroll
             for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, v[b][r]);
         }
@@ -471,8 +495,8 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
         const float2 nb = bc(-beta);
 #pragma unroll 4
         for (int i = threadIdx.x; i < tile_quads<N>(); i += NT) {
-            const int x = i / NPAIR, j = i % NPAIR;
-            const unsigned bits = (unsigned)s.sup[x] >> (2 * j);
+            const int x = ppos<N>(i / NP), j = i % NP;   // i runs over the physical quads of the tile
+            const unsigned bits = (unsigned)s.sup[x] >> ((rt * TBN) % 16 + 2 * j);
             const c2 gh = mix(from_quad(__ldg(own + i)), toff + (size_t)i);
             const c2 gp = from_quad(tile[i]);
             const float2 ore = pfma(nb, gp.re, gh.re), oim = pfma(nb, gp.im, gh.im);

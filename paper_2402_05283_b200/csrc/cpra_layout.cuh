@@ -7,22 +7,25 @@
 namespace cpra {
 
 struct Geo {
-    int N, Np, R0, R1, R2, RL;
+    int N, Np, R0, R1, R2, RL, TB;   // TB = transforms per tile (Radix<N>::TB)
 };
 // float index of the real part of element (n, y, x) of the row-tiled state; the imaginary part is 2
 // floats further (quad = [re_a, re_b, im_a, im_b])
-__device__ __forceinline__ size_t st_idx(int N, int n, int y, int x)
+__device__ __forceinline__ size_t st_idx(const Geo& g, int n, int y, int x)
 {
-    return (((size_t)n * (N / TB) + (y / TB)) * N + x) * 32 + ((y % TB) / 2) * 4 + (y & 1);
+    const int tb = g.TB, np = tb / 2;
+    return ((((size_t)n * (g.N / tb) + (y / tb)) * g.N + ppos(x, tb)) * np + (y % tb) / 2) * 4 + (y & 1);
 }
 // the same for element (n, py, px) of the column-tiled scratch
-__device__ __forceinline__ size_t sc_idx(int N, int n, int py, int px)
+__device__ __forceinline__ size_t sc_idx(const Geo& g, int n, int py, int px)
 {
-    return (((size_t)n * (N / TB) + (px / TB)) * N + py) * 32 + sw((px % TB) / 2, py) * 4 + (px & 1);
+    const int tb = g.TB, np = tb / 2;
+    return ((((size_t)n * (g.N / tb) + (px / tb)) * g.N + ppos(py, tb)) * np + sw((px % tb) / 2, py, np)) * 4 + (px & 1);
 }
-__device__ __forceinline__ size_t a_idx(int N, int RL, int n, int py, int px)
+__device__ __forceinline__ size_t a_idx(const Geo& g, int n, int py, int px)
 {
-    return ((((size_t)n * (N / TB) + (px / TB)) * (N / RL) + (py / RL)) * NPAIR + (px % TB) / 2) * (2 * RL) + (py % RL) * 2 + (px & 1);
+    const int tb = g.TB, np = tb / 2, RL = g.RL;
+    return ((((size_t)n * (g.N / tb) + (px / tb)) * (g.N / RL) + (py / RL)) * np + (px % tb) / 2) * (2 * RL) + (py % RL) * 2 + (px & 1);
 }
 __device__ __forceinline__ float2 ld_c(const float* __restrict__ a, size_t i) { return make_float2(a[i], a[i + 2]); }
 __device__ __forceinline__ void st_c(float* __restrict__ a, size_t i, float2 v) { a[i] = v.x; a[i + 2] = v.y; }
@@ -40,7 +43,7 @@ __global__ void k_set_data(const float* __restrict__ I, const unsigned char* __r
         const float v = fmaxf(I[src], 0.f);
         const bool m = mask ? (mask[src] != 0) : true;
         const int ky = (yc + h) % N, kx = (xc + h) % N;
-        Aperm[a_idx(N, g.RL, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2))] = m ? sqrtf(v) : -1.f;
+        Aperm[a_idx(g, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2))] = m ? sqrtf(v) : -1.f;
         if (m) acc += (double)v;
     }
     __shared__ double red[32];
@@ -71,21 +74,23 @@ __global__ void k_pack_support(const unsigned char* __restrict__ S, uint16_t* __
 
 // natural [n][y][x] <-> row-tiled state; `masked` multiplies by the support.  One thread per
 // element, indexed in natural order.
-__global__ void k_pack_state(const float2* __restrict__ in, float* __restrict__ st, int N, size_t total)
+__global__ void k_pack_state(const float2* __restrict__ in, float* __restrict__ st, Geo g, size_t total)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
+    const int N = g.N;
     const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    st_c(st, st_idx(N, n, y, x), in[i]);
+    st_c(st, st_idx(g, n, y, x), in[i]);
 }
 __global__ void k_unpack_state(const float* __restrict__ st, const uint16_t* __restrict__ S16,
-                               float2* __restrict__ out, int N, size_t total, int masked)
+                               float2* __restrict__ out, Geo g, size_t total, int masked)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
+    const int N = g.N;
     const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    float2 v = ld_c(st, st_idx(N, n, y, x));
-    if (masked && !((S16[((size_t)n * (N / TB) + y / TB) * N + x] >> (y % TB)) & 1)) v = make_float2(0.f, 0.f);
+    float2 v = ld_c(st, st_idx(g, n, y, x));
+    if (masked && !((S16[((size_t)n * (N / 16) + y / 16) * N + x] >> (y % 16)) & 1)) v = make_float2(0.f, 0.f);
     out[i] = v;
 }
 // natural-order spectrum [n][ky][kx] <-> column-tiled permuted scratch
@@ -95,7 +100,7 @@ __global__ void k_unpack_spectrum(const float* __restrict__ scr, float2* __restr
     if (i >= total) return;
     const int N = g.N;
     const int kx = (int)(i % N), ky = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    out[i] = ld_c(scr, sc_idx(N, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)));
+    out[i] = ld_c(scr, sc_idx(g, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)));
 }
 __global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict__ scr, Geo g, size_t total)
 {
@@ -103,7 +108,7 @@ __global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict
     if (i >= total) return;
     const int N = g.N;
     const int kx = (int)(i % N), ky = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    st_c(scr, sc_idx(N, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)), in[i]);
+    st_c(scr, sc_idx(g, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)), in[i]);
 }
 
 // A3: E_n = sqrt(num_n / den_n), E = sqrt(sum num / sum den); one block, fixed order.
@@ -182,7 +187,7 @@ __global__ void k_assemble(const float* __restrict__ scr, float2* __restrict__ v
         if (mode == 1) {
             const int pu = fft_pos(0, g.R0, g.R1, g.R2);
             for (int n = 0; n < Np; ++n) {
-                const float2 e = ld_c(scr, sc_idx(N, n, pz, pu));
+                const float2 e = ld_c(scr, sc_idx(g, n, pz, pu));
                 const double sg = (iz & 1) ? -1.0 : 1.0;
                 vr += sg * e.x; vi += sg * e.y;
             }
@@ -202,7 +207,7 @@ __global__ void k_assemble(const float* __restrict__ scr, float2* __restrict__ v
                         const int n = code & 0x3fffffff;
                         const int ku = (code >> 30) ? -r : r;
                         const int iu = ((ku % N) + N) % N;
-                        const float2 e = ld_c(scr, sc_idx(N, n, pz, fft_pos(iu, g.R0, g.R1, g.R2)));
+                        const float2 e = ld_c(scr, sc_idx(g, n, pz, fft_pos(iu, g.R0, g.R1, g.R2)));
                         const double sg = ((iz + iu) & 1) ? -1.0 : 1.0;   // origin -> centre pixel
                         sr += sg * e.x; si += sg * e.y;
                     }
