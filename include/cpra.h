@@ -201,7 +201,8 @@ int cpra_set_chunk(cpra_plan_t plan, int images);
 #define CPRA_PROFILE_COL 1     /* forward column FFT + error + modulus + inverse column FFT */
 #define CPRA_PROFILE_ROW_INV 2 /* inverse row FFT + support / HIO */
 #define CPRA_PROFILE_IMAGE 3   /* N <= 128: the whole iteration of a projection in one kernel */
-#define CPRA_PROFILE_CLASSES 4
+#define CPRA_PROFILE_WALK 4    /* inverse row FFT + HIO of iteration t fused with mix + forward row FFT of t + 1 */
+#define CPRA_PROFILE_CLASSES 5
 int cpra_profile(cpra_plan_t plan, int enable);
 int cpra_profile_read(cpra_plan_t plan, double* h_ms, long* h_launches);
 

@@ -17,8 +17,8 @@ ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_READY, ERR_WORKSPACE, ERR_CUDA, E
 ITERATE, SUPPORTED = 0, 1
 FLAG_DEFAULT, FLAG_FORCE_MULTIPASS, FLAG_NO_CHUNKING = 0, 1, 2
 MAX_K = 8
-PROFILE_CLASSES = 4
-PROFILE_NAMES = ("row_fwd", "col", "row_inv", "image")
+PROFILE_CLASSES = 5
+PROFILE_NAMES = ("row_fwd", "col", "row_inv", "image", "walk")
 
 _vp, _ci, _cf, _cl, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_long, ctypes.c_size_t
 

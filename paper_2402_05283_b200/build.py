@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "libcpra.so")
 SOURCES = [os.path.join(HERE, "csrc", "cpra_api.cu")]
-DEPENDS = SOURCES + [os.path.join(HERE, "csrc", f) for f in ("cpra_fft.cuh", "cpra_kernels.cuh", "cpra_layout.cuh", "cpra_image.cuh")] + [
+DEPENDS = SOURCES + [os.path.join(HERE, "csrc", f) for f in ("cpra_fft.cuh", "cpra_kernels.cuh", "cpra_layout.cuh", "cpra_image.cuh", "cpra_walk.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "cpra.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]

@@ -11,6 +11,7 @@
 #include "../../include/cpra.h"
 #include "cpra_layout.cuh"
 #include "cpra_image.cuh"
+#include "cpra_walk.cuh"
 
 using namespace cpra;
 
@@ -27,6 +28,7 @@ struct cpra_plan_s {
     uint16_t* S16 = nullptr;
     float4* st[2] = {nullptr, nullptr};
     float4* scr = nullptr;
+    float4* scr2 = nullptr;   // second spectrum buffer: k_row_walk reads one and writes the other
     double* partial = nullptr;
     double* den = nullptr;
     double* uphi = nullptr;
@@ -46,6 +48,8 @@ struct cpra_plan_s {
     std::vector<int> h_ustart, h_rays;
     long launches = 0;
     int chunk = 0;  // images per L2-resident chunk; 0 = all
+    int sms = 148;     // SMs of the device
+    bool walk = true;  // use k_row_walk where the plan allows it (CPRA_WALK=0 switches it off)
     // per-kernel-class timing (cpra_profile): event pairs around every launch of the loop
     bool profiling = false;
     std::vector<cudaEvent_t> ev;      // 2 * PROF_PAIRS events, created on first use
@@ -64,7 +68,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t tw, A, S16, st0, st1, scr, partial, den, uphi, ustart, rays, total;
+    size_t tw, A, S16, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, total;
 };
 
 Layout layout_of(int N, int Np)
@@ -78,6 +82,7 @@ Layout layout_of(int N, int Np)
     L.st0 = c.take(sizeof(float2) * px);
     L.st1 = c.take(sizeof(float2) * px);
     L.scr = c.take(sizeof(float2) * px);
+    L.scr2 = c.take(sizeof(float2) * px);
     L.partial = c.take(sizeof(double) * (size_t)Np * (N / 8));   // >= N / Radix<N>::TB tiles per image
     L.den = c.take(sizeof(double) * Np);
     L.uphi = c.take(sizeof(double) * 2 * Np);
@@ -146,6 +151,7 @@ int set_attrs()
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_NONE>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_K1>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_GEN>, SM));
+    if constexpr (walk_ok<N>()) acc(allow_smem(k_row_walk<N>, walk_smem_bytes<N>()));
     if constexpr (N <= 128) {
         constexpr int ISM = image_smem_bytes<N>();
         acc(allow_smem(k_image<N, MIX_NONE>, ISM));
@@ -214,14 +220,14 @@ int mix_mode(const cpra_plan_s* p, bool fires)
 }
 
 template <int N>
-int launch_row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg)
+int launch_row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg, float4* ghat_out = nullptr)
 {
     constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
     const int smem = smem_bytes<N>();
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_FWD);
-#define ROWFWD(M) k_row_fwd<N, M><<<grid, NT, smem, p->stream>>>(cur, p->scr, p->tw, p->S16, mp, p->Np, n0, nimg)
+#define ROWFWD(M) k_row_fwd<N, M><<<grid, NT, smem, p->stream>>>(cur, p->scr, p->tw, p->S16, mp, p->Np, n0, nimg, ghat_out)
     switch (mode) {
         case MIX_NONE: ROWFWD(MIX_NONE); break;
         case MIX_K1: ROWFWD(MIX_K1); break;
@@ -233,35 +239,82 @@ int launch_row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg
 }
 
 template <int N>
-int launch_col(cpra_plan_s* p, int mode, int n0, int nimg, float scale)
+int launch_col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, float4* scr = nullptr)
 {
     constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
     const int smem = smem_bytes<N>();
     ProfScope prof(p, CPRA_PROFILE_COL);
+    if (!scr) scr = p->scr;
     switch (mode) {
-        case COL_FULL: k_col<N, COL_FULL><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
-        case COL_FWD: k_col<N, COL_FWD><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
-        default: k_col<N, COL_INV><<<grid, NT, smem, p->stream>>>(p->scr, p->A, p->tw, p->partial, n0, scale); break;
+        case COL_FULL: k_col<N, COL_FULL><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
+        case COL_FWD: k_col<N, COL_FWD><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
+        default: k_col<N, COL_INV><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
     }
     return check_launch(p);
 }
 
 template <int N>
-int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg)
+int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg,
+                   const float4* scr = nullptr, const float4* ghat_in = nullptr)
 {
     constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
     const int smem = smem_bytes<N>();
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_INV);
-#define ROWINV(H, M) k_row_inv<N, H, M><<<grid, NT, smem, p->stream>>>(p->scr, cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg)
+    if (!scr) scr = p->scr;
+#define ROWINV(H, M) k_row_inv<N, H, M><<<grid, NT, smem, p->stream>>>(scr, cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg, ghat_in)
     if (!hio) ROWINV(ROWINV_PLAIN, MIX_NONE);
     else if (mode == MIX_NONE) ROWINV(ROWINV_HIO, MIX_NONE);
     else if (mode == MIX_K1) ROWINV(ROWINV_HIO, MIX_K1);
     else ROWINV(ROWINV_HIO, MIX_GEN);
 #undef ROWINV
     return check_launch(p);
+}
+
+// K3 of one iteration fused with K1 of the next (cpra_walk.cuh): 2 CTAs per SM, each a run of tiles
+template <int N>
+int launch_walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta)
+{
+    if constexpr (walk_ok<N>()) {
+        const int total = (N / tile_batch<N>()) * p->Np;
+        const int ctas = std::min(total, 2 * p->sms);
+        const int per = (total + ctas - 1) / ctas;
+        const dim3 grid((unsigned)((total + per - 1) / per));
+        const MixParams mp = mix_params(p);
+        ProfScope prof(p, CPRA_PROFILE_WALK);
+        k_row_walk<N><<<grid, walk_threads<N>(), walk_smem_bytes<N>(), p->stream>>>(scr_in, scr_out, gh_old, gh_new, p->tw, p->S16, mp, beta, p->Np, per);
+        return check_launch(p);
+    } else {
+        return CPRA_ERR_UNSUPPORTED_SIZE;
+    }
+}
+
+// k iterations with the walking kernel: K1 (storing ghat) -> [K2 -> walk] x (k - 1) -> K2 -> K3 (reading ghat)
+template <int N>
+int iterate_walk(cpra_plan_s* p, int k, float beta, float scale)
+{
+    float4* g = p->st[p->cur];
+    float4* other = p->st[p->cur ^ 1];
+    int rc = launch_row_fwd<N>(p, g, MIX_K1, 0, p->Np, other);
+    float4 *sin = p->scr, *sout = p->scr2, *gh_old = other, *gh_new = g;
+    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
+        rc = launch_col<N>(p, COL_FULL, 0, p->Np, scale, sin);
+        if (rc != CPRA_OK) break;
+        if (it == k - 1) {
+            rc = launch_row_inv<N>(p, gh_old, gh_new, true, MIX_K1, beta, 1.0f, 0, p->Np, sin, gh_old);
+        } else {
+            rc = launch_walk<N>(p, sin, sout, gh_old, gh_new, beta);
+            std::swap(sin, sout);
+            std::swap(gh_old, gh_new);
+        }
+    }
+    if (rc != CPRA_OK) return rc;
+    p->cur = (gh_new == p->st[0]) ? 0 : 1;
+    p->t += k;
+    p->have_error = true;
+    return CPRA_OK;
 }
 
 // the whole iteration of every projection in one launch (N <= 128, cpra_image.cuh)
@@ -351,6 +404,14 @@ int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream
     p->angles.assign(Np, 0.0);
     { auto f = [&]() -> int { CPRA_DISPATCH_N(N, build_twiddles<NN>(p->h_tw)); return 0; }; f(); }
     if (const char* e = std::getenv("CPRA_CHUNK")) p->chunk = std::max(0, std::atoi(e));
+    if (const char* e = std::getenv("CPRA_WALK")) p->walk = std::atoi(e) != 0;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            p->sms = sms;
+        (void)cudaGetLastError();
+    }
     *out = p;
     return CPRA_OK;
 }
@@ -383,6 +444,7 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
     p->st[0] = (float4*)(w + L.st0);
     p->st[1] = (float4*)(w + L.st1);
     p->scr = (float4*)(w + L.scr);
+    p->scr2 = (float4*)(w + L.scr2);
     p->partial = (double*)(w + L.partial);
     p->den = (double*)(w + L.den);
     p->uphi = (double*)(w + L.uphi);
@@ -478,6 +540,12 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     if (!p->have_data || !p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
+    // the walking kernel serves the default carousel (K = 1 every iteration) on plans with 8-row tiles
+    if (k > 0 && p->walk && chunk == p->Np && p->K == 1 && p->n_ei == 1 && p->Np >= 3) {
+        int rc = CPRA_ERR_UNSUPPORTED_SIZE;
+        { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, if constexpr (walk_ok<NN>()) rc = iterate_walk<NN>(p, k, beta, scale)); return 0; }; f(); }
+        if (rc != CPRA_ERR_UNSUPPORTED_SIZE) return rc;
+    }
     for (int it = 0; it < k; ++it) {
         const int mode = mix_mode(p, (p->t % p->n_ei) == 0);
         const float4* cur = p->st[p->cur];

@@ -41,7 +41,7 @@ template <> struct Radix<32>   { static constexpr int TB = 16, S = 2, R0 = 8,  R
 template <> struct Radix<64>   { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 template <> struct Radix<128>  { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 16, R2 = 1, NT = 64,  MINB = 6; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 template <> struct Radix<256>  { static constexpr int TB = 16, S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128, MINB = 4; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
-template <> struct Radix<512>  { static constexpr int TB = 16, S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 256, MINB = 3; static constexpr bool PF = true; static constexpr int MINBF = 2; };
+template <> struct Radix<512>  { static constexpr int TB = 8, S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 128, MINB = 6; static constexpr bool PF = true; static constexpr int MINBF = 4; };
 template <> struct Radix<1024> { static constexpr int TB = 8, S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 256, MINB = 2; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 
 template <int N> __host__ __device__ constexpr int tile_batch() { return Radix<N>::TB; }

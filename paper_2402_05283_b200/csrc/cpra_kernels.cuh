@@ -183,8 +183,10 @@ __device__ __forceinline__ void load_transposed(const float4* __restrict__ tile,
 template <int N, int MODE>
 __global__ void __launch_bounds__(Radix<N>::NT, (Radix<N>::PF && (MODE == MIX_K1 || MODE == MIX_GEN)) ? Radix<N>::MINBF : Radix<N>::MINB)
 k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2* __restrict__ twg,
-          const uint16_t* __restrict__ S16, MixParams mp, int Np, int n0, int nimg)
+          const uint16_t* __restrict__ S16, MixParams mp, int Np, int n0, int nimg, float4* __restrict__ ghat_out)
 {
+    // ghat_out != nullptr: the mixed input ghat_n is also stored (state layout) for the HIO update of
+    // this iteration (read by k_row_inv / k_row_walk instead of being recomputed from three tiles)
     using RX = Radix<N>;
     constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>();
     constexpr int NT = RX::NT, NRT = N / TBN, NCT = N / TBN, RL = last_radix<N>();
@@ -220,6 +222,7 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
             if (!(bits & 1)) { v.re.x = 0.f; v.im.x = 0.f; }
             if (!(bits & 2)) { v.re.y = 0.f; v.im.y = 0.f; }
         }
+        if (ghat_out) ghat_out[(size_t)n * istride + toff + (size_t)tq(x, j)] = to_quad(v);
         return v;
     };
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[tq(p, j)]); };
@@ -245,6 +248,10 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
                 c2 v[R0];
 #pragma unroll
                 for (int r = 0; r < R0; ++r) v[r] = mix.combine(ld_s(q + M0 * r, j), nbv[it][r]);
+                if (ghat_out) {
+#pragma unroll
+                    for (int r = 0; r < R0; ++r) ghat_out[(size_t)n * istride + toff + (size_t)tq(q + M0 * r, j)] = to_quad(v[r]);
+                }
                 dft<R0, false>(v);
                 twiddle<R0, false>(v, s.tw0, q);
 #pragma unroll
@@ -424,7 +431,7 @@ template <int N, int MODE, int MIXMODE>
 __global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
 k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4* __restrict__ nxt,
           const float2* __restrict__ twg, const uint16_t* __restrict__ S16, MixParams mp, float beta,
-          float scale, int Np, int n0, int nimg)
+          float scale, int Np, int n0, int nimg, const float4* __restrict__ ghat_in)
 {
     using RX = Radix<N>;
     constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>();
@@ -497,7 +504,9 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
         for (int i = threadIdx.x; i < tile_quads<N>(); i += NT) {
             const int x = ppos<N>(i / NP), j = i % NP;   // i runs over the physical quads of the tile
             const unsigned bits = (unsigned)s.sup[x] >> ((rt * TBN) % 16 + 2 * j);
-            const c2 gh = mix(from_quad(__ldg(own + i)), toff + (size_t)i);
+            // ghat: stored by k_row_fwd / k_row_walk (ghat_in), else recomputed from the previous state
+            const c2 gh = ghat_in ? from_quad(__ldg(ghat_in + (size_t)n * istride + toff + i))
+                                  : mix(from_quad(__ldg(own + i)), toff + (size_t)i);
             const c2 gp = from_quad(tile[i]);
             const float2 ore = pfma(nb, gp.re, gh.re), oim = pfma(nb, gp.im, gh.im);
             float4 o;

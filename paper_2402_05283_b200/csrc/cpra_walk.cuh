@@ -1,0 +1,206 @@
+// cpra_walk.cuh -- K3 of iteration t fused with K1 of iteration t + 1 in a CTA that WALKS along n
+// (sm_100a; plans with 8-row tiles: a tile is N x 64 B = 32 KiB at N = 512).
+//
+// The carousel mix (Eq. (4)) needs the NEW states of projections n-1, n, n+1.  A CTA
+// that owns a run of consecutive n for one row tile rt keeps the last three new tiles in shared
+// memory (3 slots), so the mix reads no neighbour from L2 or HBM at all, and the forward row FFT of
+// iteration t + 1 follows the support / HIO update of iteration t without the state ever being
+// written as g:
+//     A(i):  spectrum tile of projection m_i (after the column pass)  --bulk copies-->  slot i % 3
+//            inverse FFT along x, in place; the last stage stays in registers:
+//            g_new = S ? g' : ghat_old - beta g'   (ghat_old = the mixed input of iteration t, stored
+//            by the previous walk: ONE 128-bit load per quad, requested before the tile is waited for)
+//            g_new goes back to the slot and stays in the registers v
+//     B(i):  ghat_new(m_i) = a0 g_new(m_i) + a1 (g_new(m_{i-1}) + g_new(m_{i+1})):  m_{i-1} from the
+//            registers gm, m_i from slot i % 3, m_{i+1} from v (A(i+1) ran just before); stored for the
+//            next HIO; forward FFT along x in place in slot i % 3, transposed, bulk-stored into the
+//            OTHER scratch buffer; then the tile of m_{i+3} is loaded into that slot: it is needed
+//            a whole step later, so its latency is covered.
+// HBM traffic of a walk: spectrum in 8 + ghat_old 8 + support 1/8 + ghat_new 8 + spectrum out 8 =
+// 32.125 B/px, against 16 + 24.125 for K1 + K3, and no neighbour loads.  The two tiles next to a run
+// (halo) are inverse-transformed twice (by this CTA and by their owner): the spectra are therefore
+// read from one scratch buffer and written to the other.
+#pragma once
+#include "cpra_kernels.cuh"
+
+namespace cpra {
+
+template <int N> __host__ __device__ constexpr bool walk_ok() { return tile_batch<N>() == 8 && Radix<N>::S == 3 && N <= 512; }
+constexpr int WALK_SLOTS = 3;
+// slots + twiddles + 3 mbarriers + support words of the 3 slots
+template <int N> __host__ __device__ constexpr int walk_smem_bytes()
+{
+    return WALK_SLOTS * tile_bytes<N>() + tw_bytes<N>() + 32 + WALK_SLOTS * 2 * N;
+}
+template <int N> __host__ __device__ constexpr int walk_threads() { return tile_pairs<N>() * (N / last_radix<N>()); }
+
+template <int N>
+__global__ void __launch_bounds__(walk_threads<N>(), 2)
+k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, const float4* __restrict__ gh_old,
+           float4* __restrict__ gh_new, const float2* __restrict__ twg, const uint16_t* __restrict__ S16,
+           MixParams mp, float beta, int Np, int per_cta)
+{
+    using RX = Radix<N>;
+    constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>(), NT = walk_threads<N>();
+    constexpr int NRT = N / TBN, NCT = N / TBN, R0 = RX::R0, R1 = RX::R1, RL = RX::R2, M0 = N / R0;
+    static_assert(NP * M0 == NT && NP * (N / R1) == NT && RL == 8, "one butterfly per thread in every stage");
+    extern __shared__ __align__(128) float4 sm[];
+    float4* const slots = sm;
+    const float2* const tw0 = reinterpret_cast<const float2*>(sm + WALK_SLOTS * tile_quads<N>());
+    const float2* const tw1 = tw0 + tw_count_stage0<N>();
+    uint64_t* const full = reinterpret_cast<uint64_t*>(const_cast<float2*>(tw0) + tw_count<N>());   // [3] + 1 for the twiddles
+    uint16_t* const sup = reinterpret_cast<uint16_t*>(full + 4);                                     // [3][N]
+    const size_t istride = (size_t)N * N / 2;
+    const int total = NRT * Np;
+    const int u0 = (int)blockIdx.x * per_cta, u1 = min(total, u0 + per_cta);
+    if (u0 >= u1) return;
+    const int j = threadIdx.x % NP, q = threadIdx.x / NP;   // this thread's butterfly in every stage
+    constexpr int IO = NCT < NT ? NCT : NT;   // threads that issue the bulk copies
+    const bool io = threadIdx.x < IO;
+
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < 4; ++b) mbar_init(full + b, 1);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        mbar_expect_tx(full + 3, tw_bytes<N>());
+        bulk_load(const_cast<float2*>(tw0), twg, tw_bytes<N>(), full + 3);
+    }
+    unsigned phase = 0;   // bit s = parity of the next completion of full[s]
+    auto tq = [&](int p, int jj) -> int { return ppos<N>(p) * NP + jj; };
+    const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]), nbeta = bc(-beta);
+
+    // issue the bulk loads of projection m's spectrum tile (row tile rt) and support words into slot s
+    // (called by the threads io: one 512-byte block each, so that no warp spends a pass issuing copies)
+    auto load_tile = [&](int m, int rt, int s) {
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(full + s, tile_bytes<N>() + 2 * N);
+            bulk_load(sup + s * N, S16 + ((size_t)m * (N / 16) + (rt * TBN) / 16) * N, 2 * N, full + s);
+        }
+        const float4* __restrict__ src = scr_in + (size_t)m * istride + (size_t)rt * TBN * NP;
+        float4* dst = slots + s * tile_quads<N>();
+        for (int ct = threadIdx.x; ct < NCT; ct += IO)
+            bulk_load(dst + ct * TBN * NP, src + (size_t)ct * tile_quads<N>(), TBN * NP * 16, full + s);
+    };
+
+    mbar_wait(full + 3, 0);
+    for (int u = u0; u < u1;) {
+        // a run: consecutive n in [na, nb] of one row tile rt
+        const int rt = u / Np, na = u % Np, nb = min(Np - 1, na + (u1 - u) - 1), len = nb - na + 1;
+        const int sshift = (rt * TBN) % 16;
+        auto proj = [&](int i) -> int { int m = na - 1 + i; return m < 0 ? m + Np : (m >= Np ? m - Np : m); };   // i = 0 .. len + 1
+        if (io) {
+            for (int i = 0; i < 3 && i < len + 2; ++i) load_tile(proj(i), rt, i);
+        }
+        // A(i): inverse FFT along x + support / HIO of projection proj(i) in slot i % 3.  The last
+        // stage and the update happen in registers (ghat_old requested before the tile is waited
+        // for); the new state goes back to the slot AND stays in v for the mix of B(i - 1).
+        c2 v[R0];
+        int pend_tile = -1, pend_slot = 0;   // refill of the slot B stored from, issued one pass into the next A
+        auto stepA = [&](int i) {
+            const int s = i % 3, m = proj(i);
+            float4* const tile = sm + s * tile_quads<N>();
+            const float4* __restrict__ gh = gh_old + (size_t)m * istride + (size_t)rt * tile_quads<N>();
+            c2 g0[R0];
+#pragma unroll
+            for (int r = 0; r < R0; ++r) g0[r] = from_quad(__ldg(gh + tq(q + M0 * r, j)));
+            mbar_wait(full + s, (phase >> s) & 1u);
+            phase ^= 1u << s;
+            auto ld_s = [&](int p, int jj) -> c2 { return from_quad(tile[tq(p, jj)]); };
+            auto st_s = [&](int p, int jj, c2 w) { st_quad(tile + tq(p, jj), w); };
+            {
+                c2 w[RL];
+                load_transposed<N>(tile, w, q, j, rt);
+                dft<RL, true>(w);
+                __syncthreads();
+#pragma unroll
+                for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, w[r]);
+            }
+            __syncthreads();
+            fft_stage<N, R1, N / R0, true, NT, 1>(tw1, ld_s, st_s);
+            __syncthreads();
+            if (io && pend_tile >= 0) {   // the store of the last B has been read out by now: no one waits here
+                bulk_wait_read0();
+                load_tile(proj(pend_tile), rt, pend_slot);
+            }
+            pend_tile = -1;
+#pragma unroll
+            for (int r = 0; r < R0; ++r) v[r] = ld_s(q + M0 * r, j);
+            twiddle<R0, true>(v, tw0, q);
+            dft<R0, true>(v);
+            const uint16_t* __restrict__ sp = sup + s * N;
+#pragma unroll
+            for (int r = 0; r < R0; ++r) {
+                const unsigned bits = (unsigned)sp[q + M0 * r] >> (sshift + 2 * j);
+                const float2 ore = pfma(nbeta, v[r].re, g0[r].re), oim = pfma(nbeta, v[r].im, g0[r].im);
+                v[r].re = make_float2((bits & 1) ? v[r].re.x : ore.x, (bits & 2) ? v[r].re.y : ore.y);
+                v[r].im = make_float2((bits & 1) ? v[r].im.x : oim.x, (bits & 2) ? v[r].im.y : oim.y);
+                st_s(q + M0 * r, j, v[r]);
+            }
+            // no barrier: the quads written here are read back by this same thread (the mix of B(i))
+        };
+        // B(i): ghat_new(m_i) from gm (registers: g_new(m_{i-1})), slot i % 3 (g_new(m_i)) and v
+        // (registers: g_new(m_{i+1})); forward FFT along x in place in slot i % 3, store; refill it
+        // with the tile of m_{i+3}.  The quads read from the slot become the next gm.
+        c2 gm[R0];
+        auto stepB = [&](int i) {
+            const int m = proj(i), s0 = i % 3;
+            float4* const t0 = sm + s0 * tile_quads<N>();
+            float4* __restrict__ gout = gh_new + (size_t)m * istride + (size_t)rt * tile_quads<N>();
+            auto ld_s = [&](int p, int jj) -> c2 { return from_quad(t0[tq(p, jj)]); };
+            auto st_s = [&](int p, int jj, c2 w) { st_quad(t0 + tq(p, jj), w); };
+            {
+                c2 w[R0];
+#pragma unroll
+                for (int r = 0; r < R0; ++r) {
+                    const int i2 = tq(q + M0 * r, j);
+                    const c2 own = from_quad(t0[i2]);
+                    w[r] = c2{pfma(a0, own.re, pmul(a1, padd(gm[r].re, v[r].re))), pfma(a0, own.im, pmul(a1, padd(gm[r].im, v[r].im)))};
+                    gm[r] = own;
+                    gout[i2] = to_quad(w[r]);
+                }
+                dft<R0, false>(w);
+                twiddle<R0, false>(w, tw0, q);
+#pragma unroll
+                for (int r = 0; r < R0; ++r) st_s(q + M0 * r, j, w[r]);
+            }
+            __syncthreads();
+            fft_stage<N, R1, N / R0, false, NT, 1>(tw1, ld_s, st_s);
+            __syncthreads();
+            {
+                c2 w[RL];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) w[r] = ld_s(q * RL + r, j);
+                dft<RL, false>(w);
+                __syncthreads();
+                store_transposed<N>(t0, w, q, j, rt);
+            }
+            fence_async_smem();
+            __syncthreads();
+            if (io) {
+                float4* __restrict__ dst = scr_out + (size_t)m * istride + (size_t)rt * TBN * NP;
+                for (int ct = threadIdx.x; ct < NCT; ct += IO)
+                    bulk_store(dst + (size_t)ct * tile_quads<N>(), t0 + ct * TBN * NP, TBN * NP * 16);
+                bulk_commit();
+            }
+            pend_tile = (i + 3 <= len + 1) ? i + 3 : -1;
+            pend_slot = s0;
+        };
+        // A(0) A(1) A(2) B(1) A(3) B(2) ... A(len + 1) B(len)   (one call site each: both bodies inline)
+        for (int i = 0; i <= len + 1; ++i) {
+            stepA(i);
+            if (i == 0) {   // the first halo tile is only needed in registers: its slot takes the tile of m_3 at once
+#pragma unroll
+                for (int r = 0; r < R0; ++r) gm[r] = v[r];
+                __syncthreads();   // every thread is done with slot 0
+                if (io && 3 <= len + 1) load_tile(proj(3), rt, 0);
+            }
+            if (i >= 2) stepB(i - 1);
+        }
+        if (io) bulk_wait_read0();
+        __syncthreads();   // the last store has been read out (warp 0 waited) before the next run reloads the slots
+        u += len;
+    }
+}
+
+}  // namespace cpra
