@@ -101,9 +101,9 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
             const int s = i % 3, m = proj(i);
             float4* const tile = sm + s * tile_quads<N>();
             const float4* __restrict__ gh = gh_old + (size_t)m * istride + (size_t)rt * tile_quads<N>();
-            c2 g0[R0];
+            // ghat_old: pulled into L2 now, into registers two passes later (keeps 32 registers free)
 #pragma unroll
-            for (int r = 0; r < R0; ++r) g0[r] = from_quad(__ldg(gh + tq(q + M0 * r, j)));
+            for (int r = 0; r < R0; ++r) asm volatile("prefetch.global.L2 [%0];" ::"l"(gh + tq(q + M0 * r, j)));
             mbar_wait(full + s, (phase >> s) & 1u);
             phase ^= 1u << s;
             auto ld_s = [&](int p, int jj) -> c2 { return from_quad(tile[tq(p, jj)]); };
@@ -117,6 +117,9 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
                 for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, w[r]);
             }
             __syncthreads();
+            c2 g0[R0];
+#pragma unroll
+            for (int r = 0; r < R0; ++r) g0[r] = from_quad(__ldg(gh + tq(q + M0 * r, j)));
             fft_stage<N, R1, N / R0, true, NT, 1>(tw1, ld_s, st_s);
             __syncthreads();
             if (io && pend_tile >= 0) {   // the store of the last B has been read out by now: no one waits here
