@@ -268,6 +268,39 @@ def test_carousel_variants(torch_cuda, alpha, n_ei):
     assert abs(Eg - o.get_error()[1]) <= TOL_E * o.get_error()[1]
 
 
+@pytest.mark.parametrize("N,alpha,n_ei,chunk", [(512, (0.5, 0.2, 0.05), 1, 0), (512, (0.6, 0.2), 1, 2), (512, (0.6, 0.2), 3, 0),
+                                                (1024, (0.5, 0.2, 0.05), 1, 0), (256, (0.4, 0.15, 0.1, 0.05), 2, 0)])
+def test_tile_kernels_on_8_row_plans(torch_cuda, N, alpha, n_ei, chunk):
+    """N = 512 runs the walking kernel for the default carousel; a wider carousel (K > 1), n_ei > 1
+    and chunked runs go through the three tile kernels (8-row tiles at N >= 512): against the oracle."""
+    p = cpra_inputs.random_stack(N, max(5, 2 * len(alpha) - 1), seed=N + len(alpha), beamstop=3)
+    o, g = _oracle(p, alpha, n_ei), _gpu(p, alpha, n_ei)
+    if chunk:
+        g.set_chunk(chunk)
+    o.iterate(3, 0.9)
+    g.iterate(3, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 3 * TOL_1
+    E, Eg = _errors(g)
+    Eo, Ego = o.get_error()
+    assert np.abs(E - Eo).max() <= TOL_E * Eo.max() and abs(Eg - Ego) <= TOL_E * Ego
+
+
+def test_walking_kernel_runs_and_seams(torch_cuda):
+    """The walking kernel at N = 512 with N_p = 7 (runs shorter than the 3-slot pipeline, wrap-around
+    halos inside a run) and with calls split so that K1 / K3 (first / last iteration of a call) and
+    the walk (iterations in between) alternate: against the oracle, and bit-identical to one call."""
+    p = cpra_inputs.random_stack(512, 7, seed=77, beamstop=5)
+    o, g, h = _oracle(p), _gpu(p), _gpu(p)
+    o.iterate(6, 0.9)
+    g.iterate(6, 0.9)
+    for k in (1, 3, 2):
+        h.iterate(k, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 6 * TOL_1
+    assert np.array_equal(_get(g).view(np.uint32), _get(h).view(np.uint32))
+    _, Eg = _errors(g)
+    assert abs(Eg - o.get_error()[1]) <= TOL_E * o.get_error()[1]
+
+
 @pytest.mark.parametrize("N,Np", [(16, 1), (16, 2), (32, 3), (64, 1), (128, 5), (256, 2), (512, 1), (1024, 1)])
 def test_small_and_ragged_stacks(torch_cuda, N, Np):
     """Np = 1 and 2 (no room for K = 1: default falls back to no coupling), Np = 3 (every image is
