@@ -654,7 +654,10 @@ int cpra_assemble_3d(cpra_plan_t p, float* d_vol, float* d_weight)
     const int zsplit = std::max(1, std::min(N, 4096 / std::max(1, (N * N) / 256)));
     const int zper = (N + zsplit - 1) / zsplit;
     const dim3 grid(blocks_for((size_t)N * N, 128), (unsigned)((N + zper - 1) / zper));
-    k_assemble<<<grid, 128, 0, p->stream>>>((const float*)p->scr, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
+    const size_t total = (size_t)p->Np * N * N;
+    k_unpack_spectrum_T<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->scr, (float2*)p->scr2, p->geo, total);
+    if (int rc2 = check_launch(p)) return rc2;
+    k_assemble<<<grid, 128, 0, p->stream>>>((const float2*)p->scr2, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
     return check_launch(p);
 }
 

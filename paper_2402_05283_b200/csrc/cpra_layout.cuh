@@ -102,6 +102,16 @@ __global__ void k_unpack_spectrum(const float* __restrict__ scr, float2* __restr
     const int kx = (int)(i % N), ky = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
     out[i] = ld_c(scr, sc_idx(g, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)));
 }
+// spectrum of the assembly: column-tiled permuted scratch -> natural order, TRANSPOSED: Et[n][ku][kz],
+// kz fastest, so that the gather kernel, which walks kz for fixed (n, ku), streams contiguous memory
+__global__ void k_unpack_spectrum_T(const float* __restrict__ scr, float2* __restrict__ Et, Geo g, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = g.N;
+    const int kz = (int)(i % N), ku = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+    Et[i] = ld_c(scr, sc_idx(g, n, fft_pos(kz, g.R0, g.R1, g.R2), fft_pos(ku, g.R0, g.R1, g.R2)));
+}
 __global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict__ scr, Geo g, size_t total)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -139,13 +149,14 @@ __global__ void k_finalize_error(const double* __restrict__ partial, const doubl
 
 // ------------------------------------------------------------------------------------------------
 // A7: Fourier-slice assembly (slice theorem PAPER.md:35-44; reading A17).
-// scr holds E_n = F[S_n g_n] in the permuted column-tiled layout.  One thread per (ky, kx) computes
-// the polar geometry in fp64 once, then walks kz.
+// Et holds E_n = F[S_n g_n] in natural order, [n][ku][kz] (k_unpack_spectrum_T).  One thread per
+// (ky, kx) computes the polar geometry in fp64 once, then walks kz: each of its taps is a contiguous
+// stream.
 //   uphi[U]      sorted unique ray directions in [0, 2 pi)
 //   ustart[U+1]  contributors of unique ray u are rays[ustart[u] .. ustart[u+1])
 //   rays[]       n | (neg << 30): the slice and whether the ray is its ku <= 0 half
 // ------------------------------------------------------------------------------------------------
-__global__ void k_assemble(const float* __restrict__ scr, float2* __restrict__ vol, float* __restrict__ wgt,
+__global__ void k_assemble(const float2* __restrict__ Et, float2* __restrict__ vol, float* __restrict__ wgt,
                            const double* __restrict__ uphi, const int* __restrict__ ustart,
                            const int* __restrict__ rays, int U, Geo g, int zper)
 {
@@ -181,13 +192,11 @@ __global__ void k_assemble(const float* __restrict__ scr, float2* __restrict__ v
     const int z0 = blockIdx.y * zper, z1 = min(N, z0 + zper);
     for (int iz = z0; iz < z1; ++iz) {
         const int kz = iz < h ? iz : iz - N;
-        const int pz = fft_pos(iz, g.R0, g.R1, g.R2);
         double vr = 0.0, vi = 0.0;
         float w = 0.f;
         if (mode == 1) {
-            const int pu = fft_pos(0, g.R0, g.R1, g.R2);
             for (int n = 0; n < Np; ++n) {
-                const float2 e = ld_c(scr, sc_idx(g, n, pz, pu));
+                const float2 e = __ldg(Et + (size_t)n * N * N + iz);
                 const double sg = (iz & 1) ? -1.0 : 1.0;
                 vr += sg * e.x; vi += sg * e.y;
             }
@@ -207,7 +216,7 @@ __global__ void k_assemble(const float* __restrict__ scr, float2* __restrict__ v
                         const int n = code & 0x3fffffff;
                         const int ku = (code >> 30) ? -r : r;
                         const int iu = ((ku % N) + N) % N;
-                        const float2 e = ld_c(scr, sc_idx(g, n, pz, fft_pos(iu, g.R0, g.R1, g.R2)));
+                        const float2 e = __ldg(Et + ((size_t)n * N + iu) * N + iz);
                         const double sg = ((iz + iu) & 1) ? -1.0 : 1.0;   // origin -> centre pixel
                         sr += sg * e.x; si += sg * e.y;
                     }
