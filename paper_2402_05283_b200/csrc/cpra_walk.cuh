@@ -44,6 +44,7 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
     constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>(), NT = walk_threads<N>();
     constexpr int NRT = N / TBN, NCT = N / TBN, R0 = RX::R0, R1 = RX::R1, RL = RX::R2, M0 = N / R0;
     static_assert(NP * M0 == NT && NP * (N / R1) == NT && RL == 8, "one butterfly per thread in every stage");
+    static_assert(NP == 4 && R1 == 8, "the two inner stages of a 64-position block must belong to one warp");
     extern __shared__ __align__(128) float4 sm[];
     float4* const slots = sm;
     const float2* const tw0 = reinterpret_cast<const float2*>(sm + WALK_SLOTS * tile_quads<N>());
@@ -112,11 +113,11 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
                 c2 w[RL];
                 load_transposed<N>(tile, w, q, j, rt);
                 dft<RL, true>(w);
-                __syncthreads();
-#pragma unroll
+                __syncwarp();   // positions [64 b, 64 b + 64) of a tile belong to warp b in the two
+#pragma unroll                  // inner stages (radix 8 x 8, 4 pairs): their exchanges stay inside a warp
                 for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, w[r]);
             }
-            __syncthreads();
+            __syncwarp();
             c2 g0[R0];
 #pragma unroll
             for (int r = 0; r < R0; ++r) g0[r] = from_quad(__ldg(gh + tq(q + M0 * r, j)));
@@ -169,13 +170,13 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
             }
             __syncthreads();
             fft_stage<N, R1, N / R0, false, NT, 1>(tw1, ld_s, st_s);
-            __syncthreads();
+            __syncwarp();
             {
                 c2 w[RL];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) w[r] = ld_s(q * RL + r, j);
                 dft<RL, false>(w);
-                __syncthreads();
+                __syncwarp();
                 store_transposed<N>(t0, w, q, j, rt);
             }
             fence_async_smem();
