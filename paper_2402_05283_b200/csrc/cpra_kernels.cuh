@@ -121,6 +121,18 @@ struct MixLoader {
     }
 };
 
+// Barrier between the two inner stages of a 3-stage plan.  With 4 pairs per position and radices
+// R1 = RL = 8, butterfly bf of either stage works inside the 64-position block bf / 32, i.e. every
+// warp owns whole blocks: the exchange stays inside the warp and a warp barrier is enough.
+template <int N> __host__ __device__ constexpr bool inner_stages_warp_local()
+{
+    return Radix<N>::S == 3 && tile_pairs<N>() == 4 && Radix<N>::R1 == 8 && Radix<N>::R2 == 8;
+}
+template <int N> __device__ __forceinline__ void inner_sync()
+{
+    if constexpr (inner_stages_warp_local<N>()) __syncwarp(); else __syncthreads();
+}
+
 // shared-memory carve-up of the three kernels
 template <int N>
 struct Smem {
@@ -264,7 +276,7 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
     __syncthreads();
     if constexpr (RX::S == 3) {
         fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);
-        __syncthreads();
+        inner_sync<N>();
     }
     // last stage (contiguous positions, no twiddles) + transposition into the scratch layout
     c2 v[B][RL];
@@ -275,7 +287,7 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
         for (int r = 0; r < RL; ++r) v[b][r] = ld_s(q * RL + r, j);
         dft<RL, false>(v[b]);
     }
-    __syncthreads();
+    inner_sync<N>();   // (the block a butterfly is transposed into lies in its own 64-position block)
 #pragma unroll
     for (int b = 0; b < B; ++b) {
         const int bf = (int)threadIdx.x + b * NT;
@@ -342,6 +354,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
     constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>();
     constexpr int NT = RX::NT, NCT = N / TBN, RL = last_radix<N>();
     extern __shared__ __align__(128) float4 sm[];
+    __shared__ float red[32];   // per-warp error sums of the tile
     const Smem<N> s(sm);
     float4* __restrict__ tile = s.tile;
     const int n = n0 + (int)(blockIdx.x / (unsigned)NCT);
@@ -365,7 +378,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
         __syncthreads();
         if constexpr (RX::S == 3) {
             fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);
-            __syncthreads();
+            inner_sync<N>();
         }
     }
     if constexpr (MODE == COL_FWD) {
@@ -388,26 +401,23 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
         };
         fft_stage_mid<N, RL, NT, 1>(ld_s, pw, st_s);
         float acc = acc2.x + acc2.y;
-        // block reduction of the error numerator (fixed order: deterministic)
-        __shared__ float red[32];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
         if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double t = 0.0;
-            for (int w = 0; w < NT / 32; ++w) t += (double)red[w];
-            partial[(size_t)n * NCT + ct] = t;
-        }
     }
-    if constexpr (MODE == COL_INV) {
-        fft_stage<N, RL, RL, true, NT, 1>(s.tw0, ld_s, st_s);
-        __syncthreads();
-    }
+    if constexpr (MODE == COL_INV) fft_stage<N, RL, RL, true, NT, 1>(s.tw0, ld_s, st_s);
     if constexpr (MODE != COL_FWD) {
         if constexpr (RX::S == 3) {
+            inner_sync<N>();
             fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(s.tw1, ld_s, st_s);
-            __syncthreads();
+        }
+        __syncthreads();
+        if constexpr (MODE == COL_FULL) {
+            if (threadIdx.x == 0) {   // error numerator of the tile, fixed order: deterministic
+                double t = 0.0;
+                for (int w = 0; w < NT / 32; ++w) t += (double)red[w];
+                partial[(size_t)n * NCT + ct] = t;
+            }
         }
         fft_stage<N, RX::R0, N, true, NT, 1>(s.tw0, ld_s, st_s);
     }
@@ -473,7 +483,7 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
             load_transposed<N>(tile, v[b], bf / NP, bf % NP, rt);
             dft<RL, true>(v[b]);
         }
-        __syncthreads();
+        inner_sync<N>();
 #pragma unroll
         for (int b = 0; b < B; ++b) {
             const int bf = (int)threadIdx.x + b * NT, j = bf % NP, q = bf / NP;
@@ -481,7 +491,7 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
             for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, v[b][r]);
         }
     }
-    __syncthreads();
+    inner_sync<N>();
     if constexpr (RX::S == 3) {
         fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(s.tw1, ld_s, st_s);
         __syncthreads();
