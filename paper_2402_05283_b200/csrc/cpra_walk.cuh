@@ -68,7 +68,18 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
         bulk_load(const_cast<float2*>(tw0), twg, tw_bytes<N>(), full + 3);
     }
     unsigned phase = 0;   // bit s = parity of the next completion of full[s]
-    auto tq = [&](int p, int jj) -> int { return ppos<N>(p) * NP + jj; };
+    // Quad offsets of this thread's butterfly in the three stages, as one base (two for the stages
+    // whose positions cross 8-blocks of alternating parity, see ppos) plus a compile-time multiple of r:
+    //   stage 0 (stride M0):    p = q + M0 r            ppos(p) = ppos(q) + M0 r
+    //   stage 1 (stride 8):     p = 64 b + n2 + 8 r     ppos(p) = p ^ (r & 1)
+    //   last    (contiguous):   p = 8 q + r             ppos(p) = 8 q + (r ^ (q & 1))
+    const int o0 = ppos<N>(q) * NP + j;
+    const int o1e = ((q / 8) * 64 + (q % 8)) * NP + j, o1o = ((q / 8) * 64 + ((q % 8) ^ 1)) * NP + j;
+    const int oLe = (8 * q + (q & 1)) * NP + j, oLo = (8 * q + 1 - (q & 1)) * NP + j;
+    auto i0 = [&](int r) -> int { return o0 + r * (M0 * NP); };
+    auto i1 = [&](int r) -> int { return ((r & 1) ? o1o : o1e) + r * (8 * NP); };
+    auto iL = [&](int r) -> int { return ((r & 1) ? oLo : oLe) + (r & ~1) * NP; };
+    static_assert(R0 == 8 && N / R0 == 64, "offsets above assume an 8 x 8 x 8 plan");
     const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]), nbeta = bc(-beta);
 
     // issue the bulk loads of projection m's spectrum tile (row tile rt) and support words into slot s
@@ -104,24 +115,30 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
             const float4* __restrict__ gh = gh_old + (size_t)m * istride + (size_t)rt * tile_quads<N>();
             // ghat_old: pulled into L2 now, into registers two passes later (keeps 32 registers free)
 #pragma unroll
-            for (int r = 0; r < R0; ++r) asm volatile("prefetch.global.L2 [%0];" ::"l"(gh + tq(q + M0 * r, j)));
+            for (int r = 0; r < R0; ++r) asm volatile("prefetch.global.L2 [%0];" ::"l"(gh + i0(r)));
             mbar_wait(full + s, (phase >> s) & 1u);
             phase ^= 1u << s;
-            auto ld_s = [&](int p, int jj) -> c2 { return from_quad(tile[tq(p, jj)]); };
-            auto st_s = [&](int p, int jj, c2 w) { st_quad(tile + tq(p, jj), w); };
             {
                 c2 w[RL];
                 load_transposed<N>(tile, w, q, j, rt);
                 dft<RL, true>(w);
                 __syncwarp();   // positions [64 b, 64 b + 64) of a tile belong to warp b in the two
 #pragma unroll                  // inner stages (radix 8 x 8, 4 pairs): their exchanges stay inside a warp
-                for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, w[r]);
+                for (int r = 0; r < RL; ++r) st_quad(tile + iL(r), w[r]);
             }
             __syncwarp();
             c2 g0[R0];
 #pragma unroll
-            for (int r = 0; r < R0; ++r) g0[r] = from_quad(__ldg(gh + tq(q + M0 * r, j)));
-            fft_stage<N, R1, N / R0, true, NT, 1>(tw1, ld_s, st_s);
+            for (int r = 0; r < R0; ++r) g0[r] = from_quad(__ldg(gh + i0(r)));
+            {
+                c2 w[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) w[r] = from_quad(tile[i1(r)]);
+                twiddle<R1, true>(w, tw1, q % 8);
+                dft<R1, true>(w);
+#pragma unroll
+                for (int r = 0; r < R1; ++r) st_quad(tile + i1(r), w[r]);
+            }
             __syncthreads();
             if (io && pend_tile >= 0) {   // the store of the last B has been read out by now: no one waits here
                 bulk_wait_read0();
@@ -129,7 +146,7 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
             }
             pend_tile = -1;
 #pragma unroll
-            for (int r = 0; r < R0; ++r) v[r] = ld_s(q + M0 * r, j);
+            for (int r = 0; r < R0; ++r) v[r] = from_quad(tile[i0(r)]);
             twiddle<R0, true>(v, tw0, q);
             dft<R0, true>(v);
             const uint16_t* __restrict__ sp = sup + s * N;
@@ -139,7 +156,7 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
                 const float2 ore = pfma(nbeta, v[r].re, g0[r].re), oim = pfma(nbeta, v[r].im, g0[r].im);
                 v[r].re = make_float2((bits & 1) ? v[r].re.x : ore.x, (bits & 2) ? v[r].re.y : ore.y);
                 v[r].im = make_float2((bits & 1) ? v[r].im.x : oim.x, (bits & 2) ? v[r].im.y : oim.y);
-                st_s(q + M0 * r, j, v[r]);
+                st_quad(tile + i0(r), v[r]);
             }
             // no barrier: the quads written here are read back by this same thread (the mix of B(i))
         };
@@ -151,13 +168,11 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
             const int m = proj(i), s0 = i % 3;
             float4* const t0 = sm + s0 * tile_quads<N>();
             float4* __restrict__ gout = gh_new + (size_t)m * istride + (size_t)rt * tile_quads<N>();
-            auto ld_s = [&](int p, int jj) -> c2 { return from_quad(t0[tq(p, jj)]); };
-            auto st_s = [&](int p, int jj, c2 w) { st_quad(t0 + tq(p, jj), w); };
             {
                 c2 w[R0];
 #pragma unroll
                 for (int r = 0; r < R0; ++r) {
-                    const int i2 = tq(q + M0 * r, j);
+                    const int i2 = i0(r);
                     const c2 own = from_quad(t0[i2]);
                     w[r] = c2{pfma(a0, own.re, pmul(a1, padd(gm[r].re, v[r].re))), pfma(a0, own.im, pmul(a1, padd(gm[r].im, v[r].im)))};
                     gm[r] = own;
@@ -166,15 +181,23 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
                 dft<R0, false>(w);
                 twiddle<R0, false>(w, tw0, q);
 #pragma unroll
-                for (int r = 0; r < R0; ++r) st_s(q + M0 * r, j, w[r]);
+                for (int r = 0; r < R0; ++r) st_quad(t0 + i0(r), w[r]);
             }
             __syncthreads();
-            fft_stage<N, R1, N / R0, false, NT, 1>(tw1, ld_s, st_s);
+            {
+                c2 w[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) w[r] = from_quad(t0[i1(r)]);
+                dft<R1, false>(w);
+                twiddle<R1, false>(w, tw1, q % 8);
+#pragma unroll
+                for (int r = 0; r < R1; ++r) st_quad(t0 + i1(r), w[r]);
+            }
             __syncwarp();
             {
                 c2 w[RL];
 #pragma unroll
-                for (int r = 0; r < RL; ++r) w[r] = ld_s(q * RL + r, j);
+                for (int r = 0; r < RL; ++r) w[r] = from_quad(t0[iL(r)]);
                 dft<RL, false>(w);
                 __syncwarp();
                 store_transposed<N>(t0, w, q, j, rt);
