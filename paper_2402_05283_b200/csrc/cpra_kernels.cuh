@@ -133,6 +133,76 @@ template <int N> __device__ __forceinline__ void inner_sync()
     if constexpr (inner_stages_warp_local<N>()) __syncwarp(); else __syncthreads();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Stages of the 8-wide plans with inner radices 8 x 8 (N = 512, 1024) with the quad offsets of a
+// butterfly written as ONE base (two where the positions cross 8-blocks of alternating parity, see
+// ppos) plus compile-time multiples of r, instead of position arithmetic per access:
+//   stage 0 (stride M0 = 64): p = n2 + M0 r            ppos(p) = ppos(n2) + M0 r,  slot key (p >> 1) & 3 = (n2 >> 1) & 3
+//   stage 1 (stride 8):       p = 64 b + n2 + 8 r      ppos(p) = p ^ (r & 1),      slot key (n2 >> 1) & 3
+//   last    (contiguous):     p = 8 q + r              ppos(p) = 8 q + (r ^ (q & 1)), slot key (r >> 1) & 3
+// SWZ = the scratch layout (slot = pair ^ key); otherwise the state layout (slot = pair).
+// ------------------------------------------------------------------------------------------------
+template <int N, bool INV, bool SWZ, int NT>
+__device__ __forceinline__ void stage0_8(float4* __restrict__ tile, const float2* __restrict__ tw0)
+{
+    constexpr int R = Radix<N>::R0, M0 = N / R, NP = 4, NBF = NP * M0, ITERS = (NBF + NT - 1) / NT;
+    static_assert(M0 == 64, "stage 0 of the 8-wide plans has stride 64");
+#pragma unroll 1
+    for (int it = 0; it < ITERS; ++it) {
+        const int bf = (int)threadIdx.x + it * NT;
+        if ((NBF % NT) != 0 && bf >= NBF) break;
+        const int j = bf % NP, n2 = bf / NP;
+        float4* __restrict__ b = tile + ppos(n2, 8) * NP + (SWZ ? (j ^ ((n2 >> 1) & 3)) : j);
+        c2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = from_quad(b[r * (M0 * NP)]);
+        if constexpr (INV) twiddle<R, true>(v, tw0, n2);
+        dft<R, INV>(v);
+        if constexpr (!INV) twiddle<R, false>(v, tw0, n2);
+#pragma unroll
+        for (int r = 0; r < R; ++r) st_quad(b + r * (M0 * NP), v[r]);
+    }
+}
+template <int N, bool INV, bool SWZ, int NT>
+__device__ __forceinline__ void stage1_8(float4* __restrict__ tile, const float2* __restrict__ tw1)
+{
+    constexpr int R = 8, NP = 4, NBF = NP * (N / R), ITERS = (NBF + NT - 1) / NT;
+#pragma unroll 1
+    for (int it = 0; it < ITERS; ++it) {
+        const int bf = (int)threadIdx.x + it * NT;
+        if ((NBF % NT) != 0 && bf >= NBF) break;
+        const int j = bf % NP, q = bf / NP, blk = q / 8, n2 = q % 8;
+        const int slot = SWZ ? (j ^ ((n2 >> 1) & 3)) : j;
+        float4* __restrict__ be = tile + (blk * 64 + n2) * NP + slot;
+        float4* __restrict__ bo = tile + (blk * 64 + (n2 ^ 1)) * NP + slot;
+        c2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = from_quad(((r & 1) ? bo : be)[r * (8 * NP)]);
+        if constexpr (INV) twiddle<R, true>(v, tw1, n2);
+        dft<R, INV>(v);
+        if constexpr (!INV) twiddle<R, false>(v, tw1, n2);
+#pragma unroll
+        for (int r = 0; r < R; ++r) st_quad(((r & 1) ? bo : be) + r * (8 * NP), v[r]);
+    }
+}
+// quad of element r of the contiguous butterfly q, pair j
+template <bool SWZ>
+struct Last8 {
+    float4* pe;
+    float4* po;
+    int j;
+    __device__ __forceinline__ Last8(float4* tile, int q, int j_) : j(j_)
+    {
+        const int s = q & 1;
+        pe = tile + (8 * q + s) * 4;
+        po = tile + (8 * q + 1 - s) * 4;
+    }
+    __device__ __forceinline__ float4* operator()(int r) const
+    {
+        return ((r & 1) ? po : pe) + (r & ~1) * 4 + (SWZ ? (j ^ (r >> 1)) : j);
+    }
+};
+
 // shared-memory carve-up of the three kernels
 template <int N>
 struct Smem {
@@ -373,11 +443,14 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[ppos<N>(p) * NP + sw(j, p, NP)]); };
     auto st_s = [&](int p, int j, c2 v) { st_quad(tile + ppos<N>(p) * NP + sw(j, p, NP), v); };
 
+    constexpr bool FAST = inner_stages_warp_local<N>();   // 8-wide, inner radices 8 x 8: affine offsets
     if constexpr (MODE == COL_FULL || MODE == COL_FWD) {
-        fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_s, st_s);
+        if constexpr (FAST) stage0_8<N, false, true, NT>(tile, s.tw0);
+        else fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_s, st_s);
         __syncthreads();
         if constexpr (RX::S == 3) {
-            fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);
+            if constexpr (FAST) stage1_8<N, false, true, NT>(tile, s.tw1);
+            else fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);
             inner_sync<N>();
         }
     }
@@ -399,7 +472,24 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
 #pragma unroll
             for (int r = 0; r < RL; ++r) modulus_pair(v[r], a[r], scale, acc2);
         };
-        fft_stage_mid<N, RL, NT, 1>(ld_s, pw, st_s);
+        if constexpr (FAST) {
+            constexpr int NBF = NP * (N / RL), ITERS = (NBF + NT - 1) / NT;
+#pragma unroll 1
+            for (int it = 0; it < ITERS; ++it) {
+                const int bf = (int)threadIdx.x + it * NT, j = bf % NP, q = bf / NP;
+                const Last8<true> at(tile, q, j);
+                c2 v[RL];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) v[r] = from_quad(*at(r));
+                dft<RL, false>(v);
+                pw(v, q, j);
+                dft<RL, true>(v);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) st_quad(at(r), v[r]);
+            }
+        } else {
+            fft_stage_mid<N, RL, NT, 1>(ld_s, pw, st_s);
+        }
         float acc = acc2.x + acc2.y;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -409,7 +499,8 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
     if constexpr (MODE != COL_FWD) {
         if constexpr (RX::S == 3) {
             inner_sync<N>();
-            fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(s.tw1, ld_s, st_s);
+            if constexpr (FAST) stage1_8<N, true, true, NT>(tile, s.tw1);
+            else fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(s.tw1, ld_s, st_s);
         }
         __syncthreads();
         if constexpr (MODE == COL_FULL) {
@@ -419,7 +510,8 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
                 partial[(size_t)n * NCT + ct] = t;
             }
         }
-        fft_stage<N, RX::R0, N, true, NT, 1>(s.tw0, ld_s, st_s);
+        if constexpr (FAST) stage0_8<N, true, true, NT>(tile, s.tw0);
+        else fft_stage<N, RX::R0, N, true, NT, 1>(s.tw0, ld_s, st_s);
     }
     fence_async_smem();
     __syncthreads();
