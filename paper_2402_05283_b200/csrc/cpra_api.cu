@@ -10,6 +10,8 @@
 
 #include "../../include/cpra.h"
 #include "cpra_layout.cuh"
+#include <cuda.h>
+
 #include "cpra_image.cuh"
 #include "cpra_walk.cuh"
 
@@ -29,6 +31,8 @@ struct cpra_plan_s {
     float4* st[2] = {nullptr, nullptr};
     float4* scr = nullptr;
     float4* scr2 = nullptr;   // second spectrum buffer: k_row_walk reads one and writes the other
+    CUtensorMap tm_scr[2];    // TMA descriptors of scr and scr2 for k_row_walk
+    bool have_tmap = false;
     double* partial = nullptr;
     double* den = nullptr;
     double* uphi = nullptr;
@@ -273,6 +277,29 @@ int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int
     return check_launch(p);
 }
 
+// TMA descriptor of a spectrum buffer as the contiguous tensor [n][ct][rt][TB*TB*2 floats], box = all
+// column tiles of one row tile.  cuTensorMapEncodeTiled is fetched through the runtime, so that the
+// library does not link against the driver.
+bool encode_scratch_tmap(CUtensorMap* tm, void* base, int N, int Np, int tb)
+{
+    typedef CUresult (*Encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t blk = (cuuint64_t)tb * tb * 2, nt = (cuuint64_t)(N / tb);
+    const cuuint64_t dims[4] = {blk, nt, nt, (cuuint64_t)Np};
+    const cuuint64_t strides[3] = {blk * 4, blk * 4 * nt, blk * 4 * nt * nt};
+    const cuuint32_t box[4] = {(cuuint32_t)blk, 1u, (cuuint32_t)nt, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    return ((Encode)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // K3 of one iteration fused with K1 of the next (cpra_walk.cuh): 2 CTAs per SM, each a run of tiles
 template <int N>
 int launch_walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta)
@@ -284,7 +311,9 @@ int launch_walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const flo
         const dim3 grid((unsigned)((total + per - 1) / per));
         const MixParams mp = mix_params(p);
         ProfScope prof(p, CPRA_PROFILE_WALK);
-        k_row_walk<N><<<grid, walk_threads<N>(), walk_smem_bytes<N>(), p->stream>>>(scr_in, scr_out, gh_old, gh_new, p->tw, p->S16, mp, beta, p->Np, per);
+        const CUtensorMap& tin = p->tm_scr[scr_in == p->scr ? 0 : 1];
+        const CUtensorMap& tout = p->tm_scr[scr_out == p->scr ? 0 : 1];
+        k_row_walk<N><<<grid, walk_threads<N>(), walk_smem_bytes<N>(), p->stream>>>(tin, tout, gh_old, gh_new, p->tw, p->S16, mp, beta, p->Np, per);
         return check_launch(p);
     } else {
         return CPRA_ERR_UNSUPPORTED_SIZE;
@@ -458,6 +487,10 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
         if (rc != CPRA_OK) { p->ws = nullptr; return rc; }
         p->attrs_set = true;
     }
+    p->have_tmap = false;
+    { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, if constexpr (walk_ok<NN>()) p->have_tmap =
+          encode_scratch_tmap(&p->tm_scr[0], p->scr, p->N, p->Np, tile_batch<NN>()) &&
+          encode_scratch_tmap(&p->tm_scr[1], p->scr2, p->N, p->Np, tile_batch<NN>())); return 0; }; f(); }
     if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float2) * p->h_tw.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
         p->ws = nullptr;
         return CPRA_ERR_CUDA;
@@ -541,7 +574,7 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
     // the walking kernel serves the default carousel (K = 1 every iteration) on plans with 8-row tiles
-    if (k > 0 && p->walk && chunk == p->Np && p->K == 1 && p->n_ei == 1 && p->Np >= 3) {
+    if (k > 0 && p->walk && p->have_tmap && chunk == p->Np && p->K == 1 && p->n_ei == 1 && p->Np >= 3) {
         int rc = CPRA_ERR_UNSUPPORTED_SIZE;
         { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, if constexpr (walk_ok<NN>()) rc = iterate_walk<NN>(p, k, beta, scale)); return 0; }; f(); }
         if (rc != CPRA_ERR_UNSUPPORTED_SIZE) return rc;

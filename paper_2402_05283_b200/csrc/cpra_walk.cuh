@@ -21,6 +21,7 @@
 // (halo) are inverse-transformed twice (by this CTA and by their owner): the spectra are therefore
 // read from one scratch buffer and written to the other.
 #pragma once
+#include <cuda.h>   // CUtensorMap (type only; the encoder is fetched through the runtime, see cpra_api.cu)
 #include "cpra_kernels.cuh"
 
 namespace cpra {
@@ -34,9 +35,24 @@ template <int N> __host__ __device__ constexpr int walk_smem_bytes()
 }
 template <int N> __host__ __device__ constexpr int walk_threads() { return tile_pairs<N>() * (N / last_radix<N>()); }
 
+// One TMA tensor instruction moves the N/8 blocks (512 B each, one per column tile) of a row tile
+// between shared memory and the spectrum buffer, described as the contiguous 4D tensor
+// [n][ct][rt][128 floats] with box {128, 1, N/8, 1}.  (One bulk copy per block would have to be issued
+// lane by lane: the copy instructions take their addresses from uniform registers.)
+__device__ __forceinline__ void tma_load_tile(void* smem_dst, const CUtensorMap* tm, int rt, int n, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(0), "r"(rt), "r"(0), "r"(n), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_tile(const CUtensorMap* tm, int rt, int n, const void* smem_src)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+                 ::"l"(tm), "r"(0), "r"(rt), "r"(0), "r"(n), "r"(smem_u32(smem_src)) : "memory");
+}
+
 template <int N>
 __global__ void __launch_bounds__(walk_threads<N>(), 2)
-k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, const float4* __restrict__ gh_old,
+k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out, const float4* __restrict__ gh_old,
            float4* __restrict__ gh_new, const float2* __restrict__ twg, const uint16_t* __restrict__ S16,
            MixParams mp, float beta, int Np, int per_cta)
 {
@@ -56,8 +72,7 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
     const int u0 = (int)blockIdx.x * per_cta, u1 = min(total, u0 + per_cta);
     if (u0 >= u1) return;
     const int j = threadIdx.x % NP, q = threadIdx.x / NP;   // this thread's butterfly in every stage
-    constexpr int IO = NCT < NT ? NCT : NT;   // threads that issue the bulk copies
-    const bool io = threadIdx.x < IO;
+    const bool io = threadIdx.x == 0;   // the thread that issues the copies
 
     if (threadIdx.x == 0) {
         for (int b = 0; b < 4; ++b) mbar_init(full + b, 1);
@@ -82,17 +97,11 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
     static_assert(R0 == 8 && N / R0 == 64, "offsets above assume an 8 x 8 x 8 plan");
     const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]), nbeta = bc(-beta);
 
-    // issue the bulk loads of projection m's spectrum tile (row tile rt) and support words into slot s
-    // (called by the threads io: one 512-byte block each, so that no warp spends a pass issuing copies)
+    // issue the loads of projection m's spectrum tile (row tile rt) and support words into slot s
     auto load_tile = [&](int m, int rt, int s) {
-        if (threadIdx.x == 0) {
-            mbar_expect_tx(full + s, tile_bytes<N>() + 2 * N);
-            bulk_load(sup + s * N, S16 + ((size_t)m * (N / 16) + (rt * TBN) / 16) * N, 2 * N, full + s);
-        }
-        const float4* __restrict__ src = scr_in + (size_t)m * istride + (size_t)rt * TBN * NP;
-        float4* dst = slots + s * tile_quads<N>();
-        for (int ct = threadIdx.x; ct < NCT; ct += IO)
-            bulk_load(dst + ct * TBN * NP, src + (size_t)ct * tile_quads<N>(), TBN * NP * 16, full + s);
+        mbar_expect_tx(full + s, tile_bytes<N>() + 2 * N);
+        tma_load_tile(slots + s * tile_quads<N>(), &tm_in, rt, m, full + s);
+        bulk_load(sup + s * N, S16 + ((size_t)m * (N / 16) + (rt * TBN) / 16) * N, 2 * N, full + s);
     };
 
     mbar_wait(full + 3, 0);
@@ -205,9 +214,7 @@ k_row_walk(const float4* __restrict__ scr_in, float4* __restrict__ scr_out, cons
             fence_async_smem();
             __syncthreads();
             if (io) {
-                float4* __restrict__ dst = scr_out + (size_t)m * istride + (size_t)rt * TBN * NP;
-                for (int ct = threadIdx.x; ct < NCT; ct += IO)
-                    bulk_store(dst + (size_t)ct * tile_quads<N>(), t0 + ct * TBN * NP, TBN * NP * 16);
+                tma_store_tile(&tm_out, rt, m, t0);
                 bulk_commit();
             }
             pend_tile = (i + 3 <= len + 1) ? i + 3 : -1;
