@@ -231,7 +231,7 @@ int launch_row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg
     const int smem = smem_bytes<N>();
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_FWD);
-#define ROWFWD(M) k_row_fwd<N, M><<<grid, NT, smem, p->stream>>>(cur, p->scr, p->tw, p->S16, mp, p->Np, n0, nimg, ghat_out)
+#define ROWFWD(M) k_row_fwd<N, M><<<grid, NT, smem, p->stream>>>(cur, p->tm_scr[0], p->tw, p->S16, mp, p->Np, n0, nimg, ghat_out)
     switch (mode) {
         case MIX_NONE: ROWFWD(MIX_NONE); break;
         case MIX_K1: ROWFWD(MIX_K1); break;
@@ -268,7 +268,7 @@ int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int
     const MixParams mp = mix_params(p);
     ProfScope prof(p, CPRA_PROFILE_ROW_INV);
     if (!scr) scr = p->scr;
-#define ROWINV(H, M) k_row_inv<N, H, M><<<grid, NT, smem, p->stream>>>(scr, cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg, ghat_in)
+#define ROWINV(H, M) k_row_inv<N, H, M><<<grid, NT, smem, p->stream>>>(p->tm_scr[scr == p->scr ? 0 : 1], cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg, ghat_in)
     if (!hio) ROWINV(ROWINV_PLAIN, MIX_NONE);
     else if (mode == MIX_NONE) ROWINV(ROWINV_HIO, MIX_NONE);
     else if (mode == MIX_K1) ROWINV(ROWINV_HIO, MIX_K1);
@@ -277,8 +277,8 @@ int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int
     return check_launch(p);
 }
 
-// TMA descriptor of a spectrum buffer as the contiguous tensor [n][ct][rt][TB*TB*2 floats], box = all
-// column tiles of one row tile.  cuTensorMapEncodeTiled is fetched through the runtime, so that the
+// TMA descriptor of a spectrum buffer as the contiguous tensor [n][ct][rt][split][inner floats], box =
+// all column tiles of one row tile (see tma_load_tile).  cuTensorMapEncodeTiled is fetched through the runtime, so that the
 // library does not link against the driver.
 bool encode_scratch_tmap(CUtensorMap* tm, void* base, int N, int Np, int tb)
 {
@@ -291,12 +291,13 @@ bool encode_scratch_tmap(CUtensorMap* tm, void* base, int N, int Np, int tb)
         (void)cudaGetLastError();
         return false;
     }
-    const cuuint64_t blk = (cuuint64_t)tb * tb * 2, nt = (cuuint64_t)(N / tb);
-    const cuuint64_t dims[4] = {blk, nt, nt, (cuuint64_t)Np};
-    const cuuint64_t strides[3] = {blk * 4, blk * 4 * nt, blk * 4 * nt * nt};
-    const cuuint32_t box[4] = {(cuuint32_t)blk, 1u, (cuuint32_t)nt, 1u};
-    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
-    return ((Encode)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    const cuuint64_t blk = (cuuint64_t)tb * tb * 2, nt = (cuuint64_t)(N / tb);   // floats per block, tiles per side
+    const cuuint64_t inner = blk < 256 ? blk : 256, split = blk / inner;          // box dimensions are limited to 256
+    const cuuint64_t dims[5] = {inner, split, nt, nt, (cuuint64_t)Np};
+    const cuuint64_t strides[4] = {inner * 4, blk * 4, blk * 4 * nt, blk * 4 * nt * nt};
+    const cuuint32_t box[5] = {(cuuint32_t)inner, (cuuint32_t)split, 1u, (cuuint32_t)nt, 1u};
+    const cuuint32_t estr[5] = {1u, 1u, 1u, 1u, 1u};
+    return ((Encode)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -488,9 +489,9 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
         p->attrs_set = true;
     }
     p->have_tmap = false;
-    { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, if constexpr (walk_ok<NN>()) p->have_tmap =
-          encode_scratch_tmap(&p->tm_scr[0], p->scr, p->N, p->Np, tile_batch<NN>()) &&
-          encode_scratch_tmap(&p->tm_scr[1], p->scr2, p->N, p->Np, tile_batch<NN>())); return 0; }; f(); }
+    p->have_tmap = encode_scratch_tmap(&p->tm_scr[0], p->scr, p->N, p->Np, p->geo.TB) &&
+                   encode_scratch_tmap(&p->tm_scr[1], p->scr2, p->N, p->Np, p->geo.TB);
+    if (!p->have_tmap) { p->ws = nullptr; return CPRA_ERR_CUDA; }   // the row kernels move their tiles by TMA tensor copies
     if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float2) * p->h_tw.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
         p->ws = nullptr;
         return CPRA_ERR_CUDA;

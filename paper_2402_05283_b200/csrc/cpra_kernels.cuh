@@ -14,6 +14,8 @@
 //                                 thread needs in the fused middle stage are contiguous
 //   support   [n][rt][x] u16      bit b = S(y = 16 rt + b, x)       (1 bit per pixel)
 #pragma once
+#include <cuda.h>   // CUtensorMap (type only; the encoder is fetched through the runtime, see cpra_api.cu)
+
 #include "cpra_fft.cuh"
 
 namespace cpra {
@@ -120,6 +122,22 @@ struct MixLoader {
         }
     }
 };
+
+// One TMA tensor instruction moves the N/TB blocks (TB x TB complex each, one per column tile) of a
+// row tile between shared memory and a spectrum buffer, described as the contiguous 5D tensor
+// [n][ct][rt][split][inner floats] (a block = split x inner floats, inner <= 256) with the box
+// {inner, split, 1, N/TB, 1}.  (One bulk copy per block would have to be issued lane by lane: the
+// copy instructions take their addresses from uniform registers.)
+__device__ __forceinline__ void tma_load_tile(void* smem_dst, const CUtensorMap* tm, int rt, int n, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(0), "r"(0), "r"(rt), "r"(0), "r"(n), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_tile(const CUtensorMap* tm, int rt, int n, const void* smem_src)
+{
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4, %5}], [%6];"
+                 ::"l"(tm), "r"(0), "r"(0), "r"(rt), "r"(0), "r"(n), "r"(smem_u32(smem_src)) : "memory");
+}
 
 // Barrier between the two inner stages of a 3-stage plan.  With 4 pairs per position and radices
 // R1 = RL = 8, butterfly bf of either stage works inside the 64-position block bf / 32, i.e. every
@@ -264,7 +282,7 @@ __device__ __forceinline__ void load_transposed(const float4* __restrict__ tile,
 // ------------------------------------------------------------------------------------------------
 template <int N, int MODE>
 __global__ void __launch_bounds__(Radix<N>::NT, (Radix<N>::PF && (MODE == MIX_K1 || MODE == MIX_GEN)) ? Radix<N>::MINBF : Radix<N>::MINB)
-k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2* __restrict__ twg,
+k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm_scr, const float2* __restrict__ twg,
           const uint16_t* __restrict__ S16, MixParams mp, int Np, int n0, int nimg, float4* __restrict__ ghat_out)
 {
     // ghat_out != nullptr: the mixed input ghat_n is also stored (state layout) for the HIO update of
@@ -365,11 +383,12 @@ k_row_fwd(const float4* __restrict__ cur, float4* __restrict__ scr, const float2
     }
     fence_async_smem();
     __syncthreads();
-    // block ct of the tile -> rows [TBN rt, TBN rt + TBN) of scratch tile (n, ct): TBN x TBN x 8 bytes each
-    float4* __restrict__ dst = scr + (size_t)n * istride + (size_t)rt * TBN * NP;
-    for (int ct = threadIdx.x; ct < NCT; ct += NT)
-        bulk_store(dst + (size_t)ct * tile_quads<N>(), tile + ct * TBN * NP, TBN * NP * 16);
-    if (threadIdx.x < NCT) { bulk_commit(); bulk_wait_read0(); }
+    // block ct of the tile -> rows [TBN rt, TBN rt + TBN) of scratch tile (n, ct), all ct in one instruction
+    if (threadIdx.x == 0) {
+        tma_store_tile(&tm_scr, rt, n, tile);
+        bulk_commit();
+        bulk_wait_read0();
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -531,7 +550,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
 // ------------------------------------------------------------------------------------------------
 template <int N, int MODE, int MIXMODE>
 __global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
-k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4* __restrict__ nxt,
+k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__ cur, float4* __restrict__ nxt,
           const float2* __restrict__ twg, const uint16_t* __restrict__ S16, MixParams mp, float beta,
           float scale, int Np, int n0, int nimg, const float4* __restrict__ ghat_in)
 {
@@ -553,13 +572,7 @@ k_row_inv(const float4* __restrict__ scr, const float4* __restrict__ cur, float4
         mbar_expect_tx(s.bar, tile_bytes<N>() + tw_bytes<N>() + (MODE == ROWINV_HIO ? 2 * N : 0));
         bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
         if constexpr (MODE == ROWINV_HIO) bulk_load(s.sup, S16 + ((size_t)n * (N / 16) + (rt * TBN) / 16) * N, 2 * N, s.bar);
-    }
-    __syncwarp();
-    {
-        const float4* __restrict__ src = scr + (size_t)n * istride + (size_t)rt * TBN * NP;
-        if (threadIdx.x < 32)
-            for (int ct = threadIdx.x; ct < NCT; ct += 32)
-                bulk_load(tile + ct * TBN * NP, src + (size_t)ct * tile_quads<N>(), TBN * NP * 16, s.bar);
+        tma_load_tile(tile, &tm_scr, rt, n, s.bar);
     }
     mbar_wait(s.bar, 0);
 

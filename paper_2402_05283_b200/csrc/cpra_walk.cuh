@@ -21,7 +21,6 @@
 // (halo) are inverse-transformed twice (by this CTA and by their owner): the spectra are therefore
 // read from one scratch buffer and written to the other.
 #pragma once
-#include <cuda.h>   // CUtensorMap (type only; the encoder is fetched through the runtime, see cpra_api.cu)
 #include "cpra_kernels.cuh"
 
 namespace cpra {
@@ -34,21 +33,6 @@ template <int N> __host__ __device__ constexpr int walk_smem_bytes()
     return WALK_SLOTS * tile_bytes<N>() + tw_bytes<N>() + 32 + WALK_SLOTS * 2 * N;
 }
 template <int N> __host__ __device__ constexpr int walk_threads() { return tile_pairs<N>() * (N / last_radix<N>()); }
-
-// One TMA tensor instruction moves the N/8 blocks (512 B each, one per column tile) of a row tile
-// between shared memory and the spectrum buffer, described as the contiguous 4D tensor
-// [n][ct][rt][128 floats] with box {128, 1, N/8, 1}.  (One bulk copy per block would have to be issued
-// lane by lane: the copy instructions take their addresses from uniform registers.)
-__device__ __forceinline__ void tma_load_tile(void* smem_dst, const CUtensorMap* tm, int rt, int n, uint64_t* bar)
-{
-    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(0), "r"(rt), "r"(0), "r"(n), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tma_store_tile(const CUtensorMap* tm, int rt, int n, const void* smem_src)
-{
-    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
-                 ::"l"(tm), "r"(0), "r"(rt), "r"(0), "r"(n), "r"(smem_u32(smem_src)) : "memory");
-}
 
 template <int N>
 __global__ void __launch_bounds__(walk_threads<N>(), 2)
