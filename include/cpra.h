@@ -134,6 +134,20 @@ int cpra_set_iteration(cpra_plan_t plan, long t);
 int cpra_iterate(cpra_plan_t plan, int k, float beta);
 
 /*
+ * Real-space update rule of step 6 (default CPRA_UPDATE_HIO).  The paper's reconstructions use HIO
+ * (P:98 ref [22]) and RAAR with beta = 0.9 (P:98 ref [38]); all keep g' inside the support and
+ * differ outside it (reading A22):
+ *   CPRA_UPDATE_HIO   S_n = 0:  g_n <- ghat_n - beta g'_n
+ *   CPRA_UPDATE_RAAR  S_n = 0:  g_n <- beta ghat_n + (1 - 2 beta) g'_n
+ *   CPRA_UPDATE_ER    S_n = 0:  g_n <- 0                  (error reduction; beta unused)
+ * Takes effect from the next cpra_iterate call.  Errors: INVALID_ARG.
+ */
+#define CPRA_UPDATE_HIO 0
+#define CPRA_UPDATE_RAAR 1
+#define CPRA_UPDATE_ER 2
+int cpra_set_update(cpra_plan_t plan, int rule);
+
+/*
  * Reconstruction error of the LAST iteration run (evaluated on its input, before the modulus
  * step; A9): d_E [Np] fp32, E_n = sqrt(num_n / den_n) (0 where den_n = 0); d_Eglobal [1] fp32,
  * sqrt(sum_n num_n / sum_n den_n).  Either pointer may be NULL.  Device-side reduction, fixed

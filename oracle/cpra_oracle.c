@@ -212,6 +212,32 @@ static void hio_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t
     }
 }
 
+/* The other real-space updates the paper uses or names (reading A22 of DESIGN.md), same support
+ * constraint, no positivity:
+ *   RAAR (ref [38], beta P:104):  x <- (beta/2)(R_S R_M + I) x + (1 - beta) P_M x,  R = 2P - I,
+ *        P_M x = g', P_S = multiplication by S.  Written out:  S=1: g';  S=0: beta ghat + (1 - 2 beta) g'.
+ *   ER (error reduction, the plain alternating projection P_S P_M):  S=1: g';  S=0: 0. */
+#define ORACLE_UPDATE_HIO 0
+#define ORACLE_UPDATE_RAAR 1
+#define ORACLE_UPDATE_ER 2
+static void raar_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px, real beta)
+{
+    for (size_t i = 0; i < px; ++i) {
+        if (S[i]) { ghat[i] = gp[i]; }
+        else {
+            ghat[i].re = beta * ghat[i].re + ((real)1 - (real)2 * beta) * gp[i].re;
+            ghat[i].im = beta * ghat[i].im + ((real)1 - (real)2 * beta) * gp[i].im;
+        }
+    }
+}
+static void er_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px)
+{
+    for (size_t i = 0; i < px; ++i) {
+        if (S[i]) { ghat[i] = gp[i]; }
+        else { ghat[i].re = 0; ghat[i].im = 0; }
+    }
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* Plan / state                                                                                */
 /* ------------------------------------------------------------------------------------------ */
@@ -226,6 +252,7 @@ typedef struct oracle_plan_s {
     cplx* g;              /* state */
     cplx* tmp;            /* mixed copy ghat */
     int K; real alpha[64]; int n_ei;
+    int update;   /* ORACLE_UPDATE_*; HIO by default */
     long t;
     double* E; double Eglobal;
     int have_data, have_support, have_estimate, have_error;
@@ -305,6 +332,14 @@ int oracle_set_carousel(oracle_plan_t p, int K, const double* alpha, int n_ei)
     return ORACLE_OK;
 }
 
+/* real-space update rule of step 6: ORACLE_UPDATE_HIO (default), _RAAR, _ER */
+int oracle_set_update(oracle_plan_t p, int rule)
+{
+    if (!p || rule < 0 || rule > 2) return ORACLE_ERR_INVALID_ARG;
+    p->update = rule;
+    return ORACLE_OK;
+}
+
 /* g0: interleaved complex double [Np][N][N]; resets t = 0. */
 int oracle_set_estimate(oracle_plan_t p, const double* g0)
 {
@@ -341,7 +376,9 @@ int oracle_iterate(oracle_plan_t p, int k, double beta_d)
             fft2d(G, N, -1);                                                     /* 2 */
             const double num = modulus_image(G, p->A + (size_t)n * px, p->M + (size_t)n * px, px); /* 3, 4 */
             fft2d(G, N, +1);                                                     /* 5 */
-            hio_image(ghat, G, p->S + (size_t)n * px, px, beta);                 /* 6 */
+            if (p->update == ORACLE_UPDATE_RAAR) raar_image(ghat, G, p->S + (size_t)n * px, px, beta);
+            else if (p->update == ORACLE_UPDATE_ER) er_image(ghat, G, p->S + (size_t)n * px, px);
+            else hio_image(ghat, G, p->S + (size_t)n * px, px, beta);            /* 6 */
             free(G);
             p->E[n] = p->den[n] > 0.0 ? sqrt(num / p->den[n]) : 0.0;
             numtot += num; dentot += p->den[n];

@@ -39,6 +39,7 @@ def _lib(precision: str = "f64"):
         lib.oracle_set_data.argtypes = [vp, vp, vp, vp]
         lib.oracle_set_support.argtypes = [vp, vp]
         lib.oracle_set_carousel.argtypes = [vp, ci, vp, ci]
+        lib.oracle_set_update.argtypes = [vp, ci]
         lib.oracle_set_estimate.argtypes = [vp, vp]
         lib.oracle_set_iteration.argtypes = [vp, ctypes.c_long]
         lib.oracle_get_iteration.argtypes = [vp]
@@ -159,6 +160,11 @@ class Oracle:
     @property
     def iteration(self):
         return int(self._l.oracle_get_iteration(self._h))
+
+    def set_update(self, rule):
+        """Real-space update of step 6: "hio" (default), "raar" or "er" (reading A22)."""
+        _chk(self._l.oracle_set_update(self._h, {"hio": 0, "raar": 1, "er": 2}[rule]), "oracle_set_update")
+        return self
 
     def iterate(self, k, beta=0.9):
         _chk(self._l.oracle_iterate(self._h, int(k), float(beta)), "oracle_iterate")

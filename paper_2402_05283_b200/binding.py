@@ -41,6 +41,7 @@ SIGNATURES = {
     "cpra_host_staging_bytes": (_ci, [_vp, ctypes.POINTER(_sz)]),
     "cpra_reconstruct_host": (_ci, [_vp, _vp, _sz, _vp, _vp, _vp, _vp, _vp, _ci, _cf, _vp, _vp, _vp]),
     "cpra_set_chunk": (_ci, [_vp, _ci]),
+    "cpra_set_update": (_ci, [_vp, _ci]),
     "cpra_profile": (_ci, [_vp, _ci]),
     "cpra_profile_read": (_ci, [_vp, _vp, _vp]),
     "cpra_launch_count": (_ci, [_vp, ctypes.POINTER(_cl)]),
@@ -206,6 +207,11 @@ class Plan:
         out = torch.empty_like(stack)
         _chk(self._l.cpra_fft2(self._h, _dptr(stack, torch.complex64, self._px), out.data_ptr(), int(sign)), "cpra_fft2")
         return out
+
+    def set_update(self, rule: str):
+        """Real-space update rule: "hio" (default), "raar" or "er"."""
+        _chk(self._l.cpra_set_update(self._h, {"hio": 0, "raar": 1, "er": 2}[rule]), "cpra_set_update")
+        return self
 
     def profile(self, enable: bool):
         _chk(self._l.cpra_profile(self._h, int(bool(enable))), "cpra_profile")

@@ -43,6 +43,7 @@ struct cpra_plan_s {
     int K = 1;
     float alpha[MAXK + 1] = {0};
     int n_ei = 1;
+    int update = CPRA_UPDATE_HIO;
     long t = 0;
     bool have_data = false, have_support = false, have_estimate = false, have_error = false;
     bool attrs_set = false;
@@ -165,11 +166,15 @@ int set_attrs()
     return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
 }
 
-MixParams mix_params(const cpra_plan_s* p)
+MixParams mix_params(const cpra_plan_s* p, float beta = 0.f)
 {
     MixParams mp;
     mp.K = p->K;
     for (int j = 0; j <= MAXK; ++j) mp.a[j] = j <= p->K ? p->alpha[j] : 0.f;
+    // coefficients of the update outside the support (cpra_set_update)
+    if (p->update == CPRA_UPDATE_RAAR) { mp.c_ghat = beta; mp.c_gp = 1.0f - 2.0f * beta; }
+    else if (p->update == CPRA_UPDATE_ER) { mp.c_ghat = 0.f; mp.c_gp = 0.f; }
+    else { mp.c_ghat = 1.0f; mp.c_gp = -beta; }
     return mp;
 }
 
@@ -265,7 +270,7 @@ int launch_row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int
     constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
     const int smem = smem_bytes<N>();
-    const MixParams mp = mix_params(p);
+    const MixParams mp = mix_params(p, beta);
     ProfScope prof(p, CPRA_PROFILE_ROW_INV);
     if (!scr) scr = p->scr;
 #define ROWINV(H, M) k_row_inv<N, H, M><<<grid, NT, smem, p->stream>>>(p->tm_scr[scr == p->scr ? 0 : 1], cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg, ghat_in)
@@ -310,7 +315,7 @@ int launch_walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const flo
         const int ctas = std::min(total, 2 * p->sms);
         const int per = (total + ctas - 1) / ctas;
         const dim3 grid((unsigned)((total + per - 1) / per));
-        const MixParams mp = mix_params(p);
+        const MixParams mp = mix_params(p, beta);
         ProfScope prof(p, CPRA_PROFILE_WALK);
         const CUtensorMap& tin = p->tm_scr[scr_in == p->scr ? 0 : 1];
         const CUtensorMap& tout = p->tm_scr[scr_out == p->scr ? 0 : 1];
@@ -354,7 +359,7 @@ int launch_image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float
     if constexpr (N <= 128) {
         constexpr int NT = image_threads<N>(), ISM = image_smem_bytes<N>();
         const dim3 grid((unsigned)p->Np);
-        const MixParams mp = mix_params(p);
+        const MixParams mp = mix_params(p, beta);
         ProfScope prof(p, CPRA_PROFILE_IMAGE);
 #define IMG(M) k_image<N, M><<<grid, NT, ISM, p->stream>>>(cur, nxt, p->A, p->tw, p->S16, p->partial, mp, beta, scale, p->Np, 0)
         if (mode == MIX_NONE) IMG(MIX_NONE);
@@ -530,6 +535,13 @@ int cpra_set_carousel(cpra_plan_t p, int K, const double* h_alpha, int n_ei)
     p->K = K;
     for (int j = 0; j <= MAXK; ++j) p->alpha[j] = j <= K ? (float)h_alpha[j] : 0.f;
     p->n_ei = n_ei;
+    return CPRA_OK;
+}
+
+int cpra_set_update(cpra_plan_t p, int rule)
+{
+    if (!p || (rule != CPRA_UPDATE_HIO && rule != CPRA_UPDATE_RAAR && rule != CPRA_UPDATE_ER)) return CPRA_ERR_INVALID_ARG;
+    p->update = rule;
     return CPRA_OK;
 }
 

@@ -177,14 +177,13 @@ k_image(const float4* __restrict__ cur, float4* __restrict__ nxt, const float* _
     {
         const float4* __restrict__ own = cur + (size_t)n * istride;
         const uint16_t* __restrict__ Simg = S16 + (size_t)n * NRT * N;
-        const float2 nb = bc(-beta);
 #pragma unroll 4
         for (int i = threadIdx.x; i < image_quads<N>(); i += NT) {
             const int j = i % NPAIR, tx = i / NPAIR;   // tx = rt N + x
             const unsigned bits = (unsigned)Simg[tx] >> (2 * j);
             const c2 gh = mix(from_quad(__ldg(own + i)), (size_t)i);
             const c2 gp = from_quad(img[i]);
-            const float2 ore = pfma(nb, gp.re, gh.re), oim = pfma(nb, gp.im, gh.im);
+            const float2 ore = update_outside(mp, gp.re, gh.re), oim = update_outside(mp, gp.im, gh.im);
             float4 o;
             o.x = (bits & 1) ? gp.re.x : ore.x;
             o.y = (bits & 2) ? gp.re.y : ore.y;

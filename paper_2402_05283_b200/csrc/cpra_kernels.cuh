@@ -24,7 +24,16 @@ constexpr int MAXK = 8;  // = CPRA_MAX_K
 struct MixParams {
     int K;
     float a[MAXK + 1];
+    // real-space update outside the support: g <- c_ghat ghat + c_gp g'   (HIO: 1, -beta;  RAAR: beta,
+    // 1 - 2 beta;  ER: 0, 0;  cpra_set_update).  Inside the support g <- g' for all of them.
+    float c_ghat, c_gp;
 };
+// the update outside the support on a pair; with c_ghat = 1 (HIO) the product is exact, so the result
+// is the single fma ghat - beta g'
+__device__ __forceinline__ float2 update_outside(const MixParams& mp, float2 gp, float2 gh)
+{
+    return pfma(bc(mp.c_gp), gp, pmul(bc(mp.c_ghat), gh));
+}
 
 enum { MIX_NONE = 0, MIX_K1 = 1, MIX_GEN = 2, MIX_MASK = 3 };
 enum { COL_FULL = 0, COL_FWD = 1, COL_INV = 2 };
@@ -614,7 +623,6 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
     } else {
         const MixLoader<MIXMODE> mix(cur, istride, n, Np, mp);
         const float4* __restrict__ own = cur + (size_t)n * istride + toff;
-        const float2 nb = bc(-beta);
 #pragma unroll 4
         for (int i = threadIdx.x; i < tile_quads<N>(); i += NT) {
             const int x = ppos<N>(i / NP), j = i % NP;   // i runs over the physical quads of the tile
@@ -623,7 +631,7 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
             const c2 gh = ghat_in ? from_quad(__ldg(ghat_in + (size_t)n * istride + toff + i))
                                   : mix(from_quad(__ldg(own + i)), toff + (size_t)i);
             const c2 gp = from_quad(tile[i]);
-            const float2 ore = pfma(nb, gp.re, gh.re), oim = pfma(nb, gp.im, gh.im);
+            const float2 ore = update_outside(mp, gp.re, gh.re), oim = update_outside(mp, gp.im, gh.im);
             float4 o;
             o.x = (bits & 1) ? gp.re.x : ore.x;
             o.y = (bits & 2) ? gp.re.y : ore.y;

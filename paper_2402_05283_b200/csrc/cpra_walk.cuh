@@ -79,7 +79,7 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     auto i1 = [&](int r) -> int { return ((r & 1) ? o1o : o1e) + r * (8 * NP); };
     auto iL = [&](int r) -> int { return ((r & 1) ? oLo : oLe) + (r & ~1) * NP; };
     static_assert(R0 == 8 && N / R0 == 64, "offsets above assume an 8 x 8 x 8 plan");
-    const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]), nbeta = bc(-beta);
+    const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]);
 
     // issue the loads of projection m's spectrum tile (row tile rt) and support words into slot s
     auto load_tile = [&](int m, int rt, int s) {
@@ -146,7 +146,7 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
 #pragma unroll
             for (int r = 0; r < R0; ++r) {
                 const unsigned bits = (unsigned)sp[q + M0 * r] >> (sshift + 2 * j);
-                const float2 ore = pfma(nbeta, v[r].re, g0[r].re), oim = pfma(nbeta, v[r].im, g0[r].im);
+                const float2 ore = update_outside(mp, v[r].re, g0[r].re), oim = update_outside(mp, v[r].im, g0[r].im);
                 v[r].re = make_float2((bits & 1) ? v[r].re.x : ore.x, (bits & 2) ? v[r].re.y : ore.y);
                 v[r].im = make_float2((bits & 1) ? v[r].im.x : oim.x, (bits & 2) ? v[r].im.y : oim.y);
                 st_quad(tile + i0(r), v[r]);

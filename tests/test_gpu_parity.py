@@ -285,6 +285,22 @@ def test_tile_kernels_on_8_row_plans(torch_cuda, N, alpha, n_ei, chunk):
     assert np.abs(E - Eo).max() <= TOL_E * Eo.max() and abs(Eg - Ego) <= TOL_E * Ego
 
 
+@pytest.mark.parametrize("rule", ["raar", "er"])
+@pytest.mark.parametrize("N,Np", [(64, 6), (256, 4), (512, 5)])
+def test_update_rules(torch_cuda, rule, N, Np):
+    """RAAR and ER (cpra_set_update, reading A22) through the whole-image
+    kernel (N = 64), the tile kernels (N = 256) and the walking kernel (N = 512), against the oracle."""
+    p = cpra_inputs.random_stack(N, Np, seed=N + Np, beamstop=3)
+    o, g = _oracle(p), _gpu(p)
+    o.set_update(rule)
+    g.set_update(rule)
+    o.iterate(3, 0.9)
+    g.iterate(3, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 3 * TOL_1
+    _, Eg = _errors(g)
+    assert abs(Eg - o.get_error()[1]) <= TOL_E * o.get_error()[1]
+
+
 def test_walking_kernel_runs_and_seams(torch_cuda):
     """The walking kernel at N = 512 with N_p = 7 (runs shorter than the 3-slot pipeline, wrap-around
     halos inside a run) and with calls split so that K1 / K3 (first / last iteration of a call) and

@@ -177,3 +177,65 @@ def test_trajectory_error_decreases_on_tiny(tiny_problem):
     e0 = o.get_error()[1]
     o.iterate(49, 0.9)
     assert o.get_error()[1] < 0.35 * e0
+
+
+# ------------------------------------------------------------------------------------------------
+# the other real-space updates (reading A22): RAAR (PAPER.md:98 ref [38], :104) and ER
+# ------------------------------------------------------------------------------------------------
+def _one_uncoupled_iteration(rule, beta, S):
+    """One iteration with K = 0 on a seeded random stack, and the modulus-constrained estimate g'
+    computed here with numpy's FFT (independent of the oracle's transforms)."""
+    rng = np.random.default_rng(5)
+    N, Np = 16, 3
+    g0 = rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))
+    I_native = rng.gamma(2.0, 3.0, size=(Np, N, N))
+    G = np.fft.fft2(g0)
+    gp = np.fft.ifft2(np.sqrt(I_native) * G / np.abs(G))
+    o = Oracle(N, Np)
+    o.set_data(np.fft.fftshift(I_native, axes=(-2, -1)), None, np.zeros(Np))
+    o.set_support(S)
+    o.set_carousel([1.0], 1)
+    o.set_update(rule)
+    o.set_estimate(g0)
+    o.iterate(1, beta)
+    return g0, gp, o.get_projections(0)
+
+
+def test_raar_and_er_outside_and_inside_the_support():
+    S = np.zeros((3, 16, 16), np.uint8)
+    S[:, 4:12, 5:11] = 1
+    inside = S.astype(bool)
+    for beta in (0.9, 0.5, 0.3):
+        g0, gp, out = _one_uncoupled_iteration("raar", beta, S)
+        assert np.abs(out[inside] - gp[inside]).max() < 1e-12
+        assert np.abs(out[~inside] - (beta * g0 + (1 - 2 * beta) * gp)[~inside]).max() < 1e-12
+        g0, gp, out = _one_uncoupled_iteration("hio", beta, S)
+        assert np.abs(out[~inside] - (g0 - beta * gp)[~inside]).max() < 1e-12
+    g0, gp, out = _one_uncoupled_iteration("er", 0.9, S)
+    assert np.abs(out[inside] - gp[inside]).max() < 1e-12 and np.all(out[~inside] == 0)
+
+
+def test_raar_is_the_relaxed_reflection_formula():
+    """RAAR as its authors define it: x+ = beta/2 (R_S R_M + I) x + (1 - beta) P_M x with R = 2P - I,
+    evaluated with numpy operators on the whole image, against the oracle's pointwise form."""
+    beta = 0.9
+    S = np.zeros((3, 16, 16), np.uint8)
+    S[:, 3:13, 2:9] = 1
+    g0, gp, out = _one_uncoupled_iteration("raar", beta, S)
+    RM = 2 * gp - g0
+    RSRM = 2 * S * RM - RM
+    ref = 0.5 * beta * (RSRM + g0) + (1 - beta) * gp
+    assert np.abs(out - ref).max() < 1e-12
+
+
+def test_true_object_is_a_fixed_point_of_raar_and_er():
+    p, P, I_c, S = _exact_problem()
+    for rule in ("raar", "er"):
+        o = Oracle(p.N, p.Np)
+        o.set_data(I_c, None, p.angles)
+        o.set_support(S)
+        o.set_carousel([1.0], 1)
+        o.set_update(rule)
+        o.set_estimate(P)
+        o.iterate(3, 0.9)
+        assert np.abs(o.get_projections(0) - P).max() <= 1e-12 * np.abs(P).max()
