@@ -308,14 +308,15 @@ bool encode_scratch_tmap(CUtensorMap* tm, void* base, int N, int Np, int tb)
 
 // K3 of one iteration fused with K1 of the next (cpra_walk.cuh): 2 CTAs per SM, each a run of tiles
 template <int N>
-int launch_walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta)
+int launch_walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta, bool fires)
 {
     if constexpr (walk_ok<N>()) {
         const int total = (N / tile_batch<N>()) * p->Np;
         const int ctas = std::min(total, 2 * p->sms);
         const int per = (total + ctas - 1) / ctas;
         const dim3 grid((unsigned)((total + per - 1) / per));
-        const MixParams mp = mix_params(p, beta);
+        MixParams mp = mix_params(p, beta);
+        if (!fires) { mp.a[0] = 1.0f; mp.a[1] = 0.0f; }   // no mix before the next iteration (n_ei > 1): ghat = g exactly
         ProfScope prof(p, CPRA_PROFILE_WALK);
         const CUtensorMap& tin = p->tm_scr[scr_in == p->scr ? 0 : 1];
         const CUtensorMap& tout = p->tm_scr[scr_out == p->scr ? 0 : 1];
@@ -326,13 +327,15 @@ int launch_walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const flo
     }
 }
 
-// k iterations with the walking kernel: K1 (storing ghat) -> [K2 -> walk] x (k - 1) -> K2 -> K3 (reading ghat)
+// k iterations with the walking kernel: K1 (storing ghat) -> [K2 -> walk] x (k - 1) -> K2 -> K3 (reading ghat).
+// With n_ei > 1 the walk of an iteration that is not followed by a mix runs with weights (1, 0).
 template <int N>
 int iterate_walk(cpra_plan_s* p, int k, float beta, float scale)
 {
     float4* g = p->st[p->cur];
     float4* other = p->st[p->cur ^ 1];
-    int rc = launch_row_fwd<N>(p, g, MIX_K1, 0, p->Np, other);
+    auto fires = [&](long t) { return (t % p->n_ei) == 0; };   // does the carousel mix open iteration t (reading A3)
+    int rc = launch_row_fwd<N>(p, g, fires(p->t) ? MIX_K1 : MIX_NONE, 0, p->Np, other);
     float4 *sin = p->scr, *sout = p->scr2, *gh_old = other, *gh_new = g;
     for (int it = 0; it < k && rc == CPRA_OK; ++it) {
         rc = launch_col<N>(p, COL_FULL, 0, p->Np, scale, sin);
@@ -340,7 +343,7 @@ int iterate_walk(cpra_plan_s* p, int k, float beta, float scale)
         if (it == k - 1) {
             rc = launch_row_inv<N>(p, gh_old, gh_new, true, MIX_K1, beta, 1.0f, 0, p->Np, sin, gh_old);
         } else {
-            rc = launch_walk<N>(p, sin, sout, gh_old, gh_new, beta);
+            rc = launch_walk<N>(p, sin, sout, gh_old, gh_new, beta, fires(p->t + it + 1));
             std::swap(sin, sout);
             std::swap(gh_old, gh_new);
         }
@@ -587,7 +590,7 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
     // the walking kernel serves the default carousel (K = 1 every iteration) on plans with 8-row tiles
-    if (k > 0 && p->walk && p->have_tmap && chunk == p->Np && p->K == 1 && p->n_ei == 1 && p->Np >= 3) {
+    if (k > 0 && p->walk && p->have_tmap && chunk == p->Np && p->K == 1 && p->Np >= 3) {
         int rc = CPRA_ERR_UNSUPPORTED_SIZE;
         { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, if constexpr (walk_ok<NN>()) rc = iterate_walk<NN>(p, k, beta, scale)); return 0; }; f(); }
         if (rc != CPRA_ERR_UNSUPPORTED_SIZE) return rc;

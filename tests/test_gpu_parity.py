@@ -301,12 +301,14 @@ def test_update_rules(torch_cuda, rule, N, Np):
     assert abs(Eg - o.get_error()[1]) <= TOL_E * o.get_error()[1]
 
 
-def test_walking_kernel_runs_and_seams(torch_cuda):
+@pytest.mark.parametrize("n_ei", [1, 2, 3])
+def test_walking_kernel_runs_and_seams(torch_cuda, n_ei):
     """The walking kernel at N = 512 with N_p = 7 (runs shorter than the 3-slot pipeline, wrap-around
     halos inside a run) and with calls split so that K1 / K3 (first / last iteration of a call) and
-    the walk (iterations in between) alternate: against the oracle, and bit-identical to one call."""
+    the walk (iterations in between) alternate, for n_ei = 1, 2, 3 (the walk of an iteration that no mix
+    follows runs with weights (1, 0)): against the oracle, and bit-identical to one call."""
     p = cpra_inputs.random_stack(512, 7, seed=77, beamstop=5)
-    o, g, h = _oracle(p), _gpu(p), _gpu(p)
+    o, g, h = _oracle(p, n_ei=n_ei), _gpu(p, n_ei=n_ei), _gpu(p, n_ei=n_ei)
     o.iterate(6, 0.9)
     g.iterate(6, 0.9)
     for k in (1, 3, 2):
