@@ -303,6 +303,7 @@ k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm
     static_assert(B * NT == NP * (N / RL) && B >= 1, "last stage must fill the CTA exactly");
     constexpr int R0 = RX::R0, M0 = N / R0, NBF0 = NP * M0, IT0 = (NBF0 + NT - 1) / NT;
     constexpr bool PFMIX = RX::PF && (MODE == MIX_K1 || MODE == MIX_GEN);
+    constexpr bool FAST = inner_stages_warp_local<N>();   // 8-wide, inner radices 8 x 8: affine offsets
     extern __shared__ __align__(128) float4 sm[];
     const Smem<N> s(sm);
     float4* __restrict__ tile = s.tile;
@@ -367,12 +368,38 @@ k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm
                 for (int r = 0; r < R0; ++r) st_s(q + M0 * r, j, v[r]);
             }
         }
+    } else if constexpr (FAST) {
+        // 8-wide plans: the butterfly's quads are one base + compile-time multiples of r, in shared
+        // memory and (same layout) in the neighbours' tiles
+#pragma unroll 1
+        for (int it = 0; it < IT0; ++it) {
+            const int bf = (int)threadIdx.x + it * NT;
+            if ((NBF0 % NT) != 0 && bf >= NBF0) break;
+            const int j = bf % NP, n2 = bf / NP, o = ppos(n2, 8) * NP + j;
+            c2 v[R0];
+#pragma unroll
+            for (int r = 0; r < R0; ++r) {
+                const int idx = o + r * (M0 * NP);
+                v[r] = mix(from_quad(tile[idx]), toff + (size_t)idx);
+                if constexpr (MODE == MIX_MASK) {
+                    const unsigned bits = (unsigned)Srow[n2 + M0 * r] >> (sshift + 2 * j);
+                    if (!(bits & 1)) { v[r].re.x = 0.f; v[r].im.x = 0.f; }
+                    if (!(bits & 2)) { v[r].re.y = 0.f; v[r].im.y = 0.f; }
+                }
+                if (ghat_out) ghat_out[(size_t)n * istride + toff + (size_t)idx] = to_quad(v[r]);
+            }
+            dft<R0, false>(v);
+            twiddle<R0, false>(v, s.tw0, n2);
+#pragma unroll
+            for (int r = 0; r < R0; ++r) st_quad(tile + o + r * (M0 * NP), v[r]);
+        }
     } else {
         fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_first, st_s);
     }
     __syncthreads();
     if constexpr (RX::S == 3) {
-        fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);
+        if constexpr (FAST) stage1_8<N, false, false, NT>(tile, s.tw1);
+        else fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);
         inner_sync<N>();
     }
     // last stage (contiguous positions, no twiddles) + transposition into the scratch layout
@@ -381,7 +408,14 @@ k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm
     for (int b = 0; b < B; ++b) {
         const int bf = (int)threadIdx.x + b * NT, j = bf % NP, q = bf / NP;
 #pragma unroll
-        for (int r = 0; r < RL; ++r) v[b][r] = ld_s(q * RL + r, j);
+        if constexpr (FAST) {
+            const Last8<false> at(tile, q, j);
+#pragma unroll
+            for (int r = 0; r < RL; ++r) v[b][r] = from_quad(*at(r));
+        } else {
+#pragma unroll
+            for (int r = 0; r < RL; ++r) v[b][r] = ld_s(q * RL + r, j);
+        }
         dft<RL, false>(v[b]);
     }
     inner_sync<N>();   // (the block a butterfly is transposed into lies in its own 64-position block)
@@ -558,7 +592,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
 // transposes them into the row layout; the new state tile leaves by one bulk copy.
 // ------------------------------------------------------------------------------------------------
 template <int N, int MODE, int MIXMODE>
-__global__ void __launch_bounds__(Radix<N>::NT, Radix<N>::MINB)
+__global__ void __launch_bounds__(Radix<N>::NT, N == 1024 ? 3 : Radix<N>::MINB)   // (N = 1024: 84 registers without a cap; 80 lets a third CTA in)
 k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__ cur, float4* __restrict__ nxt,
           const float2* __restrict__ twg, const uint16_t* __restrict__ S16, MixParams mp, float beta,
           float scale, int Np, int n0, int nimg, const float4* __restrict__ ghat_in)
@@ -567,6 +601,7 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
     constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>();
     constexpr int NT = RX::NT, NRT = N / TBN, NCT = N / TBN, RL = last_radix<N>();
     constexpr int B = NP * (N / RL) / NT;
+    constexpr bool FAST = inner_stages_warp_local<N>();   // 8-wide, inner radices 8 x 8: affine offsets
     extern __shared__ __align__(128) float4 sm[];
     const Smem<N> s(sm);
     float4* __restrict__ tile = s.tile;
@@ -601,16 +636,24 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
 #pragma unroll
         for (int b = 0; b < B; ++b) {
             const int bf = (int)threadIdx.x + b * NT, j = bf % NP, q = bf / NP;
+            if constexpr (FAST) {
+                const Last8<false> at(tile, q, j);
 #pragma unroll
-            for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, v[b][r]);
+                for (int r = 0; r < RL; ++r) st_quad(at(r), v[b][r]);
+            } else {
+#pragma unroll
+                for (int r = 0; r < RL; ++r) st_s(q * RL + r, j, v[b][r]);
+            }
         }
     }
     inner_sync<N>();
     if constexpr (RX::S == 3) {
-        fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(s.tw1, ld_s, st_s);
+        if constexpr (FAST) stage1_8<N, true, false, NT>(tile, s.tw1);
+        else fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(s.tw1, ld_s, st_s);
         __syncthreads();
     }
-    fft_stage<N, RX::R0, N, true, NT, 1>(s.tw0, ld_s, st_s);
+    if constexpr (FAST) stage0_8<N, true, false, NT>(tile, s.tw0);
+    else fft_stage<N, RX::R0, N, true, NT, 1>(s.tw0, ld_s, st_s);
     __syncthreads();
 
     // epilogue over the quads of the tile: each thread rewrites its own quads in place
