@@ -53,7 +53,10 @@ __host__ __device__ __forceinline__ int sw(int j, int py, int np = NPAIR) { retu
 // They do in every stage with stride > 1 (consecutive n2); in the stage with contiguous positions
 // (radix 8) they are 8 apart, so odd 8-blocks swap their even and odd positions.  HBM tiles have the
 // same order (they are bulk-copied verbatim).
-__host__ __device__ __forceinline__ int ppos(int p, int tb) { return tb == 16 ? p : p ^ ((p >> 3) & 1); }
+// `par` (scratch tiles: the parity of the column tile ct) inverts the choice of the swapped blocks, so
+// that the two 8 x 8 blocks (rt, ct), (rt, ct + 1) that a quarter-warp of a row kernel transposes at
+// once have their rows in opposite halves of the bank window too.
+__host__ __device__ __forceinline__ int ppos(int p, int tb, int par = 0) { return tb == 16 ? p : p ^ (((p >> 3) + par) & 1); }
 template <int N> __host__ __device__ __forceinline__ int ppos(int p)
 {
     static_assert(tile_batch<N>() == 16 || last_radix<N>() == 8, "8-wide tiles: the contiguous stage must be radix 8");
@@ -170,7 +173,7 @@ template <int N> __device__ __forceinline__ void inner_sync()
 // SWZ = the scratch layout (slot = pair ^ key); otherwise the state layout (slot = pair).
 // ------------------------------------------------------------------------------------------------
 template <int N, bool INV, bool SWZ, int NT>
-__device__ __forceinline__ void stage0_8(float4* __restrict__ tile, const float2* __restrict__ tw0)
+__device__ __forceinline__ void stage0_8(float4* __restrict__ tile, const float2* __restrict__ tw0, int par = 0)
 {
     constexpr int R = Radix<N>::R0, M0 = N / R, NP = 4, NBF = NP * M0, ITERS = (NBF + NT - 1) / NT;
     static_assert(M0 == 64, "stage 0 of the 8-wide plans has stride 64");
@@ -179,7 +182,7 @@ __device__ __forceinline__ void stage0_8(float4* __restrict__ tile, const float2
         const int bf = (int)threadIdx.x + it * NT;
         if ((NBF % NT) != 0 && bf >= NBF) break;
         const int j = bf % NP, n2 = bf / NP;
-        float4* __restrict__ b = tile + ppos(n2, 8) * NP + (SWZ ? (j ^ ((n2 >> 1) & 3)) : j);
+        float4* __restrict__ b = tile + ppos(n2, 8, par) * NP + (SWZ ? (j ^ ((n2 >> 1) & 3)) : j);
         c2 v[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) v[r] = from_quad(b[r * (M0 * NP)]);
@@ -191,7 +194,7 @@ __device__ __forceinline__ void stage0_8(float4* __restrict__ tile, const float2
     }
 }
 template <int N, bool INV, bool SWZ, int NT>
-__device__ __forceinline__ void stage1_8(float4* __restrict__ tile, const float2* __restrict__ tw1)
+__device__ __forceinline__ void stage1_8(float4* __restrict__ tile, const float2* __restrict__ tw1, int par = 0)
 {
     constexpr int R = 8, NP = 4, NBF = NP * (N / R), ITERS = (NBF + NT - 1) / NT;
 #pragma unroll 1
@@ -200,8 +203,8 @@ __device__ __forceinline__ void stage1_8(float4* __restrict__ tile, const float2
         if ((NBF % NT) != 0 && bf >= NBF) break;
         const int j = bf % NP, q = bf / NP, blk = q / 8, n2 = q % 8;
         const int slot = SWZ ? (j ^ ((n2 >> 1) & 3)) : j;
-        float4* __restrict__ be = tile + (blk * 64 + n2) * NP + slot;
-        float4* __restrict__ bo = tile + (blk * 64 + (n2 ^ 1)) * NP + slot;
+        float4* __restrict__ be = tile + (blk * 64 + (n2 ^ par)) * NP + slot;         // even r (8-block 8 blk + r)
+        float4* __restrict__ bo = tile + (blk * 64 + (n2 ^ 1 ^ par)) * NP + slot;     // odd r
         c2 v[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) v[r] = from_quad(((r & 1) ? bo : be)[r * (8 * NP)]);
@@ -218,9 +221,9 @@ struct Last8 {
     float4* pe;
     float4* po;
     int j;
-    __device__ __forceinline__ Last8(float4* tile, int q, int j_) : j(j_)
+    __device__ __forceinline__ Last8(float4* tile, int q, int j_, int par = 0) : j(j_)
     {
-        const int s = q & 1;
+        const int s = (q + par) & 1;
         pe = tile + (8 * q + s) * 4;
         po = tile + (8 * q + 1 - s) * 4;
     }
@@ -252,14 +255,14 @@ struct Smem {
 // occupies the same 2 KiB of shared memory: position (16 ct + row) , slot jc ^ j.
 // ------------------------------------------------------------------------------------------------
 // `rt` = the row tile: inside its 8-row block the rows sit in the physical order of the column tile,
-// ppos(TB rt + r) = TB rt + (r ^ flip).  (With 8-wide tiles the two butterflies of a quarter-warp hit
-// the same half of the bank window here: a 2-way conflict on these 2 of the kernel's accesses.)
+// ppos(TB rt + r, ct) = TB rt + (r ^ flip), flip = (rt + ct) & 1: the two blocks ct, ct + 1 that a
+// quarter-warp handles together lie in opposite halves of the bank window (conflict-free).
 template <int N>
 __device__ __forceinline__ void store_transposed(float4* __restrict__ tile, const c2 (&v)[last_radix<N>()], int q, int j, int rt)
 {
     constexpr int RL = last_radix<N>(), TBN = tile_batch<N>(), NP = tile_pairs<N>();
     const int p0 = q * RL, ct = p0 / TBN, jc0 = (p0 % TBN) / 2;
-    const int r0 = ppos<N>(TBN * rt + 2 * j) % TBN, r1 = ppos<N>(TBN * rt + 2 * j + 1) % TBN;
+    const int r0 = ppos(TBN * rt + 2 * j, TBN, ct & 1) % TBN, r1 = ppos(TBN * rt + 2 * j + 1, TBN, ct & 1) % TBN;
 #pragma unroll
     for (int i = 0; i < RL / 2; ++i) {
         const int slot = (jc0 + i) ^ j;
@@ -272,7 +275,7 @@ __device__ __forceinline__ void load_transposed(const float4* __restrict__ tile,
 {
     constexpr int RL = last_radix<N>(), TBN = tile_batch<N>(), NP = tile_pairs<N>();
     const int p0 = q * RL, ct = p0 / TBN, jc0 = (p0 % TBN) / 2;
-    const int r0 = ppos<N>(TBN * rt + 2 * j) % TBN, r1 = ppos<N>(TBN * rt + 2 * j + 1) % TBN;
+    const int r0 = ppos(TBN * rt + 2 * j, TBN, ct & 1) % TBN, r1 = ppos(TBN * rt + 2 * j + 1, TBN, ct & 1) % TBN;
 #pragma unroll
     for (int i = 0; i < RL / 2; ++i) {
         const int slot = (jc0 + i) ^ j;
@@ -502,16 +505,17 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
     }
     mbar_wait(s.bar, 0);
 
-    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[ppos<N>(p) * NP + sw(j, p, NP)]); };
-    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + ppos<N>(p) * NP + sw(j, p, NP), v); };
+    const int par = ct & 1;   // see ppos
+    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[ppos(p, TBN, par) * NP + sw(j, p, NP)]); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + ppos(p, TBN, par) * NP + sw(j, p, NP), v); };
 
     constexpr bool FAST = inner_stages_warp_local<N>();   // 8-wide, inner radices 8 x 8: affine offsets
     if constexpr (MODE == COL_FULL || MODE == COL_FWD) {
-        if constexpr (FAST) stage0_8<N, false, true, NT>(tile, s.tw0);
+        if constexpr (FAST) stage0_8<N, false, true, NT>(tile, s.tw0, par);
         else fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_s, st_s);
         __syncthreads();
         if constexpr (RX::S == 3) {
-            if constexpr (FAST) stage1_8<N, false, true, NT>(tile, s.tw1);
+            if constexpr (FAST) stage1_8<N, false, true, NT>(tile, s.tw1, par);
             else fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(s.tw1, ld_s, st_s);
             inner_sync<N>();
         }
@@ -539,7 +543,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
 #pragma unroll 1
             for (int it = 0; it < ITERS; ++it) {
                 const int bf = (int)threadIdx.x + it * NT, j = bf % NP, q = bf / NP;
-                const Last8<true> at(tile, q, j);
+                const Last8<true> at(tile, q, j, par);
                 c2 v[RL];
 #pragma unroll
                 for (int r = 0; r < RL; ++r) v[r] = from_quad(*at(r));
@@ -561,7 +565,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
     if constexpr (MODE != COL_FWD) {
         if constexpr (RX::S == 3) {
             inner_sync<N>();
-            if constexpr (FAST) stage1_8<N, true, true, NT>(tile, s.tw1);
+            if constexpr (FAST) stage1_8<N, true, true, NT>(tile, s.tw1, par);
             else fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(s.tw1, ld_s, st_s);
         }
         __syncthreads();
@@ -572,7 +576,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
                 partial[(size_t)n * NCT + ct] = t;
             }
         }
-        if constexpr (FAST) stage0_8<N, true, true, NT>(tile, s.tw0);
+        if constexpr (FAST) stage0_8<N, true, true, NT>(tile, s.tw0, par);
         else fft_stage<N, RX::R0, N, true, NT, 1>(s.tw0, ld_s, st_s);
     }
     fence_async_smem();

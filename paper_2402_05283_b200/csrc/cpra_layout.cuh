@@ -20,7 +20,7 @@ __device__ __forceinline__ size_t st_idx(const Geo& g, int n, int y, int x)
 __device__ __forceinline__ size_t sc_idx(const Geo& g, int n, int py, int px)
 {
     const int tb = g.TB, np = tb / 2;
-    return ((((size_t)n * (g.N / tb) + (px / tb)) * g.N + ppos(py, tb)) * np + sw((px % tb) / 2, py, np)) * 4 + (px & 1);
+    return ((((size_t)n * (g.N / tb) + (px / tb)) * g.N + ppos(py, tb, (px / tb) & 1)) * np + sw((px % tb) / 2, py, np)) * 4 + (px & 1);
 }
 __device__ __forceinline__ size_t a_idx(const Geo& g, int n, int py, int px)
 {
