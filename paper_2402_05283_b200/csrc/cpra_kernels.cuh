@@ -1,18 +1,20 @@
-// cpra_kernels.cuh -- the three hot kernels of the CPRA loop (sm_100a).  See DESIGN.md "Kernels".
+// cpra_kernels.cuh -- the three tile kernels of the CPRA loop (sm_100a).  See DESIGN.md "Kernels".
 //
 // HBM layouts.  The unit everywhere is the quad [re_a, re_b, im_a, im_b] (16 B) of a batch pair
-// (cpra_fft.cuh); a tile is N positions x 8 quads = N x 128 B, contiguous in HBM, and has the SAME
-// byte layout in shared memory, so a tile moves with one asynchronous bulk copy (TMA 1D) each way
-// and never passes through registers on its way in or out.
+// (cpra_fft.cuh).  A tile is N positions x TB/2 quads (TB = Radix<N>::TB transforms per tile: 16, or 8
+// at N >= 512), contiguous in HBM, and has the SAME byte layout in shared memory, so it moves with
+// asynchronous bulk / tensor copies (TMA) each way and never passes through registers on its way in
+// or out.  Written for TB = 16:
 //   state g   [n][rt][x][j]       rt = y/16; quad j = rows (16 rt + 2j, + 2j + 1) at column x
 //   scratch   [n][ct][py][j^s]    ct = px/16; quad j = columns (16 ct + 2j, + 2j + 1) at row py,
-//                                 stored at slot j ^ s, s = (py >> 1) & 7.  py, px are digit-reversed
-//                                 frequency positions after the respective forward transform.
-//                                 The XOR makes the 16 x 16 block transposition that the row
-//                                 kernels do between their own layout and this one conflict-free.
+//                                 stored at slot j ^ s, s = (py >> 1) & (TB/2 - 1).  py, px are
+//                                 digit-reversed frequency positions after the respective forward
+//                                 transform.  The XOR makes the TB x TB block transposition that the
+//                                 row kernels do between their own layout and this one conflict-free.
 //   A=sqrt(I) [n][ct][q][j][r][e] fp32; py = RL q + r, px = 16 ct + 2j + e: the 2 RL values one
 //                                 thread needs in the fused middle stage are contiguous
-//   support   [n][rt][x] u16      bit b = S(y = 16 rt + b, x)       (1 bit per pixel)
+//   support   [n][y/16][x] u16    bit b = S(y = 16 (y/16) + b, x)   (1 bit per pixel)
+// With TB = 8 the positions of a tile are additionally permuted inside aligned pairs (ppos below).
 #pragma once
 #include <cuda.h>   // CUtensorMap (type only; the encoder is fetched through the runtime, see cpra_api.cu)
 
