@@ -624,6 +624,13 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
         if constexpr (MODE == ROWINV_HIO) bulk_load(s.sup, S16 + ((size_t)n * (N / 16) + (rt * TBN) / 16) * N, 2 * N, s.bar);
         tma_load_tile(tile, &tm_scr, rt, n, s.bar);
     }
+    if constexpr (MODE != ROWINV_PLAIN) {
+        // the epilogue's own-tile loads (ghat, or the previous state it is recomputed from; the
+        // neighbours' tiles are pulled in by the CTAs of n - 1 and n + 1) are requested into L2 now:
+        // they arrive while the stages run
+        const char* pf = reinterpret_cast<const char*>((ghat_in ? ghat_in : cur) + (size_t)n * istride + toff);
+        for (int l = threadIdx.x; l < tile_bytes<N>() / 128; l += NT) asm volatile("prefetch.global.L2 [%0];" ::"l"(pf + (size_t)l * 128));
+    }
     mbar_wait(s.bar, 0);
 
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[ppos<N>(p) * NP + j]); };

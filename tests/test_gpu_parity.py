@@ -228,9 +228,10 @@ def test_tiny_full_run(torch_cuda, problems):
 # ------------------------------------------------------------------------------------------------
 # full BASELINE.json sizes, in the launch configuration bench.py times, on sampled projections
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("cfg", [2, 3, 4])
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
 def test_full_size_sampled_projections(torch_cuda, cfg):
-    """Two iterations of the whole workload (config 4 = the headline: N = 512, N_p = 360) on the
+    """Two iterations of the whole workload (config 4 = the headline: N = 512, N_p = 360; config 5 = the
+    large detector: N = 1024, N_p = 180) on the
     GPU.  With K = 1 projection n after two iterations depends on projections n-2 .. n+2 only, so the
     oracle run on that 5-stack (its wrap-around touches only the two outer members, whose second
     iteration is not used) reproduces projection n exactly: checked for n at the seam and inside."""
