@@ -505,6 +505,12 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
         bulk_load(tile, g, tile_bytes<N>(), s.bar);
         bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
     }
+    if constexpr (MODE == COL_FULL) {
+        // sqrt(I) of this tile (one contiguous chunk, read by the fused middle stage) is requested
+        // into L2 now: it arrives while the forward stages run
+        const char* pf = reinterpret_cast<const char*>(Aperm + ((size_t)n * NCT + ct) * N * TBN);
+        for (int l = threadIdx.x; l < N * TBN * 4 / 128; l += NT) asm volatile("prefetch.global.L2 [%0];" ::"l"(pf + (size_t)l * 128));
+    }
     mbar_wait(s.bar, 0);
 
     const int par = ct & 1;   // see ppos
@@ -624,10 +630,11 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
         if constexpr (MODE == ROWINV_HIO) bulk_load(s.sup, S16 + ((size_t)n * (N / 16) + (rt * TBN) / 16) * N, 2 * N, s.bar);
         tma_load_tile(tile, &tm_scr, rt, n, s.bar);
     }
-    if constexpr (MODE != ROWINV_PLAIN) {
+    if constexpr (MODE != ROWINV_PLAIN && N >= 1024) {
         // the epilogue's own-tile loads (ghat, or the previous state it is recomputed from; the
         // neighbours' tiles are pulled in by the CTAs of n - 1 and n + 1) are requested into L2 now:
-        // they arrive while the stages run
+        // they arrive while the stages run.  Three CTAs per SM at N = 1024 do not hide that latency
+        // (0.995 -> 0.883 ms); six at N = 512 do, and the early requests cost 15 % there.
         const char* pf = reinterpret_cast<const char*>((ghat_in ? ghat_in : cur) + (size_t)n * istride + toff);
         for (int l = threadIdx.x; l < tile_bytes<N>() / 128; l += NT) asm volatile("prefetch.global.L2 [%0];" ::"l"(pf + (size_t)l * 128));
     }
