@@ -328,6 +328,17 @@ k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm
     const uint16_t* __restrict__ Srow = S16 + ((size_t)n * (N / 16) + (rt * TBN) / 16) * N;   // 16-row words
     const int sshift = (rt * TBN) % 16;
     auto tq = [&](int p, int j) -> int { return ppos<N>(p) * NP + j; };   // quad of (position, pair) in a state tile
+    if constexpr (!PFMIX && MODE == MIX_K1 && N <= 256) {
+        // the two neighbour tiles (read with 128-bit loads inside the first stage) are requested into L2
+        // before the own tile is waited for (N = 256: 148.5 -> 146.5 us per iteration at N_p = 180; at
+        // N = 1024 the same requests make the kernel 8 % slower)
+        const char* pm = reinterpret_cast<const char*>(mix.cm + toff);
+        const char* pp = reinterpret_cast<const char*>(mix.cp + toff);
+        for (int l = threadIdx.x; l < tile_bytes<N>() / 128; l += NT) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(pm + (size_t)l * 128));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(pp + (size_t)l * 128));
+        }
+    }
     if constexpr (!PFMIX) mbar_wait(s.bar, 0);
 
     auto ld_first = [&](int x, int j) -> c2 {
