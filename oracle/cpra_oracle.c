@@ -28,7 +28,10 @@
  *
  * Pins (tests/test_oracle_*.py): brute-force O(N^4) DFT below (separate code path), numpy.fft,
  * Parseval, shift theorem, Fourier-slice identity, idempotence of the two projections, closed-form
- * HIO decay, circulant eigenvalues of the mix, fixed point of the true object, error closed forms.
+ * HIO decay, circulant eigenvalues of the mix, fixed point of the true object, error closed forms;
+ * the feedback operand of step 6 under coupling (one-hot stack, nothing measured: (1 - beta) alpha
+ * outside the support), the clamp of negative intensities (|F[g']| = 0 there), and the averaging of
+ * duplicate rays in the assembly (slices with different constant spectra on a 360 degree scan).
  * Full multi-iteration trajectories have no external pin: PARITY UNPINNED beyond those invariants.
  *
  * Layout: images row-major [n][y][x], x fastest; complex = interleaved (re, im).  All I/O arrays of

@@ -138,3 +138,35 @@ def test_assembly_merges_duplicate_rays_on_a_360_scan():
     off_axis = inside & (k != 0)
     for v in vols:
         assert np.abs(v[:, 0, :][:, off_axis] - F3[:, 0, :][:, off_axis]).max() < 1e-9 * np.abs(F3).max()
+
+
+def test_assembly_averages_duplicate_rays_carrying_different_data():
+    """Step (ii) of the assembly: on a [0, 360) scan the ku <= 0 half of slice n points the same way
+    as the ku >= 0 half of slice n + Np/2; the two are ONE ray whose samples are the MEAN of the
+    contributors.  Give every slice a different constant spectrum c_n (g_n = c_n delta at the centre
+    pixel: F2 = c_n (-1)^(kz+ku), which step (i) turns into the constant c_n): the voxels on the
+    ray of direction theta_n then hold (c_n + c_{n+Np/2}) / 2 -- not c_n, not c_{n+Np/2} (first / last
+    contributor wins) -- and the axis rho = 0 holds the mean of all c_n."""
+    N, Np, h = 16, 4, 8
+    c = np.array([1.0 + 0.5j, -2.0 + 1.0j, 4.0 - 1.5j, 0.5 + 3.0j])
+    ang = 2 * np.pi * np.arange(Np) / Np                     # 0, 90, 180, 270 degrees
+    P = np.zeros((Np, N, N), complex)
+    P[:, h, h] = c
+    o = Oracle(N, Np)
+    o.set_data(np.ones((Np, N, N)), None, ang)
+    o.set_support(np.ones((Np, N, N), np.uint8))
+    o.set_estimate(P)
+    vol, w = o.assemble_3d()
+    m02, m13 = (c[0] + c[2]) / 2, (c[1] + c[3]) / 2
+    for kz in (0, 1, 5, -3):
+        for r in range(1, h):
+            sg = (-1.0) ** (kz + r)                          # step (iv): (-1)^(kx+ky+kz)
+            assert abs(vol[kz % N, 0, r] - sg * m02) < 1e-13, (kz, r)          # direction 0: slices 0 (+) and 2 (-)
+            assert abs(vol[kz % N, 0, -r] - sg * m02) < 1e-13, (kz, r)         # direction 180
+            assert abs(vol[kz % N, r, 0] - sg * m13) < 1e-13, (kz, r)          # direction 90: slices 1 (+) and 3 (-)
+            assert abs(vol[kz % N, -r, 0] - sg * m13) < 1e-13, (kz, r)         # direction 270
+        assert abs(vol[kz % N, 0, 0] - (-1.0) ** kz * c.mean()) < 1e-13
+    # on the diagonal (45 degrees: halfway between two merged rays; rho = r sqrt(2) is bracketed by
+    # constant radial samples) the bilinear value is the mean of the two ray means
+    assert abs(vol[0, 2, 2] - (m02 + m13) / 2) < 1e-13
+    assert abs(m02 - c[0]) > 0.5 and abs(m02 - c[2]) > 0.5   # averaging is distinguishable from one winner

@@ -239,3 +239,40 @@ def test_true_object_is_a_fixed_point_of_raar_and_er():
         o.set_estimate(P)
         o.iterate(3, 0.9)
         assert np.abs(o.get_projections(0) - P).max() <= 1e-12 * np.abs(P).max()
+
+
+# ------------------------------------------------------------------------------------------------
+# which state feeds the HIO / RAAR feedback term when the carousel fires (SURVEY.md 8(c) step 6:
+# ghat, the MIXED stack -- PAPER.md:58-62: the mix forms "the initial guess for each PO" of the
+# episode, and the conventional iteration that follows starts from that guess)
+# ------------------------------------------------------------------------------------------------
+def test_feedback_term_uses_the_mixed_stack_closed_form():
+    """Nothing measured (M = 0: G' = G, so g' = ghat), K = 1, a one-hot stack at n = j.  Outside the
+    support one iteration leaves (1 - beta) alpha_|n-j| X for HIO (ghat - beta ghat) and for RAAR
+    (beta ghat + (1 - 2 beta) ghat); with the pre-mix g_n as the feedback operand it would be
+    (delta_nj - beta alpha_|n-j|) X instead.  Inside the support: alpha_|n-j| X."""
+    Np, N, beta = 6, 8, 0.9
+    al = {0: 0.6, 1: 0.2}
+    rng = np.random.default_rng(21)
+    X = rng.normal(size=(N, N)) + 1j * rng.normal(size=(N, N))
+    S = np.zeros((Np, N, N), np.uint8)
+    S[:, 2:6, 1:5] = 1
+    inside = S[0].astype(bool)
+    for rule in ("hio", "raar"):
+        for j in (0, 3, Np - 1):
+            g = np.zeros((Np, N, N), complex)
+            g[j] = X
+            o = Oracle(N, Np)
+            o.set_data(np.ones((Np, N, N)), np.zeros((Np, N, N), np.uint8))     # M = 0 everywhere
+            o.set_support(S)
+            o.set_update(rule)
+            o.set_estimate(g)
+            o.iterate(1, beta)
+            out = o.get_projections(0)
+            for n in range(Np):
+                d = abs((n - j + Np // 2) % Np - Np // 2)
+                a = al.get(d, 0.0)
+                assert np.abs(out[n][inside] - a * X[inside]).max() < 1e-14, (rule, j, n)
+                assert np.abs(out[n][~inside] - (1 - beta) * a * X[~inside]).max() < 1e-14, (rule, j, n)
+            # the two readings differ by O(1) here, so the pin cannot pass by accident
+            assert np.abs((1 - beta) * al[0] * X[~inside] - (1 - beta * al[0]) * X[~inside]).max() > 0.1

@@ -160,3 +160,45 @@ def test_full_support_one_iteration_matches_modulus_then_nothing_changes():
     o.iterate(1, 0.9)
     assert np.abs(o.get_projections(0) - g1).max() < 1e-13             # second iteration: no change
     assert o.get_error()[1] < 1e-13
+
+
+# ---------------------------------------------------------------- A0: negative intensities
+def test_negative_intensity_is_clamped_to_zero_amplitude():
+    """I = |E|^2 cannot be negative; reading A14: I < 0 => A = 0.  With everything
+    measured and S = 1 everywhere one iteration returns g' itself, whose Fourier modulus (numpy's
+    FFT, not the oracle's) is exactly A: 0 on the pixels with I < 0, sqrt(I) elsewhere -- not
+    sqrt(|I|).  den_n counts the clamped intensities: a zero estimate has num_n = sum A^2 = den_n."""
+    Np, N = 3, 8
+    rng = np.random.default_rng(31)
+    I_c = rng.gamma(2.0, 3.0, size=(Np, N, N))
+    neg = rng.uniform(size=(Np, N, N)) < 0.3
+    I_c[neg] *= -1.0
+    g0 = _stack(Np, N, 32)
+    o = Oracle(N, Np)
+    o.set_data(I_c)
+    o.set_support(np.ones((Np, N, N), np.uint8))
+    o.set_carousel([1.0], 1)
+    o.set_estimate(g0)
+    o.iterate(1, 0.9)
+    mod = np.abs(np.fft.fftshift(np.fft.fft2(o.get_projections(0)), axes=(-2, -1)))     # detector-centred
+    assert neg.any() and mod[neg].max() < 1e-12
+    assert np.abs(mod[~neg] - np.sqrt(I_c[~neg])).max() < 1e-12
+    z = Oracle(N, Np)
+    z.set_data(I_c)
+    z.set_support(np.ones((Np, N, N), np.uint8))
+    z.set_carousel([1.0], 1)
+    z.set_estimate(np.zeros((Np, N, N), complex))
+    z.iterate(1, 0.9)
+    E, Eg = z.get_error()
+    assert np.abs(E - 1.0).max() < 1e-14 and abs(Eg - 1.0) < 1e-14
+    # and the error of g0 is normalised by the clamped sum, not by sum |I|
+    G = np.abs(np.fft.fftshift(np.fft.fft2(g0), axes=(-2, -1)))
+    A = np.sqrt(np.maximum(I_c, 0.0))
+    want = np.sqrt(((G - A) ** 2).sum(axis=(1, 2)) / np.maximum(I_c, 0.0).sum(axis=(1, 2)))
+    o2 = Oracle(N, Np)
+    o2.set_data(I_c)
+    o2.set_support(np.ones((Np, N, N), np.uint8))
+    o2.set_carousel([1.0], 1)
+    o2.set_estimate(g0)
+    o2.iterate(1, 0.9)
+    assert np.abs(o2.get_error()[0] - want).max() < 1e-12
