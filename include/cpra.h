@@ -57,13 +57,19 @@ enum {
 #define CPRA_FLAG_DEFAULT 0u
 #define CPRA_FLAG_FORCE_MULTIPASS 1u /* never use the one-CTA-per-image shared-memory kernel (N <= 128) */
 #define CPRA_FLAG_NO_CHUNKING 2u     /* run every pass over all Np images (no L2-resident chunking) */
+#define CPRA_FLAG_NO_WALK 4u         /* never fuse the inverse row pass of iteration t with the forward row pass of
+                                        t + 1 (k_row_walk): every iteration runs the three tile kernels.  Same
+                                        arithmetic per pixel; for tests and for timing the two structures */
+#define CPRA_FLAG_ALL 7u             /* every defined bit; any other bit makes cpra_plan fail with INVALID_ARG */
 
 /*
  * Create a plan for Np projections of N x N pixels ("a scattered intensity map ... of N x N
  * pixels is collected" for each of the N_p angles).  `cuda_stream` is a cudaStream_t (NULL = the
  * legacy default stream); all later work of this plan is enqueued on it.  Host-only: no device work.
  * Defaults: carousel weights alpha = (0.6, 0.2), K = 1, n_ei = 1 (K = 0, alpha_0 = 1 if Np < 3).
- * Errors: INVALID_ARG (out NULL), UNSUPPORTED_SIZE.
+ * Every behaviour switch of the library is a flag bit or a call of this header: the library reads
+ * no environment variable.
+ * Errors: INVALID_ARG (out NULL, undefined flag bits), UNSUPPORTED_SIZE.
  */
 int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream);
 
@@ -170,7 +176,9 @@ int cpra_get_projections(cpra_plan_t plan, int which, float* d_out);
  * only says "interpolate").  d_vol: interleaved complex fp32 [N][N][N] (kz, ky, kx), native FFT
  * order, comparable with the 3D FT of an object centred at (N/2, N/2, N/2); voxels with
  * sqrt(kx^2+ky^2) > N/2-1 are zero.  d_weight: fp32 [N][N][N], 1 where a value was written, 0
- * elsewhere; may be NULL.  One-shot, outside the timed loop.
+ * elsewhere; may be NULL.  One-shot, outside the timed loop.  Needs data (for the angles), support
+ * and an estimate -- NOT an iteration: assembling the starting estimate is allowed (the slices are
+ * then F[S g0]).  Overwrites the FFT scratch only; the loop state is untouched.
  * Errors: INVALID_ARG, NOT_READY (data, support or estimate missing), CUDA.
  */
 int cpra_assemble_3d(cpra_plan_t plan, float* d_vol, float* d_weight);

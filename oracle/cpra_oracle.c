@@ -168,7 +168,7 @@ int oracle_fft2(const double* in, double* out, int N, int count, int sign)
 
 /* Eq. (4), reading A1 (weights on n+-1, n+-2, ...; periodic in n) and A4 (Jacobi):
  * out_n = sum_{j=-K}^{K} alpha_|j| in_{(n+j) mod Np}.  in and out must not alias. */
-static void mix_stack(const cplx* in, cplx* out, int Np, size_t px, int K, const real* alpha)
+static void mix_stack(const cplx* in, cplx* out, int Np, size_t px, int K, const real* alpha, int N, int flip_seam)
 {
     #pragma omp parallel for schedule(static)
     for (int n = 0; n < Np; ++n) {
@@ -178,7 +178,20 @@ static void mix_stack(const cplx* in, cplx* out, int Np, size_t px, int K, const
             const int m = ((n + j) % Np + Np) % Np;
             const real a = alpha[j < 0 ? -j : j];
             const cplx* s = in + (size_t)m * px;
-            for (size_t i = 0; i < px; ++i) { o[i].re += a * s[i].re; o[i].im += a * s[i].im; }
+            /* Reading A5b (seam of a [0, 180) scan): projection n + Np is projection n seen from the
+             * other side, P(theta + 180)(z, u) = P(theta)(z, -u) (rotation about one axis), so
+             * a neighbour reached by wrapping ONCE round the end of the stack is read mirrored in u about
+             * the centre pixel N/2: u -> (N - u) mod N.  (2K + 1 <= Np: never more than one wrap.) */
+            const int wrapped = (n + j < 0) || (n + j >= Np);
+            if (flip_seam && wrapped) {
+                for (int y = 0; y < N; ++y)
+                    for (int x = 0; x < N; ++x) {
+                        const cplx v = s[(size_t)y * N + (size_t)((N - x) % N)];
+                        o[(size_t)y * N + x].re += a * v.re; o[(size_t)y * N + x].im += a * v.im;
+                    }
+            } else {
+                for (size_t i = 0; i < px; ++i) { o[i].re += a * s[i].re; o[i].im += a * s[i].im; }
+            }
         }
     }
 }
@@ -255,6 +268,9 @@ typedef struct oracle_plan_s {
     cplx* g;              /* state */
     cplx* tmp;            /* mixed copy ghat */
     int K; real alpha[64]; int n_ei;
+    int flip_seam;        /* reading A5b: mirror the neighbours taken across the ends of the stack */
+    /* Step C bank (oracle_merge_*): the N_l lowest-error episodes offered so far */
+    int NL, bank_count; cplx* bank; double* bank_E;
     int update;   /* ORACLE_UPDATE_*; HIO by default */
     long t;
     double* E; double Eglobal;
@@ -287,7 +303,7 @@ int oracle_destroy(oracle_plan_t p)
 {
     if (!p) return ORACLE_ERR_INVALID_ARG;
     free(p->A); free(p->M); free(p->S); free(p->den); free(p->angles);
-    free(p->g); free(p->tmp); free(p->E); free(p);
+    free(p->g); free(p->tmp); free(p->E); free(p->bank); free(p->bank_E); free(p);
     return ORACLE_OK;
 }
 
@@ -367,7 +383,7 @@ int oracle_iterate(oracle_plan_t p, int k, double beta_d)
         /* 1. mix (Eq. (4)) at the start of an episode; otherwise ghat = g */
         const int do_mix = (p->t % p->n_ei) == 0;
         if (do_mix) {
-            mix_stack(p->g, p->tmp, Np, px, p->K, p->alpha);
+            mix_stack(p->g, p->tmp, Np, px, p->K, p->alpha, N, p->flip_seam);
             cplx* sw = p->g; p->g = p->tmp; p->tmp = sw;            /* p->g now holds ghat */
         }
         double numtot = 0.0, dentot = 0.0;
@@ -425,7 +441,7 @@ int oracle_mix(const double* in, double* out, int N, int Np, int K, const double
     real al[64];
     for (int j = 0; j <= K; ++j) al[j] = (real)alpha[j];
     for (size_t i = 0; i < tot; ++i) { a[i].re = (real)in[2 * i]; a[i].im = (real)in[2 * i + 1]; }
-    mix_stack(a, b, Np, px, K, al);
+    mix_stack(a, b, Np, px, K, al, N, 0);
     for (size_t i = 0; i < tot; ++i) { out[2 * i] = b[i].re; out[2 * i + 1] = b[i].im; }
     free(a); free(b);
     return ORACLE_OK;
@@ -593,6 +609,336 @@ int oracle_assemble_3d(oracle_plan_t p, double* vol, double* weight)
         }
     }
     free(E); free(rays); free(ustart); free(uphi);
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* seam of a 180 degree scan, shrink-wrap                                    */
+/* ------------------------------------------------------------------------------------------ */
+
+/* flip = 1: neighbours taken across the ends of the stack are mirrored in u (see mix_stack). */
+int oracle_set_seam(oracle_plan_t p, int flip)
+{
+    if (!p || (flip != 0 && flip != 1)) return ORACLE_ERR_INVALID_ARG;
+    p->flip_seam = flip;
+    return ORACLE_OK;
+}
+
+/* Eq. (4) with the seam flag, stand-alone (for the pins). */
+int oracle_mix_seam(const double* in, double* out, int N, int Np, int K, const double* alpha, int flip)
+{
+    if (!in || !out || !alpha || K < 0 || K > 63 || 2 * K + 1 > Np) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N, tot = px * Np;
+    cplx* a = (cplx*)malloc(sizeof(cplx) * tot); cplx* b = (cplx*)malloc(sizeof(cplx) * tot);
+    real al[64];
+    for (int j = 0; j <= K; ++j) al[j] = (real)alpha[j];
+    for (size_t i = 0; i < tot; ++i) { a[i].re = (real)in[2 * i]; a[i].im = (real)in[2 * i + 1]; }
+    mix_stack(a, b, Np, px, K, al, N, flip);
+    for (size_t i = 0; i < tot; ++i) { out[2 * i] = b[i].re; out[2 * i + 1] = b[i].im; }
+    free(a); free(b);
+    return ORACLE_OK;
+}
+
+/* Periodic Gaussian blur of a real image, width sigma pixels, done in Fourier space:
+ * B = F^-1[ F[a] . exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2) ], ky, kx signed integer frequencies
+ * (the transform of a Gaussian of standard deviation sigma sampled on the N-periodic grid). */
+static void blur_image(const real* a, real* b, int N, double sigma)
+{
+    const size_t px = (size_t)N * N;
+    cplx* w = (cplx*)malloc(sizeof(cplx) * px);
+    for (size_t i = 0; i < px; ++i) { w[i].re = a[i]; w[i].im = 0; }
+    fft2d(w, N, -1);
+    for (int iy = 0; iy < N; ++iy) {
+        const int ky = iy < N / 2 ? iy : iy - N;
+        for (int ix = 0; ix < N; ++ix) {
+            const int kx = ix < N / 2 ? ix : ix - N;
+            const real f = (real)exp(-2.0 * PI * PI * sigma * sigma * ((double)ky * ky + (double)kx * kx) / ((double)N * N));
+            w[(size_t)iy * N + ix].re *= f; w[(size_t)iy * N + ix].im *= f;
+        }
+    }
+    fft2d(w, N, +1);
+    for (size_t i = 0; i < px; ++i) b[i] = w[i].re;
+    free(w);
+}
+
+int oracle_blur(const double* in, double* out, int N, double sigma)
+{
+    if (!in || !out || !is_pow2(N) || !(sigma >= 0.0)) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N;
+    real* a = (real*)malloc(sizeof(real) * px); real* b = (real*)malloc(sizeof(real) * px);
+    for (size_t i = 0; i < px; ++i) a[i] = (real)in[i];
+    blur_image(a, b, N, sigma);
+    for (size_t i = 0; i < px; ++i) out[i] = (double)b[i];
+    free(a); free(b);
+    return ORACLE_OK;
+}
+
+/* Shrink-wrap support update ("2D CSWA" ref [35]; "an extra 2D CSWA iteration to obtain a
+ * tighter space constraint"), reading A23: for every projection
+ *     b_n = G_sigma * |S_n g_n|   (the current estimate restricted to the current support, blurred),
+ *     S_n <- [ b_n >= threshold . max_pixels b_n ]        (all zero if the maximum is not positive).
+ * blurred (optional, [Np][N][N] double) receives b_n so that a comparison can set aside the pixels
+ * whose b_n lies within rounding of the threshold. */
+int oracle_shrinkwrap(oracle_plan_t p, double sigma, double threshold, double* blurred)
+{
+    if (!p || !(sigma >= 0.0) || !(threshold >= 0.0)) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_support || !p->have_estimate) return ORACLE_ERR_NOT_READY;
+    const int N = p->N;
+    const size_t px = p->px;
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int n = 0; n < p->Np; ++n) {
+        real* a = (real*)malloc(sizeof(real) * px); real* b = (real*)malloc(sizeof(real) * px);
+        for (size_t i = 0; i < px; ++i) {
+            const size_t gi = (size_t)n * px + i;
+            a[i] = p->S[gi] ? (real)sqrt((double)(p->g[gi].re * p->g[gi].re + p->g[gi].im * p->g[gi].im)) : (real)0;
+        }
+        blur_image(a, b, N, sigma);
+        real m = b[0];
+        for (size_t i = 1; i < px; ++i) if (b[i] > m) m = b[i];
+        for (size_t i = 0; i < px; ++i) {
+            p->S[(size_t)n * px + i] = (m > 0 && b[i] >= (real)threshold * m) ? 1 : 0;
+            if (blurred) blurred[(size_t)n * px + i] = (double)b[i];
+        }
+        free(a); free(b);
+    }
+    return ORACLE_OK;
+}
+
+int oracle_get_support(oracle_plan_t p, unsigned char* S)
+{
+    if (!p || !S) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_support) return ORACLE_ERR_NOT_READY;
+    memcpy(S, p->S, p->px * (size_t)p->Np);
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Step A (pre-reconstruction) and Step C (repeating and merging)           */
+/* ------------------------------------------------------------------------------------------ */
+
+/* Step A: "Pre-reconstruct a single PO ... via the conventional 2D CXDI algorithm": k iterations of
+ * steps 2-6 of the loop on projection n alone (no mix: a single PO has no neighbours in Step A); the
+ * other projections and the iteration counter t are untouched. */
+int oracle_prereconstruct(oracle_plan_t p, int n, int k, double beta_d)
+{
+    if (!p || n < 0 || n >= p->Np || k < 0 || !isfinite(beta_d)) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_data || !p->have_support || !p->have_estimate) return ORACLE_ERR_NOT_READY;
+    const real beta = (real)beta_d;
+    const size_t px = p->px;
+    cplx* ghat = p->g + (size_t)n * px;
+    cplx* G = (cplx*)malloc(sizeof(cplx) * px);
+    for (int it = 0; it < k; ++it) {
+        memcpy(G, ghat, sizeof(cplx) * px);
+        fft2d(G, p->N, -1);
+        (void)modulus_image(G, p->A + (size_t)n * px, p->M + (size_t)n * px, px);
+        fft2d(G, p->N, +1);
+        if (p->update == ORACLE_UPDATE_RAAR) raar_image(ghat, G, p->S + (size_t)n * px, px, beta);
+        else if (p->update == ORACLE_UPDATE_ER) er_image(ghat, G, p->S + (size_t)n * px, px);
+        else hio_image(ghat, G, p->S + (size_t)n * px, px, beta);
+    }
+    free(G);
+    return ORACLE_OK;
+}
+
+/* Centre of mass of one PO about the centre pixel (N/2, N/2), mass = |O| ("we move the mass center
+ * of each PO by Delta r_n = - int O'_n(r) r dv"; the printed integral lacks its normalisation; reading A24:
+ * com = sum |O| r / sum |O|, r = (y - N/2, x - N/2)).  com = 0 for an empty image. */
+static void center_of_mass(const cplx* o, int N, double* cy, double* cx)
+{
+    double m = 0.0, sy = 0.0, sx = 0.0;
+    for (int y = 0; y < N; ++y)
+        for (int x = 0; x < N; ++x) {
+            const cplx v = o[(size_t)y * N + x];
+            const double w = sqrt((double)v.re * v.re + (double)v.im * v.im);
+            m += w; sy += w * (double)(y - N / 2); sx += w * (double)(x - N / 2);
+        }
+    *cy = m > 0.0 ? sy / m : 0.0;
+    *cx = m > 0.0 ? sx / m : 0.0;
+}
+int oracle_center_of_mass(const double* img, int N, double* cy, double* cx)
+{
+    if (!img || !cy || !cx || N < 1) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N;
+    cplx* a = (cplx*)malloc(sizeof(cplx) * px);
+    for (size_t i = 0; i < px; ++i) { a[i].re = (real)img[2 * i]; a[i].im = (real)img[2 * i + 1]; }
+    center_of_mass(a, N, cy, cx);
+    free(a);
+    return ORACLE_OK;
+}
+/* whole-pixel shift that brings the centre of mass to the centre pixel: -round(com), halves away from 0 */
+static int shift_of(double com) { return -(int)(com >= 0.0 ? floor(com + 0.5) : -floor(-com + 0.5)); }
+
+/* Step C.  The bank keeps the N_l episodes of lowest reconstruction error among those offered
+ * ("We select a certain number N_l < N_r of the best reconstructed episodes, which have the lowest
+ * reconstruction error").  An episode is the stack of supported estimates S_n g_n (what Step D consumes). */
+int oracle_merge_begin(oracle_plan_t p, int NL)
+{
+    if (!p || NL < 1) return ORACLE_ERR_INVALID_ARG;
+    free(p->bank); free(p->bank_E);
+    p->NL = NL; p->bank_count = 0;
+    p->bank = (cplx*)calloc((size_t)NL * p->Np * p->px, sizeof(cplx));
+    p->bank_E = (double*)calloc((size_t)NL, sizeof(double));
+    return ORACLE_OK;
+}
+
+/* Offer an episode with reconstruction error E: `episode` = interleaved complex double [Np][N][N], or
+ * NULL = the plan's own S.g with the global error of its last iteration (E is then ignored).  It takes a
+ * free slot, else replaces the worst kept episode if E is lower than that one's (the first worst on ties). */
+int oracle_merge_offer(oracle_plan_t p, const double* episode, double E)
+{
+    if (!p || !p->bank) return ORACLE_ERR_INVALID_ARG;
+    if (!episode) {
+        if (!p->have_estimate || !p->have_support || !p->have_error) return ORACLE_ERR_NOT_READY;
+        E = p->Eglobal;
+    }
+    int slot = -1;
+    if (p->bank_count < p->NL) slot = p->bank_count++;
+    else {
+        int w = 0;
+        for (int e = 1; e < p->NL; ++e) if (p->bank_E[e] > p->bank_E[w]) w = e;
+        if (E < p->bank_E[w]) slot = w;
+    }
+    if (slot < 0) return ORACLE_OK;
+    const size_t tot = p->px * (size_t)p->Np;
+    cplx* dst = p->bank + (size_t)slot * tot;
+    for (size_t i = 0; i < tot; ++i) {
+        if (episode) { dst[i].re = (real)episode[2 * i]; dst[i].im = (real)episode[2 * i + 1]; }
+        else if (p->S[i]) dst[i] = p->g[i];
+        else { dst[i].re = 0; dst[i].im = 0; }
+    }
+    p->bank_E[slot] = E;
+    return ORACLE_OK;
+}
+
+/* errors of the kept episodes, in slot order; returns how many are kept through *count */
+int oracle_merge_errors(oracle_plan_t p, double* E, int* count)
+{
+    if (!p || !p->bank || !count) return ORACLE_ERR_INVALID_ARG;
+    *count = p->bank_count;
+    if (E) for (int e = 0; e < p->bank_count; ++e) E[e] = p->bank_E[e];
+    return ORACLE_OK;
+}
+
+/* The merge itself, in the paper's order:
+ *  1. every PO of every kept episode is moved by a whole number of pixels (circularly) so that its centre
+ *     of mass sits on the centre pixel:  O'(y, x) = O(y - sy, x - sx),  s = -round(com)
+ *  2. b = the kept episode of lowest error (first on ties).  For every other episode e, on ONE PO n_ref
+ *     ("one of the POs in this best episode and the same number PO in other episodes"; n_ref = -1:
+ *     summed over all POs): c = <O_b, O_e> = sum conj(O_b) O_e and c_T = <O_b, T O_e> with the twin
+ *     T O(r) = conj(O(-r)) about the centre pixel -- the image with the same Fourier modulus (P:70 prints
+ *     O(-r); that is the twin of a real object, conj(O(-r)) that of a complex one: reading A25).
+ *     An iterate without reality constraint carries a free global phase, so "Euclidean distance" is read
+ *     as the distance minimised over that phase, ||a||^2 + ||b||^2 - 2 |<a, b>| (reading A25): the twin is
+ *     taken iff |c_T| > |c|, and the episode is multiplied by conj(c)/|c| (1 if c = 0) of the chosen one.
+ *  3. out_n = mean over the kept episodes of the corrected POs
+ * out: interleaved complex double [Np][N][N].  shifts (optional): int [kept][Np][2] (sy, sx);
+ * twins (optional): int [kept] (1 = twin taken). */
+int oracle_merge_finish(oracle_plan_t p, int n_ref, double* out, int* shifts, int* twins)
+{
+    if (!p || !p->bank || !out || n_ref < -1 || n_ref >= p->Np) return ORACLE_ERR_INVALID_ARG;
+    if (p->bank_count < 1) return ORACLE_ERR_NOT_READY;
+    const int N = p->N, Np = p->Np, L = p->bank_count;
+    const size_t px = p->px, tot = px * (size_t)Np;
+    /* 1. centre-of-mass shifts */
+    cplx* tmp = (cplx*)malloc(sizeof(cplx) * px);
+    for (int e = 0; e < L; ++e)
+        for (int n = 0; n < Np; ++n) {
+            cplx* o = p->bank + (size_t)e * tot + (size_t)n * px;
+            double cy, cx;
+            center_of_mass(o, N, &cy, &cx);
+            const int sy = shift_of(cy), sx = shift_of(cx);
+            if (shifts) { shifts[((size_t)e * Np + n) * 2] = sy; shifts[((size_t)e * Np + n) * 2 + 1] = sx; }
+            memcpy(tmp, o, sizeof(cplx) * px);
+            for (int y = 0; y < N; ++y)
+                for (int x = 0; x < N; ++x)
+                    o[(size_t)y * N + x] = tmp[(size_t)(((y - sy) % N + N) % N) * N + (size_t)(((x - sx) % N + N) % N)];
+        }
+    /* 2. twin and global phase against the best episode */
+    int b = 0;
+    for (int e = 1; e < L; ++e) if (p->bank_E[e] < p->bank_E[b]) b = e;
+    for (int e = 0; e < L; ++e) {
+        if (twins) twins[e] = 0;
+        if (e == b) continue;
+        double cr = 0.0, ci = 0.0, tr = 0.0, ti = 0.0;
+        for (int n = (n_ref < 0 ? 0 : n_ref); n <= (n_ref < 0 ? Np - 1 : n_ref); ++n) {
+            const cplx* ob = p->bank + (size_t)b * tot + (size_t)n * px;
+            const cplx* oe = p->bank + (size_t)e * tot + (size_t)n * px;
+            for (int y = 0; y < N; ++y)
+                for (int x = 0; x < N; ++x) {
+                    const cplx a = ob[(size_t)y * N + x];
+                    const cplx v = oe[(size_t)y * N + x];
+                    const cplx w = oe[(size_t)((N - y) % N) * N + (size_t)((N - x) % N)];   /* T: conj of this */
+                    cr += (double)a.re * v.re + (double)a.im * v.im;      /* conj(a) v */
+                    ci += (double)a.re * v.im - (double)a.im * v.re;
+                    tr += (double)a.re * w.re - (double)a.im * w.im;      /* conj(a) conj(w) */
+                    ti += -(double)a.re * w.im - (double)a.im * w.re;
+                }
+        }
+        const double mc = sqrt(cr * cr + ci * ci), mt = sqrt(tr * tr + ti * ti);
+        const int twin = mt > mc;
+        const double m = twin ? mt : mc;
+        const double ur = m > 0.0 ? (twin ? tr : cr) / m : 1.0, ui = m > 0.0 ? -(twin ? ti : ci) / m : 0.0;   /* conj(c)/|c| */
+        if (twins) twins[e] = twin;
+        for (int n = 0; n < Np; ++n) {
+            cplx* o = p->bank + (size_t)e * tot + (size_t)n * px;
+            memcpy(tmp, o, sizeof(cplx) * px);
+            for (int y = 0; y < N; ++y)
+                for (int x = 0; x < N; ++x) {
+                    cplx v = tmp[(size_t)y * N + x];
+                    if (twin) { v = tmp[(size_t)((N - y) % N) * N + (size_t)((N - x) % N)]; v.im = -v.im; }
+                    o[(size_t)y * N + x].re = (real)(ur * v.re - ui * v.im);
+                    o[(size_t)y * N + x].im = (real)(ur * v.im + ui * v.re);
+                }
+        }
+    }
+    free(tmp);
+    /* 3. average */
+    for (size_t i = 0; i < tot; ++i) {
+        double sr = 0.0, si = 0.0;
+        for (int e = 0; e < L; ++e) { sr += (double)p->bank[(size_t)e * tot + i].re; si += (double)p->bank[(size_t)e * tot + i].im; }
+        out[2 * i] = sr / L; out[2 * i + 1] = si / L;
+    }
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* the 3D transform of Step D ("3D FTs as a set of 2D FTs")     */
+/* ------------------------------------------------------------------------------------------ */
+/* vol [N][N][N] interleaved complex double (z, y, x), in -> out (may alias): all x lines, all y lines,
+ * all z lines with the textbook fft1d.  sign = -1 forward, unnormalised; +1 inverse, / N^3. */
+int oracle_fft3(const double* in, double* out, int N, int sign)
+{
+    if (!in || !out || !is_pow2(N) || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    const size_t n3 = (size_t)N * N * N;
+    cplx* v = (cplx*)malloc(sizeof(cplx) * n3);
+    for (size_t i = 0; i < n3; ++i) { v[i].re = (real)in[2 * i]; v[i].im = (real)in[2 * i + 1]; }
+    cplx* tw = twiddle_table(N, sign);
+    #pragma omp parallel
+    {
+        cplx* line = (cplx*)malloc(sizeof(cplx) * (size_t)N);
+        #pragma omp for schedule(static)
+        for (int z = 0; z < N; ++z)
+            for (int y = 0; y < N; ++y) fft1d(v + ((size_t)z * N + y) * N, N, tw);
+        #pragma omp for schedule(static)
+        for (int z = 0; z < N; ++z)
+            for (int x = 0; x < N; ++x) {
+                for (int y = 0; y < N; ++y) line[y] = v[((size_t)z * N + y) * N + x];
+                fft1d(line, N, tw);
+                for (int y = 0; y < N; ++y) v[((size_t)z * N + y) * N + x] = line[y];
+            }
+        #pragma omp for schedule(static)
+        for (int y = 0; y < N; ++y)
+            for (int x = 0; x < N; ++x) {
+                for (int z = 0; z < N; ++z) line[z] = v[((size_t)z * N + y) * N + x];
+                fft1d(line, N, tw);
+                for (int z = 0; z < N; ++z) v[((size_t)z * N + y) * N + x] = line[z];
+            }
+        free(line);
+    }
+    free(tw);
+    const double sc = sign > 0 ? 1.0 / ((double)N * N * N) : 1.0;
+    for (size_t i = 0; i < n3; ++i) { out[2 * i] = (double)v[i].re * sc; out[2 * i + 1] = (double)v[i].im * sc; }
+    free(v);
     return ORACLE_OK;
 }
 

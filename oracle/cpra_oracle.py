@@ -54,6 +54,18 @@ def _lib(precision: str = "f64"):
         lib.oracle_modulus.argtypes = [vp, vp, vp, ci, vp]
         lib.oracle_hio.argtypes = [vp, vp, vp, ci, cd]
         lib.oracle_real_name.restype = ctypes.c_char_p
+        lib.oracle_set_seam.argtypes = [vp, ci]
+        lib.oracle_mix_seam.argtypes = [vp, vp, ci, ci, ci, vp, ci]
+        lib.oracle_blur.argtypes = [vp, vp, ci, cd]
+        lib.oracle_shrinkwrap.argtypes = [vp, cd, cd, vp]
+        lib.oracle_get_support.argtypes = [vp, vp]
+        lib.oracle_prereconstruct.argtypes = [vp, ci, ci, cd]
+        lib.oracle_center_of_mass.argtypes = [vp, ci, vp, vp]
+        lib.oracle_merge_begin.argtypes = [vp, ci]
+        lib.oracle_merge_offer.argtypes = [vp, vp, cd]
+        lib.oracle_merge_errors.argtypes = [vp, vp, vp]
+        lib.oracle_merge_finish.argtypes = [vp, ci, vp, vp, vp]
+        lib.oracle_fft3.argtypes = [vp, vp, ci, ci]
         _LIBS[precision] = lib
     return _LIBS[precision]
 
@@ -115,6 +127,40 @@ def hio(ghat, gp, S, beta, precision="f64"):
     s = np.ascontiguousarray(S, dtype=np.uint8)
     _chk(_lib(precision).oracle_hio(a.ctypes.data, b.ctypes.data, s.ctypes.data, a.shape[-1], float(beta)), "oracle_hio")
     return a
+
+
+def mix_seam(stack, alpha, flip, precision="f64"):
+    """Eq. (4) with the seam flag of reading A5b (flip=1: neighbours across the ends of the stack mirrored in u)."""
+    a = _c128(stack)
+    Np, N = a.shape[0], a.shape[-1]
+    al = np.ascontiguousarray(alpha, dtype=np.float64)
+    out = np.empty_like(a)
+    _chk(_lib(precision).oracle_mix_seam(a.ctypes.data, out.ctypes.data, N, Np, len(al) - 1, al.ctypes.data, int(flip)), "oracle_mix_seam")
+    return out
+
+
+def blur(img, sigma, precision="f64"):
+    """Periodic Gaussian blur of one real N x N image (the blur of the shrink-wrap update)."""
+    a = np.ascontiguousarray(img, dtype=np.float64)
+    out = np.empty_like(a)
+    _chk(_lib(precision).oracle_blur(a.ctypes.data, out.ctypes.data, a.shape[-1], float(sigma)), "oracle_blur")
+    return out
+
+
+def center_of_mass(img):
+    """(cy, cx) of |img| about the centre pixel (N/2, N/2)."""
+    a = _c128(img)
+    cy, cx = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _chk(_lib().oracle_center_of_mass(a.ctypes.data, a.shape[-1], ctypes.addressof(cy), ctypes.addressof(cx)), "oracle_center_of_mass")
+    return cy.value, cx.value
+
+
+def fft3(vol, sign=-1, precision="f64"):
+    """3D FFT of a cube [N,N,N] (z, y, x) as x, y and z lines of the radix-2 routine (sign=+1: inverse, /N^3)."""
+    a = _c128(vol)
+    out = np.empty_like(a)
+    _chk(_lib(precision).oracle_fft3(a.ctypes.data, out.ctypes.data, a.shape[-1], sign), "oracle_fft3")
+    return out
 
 
 class Oracle:
@@ -186,6 +232,48 @@ class Oracle:
         _chk(self._l.oracle_assemble_3d(self._h, vol.ctypes.data, None if w is None else w.ctypes.data),
              "oracle_assemble_3d")
         return (vol, w) if want_weight else vol
+
+    # -- seam, shrink-wrap, Step A, Step C ------------------------------------------
+    def set_seam(self, flip):
+        _chk(self._l.oracle_set_seam(self._h, int(bool(flip))), "oracle_set_seam")
+        return self
+
+    def shrinkwrap(self, sigma, threshold, want_blurred=False):
+        b = np.empty((self.Np, self.N, self.N), dtype=np.float64) if want_blurred else None
+        _chk(self._l.oracle_shrinkwrap(self._h, float(sigma), float(threshold), None if b is None else b.ctypes.data),
+             "oracle_shrinkwrap")
+        return b
+
+    def get_support(self):
+        S = np.empty((self.Np, self.N, self.N), dtype=np.uint8)
+        _chk(self._l.oracle_get_support(self._h, S.ctypes.data), "oracle_get_support")
+        return S
+
+    def prereconstruct(self, n, k, beta=0.9):
+        _chk(self._l.oracle_prereconstruct(self._h, int(n), int(k), float(beta)), "oracle_prereconstruct")
+
+    def merge_begin(self, NL):
+        _chk(self._l.oracle_merge_begin(self._h, int(NL)), "oracle_merge_begin")
+
+    def merge_offer(self, episode=None, E=0.0):
+        e = None if episode is None else _c128(episode)
+        _chk(self._l.oracle_merge_offer(self._h, None if e is None else e.ctypes.data, float(E)), "oracle_merge_offer")
+
+    def merge_errors(self):
+        n = ctypes.c_int(0)
+        _chk(self._l.oracle_merge_errors(self._h, None, ctypes.addressof(n)), "oracle_merge_errors")
+        E = np.empty(n.value, dtype=np.float64)
+        _chk(self._l.oracle_merge_errors(self._h, E.ctypes.data, ctypes.addressof(n)), "oracle_merge_errors")
+        return E
+
+    def merge_finish(self, n_ref=0):
+        """Returns (final episode [Np,N,N] complex128, shifts [kept,Np,2] int32, twins [kept] int32)."""
+        kept = len(self.merge_errors())
+        out = np.empty((self.Np, self.N, self.N), dtype=np.complex128)
+        sh = np.zeros((kept, self.Np, 2), dtype=np.int32)
+        tw = np.zeros(kept, dtype=np.int32)
+        _chk(self._l.oracle_merge_finish(self._h, int(n_ref), out.ctypes.data, sh.ctypes.data, tw.ctypes.data), "oracle_merge_finish")
+        return out, sh, tw
 
     def load(self, problem, alpha=(0.6, 0.2), n_ei=1):
         """Convenience: feed a cpra_inputs.Problem."""

@@ -15,7 +15,7 @@ from . import build as _build
 CPRA_OK = 0
 ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_READY, ERR_WORKSPACE, ERR_CUDA, ERR_INVALID_VALUE = -1, -2, -3, -4, -5, -6
 ITERATE, SUPPORTED = 0, 1
-FLAG_DEFAULT, FLAG_FORCE_MULTIPASS, FLAG_NO_CHUNKING = 0, 1, 2
+FLAG_DEFAULT, FLAG_FORCE_MULTIPASS, FLAG_NO_CHUNKING, FLAG_NO_WALK = 0, 1, 2, 4
 MAX_K = 8
 PROFILE_CLASSES = 5
 PROFILE_NAMES = ("row_fwd", "col", "row_inv", "image", "walk")

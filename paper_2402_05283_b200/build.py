@@ -1,9 +1,11 @@
 """Build step of the package: nvcc-compile csrc/ into libcpra.so, in-tree, for sm_100a only.
 
-    python -m paper_2402_05283_b200.build [--force]
+    python -m paper_2402_05283_b200.build [--force] [-v]
 
-nvcc cross-compiles without a GPU.  The library is linked against the static CUDA runtime, so it
-loads (and `cpra_plan` validates arguments) on a box without a driver; compute calls then fail with
+nvcc cross-compiles without a GPU.  The kernels of each image size N are one translation unit
+(csrc/cpra_inst.cu with -DCPRA_INST_N=<N>), compiled in parallel with csrc/cpra_api.cu and linked into
+one shared library.  The library is linked against the static CUDA runtime, so it loads (and
+`cpra_plan` validates arguments) on a box without a driver; compute calls then fail with
 CPRA_ERR_CUDA -- there is no CPU fallback."""
 from __future__ import annotations
 
@@ -12,12 +14,15 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcpra.so")
-SOURCES = [os.path.join(HERE, "csrc", "cpra_api.cu")]
-DEPENDS = SOURCES + [os.path.join(HERE, "csrc", f) for f in ("cpra_fft.cuh", "cpra_kernels.cuh", "cpra_layout.cuh", "cpra_image.cuh", "cpra_walk.cuh")] + [
+SIZES = (16, 32, 64, 128, 256, 512, 1024)
+HEADERS = ["cpra_fft.cuh", "cpra_kernels.cuh", "cpra_layout.cuh", "cpra_image.cuh", "cpra_walk.cuh", "cpra_plan.cuh"]
+DEPENDS = [os.path.join(CSRC, f) for f in ["cpra_api.cu", "cpra_inst.cu"] + HEADERS] + [
     os.path.join(os.path.dirname(HERE), "include", "cpra.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "-cudart", "static"]
 
 
 def needs_build() -> bool:
@@ -28,10 +33,26 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
-        subprocess.check_call(cmd)
+    if not (force or needs_build()):
+        return LIB
+    nvcc = os.environ.get("NVCC", "nvcc")
+    os.makedirs(OBJ, exist_ok=True)
+    extra = ["-Xptxas", "-v"] if verbose else []
+    units = [("cpra_api.o", "cpra_api.cu", [])] + [(f"cpra_inst_{n}.o", "cpra_inst.cu", [f"-DCPRA_INST_N={n}"]) for n in SIZES]
+    procs = []
+    for obj, src, defs in units:
+        cmd = [nvcc] + NVCC_FLAGS + extra + defs + ["-c", "-o", os.path.join(OBJ, obj), os.path.join(CSRC, src)]
+        procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+    failed = None
+    for cmd, pr in procs:
+        out, _ = pr.communicate()
+        if verbose or pr.returncode != 0:
+            sys.stderr.write(out)
+        if pr.returncode != 0 and failed is None:
+            failed = cmd
+    if failed is not None:
+        raise subprocess.CalledProcessError(1, failed)
+    subprocess.check_call([nvcc] + NVCC_FLAGS + ["-shared", "-o", LIB] + [os.path.join(OBJ, u[0]) for u in units])
     return LIB
 
 

@@ -23,6 +23,10 @@
 namespace cpra {
 
 constexpr int MAXK = 8;  // = CPRA_MAX_K
+// sizes and radices of a plan, for the layout kernels of cpra_layout.cuh (runtime, not templated)
+struct Geo {
+    int N, Np, R0, R1, R2, RL, TB;   // TB = transforms per tile (Radix<N>::TB)
+};
 struct MixParams {
     int K;
     float a[MAXK + 1];

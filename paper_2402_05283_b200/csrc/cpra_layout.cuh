@@ -6,9 +6,6 @@
 
 namespace cpra {
 
-struct Geo {
-    int N, Np, R0, R1, R2, RL, TB;   // TB = transforms per tile (Radix<N>::TB)
-};
 // float index of the real part of element (n, y, x) of the row-tiled state; the imaginary part is 2
 // floats further (quad = [re_a, re_b, im_a, im_b])
 __device__ __forceinline__ size_t st_idx(const Geo& g, int n, int y, int x)

@@ -1,0 +1,398 @@
+// cpra_plan.cuh -- the plan object behind include/cpra.h and the per-size launch logic.
+// Host code only decides what to enqueue; every step of the path runs in the kernels of cpra_kernels.cuh
+// / cpra_walk.cuh / cpra_image.cuh.  The kernels of one image size N are instantiated in ONE translation
+// unit (cpra_inst.cu compiled with -DCPRA_INST_N=<N>: `template struct Launch<N>`), so that the sizes
+// build in parallel; cpra_api.cu sees `extern template` declarations only.
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/cpra.h"
+#include <cuda.h>
+
+#include "cpra_image.cuh"
+#include "cpra_walk.cuh"
+
+struct cpra_plan_s {
+    int N = 0, Np = 0;
+    unsigned flags = 0;
+    cudaStream_t stream = nullptr;
+    cpra::Geo geo{};
+    // workspace carve-up
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    float2* tw = nullptr;
+    float* A = nullptr;
+    uint16_t* S16 = nullptr;
+    float4* st[2] = {nullptr, nullptr};
+    float4* scr = nullptr;
+    float4* scr2 = nullptr;   // second spectrum buffer: k_row_walk reads one and writes the other
+    CUtensorMap tm_scr[2];    // TMA descriptors of scr and scr2 for k_row_walk
+    bool have_tmap = false;
+    double* partial = nullptr;
+    double* den = nullptr;
+    double* uphi = nullptr;
+    int* ustart = nullptr;
+    int* rays = nullptr;
+    int cur = 0;
+    // parameters / state
+    int K = 1;
+    float alpha[cpra::MAXK + 1] = {0};
+    int n_ei = 1;
+    int update = CPRA_UPDATE_HIO;
+    long t = 0;
+    bool have_data = false, have_support = false, have_estimate = false, have_error = false;
+    bool attrs_set = false;
+    std::vector<double> angles;
+    std::vector<float2> h_tw;
+    std::vector<double> h_uphi;
+    std::vector<int> h_ustart, h_rays;
+    long launches = 0;
+    int chunk = 0;  // images per L2-resident chunk; 0 = all
+    int sms = 148;     // SMs of the device
+    bool walk = true;  // use k_row_walk where the plan allows it (CPRA_FLAG_NO_WALK switches it off)
+    // per-kernel-class timing (cpra_profile): event pairs around every launch of the loop
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev;      // 2 * PROF_PAIRS events, created on first use
+    std::vector<int> ev_cls;          // class of each recorded pair
+    double prof_ms[CPRA_PROFILE_CLASSES] = {0};
+    long prof_n[CPRA_PROFILE_CLASSES] = {0};
+};
+
+
+namespace cpra {
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Carve {
+    size_t off = 0;
+    size_t take(size_t bytes) { const size_t o = off; off = align256(off + bytes); return o; }
+};
+
+struct Layout {
+    size_t tw, A, S16, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, total;
+};
+
+inline Layout layout_of(int N, int Np)
+{
+    const size_t px = (size_t)Np * N * N;
+    Carve c;
+    Layout L;
+    L.tw = c.take(sizeof(float2) * 1024);   // >= tw_count<N>() for every N
+    L.A = c.take(sizeof(float) * px);
+    L.S16 = c.take(px / 8);
+    L.st0 = c.take(sizeof(float2) * px);
+    L.st1 = c.take(sizeof(float2) * px);
+    L.scr = c.take(sizeof(float2) * px);
+    L.scr2 = c.take(sizeof(float2) * px);
+    L.partial = c.take(sizeof(double) * (size_t)Np * (N / 8));   // >= N / Radix<N>::TB tiles per image
+    L.den = c.take(sizeof(double) * Np);
+    L.uphi = c.take(sizeof(double) * 2 * Np);
+    L.ustart = c.take(sizeof(int) * (2 * (size_t)Np + 1));
+    L.rays = c.take(sizeof(int) * 2 * (size_t)Np);
+    L.total = c.off;
+    return L;
+}
+
+inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// per-stage twiddle tables of cpra_fft.cuh: (wr, wi), w = exp(-2 pi i n2 r / L), computed in double
+// and rounded once
+template <int N>
+void build_twiddles(std::vector<float2>& t)
+{
+    using RX = Radix<N>;
+    const double PI = 3.14159265358979323846264338327950288;
+    t.clear();
+    auto stage = [&](int L, int R) {
+        const int M = L / R;
+        for (int n2 = 0; n2 < M; ++n2)
+            for (int r = 1; r < R; ++r) {
+                const double a = -2.0 * PI * (double)(n2 * r) / (double)L;
+                t.push_back(make_float2((float)std::cos(a), (float)std::sin(a)));
+            }
+    };
+    stage(N, RX::R0);
+    if (RX::S == 3) stage(N / RX::R0, RX::R1);
+    t.resize(1024, make_float2(0.f, 0.f));
+}
+
+// every launch of a size-templated kernel goes through Launch<N> (explicitly instantiated per N)
+template <int N>
+struct Launch {
+    static int set_attrs();
+    static int row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg, float4* ghat_out = nullptr);
+    static int col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, float4* scr = nullptr);
+    static int row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg,
+                       const float4* scr = nullptr, const float4* ghat_in = nullptr);
+    static int walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta, bool fires);
+    static int iterate_walk(cpra_plan_s* p, int k, float beta, float scale);
+    static int image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale);
+};
+
+#define CPRA_DISPATCH_N(N_, ...)                                                     \
+    switch (N_) {                                                                    \
+        case 16:   { constexpr int NN = 16;   __VA_ARGS__; break; }                  \
+        case 32:   { constexpr int NN = 32;   __VA_ARGS__; break; }                  \
+        case 64:   { constexpr int NN = 64;   __VA_ARGS__; break; }                  \
+        case 128:  { constexpr int NN = 128;  __VA_ARGS__; break; }                  \
+        case 256:  { constexpr int NN = 256;  __VA_ARGS__; break; }                  \
+        case 512:  { constexpr int NN = 512;  __VA_ARGS__; break; }                  \
+        case 1024: { constexpr int NN = 1024; __VA_ARGS__; break; }                  \
+        default: return CPRA_ERR_UNSUPPORTED_SIZE;                                   \
+    }
+
+template <class F>
+cudaError_t allow_smem(F* f, int bytes)
+{
+    return cudaFuncSetAttribute(reinterpret_cast<const void*>(f), cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+template <int N>
+int Launch<N>::set_attrs()
+{
+    static_assert(tw_count<N>() <= 1024, "twiddle region of the workspace too small");
+    cudaError_t e = cudaSuccess;
+    auto acc = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    constexpr int SM = smem_bytes<N>();
+    acc(allow_smem(k_row_fwd<N, MIX_NONE>, SM));
+    acc(allow_smem(k_row_fwd<N, MIX_K1>, SM));
+    acc(allow_smem(k_row_fwd<N, MIX_GEN>, SM));
+    acc(allow_smem(k_row_fwd<N, MIX_MASK>, SM));
+    acc(allow_smem(k_col<N, COL_FULL>, SM));
+    acc(allow_smem(k_col<N, COL_FWD>, SM));
+    acc(allow_smem(k_col<N, COL_INV>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_PLAIN, MIX_NONE>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_NONE>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_K1>, SM));
+    acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_GEN>, SM));
+    if constexpr (walk_ok<N>()) acc(allow_smem(k_row_walk<N>, walk_smem_bytes<N>()));
+    if constexpr (N <= 128) {
+        constexpr int ISM = image_smem_bytes<N>();
+        acc(allow_smem(k_image<N, MIX_NONE>, ISM));
+        acc(allow_smem(k_image<N, MIX_K1>, ISM));
+        acc(allow_smem(k_image<N, MIX_GEN>, ISM));
+    }
+    return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+}
+
+inline MixParams mix_params(const cpra_plan_s* p, float beta = 0.f)
+{
+    MixParams mp;
+    mp.K = p->K;
+    for (int j = 0; j <= MAXK; ++j) mp.a[j] = j <= p->K ? p->alpha[j] : 0.f;
+    // coefficients of the update outside the support (cpra_set_update)
+    if (p->update == CPRA_UPDATE_RAAR) { mp.c_ghat = beta; mp.c_gp = 1.0f - 2.0f * beta; }
+    else if (p->update == CPRA_UPDATE_ER) { mp.c_ghat = 0.f; mp.c_gp = 0.f; }
+    else { mp.c_ghat = 1.0f; mp.c_gp = -beta; }
+    return mp;
+}
+
+constexpr int PROF_PAIRS = 2048;
+
+// fold the recorded event pairs into the per-class sums (synchronises the stream)
+inline int prof_drain(cpra_plan_s* p)
+{
+    if (p->ev_cls.empty()) return CPRA_OK;
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    for (size_t i = 0; i < p->ev_cls.size(); ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p->ev[2 * i], p->ev[2 * i + 1]) != cudaSuccess) return CPRA_ERR_CUDA;
+        p->prof_ms[p->ev_cls[i]] += (double)ms;
+        p->prof_n[p->ev_cls[i]] += 1;
+    }
+    p->ev_cls.clear();
+    return CPRA_OK;
+}
+
+struct ProfScope {
+    cpra_plan_s* p;
+    bool on;
+    size_t slot = 0;
+    ProfScope(cpra_plan_s* p_, int cls) : p(p_), on(p_->profiling)
+    {
+        if (!on) return;
+        if (p->ev.empty()) {
+            p->ev.resize(2 * PROF_PAIRS);
+            for (auto& e : p->ev) cudaEventCreate(&e);
+        }
+        if (p->ev_cls.size() == PROF_PAIRS) prof_drain(p);
+        slot = p->ev_cls.size();
+        p->ev_cls.push_back(cls);
+        cudaEventRecord(p->ev[2 * slot], p->stream);
+    }
+    ~ProfScope() { if (on) cudaEventRecord(p->ev[2 * slot + 1], p->stream); }
+};
+
+inline int check_launch(cpra_plan_s* p, int n = 1)
+{
+    p->launches += n;
+    return cudaGetLastError() == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+}
+
+// mix mode of one iteration: does the carousel fire, and which kernel variant serves it
+inline int mix_mode(const cpra_plan_s* p, bool fires)
+{
+    if (!fires) return MIX_NONE;
+    if (p->K == 0) return p->alpha[0] == 1.0f ? MIX_NONE : MIX_GEN;
+    return p->K == 1 ? MIX_K1 : MIX_GEN;
+}
+
+template <int N>
+int Launch<N>::row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg, float4* ghat_out)
+{
+    constexpr int NT = Radix<N>::NT;
+    const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
+    const int smem = smem_bytes<N>();
+    const MixParams mp = mix_params(p);
+    ProfScope prof(p, CPRA_PROFILE_ROW_FWD);
+#define ROWFWD(M) k_row_fwd<N, M><<<grid, NT, smem, p->stream>>>(cur, p->tm_scr[0], p->tw, p->S16, mp, p->Np, n0, nimg, ghat_out)
+    switch (mode) {
+        case MIX_NONE: ROWFWD(MIX_NONE); break;
+        case MIX_K1: ROWFWD(MIX_K1); break;
+        case MIX_GEN: ROWFWD(MIX_GEN); break;
+        default: ROWFWD(MIX_MASK); break;
+    }
+#undef ROWFWD
+    return check_launch(p);
+}
+
+template <int N>
+int Launch<N>::col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, float4* scr)
+{
+    constexpr int NT = Radix<N>::NT;
+    const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
+    const int smem = smem_bytes<N>();
+    ProfScope prof(p, CPRA_PROFILE_COL);
+    if (!scr) scr = p->scr;
+    switch (mode) {
+        case COL_FULL: k_col<N, COL_FULL><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
+        case COL_FWD: k_col<N, COL_FWD><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
+        default: k_col<N, COL_INV><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
+    }
+    return check_launch(p);
+}
+
+template <int N>
+int Launch<N>::row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg,
+                       const float4* scr, const float4* ghat_in)
+{
+    constexpr int NT = Radix<N>::NT;
+    const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
+    const int smem = smem_bytes<N>();
+    const MixParams mp = mix_params(p, beta);
+    ProfScope prof(p, CPRA_PROFILE_ROW_INV);
+    if (!scr) scr = p->scr;
+#define ROWINV(H, M) k_row_inv<N, H, M><<<grid, NT, smem, p->stream>>>(p->tm_scr[scr == p->scr ? 0 : 1], cur, nxt, p->tw, p->S16, mp, beta, scale, p->Np, n0, nimg, ghat_in)
+    if (!hio) ROWINV(ROWINV_PLAIN, MIX_NONE);
+    else if (mode == MIX_NONE) ROWINV(ROWINV_HIO, MIX_NONE);
+    else if (mode == MIX_K1) ROWINV(ROWINV_HIO, MIX_K1);
+    else ROWINV(ROWINV_HIO, MIX_GEN);
+#undef ROWINV
+    return check_launch(p);
+}
+
+// TMA descriptor of a spectrum buffer as the contiguous tensor [n][ct][rt][split][inner floats], box =
+// all column tiles of one row tile (see tma_load_tile).  cuTensorMapEncodeTiled is fetched through the runtime, so that the
+// library does not link against the driver.
+inline bool encode_scratch_tmap(CUtensorMap* tm, void* base, int N, int Np, int tb)
+{
+    typedef CUresult (*Encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t blk = (cuuint64_t)tb * tb * 2, nt = (cuuint64_t)(N / tb);   // floats per block, tiles per side
+    const cuuint64_t inner = blk < 256 ? blk : 256, split = blk / inner;          // box dimensions are limited to 256
+    const cuuint64_t dims[5] = {inner, split, nt, nt, (cuuint64_t)Np};
+    const cuuint64_t strides[4] = {inner * 4, blk * 4, blk * 4 * nt, blk * 4 * nt * nt};
+    const cuuint32_t box[5] = {(cuuint32_t)inner, (cuuint32_t)split, 1u, (cuuint32_t)nt, 1u};
+    const cuuint32_t estr[5] = {1u, 1u, 1u, 1u, 1u};
+    return ((Encode)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// K3 of one iteration fused with K1 of the next (cpra_walk.cuh): 2 CTAs per SM, each a run of tiles
+template <int N>
+int Launch<N>::walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta, bool fires)
+{
+    if constexpr (walk_ok<N>()) {
+        const int total = (N / tile_batch<N>()) * p->Np;
+        const int ctas = std::min(total, 2 * p->sms);
+        const int per = (total + ctas - 1) / ctas;
+        const dim3 grid((unsigned)((total + per - 1) / per));
+        MixParams mp = mix_params(p, beta);
+        if (!fires) { mp.a[0] = 1.0f; mp.a[1] = 0.0f; }   // no mix before the next iteration (n_ei > 1): ghat = g exactly
+        ProfScope prof(p, CPRA_PROFILE_WALK);
+        const CUtensorMap& tin = p->tm_scr[scr_in == p->scr ? 0 : 1];
+        const CUtensorMap& tout = p->tm_scr[scr_out == p->scr ? 0 : 1];
+        k_row_walk<N><<<grid, walk_threads<N>(), walk_smem_bytes<N>(), p->stream>>>(tin, tout, gh_old, gh_new, p->tw, p->S16, mp, beta, p->Np, per);
+        return check_launch(p);
+    } else {
+        return CPRA_ERR_UNSUPPORTED_SIZE;
+    }
+}
+
+// k iterations with the walking kernel: K1 (storing ghat) -> [K2 -> walk] x (k - 1) -> K2 -> K3 (reading ghat).
+// With n_ei > 1 the walk of an iteration that is not followed by a mix runs with weights (1, 0).
+template <int N>
+int Launch<N>::iterate_walk(cpra_plan_s* p, int k, float beta, float scale)
+{
+    float4* g = p->st[p->cur];
+    float4* other = p->st[p->cur ^ 1];
+    auto fires = [&](long t) { return (t % p->n_ei) == 0; };   // does the carousel mix open iteration t (reading A3)
+    int rc = row_fwd(p, g, fires(p->t) ? MIX_K1 : MIX_NONE, 0, p->Np, other);
+    float4 *sin = p->scr, *sout = p->scr2, *gh_old = other, *gh_new = g;
+    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
+        rc = col(p, COL_FULL, 0, p->Np, scale, sin);
+        if (rc != CPRA_OK) break;
+        if (it == k - 1) {
+            rc = row_inv(p, gh_old, gh_new, true, MIX_K1, beta, 1.0f, 0, p->Np, sin, gh_old);
+        } else {
+            rc = walk(p, sin, sout, gh_old, gh_new, beta, fires(p->t + it + 1));
+            std::swap(sin, sout);
+            std::swap(gh_old, gh_new);
+        }
+    }
+    if (rc != CPRA_OK) return rc;
+    p->cur = (gh_new == p->st[0]) ? 0 : 1;
+    p->t += k;
+    p->have_error = true;
+    return CPRA_OK;
+}
+
+// the whole iteration of every projection in one launch (N <= 128, cpra_image.cuh)
+template <int N>
+int Launch<N>::image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale)
+{
+    if constexpr (N <= 128) {
+        constexpr int NT = image_threads<N>(), ISM = image_smem_bytes<N>();
+        const dim3 grid((unsigned)p->Np);
+        const MixParams mp = mix_params(p, beta);
+        ProfScope prof(p, CPRA_PROFILE_IMAGE);
+#define IMG(M) k_image<N, M><<<grid, NT, ISM, p->stream>>>(cur, nxt, p->A, p->tw, p->S16, p->partial, mp, beta, scale, p->Np, 0)
+        if (mode == MIX_NONE) IMG(MIX_NONE);
+        else if (mode == MIX_K1) IMG(MIX_K1);
+        else IMG(MIX_GEN);
+#undef IMG
+        return check_launch(p);
+    } else {
+        return CPRA_ERR_UNSUPPORTED_SIZE;
+    }
+}
+
+#define CPRA_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
+#ifndef CPRA_INST_N
+#define CPRA_EXTERN_LAUNCH(N_) extern template struct Launch<N_>;
+CPRA_FOR_EACH_N(CPRA_EXTERN_LAUNCH)
+#undef CPRA_EXTERN_LAUNCH
+#endif
+
+}  // namespace cpra

@@ -40,6 +40,9 @@ def test_host_only_argument_validation():
     for N in (0, 8, 48, 100, 2048):
         assert L.cpra_plan(ctypes.byref(h), N, 4, 0, None) == cpra.ERR_UNSUPPORTED_SIZE
     assert L.cpra_plan(ctypes.byref(h), 64, 0, 0, None) == cpra.ERR_UNSUPPORTED_SIZE
+    assert L.cpra_plan(ctypes.byref(h), 64, 5, 8, None) == cpra.ERR_INVALID_ARG       # undefined flag bit
+    assert L.cpra_plan(ctypes.byref(h), 64, 5, cpra.FLAG_NO_WALK | cpra.FLAG_NO_CHUNKING, None) == cpra.CPRA_OK
+    assert L.cpra_destroy(h) == cpra.CPRA_OK
     assert L.cpra_plan(ctypes.byref(h), 64, 5, 0, None) == cpra.CPRA_OK
     nb = ctypes.c_size_t()
     assert L.cpra_workspace_bytes(h, ctypes.byref(nb)) == cpra.CPRA_OK

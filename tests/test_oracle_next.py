@@ -1,0 +1,305 @@
+"""Pins for the oracle's SURVEY.md 8(f) functions: the seam of a 180 degree scan and shrink-wrap (f2),
+Step A and Step C (f1), the 3D transform of Step D (f3).  No expected value comes from the oracle
+itself: each test states a closed form, an identity of the forward model, or an independent library
+routine (numpy)."""
+import numpy as np
+
+import cpra_inputs
+from oracle import Oracle, blur, center_of_mass, fft3, mix, mix_seam
+
+
+def _stack(Np, N, seed):
+    rng = np.random.default_rng(seed)
+    return rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))
+
+
+# ---------------------------------------------------------------- f2: seam of a [0, 180) scan
+def test_seam_flip_equals_the_full_turn_carousel():
+    """one rotation axis, so the projection at theta + 180 degrees is the projection at
+    theta mirrored in u.  The first half of a [0, 360) scan of 2 Np angles IS the [0, 180) scan of Np
+    angles; mixing the full-turn stack needs no flip (true periodicity), and its first half must equal
+    the flipped-seam mix of the half-turn stack -- for the generator's projections exactly."""
+    N, Np = 16, 6
+    rng = np.random.default_rng(4)
+    obj = rng.uniform(size=(8, 8, 8))
+    full = cpra_inputs.project(obj, N, 2 * np.pi * np.arange(2 * Np) / (2 * Np))
+    half = full[:Np]
+    # the forward model's symmetry itself (columns 1..N-1 mirror about N/2; column 0 has no partner)
+    assert np.abs(full[Np:, :, 1:] - full[:Np, :, :0:-1]).max() < 1e-12
+    for alpha in ([0.6, 0.2], [0.4, 0.2, 0.1]):
+        want = mix(full, alpha)[:Np]
+        got = mix_seam(half, alpha, 1)
+        assert np.abs(got - want).max() < 1e-12
+        # and the literal wrap (reading A5) differs at the seam projections only
+        lit = mix_seam(half, alpha, 0)
+        K = len(alpha) - 1
+        assert np.abs(lit[K:Np - K] - want[K:Np - K]).max() < 1e-12
+        assert np.abs(lit[0] - want[0]).max() > 1e-3 and np.abs(lit[Np - 1] - want[Np - 1]).max() > 1e-3
+
+
+def test_seam_flip_index_convention_and_loop_use():
+    """One-hot stacks: with the flip, projection 0 receives alpha_1 times projection Np-1 read at column
+    (N - x) mod N (column 0 and the centre column N/2 map to themselves), rows untouched; the loop uses the
+    same mix (M = 0, S = 1: one iteration returns the mixed stack)."""
+    N, Np = 8, 5
+    img = _stack(1, N, 7)[0]
+    mirrored = img[:, (N - np.arange(N)) % N]
+    assert np.array_equal(mirrored[:, 0], img[:, 0]) and np.array_equal(mirrored[:, N // 2], img[:, N // 2])
+    for j, tgt in ((Np - 1, 0), (0, Np - 1)):
+        g = np.zeros((Np, N, N), complex)
+        g[j] = img
+        m = mix_seam(g, [0.6, 0.2], 1)
+        assert np.abs(m[tgt] - 0.2 * mirrored).max() < 1e-15
+        assert np.abs(m[j] - 0.6 * img).max() < 1e-15
+        inner = (j + (1 if j == 0 else -1)) % Np
+        assert np.abs(m[inner] - 0.2 * img).max() < 1e-15          # the neighbour inside the stack: no flip
+        o = Oracle(N, Np)
+        o.set_data(np.ones((Np, N, N)), np.zeros((Np, N, N), np.uint8))
+        o.set_support(np.ones((Np, N, N), np.uint8))
+        o.set_seam(1)
+        o.set_estimate(g)
+        o.iterate(1, 0.9)
+        assert np.abs(o.get_projections(0) - m).max() < 1e-15
+
+
+# ---------------------------------------------------------------- f2: shrink-wrap
+def test_blur_of_a_delta_is_the_periodic_gaussian():
+    N, sig = 32, 2.5            # exp(-2 pi^2 sigma^2 / 4) = 4e-14 at Nyquist: the sampled transfer function is exact
+    a = np.zeros((N, N))
+    a[5, 9] = 2.5
+    b = blur(a, sig)
+    # closed form: the N-periodic sum of a continuous Gaussian of standard deviation sigma, sampled
+    d = N * np.arange(-3, 4)                                        # the periodic images
+    g1 = lambda c: np.array([np.exp(-0.5 * ((i - c + d) / sig) ** 2).sum() for i in range(N)]) / (sig * np.sqrt(2 * np.pi))
+    want = 2.5 * g1(5)[:, None] * g1(9)[None, :]
+    assert np.abs(b - want).max() < 1e-12
+    assert abs(b.sum() - 2.5) < 1e-12                               # mass conserved
+    assert np.abs(blur(a, 0.0) - a).max() < 1e-13                   # sigma = 0: identity
+    # independent library route: numpy's FFT with the same transfer function
+    k = np.fft.fftfreq(N, 1.0 / N)
+    H = np.exp(-2 * np.pi ** 2 * sig ** 2 * (k[:, None] ** 2 + k[None, :] ** 2) / N ** 2)
+    r = np.random.default_rng(2).uniform(size=(N, N))
+    assert np.abs(blur(r, sig) - np.fft.ifft2(np.fft.fft2(r) * H).real).max() < 1e-12
+
+
+def _sw_plan(g, S):
+    Np, N = g.shape[0], g.shape[-1]
+    o = Oracle(N, Np)
+    o.set_data(np.ones((Np, N, N)))
+    o.set_support(S)
+    o.set_estimate(g)
+    return o
+
+
+def test_shrinkwrap_threshold_support_and_idempotence():
+    N, Np = 32, 3
+    rng = np.random.default_rng(9)
+    g = np.zeros((Np, N, N), complex)
+    g[:, 10:20, 8:22] = rng.uniform(0.5, 1.0, size=(Np, 10, 14)) * np.exp(1j * rng.uniform(0, 6, size=(Np, 10, 14)))
+    g[:, 2, 2] = 5.0                                                # a bright pixel OUTSIDE the current support
+    S = np.zeros((Np, N, N), np.uint8)
+    S[:, 6:26, 4:28] = 1
+    # sigma = 0: no blur, the new support is |S g| >= thr max|S g| exactly (the outside pixel is ignored)
+    o = _sw_plan(g, S)
+    o.shrinkwrap(0.0, 0.2)
+    a = np.abs(g) * S
+    want = (a >= 0.2 * a.max(axis=(1, 2), keepdims=True)).astype(np.uint8)
+    assert np.array_equal(o.get_support(), want) and want[:, 2, 2].max() == 0
+    # idempotent on a binary image with sigma = 0
+    ob = _sw_plan(want.astype(complex), want)
+    ob.shrinkwrap(0.0, 0.5)
+    assert np.array_equal(ob.get_support(), want)
+    # with a blur: against numpy's FFT, away from the threshold
+    o = _sw_plan(g, S)
+    b = o.shrinkwrap(1.5, 0.2, want_blurred=True)
+    k = np.fft.fftfreq(N, 1.0 / N)
+    H = np.exp(-2 * np.pi ** 2 * 1.5 ** 2 * (k[:, None] ** 2 + k[None, :] ** 2) / N ** 2)
+    ref = np.fft.ifft2(np.fft.fft2(a) * H).real
+    assert np.abs(b - ref).max() < 1e-12
+    clear = np.abs(ref - 0.2 * ref.max(axis=(1, 2), keepdims=True)) > 1e-9
+    assert np.array_equal(o.get_support()[clear], (ref >= 0.2 * ref.max(axis=(1, 2), keepdims=True))[clear].astype(np.uint8))
+    assert o.get_support().sum() > want.sum()                       # the blur widens the thresholded region
+    # an empty estimate gives an empty support
+    oz = _sw_plan(np.zeros((Np, N, N), complex), S)
+    oz.shrinkwrap(1.0, 0.2)
+    assert oz.get_support().sum() == 0
+
+
+# ---------------------------------------------------------------- f1: Step A
+def test_prereconstruct_is_the_uncoupled_loop_on_one_projection():
+    p = cpra_inputs.make_problem(2, Np=4, N=32)
+    g0 = p.estimate.astype(np.complex128)
+    a = Oracle(p.N, p.Np).load(p)
+    a.prereconstruct(2, 5, 0.9)
+    out = a.get_projections(0)
+    for n in (0, 1, 3):
+        assert np.array_equal(out[n], g0[n])                        # the other projections are untouched
+    assert a.iteration == 0
+    # the same five iterations through the loop with the coupling switched off (K = 0)
+    b = Oracle(p.N, p.Np).load(p, alpha=(1.0,))
+    b.iterate(5, 0.9)
+    assert np.abs(out[2] - b.get_projections(0)[2]).max() <= 1e-13 * np.abs(g0).max()
+    assert np.abs(out[2] - g0[2]).max() > 1e-3 * np.abs(g0).max()
+
+
+# ---------------------------------------------------------------- f1: Step C
+def test_center_of_mass_closed_forms():
+    N = 16
+    a = np.zeros((N, N), complex)
+    a[N // 2 + 3, N // 2 - 5] = 2.0j                                # a delta: its position, whatever its phase
+    assert center_of_mass(a) == (3.0, -5.0)
+    a[N // 2 + 3, N // 2 - 1] = -6.0                                # two masses 2 and 6 on one row
+    cy, cx = center_of_mass(a)
+    assert abs(cy - 3.0) < 1e-15 and abs(cx - (-5 * 2 - 1 * 6) / 8) < 1e-15
+    assert center_of_mass(np.zeros((N, N), complex)) == (0.0, 0.0)
+
+
+def _episode(Np, N, seed):
+    """A compact asymmetric complex blob per projection, centre of mass near the centre pixel."""
+    rng = np.random.default_rng(seed)
+    e = np.zeros((Np, N, N), complex)
+    e[:, N // 2 - 3:N // 2 + 4, N // 2 - 2:N // 2 + 5] = rng.uniform(0.2, 1.0, size=(Np, 7, 7)) * np.exp(1j * rng.uniform(0, 6, size=(Np, 7, 7)))
+    e[:, N // 2 - 3, N // 2 - 2] = 3.0                              # a heavy corner: clearly not centro-symmetric
+    return e
+
+
+def _twin(e):
+    N = e.shape[-1]
+    i = (N - np.arange(N)) % N
+    return np.conj(e[..., i, :][..., :, i])
+
+
+def _merge(episodes, errors, N, Np, NL, n_ref=0):
+    o = Oracle(N, Np)
+    o.merge_begin(NL)
+    for e, E in zip(episodes, errors):
+        o.merge_offer(e, E)
+    return o, o.merge_finish(n_ref)
+
+
+def test_merge_keeps_the_lowest_errors():
+    N, Np = 16, 3
+    eps = [_episode(Np, N, s) for s in range(6)]
+    errs = [0.5, 0.2, 0.9, 0.1, 0.3, 0.05]
+    o = Oracle(N, Np)
+    o.merge_begin(3)
+    for e, E in zip(eps, errs):
+        o.merge_offer(e, E)
+    assert sorted(o.merge_errors()) == [0.05, 0.1, 0.2]             # N_l lowest of N_r
+
+
+def test_merge_of_copies_is_the_identity_and_undoes_shift_twin_and_phase():
+    """Step C on N_l versions of ONE episode that differ exactly by the ambiguities the paper lists
+    (PAPER.md:64 displacement, :70 central inversion) and by the free global phase of an unconstrained
+    iterate: the result is the centred episode itself (averaging equal things is the identity)."""
+    N, Np = 16, 4
+    base = _episode(Np, N, 1)
+    # centre it first (whole pixels), so that "the centred episode" is known in closed form
+    ref = np.empty_like(base)
+    for n in range(Np):
+        cy, cx = center_of_mass(base[n])
+        ref[n] = np.roll(base[n], (-int(np.floor(cy + 0.5)), -int(np.floor(cx + 0.5))), axis=(0, 1))
+        cy, cx = center_of_mass(ref[n])
+        assert abs(cy) <= 0.5 and abs(cx) <= 0.5
+    v1 = np.stack([np.roll(ref[n], (2 - n, n - 1), axis=(0, 1)) for n in range(Np)])        # displaced, per PO
+    v2 = _twin(ref) * np.exp(0.8j)                                                            # twin + phase
+    v3 = np.roll(_twin(ref), (1, -2), axis=(1, 2)) * np.exp(-2.1j)                            # all three
+    o, (out, sh, tw) = _merge([ref, v1, v2, v3], [0.1, 0.2, 0.3, 0.4], N, Np, 4)
+    assert np.abs(out - ref).max() < 1e-13
+    assert list(tw) == [0, 0, 1, 1]
+    assert [tuple(sh[1, n]) for n in range(Np)] == [(-(2 - n), -(n - 1)) for n in range(Np)]
+    assert np.all(sh[0] == 0)
+    # the twin of a centred PO is centred on the same pixel or one off (|com| <= 1/2 flips sign): whole-pixel
+    # shifts of v2 are 0 here because ref's centre of mass is not on a half-pixel
+    # the decision uses ONE PO (n_ref); summed over all POs (n_ref = -1) it is the same here
+    o, (out_all, _, tw_all) = _merge([ref, v1, v2, v3], [0.1, 0.2, 0.3, 0.4], N, Np, 4, n_ref=-1)
+    assert list(tw_all) == [0, 0, 1, 1] and np.abs(out_all - ref).max() < 1e-13
+
+
+def test_merge_distance_zero_to_one_version_positive_to_the_other():
+    """the distance to the best episode is taken for the PO and for its central inversion; for
+    an episode that IS the twin of the best one, the inverted version is at distance 0 and the plain one is
+    not -- and the average of the best episode with its own twin, once corrected, is the best episode."""
+    N, Np = 16, 2
+    ref = _episode(Np, N, 3)
+    for n in range(Np):
+        cy, cx = center_of_mass(ref[n])
+        ref[n] = np.roll(ref[n], (-int(np.floor(cy + 0.5)), -int(np.floor(cx + 0.5))), axis=(0, 1))
+    t = _twin(ref)
+    d_plain = np.linalg.norm(t[0] - ref[0])
+    d_inv = np.linalg.norm(_twin(t)[0] - ref[0])
+    assert d_inv == 0.0 and d_plain > 0.5 * np.linalg.norm(ref[0])
+    _, (out, sh, tw) = _merge([ref, t], [0.1, 0.2], N, Np, 2)
+    assert list(tw) == [0, 1] and np.abs(out - ref).max() < 1e-13
+    # offered the other way round the twin is the best episode and the result is the twin (the ambiguity
+    # is resolved relative to the best episode, not absolutely)
+    _, (out2, _, tw2) = _merge([ref, t], [0.2, 0.1], N, Np, 2)
+    assert list(tw2) == [1, 0] and np.abs(out2 - t).max() < 1e-13
+
+
+def test_merge_averages_different_episodes():
+    N, Np = 16, 2
+    a, b = _episode(Np, N, 5), _episode(Np, N, 6)
+    o, (out, sh, tw) = _merge([a, b], [0.1, 0.2], N, Np, 2)
+    # by hand with numpy: shifts, then twin / phase of b against a on PO 0, then the mean
+    def centred(e):
+        r = np.empty_like(e)
+        for n in range(Np):
+            cy, cx = center_of_mass(e[n])
+            f = lambda c: -int(np.floor(c + 0.5)) if c >= 0 else int(np.floor(-c + 0.5))
+            r[n] = np.roll(e[n], (f(cy), f(cx)), axis=(0, 1))
+        return r
+    ca, cb = centred(a), centred(b)
+    c, ct = np.vdot(ca[0], cb[0]), np.vdot(ca[0], _twin(cb)[0])
+    if abs(ct) > abs(c):
+        cb, c = _twin(cb), ct
+    cb = cb * np.conj(c) / abs(c)
+    assert np.abs(out - 0.5 * (ca + cb)).max() < 1e-13
+    assert abs(np.vdot(ca[0], cb[0]).imag) < 1e-12 and np.vdot(ca[0], cb[0]).real > 0     # phases aligned
+
+
+def test_merge_offer_from_the_plan_takes_the_supported_estimate_and_its_error():
+    p = cpra_inputs.make_problem(2, Np=4, N=32)
+    o = Oracle(p.N, p.Np).load(p)
+    o.iterate(3, 0.9)
+    o.merge_begin(2)
+    o.merge_offer()
+    assert o.merge_errors()[0] == o.get_error()[1]
+    out, sh, tw = o.merge_finish(0)
+    s = o.get_projections(1)
+    want = np.stack([np.roll(s[n], tuple(sh[0, n]), axis=(0, 1)) for n in range(p.Np)])
+    assert np.abs(out - want).max() == 0.0
+
+
+# ---------------------------------------------------------------- f3: 3D transform
+def test_fft3_against_numpy_and_round_trip():
+    for N in (4, 8, 16):
+        rng = np.random.default_rng(N)
+        v = rng.normal(size=(N, N, N)) + 1j * rng.normal(size=(N, N, N))
+        F = fft3(v, -1)
+        assert np.abs(F - np.fft.fftn(v)).max() < 1e-12 * np.abs(F).max()
+        assert np.abs(fft3(F, +1) - v).max() < 1e-13
+    # a delta at (z0, y0, x0): plane wave with the e^{-2 pi i ...} sign on every axis, axes not swapped
+    N = 8
+    d = np.zeros((N, N, N), complex)
+    d[1, 2, 3] = 1.0
+    kz, ky, kx = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    assert np.abs(fft3(d, -1) - np.exp(-2j * np.pi * (1 * kz + 2 * ky + 3 * kx) / N)).max() < 1e-13
+
+
+def test_fft3_of_the_assembled_spectrum_returns_the_object(tiny_problem):
+    """Step D end to end on the oracle: slices of the true projections -> E(q) -> inverse 3D FT ~ the
+    object (up to the interpolation between slices): correlation with the true object close to 1."""
+    p = tiny_problem
+    N = p.N
+    o = Oracle(N, p.Np)
+    o.set_data(np.ones((p.Np, N, N)), None, p.angles)
+    o.set_support(np.ones((p.Np, N, N), np.uint8))
+    o.set_estimate(p.projections)
+    vol, w = o.assemble_3d()
+    rec = fft3(vol, +1)
+    pad = np.zeros((N, N, N))
+    off = (N - p.obj.shape[0]) // 2
+    pad[off:off + p.obj.shape[0], off:off + p.obj.shape[0], off:off + p.obj.shape[0]] = p.obj
+    corr = abs(np.vdot(pad, rec)) / (np.linalg.norm(pad) * np.linalg.norm(rec))
+    assert corr > 0.97, corr
