@@ -191,6 +191,84 @@ int cpra_assemble_3d(cpra_plan_t plan, float* d_vol, float* d_weight);
  */
 int cpra_fft2(cpra_plan_t plan, const float* d_in, float* d_out, int sign);
 
+/* ---------------------------------------------------------------------------------------------------
+ * Around the loop: the steps of the paper's procedure that wrap the iteration.
+ * All of them enqueue on the plan's stream; none synchronises or copies to the host.
+ * ------------------------------------------------------------------------------------------------- */
+
+/*
+ * Seam of a scan over [0, 180 degrees) (reading A5b).  The paper's stack is "periodic" in n
+ * (P:54); with one rotation axis the projection at theta + 180 degrees is the projection at
+ * theta mirrored in u, so true periodicity needs the neighbour that is reached by wrapping round the end
+ * of the stack to be read mirrored: pixel (y, x) of it is taken at (y, (N - x) mod N).  flip = 0 (default):
+ * literal wrap (exact for a [0, 360) scan); flip = 1: mirrored wrap.  Takes effect from the next
+ * cpra_iterate.  Errors: INVALID_ARG.
+ */
+int cpra_set_seam(cpra_plan_t plan, int flip);
+
+/*
+ * Shrink-wrap update of the support ("2D CSWA" ref [35]; "At the end of each episode, we perform
+ * an extra 2D CSWA iteration to obtain a tighter space constraint"; reading A23).  For every n:
+ *     b_n = G_sigma * |S_n g_n|     periodic Gaussian blur, sigma in pixels, of the supported estimate
+ *     S_n <- [ b_n >= threshold * max over the pixels of b_n ]      (empty if that maximum is <= 0)
+ * d_blurred: optional fp32 [Np][N][N], receives b_n (so that a caller can see how close to the threshold a
+ * pixel was); may be NULL.  Uses the FFT scratch and the spare state buffer; the iterate is untouched.
+ * Errors: INVALID_ARG (sigma or threshold negative / not finite), NOT_READY (support or estimate missing), CUDA.
+ */
+int cpra_shrinkwrap(cpra_plan_t plan, float sigma, float threshold, float* d_blurred);
+
+/* The current support as u8 [Np][N][N] (1 = inside).  Errors: INVALID_ARG, NOT_READY, CUDA. */
+int cpra_get_support(cpra_plan_t plan, unsigned char* d_S);
+
+/*
+ * Step A: "Pre-reconstruct a single PO ... via the conventional 2D CXDI algorithm", k iterations of
+ * steps 2-6 of cpra_iterate on projection n alone (no carousel mix: one PO has no neighbours yet).  The other
+ * projections and the iteration counter are untouched; cpra_get_error is NOT_READY until the next cpra_iterate.
+ * Errors: INVALID_ARG (n out of range, k < 0, beta not finite), NOT_READY, WORKSPACE, CUDA.
+ */
+int cpra_prereconstruct(cpra_plan_t plan, int n, int k, float beta);
+
+/*
+ * Step C: "Repeat step A and B multiple times ... We select a certain number N_l < N_r of the best
+ * reconstructed episodes, which have the lowest reconstruction error", align them and average.
+ * The bank of kept episodes lives in a caller-owned DEVICE buffer (cpra_merge_bytes; 256-byte aligned):
+ * N_l stacks of complex fp32 [Np][N][N] plus a few hundred bytes per episode.
+ *   cpra_merge_bind    attach the buffer and empty the bank.
+ *   cpra_merge_offer   offer one episode: d_episode = complex fp32 [Np][N][N] with its error E, or NULL = the
+ *                      plan's own supported estimate S_n g_n with the global error of its last iteration (E
+ *                      ignored; needs an iteration).  It takes a free slot, else replaces the worst kept episode
+ *                      if its error is lower (decided on the device, no host sync).
+ *   cpra_merge_errors  d_E: double [N_l] errors in slot order (first *d_count are valid); d_count: int [1].
+ *   cpra_merge_get     copy the episode of one slot out (for moving banks between GPUs).
+ *   cpra_merge_finish  the merge, in the paper's order (readings A24, A25):
+ *        1. every PO of every kept episode is shifted circularly by a whole number of pixels, -round(com),
+ *           com = sum |O| r / sum |O| about the centre pixel ("we move the mass center of each PO");
+ *        2. against the kept episode of lowest error, on projection n_ref (n_ref = -1: all projections): the
+ *           episode or its twin conj(O(-r)) is taken, whichever has the larger |<O_best, .>| -- the smaller
+ *           Euclidean distance once the free global phase of an unconstrained iterate is taken out -- and is
+ *           multiplied by that unit phase;
+ *        3. d_out [Np][N][N] complex fp32 = the mean of the corrected episodes.
+ *        d_shifts: optional int [N_l][Np][2] (sy, sx); d_twins: optional int [N_l].
+ * Errors: INVALID_ARG, WORKSPACE (buffer too small / misaligned), NOT_READY (no bank bound; offer from the plan
+ * before an iteration), CUDA.
+ */
+int cpra_merge_bytes(cpra_plan_t plan, int n_keep, size_t* bytes);
+int cpra_merge_bind(cpra_plan_t plan, void* d_buf, size_t bytes, int n_keep);
+int cpra_merge_offer(cpra_plan_t plan, const float* d_episode, double E);
+int cpra_merge_errors(cpra_plan_t plan, double* d_E, int* d_count);
+int cpra_merge_get(cpra_plan_t plan, int slot, float* d_episode);
+int cpra_merge_finish(cpra_plan_t plan, int n_ref, float* d_out, int* d_shifts, int* d_twins);
+
+/*
+ * Step D ("performing 3D FTs as a set of 2D FTs"): the 3D transform of a cube, on a plan created
+ * with Np == N.  d_in, d_out: complex fp32 [N][N][N] (z, y, x), natural order, may not alias; sign = -1
+ * forward (unnormalised), +1 inverse (/ N^3).  The (y, x) transforms of the N slices run through the loop's
+ * own kernels (as cpra_fft2), the z lines through one more pass.  With sign = +1 on the output of
+ * cpra_assemble_3d this gives the object O(r) centred at (N/2, N/2, N/2).
+ * Errors: INVALID_ARG (Np != N), WORKSPACE, CUDA.
+ */
+int cpra_fft3(cpra_plan_t plan, const float* d_in, float* d_out, int sign);
+
 /*
  * End-to-end convenience with HOST buffers (pinned memory recommended): uploads the inputs,
  * runs k iterations, downloads the result and synchronises the plan's stream.
@@ -210,6 +288,13 @@ int cpra_reconstruct_host(cpra_plan_t plan, void* d_stage, size_t stage_bytes,
  * intermediate spectrum stays in the 126 MB L2 between the three passes; 0 = one chunk (all images).
  * Results are bit-identical for every chunk size.  Errors: INVALID_ARG. */
 int cpra_set_chunk(cpra_plan_t plan, int images);
+
+/* Tuning knob: run every iteration as ONE launch of the whole-image kernel with each projection spread over
+ * the shared memories of a thread-block cluster of `ctas_per_image` CTAs (1, 2, 4, 8 or 16; N <= 256 and
+ * N / 16 divisible by it; ignored where the plan does not allow it).  0 = the library's own choice (default),
+ * -1 = never.  Results agree with the other kernel paths to rounding (same stages, same arithmetic per pixel).
+ * Errors: INVALID_ARG. */
+int cpra_set_cluster(cpra_plan_t plan, int ctas_per_image);
 
 /*
  * Per-kernel timing for the roofline report (bench.py): while enabled, every kernel launch of

@@ -45,6 +45,18 @@ SIGNATURES = {
     "cpra_profile": (_ci, [_vp, _ci]),
     "cpra_profile_read": (_ci, [_vp, _vp, _vp]),
     "cpra_launch_count": (_ci, [_vp, ctypes.POINTER(_cl)]),
+    "cpra_set_seam": (_ci, [_vp, _ci]),
+    "cpra_set_cluster": (_ci, [_vp, _ci]),
+    "cpra_shrinkwrap": (_ci, [_vp, _cf, _cf, _vp]),
+    "cpra_get_support": (_ci, [_vp, _vp]),
+    "cpra_prereconstruct": (_ci, [_vp, _ci, _ci, _cf]),
+    "cpra_merge_bytes": (_ci, [_vp, _ci, ctypes.POINTER(_sz)]),
+    "cpra_merge_bind": (_ci, [_vp, _vp, _sz, _ci]),
+    "cpra_merge_offer": (_ci, [_vp, _vp, ctypes.c_double]),
+    "cpra_merge_errors": (_ci, [_vp, _vp, _vp]),
+    "cpra_merge_get": (_ci, [_vp, _ci, _vp]),
+    "cpra_merge_finish": (_ci, [_vp, _ci, _vp, _vp, _vp]),
+    "cpra_fft3": (_ci, [_vp, _vp, _vp, _ci]),
     "cpra_destroy": (_ci, [_vp]),
     "cpra_status_string": (ctypes.c_char_p, [_ci]),
 }
@@ -133,6 +145,7 @@ class Plan:
             self._h = _vp()
         self._ws = None
         self._stage = None
+        self._bank = None
 
     def __del__(self):
         try:
@@ -177,6 +190,10 @@ class Plan:
     def set_chunk(self, images: int):
         _chk(self._l.cpra_set_chunk(self._h, int(images)), "cpra_set_chunk")
 
+    def set_cluster(self, ctas_per_image: int):
+        _chk(self._l.cpra_set_cluster(self._h, int(ctas_per_image)), "cpra_set_cluster")
+        return self
+
     def iterate(self, k: int, beta: float = 0.9):
         _chk(self._l.cpra_iterate(self._h, int(k), float(beta)), "cpra_iterate")
 
@@ -212,6 +229,68 @@ class Plan:
         """Real-space update rule: "hio" (default), "raar" or "er"."""
         _chk(self._l.cpra_set_update(self._h, {"hio": 0, "raar": 1, "er": 2}[rule]), "cpra_set_update")
         return self
+
+    # -- around the loop (SURVEY.md 8(f)) -------------------------------------------------------------
+    def set_seam(self, flip: bool):
+        _chk(self._l.cpra_set_seam(self._h, int(bool(flip))), "cpra_set_seam")
+        return self
+
+    def shrinkwrap(self, sigma: float, threshold: float, want_blurred: bool = False):
+        import torch
+        b = torch.empty((self.Np, self.N, self.N), dtype=torch.float32, device=self.device) if want_blurred else None
+        _chk(self._l.cpra_shrinkwrap(self._h, float(sigma), float(threshold), None if b is None else b.data_ptr()), "cpra_shrinkwrap")
+        return b
+
+    def get_support(self):
+        import torch
+        S = torch.empty((self.Np, self.N, self.N), dtype=torch.uint8, device=self.device)
+        _chk(self._l.cpra_get_support(self._h, S.data_ptr()), "cpra_get_support")
+        return S
+
+    def prereconstruct(self, n: int, k: int, beta: float = 0.9):
+        _chk(self._l.cpra_prereconstruct(self._h, int(n), int(k), float(beta)), "cpra_prereconstruct")
+
+    def merge_begin(self, n_keep: int):
+        """Allocate (torch) and bind the bank of the n_keep lowest-error episodes."""
+        import torch
+        nb = _sz()
+        _chk(self._l.cpra_merge_bytes(self._h, int(n_keep), ctypes.byref(nb)), "cpra_merge_bytes")
+        self._bank = torch.empty(int(nb.value), dtype=torch.uint8, device=self.device)
+        self._n_keep = int(n_keep)
+        _chk(self._l.cpra_merge_bind(self._h, _vp(self._bank.data_ptr()), int(nb.value), int(n_keep)), "cpra_merge_bind")
+
+    def merge_offer(self, episode=None, E: float = 0.0):
+        import torch
+        _chk(self._l.cpra_merge_offer(self._h, _dptr(episode, torch.complex64, self._px), float(E)), "cpra_merge_offer")
+
+    def merge_errors(self):
+        """(errors double[n_keep] CUDA tensor in slot order, count int32[1] CUDA tensor)."""
+        import torch
+        E = torch.empty(self._n_keep, dtype=torch.float64, device=self.device)
+        c = torch.empty(1, dtype=torch.int32, device=self.device)
+        _chk(self._l.cpra_merge_errors(self._h, E.data_ptr(), c.data_ptr()), "cpra_merge_errors")
+        return E, c
+
+    def merge_get(self, slot: int):
+        import torch
+        out = torch.empty((self.Np, self.N, self.N), dtype=torch.complex64, device=self.device)
+        _chk(self._l.cpra_merge_get(self._h, int(slot), out.data_ptr()), "cpra_merge_get")
+        return out
+
+    def merge_finish(self, n_ref: int = 0):
+        """(final episode complex64 [Np,N,N], shifts int32 [n_keep,Np,2], twins int32 [n_keep]) on the device."""
+        import torch
+        out = torch.empty((self.Np, self.N, self.N), dtype=torch.complex64, device=self.device)
+        sh = torch.zeros((self._n_keep, self.Np, 2), dtype=torch.int32, device=self.device)
+        tw = torch.zeros(self._n_keep, dtype=torch.int32, device=self.device)
+        _chk(self._l.cpra_merge_finish(self._h, int(n_ref), out.data_ptr(), sh.data_ptr(), tw.data_ptr()), "cpra_merge_finish")
+        return out, sh, tw
+
+    def fft3(self, vol, sign: int = -1):
+        import torch
+        out = torch.empty_like(vol)
+        _chk(self._l.cpra_fft3(self._h, _dptr(vol, torch.complex64, self.N ** 3), out.data_ptr(), int(sign)), "cpra_fft3")
+        return out
 
     def profile(self, enable: bool):
         _chk(self._l.cpra_profile(self._h, int(bool(enable))), "cpra_profile")

@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcpra.so")
 SIZES = (16, 32, 64, 128, 256, 512, 1024)
-HEADERS = ["cpra_fft.cuh", "cpra_kernels.cuh", "cpra_layout.cuh", "cpra_image.cuh", "cpra_walk.cuh", "cpra_plan.cuh"]
+HEADERS = ["cpra_fft.cuh", "cpra_kernels.cuh", "cpra_layout.cuh", "cpra_image.cuh", "cpra_walk.cuh", "cpra_plan.cuh", "cpra_next.cuh", "cpra_cluster.cuh"]
 DEPENDS = [os.path.join(CSRC, f) for f in ["cpra_api.cu", "cpra_inst.cu"] + HEADERS] + [
     os.path.join(os.path.dirname(HERE), "include", "cpra.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

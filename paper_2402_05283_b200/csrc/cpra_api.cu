@@ -3,6 +3,7 @@
 // There is no CPU fallback.
 #include "cpra_plan.cuh"
 #include "cpra_layout.cuh"
+#include "cpra_next.cuh"
 
 using namespace cpra;
 
@@ -36,6 +37,37 @@ void build_rays(cpra_plan_s* p)
         p->h_rays.push_back(rays[i].n | (rays[i].neg << 30));
     }
     p->h_ustart.push_back((int)rays.size());
+}
+
+// the caller-owned bank buffer of Step C, carved up (cpra_merge_bytes states the size)
+struct BankLayout { size_t ep, E, phase, partial, shift, twin, ints, Ein, total; };
+BankLayout bank_layout(int N, int Np, int NL)
+{
+    const size_t px = (size_t)Np * N * N;
+    Carve c;
+    BankLayout L;
+    L.ep = c.take(sizeof(float2) * px * NL);
+    L.E = c.take(sizeof(double) * NL);
+    L.phase = c.take(sizeof(double) * 2 * NL);
+    L.partial = c.take(sizeof(double) * 4 * MERGE_BLOCKS * NL);
+    L.shift = c.take(sizeof(int) * 2 * (size_t)Np * NL);
+    L.twin = c.take(sizeof(int) * NL);
+    L.ints = c.take(sizeof(int) * 4);
+    L.Ein = c.take(sizeof(float) * 2);
+    L.total = c.off;
+    return L;
+}
+Bank bank_of(const cpra_plan_s* p)
+{
+    const BankLayout L = bank_layout(p->N, p->Np, p->bank_NL);
+    char* w = p->bank_buf;
+    Bank b;
+    b.ep = (float2*)(w + L.ep); b.E = (double*)(w + L.E); b.phase = (double*)(w + L.phase);
+    b.partial = (double*)(w + L.partial); b.shift = (int*)(w + L.shift); b.twin = (int*)(w + L.twin);
+    b.count = (int*)(w + L.ints); b.slot = b.count + 1; b.best = b.count + 2;
+    b.Ein = (float*)(w + L.Ein);
+    b.NL = p->bank_NL;
+    return b;
 }
 
 }  // namespace
@@ -121,6 +153,7 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
     p->uphi = (double*)(w + L.uphi);
     p->ustart = (int*)(w + L.ustart);
     p->rays = (int*)(w + L.rays);
+    p->mx = (float*)(w + L.mx);
     p->cur = 0;
     p->have_data = p->have_support = p->have_estimate = p->have_error = false;
     if (!p->attrs_set) {
@@ -223,15 +256,31 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
     // the walking kernel serves the default carousel (K = 1 every iteration) on plans with 8-row tiles
-    if (k > 0 && p->walk && p->have_tmap && chunk == p->Np && p->K == 1 && p->Np >= 3) {
+    if (k > 0 && p->walk && p->cluster <= 0 && p->have_tmap && chunk == p->Np && p->K == 1 && p->Np >= 3) {
         int rc = CPRA_ERR_UNSUPPORTED_SIZE;
         { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, if constexpr (walk_ok<NN>()) rc = Launch<NN>::iterate_walk(p, k, beta, scale)); return 0; }; f(); }
         if (rc != CPRA_ERR_UNSUPPORTED_SIZE) return rc;
+    }
+    // whole-image kernel on a cluster of C CTAs per projection (cpra_set_cluster; cpra_cluster.cuh)
+    int C = p->cluster;
+    if (C > 0) {
+        bool ok = false;
+        { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, ok = Launch<NN>::image_cl_ok(C)); return 0; }; f(); }
+        if (!ok || (p->flags & CPRA_FLAG_FORCE_MULTIPASS) || chunk != p->Np) C = 0;
     }
     for (int it = 0; it < k; ++it) {
         const int mode = mix_mode(p, (p->t % p->n_ei) == 0);
         const float4* cur = p->st[p->cur];
         float4* nxt = p->st[p->cur ^ 1];
+        if (C > 0) {
+            int rc = CPRA_OK;
+            { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::image_cl(p, cur, nxt, mode, beta, scale, C)); return 0; }; f(); }
+            if (rc != CPRA_OK) return rc;
+            p->cur ^= 1;
+            p->t += 1;
+            p->have_error = true;
+            continue;
+        }
         if (p->N <= 128 && !(p->flags & CPRA_FLAG_FORCE_MULTIPASS)) {
             int rc = CPRA_OK;
             { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::image(p, cur, nxt, mode, beta, scale)); return 0; }; f(); }
@@ -341,6 +390,190 @@ int cpra_assemble_3d(cpra_plan_t p, float* d_vol, float* d_weight)
     if (int rc2 = check_launch(p)) return rc2;
     k_assemble<<<grid, 128, 0, p->stream>>>((const float2*)p->scr2, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
     return check_launch(p);
+}
+
+int cpra_set_cluster(cpra_plan_t p, int ctas_per_image)
+{
+    if (!p || ctas_per_image < -1 || ctas_per_image > 16) return CPRA_ERR_INVALID_ARG;
+    p->cluster = ctas_per_image;
+    return CPRA_OK;
+}
+
+int cpra_set_seam(cpra_plan_t p, int flip)
+{
+    if (!p || (flip != 0 && flip != 1)) return CPRA_ERR_INVALID_ARG;
+    p->flip_seam = flip;
+    return CPRA_OK;
+}
+
+int cpra_get_support(cpra_plan_t p, unsigned char* d_S)
+{
+    if (!p || !d_S) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_support) return CPRA_ERR_NOT_READY;
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    k_unpack_support<<<blocks_for(total, 256), 256, 0, p->stream>>>(p->S16, d_S, p->N, total);
+    return check_launch(p);
+}
+
+int cpra_shrinkwrap(cpra_plan_t p, float sigma, float threshold, float* d_blurred)
+{
+    if (!p || !(sigma >= 0.f) || !(threshold >= 0.f) || !std::isfinite(sigma) || !std::isfinite(threshold)) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
+    const size_t total = (size_t)p->Np * p->N * p->N, nquads = total / 2;
+    float4* tmp = p->st[p->cur ^ 1];
+    // |S g| -> forward 2D FT -> Gaussian transfer function -> inverse 2D FT -> per-image maximum -> threshold
+    k_abs_supported<<<blocks_for(nquads, 256), 256, 0, p->stream>>>(p->st[p->cur], p->S16, tmp, p->geo, nquads);
+    int rc = check_launch(p);
+    if (rc) return rc;
+    { auto f = [&]() -> int {
+        CPRA_DISPATCH_N(p->N,
+            rc = Launch<NN>::row_fwd(p, tmp, MIX_NONE, 0, p->Np);
+            if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
+        return 0; }; f(); }
+    if (rc) return rc;
+    k_gauss_filter<<<blocks_for(total, 256), 256, 0, p->stream>>>((float*)p->scr, p->geo, total, sigma);
+    if ((rc = check_launch(p))) return rc;
+    const float scale = 1.0f / ((float)p->N * (float)p->N);
+    { auto f = [&]() -> int {
+        CPRA_DISPATCH_N(p->N,
+            rc = Launch<NN>::col(p, COL_INV, 0, p->Np, 1.0f);
+            if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, tmp, tmp, false, MIX_NONE, 0.f, scale, 0, p->Np));
+        return 0; }; f(); }
+    if (rc) return rc;
+    k_image_max<<<p->Np, 256, 0, p->stream>>>(tmp, p->mx, p->geo);
+    if ((rc = check_launch(p))) return rc;
+    if (d_blurred) {
+        k_unpack_real<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)tmp, d_blurred, p->geo, total);
+        if ((rc = check_launch(p))) return rc;
+    }
+    const size_t total16 = total / 16;
+    k_threshold_pack<<<blocks_for(total16, 256), 256, 0, p->stream>>>((const float*)tmp, p->mx, p->S16, p->geo, total16, threshold);
+    return check_launch(p);
+}
+
+int cpra_prereconstruct(cpra_plan_t p, int n, int k, float beta)
+{
+    if (!p || n < 0 || n >= p->Np || k < 0 || !std::isfinite(beta)) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_data || !p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
+    if (k == 0) return CPRA_OK;
+    const float scale = 1.0f / ((float)p->N * (float)p->N);
+    // the conventional 2D iteration on projection n alone: no mix, the three tile kernels on a one-image grid;
+    // the image ping-pongs between the two state buffers, the other projections stay where they are
+    int rc = CPRA_OK, src = p->cur;
+    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
+        const float4* cur = p->st[src];
+        float4* nxt = p->st[src ^ 1];
+        { auto f = [&]() -> int {
+            CPRA_DISPATCH_N(p->N,
+                rc = Launch<NN>::row_fwd(p, cur, MIX_NONE, n, 1);
+                if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FULL, n, 1, scale);
+                if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, cur, nxt, true, MIX_NONE, beta, 1.0f, n, 1));
+            return 0; }; f(); }
+        src ^= 1;
+    }
+    if (rc) return rc;
+    if (src != p->cur) {
+        const size_t ib = sizeof(float2) * (size_t)p->N * p->N;
+        if (cudaMemcpyAsync((char*)p->st[p->cur] + ib * n, (const char*)p->st[src] + ib * n, ib, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess)
+            return CPRA_ERR_CUDA;
+    }
+    p->have_error = false;   // the error partials of projection n now belong to the pre-reconstruction
+    return CPRA_OK;
+}
+
+int cpra_merge_bytes(cpra_plan_t p, int NL, size_t* bytes)
+{
+    if (!p || !bytes || NL < 1 || NL > 1024) return CPRA_ERR_INVALID_ARG;
+    *bytes = bank_layout(p->N, p->Np, NL).total;
+    return CPRA_OK;
+}
+
+int cpra_merge_bind(cpra_plan_t p, void* d_buf, size_t bytes, int NL)
+{
+    if (!p || !d_buf || NL < 1 || NL > 1024) return CPRA_ERR_INVALID_ARG;
+    const BankLayout L = bank_layout(p->N, p->Np, NL);
+    if (bytes < L.total || ((uintptr_t)d_buf & 255)) return CPRA_ERR_WORKSPACE;
+    p->bank_buf = (char*)d_buf; p->bank_bytes = bytes; p->bank_NL = NL;
+    // everything but the episodes themselves starts at zero (count = 0: the bank is empty)
+    if (cudaMemsetAsync(p->bank_buf + L.E, 0, L.total - L.E, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    return CPRA_OK;
+}
+
+int cpra_merge_offer(cpra_plan_t p, const float* d_episode, double E)
+{
+    if (!p) return CPRA_ERR_INVALID_ARG;
+    if (!p->bank_buf) return CPRA_ERR_NOT_READY;
+    const Bank b = bank_of(p);
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    if (!d_episode) {
+        if (int rc = ready(p)) return rc;
+        if (!p->have_estimate || !p->have_support || !p->have_error) return CPRA_ERR_NOT_READY;
+        k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, nullptr, b.Ein, p->Np, p->N / p->geo.TB);
+        if (int rc = check_launch(p)) return rc;
+        k_offer_select<<<1, 1, 0, p->stream>>>(b, b.Ein, 0.0);
+    } else {
+        if (!std::isfinite(E)) return CPRA_ERR_INVALID_ARG;
+        k_offer_select<<<1, 1, 0, p->stream>>>(b, nullptr, E);
+    }
+    if (int rc = check_launch(p)) return rc;
+    k_offer_copy<<<blocks_for(total, 256), 256, 0, p->stream>>>(b, (const float2*)d_episode, d_episode ? nullptr : (const float*)p->st[p->cur],
+                                                                 p->S16, p->geo, total);
+    return check_launch(p);
+}
+
+int cpra_merge_errors(cpra_plan_t p, double* d_E, int* d_count)
+{
+    if (!p || (!d_E && !d_count)) return CPRA_ERR_INVALID_ARG;
+    if (!p->bank_buf) return CPRA_ERR_NOT_READY;
+    const Bank b = bank_of(p);
+    if (d_E && cudaMemcpyAsync(d_E, b.E, sizeof(double) * p->bank_NL, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    if (d_count && cudaMemcpyAsync(d_count, b.count, sizeof(int), cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    return CPRA_OK;
+}
+
+int cpra_merge_get(cpra_plan_t p, int slot, float* d_episode)
+{
+    if (!p || !d_episode || slot < 0) return CPRA_ERR_INVALID_ARG;
+    if (!p->bank_buf) return CPRA_ERR_NOT_READY;
+    if (slot >= p->bank_NL) return CPRA_ERR_INVALID_ARG;
+    const Bank b = bank_of(p);
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    if (cudaMemcpyAsync(d_episode, b.ep + (size_t)slot * total, sizeof(float2) * total, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    return CPRA_OK;
+}
+
+int cpra_merge_finish(cpra_plan_t p, int n_ref, float* d_out, int* d_shifts, int* d_twins)
+{
+    if (!p || !d_out || n_ref < -1 || n_ref >= p->Np) return CPRA_ERR_INVALID_ARG;
+    if (!p->bank_buf) return CPRA_ERR_NOT_READY;
+    const Bank b = bank_of(p);
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    k_merge_com<<<(unsigned)(p->bank_NL * p->Np), 256, 0, p->stream>>>(b, p->geo);
+    if (int rc = check_launch(p)) return rc;
+    k_merge_best<<<1, 1, 0, p->stream>>>(b);
+    if (int rc = check_launch(p)) return rc;
+    k_merge_inner<<<dim3(MERGE_BLOCKS, (unsigned)p->bank_NL), 256, 0, p->stream>>>(b, p->geo, n_ref);
+    if (int rc = check_launch(p)) return rc;
+    k_merge_decide<<<1, 1024, 0, p->stream>>>(b);
+    if (int rc = check_launch(p)) return rc;
+    k_merge_average<<<blocks_for(total, 256), 256, 0, p->stream>>>(b, (float2*)d_out, p->geo, total);
+    if (int rc = check_launch(p)) return rc;
+    if (d_shifts && cudaMemcpyAsync(d_shifts, b.shift, sizeof(int) * 2 * (size_t)p->Np * p->bank_NL, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    if (d_twins && cudaMemcpyAsync(d_twins, b.twin, sizeof(int) * p->bank_NL, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    return CPRA_OK;
+}
+
+int cpra_fft3(cpra_plan_t p, const float* d_in, float* d_out, int sign)
+{
+    if (!p || !d_in || !d_out || (sign != 1 && sign != -1)) return CPRA_ERR_INVALID_ARG;
+    if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;   // a cube is a stack of N slices of N x N
+    int rc = cpra_fft2(p, d_in, d_out, sign);          // the (y, x) transforms of all z slices
+    if (rc) return rc;
+    { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::fftz(p, (float2*)d_out, sign)); return 0; }; f(); }
+    return rc;
 }
 
 int cpra_host_staging_bytes(cpra_plan_t p, size_t* bytes)

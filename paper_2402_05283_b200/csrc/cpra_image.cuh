@@ -102,7 +102,7 @@ k_image(const float4* __restrict__ cur, float4* __restrict__ nxt, const float* _
         bulk_load(img, cur + (size_t)n * istride, image_bytes<N>(), bar);
         bulk_load(const_cast<float2*>(tw0), twg, tw_bytes<N>(), bar);
     }
-    const MixLoader<MIXMODE> mix(cur, istride, n, Np, mp);
+    const MixLoader<MIXMODE> mix(cur, istride, n, Np, mp, N, TB);
     mbar_wait(bar, 0);
 
     auto ld_row = [&](int t, int p, int j) -> c2 { return from_quad(img[(t * N + p) * NPAIR + j]); };

@@ -33,6 +33,9 @@ struct MixParams {
     // real-space update outside the support: g <- c_ghat ghat + c_gp g'   (HIO: 1, -beta;  RAAR: beta,
     // 1 - 2 beta;  ER: 0, 0;  cpra_set_update).  Inside the support g <- g' for all of them.
     float c_ghat, c_gp;
+    // cpra_set_seam: a neighbour reached by wrapping round the end of the stack is read mirrored in u
+    // (x -> (N - x) mod N about the centre pixel): the seam of a [0, 180) scan, reading A5b
+    int flip_seam;
 };
 // the update outside the support on a pair; with c_ghat = 1 (HIO) the product is exact, so the result
 // is the single fma ghat - beta g'
@@ -79,28 +82,49 @@ struct MixLoader {
     size_t istride;
     int n, Np;
     MixParams mp;
+    int N, tb;          // image size and transforms per tile (for the mirrored read across the seam)
+    bool flm, flp;      // K = 1: the lower / upper neighbour lies across the seam and is read mirrored
 
-    __device__ __forceinline__ MixLoader(const float4* cur, size_t istride_, int n_, int Np_, const MixParams& mp_)
-        : base(cur), istride(istride_), n(n_), Np(Np_), mp(mp_)
+    __device__ __forceinline__ MixLoader(const float4* cur, size_t istride_, int n_, int Np_, const MixParams& mp_, int N_, int tb_)
+        : base(cur), istride(istride_), n(n_), Np(Np_), mp(mp_), N(N_), tb(tb_)
     {
         cm = cur + (size_t)(n_ == 0 ? Np_ - 1 : n_ - 1) * istride_;
         cp = cur + (size_t)(n_ == Np_ - 1 ? 0 : n_ + 1) * istride_;
+        flm = mp_.flip_seam && n_ == 0;
+        flp = mp_.flip_seam && n_ == Np_ - 1;
+    }
+    // quad offset (inside an image, state layout) of the pixel mirrored in x: same row tile and row pair,
+    // position x -> (N - x) mod N
+    __device__ __forceinline__ size_t mirrored(size_t q) const
+    {
+        const int np = tb / 2, tq = N * np;
+        const int loc = (int)(q % (size_t)tq), j = loc % np, x = ppos(loc / np, tb);
+        return q - (size_t)loc + (size_t)(ppos((N - x) & (N - 1), tb) * np + j);
+    }
+    __device__ __forceinline__ c2 ldm(size_t q) const { return from_quad(__ldg(cm + (flm ? mirrored(q) : q))); }
+    __device__ __forceinline__ c2 ldp(size_t q) const { return from_quad(__ldg(cp + (flp ? mirrored(q) : q))); }
+    // general K: image (n + d) mod Np, mirrored if the step d wrapped round the end of the stack
+    __device__ __forceinline__ c2 ldk(int d, size_t q) const
+    {
+        int m = n + d;
+        const bool wrapped = m < 0 || m >= Np;
+        if (m < 0) m += Np;
+        if (m >= Np) m -= Np;
+        return from_quad(__ldg(base + (size_t)m * istride + ((wrapped && mp.flip_seam) ? mirrored(q) : q)));
     }
     // the neighbours' share of the mix at quad q: sum_k a_k (g_{n-k} + g_{n+k}), and its combination
     // with the own quad: a_0 own + nb
     __device__ __forceinline__ c2 nbsum(size_t q) const
     {
         if constexpr (MODE == MIX_K1) {
-            const c2 m = from_quad(__ldg(cm + q)), p = from_quad(__ldg(cp + q));
+            const c2 m = ldm(q), p = ldp(q);
             const float2 a1 = bc(mp.a[1]);
             return c2{pmul(a1, padd(m.re, p.re)), pmul(a1, padd(m.im, p.im))};
         } else if constexpr (MODE == MIX_GEN) {
             c2 acc{make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
             for (int k = 1; k <= mp.K; ++k) {
-                int nm = n - k; if (nm < 0) nm += Np;
-                int np = n + k; if (np >= Np) np -= Np;
-                const c2 m = from_quad(__ldg(base + (size_t)nm * istride + q));
-                const c2 p = from_quad(__ldg(base + (size_t)np * istride + q));
+                const c2 m = ldk(-k, q);
+                const c2 p = ldk(k, q);
                 acc.re = pfma(bc(mp.a[k]), padd(m.re, p.re), acc.re);
                 acc.im = pfma(bc(mp.a[k]), padd(m.im, p.im), acc.im);
             }
@@ -123,16 +147,14 @@ struct MixLoader {
         if constexpr (MODE == MIX_NONE || MODE == MIX_MASK) {
             return own;
         } else if constexpr (MODE == MIX_K1) {
-            const c2 m = from_quad(__ldg(cm + q)), p = from_quad(__ldg(cp + q));
+            const c2 m = ldm(q), p = ldp(q);
             const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]);
             return c2{pfma(a0, own.re, pmul(a1, padd(m.re, p.re))), pfma(a0, own.im, pmul(a1, padd(m.im, p.im)))};
         } else {
             c2 acc{pmul(bc(mp.a[0]), own.re), pmul(bc(mp.a[0]), own.im)};
             for (int k = 1; k <= mp.K; ++k) {
-                int nm = n - k; if (nm < 0) nm += Np;
-                int np = n + k; if (np >= Np) np -= Np;
-                const c2 m = from_quad(__ldg(base + (size_t)nm * istride + q));
-                const c2 p = from_quad(__ldg(base + (size_t)np * istride + q));
+                const c2 m = ldk(-k, q);
+                const c2 p = ldk(k, q);
                 acc.re = pfma(bc(mp.a[k]), padd(m.re, p.re), acc.re);
                 acc.im = pfma(bc(mp.a[k]), padd(m.im, p.im), acc.im);
             }
@@ -328,7 +350,7 @@ k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm
         bulk_load(tile, cur + (size_t)n * istride + toff, tile_bytes<N>(), s.bar);
         bulk_load(const_cast<float2*>(s.tw0), twg, tw_bytes<N>(), s.bar);
     }
-    const MixLoader<MODE> mix(cur, istride, n, Np, mp);
+    const MixLoader<MODE> mix(cur, istride, n, Np, mp, N, TBN);
     const uint16_t* __restrict__ Srow = S16 + ((size_t)n * (N / 16) + (rt * TBN) / 16) * N;   // 16-row words
     const int sshift = (rt * TBN) % 16;
     auto tq = [&](int p, int j) -> int { return ppos<N>(p) * NP + j; };   // quad of (position, pair) in a state tile
@@ -699,7 +721,7 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
             tile[i] = v;
         }
     } else {
-        const MixLoader<MIXMODE> mix(cur, istride, n, Np, mp);
+        const MixLoader<MIXMODE> mix(cur, istride, n, Np, mp, N, TBN);
         const float4* __restrict__ own = cur + (size_t)n * istride + toff;
 #pragma unroll 4
         for (int i = threadIdx.x; i < tile_quads<N>(); i += NT) {
@@ -724,6 +746,53 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
         bulk_store(nxt + (size_t)n * istride + toff, tile, tile_bytes<N>());
         bulk_commit();
         bulk_wait_read0();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// f3: the z pass of the 3D transform of Step D ("3D FTs as a set of 2D
+// FTs"): the 2D transforms of the N slices run through the loop's own row / column kernels; this kernel
+// transforms the z lines of a natural-order cube vol[z][y][x] in place.  One CTA = TB columns x at one y:
+// an [N][TB/2] tile of quads, the same stages as k_col; the forward transform leaves X[k] at position
+// pos(k), so the store (forward) / load (inverse) goes through fft_pos.  One-shot, not on the timed path.
+// ------------------------------------------------------------------------------------------------
+template <int N, bool INV>
+__global__ void __launch_bounds__(Radix<N>::NT)
+k_fft_z(float2* __restrict__ vol, const float2* __restrict__ twg, float scale)
+{
+    using RX = Radix<N>;
+    constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>(), NT = RX::NT, RL = last_radix<N>();
+    extern __shared__ __align__(128) float4 sm[];
+    float4* __restrict__ tile = sm;
+    float2* tw0 = reinterpret_cast<float2*>(sm + tile_quads<N>());
+    const float2* tw1 = tw0 + tw_count_stage0<N>();
+    const int y = blockIdx.y, x0 = blockIdx.x * TBN;
+    float4* __restrict__ v4 = reinterpret_cast<float4*>(vol);   // two complex numbers (re_a, im_a, re_b, im_b)
+    for (int i = threadIdx.x; i < tw_count<N>(); i += NT) tw0[i] = twg[i];
+    for (int i = threadIdx.x; i < N * NP; i += NT) {
+        const int z = i / NP, j = i % NP;
+        const float4 a = v4[(((size_t)z * N + y) * N + x0) / 2 + j];
+        tile[(INV ? fft_pos(z, RX::R0, RX::R1, RX::R2) : z) * NP + j] = make_float4(a.x, a.z, a.y, a.w);
+    }
+    __syncthreads();
+    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NP + j]); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NP + j, v); };
+    if constexpr (!INV) {
+        fft_stage<N, RX::R0, N, false, NT, 1>(tw0, ld_s, st_s);
+        __syncthreads();
+        if constexpr (RX::S == 3) { fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(tw1, ld_s, st_s); __syncthreads(); }
+        fft_stage<N, RL, RL, false, NT, 1>(tw0, ld_s, st_s);
+    } else {
+        fft_stage<N, RL, RL, true, NT, 1>(tw0, ld_s, st_s);
+        __syncthreads();
+        if constexpr (RX::S == 3) { fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(tw1, ld_s, st_s); __syncthreads(); }
+        fft_stage<N, RX::R0, N, true, NT, 1>(tw0, ld_s, st_s);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < N * NP; i += NT) {
+        const int z = i / NP, j = i % NP;
+        const float4 q = tile[(INV ? z : fft_pos(z, RX::R0, RX::R1, RX::R2)) * NP + j];
+        v4[(((size_t)z * N + y) * N + x0) / 2 + j] = make_float4(q.x * scale, q.z * scale, q.y * scale, q.w * scale);
     }
 }
 

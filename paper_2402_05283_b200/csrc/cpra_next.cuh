@@ -1,0 +1,264 @@
+// cpra_next.cuh -- one-off kernels around the loop: shrink-wrap support update (f2), the
+// episode bank and merge of Step C (f1).  Pointwise / reduction work on natural [n][y][x] arrays or through
+// the index helpers of cpra_layout.cuh; none of it is on the timed path.  Reductions run in a fixed order in
+// double precision: every result is deterministic.
+#pragma once
+#include "cpra_layout.cuh"
+
+namespace cpra {
+
+// ---------------------------------------------------------------------------------------------------
+// f2: shrink-wrap (PAPER.md:82 "2D CSWA" ref [35], :104; reading A23)
+//     b_n = G_sigma * |S_n g_n|,   S_n <- [ b_n >= threshold max b_n ]
+// The blur is a product in Fourier space between the loop's own forward and inverse FFT kernels.
+// ---------------------------------------------------------------------------------------------------
+// state -> (|S g|, 0) in the state layout (one thread per quad)
+__global__ void k_abs_supported(const float4* __restrict__ st, const uint16_t* __restrict__ S16, float4* __restrict__ out,
+                                Geo g, size_t nquads)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nquads) return;
+    const int np = g.TB / 2;
+    const size_t pos = i / np;                 // (n * NRT + rt) * N + physical position
+    const int j = (int)(i % np);
+    const int x = ppos((int)(pos % g.N), g.TB);
+    const size_t nrt = pos / g.N;              // n * (N / TB) + rt
+    const int rt = (int)(nrt % (g.N / g.TB));
+    const size_t n = nrt / (g.N / g.TB);
+    const int y0 = rt * g.TB + 2 * j;
+    const unsigned bits = (unsigned)S16[(n * (g.N / 16) + y0 / 16) * g.N + x] >> (y0 % 16);
+    const float4 v = st[i];
+    out[i] = make_float4((bits & 1) ? sqrtf(v.x * v.x + v.z * v.z) : 0.f, (bits & 2) ? sqrtf(v.y * v.y + v.w * v.w) : 0.f, 0.f, 0.f);
+}
+// spectrum (scratch layout) *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2); one thread per natural (n, ky, kx)
+__global__ void k_gauss_filter(float* __restrict__ scr, Geo g, size_t total, float sigma)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = g.N;
+    const int ix = (int)(i % N), iy = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+    const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N;
+    const double s = (double)sigma;
+    const float f = (float)exp(-2.0 * 9.86960440108935861883 * s * s * ((double)ky * ky + (double)kx * kx) / ((double)N * N));
+    const size_t o = sc_idx(g, n, fft_pos(iy, g.R0, g.R1, g.R2), fft_pos(ix, g.R0, g.R1, g.R2));
+    scr[o] *= f;
+    scr[o + 2] *= f;
+}
+// per-image maximum of the real part of a state-layout stack (one block per image)
+__global__ void k_image_max(const float4* __restrict__ st, float* __restrict__ mx, Geo g)
+{
+    const size_t nq = (size_t)g.N * g.N / 2;
+    const float4* __restrict__ p = st + (size_t)blockIdx.x * nq;
+    float m = -3.402823466e38f;
+    for (size_t i = threadIdx.x; i < nq; i += blockDim.x) { const float4 v = p[i]; m = fmaxf(m, fmaxf(v.x, v.y)); }
+    __shared__ float red[32];
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, red[w]);
+        mx[blockIdx.x] = m;
+    }
+}
+// S16 word (n, y / 16, x): bit b = [ b(16 (y/16) + b, x) >= threshold * max_n ], max_n > 0
+__global__ void k_threshold_pack(const float* __restrict__ st, const float* __restrict__ mx, uint16_t* __restrict__ S16,
+                                 Geo g, size_t total16, float threshold)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total16) return;
+    const int N = g.N;
+    const int x = (int)(i % N);
+    const size_t nr = i / N;
+    const int r16 = (int)(nr % (N / 16));
+    const int n = (int)(nr / (N / 16));
+    const float m = mx[n];
+    const float t = threshold * m;
+    unsigned bits = 0;
+    for (int b = 0; b < 16; ++b)
+        if (m > 0.f && st[st_idx(g, n, r16 * 16 + b, x)] >= t) bits |= 1u << b;
+    S16[i] = (uint16_t)bits;
+}
+// bit-packed support -> u8 [n][y][x]
+__global__ void k_unpack_support(const uint16_t* __restrict__ S16, unsigned char* __restrict__ S, int N, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int x = (int)(i % N), y = (int)((i / N) % N);
+    const size_t n = i / ((size_t)N * N);
+    S[i] = (S16[(n * (N / 16) + y / 16) * N + x] >> (y % 16)) & 1;
+}
+// blurred image (real part of a state-layout stack) -> natural float [n][y][x] (diagnostic output of the shrink-wrap)
+__global__ void k_unpack_real(const float* __restrict__ st, float* __restrict__ out, Geo g, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = g.N;
+    out[i] = st[st_idx(g, (int)(i / ((size_t)N * N)), (int)((i / N) % N), (int)(i % N))];
+}
+
+// ---------------------------------------------------------------------------------------------------
+// f1: Step C.  The bank holds the N_l lowest-error episodes offered so far, natural
+// [slot][n][y][x] complex fp32; an episode is the stack of supported estimates S_n g_n.
+// ---------------------------------------------------------------------------------------------------
+struct Bank {
+    float2* ep;        // [NL][Np][N][N]
+    double* E;         // [NL] reconstruction error of the kept episodes
+    int* count;        // [1] episodes kept
+    int* slot;         // [1] slot chosen by the last offer (-1: rejected)
+    float* Ein;        // [2] staging for the offered error when it comes from the plan (E global)
+    int* shift;        // [NL][Np][2] whole-pixel shifts (sy, sx) of the merge
+    double* partial;   // [NL][MERGE_BLOCKS][4] partial inner products (c, c_T)
+    int* twin;         // [NL]
+    double* phase;     // [NL][2] unit factor conj(c)/|c| applied to the episode
+    int* best;         // [1]
+    int NL;
+};
+constexpr int MERGE_BLOCKS = 64;
+
+// the rule of the bank: a free slot, else the worst kept episode if the offer is better (first worst on ties)
+__global__ void k_offer_select(Bank b, const float* __restrict__ E_dev, double E_host)
+{
+    const double E = E_dev ? (double)*E_dev : E_host;
+    int slot = -1;
+    if (*b.count < b.NL) slot = (*b.count)++;
+    else {
+        int w = 0;
+        for (int e = 1; e < b.NL; ++e) if (b.E[e] > b.E[w]) w = e;
+        if (E < b.E[w]) slot = w;
+    }
+    if (slot >= 0) b.E[slot] = E;
+    *b.slot = slot;
+}
+// copy the offered episode into the chosen slot: from a natural array, or from the plan's state (S g)
+__global__ void k_offer_copy(Bank b, const float2* __restrict__ src, const float* __restrict__ st, const uint16_t* __restrict__ S16,
+                             Geo g, size_t total)
+{
+    const int slot = *b.slot;
+    if (slot < 0) return;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    float2 v;
+    if (src) v = src[i];
+    else {
+        const int N = g.N;
+        const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+        v = ld_c(st, st_idx(g, n, y, x));
+        if (!((S16[((size_t)n * (N / 16) + y / 16) * N + x] >> (y % 16)) & 1)) v = make_float2(0.f, 0.f);
+    }
+    b.ep[(size_t)slot * total + i] = v;
+}
+
+__device__ __forceinline__ double block_sum(double v, double* red)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+    for (int w = 0; w < (int)blockDim.x / 32; ++w) s += red[w];
+    return s;
+}
+// centre of mass of |O| about the centre pixel -> whole-pixel shift -round(com) (halves away from zero);
+// one block per (episode, projection).  PAPER.md:64, reading A24.
+__global__ void k_merge_com(Bank b, Geo g)
+{
+    const int e = blockIdx.x / g.Np, n = blockIdx.x % g.Np, N = g.N;
+    if (e >= *b.count) return;
+    __shared__ double red[32];
+    const float2* __restrict__ o = b.ep + ((size_t)e * g.Np + n) * N * N;
+    double m = 0.0, sy = 0.0, sx = 0.0;
+    for (int i = threadIdx.x; i < N * N; i += blockDim.x) {
+        const float2 v = o[i];
+        const double w = sqrt((double)v.x * v.x + (double)v.y * v.y);
+        m += w; sy += w * (double)(i / N - N / 2); sx += w * (double)(i % N - N / 2);
+    }
+    m = block_sum(m, red); sy = block_sum(sy, red); sx = block_sum(sx, red);
+    if (threadIdx.x == 0) {
+        const double cy = m > 0.0 ? sy / m : 0.0, cx = m > 0.0 ? sx / m : 0.0;
+        b.shift[((size_t)e * g.Np + n) * 2] = -(int)(cy >= 0.0 ? floor(cy + 0.5) : -floor(-cy + 0.5));
+        b.shift[((size_t)e * g.Np + n) * 2 + 1] = -(int)(cx >= 0.0 ? floor(cx + 0.5) : -floor(-cx + 0.5));
+    }
+}
+__global__ void k_merge_best(Bank b)
+{
+    int w = 0;
+    for (int e = 1; e < *b.count; ++e) if (b.E[e] < b.E[w]) w = e;
+    *b.best = w;
+}
+__device__ __forceinline__ int wrapi(int a, int N) { return ((a % N) + N) % N; }
+// inner products of the centred best episode with the centred episode e and with its twin T O = conj(O(-r)),
+// on projection n_ref (or all of them, n_ref = -1): grid (MERGE_BLOCKS, NL)
+__global__ void k_merge_inner(Bank b, Geo g, int n_ref)
+{
+    const int e = blockIdx.y, N = g.N, Np = g.Np;
+    if (e >= *b.count) return;
+    const int best = *b.best;
+    __shared__ double red[32];
+    double cr = 0.0, ci = 0.0, tr = 0.0, ti = 0.0;
+    if (e != best) {
+        const int n0 = n_ref < 0 ? 0 : n_ref, n1 = n_ref < 0 ? Np : n_ref + 1;
+        const size_t px = (size_t)N * N, cnt = (size_t)(n1 - n0) * px;
+        const size_t per = (cnt + gridDim.x - 1) / gridDim.x;
+        const size_t i0 = (size_t)blockIdx.x * per, i1 = min(cnt, i0 + per);
+        for (size_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+            const int n = n0 + (int)(i / px), y = (int)((i % px) / N), x = (int)(i % N);
+            const int* sb = b.shift + ((size_t)best * Np + n) * 2;
+            const int* se = b.shift + ((size_t)e * Np + n) * 2;
+            const float2 a = b.ep[((size_t)best * Np + n) * px + (size_t)wrapi(y - sb[0], N) * N + wrapi(x - sb[1], N)];
+            const float2 v = b.ep[((size_t)e * Np + n) * px + (size_t)wrapi(y - se[0], N) * N + wrapi(x - se[1], N)];
+            const float2 w = b.ep[((size_t)e * Np + n) * px + (size_t)wrapi(-y - se[0], N) * N + wrapi(-x - se[1], N)];
+            cr += (double)a.x * v.x + (double)a.y * v.y;
+            ci += (double)a.x * v.y - (double)a.y * v.x;
+            tr += (double)a.x * w.x - (double)a.y * w.y;
+            ti += -(double)a.x * w.y - (double)a.y * w.x;
+        }
+    }
+    cr = block_sum(cr, red); ci = block_sum(ci, red); tr = block_sum(tr, red); ti = block_sum(ti, red);
+    if (threadIdx.x == 0) {
+        double* o = b.partial + ((size_t)e * gridDim.x + blockIdx.x) * 4;
+        o[0] = cr; o[1] = ci; o[2] = tr; o[3] = ti;
+    }
+}
+// twin iff |c_T| > |c|; the episode is multiplied by conj(c)/|c| of the chosen product (reading A25)
+__global__ void k_merge_decide(Bank b)
+{
+    const int e = threadIdx.x;
+    if (e >= *b.count) return;
+    double cr = 0.0, ci = 0.0, tr = 0.0, ti = 0.0;
+    for (int k = 0; k < MERGE_BLOCKS; ++k) {
+        const double* o = b.partial + ((size_t)e * MERGE_BLOCKS + k) * 4;
+        cr += o[0]; ci += o[1]; tr += o[2]; ti += o[3];
+    }
+    int twin = 0;
+    double ur = 1.0, ui = 0.0;
+    if (e != *b.best) {
+        const double mc = sqrt(cr * cr + ci * ci), mt = sqrt(tr * tr + ti * ti);
+        twin = mt > mc;
+        const double m = twin ? mt : mc;
+        if (m > 0.0) { ur = (twin ? tr : cr) / m; ui = -(twin ? ti : ci) / m; }
+    }
+    b.twin[e] = twin;
+    b.phase[2 * e] = ur; b.phase[2 * e + 1] = ui;
+}
+// out_n = mean over the kept episodes of  u_e . (twin_e ? T : 1) shift_e O_e,n   -- one gather, no intermediate
+__global__ void k_merge_average(Bank b, float2* __restrict__ out, Geo g, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = g.N, Np = g.Np, L = *b.count;
+    const size_t px = (size_t)N * N;
+    const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / px);
+    double sr = 0.0, si = 0.0;
+    for (int e = 0; e < L; ++e) {
+        const int* s = b.shift + ((size_t)e * Np + n) * 2;
+        const int tw = b.twin[e];
+        float2 v = b.ep[((size_t)e * Np + n) * px + (size_t)wrapi((tw ? -y : y) - s[0], N) * N + wrapi((tw ? -x : x) - s[1], N)];
+        if (tw) v.y = -v.y;
+        const double ur = b.phase[2 * e], ui = b.phase[2 * e + 1];
+        sr += ur * (double)v.x - ui * (double)v.y;
+        si += ur * (double)v.y + ui * (double)v.x;
+    }
+    out[i] = make_float2((float)(sr / L), (float)(si / L));
+}
+
+}  // namespace cpra

@@ -14,6 +14,7 @@
 #include <cuda.h>
 
 #include "cpra_image.cuh"
+#include "cpra_cluster.cuh"
 #include "cpra_walk.cuh"
 
 struct cpra_plan_s {
@@ -37,12 +38,19 @@ struct cpra_plan_s {
     double* uphi = nullptr;
     int* ustart = nullptr;
     int* rays = nullptr;
+    float* mx = nullptr;      // per-image maxima of the shrink-wrap update
     int cur = 0;
     // parameters / state
     int K = 1;
     float alpha[cpra::MAXK + 1] = {0};
     int n_ei = 1;
     int update = CPRA_UPDATE_HIO;
+    int flip_seam = 0;        // cpra_set_seam
+    int cluster = 0;          // cpra_set_cluster: CTAs per image of the whole-image kernel (0 = library default, -1 = never)
+    // Step C bank (cpra_merge_*): caller-owned device buffer
+    char* bank_buf = nullptr;
+    size_t bank_bytes = 0;
+    int bank_NL = 0;
     long t = 0;
     bool have_data = false, have_support = false, have_estimate = false, have_error = false;
     bool attrs_set = false;
@@ -73,7 +81,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t tw, A, S16, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, total;
+    size_t tw, A, S16, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, mx, total;
 };
 
 inline Layout layout_of(int N, int Np)
@@ -93,6 +101,7 @@ inline Layout layout_of(int N, int Np)
     L.uphi = c.take(sizeof(double) * 2 * Np);
     L.ustart = c.take(sizeof(int) * (2 * (size_t)Np + 1));
     L.rays = c.take(sizeof(int) * 2 * (size_t)Np);
+    L.mx = c.take(sizeof(float) * (size_t)Np);
     L.total = c.off;
     return L;
 }
@@ -131,6 +140,9 @@ struct Launch {
     static int walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta, bool fires);
     static int iterate_walk(cpra_plan_s* p, int k, float beta, float scale);
     static int image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale);
+    static int fftz(cpra_plan_s* p, float2* vol, int sign);
+    static int image_cl(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale, int C);
+    static bool image_cl_ok(int C);
 };
 
 #define CPRA_DISPATCH_N(N_, ...)                                                     \
@@ -149,6 +161,22 @@ template <class F>
 cudaError_t allow_smem(F* f, int bytes)
 {
     return cudaFuncSetAttribute(reinterpret_cast<const void*>(f), cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+template <int N, int C, class ACC>
+void set_attrs_cl(ACC& acc)
+{
+    if constexpr (cl_ok<N, C>()) {
+        constexpr int SMB = cl_smem_bytes<N, C>();
+        acc(allow_smem(k_image_cl<N, C, MIX_NONE>, SMB));
+        acc(allow_smem(k_image_cl<N, C, MIX_K1>, SMB));
+        acc(allow_smem(k_image_cl<N, C, MIX_GEN>, SMB));
+        if constexpr (C > 8) {
+            acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_NONE>), cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_K1>), cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_GEN>), cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        }
+    }
 }
 
 template <int N>
@@ -170,6 +198,9 @@ int Launch<N>::set_attrs()
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_K1>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_GEN>, SM));
     if constexpr (walk_ok<N>()) acc(allow_smem(k_row_walk<N>, walk_smem_bytes<N>()));
+    set_attrs_cl<N, 1>(acc); set_attrs_cl<N, 2>(acc); set_attrs_cl<N, 4>(acc); set_attrs_cl<N, 8>(acc); set_attrs_cl<N, 16>(acc);
+    acc(allow_smem(k_fft_z<N, false>, SM));
+    acc(allow_smem(k_fft_z<N, true>, SM));
     if constexpr (N <= 128) {
         constexpr int ISM = image_smem_bytes<N>();
         acc(allow_smem(k_image<N, MIX_NONE>, ISM));
@@ -188,6 +219,7 @@ inline MixParams mix_params(const cpra_plan_s* p, float beta = 0.f)
     if (p->update == CPRA_UPDATE_RAAR) { mp.c_ghat = beta; mp.c_gp = 1.0f - 2.0f * beta; }
     else if (p->update == CPRA_UPDATE_ER) { mp.c_ghat = 0.f; mp.c_gp = 0.f; }
     else { mp.c_ghat = 1.0f; mp.c_gp = -beta; }
+    mp.flip_seam = p->flip_seam;
     return mp;
 }
 
@@ -386,6 +418,66 @@ int Launch<N>::image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, f
     } else {
         return CPRA_ERR_UNSUPPORTED_SIZE;
     }
+}
+
+// z lines of a natural-order N^3 cube, in place (sign = -1 forward, +1 inverse scaled by 1/N)
+template <int N>
+int Launch<N>::fftz(cpra_plan_s* p, float2* vol, int sign)
+{
+    const dim3 grid((unsigned)(N / tile_batch<N>()), (unsigned)N);
+    if (sign < 0) k_fft_z<N, false><<<grid, Radix<N>::NT, smem_bytes<N>(), p->stream>>>(vol, p->tw, 1.0f);
+    else k_fft_z<N, true><<<grid, Radix<N>::NT, smem_bytes<N>(), p->stream>>>(vol, p->tw, 1.0f / (float)N);
+    return check_launch(p);
+}
+
+// the whole iteration of every projection in one launch, C CTAs per image (cpra_cluster.cuh); cluster launch
+// with programmatic stream serialization (the next launch's prologue overlaps this one's tail)
+template <int N, int C>
+int launch_image_cl(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale)
+{
+    if constexpr (cl_ok<N, C>()) {
+        const MixParams mp = mix_params(p, beta);
+        ProfScope prof(p, CPRA_PROFILE_IMAGE);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)p->Np * C);
+        cfg.blockDim = dim3(cl_threads<N, C>());
+        cfg.dynamicSmemBytes = cl_smem_bytes<N, C>();
+        cfg.stream = p->stream;
+        cudaLaunchAttribute at[2];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 2;
+        float4* gh = p->scr;   // the FFT scratch is free on this path: it holds ghat
+        cudaError_t e;
+        if (mode == MIX_NONE) e = cudaLaunchKernelEx(&cfg, k_image_cl<N, C, MIX_NONE>, cur, nxt, gh, (const float*)p->A, (const float2*)p->tw, (const uint16_t*)p->S16, p->partial, mp, beta, scale, p->Np);
+        else if (mode == MIX_K1) e = cudaLaunchKernelEx(&cfg, k_image_cl<N, C, MIX_K1>, cur, nxt, gh, (const float*)p->A, (const float2*)p->tw, (const uint16_t*)p->S16, p->partial, mp, beta, scale, p->Np);
+        else e = cudaLaunchKernelEx(&cfg, k_image_cl<N, C, MIX_GEN>, cur, nxt, gh, (const float*)p->A, (const float2*)p->tw, (const uint16_t*)p->S16, p->partial, mp, beta, scale, p->Np);
+        p->launches += 1;
+        return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+    } else {
+        return CPRA_ERR_UNSUPPORTED_SIZE;
+    }
+}
+template <int N>
+int Launch<N>::image_cl(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale, int C)
+{
+    switch (C) {
+        case 1: return launch_image_cl<N, 1>(p, cur, nxt, mode, beta, scale);
+        case 2: return launch_image_cl<N, 2>(p, cur, nxt, mode, beta, scale);
+        case 4: return launch_image_cl<N, 4>(p, cur, nxt, mode, beta, scale);
+        case 8: return launch_image_cl<N, 8>(p, cur, nxt, mode, beta, scale);
+        case 16: return launch_image_cl<N, 16>(p, cur, nxt, mode, beta, scale);
+        default: return CPRA_ERR_UNSUPPORTED_SIZE;
+    }
+}
+template <int N>
+bool Launch<N>::image_cl_ok(int C)
+{
+    return (C == 1 && cl_ok<N, 1>()) || (C == 2 && cl_ok<N, 2>()) || (C == 4 && cl_ok<N, 4>()) || (C == 8 && cl_ok<N, 8>()) ||
+           (C == 16 && cl_ok<N, 16>());
 }
 
 #define CPRA_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)

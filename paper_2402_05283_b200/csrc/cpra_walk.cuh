@@ -78,6 +78,9 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     auto i0 = [&](int r) -> int { return o0 + r * (M0 * NP); };
     auto i1 = [&](int r) -> int { return ((r & 1) ? o1o : o1e) + r * (8 * NP); };
     auto iL = [&](int r) -> int { return ((r & 1) ? oLo : oLe) + (r & ~1) * NP; };
+    // the quad of the stage-0 element r of this thread MIRRORED in x (position p -> (N - p) mod N): read for a
+    // halo tile that lies across the seam of a [0, 180) scan (cpra_set_seam, reading A5b)
+    auto i0m = [&](int r) -> int { return ppos<N>((N - (q + M0 * r)) & (N - 1)) * NP + j; };
     static_assert(R0 == 8 && N / R0 == 64, "offsets above assume an 8 x 8 x 8 plan");
     const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]);
 
@@ -207,6 +210,14 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
         // A(0) A(1) A(2) B(1) A(3) B(2) ... A(len + 1) B(len)   (one call site each: both bodies inline)
         for (int i = 0; i <= len + 1; ++i) {
             stepA(i);
+            // a halo tile reached by wrapping round the end of the stack is used mirrored in x
+            const bool mirror = mp.flip_seam && ((i == 0 && na == 0) || (i == len + 1 && nb == Np - 1));
+            if (mirror) {
+                __syncthreads();   // the new state of the halo tile is complete in its slot
+                const float4* const th = sm + (i % 3) * tile_quads<N>();
+#pragma unroll
+                for (int r = 0; r < R0; ++r) v[r] = from_quad(th[i0m(r)]);
+            }
             if (i == 0) {   // the first halo tile is only needed in registers: its slot takes the tile of m_3 at once
 #pragma unroll
                 for (int r = 0; r < R0; ++r) gm[r] = v[r];

@@ -1,0 +1,299 @@
+"""Parity of the steps around the loop (seam of a 180 degree scan, shrink-wrap, Step A,
+Step C, the 3D transform of Step D) with the FP64 oracle, through the C ABI.  Integer outputs (support
+bits, shifts, twin decisions) are compared exactly; where floating point decides a bit, the pixels whose
+value lies within rounding of the threshold are set aside and counted.
+
+Run on the B200 box:  python -m pytest tests -m gpu -x -q"""
+import numpy as np
+import pytest
+
+import cpra_inputs
+from conftest import rel_l2
+
+pytestmark = pytest.mark.gpu
+TOL_1 = 1e-5
+TOL_E = 1e-4
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "the gpu-marked tests need a CUDA device"
+    return torch
+
+
+def _gpu(problem, alpha=(0.6, 0.2), n_ei=1, flags=0):
+    import paper_2402_05283_b200 as cpra
+    return cpra.Plan(problem.N, problem.Np, flags=flags).load(problem, alpha, n_ei)
+
+
+def _oracle(problem, alpha=(0.6, 0.2), n_ei=1):
+    from oracle import Oracle
+    return Oracle(problem.N, problem.Np).load(problem, alpha, n_ei)
+
+
+def _get(plan, which=0):
+    return plan.get_projections(which).cpu().numpy()
+
+
+# ------------------------------------------------------------------------------------------------
+# f2: mirrored wrap at the seam of a [0, 180) scan, every kernel family that evaluates the mix
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,Np,alpha,n_ei,flags", [
+    (64, 7, (0.6, 0.2), 1, 0),            # whole-image kernel, K = 1
+    (128, 6, (0.5, 0.2, 0.05), 1, 0),     # whole-image kernel, K = 2
+    (256, 6, (0.6, 0.2), 1, 0),           # tile kernels
+    (256, 7, (0.4, 0.15, 0.1, 0.05), 2, 0),
+    (512, 7, (0.6, 0.2), 1, 0),           # fused inverse-row / forward-row kernel: mirrored halo tiles
+    (512, 3, (0.6, 0.2), 1, 0),           # every projection is a seam neighbour
+    (512, 7, (0.6, 0.2), 2, 0),
+    (512, 6, (0.6, 0.2), 1, 4),           # CPRA_FLAG_NO_WALK: the tile kernels at N = 512
+    (512, 5, (0.5, 0.2, 0.05), 1, 0),
+    (1024, 3, (0.6, 0.2), 1, 0),
+])
+def test_seam_flip(torch_cuda, N, Np, alpha, n_ei, flags):
+    p = cpra_inputs.random_stack(N, Np, seed=900 + N + Np, beamstop=3)
+    o = _oracle(p, alpha, n_ei).set_seam(1)
+    g = _gpu(p, alpha, n_ei, flags).set_seam(True)
+    lit = _oracle(p, alpha, n_ei)
+    for plan in (o, g, lit):
+        plan.iterate(4, 0.9)
+    ref = o.get_projections(0)
+    assert rel_l2(_get(g), ref) <= 4 * TOL_1
+    assert rel_l2(lit.get_projections(0), ref) > 1e-2                 # the flag matters on this input
+    E, Eg = g.get_error()
+    assert abs(float(Eg.cpu()[0]) - o.get_error()[1]) <= TOL_E * o.get_error()[1]
+    # split calls: K1 / K3 and the fused kernel alternate, bit-identical
+    h = _gpu(p, alpha, n_ei, flags).set_seam(True)
+    for k in (1, 2, 1):
+        h.iterate(k, 0.9)
+    assert np.array_equal(_get(h).view(np.uint32), _get(g).view(np.uint32))
+
+
+def test_seam_flip_on_config_2_and_3(torch_cuda):
+    for cfg, Np in ((2, 12), (3, 6)):
+        p = cpra_inputs.make_problem(cfg, Np=Np)
+        o, g = _oracle(p).set_seam(1), _gpu(p).set_seam(True)
+        o.iterate(3, p.beta)
+        g.iterate(3, p.beta)
+        assert rel_l2(_get(g), o.get_projections(0)) <= 3 * TOL_1, cfg
+
+
+# ------------------------------------------------------------------------------------------------
+# f2: shrink-wrap
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,Np,N", [(1, 8, None), (2, 12, None), (3, 6, None), (4, 4, None), (5, 3, None)])
+def test_shrinkwrap(torch_cuda, cfg, Np, N):
+    p = cpra_inputs.make_problem(cfg, Np=Np, N=N)
+    o, g = _oracle(p), _gpu(p)
+    o.iterate(5, p.beta)
+    g.iterate(5, p.beta)
+    sigma, thr = 2.0, 0.15
+    bo = o.shrinkwrap(sigma, thr, want_blurred=True)
+    bg = g.shrinkwrap(sigma, thr, want_blurred=True).cpu().numpy().astype(np.float64)
+    mx = bo.max(axis=(1, 2), keepdims=True)
+    assert np.abs(bg - bo).max() <= 2e-5 * mx.max()
+    So, Sg = o.get_support(), g.get_support().cpu().numpy()
+    clear = np.abs(bo - thr * mx) > 5e-5 * mx                         # away from the threshold the bit is unique
+    assert np.array_equal(So[clear], Sg[clear])
+    assert (~clear).mean() < 2e-3
+    assert 0 < Sg.sum() < p.support.sum() * 1.5
+    # the loop goes on with the new support: same support on both sides, then two more iterations
+    o.set_support(Sg)
+    o.iterate(2, p.beta)
+    g.iterate(2, p.beta)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 1e-4             # 7 iterations of drift
+    assert rel_l2(_get(g, 1), o.get_projections(1)) <= 1e-4
+
+
+def test_shrinkwrap_sigma_zero_and_empty(torch_cuda):
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(64, 4, seed=71)
+    g = _gpu(p)
+    g.shrinkwrap(0.0, 0.5)
+    a = np.abs(p.estimate) * p.support
+    b = np.abs(a - 0.5 * a.max(axis=(1, 2), keepdims=True)) > 1e-5 * a.max()
+    want = a >= 0.5 * a.max(axis=(1, 2), keepdims=True)
+    assert np.array_equal(g.get_support().cpu().numpy()[b].astype(bool), want[b])
+    z = cpra_inputs.random_stack(64, 4, seed=72)
+    z.estimate[:] = 0
+    g = _gpu(z)
+    g.shrinkwrap(1.0, 0.2)
+    assert int(g.get_support().sum()) == 0
+    with pytest.raises(cpra.CpraError) as e:
+        g.shrinkwrap(-1.0, 0.2)
+    assert e.value.code == cpra.ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------------
+# f1: Step A
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,Np,n,k", [(64, 5, 0, 3), (64, 5, 4, 4), (256, 4, 2, 3), (512, 3, 1, 2), (1024, 2, 1, 1)])
+def test_prereconstruct(torch_cuda, N, Np, n, k):
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(N, Np, seed=500 + N + k, beamstop=3)
+    alpha = (0.6, 0.2) if Np >= 3 else (1.0,)
+    o, g = _oracle(p, alpha), _gpu(p, alpha)
+    o.prereconstruct(n, k, 0.9)
+    g.prereconstruct(n, k, 0.9)
+    out, ref = _get(g), o.get_projections(0)
+    assert rel_l2(out[n], ref[n]) <= k * TOL_1
+    for m in range(Np):
+        if m != n:
+            assert np.array_equal(out[m], p.estimate[m])              # untouched, bit for bit
+    assert g.iteration == 0
+    with pytest.raises(cpra.CpraError) as e:
+        g.get_error()
+    assert e.value.code == cpra.ERR_NOT_READY
+    # Step B follows on the pre-reconstructed stack
+    o.iterate(2, 0.9)
+    g.iterate(2, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= (k + 2) * TOL_1
+
+
+def test_prereconstruct_many_iterations(torch_cuda):
+    """N_i^pre = 200 iterations on PO 0: the same as 200 iterations of the uncoupled loop for that
+    projection (up to the drift of 200 chaotic iterations through different kernels), the others untouched."""
+    p = cpra_inputs.make_problem(1, Np=4)
+    loop = _gpu(p, (1.0,))
+    loop.iterate(201, p.beta)
+    e_loop = loop.get_error()[0].cpu().numpy()
+    one = _gpu(p, (1.0,))
+    one.iterate(1, p.beta)
+    e_one = one.get_error()[0].cpu().numpy()
+    g = _gpu(p, (1.0,))
+    g.prereconstruct(0, 200, p.beta)
+    g.iterate(1, p.beta)
+    e = g.get_error()[0].cpu().numpy()
+    assert abs(e[0] - e_loop[0]) <= 0.05 * e_loop[0] and e[0] > 100 * e_one[0]
+    assert np.array_equal(e[1:], e_one[1:])
+
+
+# ------------------------------------------------------------------------------------------------
+# f1: Step C
+# ------------------------------------------------------------------------------------------------
+def _blob_episode(Np, N, seed):
+    rng = np.random.default_rng(seed)
+    e = np.zeros((Np, N, N), np.complex64)
+    h = N // 2
+    e[:, h - 5:h + 6, h - 4:h + 7] = (rng.uniform(0.2, 1.0, size=(Np, 11, 11)) * np.exp(1j * rng.uniform(0, 6, size=(Np, 11, 11)))).astype(np.complex64)
+    e[:, h - 5, h - 4] = 3.0
+    return e
+
+
+def _twin(e):
+    N = e.shape[-1]
+    i = (N - np.arange(N)) % N
+    return np.conj(e[..., i, :][..., :, i])
+
+
+@pytest.mark.parametrize("N,Np,n_ref", [(32, 3, 0), (64, 5, 2), (64, 4, -1), (256, 2, 1)])
+def test_merge_against_oracle(torch_cuda, N, Np, n_ref):
+    import paper_2402_05283_b200 as cpra
+    from oracle import Oracle
+    base = _blob_episode(Np, N, 1)
+    eps = [base,
+           np.stack([np.roll(base[n], (3 - n, n - 2), axis=(0, 1)) for n in range(Np)]),
+           (_twin(base) * np.exp(0.8j)).astype(np.complex64),
+           _blob_episode(Np, N, 2),
+           (np.roll(_twin(_blob_episode(Np, N, 3)), (2, -3), axis=(1, 2)) * np.exp(-2j)).astype(np.complex64),
+           _blob_episode(Np, N, 4)]
+    errs = [0.30, 0.20, 0.25, 0.10, 0.40, 0.15]
+    o = Oracle(N, Np)
+    o.merge_begin(4)
+    g = cpra.Plan(N, Np)
+    g.merge_begin(4)
+    for e, E in zip(eps, errs):
+        o.merge_offer(e, E)
+        g.merge_offer(torch_cuda.from_numpy(np.ascontiguousarray(e)).cuda(), E)
+    Eg, cnt = g.merge_errors()
+    assert int(cnt.cpu()[0]) == 4 and np.array_equal(Eg.cpu().numpy(), o.merge_errors())     # same slots, same errors
+    out_o, sh_o, tw_o = o.merge_finish(n_ref)
+    out_g, sh_g, tw_g = g.merge_finish(n_ref)
+    assert np.array_equal(sh_g.cpu().numpy(), sh_o) and np.array_equal(tw_g.cpu().numpy(), tw_o)
+    assert tw_o.sum() >= 1 and np.abs(sh_o).sum() > 0
+    assert rel_l2(out_g.cpu().numpy(), out_o) <= 1e-6
+    assert np.array_equal(g.merge_get(1).cpu().numpy(), eps[1])
+
+
+def test_merge_of_restarts_from_the_plan(torch_cuda):
+    """Steps A + B + C on config 1: N_r = 6 random restarts, N_l = 3 kept, each restart pre-reconstructs PO 0
+    and runs the coupled loop; the bank is fed from the plan on the device.  Decisions equal the oracle's;
+    the merged episode agrees to the drift of the iterates it is made of."""
+    import paper_2402_05283_b200 as cpra
+    from oracle import Oracle
+    p = cpra_inputs.make_problem(1, Np=8)
+    g = cpra.Plan(p.N, p.Np).load(p)
+    o = Oracle(p.N, p.Np).load(p)
+    g.merge_begin(3)
+    o.merge_begin(3)
+    for r in range(6):
+        g0 = cpra_inputs.random_phase_estimate(p.intensity, p.mask, r)
+        g.set_estimate(torch_cuda.from_numpy(g0).cuda())
+        o.set_estimate(g0)
+        for plan in (g, o):
+            plan.prereconstruct(0, 6, p.beta)
+            plan.iterate(6, p.beta)
+            plan.merge_offer()
+    Eg, cnt = g.merge_errors()
+    Eo = o.merge_errors()
+    assert int(cnt.cpu()[0]) == 3 and np.abs(Eg.cpu().numpy() - Eo).max() <= TOL_E * Eo.max()
+    out_o, sh_o, tw_o = o.merge_finish(0)
+    out_g, sh_g, tw_g = g.merge_finish(0)
+    assert np.array_equal(tw_g.cpu().numpy(), tw_o)
+    assert (sh_g.cpu().numpy() != sh_o).mean() <= 0.05                  # a centre of mass within 1e-5 of a half pixel may round either way
+    if np.array_equal(sh_g.cpu().numpy(), sh_o):
+        assert rel_l2(out_g.cpu().numpy(), out_o) <= 2e-4
+
+
+# ------------------------------------------------------------------------------------------------
+# f3: the 3D transform of Step D
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [16, 32, 64, 128, 256])
+def test_fft3(torch_cuda, N):
+    import paper_2402_05283_b200 as cpra
+    rng = np.random.default_rng(N)
+    v = (rng.normal(size=(N, N, N)) + 1j * rng.normal(size=(N, N, N))).astype(np.complex64)
+    plan = cpra.Plan(N, N)
+    d = torch_cuda.from_numpy(v).cuda()
+    F = plan.fft3(d, -1)
+    ref = np.fft.fftn(v.astype(np.complex128))
+    assert rel_l2(F.cpu().numpy(), ref) <= 3e-6
+    B = plan.fft3(F, +1).cpu().numpy()
+    assert rel_l2(B, v) <= 4e-6
+    if N <= 64:
+        from oracle import fft3
+        assert rel_l2(F.cpu().numpy(), fft3(v, -1)) <= 3e-6
+    dl = np.zeros((N, N, N), np.complex64)
+    dl[1, 2, 3] = 1.0
+    Fd = plan.fft3(torch_cuda.from_numpy(dl).cuda(), -1).cpu().numpy()
+    kz, ky, kx = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    assert np.abs(Fd - np.exp(-2j * np.pi * (kz + 2 * ky + 3 * kx) / N)).max() < 2e-5
+    with pytest.raises(cpra.CpraError) as e:
+        cpra.Plan(N, N + 1).fft3(d, -1)
+    assert e.value.code in (cpra.ERR_INVALID_ARG,)
+
+
+def test_step_d_assemble_then_inverse_3d(torch_cuda):
+    """Steps D's two transforms chained on the device: slices of the true projections -> E(q) -> O(r),
+    against the same chain on the oracle, and against the object itself (correlation)."""
+    import paper_2402_05283_b200 as cpra
+    from oracle import Oracle, fft3
+    p = cpra_inputs.make_problem(1, keep_object=True, noise=False)
+    N = p.N
+    g = cpra.Plan(N, p.Np)
+    g.set_data(torch_cuda.from_numpy(p.intensity).cuda(), None, p.angles)
+    g.set_support(torch_cuda.ones((p.Np, N, N), dtype=torch_cuda.uint8, device="cuda"))
+    g.set_estimate(torch_cuda.from_numpy(p.projections.astype(np.complex64)).cuda())
+    vol, w = g.assemble_3d()
+    rec = cpra.Plan(N, N).fft3(vol, +1).cpu().numpy()
+    o = Oracle(N, p.Np)
+    o.set_data(np.ones((p.Np, N, N)), None, p.angles)
+    o.set_support(np.ones((p.Np, N, N), np.uint8))
+    o.set_estimate(p.projections.astype(np.complex64))
+    ref = fft3(o.assemble_3d()[0], +1)
+    assert rel_l2(rec, ref) <= 3 * TOL_1
+    pad = np.zeros((N, N, N))
+    off = (N - p.obj.shape[0]) // 2
+    pad[off:off + p.obj.shape[0], off:off + p.obj.shape[0], off:off + p.obj.shape[0]] = p.obj
+    assert abs(np.vdot(pad, rec)) / (np.linalg.norm(pad) * np.linalg.norm(rec)) > 0.97
