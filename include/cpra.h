@@ -296,6 +296,13 @@ int cpra_set_chunk(cpra_plan_t plan, int images);
  * Errors: INVALID_ARG. */
 int cpra_set_cluster(cpra_plan_t plan, int ctas_per_image);
 
+/* Tuning knob: CTAs per SM of the fused inverse-row / forward-row kernel (k_row_walk).  Each CTA walks a run
+ * of consecutive projections for one row tile and transforms the two tiles next to its run a second time, so
+ * more CTAs mean more parallelism and shorter runs (more duplicated work).  0 = the library's choice (default:
+ * 2 at N = 512, 4 at N = 256); values above what registers and shared memory allow only shorten the runs.
+ * Results do not depend on it.  Errors: INVALID_ARG. */
+int cpra_set_walk_ctas(cpra_plan_t plan, int per_sm);
+
 /*
  * Per-kernel timing for the roofline report (bench.py): while enabled, every kernel launch of
  * cpra_iterate is bracketed by CUDA events on the plan's stream, summed per kernel class.

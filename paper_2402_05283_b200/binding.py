@@ -47,6 +47,7 @@ SIGNATURES = {
     "cpra_launch_count": (_ci, [_vp, ctypes.POINTER(_cl)]),
     "cpra_set_seam": (_ci, [_vp, _ci]),
     "cpra_set_cluster": (_ci, [_vp, _ci]),
+    "cpra_set_walk_ctas": (_ci, [_vp, _ci]),
     "cpra_shrinkwrap": (_ci, [_vp, _cf, _cf, _vp]),
     "cpra_get_support": (_ci, [_vp, _vp]),
     "cpra_prereconstruct": (_ci, [_vp, _ci, _ci, _cf]),
@@ -189,6 +190,10 @@ class Plan:
 
     def set_chunk(self, images: int):
         _chk(self._l.cpra_set_chunk(self._h, int(images)), "cpra_set_chunk")
+
+    def set_walk_ctas(self, per_sm: int):
+        _chk(self._l.cpra_set_walk_ctas(self._h, int(per_sm)), "cpra_set_walk_ctas")
+        return self
 
     def set_cluster(self, ctas_per_image: int):
         _chk(self._l.cpra_set_cluster(self._h, int(ctas_per_image)), "cpra_set_cluster")

@@ -268,6 +268,8 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
         { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, ok = Launch<NN>::image_cl_ok(C)); return 0; }; f(); }
         if (!ok || (p->flags & CPRA_FLAG_FORCE_MULTIPASS) || chunk != p->Np) C = 0;
     }
+    bool have_image = false;
+    { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, have_image = Launch<NN>::has_image()); return 0; }; f(); }
     for (int it = 0; it < k; ++it) {
         const int mode = mix_mode(p, (p->t % p->n_ei) == 0);
         const float4* cur = p->st[p->cur];
@@ -281,7 +283,7 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
             p->have_error = true;
             continue;
         }
-        if (p->N <= 128 && !(p->flags & CPRA_FLAG_FORCE_MULTIPASS)) {
+        if (have_image && !(p->flags & CPRA_FLAG_FORCE_MULTIPASS)) {
             int rc = CPRA_OK;
             { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::image(p, cur, nxt, mode, beta, scale)); return 0; }; f(); }
             if (rc != CPRA_OK) return rc;
@@ -396,6 +398,13 @@ int cpra_set_cluster(cpra_plan_t p, int ctas_per_image)
 {
     if (!p || ctas_per_image < -1 || ctas_per_image > 16) return CPRA_ERR_INVALID_ARG;
     p->cluster = ctas_per_image;
+    return CPRA_OK;
+}
+
+int cpra_set_walk_ctas(cpra_plan_t p, int per_sm)
+{
+    if (!p || per_sm < 0 || per_sm > 8) return CPRA_ERR_INVALID_ARG;
+    p->walk_ctas = per_sm;
     return CPRA_OK;
 }
 

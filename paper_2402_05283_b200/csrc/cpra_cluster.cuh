@@ -28,6 +28,10 @@ __device__ __forceinline__ uint32_t cluster_ctarank()
 }
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// arrive without release semantics: for a barrier that only protects shared memory against being OVERWRITTEN
+// after it was read (the reads have returned their values before the arrive is issued), so that the arrive
+// does not wait for this thread's outstanding global stores (ghat)
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 // shared::cta address -> shared::cluster address of the same offset in CTA `rank`
 __device__ __forceinline__ uint32_t mapa(uint32_t a, uint32_t rank)
 {
@@ -52,6 +56,13 @@ template <int N, int C> __host__ __device__ constexpr int cl_tiles() { return (N
 template <int N, int C> __host__ __device__ constexpr int cl_threads() { return cl_tiles<N, C>() * NPAIR * (N / last_radix<N>()); }
 template <int N, int C> __host__ __device__ constexpr int cl_quads() { return cl_tiles<N, C>() * N * NPAIR; }
 template <int N, int C> __host__ __device__ constexpr int cl_smem_bytes() { return cl_quads<N, C>() * 16 + tw_bytes<N>() + 16 + 32 * 4; }
+// CTAs per SM the register allocation is held to: what shared memory allows, at no fewer than 80 registers per thread
+template <int N, int C> __host__ __device__ constexpr int cl_min_blocks()
+{
+    const int by_smem = (220 * 1024) / cl_smem_bytes<N, C>(), by_regs = 65536 / (cl_threads<N, C>() * 80);
+    const int m = by_smem < by_regs ? by_smem : by_regs;
+    return m < 1 ? 1 : (m > 16 ? 16 : m);
+}
 template <int N, int C> __host__ __device__ constexpr bool cl_ok()
 {
     return Radix<N>::S == 2 && tile_batch<N>() == TB && N >= 64 && N <= 256 && C >= 1 && C <= 16 && (N / TB) % C == 0 &&
@@ -85,7 +96,7 @@ __device__ __forceinline__ void cl_stage(const float2* __restrict__ tws, LD ld, 
 }
 
 template <int N, int C, int MIXMODE>
-__global__ void __launch_bounds__(cl_threads<N, C>())
+__global__ void __launch_bounds__(cl_threads<N, C>(), cl_min_blocks<N, C>())
 k_image_cl(const float4* __restrict__ cur, float4* __restrict__ nxt, float4* __restrict__ gh, const float* __restrict__ Aperm,
            const float2* __restrict__ twg, const uint16_t* __restrict__ S16, double* __restrict__ partial,
            MixParams mp, float beta, float scale, int Np)
@@ -145,8 +156,8 @@ k_image_cl(const float4* __restrict__ cur, float4* __restrict__ nxt, float4* __r
         c2 v[RL];
 #pragma unroll
         for (int r = 0; r < RL; ++r) v[r] = ld_row(lt, lq * RL + r, lj);
-        cluster_arrive();                            // this CTA has read its rows ...
-        dft<RL, false>(v);
+        dft<RL, false>(v);                           // (consumes the loads: they have returned)
+        cluster_arrive_relaxed();                    // this CTA has read its rows ...
         cluster_wait();                              // ... and so has every CTA of the cluster: the tiles may be overwritten
 #pragma unroll
         for (int i = 0; i < RL / 2; ++i) {
@@ -201,8 +212,8 @@ k_image_cl(const float4* __restrict__ cur, float4* __restrict__ nxt, float4* __r
             v[2 * i] = c2{make_float2(x.x, y.x), make_float2(x.z, y.z)};
             v[2 * i + 1] = c2{make_float2(x.y, y.y), make_float2(x.w, y.w)};
         }
-        cluster_arrive();                            // this CTA has pulled its pieces ...
-        dft<RL, true>(v);
+        dft<RL, true>(v);                            // (consumes the loads: they have returned)
+        cluster_arrive_relaxed();                    // this CTA has pulled its pieces ...
         cluster_wait();                              // ... and so has every CTA: the tiles may be overwritten
 #pragma unroll
         for (int r = 0; r < RL; ++r) st_row(lt, lq * RL + r, lj, v[r]);

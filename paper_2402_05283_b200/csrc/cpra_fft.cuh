@@ -35,14 +35,17 @@ constexpr int NPAIR = 8;   // batch pairs = quads per position (Radix<N>::TB / 2
 // per SM the register allocation is held to (shared memory allows that many).  PF: k_row_fwd
 // requests the neighbours' share of the mix for all its first-stage butterflies before it waits for its
 // own tile (MINBF = its CTAs per SM: the prefetch needs 2 x 32 more registers).  N = 1024: three CTAs
-// of 256 threads (85 registers, 64 KiB tiles) beat two without a cap (k_col 112 -> 40 B of spills,
+// N = 256 runs the 8-wide 4 x 8 x 8 plan (16 KiB tiles, k_row_walk: 146 -> 120 us per iteration at N_p = 180).  The
+// same 2 x 8 x 8 plan at N = 128 measured 36.9 us against 45.1 us for the whole-image kernel at N_p = 180 and
+// 24.6 against 24.6 at N_p = 90 (config 2); N = 128 stays on the image-resident kernel (cpra_image.cuh).
+// N = 1024: three CTAs of 256 threads (85 registers, 64 KiB tiles) beat two without a cap (k_col 112 -> 40 B of spills,
 // k_row_fwd 128 -> 4 B): 2.498 -> 2.291 ms per iteration at N_p = 180; five instead of four at N = 256: no gain.
 template <int N> struct Radix;
 template <> struct Radix<16>   { static constexpr int TB = 16, S = 2, R0 = 4,  R1 = 4,  R2 = 1, NT = 32,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 template <> struct Radix<32>   { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 4,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 template <> struct Radix<64>   { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 8,  R2 = 1, NT = 64,  MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 template <> struct Radix<128>  { static constexpr int TB = 16, S = 2, R0 = 8,  R1 = 16, R2 = 1, NT = 64,  MINB = 6; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
-template <> struct Radix<256>  { static constexpr int TB = 16, S = 2, R0 = 16, R1 = 16, R2 = 1, NT = 128, MINB = 4; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
+template <> struct Radix<256>  { static constexpr int TB = 8, S = 3, R0 = 4,  R1 = 8,  R2 = 8, NT = 128, MINB = 8; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 template <> struct Radix<512>  { static constexpr int TB = 8, S = 3, R0 = 8,  R1 = 8,  R2 = 8, NT = 128, MINB = 6; static constexpr bool PF = true; static constexpr int MINBF = 4; };
 template <> struct Radix<1024> { static constexpr int TB = 8, S = 3, R0 = 16, R1 = 8,  R2 = 8, NT = 256, MINB = 3; static constexpr bool PF = false; static constexpr int MINBF = MINB; };
 

@@ -84,7 +84,7 @@ k_image(const float4* __restrict__ cur, float4* __restrict__ nxt, const float* _
         MixParams mp, float beta, float scale, int Np, int n0)
 {
     using RX = Radix<N>;
-    static_assert(RX::S == 2, "whole-image kernel: two-stage plans only");
+    static_assert(RX::S == 2 && tile_batch<N>() == TB, "whole-image kernel: 16-wide two-stage plans only");
     constexpr int NT = image_threads<N>(), NRT = N / TB, NCT = N / TB, R0 = RX::R0, RL = RX::R1;
     constexpr int NBFL = NPAIR * (N / RL);   // last-stage butterflies per tile; NT = NRT * NBFL
     extern __shared__ __align__(128) float4 sm[];

@@ -46,6 +46,7 @@ struct cpra_plan_s {
     int n_ei = 1;
     int update = CPRA_UPDATE_HIO;
     int flip_seam = 0;        // cpra_set_seam
+    int walk_ctas = 0;        // cpra_set_walk_ctas: CTAs per SM of the fused row kernel (0 = library default)
     int cluster = 0;          // cpra_set_cluster: CTAs per image of the whole-image kernel (0 = library default, -1 = never)
     // Step C bank (cpra_merge_*): caller-owned device buffer
     char* bank_buf = nullptr;
@@ -130,6 +131,9 @@ void build_twiddles(std::vector<float2>& t)
 }
 
 // every launch of a size-templated kernel goes through Launch<N> (explicitly instantiated per N)
+// the one-CTA-per-image kernel exists for the 16-wide two-stage plans
+template <int N> constexpr bool image_ok() { return N <= 128 && Radix<N>::S == 2 && tile_batch<N>() == TB; }
+
 template <int N>
 struct Launch {
     static int set_attrs();
@@ -143,6 +147,7 @@ struct Launch {
     static int fftz(cpra_plan_s* p, float2* vol, int sign);
     static int image_cl(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale, int C);
     static bool image_cl_ok(int C);
+    static bool has_image() { return image_ok<N>(); }
 };
 
 #define CPRA_DISPATCH_N(N_, ...)                                                     \
@@ -171,6 +176,10 @@ void set_attrs_cl(ACC& acc)
         acc(allow_smem(k_image_cl<N, C, MIX_NONE>, SMB));
         acc(allow_smem(k_image_cl<N, C, MIX_K1>, SMB));
         acc(allow_smem(k_image_cl<N, C, MIX_GEN>, SMB));
+        // cluster launches get the smallest shared-memory carveout that fits ONE block unless told otherwise
+        acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_NONE>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_K1>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_GEN>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         if constexpr (C > 8) {
             acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_NONE>), cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
             acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_image_cl<N, C, MIX_K1>), cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
@@ -201,7 +210,7 @@ int Launch<N>::set_attrs()
     set_attrs_cl<N, 1>(acc); set_attrs_cl<N, 2>(acc); set_attrs_cl<N, 4>(acc); set_attrs_cl<N, 8>(acc); set_attrs_cl<N, 16>(acc);
     acc(allow_smem(k_fft_z<N, false>, SM));
     acc(allow_smem(k_fft_z<N, true>, SM));
-    if constexpr (N <= 128) {
+    if constexpr (image_ok<N>()) {
         constexpr int ISM = image_smem_bytes<N>();
         acc(allow_smem(k_image<N, MIX_NONE>, ISM));
         acc(allow_smem(k_image<N, MIX_K1>, ISM));
@@ -357,7 +366,8 @@ int Launch<N>::walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const
 {
     if constexpr (walk_ok<N>()) {
         const int total = (N / tile_batch<N>()) * p->Np;
-        const int ctas = std::min(total, 2 * p->sms);
+        const int per_sm = p->walk_ctas > 0 ? p->walk_ctas : (N >= 512 ? 2 : 4);   // what the kernel's registers / shared memory allow
+        const int ctas = std::min(total, per_sm * p->sms);
         const int per = (total + ctas - 1) / ctas;
         const dim3 grid((unsigned)((total + per - 1) / per));
         MixParams mp = mix_params(p, beta);
@@ -404,7 +414,7 @@ int Launch<N>::iterate_walk(cpra_plan_s* p, int k, float beta, float scale)
 template <int N>
 int Launch<N>::image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale)
 {
-    if constexpr (N <= 128) {
+    if constexpr (image_ok<N>()) {
         constexpr int NT = image_threads<N>(), ISM = image_smem_bytes<N>();
         const dim3 grid((unsigned)p->Np);
         const MixParams mp = mix_params(p, beta);

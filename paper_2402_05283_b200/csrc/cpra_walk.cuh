@@ -35,7 +35,7 @@ template <int N> __host__ __device__ constexpr int walk_smem_bytes()
 template <int N> __host__ __device__ constexpr int walk_threads() { return tile_pairs<N>() * (N / last_radix<N>()); }
 
 template <int N>
-__global__ void __launch_bounds__(walk_threads<N>(), 2)
+__global__ void __launch_bounds__(walk_threads<N>(), N >= 512 ? 2 : 4)
 k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out, const float4* __restrict__ gh_old,
            float4* __restrict__ gh_new, const float2* __restrict__ twg, const uint16_t* __restrict__ S16,
            MixParams mp, float beta, int Np, int per_cta)
@@ -43,7 +43,10 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     using RX = Radix<N>;
     constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>(), NT = walk_threads<N>();
     constexpr int NRT = N / TBN, NCT = N / TBN, R0 = RX::R0, R1 = RX::R1, RL = RX::R2, M0 = N / R0;
-    static_assert(NP * M0 == NT && NP * (N / R1) == NT && RL == 8, "one butterfly per thread in every stage");
+    // every thread owns E0 = 8 elements of the tile in the first-stage arrangement: B0 butterflies of radix R0
+    // (N = 512: one of radix 8; N = 256: two of radix 4), and one radix-8 butterfly in each inner stage
+    constexpr int QN = NT / NP, B0 = NP * M0 / NT, E0 = B0 * R0;
+    static_assert(B0 * NT == NP * M0 && E0 == 8 && NP * (N / R1) == NT && RL == 8, "8 first-stage elements and one inner butterfly per thread");
     static_assert(NP == 4 && R1 == 8, "the two inner stages of a 64-position block must belong to one warp");
     extern __shared__ __align__(128) float4 sm[];
     float4* const slots = sm;
@@ -69,19 +72,37 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     unsigned phase = 0;   // bit s = parity of the next completion of full[s]
     // Quad offsets of this thread's butterfly in the three stages, as one base (two for the stages
     // whose positions cross 8-blocks of alternating parity, see ppos) plus a compile-time multiple of r:
-    //   stage 0 (stride M0):    p = q + M0 r            ppos(p) = ppos(q) + M0 r
+    //   stage 0 (stride M0):    p = q + QN b + M0 r     ppos(p) = ppos(q) + QN b + M0 r   (element e = R0 b + r)
     //   stage 1 (stride 8):     p = 64 b + n2 + 8 r     ppos(p) = p ^ (r & 1)
     //   last    (contiguous):   p = 8 q + r             ppos(p) = 8 q + (r ^ (q & 1))
     const int o0 = ppos<N>(q) * NP + j;
     const int o1e = ((q / 8) * 64 + (q % 8)) * NP + j, o1o = ((q / 8) * 64 + ((q % 8) ^ 1)) * NP + j;
     const int oLe = (8 * q + (q & 1)) * NP + j, oLo = (8 * q + 1 - (q & 1)) * NP + j;
-    auto i0 = [&](int r) -> int { return o0 + r * (M0 * NP); };
+    auto p0 = [&](int e) -> int { return q + QN * (e / R0) + M0 * (e % R0); };   // position of first-stage element e
+    auto i0 = [&](int e) -> int { return o0 + (e / R0) * (QN * NP) + (e % R0) * (M0 * NP); };
     auto i1 = [&](int r) -> int { return ((r & 1) ? o1o : o1e) + r * (8 * NP); };
     auto iL = [&](int r) -> int { return ((r & 1) ? oLo : oLe) + (r & ~1) * NP; };
     // the quad of the stage-0 element r of this thread MIRRORED in x (position p -> (N - p) mod N): read for a
     // halo tile that lies across the seam of a [0, 180) scan (cpra_set_seam, reading A5b)
-    auto i0m = [&](int r) -> int { return ppos<N>((N - (q + M0 * r)) & (N - 1)) * NP + j; };
-    static_assert(R0 == 8 && N / R0 == 64, "offsets above assume an 8 x 8 x 8 plan");
+    auto i0m = [&](int e) -> int { return ppos<N>((N - p0(e)) & (N - 1)) * NP + j; };
+    static_assert(N / R0 == 64 && QN % 16 == 0, "offsets above assume inner radices 8 x 8 (64-position blocks)");
+    // the B0 first-stage butterflies of this thread (twiddle index n2 = q + QN b)
+    auto stage0_inv = [&](c2 (&a)[E0]) {
+#pragma unroll
+        for (int b = 0; b < B0; ++b) {
+            c2(&u)[R0] = *reinterpret_cast<c2(*)[R0]>(&a[b * R0]);
+            twiddle<R0, true>(u, tw0, q + QN * b);
+            dft<R0, true>(u);
+        }
+    };
+    auto stage0_fwd = [&](c2 (&a)[E0]) {
+#pragma unroll
+        for (int b = 0; b < B0; ++b) {
+            c2(&u)[R0] = *reinterpret_cast<c2(*)[R0]>(&a[b * R0]);
+            dft<R0, false>(u);
+            twiddle<R0, false>(u, tw0, q + QN * b);
+        }
+    };
     const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]);
 
     // issue the loads of projection m's spectrum tile (row tile rt) and support words into slot s
@@ -103,7 +124,7 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
         // A(i): inverse FFT along x + support / HIO of projection proj(i) in slot i % 3.  The last
         // stage and the update happen in registers (ghat_old requested before the tile is waited
         // for); the new state goes back to the slot AND stays in v for the mix of B(i - 1).
-        c2 v[R0];
+        c2 v[E0];
         int pend_tile = -1, pend_slot = 0;   // refill of the slot B stored from, issued one pass into the next A
         auto stepA = [&](int i) {
             const int s = i % 3, m = proj(i);
@@ -111,7 +132,7 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             const float4* __restrict__ gh = gh_old + (size_t)m * istride + (size_t)rt * tile_quads<N>();
             // ghat_old: pulled into L2 now, into registers two passes later (keeps 32 registers free)
 #pragma unroll
-            for (int r = 0; r < R0; ++r) asm volatile("prefetch.global.L2 [%0];" ::"l"(gh + i0(r)));
+            for (int r = 0; r < E0; ++r) asm volatile("prefetch.global.L2 [%0];" ::"l"(gh + i0(r)));
             mbar_wait(full + s, (phase >> s) & 1u);
             phase ^= 1u << s;
             {
@@ -123,9 +144,9 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 for (int r = 0; r < RL; ++r) st_quad(tile + iL(r), w[r]);
             }
             __syncwarp();
-            c2 g0[R0];
+            c2 g0[E0];
 #pragma unroll
-            for (int r = 0; r < R0; ++r) g0[r] = from_quad(__ldg(gh + i0(r)));
+            for (int r = 0; r < E0; ++r) g0[r] = from_quad(__ldg(gh + i0(r)));
             {
                 c2 w[R1];
 #pragma unroll
@@ -142,13 +163,12 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             }
             pend_tile = -1;
 #pragma unroll
-            for (int r = 0; r < R0; ++r) v[r] = from_quad(tile[i0(r)]);
-            twiddle<R0, true>(v, tw0, q);
-            dft<R0, true>(v);
+            for (int r = 0; r < E0; ++r) v[r] = from_quad(tile[i0(r)]);
+            stage0_inv(v);
             const uint16_t* __restrict__ sp = sup + s * N;
 #pragma unroll
-            for (int r = 0; r < R0; ++r) {
-                const unsigned bits = (unsigned)sp[q + M0 * r] >> (sshift + 2 * j);
+            for (int r = 0; r < E0; ++r) {
+                const unsigned bits = (unsigned)sp[p0(r)] >> (sshift + 2 * j);
                 const float2 ore = update_outside(mp, v[r].re, g0[r].re), oim = update_outside(mp, v[r].im, g0[r].im);
                 v[r].re = make_float2((bits & 1) ? v[r].re.x : ore.x, (bits & 2) ? v[r].re.y : ore.y);
                 v[r].im = make_float2((bits & 1) ? v[r].im.x : oim.x, (bits & 2) ? v[r].im.y : oim.y);
@@ -159,25 +179,24 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
         // B(i): ghat_new(m_i) from gm (registers: g_new(m_{i-1})), slot i % 3 (g_new(m_i)) and v
         // (registers: g_new(m_{i+1})); forward FFT along x in place in slot i % 3, store; refill it
         // with the tile of m_{i+3}.  The quads read from the slot become the next gm.
-        c2 gm[R0];
+        c2 gm[E0];
         auto stepB = [&](int i) {
             const int m = proj(i), s0 = i % 3;
             float4* const t0 = sm + s0 * tile_quads<N>();
             float4* __restrict__ gout = gh_new + (size_t)m * istride + (size_t)rt * tile_quads<N>();
             {
-                c2 w[R0];
+                c2 w[E0];
 #pragma unroll
-                for (int r = 0; r < R0; ++r) {
+                for (int r = 0; r < E0; ++r) {
                     const int i2 = i0(r);
                     const c2 own = from_quad(t0[i2]);
                     w[r] = c2{pfma(a0, own.re, pmul(a1, padd(gm[r].re, v[r].re))), pfma(a0, own.im, pmul(a1, padd(gm[r].im, v[r].im)))};
                     gm[r] = own;
                     gout[i2] = to_quad(w[r]);
                 }
-                dft<R0, false>(w);
-                twiddle<R0, false>(w, tw0, q);
+                stage0_fwd(w);
 #pragma unroll
-                for (int r = 0; r < R0; ++r) st_quad(t0 + i0(r), w[r]);
+                for (int r = 0; r < E0; ++r) st_quad(t0 + i0(r), w[r]);
             }
             __syncthreads();
             {
@@ -216,11 +235,11 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 __syncthreads();   // the new state of the halo tile is complete in its slot
                 const float4* const th = sm + (i % 3) * tile_quads<N>();
 #pragma unroll
-                for (int r = 0; r < R0; ++r) v[r] = from_quad(th[i0m(r)]);
+                for (int r = 0; r < E0; ++r) v[r] = from_quad(th[i0m(r)]);
             }
             if (i == 0) {   // the first halo tile is only needed in registers: its slot takes the tile of m_3 at once
 #pragma unroll
-                for (int r = 0; r < R0; ++r) gm[r] = v[r];
+                for (int r = 0; r < E0; ++r) gm[r] = v[r];
                 __syncthreads();   // every thread is done with slot 0
                 if (io && 3 <= len + 1) load_tile(proj(3), rt, 0);
             }
