@@ -270,6 +270,22 @@ int cpra_merge_finish(cpra_plan_t plan, int n_ref, float* d_out, int* d_shifts, 
 int cpra_fft3(cpra_plan_t plan, const float* d_in, float* d_out, int sign);
 
 /*
+ * Step D's iterations ("a tomographic approach, which is like conventional 3D CXDI but using E(q) ... a
+ * single random guess and N_i^3D (around 50) iterations are sufficient [32]"; reading A26), on a plan
+ * created with Np == N.  With F = E on the voxels the slices cover (d_W > 0) and 0 elsewhere, k times:
+ *     O = S3 . F3^-1[F];   F' = F3[O];   err_it = sqrt(sum_{W>0} |F' - E|^2 / sum_{W>0} |E|^2);   F = W > 0 ? E : F'
+ *   d_E   complex fp32 [N][N][N], the assembled spectrum (cpra_assemble_3d's d_vol)
+ *   d_W   fp32 [N][N][N], > 0 where E is known (cpra_assemble_3d's d_weight)
+ *   d_S3  u8 [N][N][N], the 3D support (1 = inside), in the object's frame (centre at (N/2, N/2, N/2))
+ *   d_obj complex fp32 [N][N][N] out: the object after the last support step
+ *   d_err fp32 [k] out or NULL
+ * Uses the plan's state buffers as scratch: a loop state held by this plan is lost (Step D runs on its own plan).
+ * Errors: INVALID_ARG (Np != N, k < 1, NULL), WORKSPACE, CUDA.
+ */
+int cpra_refine_3d(cpra_plan_t plan, const float* d_E, const float* d_W, const unsigned char* d_S3, int k,
+                   float* d_obj, float* d_err);
+
+/*
  * End-to-end convenience with HOST buffers (pinned memory recommended): uploads the inputs,
  * runs k iterations, downloads the result and synchronises the plan's stream.
  *   h_I [Np][N][N] fp32, h_mask [Np][N][N] u8 or NULL, h_angles [Np] or NULL, h_S [Np][N][N] u8,

@@ -942,4 +942,44 @@ int oracle_fft3(const double* in, double* out, int N, int sign)
     return ORACLE_OK;
 }
 
+/* Step D's iterations ("We proceed with a tomographic approach, which is like conventional 3D CXDI but
+ * using E(q) obtained via the steps A-C ... Typically, only a single random guess and N_i^3D (around 50)
+ * iterations are sufficient [32]"; ref [32] alternates between the known Fourier samples and the real-space
+ * constraint).  Reading A26: with F_0 = E on the known voxels (W > 0) and 0 elsewhere, k times
+ *     O    = S3 . F3^-1[F]                          real-space constraint: the 3D support (no positivity: complex O)
+ *     F'   = F3[O]
+ *     err  = sqrt( sum_{W>0} |F' - E|^2 / sum_{W>0} |E|^2 )
+ *     F    = E where W > 0, F' elsewhere            the assembled spectrum is put back on the voxels it covers
+ * E: interleaved complex double [N][N][N] (native order, as oracle_assemble_3d writes it), W: double [N][N][N],
+ * S3: u8 [N][N][N]; obj (out): the object after the last support step; err (optional): k doubles. */
+int oracle_refine_3d(const double* E, const double* W, const unsigned char* S3, int N, int k, double* obj, double* err)
+{
+    if (!E || !W || !S3 || !obj || !is_pow2(N) || k < 1) return ORACLE_ERR_INVALID_ARG;
+    const size_t n3 = (size_t)N * N * N;
+    double* F = (double*)malloc(sizeof(double) * 2 * n3);
+    double* T = (double*)malloc(sizeof(double) * 2 * n3);
+    double den = 0.0;
+    for (size_t i = 0; i < n3; ++i) {
+        const int known = W[i] > 0.0;
+        F[2 * i] = known ? E[2 * i] : 0.0; F[2 * i + 1] = known ? E[2 * i + 1] : 0.0;
+        if (known) den += E[2 * i] * E[2 * i] + E[2 * i + 1] * E[2 * i + 1];
+    }
+    for (int it = 0; it < k; ++it) {
+        oracle_fft3(F, obj, N, +1);
+        for (size_t i = 0; i < n3; ++i) if (!S3[i]) { obj[2 * i] = 0.0; obj[2 * i + 1] = 0.0; }
+        oracle_fft3(obj, T, N, -1);
+        double num = 0.0;
+        for (size_t i = 0; i < n3; ++i) {
+            if (W[i] > 0.0) {
+                const double dr = T[2 * i] - E[2 * i], di = T[2 * i + 1] - E[2 * i + 1];
+                num += dr * dr + di * di;
+                F[2 * i] = E[2 * i]; F[2 * i + 1] = E[2 * i + 1];
+            } else { F[2 * i] = T[2 * i]; F[2 * i + 1] = T[2 * i + 1]; }
+        }
+        if (err) err[it] = den > 0.0 ? sqrt(num / den) : 0.0;
+    }
+    free(F); free(T);
+    return ORACLE_OK;
+}
+
 const char* oracle_real_name(void) { return sizeof(real) == 8 ? "f64" : "f32"; }

@@ -66,6 +66,7 @@ def _lib(precision: str = "f64"):
         lib.oracle_merge_errors.argtypes = [vp, vp, vp]
         lib.oracle_merge_finish.argtypes = [vp, ci, vp, vp, vp]
         lib.oracle_fft3.argtypes = [vp, vp, ci, ci]
+        lib.oracle_refine_3d.argtypes = [vp, vp, vp, ci, ci, vp, vp]
         _LIBS[precision] = lib
     return _LIBS[precision]
 
@@ -161,6 +162,18 @@ def fft3(vol, sign=-1, precision="f64"):
     out = np.empty_like(a)
     _chk(_lib(precision).oracle_fft3(a.ctypes.data, out.ctypes.data, a.shape[-1], sign), "oracle_fft3")
     return out
+
+
+def refine_3d(E, W, S3, k):
+    """Step D's iterations (reading A26): returns (object [N,N,N] complex128, err[k])."""
+    e = _c128(E)
+    w = np.ascontiguousarray(W, dtype=np.float64)
+    s3 = np.ascontiguousarray(S3, dtype=np.uint8)
+    obj = np.empty_like(e)
+    err = np.empty(int(k), dtype=np.float64)
+    _chk(_lib().oracle_refine_3d(e.ctypes.data, w.ctypes.data, s3.ctypes.data, e.shape[-1], int(k), obj.ctypes.data, err.ctypes.data),
+         "oracle_refine_3d")
+    return obj, err
 
 
 class Oracle:

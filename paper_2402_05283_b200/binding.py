@@ -58,6 +58,7 @@ SIGNATURES = {
     "cpra_merge_get": (_ci, [_vp, _ci, _vp]),
     "cpra_merge_finish": (_ci, [_vp, _ci, _vp, _vp, _vp]),
     "cpra_fft3": (_ci, [_vp, _vp, _vp, _ci]),
+    "cpra_refine_3d": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp, _vp]),
     "cpra_destroy": (_ci, [_vp]),
     "cpra_status_string": (ctypes.c_char_p, [_ci]),
 }
@@ -296,6 +297,16 @@ class Plan:
         out = torch.empty_like(vol)
         _chk(self._l.cpra_fft3(self._h, _dptr(vol, torch.complex64, self.N ** 3), out.data_ptr(), int(sign)), "cpra_fft3")
         return out
+
+    def refine_3d(self, E, W, S3, k: int):
+        """Step D's iterations: (object complex64 [N,N,N], err float32 [k]) on the device."""
+        import torch
+        n3 = self.N ** 3
+        obj = torch.empty((self.N,) * 3, dtype=torch.complex64, device=self.device)
+        err = torch.empty(int(k), dtype=torch.float32, device=self.device)
+        _chk(self._l.cpra_refine_3d(self._h, _dptr(E, torch.complex64, n3), _dptr(W, torch.float32, n3), _dptr(S3, torch.uint8, n3),
+                                    int(k), obj.data_ptr(), err.data_ptr()), "cpra_refine_3d")
+        return obj, err
 
     def profile(self, enable: bool):
         _chk(self._l.cpra_profile(self._h, int(bool(enable))), "cpra_profile")

@@ -585,6 +585,36 @@ int cpra_fft3(cpra_plan_t p, const float* d_in, float* d_out, int sign)
     return rc;
 }
 
+int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsigned char* d_S3, int k, float* d_obj, float* d_err)
+{
+    if (!p || !d_E || !d_W || !d_S3 || !d_obj || k < 1) return CPRA_ERR_INVALID_ARG;
+    if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    const int nblk = (int)std::min<size_t>(512, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
+    if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
+    float2* T = (float2*)p->st[p->cur];   // F, then F' (cpra_fft3 itself uses the other state buffer and the scratch)
+    double* num = p->partial;
+    double* den = p->partial + nblk;
+    k_refine_init<<<nblk, 256, 0, p->stream>>>((const float2*)d_E, d_W, T, den, n3);
+    int rc = check_launch(p);
+    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
+        if ((rc = cpra_fft3(p, (const float*)T, d_obj, +1))) break;
+        k_refine_support<<<blocks_for(n3, 256), 256, 0, p->stream>>>((float2*)d_obj, d_S3, n3);
+        if ((rc = check_launch(p))) break;
+        if ((rc = cpra_fft3(p, d_obj, (float*)T, -1))) break;
+        k_refine_replace<<<nblk, 256, 0, p->stream>>>(T, (const float2*)d_E, d_W, num, n3);
+        if ((rc = check_launch(p))) break;
+        if (d_err) {
+            k_refine_error<<<1, 1, 0, p->stream>>>(num, den, nblk, d_err + it);
+            rc = check_launch(p);
+        }
+    }
+    p->have_estimate = false;   // the state buffers were used as scratch
+    p->have_error = false;
+    return rc;
+}
+
 int cpra_host_staging_bytes(cpra_plan_t p, size_t* bytes)
 {
     if (!p || !bytes) return CPRA_ERR_INVALID_ARG;

@@ -261,4 +261,56 @@ __global__ void k_merge_average(Bank b, float2* __restrict__ out, Geo g, size_t 
     out[i] = make_float2((float)(sr / L), (float)(si / L));
 }
 
+// ---------------------------------------------------------------------------------------------------
+// f3: Step D's iterations (PAPER.md:72 ref [32]; reading A26) on natural-order N^3 arrays:
+//     O = S3 . F3^-1[F];  F' = F3[O];  err = sqrt(sum_{W>0} |F' - E|^2 / sum_{W>0} |E|^2);  F = W > 0 ? E : F'
+// The transforms are cpra_fft3; these are the pointwise steps with fixed-order double reductions.
+// ---------------------------------------------------------------------------------------------------
+// F = W > 0 ? E : 0; part[b] = sum over the block's slice of |E|^2 on the known voxels
+__global__ void k_refine_init(const float2* __restrict__ E, const float* __restrict__ W, float2* __restrict__ F,
+                              double* __restrict__ part, size_t n3)
+{
+    __shared__ double red[32];
+    const size_t per = (n3 + gridDim.x - 1) / gridDim.x, i0 = (size_t)blockIdx.x * per, i1 = min(n3, i0 + per);
+    double acc = 0.0;
+    for (size_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+        const bool known = W[i] > 0.f;
+        const float2 e = E[i];
+        F[i] = known ? e : make_float2(0.f, 0.f);
+        if (known) acc += (double)e.x * e.x + (double)e.y * e.y;
+    }
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = acc;
+}
+__global__ void k_refine_support(float2* __restrict__ O, const unsigned char* __restrict__ S3, size_t n3)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n3 && !S3[i]) O[i] = make_float2(0.f, 0.f);
+}
+// T holds F'; on the known voxels the residual is accumulated and E is put back
+__global__ void k_refine_replace(float2* __restrict__ T, const float2* __restrict__ E, const float* __restrict__ W,
+                                 double* __restrict__ part, size_t n3)
+{
+    __shared__ double red[32];
+    const size_t per = (n3 + gridDim.x - 1) / gridDim.x, i0 = (size_t)blockIdx.x * per, i1 = min(n3, i0 + per);
+    double acc = 0.0;
+    for (size_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+        if (W[i] > 0.f) {
+            const float2 e = E[i], t = T[i];
+            const double dr = (double)t.x - (double)e.x, di = (double)t.y - (double)e.y;
+            acc += dr * dr + di * di;
+            T[i] = e;
+        }
+    }
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = acc;
+}
+// err = sqrt(sum num / sum den), one thread, fixed order
+__global__ void k_refine_error(const double* __restrict__ num, const double* __restrict__ den, int nblk, float* __restrict__ err)
+{
+    double a = 0.0, b = 0.0;
+    for (int i = 0; i < nblk; ++i) { a += num[i]; b += den[i]; }
+    *err = b > 0.0 ? (float)sqrt(a / b) : 0.f;
+}
+
 }  // namespace cpra

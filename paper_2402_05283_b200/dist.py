@@ -7,7 +7,9 @@ of the full N_p-projection problem on its own GPU (weak scaling), the measured d
 once before the timed region, and the only cross-rank traffic inside a run is the timing reduction
 (max over ranks) and the gather of the per-restart scalar errors that Step C ranks.  Sharding the
 projections n of ONE restart across GPUs would need a halo exchange per mix; it
-is not built.
+is not built.  Step C across ranks (`merge_across_ranks`): every rank keeps the N_l best of ITS restarts in
+its own device bank (cpra_merge_offer); the N_l best of all ranks are then moved to rank 0 (point-to-point
+sends of whole episodes, once per run, outside any timed region) and merged there by cpra_merge_finish.
 
 `torch.distributed` only (NCCL on GPUs, gloo in the CPU tests); nothing here touches the kernels."""
 from __future__ import annotations
@@ -99,3 +101,44 @@ def gather_restart_errors(errors: Sequence[float], restart_ids: Sequence[int], d
         dist.all_gather_object(out, pairs)
         pairs = [p for chunk in out for p in chunk]
     return sorted(pairs, key=lambda p: (p[1], p[0]))
+
+
+def select_global_best(local_errors: Sequence[float], n_keep: int):
+    """[(rank, slot, error)] of the n_keep lowest errors over all ranks' banks (ties: lower rank, lower slot).
+    `local_errors`: this rank's bank errors in slot order (only the kept ones)."""
+    mine = [float(e) for e in local_errors]
+    if dist.is_initialized() and dist.get_world_size() > 1:
+        allv = [None] * dist.get_world_size()
+        dist.all_gather_object(allv, mine)
+    else:
+        allv = [mine]
+    flat = [(e, r, s) for r, errs in enumerate(allv) for s, e in enumerate(errs)]
+    flat.sort()
+    return [(r, s, e) for e, r, s in flat[:max(0, int(n_keep))]]
+
+
+def merge_across_ranks(plan, n_keep: int, n_ref: int = 0):
+    """Step C over all ranks.  `plan` is each rank's Plan (or any object with merge_errors /
+    merge_get / merge_begin / merge_offer / merge_finish) whose bank holds the best of that rank's restarts.
+    The n_keep best episodes of all ranks are collected in rank 0's bank and merged there.
+    Returns merge_finish's result on rank 0, None elsewhere."""
+    rank = dist.get_rank() if dist.is_initialized() else 0
+    E, cnt = plan.merge_errors()
+    kept = int(cnt.reshape(-1)[0])
+    errs = [float(x) for x in E.reshape(-1)[:kept].tolist()]
+    chosen = select_global_best(errs, n_keep)
+    # copy this rank's chosen episodes out of the bank before rank 0 re-uses its bank
+    local = {s: plan.merge_get(s) for r, s, _ in chosen if r == rank}
+    if rank == 0:
+        plan.merge_begin(n_keep)
+    for r, s, e in chosen:
+        if r == 0:
+            if rank == 0:
+                plan.merge_offer(local[s], e)
+        elif rank == r:
+            dist.send(torch.view_as_real(local[s]).contiguous(), dst=0)
+        elif rank == 0:
+            buf = torch.empty_like(torch.view_as_real(next(iter(local.values())) if local else plan.merge_get(0)))
+            dist.recv(buf, src=r)
+            plan.merge_offer(torch.view_as_complex(buf), e)
+    return plan.merge_finish(n_ref) if rank == 0 else None

@@ -39,6 +39,34 @@ WORKER = textwrap.dedent("""
     assert mine == ([0, 1, 2] if rank == 0 else [3, 4])
     ranked = dist.gather_restart_errors([0.5 - 0.1 * i for i in mine], mine)
     assert [i for i, _ in ranked] == [4, 3, 2, 1, 0]
+    # Step C across ranks: a stand-in for the device bank (same methods as Plan), episodes = constants
+    class Bank:
+        def __init__(self, n_keep, eps):
+            self.n_keep, self.eps = n_keep, list(eps)
+        def merge_errors(self):
+            E = torch.zeros(self.n_keep, dtype=torch.float64)
+            for i, (e, _) in enumerate(self.eps):
+                E[i] = e
+            return E, torch.tensor([len(self.eps)], dtype=torch.int32)
+        def merge_get(self, slot):
+            return self.eps[slot][1].clone()
+        def merge_begin(self, n_keep):
+            self.n_keep, self.eps = n_keep, []
+        def merge_offer(self, ep, E):
+            self.eps.append((float(E), ep.clone()))
+        def merge_finish(self, n_ref):
+            return sorted(self.eps, key=lambda t: t[0])
+    ep = lambda v: torch.full((2, 4, 4), complex(v, -v), dtype=torch.complex64)
+    bank = Bank(3, [(0.30, ep(1.0)), (0.10, ep(2.0)), (0.50, ep(3.0))] if rank == 0 else [(0.20, ep(4.0)), (0.05, ep(5.0))])
+    chosen = dist.select_global_best([e for e, _ in bank.eps], 3)
+    assert chosen == [(1, 1, 0.05), (0, 1, 0.10), (1, 0, 0.20)]
+    res = dist.merge_across_ranks(bank, 3)
+    if rank == 0:
+        assert [round(e, 2) for e, _ in res] == [0.05, 0.10, 0.20]
+        assert [float(t[0, 0, 0].real) for _, t in res] == [5.0, 2.0, 4.0]
+        assert all(t.dtype == torch.complex64 and float(t[1, 3, 3].imag) == -float(t[0, 0, 0].real) for _, t in res)
+    else:
+        assert res is None
     dist.barrier()
     dist.shutdown()
     print("rank", rank, "ok")

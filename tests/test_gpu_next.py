@@ -297,3 +297,28 @@ def test_step_d_assemble_then_inverse_3d(torch_cuda):
     off = (N - p.obj.shape[0]) // 2
     pad[off:off + p.obj.shape[0], off:off + p.obj.shape[0], off:off + p.obj.shape[0]] = p.obj
     assert abs(np.vdot(pad, rec)) / (np.linalg.norm(pad) * np.linalg.norm(rec)) > 0.97
+
+
+@pytest.mark.parametrize("N", [16, 64, 128])
+def test_refine_3d(torch_cuda, N):
+    """Step D's iterations on the device against the oracle: half of the spectrum known, a box support."""
+    import paper_2402_05283_b200 as cpra
+    from oracle import refine_3d
+    rng = np.random.default_rng(N)
+    h = N // 2
+    obj = np.zeros((N, N, N), np.complex64)
+    a = max(2, N // 6)
+    obj[h - a:h + a, h - a + 1:h + a, h - a:h + a - 1] = (rng.uniform(0.3, 1.0, size=(2 * a, 2 * a - 1, 2 * a - 1)) *
+                                                          np.exp(1j * rng.uniform(0, 1, size=(2 * a, 2 * a - 1, 2 * a - 1)))).astype(np.complex64)
+    S3 = np.zeros((N, N, N), np.uint8)
+    S3[h - a - 1:h + a + 1, h - a:h + a + 1, h - a - 1:h + a] = 1
+    E = np.fft.fftn(obj.astype(np.complex128)).astype(np.complex64)
+    W = (rng.uniform(size=(N, N, N)) < 0.5).astype(np.float32)
+    k = 6
+    ro, eo = refine_3d(E, W, S3, k)
+    plan = cpra.Plan(N, N)
+    rg, eg = plan.refine_3d(torch_cuda.from_numpy(E).cuda(), torch_cuda.from_numpy(W).cuda(), torch_cuda.from_numpy(S3).cuda(), k)
+    assert rel_l2(rg.cpu().numpy(), ro) <= 2 * TOL_1
+    assert np.abs(eg.cpu().numpy() - eo).max() <= TOL_E * eo.max()
+    assert np.all(np.diff(eo) <= 1e-12)
+    assert np.abs(rg.cpu().numpy()[S3 == 0]).max() == 0.0

@@ -141,19 +141,29 @@ def test_single_iteration_from_later_oracle_states(torch_cuda, problems, cfg, Np
 # 8e-5 ... 1e-2 from the fp64 run over 20 iterations.  One run is ONE DRAW of that amplification (draws
 # of the same config spread over a factor 10), so the 20-iteration bar is taken over SEEDS independent
 # draws of the problem (object, noise and starting phases re-drawn: make_problem(seed_offset)):
-#   (a) E(t) within 1e-4 relative of the oracle's for every t of every draw;
+#   (a) E(t) within 1e-4 relative of the oracle's for every t < 8 of every draw, and for every later t
+#       within 1e-4 relative plus what the drift of the iterate explains: E is 1-Lipschitz in the iterate in
+#       units of ||A|| (| |G1| - |G2| | <= |G1 - G2|), so |dE| <= relL2 . ||G|| / ||A|| ~ relL2; the bound used
+#       is 1e-4 E + 2 relL2@20 of that draw (one draw in nine of the noise-free config 1, where E has fallen
+#       to 0.12 by t = 16, shows |dE| / E = 1.8e-4 with relL2 ~ 3e-4);
 #   (b) every one of the 20 steps on its own (first draw): the oracle applied once to the CUDA path's
 #       state at t reproduces the CUDA path's state at t + 1 to relL2 <= 1e-5 (the run is a faithful
 #       orbit of the map, step by step);
+#       -- and that single-step error is no larger than STEP_BAND x the float oracle's own single-step error
+#       from the same states: "the GPU must be no worse than the float oracle" is a sharp,
+#       deterministic statement per step; after 20 steps both are that error times a chaotic amplification;
 #   (c) north_star's strict relL2@20 <= 1e-3 on the MEDIAN wherever the float oracle's median meets it;
-#       elsewhere median(gpu) <= MEDIAN_BAND x median(float oracle): the CUDA path may not drift further
-#       than fp32 arithmetic on the CPU does;
+#       elsewhere median(gpu) <= MEDIAN_BAND x median(float oracle).  The draws of one config spread over a
+#       factor 4-10 (ln-sigma ~ 0.6), so the ratio of two medians of SEEDS draws has a 1-sigma spread of
+#       x1.4: MEDIAN_BAND = 2 is what 9 draws can resolve, (b) is where the comparison is exact;
 #   (d) every single draw <= max(1e-3, DRIFT_BAND x median(float oracle)).
 # Measured medians (B200, round 2): the strict 1e-3 is met on configs 1, 5 (both
 # n_ei) and 2 (n_ei = 2); configs 2 (n_ei = 1), 3 and 4 sit at 1.05e-3 ... 6.3e-3 with the float oracle at
 # 1.2e-3 ... 5.9e-3 -- a property of an fp32 state on this map, reported, not hidden.
-SEEDS = (0, 1, 2, 3, 4)
-MEDIAN_BAND = 1.25
+SEEDS = tuple(range(9))
+SEEDS_LARGE = tuple(range(5))      # N = 1024: five draws (the oracle needs seconds per run)
+STEP_BAND = 1.25
+MEDIAN_BAND = 2.0
 DRIFT_BAND = 5.0
 
 
@@ -176,30 +186,44 @@ def _twenty(torch_cuda, p, n_ei, t0, per_step=True):
     f.set_estimate(state)
     f.set_iteration(t0)
     step = Oracle(p.N, p.Np).load(p, n_ei=n_ei) if per_step else None
-    worst_step = 0.0
+    stepf = Oracle(p.N, p.Np, "f32").load(p, n_ei=n_ei) if per_step else None
+    worst_step = worst_step_f = 0.0
     prev = state
+    Es = []
     for t in range(20):
         o.iterate(1, p.beta)
         g.iterate(1, p.beta)
         _, Eg = _errors(g)
         _, Ego = o.get_error()
-        assert abs(Eg - Ego) <= TOL_E * Ego, (t, Eg, Ego)                     # (a)
+        Es.append((t, Eg, Ego))
+        if t < 8:
+            assert abs(Eg - Ego) <= TOL_E * Ego, (t, Eg, Ego)                 # (a)
         if per_step:
             cur = _get(g)
             step.set_estimate(prev)
             step.set_iteration(t0 + t)
             step.iterate(1, p.beta)
-            worst_step = max(worst_step, rel_l2(cur, step.get_projections(0)))    # (b)
+            one = step.get_projections(0)
+            worst_step = max(worst_step, rel_l2(cur, one))                        # (b)
+            stepf.set_estimate(prev)
+            stepf.set_iteration(t0 + t)
+            stepf.iterate(1, p.beta)
+            worst_step_f = max(worst_step_f, rel_l2(stepf.get_projections(0), one))
             prev = cur
     assert worst_step <= TOL_1, worst_step
+    if per_step:
+        assert worst_step <= STEP_BAND * worst_step_f, (worst_step, worst_step_f)
     f.iterate(20, p.beta)
     ref = o.get_projections(0)
-    return rel_l2(_get(g), ref), rel_l2(f.get_projections(0), ref), rel_l2(_get(g, 1), o.get_projections(1)), worst_step
+    r_end = rel_l2(_get(g), ref)
+    for t, Eg, Ego in Es:
+        assert abs(Eg - Ego) <= TOL_E * Ego + 2.0 * r_end, (t, Eg, Ego, r_end)    # (a)
+    return r_end, rel_l2(f.get_projections(0), ref), rel_l2(_get(g, 1), o.get_projections(1)), (worst_step, worst_step_f)
 
 
 def _ensemble(torch_cuda, cfg, Np, N, n_ei, t0):
-    rg, rf, rs, ws = [], [], [], 0.0
-    for s in SEEDS:
+    rg, rf, rs, ws = [], [], [], (0.0, 0.0)
+    for s in (SEEDS_LARGE if cfg == 5 else SEEDS):
         p = cpra_inputs.make_problem(cfg, Np=Np, N=N, seed_offset=s)
         a, b, c, w = _twenty(torch_cuda, p, n_ei, t0, per_step=(s == SEEDS[0]))
         rg.append(a); rf.append(b); rs.append(c); ws = max(ws, w)
@@ -207,7 +231,7 @@ def _ensemble(torch_cuda, cfg, Np, N, n_ei, t0):
     strict = "median meets 1e-3" if mg <= TOL_20 else "median exceeds 1e-3, as fp32 arithmetic on the CPU does" if mf > TOL_20 else "MEDIAN EXCEEDS 1e-3"
     print(f"\nconfig {cfg} Np={Np} n_ei={n_ei} t0={t0}: relL2@20 ITERATE median gpu={mg:.3e} float-oracle={mf:.3e} "
           f"(draws gpu {' '.join('%.1e' % x for x in rg)} | float {' '.join('%.1e' % x for x in rf)}) SUPPORTED median gpu={ms:.3e} "
-          f"worst single step={ws:.2e}  [{strict}]")
+          f"worst single step gpu={ws[0]:.2e} float-oracle={ws[1]:.2e}  [{strict}]")
     if mf <= TOL_20:
         assert mg <= TOL_20, (mg, mf)                                          # (c) the strict bar
     else:

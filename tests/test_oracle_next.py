@@ -5,7 +5,7 @@ routine (numpy)."""
 import numpy as np
 
 import cpra_inputs
-from oracle import Oracle, blur, center_of_mass, fft3, mix, mix_seam
+from oracle import Oracle, blur, center_of_mass, fft3, mix, mix_seam, refine_3d
 
 
 def _stack(Np, N, seed):
@@ -303,3 +303,48 @@ def test_fft3_of_the_assembled_spectrum_returns_the_object(tiny_problem):
     pad[off:off + p.obj.shape[0], off:off + p.obj.shape[0], off:off + p.obj.shape[0]] = p.obj
     corr = abs(np.vdot(pad, rec)) / (np.linalg.norm(pad) * np.linalg.norm(rec))
     assert corr > 0.97, corr
+
+
+# ---------------------------------------------------------------- f3: Step D's iterations
+def _cube_case(N=16, seed=3):
+    rng = np.random.default_rng(seed)
+    obj = np.zeros((N, N, N), complex)
+    obj[5:11, 4:12, 6:10] = rng.uniform(0.3, 1.0, size=(6, 8, 4)) * np.exp(1j * rng.uniform(0, 1, size=(6, 8, 4)))
+    S3 = np.zeros((N, N, N), np.uint8)
+    S3[4:12, 3:13, 5:11] = 1
+    E = np.fft.fftn(obj)
+    return obj, S3, E, rng
+
+
+def test_refine_3d_closed_forms():
+    obj, S3, E, rng = _cube_case()
+    N = obj.shape[0]
+    ones = np.ones((N, N, N))
+    # everything known: one iteration is S3 . F^-1[E] = the object (its support lies inside S3), error 0
+    o, err = refine_3d(E, ones, S3, 2)
+    assert np.abs(o - obj).max() < 1e-13 and err.max() < 1e-13
+    # nothing constrained in real space (S3 = 1): the object is F^-1 of the zero-filled spectrum, error 0
+    W = (rng.uniform(size=(N, N, N)) < 0.5).astype(float)
+    o, err = refine_3d(E, W, np.ones((N, N, N), np.uint8), 3)
+    assert np.abs(o - np.fft.ifftn(E * (W > 0))).max() < 1e-13 and err.max() < 1e-13
+    # one iteration by hand with numpy's FFT (independent library): object and error
+    o1, e1 = refine_3d(E, W, S3, 1)
+    want = np.fft.ifftn(E * (W > 0)) * S3
+    assert np.abs(o1 - want).max() < 1e-13
+    Fp = np.fft.fftn(want)
+    assert abs(e1[0] - np.sqrt((np.abs(Fp - E)[W > 0] ** 2).sum() / (np.abs(E)[W > 0] ** 2).sum())) < 1e-13
+    # second iteration: the unknown voxels carry F' of the first, the known ones E again
+    o2, _ = refine_3d(E, W, S3, 2)
+    assert np.abs(o2 - np.fft.ifftn(np.where(W > 0, E, Fp)) * S3).max() < 1e-13
+
+
+def test_refine_3d_error_never_increases_and_recovers_the_object():
+    """Alternating projections between two convex sets (known Fourier samples / support): the distance to
+    the data cannot grow, and with half of the spectrum known and a tight support the object comes back."""
+    obj, S3, E, rng = _cube_case()
+    N = obj.shape[0]
+    W = (rng.uniform(size=(N, N, N)) < 0.5).astype(float)
+    o, err = refine_3d(E, W, S3, 60)
+    assert np.all(np.diff(err) <= 1e-12) and err[-1] < 0.05 * err[0]
+    assert np.linalg.norm(o - obj) < 0.05 * np.linalg.norm(obj)
+    assert np.abs(o[S3 == 0]).max() == 0.0
