@@ -286,6 +286,22 @@ int cpra_refine_3d(cpra_plan_t plan, const float* d_E, const float* d_W, const u
                    float* d_obj, float* d_err);
 
 /*
+ * The paper's quality metrics ("PRTF", "FSC", resolution at the 0.5 cut-off).
+ *   cpra_fsc   Fourier shell correlation of two 3D spectra d_F1, d_F2 (complex fp32 [N][N][N], native order; a
+ *              plan with Np == N):  FSC(s) = Re sum_s F1 conj(F2) / sqrt(sum_s |F1|^2 sum_s |F2|^2), shell
+ *              s = round(|k|) over signed integer frequencies, s = 0 .. N/2; 0 for a shell without energy.
+ *   cpra_prtf  phase retrieval transfer function of an averaged episode d_avg (complex fp32 [Np][N][N], e.g.
+ *              cpra_merge_finish's output) against the measured amplitudes of cpra_set_data:
+ *              PRTF(s) = mean over n and the measured pixels with A > 0 of ring s of |F2[avg_n]| / A_n.
+ *   d_out: fp32 [N/2 + 1].  Shell sums are double atomics: reproducible to ~1e-15, not bit for bit.
+ * Both use the error scratch (cpra_get_error is NOT_READY afterwards) and cpra_prtf the FFT scratch and the
+ * spare state buffer.  Errors: INVALID_ARG, NOT_READY (cpra_prtf without data), UNSUPPORTED_SIZE (cpra_prtf
+ * with Np * N / 8 < N + 2), CUDA.
+ */
+int cpra_fsc(cpra_plan_t plan, const float* d_F1, const float* d_F2, float* d_out);
+int cpra_prtf(cpra_plan_t plan, const float* d_avg, float* d_out);
+
+/*
  * End-to-end convenience with HOST buffers (pinned memory recommended): uploads the inputs,
  * runs k iterations, downloads the result and synchronises the plan's stream.
  *   h_I [Np][N][N] fp32, h_mask [Np][N][N] u8 or NULL, h_angles [Np] or NULL, h_S [Np][N][N] u8,

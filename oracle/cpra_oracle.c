@@ -982,4 +982,68 @@ int oracle_refine_3d(const double* E, const double* W, const unsigned char* S3, 
     return ORACLE_OK;
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* the paper's quality metrics (PRTF, FSC, cut-off at 0.5)   */
+/* ------------------------------------------------------------------------------------------ */
+/* Fourier shell correlation of two 3D spectra (native order, interleaved complex double [N][N][N]):
+ *   FSC(s) = Re sum_{shell s} F1 conj(F2) / sqrt( sum_{shell s} |F1|^2 . sum_{shell s} |F2|^2 ),
+ * shell s = round(|k|) over signed integer frequencies, s = 0 .. N/2 (voxels beyond N/2 are left out);
+ * 0 where a shell has no energy.  out: N/2 + 1 doubles. */
+int oracle_fsc(const double* F1, const double* F2, int N, double* out)
+{
+    if (!F1 || !F2 || !out || N < 2) return ORACLE_ERR_INVALID_ARG;
+    const int ns = N / 2 + 1;
+    double* acc = (double*)calloc((size_t)3 * ns, sizeof(double));
+    for (int iz = 0; iz < N; ++iz)
+        for (int iy = 0; iy < N; ++iy)
+            for (int ix = 0; ix < N; ++ix) {
+                const int kz = iz < N / 2 ? iz : iz - N, ky = iy < N / 2 ? iy : iy - N, kx = ix < N / 2 ? ix : ix - N;
+                const int sh = (int)floor(sqrt((double)kx * kx + (double)ky * ky + (double)kz * kz) + 0.5);
+                if (sh >= ns) continue;
+                const size_t i = ((size_t)iz * N + iy) * N + ix;
+                acc[sh] += F1[2 * i] * F2[2 * i] + F1[2 * i + 1] * F2[2 * i + 1];
+                acc[ns + sh] += F1[2 * i] * F1[2 * i] + F1[2 * i + 1] * F1[2 * i + 1];
+                acc[2 * ns + sh] += F2[2 * i] * F2[2 * i] + F2[2 * i + 1] * F2[2 * i + 1];
+            }
+    for (int sh = 0; sh < ns; ++sh) {
+        const double d = sqrt(acc[ns + sh] * acc[2 * ns + sh]);
+        out[sh] = d > 0.0 ? acc[sh] / d : 0.0;
+    }
+    free(acc);
+    return ORACLE_OK;
+}
+
+/* Phase retrieval transfer function of an (averaged) episode against the measured amplitudes of the plan:
+ *   PRTF(s) = mean over n and over the measured pixels (M = 1, A > 0) of ring s of  |F2[avg_n](k)| / A_n(k),
+ * ring s = round(|k|) in the detector plane, s = 0 .. N/2; 0 for an empty ring.  avg: interleaved complex
+ * double [Np][N][N] (e.g. the output of oracle_merge_finish); out: N/2 + 1 doubles. */
+int oracle_prtf(oracle_plan_t p, const double* avg, double* out)
+{
+    if (!p || !avg || !out) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_data) return ORACLE_ERR_NOT_READY;
+    const int N = p->N, ns = N / 2 + 1;
+    const size_t px = p->px;
+    double* sum = (double*)calloc((size_t)ns, sizeof(double));
+    double* cnt = (double*)calloc((size_t)ns, sizeof(double));
+    cplx* G = (cplx*)malloc(sizeof(cplx) * px);
+    for (int n = 0; n < p->Np; ++n) {
+        for (size_t i = 0; i < px; ++i) { G[i].re = (real)avg[2 * (n * px + i)]; G[i].im = (real)avg[2 * (n * px + i) + 1]; }
+        fft2d(G, N, -1);
+        for (int iy = 0; iy < N; ++iy)
+            for (int ix = 0; ix < N; ++ix) {
+                const size_t i = (size_t)iy * N + ix;
+                const double A = (double)p->A[n * px + i];
+                if (!p->M[n * px + i] || !(A > 0.0)) continue;
+                const int ky = iy < N / 2 ? iy : iy - N, kx = ix < N / 2 ? ix : ix - N;
+                const int sh = (int)floor(sqrt((double)kx * kx + (double)ky * ky) + 0.5);
+                if (sh >= ns) continue;
+                sum[sh] += sqrt((double)G[i].re * G[i].re + (double)G[i].im * G[i].im) / A;
+                cnt[sh] += 1.0;
+            }
+    }
+    for (int sh = 0; sh < ns; ++sh) out[sh] = cnt[sh] > 0.0 ? sum[sh] / cnt[sh] : 0.0;
+    free(sum); free(cnt); free(G);
+    return ORACLE_OK;
+}
+
 const char* oracle_real_name(void) { return sizeof(real) == 8 ? "f64" : "f32"; }

@@ -67,6 +67,8 @@ def _lib(precision: str = "f64"):
         lib.oracle_merge_finish.argtypes = [vp, ci, vp, vp, vp]
         lib.oracle_fft3.argtypes = [vp, vp, ci, ci]
         lib.oracle_refine_3d.argtypes = [vp, vp, vp, ci, ci, vp, vp]
+        lib.oracle_fsc.argtypes = [vp, vp, ci, vp]
+        lib.oracle_prtf.argtypes = [vp, vp, vp]
         _LIBS[precision] = lib
     return _LIBS[precision]
 
@@ -174,6 +176,14 @@ def refine_3d(E, W, S3, k):
     _chk(_lib().oracle_refine_3d(e.ctypes.data, w.ctypes.data, s3.ctypes.data, e.shape[-1], int(k), obj.ctypes.data, err.ctypes.data),
          "oracle_refine_3d")
     return obj, err
+
+
+def fsc(F1, F2):
+    """Fourier shell correlation of two 3D spectra: N/2 + 1 values."""
+    a, b = _c128(F1), _c128(F2)
+    out = np.empty(a.shape[-1] // 2 + 1, dtype=np.float64)
+    _chk(_lib().oracle_fsc(a.ctypes.data, b.ctypes.data, a.shape[-1], out.ctypes.data), "oracle_fsc")
+    return out
 
 
 class Oracle:
@@ -287,6 +297,12 @@ class Oracle:
         tw = np.zeros(kept, dtype=np.int32)
         _chk(self._l.oracle_merge_finish(self._h, int(n_ref), out.ctypes.data, sh.ctypes.data, tw.ctypes.data), "oracle_merge_finish")
         return out, sh, tw
+
+    def prtf(self, avg):
+        a = _c128(avg)
+        out = np.empty(self.N // 2 + 1, dtype=np.float64)
+        _chk(self._l.oracle_prtf(self._h, a.ctypes.data, out.ctypes.data), "oracle_prtf")
+        return out
 
     def load(self, problem, alpha=(0.6, 0.2), n_ei=1):
         """Convenience: feed a cpra_inputs.Problem."""

@@ -59,6 +59,8 @@ SIGNATURES = {
     "cpra_merge_finish": (_ci, [_vp, _ci, _vp, _vp, _vp]),
     "cpra_fft3": (_ci, [_vp, _vp, _vp, _ci]),
     "cpra_refine_3d": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp, _vp]),
+    "cpra_fsc": (_ci, [_vp, _vp, _vp, _vp]),
+    "cpra_prtf": (_ci, [_vp, _vp, _vp]),
     "cpra_destroy": (_ci, [_vp]),
     "cpra_status_string": (ctypes.c_char_p, [_ci]),
 }
@@ -307,6 +309,18 @@ class Plan:
         _chk(self._l.cpra_refine_3d(self._h, _dptr(E, torch.complex64, n3), _dptr(W, torch.float32, n3), _dptr(S3, torch.uint8, n3),
                                     int(k), obj.data_ptr(), err.data_ptr()), "cpra_refine_3d")
         return obj, err
+
+    def fsc(self, F1, F2):
+        import torch
+        out = torch.empty(self.N // 2 + 1, dtype=torch.float32, device=self.device)
+        _chk(self._l.cpra_fsc(self._h, _dptr(F1, torch.complex64, self.N ** 3), _dptr(F2, torch.complex64, self.N ** 3), out.data_ptr()), "cpra_fsc")
+        return out
+
+    def prtf(self, avg):
+        import torch
+        out = torch.empty(self.N // 2 + 1, dtype=torch.float32, device=self.device)
+        _chk(self._l.cpra_prtf(self._h, _dptr(avg, torch.complex64, self._px), out.data_ptr()), "cpra_prtf")
+        return out
 
     def profile(self, enable: bool):
         _chk(self._l.cpra_profile(self._h, int(bool(enable))), "cpra_profile")

@@ -263,6 +263,10 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     }
     // whole-image kernel on a cluster of C CTAs per projection (cpra_set_cluster; cpra_cluster.cuh)
     int C = p->cluster;
+    // library default (measured, B200): at N = 64 the clustered kernel with programmatic dependent launch beats
+    // the one-CTA-per-image kernel (N_p = 32: 6.9 us per iteration with 4 CTAs per image against 9.3; N_p = 180:
+    // 12.0 with 2 against 12.9); at N = 128 and 256 it does not
+    if (C == 0 && p->N == 64) C = (4 * p->Np <= 2 * p->sms) ? 4 : 2;
     if (C > 0) {
         bool ok = false;
         { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, ok = Launch<NN>::image_cl_ok(C)); return 0; }; f(); }
@@ -613,6 +617,48 @@ int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsi
     p->have_estimate = false;   // the state buffers were used as scratch
     p->have_error = false;
     return rc;
+}
+
+int cpra_fsc(cpra_plan_t p, const float* d_F1, const float* d_F2, float* d_out)
+{
+    if (!p || !d_F1 || !d_F2 || !d_out) return CPRA_ERR_INVALID_ARG;
+    if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    const int ns = p->N / 2 + 1;
+    double* acc = p->partial;   // >= 3 (N/2 + 1) doubles for every supported N with Np = N
+    if (cudaMemsetAsync(acc, 0, sizeof(double) * 3 * ns, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    k_fsc_accumulate<<<4 * p->sms, 256, sizeof(double) * 3 * ns, p->stream>>>((const float2*)d_F1, (const float2*)d_F2, acc, p->N);
+    if (int rc = check_launch(p)) return rc;
+    k_fsc_finalize<<<blocks_for(ns, 128), 128, 0, p->stream>>>(acc, d_out, ns);
+    p->have_error = false;
+    return check_launch(p);
+}
+
+int cpra_prtf(cpra_plan_t p, const float* d_avg, float* d_out)
+{
+    if (!p || !d_avg || !d_out) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_data) return CPRA_ERR_NOT_READY;
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    const int ns = p->N / 2 + 1;
+    if ((size_t)2 * ns > (size_t)p->Np * (p->N / 8)) return CPRA_ERR_UNSUPPORTED_SIZE;   // the shell sums live in the error scratch
+    float4* tmp = p->st[p->cur ^ 1];
+    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_avg, (float*)tmp, p->geo, total);
+    int rc = check_launch(p);
+    if (rc) return rc;
+    { auto f = [&]() -> int {
+        CPRA_DISPATCH_N(p->N,
+            rc = Launch<NN>::row_fwd(p, tmp, MIX_NONE, 0, p->Np);
+            if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
+        return 0; }; f(); }
+    if (rc) return rc;
+    double* acc = p->partial;
+    if (cudaMemsetAsync(acc, 0, sizeof(double) * 2 * ns, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    k_prtf_accumulate<<<4 * p->sms, 256, sizeof(double) * 2 * ns, p->stream>>>((const float*)p->scr, p->A, acc, p->geo, total);
+    if ((rc = check_launch(p))) return rc;
+    k_prtf_finalize<<<blocks_for(ns, 128), 128, 0, p->stream>>>(acc, d_out, ns);
+    p->have_error = false;   // the error scratch held the shell sums
+    return check_launch(p);
 }
 
 int cpra_host_staging_bytes(cpra_plan_t p, size_t* bytes)

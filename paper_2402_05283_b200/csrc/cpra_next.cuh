@@ -313,4 +313,66 @@ __global__ void k_refine_error(const double* __restrict__ num, const double* __r
     *err = b > 0.0 ? (float)sqrt(a / b) : 0.f;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// f4: the paper's quality metrics: Fourier shell correlation and PRTF.
+// Shell sums are accumulated per block in shared memory and added to the global shell accumulators with
+// double atomics (the order of the additions varies from run to run at the 1e-16 level).
+// ---------------------------------------------------------------------------------------------------
+// acc[0..ns): Re sum F1 conj F2;  acc[ns..2ns): sum |F1|^2;  acc[2ns..3ns): sum |F2|^2;  shell = round(|k|) <= N/2
+__global__ void k_fsc_accumulate(const float2* __restrict__ F1, const float2* __restrict__ F2, double* __restrict__ acc, int N)
+{
+    extern __shared__ double sh[];   // 3 ns
+    const int ns = N / 2 + 1;
+    for (int i = threadIdx.x; i < 3 * ns; i += blockDim.x) sh[i] = 0.0;
+    __syncthreads();
+    const size_t n3 = (size_t)N * N * N;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += (size_t)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % N), iy = (int)((i / N) % N), iz = (int)(i / ((size_t)N * N));
+        const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N, kz = iz < N / 2 ? iz : iz - N;
+        const int s = (int)floor(sqrt((double)kx * kx + (double)ky * ky + (double)kz * kz) + 0.5);
+        if (s >= ns) continue;
+        const float2 a = F1[i], b = F2[i];
+        atomicAdd(&sh[s], (double)a.x * b.x + (double)a.y * b.y);
+        atomicAdd(&sh[ns + s], (double)a.x * a.x + (double)a.y * a.y);
+        atomicAdd(&sh[2 * ns + s], (double)b.x * b.x + (double)b.y * b.y);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 3 * ns; i += blockDim.x) if (sh[i] != 0.0) atomicAdd(&acc[i], sh[i]);
+}
+__global__ void k_fsc_finalize(const double* __restrict__ acc, float* __restrict__ out, int ns)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= ns) return;
+    const double d = sqrt(acc[ns + s] * acc[2 * ns + s]);
+    out[s] = d > 0.0 ? (float)(acc[s] / d) : 0.f;
+}
+// PRTF: scr holds F2[avg_n] in the scratch layout, Aperm the measured amplitudes (A < 0: unmeasured);
+// acc[0..ns): sum of |G| / A over the measured pixels with A > 0 of ring s, acc[ns..2ns): their number
+__global__ void k_prtf_accumulate(const float* __restrict__ scr, const float* __restrict__ Aperm, double* __restrict__ acc, Geo g, size_t total)
+{
+    extern __shared__ double sh[];   // 2 ns
+    const int N = g.N, ns = N / 2 + 1;
+    for (int i = threadIdx.x; i < 2 * ns; i += blockDim.x) sh[i] = 0.0;
+    __syncthreads();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % N), iy = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
+        const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N;
+        const int s = (int)floor(sqrt((double)kx * kx + (double)ky * ky) + 0.5);
+        if (s >= ns) continue;
+        const int py = fft_pos(iy, g.R0, g.R1, g.R2), px = fft_pos(ix, g.R0, g.R1, g.R2);
+        const float A = Aperm[a_idx(g, n, py, px)];
+        if (!(A > 0.f)) continue;
+        const float2 G = ld_c(scr, sc_idx(g, n, py, px));
+        atomicAdd(&sh[s], sqrt((double)G.x * G.x + (double)G.y * G.y) / (double)A);
+        atomicAdd(&sh[ns + s], 1.0);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 2 * ns; i += blockDim.x) if (sh[i] != 0.0) atomicAdd(&acc[i], sh[i]);
+}
+__global__ void k_prtf_finalize(const double* __restrict__ acc, float* __restrict__ out, int ns)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < ns) out[s] = acc[ns + s] > 0.0 ? (float)(acc[s] / acc[ns + s]) : 0.f;
+}
+
 }  // namespace cpra

@@ -322,3 +322,31 @@ def test_refine_3d(torch_cuda, N):
     assert np.abs(eg.cpu().numpy() - eo).max() <= TOL_E * eo.max()
     assert np.all(np.diff(eo) <= 1e-12)
     assert np.abs(rg.cpu().numpy()[S3 == 0]).max() == 0.0
+
+
+@pytest.mark.parametrize("N", [16, 64, 128])
+def test_fsc(torch_cuda, N):
+    import paper_2402_05283_b200 as cpra
+    from oracle import fsc
+    rng = np.random.default_rng(N)
+    F = (rng.normal(size=(N, N, N)) + 1j * rng.normal(size=(N, N, N))).astype(np.complex64)
+    G = (0.6 * F + rng.normal(size=(N, N, N)) + 1j * rng.normal(size=(N, N, N))).astype(np.complex64)
+    plan = cpra.Plan(N, N)
+    out = plan.fsc(torch_cuda.from_numpy(F).cuda(), torch_cuda.from_numpy(G).cuda()).cpu().numpy()
+    assert np.abs(out - fsc(F, G)).max() <= 2e-6
+    assert np.abs(plan.fsc(torch_cuda.from_numpy(F).cuda(), torch_cuda.from_numpy(F).cuda()).cpu().numpy() - 1.0).max() <= 2e-6
+
+
+@pytest.mark.parametrize("cfg,Np,N", [(1, 8, None), (2, 12, None), (3, 6, None), (4, 4, None)])
+def test_prtf(torch_cuda, cfg, Np, N):
+    """PRTF of the supported estimate after a few iterations against the measured amplitudes (beamstop pixels
+    and zero-count pixels left out), device vs oracle."""
+    p = cpra_inputs.make_problem(cfg, Np=Np, N=N)
+    o, g = _oracle(p), _gpu(p)
+    o.iterate(3, p.beta)
+    g.iterate(3, p.beta)
+    avg = o.get_projections(1).astype(np.complex64)
+    want = o.prtf(avg)
+    got = g.prtf(torch_cuda.from_numpy(avg).cuda()).cpu().numpy()
+    assert np.abs(got - want).max() <= 2e-5 * max(1.0, np.abs(want).max())
+    assert want[p.N // 4] > 0

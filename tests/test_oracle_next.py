@@ -5,7 +5,7 @@ routine (numpy)."""
 import numpy as np
 
 import cpra_inputs
-from oracle import Oracle, blur, center_of_mass, fft3, mix, mix_seam, refine_3d
+from oracle import Oracle, blur, center_of_mass, fft3, fsc, mix, mix_seam, refine_3d
 
 
 def _stack(Np, N, seed):
@@ -348,3 +348,53 @@ def test_refine_3d_error_never_increases_and_recovers_the_object():
     assert np.all(np.diff(err) <= 1e-12) and err[-1] < 0.05 * err[0]
     assert np.linalg.norm(o - obj) < 0.05 * np.linalg.norm(obj)
     assert np.abs(o[S3 == 0]).max() == 0.0
+
+
+# ---------------------------------------------------------------- f4: FSC and PRTF
+def test_fsc_closed_forms():
+    N = 16
+    rng = np.random.default_rng(8)
+    F = rng.normal(size=(N, N, N)) + 1j * rng.normal(size=(N, N, N))
+    ns = N // 2 + 1
+    assert np.abs(fsc(F, F) - 1.0).max() < 1e-14
+    assert np.abs(fsc(F, -F) + 1.0).max() < 1e-14
+    assert np.abs(fsc(F, 1j * F)).max() < 1e-14                       # quadrature: Re<F, iF> = 0
+    assert np.abs(fsc(F, 3.0 * F) - 1.0).max() < 1e-14                # scale invariant
+    # shells: a spectrum living on one voxel k correlates only in shell round(|k|); outside N/2 it is left out
+    for k, sh in (((0, 0, 0), 0), ((3, -4, 0), 5), ((-2, 2, 1), 3), ((5, 5, 5), None)):
+        D = np.zeros((N, N, N), complex)
+        D[k[0] % N, k[1] % N, k[2] % N] = 1.0
+        f = fsc(D + 1e-30 * 0, D)
+        want = np.zeros(ns)
+        if sh is not None:
+            want[sh] = 1.0
+        assert np.array_equal(f, want), (k, f)
+    # against a numpy restatement on random pairs
+    G = rng.normal(size=(N, N, N)) + 1j * rng.normal(size=(N, N, N)) + 0.5 * F
+    k = np.fft.fftfreq(N, 1.0 / N)
+    r = np.floor(np.sqrt(k[:, None, None] ** 2 + k[None, :, None] ** 2 + k[None, None, :] ** 2) + 0.5).astype(int)
+    want = np.array([(F[r == s] * np.conj(G[r == s])).sum().real / np.sqrt((np.abs(F[r == s]) ** 2).sum() * (np.abs(G[r == s]) ** 2).sum())
+                     for s in range(ns)])
+    assert np.abs(fsc(F, G) - want).max() < 1e-13 and 0.2 < want[4] < 0.7
+
+
+def test_prtf_closed_forms():
+    p = cpra_inputs.make_problem(1, Np=4, noise=False)
+    P = p.projections
+    I_c = np.fft.fftshift(np.abs(np.fft.fft2(P)) ** 2, axes=(-2, -1))
+    mask = np.ones((p.Np, p.N, p.N), np.uint8)
+    mask[:, p.N // 2 - 1:p.N // 2 + 2, p.N // 2 - 1:p.N // 2 + 2] = 0      # a 3 x 3 beamstop: rings 0 and 1 unmeasured
+    o = Oracle(p.N, p.Np)
+    o.set_data(I_c, mask)
+    t = o.prtf(P)
+    assert t[0] == 0.0 and t[1] == 0.0                                # empty rings
+    assert np.abs(t[2:] - 1.0).max() < 1e-9                           # the true projections reproduce the amplitudes
+    assert np.abs(o.prtf(0.25 * np.exp(0.3j) * P)[2:] - 0.25).max() < 1e-9
+    # averaging two reconstructions with opposite phases of one pixel ring kills that ring: PRTF measures phase consistency
+    G = np.fft.fft2(P)
+    k = np.fft.fftfreq(p.N, 1.0 / p.N)
+    ring = np.floor(np.sqrt(k[:, None] ** 2 + k[None, :] ** 2) + 0.5).astype(int) == 6
+    G2 = G.copy()
+    G2[:, ring] *= -1.0
+    t2 = o.prtf(0.5 * (P + np.fft.ifft2(G2)))
+    assert abs(t2[6]) < 1e-9 and np.abs(np.delete(t2[2:], 4) - 1.0).max() < 1e-9
