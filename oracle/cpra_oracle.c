@@ -95,11 +95,55 @@ static cplx* twiddle_table(int N, int sign)
     return tw;
 }
 
+static int is_pow2(int N);
+
+/* N not a power of two (the paper's own detector sizes, P:82 N = 160, P:98 N = 700): the 1D transform is
+ * the definition itself, X[k] = sum_x x[x] e^{sign 2 pi i k x / N}, O(N^2) per line, with the N roots of
+ * unity computed in double and rounded once.  tmp: N scratch elements. */
+static void dft1d_direct(cplx* a, int N, const cplx* root, cplx* tmp)
+{
+    for (int k = 0; k < N; ++k) {
+        real sr = 0, si = 0;
+        for (int x = 0; x < N; ++x) {
+            const cplx w = root[(int)(((long)k * x) % N)];
+            sr += a[x].re * w.re - a[x].im * w.im;
+            si += a[x].re * w.im + a[x].im * w.re;
+        }
+        tmp[k].re = sr; tmp[k].im = si;
+    }
+    for (int k = 0; k < N; ++k) a[k] = tmp[k];
+}
+static cplx* root_table(int N, int sign)
+{
+    cplx* r = (cplx*)malloc(sizeof(cplx) * (size_t)N);
+    for (int m = 0; m < N; ++m) {
+        const double ang = sign * 2.0 * PI * (double)m / (double)N;
+        r[m].re = (real)cos(ang); r[m].im = (real)sin(ang);
+    }
+    return r;
+}
+
 /* 2D transform of one N x N image, in place: all rows, then all columns (Eq. (3) is a
  * separable double sum).  sign=+1 additionally divides by N^2 (P:19 inverse FT; reading A10). */
 static void fft2d(cplx* img, int N, int sign)
 {
     cplx* col = (cplx*)malloc(sizeof(cplx) * (size_t)N);
+    if (!is_pow2(N)) {
+        cplx* root = root_table(N, sign);
+        cplx* tmp = (cplx*)malloc(sizeof(cplx) * (size_t)N);
+        for (int y = 0; y < N; ++y) dft1d_direct(img + (size_t)y * N, N, root, tmp);
+        for (int x = 0; x < N; ++x) {
+            for (int y = 0; y < N; ++y) col[y] = img[(size_t)y * N + x];
+            dft1d_direct(col, N, root, tmp);
+            for (int y = 0; y < N; ++y) img[(size_t)y * N + x] = col[y];
+        }
+        free(root); free(tmp); free(col);
+        if (sign > 0) {
+            const real s = (real)(1.0 / ((double)N * (double)N));
+            for (size_t i = 0; i < (size_t)N * N; ++i) { img[i].re *= s; img[i].im *= s; }
+        }
+        return;
+    }
     cplx* tw = twiddle_table(N, sign);
     for (int y = 0; y < N; ++y) fft1d(img + (size_t)y * N, N, tw);
     for (int x = 0; x < N; ++x) {
@@ -143,7 +187,7 @@ static int is_pow2(int N) { return N > 0 && (N & (N - 1)) == 0; }
 /* Exported FFT of a stack of `count` images (double I/O), the routine the loop itself uses. */
 int oracle_fft2(const double* in, double* out, int N, int count, int sign)
 {
-    if (!in || !out || !is_pow2(N) || count < 0 || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    if (!in || !out || N < 2 || count < 0 || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
     const size_t px = (size_t)N * N;
     #pragma omp parallel for schedule(dynamic, 1)
     for (int n = 0; n < count; ++n) {
@@ -281,7 +325,7 @@ typedef oracle_plan_s* oracle_plan_t;
 int oracle_plan(oracle_plan_t* out, int N, int Np)
 {
     if (!out) return ORACLE_ERR_INVALID_ARG;
-    if (!is_pow2(N) || N < 2 || N > 4096 || Np < 1) return ORACLE_ERR_UNSUPPORTED_SIZE;
+    if (N < 2 || N > 4096 || (N & 1) || Np < 1) return ORACLE_ERR_UNSUPPORTED_SIZE;   /* even N: the centre pixel is N/2 */
     oracle_plan_t p = (oracle_plan_t)calloc(1, sizeof(*p));
     p->N = N; p->Np = Np; p->px = (size_t)N * N;
     const size_t tot = p->px * (size_t)Np;

@@ -70,3 +70,48 @@ def test_rows_and_columns_not_transposed():
     img = np.tile(np.exp(2j * np.pi * 3 * x / N), (N, 1))            # varies along x only
     G = fft2(img)
     assert abs(G[0, 3] - N * N) < 1e-9 and np.abs(G).sum() - abs(G[0, 3]) < 1e-8
+
+
+def test_sizes_that_are_not_powers_of_two_against_numpy():
+    """The paper's own detector sizes are 160 = 2^5 5 and 700 = 2^2 5^2 7: for such N the
+    oracle's transform is the O(N^2)-per-line definition; numpy's FFT is the independent library."""
+    from oracle import fft2
+    for N in (12, 20, 28, 160):
+        rng = np.random.default_rng(N)
+        x = rng.normal(size=(2, N, N)) + 1j * rng.normal(size=(2, N, N))
+        F = fft2(x, -1)
+        assert np.abs(F - np.fft.fft2(x)).max() < 1e-10 * np.abs(F).max()
+        assert np.abs(fft2(F, +1) - x).max() < 1e-12
+    d = np.zeros((20, 20), complex)
+    d[3, 7] = 1.0
+    ky, kx = np.meshgrid(np.arange(20), np.arange(20), indexing="ij")
+    assert np.abs(fft2(d, -1) - np.exp(-2j * np.pi * (3 * ky + 7 * kx) / 20)).max() < 1e-13
+
+
+def test_loop_on_a_size_that_is_not_a_power_of_two():
+    """The whole iteration at N = 20: the true projections with exact intensities are a fixed point, and one
+    HIO iteration equals its definition evaluated with numpy's FFT."""
+    from oracle import Oracle
+    N, Np = 20, 3
+    rng = np.random.default_rng(5)
+    P = np.zeros((Np, N, N), complex)
+    P[:, 6:14, 5:13] = rng.uniform(0.2, 1.0, size=(Np, 8, 8))
+    I_c = np.fft.fftshift(np.abs(np.fft.fft2(P)) ** 2, axes=(-2, -1))
+    S = np.zeros((Np, N, N), np.uint8)
+    S[:, 5:15, 4:14] = 1
+    o = Oracle(N, Np)
+    o.set_data(I_c)
+    o.set_support(S)
+    o.set_carousel([1.0], 1)
+    o.set_estimate(P)
+    o.iterate(2, 0.9)
+    assert np.abs(o.get_projections(0) - P).max() < 1e-12 and o.get_error()[1] < 1e-12
+    g0 = rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))
+    o.set_carousel([0.6, 0.2], 1)
+    o.set_estimate(g0)
+    o.iterate(1, 0.9)
+    gh = 0.6 * g0 + 0.2 * (np.roll(g0, 1, axis=0) + np.roll(g0, -1, axis=0))
+    G = np.fft.fft2(gh)
+    gp = np.fft.ifft2(np.sqrt(np.fft.ifftshift(I_c, axes=(-2, -1))) * G / np.abs(G))
+    want = np.where(S == 1, gp, gh - 0.9 * gp)
+    assert np.abs(o.get_projections(0) - want).max() < 1e-12
