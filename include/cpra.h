@@ -294,9 +294,9 @@ int cpra_refine_3d(cpra_plan_t plan, const float* d_E, const float* d_W, const u
  *              cpra_merge_finish's output) against the measured amplitudes of cpra_set_data:
  *              PRTF(s) = mean over n and the measured pixels with A > 0 of ring s of |F2[avg_n]| / A_n.
  *   d_out: fp32 [N/2 + 1].  Shell sums are double atomics: reproducible to ~1e-15, not bit for bit.
- * Both use the error scratch (cpra_get_error is NOT_READY afterwards) and cpra_prtf the FFT scratch and the
- * spare state buffer.  Errors: INVALID_ARG, NOT_READY (cpra_prtf without data), UNSUPPORTED_SIZE (cpra_prtf
- * with Np * N / 8 < N + 2), CUDA.
+ * cpra_prtf uses the FFT scratch and the spare state buffer; the loop state is untouched.
+ * Errors: INVALID_ARG (cpra_fsc: Np != N), NOT_READY (cpra_prtf without data), UNSUPPORTED_SIZE (N not a power of
+ * two), CUDA.
  */
 int cpra_fsc(cpra_plan_t plan, const float* d_F1, const float* d_F2, float* d_out);
 int cpra_prtf(cpra_plan_t plan, const float* d_avg, float* d_out);

@@ -92,21 +92,24 @@ int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream
 {
     if (!out) return CPRA_ERR_INVALID_ARG;
     *out = nullptr;
-    if (!is_pow2(N) || N < 16 || N > 1024 || Np < 1 || Np >= (1 << 30)) return CPRA_ERR_UNSUPPORTED_SIZE;
+    const bool generic = !is_pow2(N) && gen_supported(N);
+    if ((!is_pow2(N) && !generic) || N < 16 || N > 1024 || Np < 1 || Np >= (1 << 30)) return CPRA_ERR_UNSUPPORTED_SIZE;
     if (flags & ~CPRA_FLAG_ALL) return CPRA_ERR_INVALID_ARG;
     cpra_plan_s* p = new (std::nothrow) cpra_plan_s;
     if (!p) return CPRA_ERR_INVALID_ARG;
     p->N = N; p->Np = Np; p->flags = flags;
     p->stream = (cudaStream_t)cuda_stream;
+    p->generic = generic;
     int R0 = 1, R1 = 1, R2 = 1, RL = 1, TBN = 16;
-    { auto f = [&]() -> int { CPRA_DISPATCH_N(N, R0 = Radix<NN>::R0; R1 = Radix<NN>::R1; R2 = Radix<NN>::R2; RL = last_radix<NN>(); TBN = tile_batch<NN>()); return 0; }; f(); }
-    p->geo = Geo{N, Np, R0, R1, R2, RL, TBN};
+    if (!generic) { auto f = [&]() -> int { CPRA_DISPATCH_N(N, R0 = Radix<NN>::R0; R1 = Radix<NN>::R1; R2 = Radix<NN>::R2; RL = last_radix<NN>(); TBN = tile_batch<NN>()); return 0; }; f(); }
+    p->geo = Geo{N, Np, R0, R1, R2, RL, generic ? (N <= 512 ? 16 : 8) : TBN};   // (generic: TB = lines per tile, for the error partials only)
     // reading A2: the paper's example weights
     if (Np >= 3) { p->K = 1; p->alpha[0] = 0.6f; p->alpha[1] = 0.2f; }
     else { p->K = 0; p->alpha[0] = 1.0f; }
     p->n_ei = 1;
     p->angles.assign(Np, 0.0);
-    { auto f = [&]() -> int { CPRA_DISPATCH_N(N, build_twiddles<NN>(p->h_tw)); return 0; }; f(); }
+    if (generic) gen_make_geo(N, Np, p->gg, p->h_tw);
+    else { auto f = [&]() -> int { CPRA_DISPATCH_N(N, build_twiddles<NN>(p->h_tw)); return 0; }; f(); }
     p->walk = !(flags & CPRA_FLAG_NO_WALK);
     {
         int dev = 0, sms = 0;
@@ -130,20 +133,21 @@ int cpra_destroy(cpra_plan_t p)
 int cpra_workspace_bytes(cpra_plan_t p, size_t* bytes)
 {
     if (!p || !bytes) return CPRA_ERR_INVALID_ARG;
-    *bytes = layout_of(p->N, p->Np).total;
+    *bytes = layout_of(p->N, p->Np, p->generic).total;
     return CPRA_OK;
 }
 
 int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
 {
     if (!p || !d_ws) return CPRA_ERR_INVALID_ARG;
-    const Layout L = layout_of(p->N, p->Np);
+    const Layout L = layout_of(p->N, p->Np, p->generic);
     if (bytes < L.total || ((uintptr_t)d_ws & 255)) return CPRA_ERR_WORKSPACE;
     char* w = (char*)d_ws;
     p->ws = w; p->ws_bytes = bytes;
     p->tw = (float2*)(w + L.tw);
     p->A = (float*)(w + L.A);
     p->S16 = (uint16_t*)(w + L.S16);
+    p->S8 = (unsigned char*)(w + L.S8);
     p->st[0] = (float4*)(w + L.st0);
     p->st[1] = (float4*)(w + L.st1);
     p->scr = (float4*)(w + L.scr);
@@ -154,18 +158,22 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
     p->ustart = (int*)(w + L.ustart);
     p->rays = (int*)(w + L.rays);
     p->mx = (float*)(w + L.mx);
+    p->shell = (double*)(w + L.shell);
     p->cur = 0;
     p->have_data = p->have_support = p->have_estimate = p->have_error = false;
     if (!p->attrs_set) {
         int rc = CPRA_OK;
-        { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::set_attrs()); return 0; }; f(); }
+        if (p->generic) rc = gen_set_attrs();
+        else { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::set_attrs()); return 0; }; f(); }
         if (rc != CPRA_OK) { p->ws = nullptr; return rc; }
         p->attrs_set = true;
     }
     p->have_tmap = false;
-    p->have_tmap = encode_scratch_tmap(&p->tm_scr[0], p->scr, p->N, p->Np, p->geo.TB) &&
-                   encode_scratch_tmap(&p->tm_scr[1], p->scr2, p->N, p->Np, p->geo.TB);
-    if (!p->have_tmap) { p->ws = nullptr; return CPRA_ERR_CUDA; }   // the row kernels move their tiles by TMA tensor copies
+    if (!p->generic) {
+        p->have_tmap = encode_scratch_tmap(&p->tm_scr[0], p->scr, p->N, p->Np, p->geo.TB) &&
+                       encode_scratch_tmap(&p->tm_scr[1], p->scr2, p->N, p->Np, p->geo.TB);
+        if (!p->have_tmap) { p->ws = nullptr; return CPRA_ERR_CUDA; }   // the row kernels move their tiles by TMA tensor copies
+    }
     if (cudaMemcpyAsync(p->tw, p->h_tw.data(), sizeof(float2) * p->h_tw.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) {
         p->ws = nullptr;
         return CPRA_ERR_CUDA;
@@ -178,8 +186,11 @@ int cpra_set_data(cpra_plan_t p, const float* d_I, const unsigned char* d_mask, 
     if (!p || !d_I) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     for (int n = 0; n < p->Np; ++n) p->angles[n] = h_angles ? h_angles[n] : 0.0;
-    k_set_data<<<p->Np, 256, 0, p->stream>>>(d_I, d_mask, p->A, p->den, p->geo);
-    if (int rc = check_launch(p)) return rc;
+    if (p->generic) { if (int rc = gen_set_data(p, d_I, d_mask)) return rc; }
+    else {
+        k_set_data<<<p->Np, 256, 0, p->stream>>>(d_I, d_mask, p->A, p->den, p->geo);
+        if (int rc = check_launch(p)) return rc;
+    }
     p->have_data = true;
     p->have_error = false;
     return CPRA_OK;
@@ -189,9 +200,12 @@ int cpra_set_support(cpra_plan_t p, const unsigned char* d_S)
 {
     if (!p || !d_S) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
-    const size_t total16 = (size_t)p->Np * p->N * p->N / TB;
-    k_pack_support<<<blocks_for(total16, 256), 256, 0, p->stream>>>(d_S, p->S16, p->N, total16);
-    if (int rc = check_launch(p)) return rc;
+    if (p->generic) { if (int rc = gen_set_support(p, d_S)) return rc; }
+    else {
+        const size_t total16 = (size_t)p->Np * p->N * p->N / TB;
+        k_pack_support<<<blocks_for(total16, 256), 256, 0, p->stream>>>(d_S, p->S16, p->N, total16);
+        if (int rc = check_launch(p)) return rc;
+    }
     p->have_support = true;
     return CPRA_OK;
 }
@@ -219,8 +233,11 @@ int cpra_set_estimate(cpra_plan_t p, const float* d_g0)
     if (!p || !d_g0) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     const size_t total = (size_t)p->Np * p->N * p->N;
-    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, (float*)p->st[p->cur], p->geo, total);
-    if (int rc = check_launch(p)) return rc;
+    if (p->generic) { if (int rc = gen_set_estimate(p, d_g0)) return rc; }
+    else {
+        k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, (float*)p->st[p->cur], p->geo, total);
+        if (int rc = check_launch(p)) return rc;
+    }
     p->t = 0;
     p->have_estimate = true;
     p->have_error = false;
@@ -253,6 +270,7 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     if (!p || k < 0 || !std::isfinite(beta)) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->have_data || !p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
+    if (p->generic) return gen_iterate(p, k, beta);
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
     // the walking kernel serves the default carousel (K = 1 every iteration) on plans with 8-row tiles
@@ -320,7 +338,7 @@ int cpra_get_error(cpra_plan_t p, float* d_E, float* d_Eglobal)
     if (int rc = ready(p)) return rc;
     if (!p->have_error) return CPRA_ERR_NOT_READY;
     if (!d_E && !d_Eglobal) return CPRA_OK;
-    k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, d_E, d_Eglobal, p->Np, p->N / p->geo.TB);
+    k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, d_E, d_Eglobal, p->Np, (p->N + p->geo.TB - 1) / p->geo.TB);
     return check_launch(p);
 }
 
@@ -329,6 +347,7 @@ int cpra_get_projections(cpra_plan_t p, int which, float* d_out)
     if (!p || !d_out || (which != CPRA_ITERATE && which != CPRA_SUPPORTED)) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->have_estimate || (which == CPRA_SUPPORTED && !p->have_support)) return CPRA_ERR_NOT_READY;
+    if (p->generic) return gen_get_projections(p, which, d_out);
     const size_t total = (size_t)p->Np * p->N * p->N;
     k_unpack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->st[p->cur], p->S16, (float2*)d_out, p->geo, total, which == CPRA_SUPPORTED);
     return check_launch(p);
@@ -338,6 +357,7 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
 {
     if (!p || !d_in || !d_out || (sign != 1 && sign != -1)) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
+    if (p->generic) return gen_fft2(p, d_in, d_out, sign);
     const size_t total = (size_t)p->Np * p->N * p->N;
     float4* tmp = p->st[p->cur ^ 1];
     const unsigned nb = blocks_for(total, 256);
@@ -378,6 +398,16 @@ int cpra_assemble_3d(cpra_plan_t p, float* d_vol, float* d_weight)
         cudaMemcpyAsync(p->ustart, p->h_ustart.data(), sizeof(int) * (U + 1), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
         cudaMemcpyAsync(p->rays, p->h_rays.data(), sizeof(int) * p->h_rays.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess)
         return CPRA_ERR_CUDA;
+    if (p->generic) {
+        // (i) E_n = F[S_n g_n], natural order, transposed; (ii)-(iv) the same gather
+        if (int rc = gen_slices(p, (float2*)p->scr2)) return rc;
+        const int N = p->N;
+        const int zsplit = std::max(1, std::min(N, 4096 / std::max(1, (N * N) / 256)));
+        const int zper = (N + zsplit - 1) / zsplit;
+        const dim3 grid(blocks_for((size_t)N * N, 128), (unsigned)((N + zper - 1) / zper));
+        k_assemble<<<grid, 128, 0, p->stream>>>((const float2*)p->scr2, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
+        return check_launch(p);
+    }
     // (i) E_n = F[S_n g_n] into the scratch
     int rc = CPRA_OK;
     { auto f = [&]() -> int {
@@ -425,6 +455,8 @@ int cpra_get_support(cpra_plan_t p, unsigned char* d_S)
     if (int rc = ready(p)) return rc;
     if (!p->have_support) return CPRA_ERR_NOT_READY;
     const size_t total = (size_t)p->Np * p->N * p->N;
+    if (p->generic)
+        return cudaMemcpyAsync(d_S, p->S8, total, cudaMemcpyDeviceToDevice, p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
     k_unpack_support<<<blocks_for(total, 256), 256, 0, p->stream>>>(p->S16, d_S, p->N, total);
     return check_launch(p);
 }
@@ -434,6 +466,7 @@ int cpra_shrinkwrap(cpra_plan_t p, float sigma, float threshold, float* d_blurre
     if (!p || !(sigma >= 0.f) || !(threshold >= 0.f) || !std::isfinite(sigma) || !std::isfinite(threshold)) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
+    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
     const size_t total = (size_t)p->Np * p->N * p->N, nquads = total / 2;
     float4* tmp = p->st[p->cur ^ 1];
     // |S g| -> forward 2D FT -> Gaussian transfer function -> inverse 2D FT -> per-image maximum -> threshold
@@ -472,6 +505,7 @@ int cpra_prereconstruct(cpra_plan_t p, int n, int k, float beta)
     if (int rc = ready(p)) return rc;
     if (!p->have_data || !p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
     if (k == 0) return CPRA_OK;
+    if (p->generic) return gen_prereconstruct(p, n, k, beta);
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     // the conventional 2D iteration on projection n alone: no mix, the three tile kernels on a one-image grid;
     // the image ping-pongs between the two state buffers, the other projections stay where they are
@@ -524,7 +558,7 @@ int cpra_merge_offer(cpra_plan_t p, const float* d_episode, double E)
     if (!d_episode) {
         if (int rc = ready(p)) return rc;
         if (!p->have_estimate || !p->have_support || !p->have_error) return CPRA_ERR_NOT_READY;
-        k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, nullptr, b.Ein, p->Np, p->N / p->geo.TB);
+        k_finalize_error<<<1, 256, 0, p->stream>>>(p->partial, p->den, nullptr, b.Ein, p->Np, (p->N + p->geo.TB - 1) / p->geo.TB);
         if (int rc = check_launch(p)) return rc;
         k_offer_select<<<1, 1, 0, p->stream>>>(b, b.Ein, 0.0);
     } else {
@@ -532,6 +566,13 @@ int cpra_merge_offer(cpra_plan_t p, const float* d_episode, double E)
         k_offer_select<<<1, 1, 0, p->stream>>>(b, nullptr, E);
     }
     if (int rc = check_launch(p)) return rc;
+    if (!d_episode && p->generic) {
+        // natural state: S g into the other state buffer (free between calls), then offered like a caller's episode
+        float2* tmp = (float2*)p->st[p->cur ^ 1];
+        if (int rc = gen_get_projections(p, CPRA_SUPPORTED, (float*)tmp)) return rc;
+        k_offer_copy<<<blocks_for(total, 256), 256, 0, p->stream>>>(b, tmp, nullptr, p->S16, p->geo, total);
+        return check_launch(p);
+    }
     k_offer_copy<<<blocks_for(total, 256), 256, 0, p->stream>>>(b, (const float2*)d_episode, d_episode ? nullptr : (const float*)p->st[p->cur],
                                                                  p->S16, p->geo, total);
     return check_launch(p);
@@ -583,6 +624,7 @@ int cpra_fft3(cpra_plan_t p, const float* d_in, float* d_out, int sign)
 {
     if (!p || !d_in || !d_out || (sign != 1 && sign != -1)) return CPRA_ERR_INVALID_ARG;
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;   // a cube is a stack of N slices of N x N
+    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
     int rc = cpra_fft2(p, d_in, d_out, sign);          // the (y, x) transforms of all z slices
     if (rc) return rc;
     { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::fftz(p, (float2*)d_out, sign)); return 0; }; f(); }
@@ -593,6 +635,7 @@ int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsi
 {
     if (!p || !d_E || !d_W || !d_S3 || !d_obj || k < 1) return CPRA_ERR_INVALID_ARG;
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
+    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
     if (int rc = ready(p)) return rc;
     const size_t n3 = (size_t)p->N * p->N * p->N;
     const int nblk = (int)std::min<size_t>(512, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
@@ -625,12 +668,11 @@ int cpra_fsc(cpra_plan_t p, const float* d_F1, const float* d_F2, float* d_out)
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     const int ns = p->N / 2 + 1;
-    double* acc = p->partial;   // >= 3 (N/2 + 1) doubles for every supported N with Np = N
+    double* acc = p->shell;
     if (cudaMemsetAsync(acc, 0, sizeof(double) * 3 * ns, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
     k_fsc_accumulate<<<4 * p->sms, 256, sizeof(double) * 3 * ns, p->stream>>>((const float2*)d_F1, (const float2*)d_F2, acc, p->N);
     if (int rc = check_launch(p)) return rc;
     k_fsc_finalize<<<blocks_for(ns, 128), 128, 0, p->stream>>>(acc, d_out, ns);
-    p->have_error = false;
     return check_launch(p);
 }
 
@@ -639,9 +681,9 @@ int cpra_prtf(cpra_plan_t p, const float* d_avg, float* d_out)
     if (!p || !d_avg || !d_out) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->have_data) return CPRA_ERR_NOT_READY;
+    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
     const size_t total = (size_t)p->Np * p->N * p->N;
     const int ns = p->N / 2 + 1;
-    if ((size_t)2 * ns > (size_t)p->Np * (p->N / 8)) return CPRA_ERR_UNSUPPORTED_SIZE;   // the shell sums live in the error scratch
     float4* tmp = p->st[p->cur ^ 1];
     k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_avg, (float*)tmp, p->geo, total);
     int rc = check_launch(p);
@@ -652,12 +694,11 @@ int cpra_prtf(cpra_plan_t p, const float* d_avg, float* d_out)
             if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
         return 0; }; f(); }
     if (rc) return rc;
-    double* acc = p->partial;
+    double* acc = p->shell;
     if (cudaMemsetAsync(acc, 0, sizeof(double) * 2 * ns, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
     k_prtf_accumulate<<<4 * p->sms, 256, sizeof(double) * 2 * ns, p->stream>>>((const float*)p->scr, p->A, acc, p->geo, total);
     if ((rc = check_launch(p))) return rc;
     k_prtf_finalize<<<blocks_for(ns, 128), 128, 0, p->stream>>>(acc, d_out, ns);
-    p->have_error = false;   // the error scratch held the shell sums
     return check_launch(p);
 }
 

@@ -16,6 +16,7 @@
 #include "cpra_image.cuh"
 #include "cpra_cluster.cuh"
 #include "cpra_walk.cuh"
+#include "cpra_generic.cuh"
 
 struct cpra_plan_s {
     int N = 0, Np = 0;
@@ -39,6 +40,7 @@ struct cpra_plan_s {
     int* ustart = nullptr;
     int* rays = nullptr;
     float* mx = nullptr;      // per-image maxima of the shrink-wrap update
+    double* shell = nullptr;  // shell sums of cpra_fsc / cpra_prtf
     int cur = 0;
     // parameters / state
     int K = 1;
@@ -47,6 +49,10 @@ struct cpra_plan_s {
     int update = CPRA_UPDATE_HIO;
     int flip_seam = 0;        // cpra_set_seam
     int walk_ctas = 0;        // cpra_set_walk_ctas: CTAs per SM of the fused row kernel (0 = library default)
+    // sizes that are not powers of two (cpra_generic.cuh): natural-layout buffers in the same workspace
+    bool generic = false;
+    cpra::GenGeo gg{};
+    unsigned char* S8 = nullptr;   // support, u8 [Np][N][N]
     int cluster = 0;          // cpra_set_cluster: CTAs per image of the whole-image kernel (0 = library default, -1 = never)
     // Step C bank (cpra_merge_*): caller-owned device buffer
     char* bank_buf = nullptr;
@@ -82,10 +88,10 @@ struct Carve {
 };
 
 struct Layout {
-    size_t tw, A, S16, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, mx, total;
+    size_t tw, A, S16, S8, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, mx, shell, total;
 };
 
-inline Layout layout_of(int N, int Np)
+inline Layout layout_of(int N, int Np, bool generic = false)
 {
     const size_t px = (size_t)Np * N * N;
     Carve c;
@@ -93,16 +99,18 @@ inline Layout layout_of(int N, int Np)
     L.tw = c.take(sizeof(float2) * 1024);   // >= tw_count<N>() for every N
     L.A = c.take(sizeof(float) * px);
     L.S16 = c.take(px / 8);
+    L.S8 = c.take(generic ? px : 0);   // sizes that are not powers of two keep the support as bytes
     L.st0 = c.take(sizeof(float2) * px);
     L.st1 = c.take(sizeof(float2) * px);
     L.scr = c.take(sizeof(float2) * px);
     L.scr2 = c.take(sizeof(float2) * px);
-    L.partial = c.take(sizeof(double) * (size_t)Np * (N / 8));   // >= N / Radix<N>::TB tiles per image
+    L.partial = c.take(sizeof(double) * (size_t)Np * (N / 8 + 1));   // >= N / Radix<N>::TB (or ceil(N / W)) tiles per image
     L.den = c.take(sizeof(double) * Np);
     L.uphi = c.take(sizeof(double) * 2 * Np);
     L.ustart = c.take(sizeof(int) * (2 * (size_t)Np + 1));
     L.rays = c.take(sizeof(int) * 2 * (size_t)Np);
     L.mx = c.take(sizeof(float) * (size_t)Np);
+    L.shell = c.take(sizeof(double) * 3 * (size_t)(N / 2 + 1));   // shell sums of cpra_fsc / cpra_prtf
     L.total = c.off;
     return L;
 }
@@ -489,6 +497,19 @@ bool Launch<N>::image_cl_ok(int C)
     return (C == 1 && cl_ok<N, 1>()) || (C == 2 && cl_ok<N, 2>()) || (C == 4 && cl_ok<N, 4>()) || (C == 8 && cl_ok<N, 8>()) ||
            (C == 16 && cl_ok<N, 16>());
 }
+
+// host side of cpra_generic.cuh (cpra_generic.cu)
+bool gen_supported(int N);
+void gen_make_geo(int N, int Np, GenGeo& g, std::vector<float2>& tw);
+int gen_set_attrs();
+int gen_set_data(cpra_plan_s* p, const float* d_I, const unsigned char* d_mask);
+int gen_set_support(cpra_plan_s* p, const unsigned char* d_S);
+int gen_set_estimate(cpra_plan_s* p, const float* d_g0);
+int gen_iterate(cpra_plan_s* p, int k, float beta);
+int gen_prereconstruct(cpra_plan_s* p, int n, int k, float beta);
+int gen_get_projections(cpra_plan_s* p, int which, float* d_out);
+int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign);
+int gen_slices(cpra_plan_s* p, float2* Et);   // E_n = F[S_n g_n], natural, transposed to [n][ku][kz]
 
 #define CPRA_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
 #ifndef CPRA_INST_N

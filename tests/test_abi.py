@@ -37,8 +37,11 @@ def test_host_only_argument_validation():
     L = cpra.lib()
     h = ctypes.c_void_p()
     assert L.cpra_plan(None, 64, 4, 0, None) == cpra.ERR_INVALID_ARG
-    for N in (0, 8, 48, 100, 2048):
+    for N in (0, 8, 15, 22, 34, 1026, 2048):      # too small / odd / a prime factor above 7 / too large
         assert L.cpra_plan(ctypes.byref(h), N, 4, 0, None) == cpra.ERR_UNSUPPORTED_SIZE
+    for N in (48, 100, 160, 700):                 # 2^a 3^b 5^c 7^d: the mixed-radix path (the paper's 160 and 700 among them)
+        assert L.cpra_plan(ctypes.byref(h), N, 4, 0, None) == cpra.CPRA_OK
+        assert L.cpra_destroy(h) == cpra.CPRA_OK
     assert L.cpra_plan(ctypes.byref(h), 64, 0, 0, None) == cpra.ERR_UNSUPPORTED_SIZE
     assert L.cpra_plan(ctypes.byref(h), 64, 5, 8, None) == cpra.ERR_INVALID_ARG       # undefined flag bit
     assert L.cpra_plan(ctypes.byref(h), 64, 5, cpra.FLAG_NO_WALK | cpra.FLAG_NO_CHUNKING, None) == cpra.CPRA_OK
@@ -79,7 +82,7 @@ def test_no_cpu_fallback_without_a_device():
         cpra.Plan(64, 4)
     assert e.value.code == cpra.ERR_CUDA
     with pytest.raises(cpra.CpraError) as e:
-        cpra.Plan(100, 4)
+        cpra.Plan(22, 4)
     assert e.value.code == cpra.ERR_UNSUPPORTED_SIZE
 
 

@@ -350,3 +350,72 @@ def test_prtf(torch_cuda, cfg, Np, N):
     got = g.prtf(torch_cuda.from_numpy(avg).cuda()).cpu().numpy()
     assert np.abs(got - want).max() <= 2e-5 * max(1.0, np.abs(want).max())
     assert want[p.N // 4] > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# f4: sizes that are not powers of two (PAPER.md:82 N = 160, :98 N = 700): the mixed-radix path
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [20, 48, 100, 160, 224, 700])
+def test_fft2_mixed_radix(torch_cuda, N):
+    import paper_2402_05283_b200 as cpra
+    Np = 2
+    rng = np.random.default_rng(N)
+    x = (rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))).astype(np.complex64)
+    plan = cpra.Plan(N, Np)
+    F = plan.fft2(torch_cuda.from_numpy(x).cuda(), -1).cpu().numpy()
+    ref = np.fft.fft2(x.astype(np.complex128))
+    assert rel_l2(F, ref) < 3e-6, rel_l2(F, ref)
+    assert rel_l2(plan.fft2(torch_cuda.from_numpy(F).cuda(), +1).cpu().numpy(), x) < 4e-6
+    d = np.zeros((Np, N, N), np.complex64)
+    d[:, 3, 5] = 1.0
+    Fd = plan.fft2(torch_cuda.from_numpy(d).cuda(), -1).cpu().numpy()
+    ky, kx = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    assert np.abs(Fd[1] - np.exp(-2j * np.pi * (3 * ky + 5 * kx) / N)).max() < 2e-5
+
+
+@pytest.mark.parametrize("N,Np,alpha,n_ei,seam,rule", [
+    (160, 6, (0.6, 0.2), 1, 0, "hio"), (160, 5, (0.5, 0.2, 0.05), 2, 1, "raar"), (48, 7, (0.6, 0.2), 1, 1, "hio"),
+    (100, 3, (0.6, 0.2), 3, 0, "er"), (700, 3, (0.6, 0.2), 1, 0, "hio"), (20, 1, (1.0,), 1, 0, "hio")])
+def test_loop_mixed_radix(torch_cuda, N, Np, alpha, n_ei, seam, rule):
+    """The loop at the paper's own detector sizes (160, 700) and other 2^a 3^b 5^c 7^d sizes against the oracle,
+    whose transform for these N is the O(N^2)-per-line definition."""
+    p = cpra_inputs.random_stack(N, Np, seed=700 + N + Np, beamstop=3)
+    o, g = _oracle(p, alpha, n_ei), _gpu(p, alpha, n_ei)
+    o.set_seam(seam); g.set_seam(bool(seam))
+    o.set_update(rule); g.set_update(rule)
+    k = 2 if N == 700 else 4
+    o.iterate(k, 0.9)
+    g.iterate(k, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= k * TOL_1
+    assert rel_l2(_get(g, 1), o.get_projections(1)) <= k * TOL_1
+    E, Eg = g.get_error()
+    Eo, Ego = o.get_error()
+    assert np.abs(E.cpu().numpy() - Eo).max() <= TOL_E * Eo.max() and abs(float(Eg.cpu()[0]) - Ego) <= TOL_E * Ego
+    # split calls are bit-identical; Step A and the bank work on these sizes too
+    h = _gpu(p, alpha, n_ei); h.set_seam(bool(seam)); h.set_update(rule)
+    for kk in ([1, 1] if k == 2 else [1, 2, 1]):
+        h.iterate(kk, 0.9)
+    assert np.array_equal(_get(h).view(np.uint32), _get(g).view(np.uint32))
+    o.prereconstruct(0, 2, 0.9)
+    g.prereconstruct(0, 2, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= (k + 2) * TOL_1
+
+
+def test_assembly_and_merge_mixed_radix(torch_cuda):
+    """Config 1 scaled to N = 160 (the paper's oxide-particle detector size): three iterations, the
+    Fourier-slice assembly and a merge from the plan, against the oracle."""
+    p = cpra_inputs.make_problem(1, Np=6, N=160)
+    o, g = _oracle(p), _gpu(p)
+    o.iterate(3, p.beta)
+    g.iterate(3, p.beta)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 3 * TOL_1
+    vo, wo = o.assemble_3d()
+    vg, wg = g.assemble_3d()
+    assert np.array_equal(wg.cpu().numpy().astype(np.float64), wo)
+    assert rel_l2(vg.cpu().numpy(), vo) <= 3 * TOL_1
+    o.merge_begin(2); g.merge_begin(2)
+    o.merge_offer(); g.merge_offer()
+    out_o, sh_o, tw_o = o.merge_finish(0)
+    out_g, sh_g, tw_g = g.merge_finish(0)
+    assert np.array_equal(sh_g.cpu().numpy()[:len(sh_o)], sh_o)       # (one episode kept of the two slots)
+    assert rel_l2(out_g.cpu().numpy(), out_o) <= 3 * TOL_1
