@@ -15,7 +15,7 @@ bool gen_supported(int N)
 // stages: 8s, then 4 / 2, then 3s, 5s, 7s; W = lines per tile; tw[m] = e^{-2 pi i m / N}
 void gen_make_geo(int N, int Np, GenGeo& g, std::vector<float2>& tw)
 {
-    g.N = N; g.Np = Np; g.W = N <= 512 ? 16 : 8; g.nf = 0;
+    g.N = N; g.Np = Np; g.W = N <= 256 ? 16 : (N <= 512 ? 8 : 4); g.nf = 0;   // lines per tile: 3-4 CTAs of 256 threads per SM
     int n = N;
     while (n % 8 == 0) { g.radix[g.nf++] = 8; n /= 8; }
     if (n % 4 == 0) { g.radix[g.nf++] = 4; n /= 4; }
@@ -37,6 +37,10 @@ int gen_set_attrs()
     acc(allow_smem(k_gen_row_fwd, SM));
     acc(allow_smem(k_gen_col, SM));
     acc(allow_smem(k_gen_row_inv, SM));
+    // as much shared memory as the SM has, whatever one block asks for (the default carveout fits fewer blocks)
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_row_fwd), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_row_inv), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
 }
 

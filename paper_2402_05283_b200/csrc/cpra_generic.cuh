@@ -17,7 +17,9 @@ struct GenGeo {
     int radix[GEN_MAXF];
 };
 constexpr int GEN_NT = 256;
-__host__ __device__ __forceinline__ int gen_wp(int W) { return W + 1; }
+// line stride of a position in shared memory, in complex numbers: even, so that the pair of lines (w, w + 1), w
+// even, is one aligned 16-byte access
+__host__ __device__ __forceinline__ int gen_wp(int W) { return W + 2; }
 __host__ __device__ __forceinline__ size_t gen_smem_bytes(int N, int W) { return (size_t)2 * N * gen_wp(W) * 8 + (size_t)N * 8 + 32 * 8 + 16; }
 
 }  // namespace cpra

@@ -7,51 +7,84 @@ namespace cpra {
 
 __device__ __forceinline__ float2 cm(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
-// W lines of length N in a (stride W + 1), result in the returned buffer; tw[m] = e^{-2 pi i m / N} in shared memory
-__device__ float2* gen_fft(float2* a, float2* b, const float2* __restrict__ tw, const GenGeo& g, bool inverse)
+// two lines (w, w + 1) as one packed value: the 16 bytes (re_w, im_w, re_w1, im_w1) of shared memory <-> c2
+__device__ __forceinline__ c2 gen_ld2(const float2* p) { const float4 q = *reinterpret_cast<const float4*>(p); return c2{make_float2(q.x, q.z), make_float2(q.y, q.w)}; }
+__device__ __forceinline__ void gen_st2(float2* p, c2 v) { *reinterpret_cast<float4*>(p) = make_float4(v.re.x, v.im.x, v.re.y, v.im.y); }
+
+// r-point DFT of packed values: the butterfly networks of cpra_fft.cuh for r = 2, 4, 8; the definition
+// out[p] = sum_q v[q] w_r^{pq} with the roots from the table for r = 3, 5, 7
+template <int R, bool INV>
+__device__ __forceinline__ void gen_small_dft(c2 (&v)[R], const float2* __restrict__ tw, int rstep)
 {
-    const int N = g.N, W = g.W, Wp = gen_wp(W);
+    if constexpr (R == 2 || R == 4 || R == 8) {
+        dft<R, INV>(v);
+    } else {
+        c2 o[R];
+#pragma unroll
+        for (int p = 0; p < R; ++p) {
+            c2 acc = v[0];
+#pragma unroll
+            for (int q = 1; q < R; ++q) {
+                const float2 t = tw[((p * q) % R) * rstep];
+                const c2 y = INV ? cmulc(v[q], bc(t.x), bc(t.y)) : cmul(v[q], bc(t.x), bc(t.y));
+                acc = cadd(acc, y);
+            }
+            o[p] = acc;
+        }
+#pragma unroll
+        for (int p = 0; p < R; ++p) v[p] = o[p];
+    }
+}
+
+// one Stockham stage of radix R over W lines (W / 2 packed pairs per position): a -> b
+template <int R, bool INV>
+__device__ __forceinline__ void gen_stage(const float2* __restrict__ a, float2* __restrict__ b, const float2* __restrict__ tw,
+                                          int N, int W, int Ns)
+{
+    const int Wp = gen_wp(W), W2 = W / 2, m = N / R, tstep = N / (Ns * R), rstep = N / R;
+    for (int i = threadIdx.x; i < m * W2; i += blockDim.x) {
+        const int w = 2 * (i % W2), j = i / W2, k = j % Ns;
+        c2 v[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            v[q] = gen_ld2(a + (j + q * m) * Wp + w);
+            if (q > 0 && Ns > 1) {
+                const float2 t = tw[q * k * tstep];          // q k tstep < N: no reduction needed
+                v[q] = INV ? cmulc(v[q], bc(t.x), bc(t.y)) : cmul(v[q], bc(t.x), bc(t.y));
+            }
+        }
+        gen_small_dft<R, INV>(v, tw, rstep);
+        const int j0 = (j / Ns) * Ns * R + k;
+#pragma unroll
+        for (int p = 0; p < R; ++p) gen_st2(b + (j0 + p * Ns) * Wp + w, v[p]);
+    }
+}
+
+// W lines of length N in a (element x of line w at x * gen_wp(W) + w), result in the returned buffer;
+// tw[m] = e^{-2 pi i m / N} in shared memory
+template <bool INV>
+__device__ float2* gen_fft_t(float2* a, float2* b, const float2* __restrict__ tw, const GenGeo& g)
+{
     int Ns = 1;
     for (int f = 0; f < g.nf; ++f) {
-        const int r = g.radix[f], m = N / r, tstep = N / (Ns * r), rstep = N / r;
-        for (int i = threadIdx.x; i < m * W; i += blockDim.x) {
-            const int w = i % W, j = i / W, k = j % Ns;
-            float2 v[8];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                if (q < r) {
-                    float2 x = a[(j + q * m) * Wp + w];
-                    if (q > 0 && k > 0) {
-                        float2 t = tw[(q * k * tstep) % N];
-                        if (inverse) t.y = -t.y;
-                        x = cm(x, t);
-                    }
-                    v[q] = x;
-                }
-            }
-            const int j0 = (j / Ns) * Ns * r + k;
-#pragma unroll
-            for (int p = 0; p < 8; ++p) {
-                if (p < r) {
-                    float2 acc = v[0];
-#pragma unroll
-                    for (int q = 1; q < 8; ++q) {
-                        if (q < r) {
-                            float2 t = tw[((p * q) % r) * rstep];
-                            if (inverse) t.y = -t.y;
-                            const float2 y = cm(v[q], t);
-                            acc.x += y.x; acc.y += y.y;
-                        }
-                    }
-                    b[(j0 + p * Ns) * Wp + w] = acc;
-                }
-            }
+        const int r = g.radix[f];
+        switch (r) {
+            case 8: gen_stage<8, INV>(a, b, tw, g.N, g.W, Ns); break;
+            case 4: gen_stage<4, INV>(a, b, tw, g.N, g.W, Ns); break;
+            case 2: gen_stage<2, INV>(a, b, tw, g.N, g.W, Ns); break;
+            case 3: gen_stage<3, INV>(a, b, tw, g.N, g.W, Ns); break;
+            case 5: gen_stage<5, INV>(a, b, tw, g.N, g.W, Ns); break;
+            default: gen_stage<7, INV>(a, b, tw, g.N, g.W, Ns); break;
         }
         __syncthreads();
         float2* t = a; a = b; b = t;
         Ns *= r;
     }
     return a;
+}
+__device__ __forceinline__ float2* gen_fft(float2* a, float2* b, const float2* __restrict__ tw, const GenGeo& g, bool inverse)
+{
+    return inverse ? gen_fft_t<true>(a, b, tw, g) : gen_fft_t<false>(a, b, tw, g);
 }
 
 struct GenSmem {
@@ -93,7 +126,7 @@ __device__ __forceinline__ float2 gen_mix(const float2* __restrict__ g, const Ge
 
 // K1: mix + forward FFT along x of W rows; spectrum rows to scr (natural [n][y][kx]).  mask_mode: multiply by the
 // support first (the slices of the assembly); ghat_out: also store the mixed input (for the update of K3).
-__global__ void __launch_bounds__(GEN_NT)
+__global__ void __launch_bounds__(GEN_NT, 3)
 k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const float2* __restrict__ twg, const unsigned char* __restrict__ S,
               MixParams mp, GenGeo gg, int n0, int fires, int mask_mode, float2* __restrict__ ghat_out)
 {
@@ -104,27 +137,34 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
     const int n = n0 + (int)(blockIdx.x / tiles), y0 = (int)(blockIdx.x % tiles) * W;
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
-    for (int i = threadIdx.x; i < N * W; i += blockDim.x) {
-        const int x = i % N, w = i / N, y = y0 + w;
-        float2 v = make_float2(0.f, 0.f);
-        if (y < N) {
-            v = gen_mix(cur, gg, mp, n, y, x, fires != 0);
-            if (mask_mode && !S[(size_t)n * px + (size_t)y * N + x]) v = make_float2(0.f, 0.f);
-            if (ghat_out) ghat_out[(size_t)n * px + (size_t)y * N + x] = v;
+    // a warp takes whole lines (x over the lanes: coalesced); unrolled so that several loads are in flight per thread
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int w = wid; w < W; w += nw) {
+        const int y = y0 + w;
+#pragma unroll 8
+        for (int x = lane; x < N; x += 32) {
+            float2 v = make_float2(0.f, 0.f);
+            if (y < N) {
+                v = gen_mix(cur, gg, mp, n, y, x, fires != 0);
+                if (mask_mode && !S[(size_t)n * px + (size_t)y * N + x]) v = make_float2(0.f, 0.f);
+                if (ghat_out) ghat_out[(size_t)n * px + (size_t)y * N + x] = v;
+            }
+            s.a[x * Wp + w] = v;
         }
-        s.a[x * Wp + w] = v;
     }
     __syncthreads();
     const float2* r = gen_fft(s.a, s.b, s.tw, gg, false);
-    for (int i = threadIdx.x; i < N * W; i += blockDim.x) {
-        const int x = i % N, w = i / N, y = y0 + w;
-        if (y < N) scr[(size_t)n * px + (size_t)y * N + x] = r[x * Wp + w];
+    for (int w = wid; w < W; w += nw) {
+        const int y = y0 + w;
+        if (y >= N) continue;
+#pragma unroll 8
+        for (int x = lane; x < N; x += 32) scr[(size_t)n * px + (size_t)y * N + x] = r[x * Wp + w];
     }
 }
 
 // K2: W columns: forward FFT along y, error metric + Fourier-modulus constraint, inverse FFT along y (unnormalised);
 // mode 0 = all three, 1 = forward only, 2 = inverse only.  A: natural native order, A < 0 = unmeasured.
-__global__ void __launch_bounds__(GEN_NT)
+__global__ void __launch_bounds__(GEN_NT, 3)
 k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* __restrict__ twg, double* __restrict__ partial,
           GenGeo gg, int n0, int mode, float scale)
 {
@@ -135,21 +175,33 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     const int n = n0 + (int)(blockIdx.x / tiles), tile = (int)(blockIdx.x % tiles), x0 = tile * W;
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
-    for (int i = threadIdx.x; i < N * W; i += blockDim.x) {
-        const int w = i % W, y = i / W, x = x0 + w;
-        s.a[y * Wp + w] = x < N ? scr[(size_t)n * px + (size_t)y * N + x] : make_float2(0.f, 0.f);
+    // thread -> (column w of the tile, rows r0, r0 + rstep, ...): a row segment of W complex numbers is contiguous
+    const int cw = threadIdx.x % W, r0 = threadIdx.x / W, rstep = blockDim.x / W, cx = x0 + cw;
+    // the tile arrives by asynchronous 8-byte copies (all of a thread's rows in flight at once); sqrt(I) of the tile is
+    // requested into L2 meanwhile
+    if (cx < N) {
+        for (int y = r0; y < N; y += rstep) {
+            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + y * Wp + cw);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(scr + (size_t)n * px + (size_t)y * N + cx) : "memory");
+        }
+        if (mode == 0 && (cw & 7) == 0)
+            for (int y = r0; y < N; y += rstep) asm volatile("prefetch.global.L2 [%0];" ::"l"(A + (size_t)n * px + (size_t)y * N + cx));
+    } else {
+        for (int y = r0; y < N; y += rstep) s.a[y * Wp + cw] = make_float2(0.f, 0.f);
     }
+    asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();
     float2* r = s.a;
     float2* other = s.b;
     if (mode != 2) { r = gen_fft(s.a, s.b, s.tw, gg, false); other = (r == s.a) ? s.b : s.a; }
     if (mode == 0) {
         double acc = 0.0;
-        for (int i = threadIdx.x; i < N * W; i += blockDim.x) {
-            const int w = i % W, ky = i / W, x = x0 + w;
+#pragma unroll 8
+        for (int ky = r0; ky < N; ky += rstep) {
+            const int w = cw, x = cx;
             if (x >= N) continue;
             float2 G = r[ky * Wp + w];
-            const float a = A[(size_t)n * px + (size_t)ky * N + x];
+            const float a = __ldg(A + (size_t)n * px + (size_t)ky * N + x);
             float f = scale;
             if (a >= 0.f) {
                 const float m2 = G.x * G.x + G.y * G.y;
@@ -177,15 +229,15 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
         }
     }
     if (mode != 1) r = gen_fft(r, other, s.tw, gg, true);
-    for (int i = threadIdx.x; i < N * W; i += blockDim.x) {
-        const int w = i % W, y = i / W, x = x0 + w;
-        if (x < N) scr[(size_t)n * px + (size_t)y * N + x] = r[y * Wp + w];
+    if (cx < N) {
+#pragma unroll 8
+        for (int y = r0; y < N; y += rstep) scr[(size_t)n * px + (size_t)y * N + cx] = r[y * Wp + cw];
     }
 }
 
 // K3: inverse FFT along x of W rows (times `scale`) + support / update (cpra_set_update); hio = 0: plain
 // scaled inverse transform.  ghat: the mixed input stored by K1, or NULL = re-mix from the previous state.
-__global__ void __launch_bounds__(GEN_NT)
+__global__ void __launch_bounds__(GEN_NT, 3)
 k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, float2* __restrict__ nxt, const float2* __restrict__ twg,
               const unsigned char* __restrict__ S, MixParams mp, GenGeo gg, int n0, int fires, int hio, float scale,
               const float2* __restrict__ ghat)
@@ -197,15 +249,20 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     const int n = n0 + (int)(blockIdx.x / tiles), y0 = (int)(blockIdx.x % tiles) * W;
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
-    for (int i = threadIdx.x; i < N * W; i += blockDim.x) {
-        const int x = i % N, w = i / N, y = y0 + w;
-        s.a[x * Wp + w] = y < N ? scr[(size_t)n * px + (size_t)y * N + x] : make_float2(0.f, 0.f);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int w = wid; w < W; w += nw) {
+        const int y = y0 + w;
+#pragma unroll 8
+        for (int x = lane; x < N; x += 32)
+            s.a[x * Wp + w] = y < N ? __ldg(scr + (size_t)n * px + (size_t)y * N + x) : make_float2(0.f, 0.f);
     }
     __syncthreads();
     const float2* r = gen_fft(s.a, s.b, s.tw, gg, true);
-    for (int i = threadIdx.x; i < N * W; i += blockDim.x) {
-        const int x = i % N, w = i / N, y = y0 + w;
-        if (y >= N) continue;
+    for (int w = wid; w < W; w += nw) {
+      const int y = y0 + w;
+      if (y >= N) continue;
+#pragma unroll 8
+      for (int x = lane; x < N; x += 32) {
         const size_t o = (size_t)n * px + (size_t)y * N + x;
         float2 gp = r[x * Wp + w];
         gp.x *= scale; gp.y *= scale;
@@ -214,6 +271,7 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
             gp = make_float2(fmaf(mp.c_gp, gp.x, mp.c_ghat * gh.x), fmaf(mp.c_gp, gp.y, mp.c_ghat * gh.y));
         }
         nxt[o] = gp;
+      }
     }
 }
 
