@@ -207,6 +207,16 @@ int cpra_fft2(cpra_plan_t plan, const float* d_in, float* d_out, int sign);
 int cpra_set_seam(cpra_plan_t plan, int flip);
 
 /*
+ * Positivity in the real-space step (the conventional companion of the support constraint for
+ * real, non-negative objects): with on = 1 a pixel INSIDE the support whose modulus-constrained estimate has
+ * Re g' < 0 is updated like a pixel outside it (HIO: ghat - beta g'; RAAR / ER accordingly).  Default 0: support
+ * only (reading A7: the headline object is complex).  The decision is a sign test in fp32, so it is not
+ * continuous in the data: two arithmetics agree on it except at pixels with |Re g'| within rounding of zero.
+ * Errors: INVALID_ARG.
+ */
+int cpra_set_positivity(cpra_plan_t plan, int on);
+
+/*
  * Shrink-wrap update of the support ("2D CSWA" ref [35]; "At the end of each episode, we perform
  * an extra 2D CSWA iteration to obtain a tighter space constraint"; reading A23).  For every n:
  *     b_n = G_sigma * |S_n g_n|     periodic Gaussian blur, sigma in pixels, of the supported estimate

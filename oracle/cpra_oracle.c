@@ -264,10 +264,11 @@ static double modulus_image(cplx* G, const real* A, const unsigned char* M, size
 /* Support / HIO update on one image (Fienup's hybrid input-output, P:98 ref [22]; beta P:104;
  * readings A6, A7: fixed support, no positivity, complex componentwise):
  *   S=1: g <- g' ;  S=0: g <- ghat - beta g'.   ghat is overwritten with the new g. */
-static void hio_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px, real beta)
+/* `pos` (oracle_set_positivity): a pixel inside the support with Re g' < 0 counts as outside. */
+static void hio_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px, real beta, int pos)
 {
     for (size_t i = 0; i < px; ++i) {
-        if (S[i]) { ghat[i] = gp[i]; }
+        if (S[i] && !(pos && gp[i].re < 0)) { ghat[i] = gp[i]; }
         else { ghat[i].re -= beta * gp[i].re; ghat[i].im -= beta * gp[i].im; }
     }
 }
@@ -280,20 +281,20 @@ static void hio_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t
 #define ORACLE_UPDATE_HIO 0
 #define ORACLE_UPDATE_RAAR 1
 #define ORACLE_UPDATE_ER 2
-static void raar_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px, real beta)
+static void raar_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px, real beta, int pos)
 {
     for (size_t i = 0; i < px; ++i) {
-        if (S[i]) { ghat[i] = gp[i]; }
+        if (S[i] && !(pos && gp[i].re < 0)) { ghat[i] = gp[i]; }
         else {
             ghat[i].re = beta * ghat[i].re + ((real)1 - (real)2 * beta) * gp[i].re;
             ghat[i].im = beta * ghat[i].im + ((real)1 - (real)2 * beta) * gp[i].im;
         }
     }
 }
-static void er_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px)
+static void er_image(cplx* ghat, const cplx* gp, const unsigned char* S, size_t px, int pos)
 {
     for (size_t i = 0; i < px; ++i) {
-        if (S[i]) { ghat[i] = gp[i]; }
+        if (S[i] && !(pos && gp[i].re < 0)) { ghat[i] = gp[i]; }
         else { ghat[i].re = 0; ghat[i].im = 0; }
     }
 }
@@ -312,6 +313,7 @@ typedef struct oracle_plan_s {
     cplx* g;              /* state */
     cplx* tmp;            /* mixed copy ghat */
     int K; real alpha[64]; int n_ei;
+    int positivity;       /* oracle_set_positivity */
     int flip_seam;        /* reading A5b: mirror the neighbours taken across the ends of the stack */
     /* Step C bank (oracle_merge_*): the N_l lowest-error episodes offered so far */
     int NL, bank_count; cplx* bank; double* bank_E;
@@ -439,9 +441,9 @@ int oracle_iterate(oracle_plan_t p, int k, double beta_d)
             fft2d(G, N, -1);                                                     /* 2 */
             const double num = modulus_image(G, p->A + (size_t)n * px, p->M + (size_t)n * px, px); /* 3, 4 */
             fft2d(G, N, +1);                                                     /* 5 */
-            if (p->update == ORACLE_UPDATE_RAAR) raar_image(ghat, G, p->S + (size_t)n * px, px, beta);
-            else if (p->update == ORACLE_UPDATE_ER) er_image(ghat, G, p->S + (size_t)n * px, px);
-            else hio_image(ghat, G, p->S + (size_t)n * px, px, beta);            /* 6 */
+            if (p->update == ORACLE_UPDATE_RAAR) raar_image(ghat, G, p->S + (size_t)n * px, px, beta, p->positivity);
+            else if (p->update == ORACLE_UPDATE_ER) er_image(ghat, G, p->S + (size_t)n * px, px, p->positivity);
+            else hio_image(ghat, G, p->S + (size_t)n * px, px, beta, p->positivity);            /* 6 */
             free(G);
             p->E[n] = p->den[n] > 0.0 ? sqrt(num / p->den[n]) : 0.0;
             numtot += num; dentot += p->den[n];
@@ -515,7 +517,7 @@ int oracle_hio(double* ghat, const double* gp, const unsigned char* S, int N, do
         a[i].re = (real)ghat[2 * i]; a[i].im = (real)ghat[2 * i + 1];
         b[i].re = (real)gp[2 * i]; b[i].im = (real)gp[2 * i + 1];
     }
-    hio_image(a, b, S, px, (real)beta);
+    hio_image(a, b, S, px, (real)beta, 0);
     for (size_t i = 0; i < px; ++i) { ghat[2 * i] = a[i].re; ghat[2 * i + 1] = a[i].im; }
     free(a); free(b);
     return ORACLE_OK;
@@ -661,6 +663,13 @@ int oracle_assemble_3d(oracle_plan_t p, double* vol, double* weight)
 /* ------------------------------------------------------------------------------------------ */
 
 /* flip = 1: neighbours taken across the ends of the stack are mirrored in u (see mix_stack). */
+int oracle_set_positivity(oracle_plan_t p, int on)
+{
+    if (!p || (on != 0 && on != 1)) return ORACLE_ERR_INVALID_ARG;
+    p->positivity = on;
+    return ORACLE_OK;
+}
+
 int oracle_set_seam(oracle_plan_t p, int flip)
 {
     if (!p || (flip != 0 && flip != 1)) return ORACLE_ERR_INVALID_ARG;
@@ -776,9 +785,9 @@ int oracle_prereconstruct(oracle_plan_t p, int n, int k, double beta_d)
         fft2d(G, p->N, -1);
         (void)modulus_image(G, p->A + (size_t)n * px, p->M + (size_t)n * px, px);
         fft2d(G, p->N, +1);
-        if (p->update == ORACLE_UPDATE_RAAR) raar_image(ghat, G, p->S + (size_t)n * px, px, beta);
-        else if (p->update == ORACLE_UPDATE_ER) er_image(ghat, G, p->S + (size_t)n * px, px);
-        else hio_image(ghat, G, p->S + (size_t)n * px, px, beta);
+        if (p->update == ORACLE_UPDATE_RAAR) raar_image(ghat, G, p->S + (size_t)n * px, px, beta, p->positivity);
+        else if (p->update == ORACLE_UPDATE_ER) er_image(ghat, G, p->S + (size_t)n * px, px, p->positivity);
+        else hio_image(ghat, G, p->S + (size_t)n * px, px, beta, p->positivity);
     }
     free(G);
     return ORACLE_OK;

@@ -55,6 +55,7 @@ def _lib(precision: str = "f64"):
         lib.oracle_hio.argtypes = [vp, vp, vp, ci, cd]
         lib.oracle_real_name.restype = ctypes.c_char_p
         lib.oracle_set_seam.argtypes = [vp, ci]
+        lib.oracle_set_positivity.argtypes = [vp, ci]
         lib.oracle_mix_seam.argtypes = [vp, vp, ci, ci, ci, vp, ci]
         lib.oracle_blur.argtypes = [vp, vp, ci, cd]
         lib.oracle_shrinkwrap.argtypes = [vp, cd, cd, vp]
@@ -257,6 +258,10 @@ class Oracle:
         return (vol, w) if want_weight else vol
 
     # -- seam, shrink-wrap, Step A, Step C ------------------------------------------
+    def set_positivity(self, on):
+        _chk(self._l.oracle_set_positivity(self._h, int(bool(on))), "oracle_set_positivity")
+        return self
+
     def set_seam(self, flip):
         _chk(self._l.oracle_set_seam(self._h, int(bool(flip))), "oracle_set_seam")
         return self

@@ -46,6 +46,7 @@ SIGNATURES = {
     "cpra_profile_read": (_ci, [_vp, _vp, _vp]),
     "cpra_launch_count": (_ci, [_vp, ctypes.POINTER(_cl)]),
     "cpra_set_seam": (_ci, [_vp, _ci]),
+    "cpra_set_positivity": (_ci, [_vp, _ci]),
     "cpra_set_cluster": (_ci, [_vp, _ci]),
     "cpra_set_walk_ctas": (_ci, [_vp, _ci]),
     "cpra_shrinkwrap": (_ci, [_vp, _cf, _cf, _vp]),
@@ -239,6 +240,10 @@ class Plan:
         return self
 
     # -- around the loop -------------------------------------------------------------
+    def set_positivity(self, on: bool):
+        _chk(self._l.cpra_set_positivity(self._h, int(bool(on))), "cpra_set_positivity")
+        return self
+
     def set_seam(self, flip: bool):
         _chk(self._l.cpra_set_seam(self._h, int(bool(flip))), "cpra_set_seam")
         return self

@@ -442,6 +442,13 @@ int cpra_set_walk_ctas(cpra_plan_t p, int per_sm)
     return CPRA_OK;
 }
 
+int cpra_set_positivity(cpra_plan_t p, int on)
+{
+    if (!p || (on != 0 && on != 1)) return CPRA_ERR_INVALID_ARG;
+    p->positivity = on;
+    return CPRA_OK;
+}
+
 int cpra_set_seam(cpra_plan_t p, int flip)
 {
     if (!p || (flip != 0 && flip != 1)) return CPRA_ERR_INVALID_ARG;

@@ -228,10 +228,11 @@ k_image_cl(const float4* __restrict__ cur, float4* __restrict__ nxt, float4* __r
 #pragma unroll 4
         for (int i = threadIdx.x; i < QUADS; i += NT) {
             const int j = i % NPAIR, tx = i / NPAIR;   // tx = (local row tile) N + x
-            const unsigned bits = (unsigned)Simg[tx] >> (2 * j);
+            unsigned bits = (unsigned)Simg[tx] >> (2 * j);
             // ghat was written by this CTA earlier in this launch: a plain (coherent) load, not the read-only path
             const c2 g0 = from_quad((MIXMODE != MIX_NONE) ? ghr[i] : __ldg(ghr + i));
             const c2 gp = from_quad(img[i]);
+            bits = inside_bits(mp, bits, gp.re);
             const float2 ore = update_outside(mp, gp.re, g0.re), oim = update_outside(mp, gp.im, g0.im);
             float4 o;
             o.x = (bits & 1) ? gp.re.x : ore.x;

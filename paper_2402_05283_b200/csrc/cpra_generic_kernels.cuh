@@ -266,7 +266,7 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
         const size_t o = (size_t)n * px + (size_t)y * N + x;
         float2 gp = r[x * Wp + w];
         gp.x *= scale; gp.y *= scale;
-        if (hio && !S[o]) {
+        if (hio && (!S[o] || (mp.positivity && gp.x < 0.f))) {
             const float2 gh = ghat ? ghat[o] : gen_mix(cur, gg, mp, n, y, x, fires != 0);
             gp = make_float2(fmaf(mp.c_gp, gp.x, mp.c_ghat * gh.x), fmaf(mp.c_gp, gp.y, mp.c_ghat * gh.y));
         }

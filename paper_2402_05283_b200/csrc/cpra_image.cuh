@@ -180,9 +180,10 @@ k_image(const float4* __restrict__ cur, float4* __restrict__ nxt, const float* _
 #pragma unroll 4
         for (int i = threadIdx.x; i < image_quads<N>(); i += NT) {
             const int j = i % NPAIR, tx = i / NPAIR;   // tx = rt N + x
-            const unsigned bits = (unsigned)Simg[tx] >> (2 * j);
+            unsigned bits = (unsigned)Simg[tx] >> (2 * j);
             const c2 gh = mix(from_quad(__ldg(own + i)), (size_t)i);
             const c2 gp = from_quad(img[i]);
+            bits = inside_bits(mp, bits, gp.re);
             const float2 ore = update_outside(mp, gp.re, gh.re), oim = update_outside(mp, gp.im, gh.im);
             float4 o;
             o.x = (bits & 1) ? gp.re.x : ore.x;

@@ -36,12 +36,25 @@ struct MixParams {
     // cpra_set_seam: a neighbour reached by wrapping round the end of the stack is read mirrored in u
     // (x -> (N - x) mod N about the centre pixel): the seam of a [0, 180) scan, reading A5b
     int flip_seam;
+    // cpra_set_positivity: a pixel inside the support whose modulus-constrained estimate has a negative real part
+    // is treated as lying outside it (the conventional positivity constraint of the real-space step)
+    int positivity;
 };
 // the update outside the support on a pair; with c_ghat = 1 (HIO) the product is exact, so the result
 // is the single fma ghat - beta g'
 __device__ __forceinline__ float2 update_outside(const MixParams& mp, float2 gp, float2 gh)
 {
     return pfma(bc(mp.c_gp), gp, pmul(bc(mp.c_ghat), gh));
+}
+
+// support bits of a pair after the optional positivity test on Re g'
+__device__ __forceinline__ unsigned inside_bits(const MixParams& mp, unsigned bits, float2 re)
+{
+    if (mp.positivity) {
+        if (re.x < 0.f) bits &= ~1u;
+        if (re.y < 0.f) bits &= ~2u;
+    }
+    return bits;
 }
 
 enum { MIX_NONE = 0, MIX_K1 = 1, MIX_GEN = 2, MIX_MASK = 3 };
@@ -726,11 +739,12 @@ k_row_inv(const __grid_constant__ CUtensorMap tm_scr, const float4* __restrict__
 #pragma unroll 4
         for (int i = threadIdx.x; i < tile_quads<N>(); i += NT) {
             const int x = ppos<N>(i / NP), j = i % NP;   // i runs over the physical quads of the tile
-            const unsigned bits = (unsigned)s.sup[x] >> ((rt * TBN) % 16 + 2 * j);
+            unsigned bits = (unsigned)s.sup[x] >> ((rt * TBN) % 16 + 2 * j);
             // ghat: stored by k_row_fwd / k_row_walk (ghat_in), else recomputed from the previous state
             const c2 gh = ghat_in ? from_quad(__ldg(ghat_in + (size_t)n * istride + toff + i))
                                   : mix(from_quad(__ldg(own + i)), toff + (size_t)i);
             const c2 gp = from_quad(tile[i]);
+            bits = inside_bits(mp, bits, gp.re);
             const float2 ore = update_outside(mp, gp.re, gh.re), oim = update_outside(mp, gp.im, gh.im);
             float4 o;
             o.x = (bits & 1) ? gp.re.x : ore.x;

@@ -48,6 +48,7 @@ struct cpra_plan_s {
     int n_ei = 1;
     int update = CPRA_UPDATE_HIO;
     int flip_seam = 0;        // cpra_set_seam
+    int positivity = 0;       // cpra_set_positivity
     int walk_ctas = 0;        // cpra_set_walk_ctas: CTAs per SM of the fused row kernel (0 = library default)
     // sizes that are not powers of two (cpra_generic.cuh): natural-layout buffers in the same workspace
     bool generic = false;
@@ -237,6 +238,7 @@ inline MixParams mix_params(const cpra_plan_s* p, float beta = 0.f)
     else if (p->update == CPRA_UPDATE_ER) { mp.c_ghat = 0.f; mp.c_gp = 0.f; }
     else { mp.c_ghat = 1.0f; mp.c_gp = -beta; }
     mp.flip_seam = p->flip_seam;
+    mp.positivity = p->positivity;
     return mp;
 }
 

@@ -168,7 +168,7 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             const uint16_t* __restrict__ sp = sup + s * N;
 #pragma unroll
             for (int r = 0; r < E0; ++r) {
-                const unsigned bits = (unsigned)sp[p0(r)] >> (sshift + 2 * j);
+                const unsigned bits = inside_bits(mp, (unsigned)sp[p0(r)] >> (sshift + 2 * j), v[r].re);
                 const float2 ore = update_outside(mp, v[r].re, g0[r].re), oim = update_outside(mp, v[r].im, g0[r].im);
                 v[r].re = make_float2((bits & 1) ? v[r].re.x : ore.x, (bits & 2) ? v[r].re.y : ore.y);
                 v[r].im = make_float2((bits & 1) ? v[r].im.x : oim.x, (bits & 2) ? v[r].im.y : oim.y);

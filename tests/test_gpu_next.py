@@ -419,3 +419,32 @@ def test_assembly_and_merge_mixed_radix(torch_cuda):
     out_g, sh_g, tw_g = g.merge_finish(0)
     assert np.array_equal(sh_g.cpu().numpy()[:len(sh_o)], sh_o)       # (one episode kept of the two slots)
     assert rel_l2(out_g.cpu().numpy(), out_o) <= 3 * TOL_1
+
+
+@pytest.mark.parametrize("N,Np,rule,flags", [(64, 5, "hio", 0), (128, 4, "raar", 0), (256, 5, "hio", 0), (512, 5, "hio", 0),
+                                             (512, 4, "er", 4), (1024, 3, "hio", 0), (160, 4, "hio", 0)])
+def test_positivity(torch_cuda, N, Np, rule, flags):
+    """cpra_set_positivity through every kernel family.  The sign test on Re g' is taken in fp32 on the device and in
+    fp64 by the oracle: after ONE iteration the two agree except at pixels whose Re g' lies within rounding of zero,
+    which are set aside (what is unique is compared) and must be rare."""
+    p = cpra_inputs.random_stack(N, Np, seed=1200 + N, beamstop=3)
+    o, g = _oracle(p), _gpu(p, flags=flags)
+    ref0 = _oracle(p)
+    for plan in (o, g):
+        plan.set_update(rule)
+        plan.set_positivity(True)
+    ref0.set_update(rule)
+    o.iterate(1, 0.9)
+    g.iterate(1, 0.9)
+    ref0.iterate(1, 0.9)
+    out, ref, plain = _get(g), o.get_projections(0), ref0.get_projections(0)
+    # inside the support without positivity the state is g' itself: its real part is what the test looked at
+    gp_re = plain.real
+    clear = ~((p.support == 1) & (np.abs(gp_re) < 1e-5 * np.abs(plain).max()))
+    assert (~clear).mean() < 1e-3
+    assert np.linalg.norm((out - ref)[clear]) <= 2 * TOL_1 * np.linalg.norm(ref[clear])
+    assert rel_l2(ref, plain) > 0.05                                   # the flag matters on this input
+    # a second iteration through the multi-iteration path stays close (a flipped pixel would show as ~1e-3)
+    o.iterate(1, 0.9)
+    g.iterate(1, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 2e-3

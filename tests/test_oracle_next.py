@@ -398,3 +398,31 @@ def test_prtf_closed_forms():
     G2[:, ring] *= -1.0
     t2 = o.prtf(0.5 * (P + np.fft.ifft2(G2)))
     assert abs(t2[6]) < 1e-9 and np.abs(np.delete(t2[2:], 4) - 1.0).max() < 1e-9
+
+
+# ---------------------------------------------------------------- f2: positivity
+def test_positivity_closed_form():
+    """Nothing measured (M = 0: g' = g), K = 0: with positivity a pixel inside the support keeps g where Re g >= 0 and
+    gets the feedback value elsewhere -- HIO (1 - beta) g, RAAR (1 - beta) g, ER 0 -- exactly like a pixel outside the
+    support; without the flag the inside pixels are untouched."""
+    N, Np, beta = 8, 2, 0.9
+    g = _stack(Np, N, 41)
+    S = np.zeros((Np, N, N), np.uint8)
+    S[:, 2:6, 1:7] = 1
+    inside = S.astype(bool)
+    neg = g.real < 0
+    for rule, outside in (("hio", 1 - beta), ("raar", 1 - beta), ("er", 0.0)):
+        for pos in (0, 1):
+            o = Oracle(N, Np)
+            o.set_data(np.ones((Np, N, N)), np.zeros((Np, N, N), np.uint8))
+            o.set_support(S)
+            o.set_carousel([1.0], 1)
+            o.set_update(rule)
+            o.set_positivity(pos)
+            o.set_estimate(g)
+            o.iterate(1, beta)
+            out = o.get_projections(0)
+            keep = inside & ~(neg & bool(pos))
+            assert np.abs(out[keep] - g[keep]).max() < 1e-14, (rule, pos)
+            assert np.abs(out[~keep] - outside * g[~keep]).max() < 1e-14, (rule, pos)
+    assert (inside & neg).sum() > 5 and (inside & ~neg).sum() > 5
