@@ -398,32 +398,41 @@ int cpra_assemble_3d(cpra_plan_t p, float* d_vol, float* d_weight)
         cudaMemcpyAsync(p->ustart, p->h_ustart.data(), sizeof(int) * (U + 1), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
         cudaMemcpyAsync(p->rays, p->h_rays.data(), sizeof(int) * p->h_rays.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess)
         return CPRA_ERR_CUDA;
+    const int N = p->N;
+    const size_t total = (size_t)p->Np * N * N;
+    // the gather with the lanes along kz needs whole 32 x 32 tiles and room for its geometry table (N^2 x 32 B in the
+    // spare state buffer); anything else takes the one-thread-per-(ky, kx) gather
+    const bool tiled = (N % 32 == 0) && (size_t)p->Np * sizeof(float2) >= sizeof(AsmGeo);
+    // (i) E_n = F[S_n g_n], natural order, transposed to Et[n][ku][kz] in the second scratch
     if (p->generic) {
-        // (i) E_n = F[S_n g_n], natural order, transposed; (ii)-(iv) the same gather
         if (int rc = gen_slices(p, (float2*)p->scr2)) return rc;
-        const int N = p->N;
-        const int zsplit = std::max(1, std::min(N, 4096 / std::max(1, (N * N) / 256)));
-        const int zper = (N + zsplit - 1) / zsplit;
-        const dim3 grid(blocks_for((size_t)N * N, 128), (unsigned)((N + zper - 1) / zper));
-        k_assemble<<<grid, 128, 0, p->stream>>>((const float2*)p->scr2, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
+    } else {
+        int rc = CPRA_OK;
+        { auto f = [&]() -> int {
+            CPRA_DISPATCH_N(p->N,
+                rc = Launch<NN>::row_fwd(p, p->st[p->cur], MIX_MASK, 0, p->Np);
+                if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
+            return 0; }; f(); }
+        if (rc) return rc;
+        const int tile_smem = N * (p->geo.TB / 2) * 16;
+        if (tile_smem <= 48 * 1024)
+            k_unpack_tile_T<<<(unsigned)(p->Np * (N / p->geo.TB)), 256, tile_smem, p->stream>>>(p->scr, (float2*)p->scr2, p->geo);
+        else
+            k_unpack_spectrum_T<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->scr, (float2*)p->scr2, p->geo, total);
+        if (int rc2 = check_launch(p)) return rc2;
+    }
+    // (ii)-(iv) gather
+    if (tiled) {
+        AsmGeo* geo = (AsmGeo*)p->st[p->cur ^ 1];
+        k_assemble_geo<<<blocks_for((size_t)N * N, 128), 128, 0, p->stream>>>(geo, p->uphi, U, N);
+        if (int rc2 = check_launch(p)) return rc2;
+        k_assemble_gather<<<(unsigned)((N / 32) * N * (N / 32)), 256, 0, p->stream>>>((const float2*)p->scr2, (float2*)d_vol, d_weight, geo,
+                                                                                     p->ustart, p->rays, N, p->Np);
         return check_launch(p);
     }
-    // (i) E_n = F[S_n g_n] into the scratch
-    int rc = CPRA_OK;
-    { auto f = [&]() -> int {
-        CPRA_DISPATCH_N(p->N,
-            rc = Launch<NN>::row_fwd(p, p->st[p->cur], MIX_MASK, 0, p->Np);
-            if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
-        return 0; }; f(); }
-    if (rc) return rc;
-    // (ii)-(iv) gather
-    const int N = p->N;
     const int zsplit = std::max(1, std::min(N, 4096 / std::max(1, (N * N) / 256)));
     const int zper = (N + zsplit - 1) / zsplit;
     const dim3 grid(blocks_for((size_t)N * N, 128), (unsigned)((N + zper - 1) / zper));
-    const size_t total = (size_t)p->Np * N * N;
-    k_unpack_spectrum_T<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->scr, (float2*)p->scr2, p->geo, total);
-    if (int rc2 = check_launch(p)) return rc2;
     k_assemble<<<grid, 128, 0, p->stream>>>((const float2*)p->scr2, (float2*)d_vol, d_weight, p->uphi, p->ustart, p->rays, U, p->geo, zper);
     return check_launch(p);
 }

@@ -230,4 +230,147 @@ __global__ void k_assemble(const float2* __restrict__ Et, float2* __restrict__ v
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// A7, round 2: the same gather (same arithmetic, same results) laid out for the memory system.
+//   k_assemble_geo     one thread per (ky, kx): the polar geometry in fp64, once, into a table
+//   k_unpack_tile_T    scratch column tile -> Et[n][ku][kz]: the tile is read as it lies in HBM and every output
+//                      row (all kz of one ku) is written contiguously
+//   k_assemble_gather  a block = 32 kx x 32 kz at one ky; the lanes of a warp run along kz, so every tap is one
+//                      coalesced 256-byte read of Et, and the tile leaves through shared memory as contiguous kx
+//                      rows of the volume.  kz tiles are the slowest grid index: the 1/16 of Et that one kz tile
+//                      touches stays in L2 while all (ky, kx) are served from it.
+// ------------------------------------------------------------------------------------------------
+struct AsmGeo {
+    int mode;        // 0: outside (rho > N/2 - 1), 1: axis (rho = 0), 2: interpolate
+    int ua, ub;      // bracketing unique rays
+    int r0;          // floor(rho)
+    double wp, wr;   // angular weight of ray ub, radial weight of sample r0 + 1
+};
+__global__ void k_assemble_geo(AsmGeo* __restrict__ geo, const double* __restrict__ uphi, int U, int N)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N * N) return;
+    const int h = N / 2, ix = i % N, iy = i / N;
+    const int kx = ix < h ? ix : ix - N, ky = iy < h ? iy : iy - N;
+    const double PI = 3.14159265358979323846264338327950288;
+    const double rho = sqrt((double)kx * kx + (double)ky * ky);
+    AsmGeo g;
+    g.mode = 0; g.ua = g.ub = 0; g.r0 = 0; g.wp = 0.0; g.wr = 0.0;
+    if (rho == 0.0) g.mode = 1;
+    else if (rho <= (double)(h - 1)) {
+        g.mode = 2;
+        double phi = atan2((double)ky, (double)kx);
+        if (phi < 0.0) phi += 2.0 * PI;
+        int a = -1;
+        for (int lo = 0, hi = U - 1; lo <= hi;) {
+            const int mid = (lo + hi) / 2;
+            if (uphi[mid] <= phi) { a = mid; lo = mid + 1; } else hi = mid - 1;
+        }
+        double pa, pb; int b;
+        if (a < 0) { a = U - 1; pa = uphi[a] - 2.0 * PI; } else pa = uphi[a];
+        b = a + 1;
+        if (b >= U) { b = 0; pb = uphi[0] + 2.0 * PI; } else pb = uphi[b];
+        g.wp = (pb > pa) ? (phi - pa) / (pb - pa) : 0.0;
+        g.r0 = (int)floor(rho);
+        g.wr = rho - (double)g.r0;
+        g.ua = a; g.ub = b;
+    }
+    geo[i] = g;
+}
+
+// position -> frequency (the inverse of fft_pos)
+__host__ __device__ __forceinline__ int fft_unpos(int pos, int R0, int R1, int R2)
+{
+    const int k2 = pos % R2, k1 = (pos / R2) % R1, k0 = pos / (R2 * R1);
+    return k0 + R0 * (k1 + R1 * k2);
+}
+// one block per scratch column tile (n, ct): TB columns x N positions, contiguous in HBM
+__global__ void k_unpack_tile_T(const float4* __restrict__ scr, float2* __restrict__ Et, Geo g)
+{
+    extern __shared__ __align__(16) float4 tile[];   // N * TB/2 quads, as in HBM
+    const int N = g.N, tb = g.TB, np = tb / 2, nct = N / tb;
+    const int n = blockIdx.x / nct, ct = blockIdx.x % nct;
+    const float4* __restrict__ src = scr + ((size_t)n * nct + ct) * (size_t)N * np;
+    for (int i = threadIdx.x; i < N * np; i += blockDim.x) tile[i] = src[i];
+    __syncthreads();
+    const float* __restrict__ t = reinterpret_cast<const float*>(tile);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int c = wid; c < tb; c += nw) {
+        const int ku = fft_unpos(ct * tb + c, g.R0, g.R1, g.R2);
+        float2* __restrict__ out = Et + ((size_t)n * N + ku) * N;
+        for (int kz = lane; kz < N; kz += 32) {
+            const int py = fft_pos(kz, g.R0, g.R1, g.R2);
+            const int q = (ppos(py, tb, ct & 1) * np + sw(c / 2, py, np)) * 4 + (c & 1);
+            out[kz] = make_float2(t[q], t[q + 2]);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_assemble_gather(const float2* __restrict__ Et, float2* __restrict__ vol, float* __restrict__ wgt, const AsmGeo* __restrict__ geo,
+                  const int* __restrict__ ustart, const int* __restrict__ rays, int N, int Np)
+{
+    __shared__ float2 tv[32][33];
+    __shared__ float tw[32];
+    const int xt = N / 32;                                   // kx tiles per row
+    const int iz0 = (int)(blockIdx.x / ((unsigned)xt * N)) * 32;     // kz tile: slowest
+    const int rem = (int)(blockIdx.x % ((unsigned)xt * N));
+    const int iy = rem / xt, ix0 = (rem % xt) * 32;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int iz = iz0 + lane, h = N / 2;
+    const int ky = iy < h ? iy : iy - N, kz = iz < h ? iz : iz - N;
+    for (int c = wid; c < 32; c += 8) {
+        const int ix = ix0 + c, kx = ix < h ? ix : ix - N;
+        const AsmGeo g = geo[iy * N + ix];
+        double vr = 0.0, vi = 0.0;
+        float w = 0.f;
+        if (g.mode == 1) {
+            const double sg = (iz & 1) ? -1.0 : 1.0;
+            for (int n = 0; n < Np; ++n) {
+                const float2 e = __ldg(Et + (size_t)n * N * N + iz);
+                vr += sg * e.x; vi += sg * e.y;
+            }
+            vr /= Np; vi /= Np; w = 1.f;
+        } else if (g.mode == 2) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const double wq = q ? g.wp : 1.0 - g.wp;
+                if (wq == 0.0) continue;
+                const int u = q ? g.ub : g.ua;
+                const int c0 = ustart[u], c1 = ustart[u + 1];
+#pragma unroll
+                for (int rr = 0; rr < 2; ++rr) {
+                    const double wrr = rr ? g.wr : 1.0 - g.wr;
+                    if (wrr == 0.0) continue;
+                    const int r = g.r0 + rr;                 // 0 <= r <= N/2 - 1
+                    double sr = 0.0, si = 0.0;
+                    for (int cc = c0; cc < c1; ++cc) {
+                        const int code = rays[cc];
+                        const int n = code & 0x3fffffff;
+                        const int iu = ((code >> 30) && r) ? N - r : r;      // -r mod N
+                        const float2 e = __ldg(Et + ((size_t)n * N + iu) * N + iz);
+                        const bool neg = (iz + iu) & 1;                      // origin -> centre pixel
+                        sr += neg ? -(double)e.x : (double)e.x;
+                        si += neg ? -(double)e.y : (double)e.y;
+                    }
+                    const double wt = wq * wrr / (double)(c1 - c0);
+                    vr += wt * sr;
+                    vi += wt * si;
+                }
+            }
+            w = 1.f;
+        }
+        if ((kx + ky + kz) & 1) { vr = -vr; vi = -vi; }
+        tv[lane][c] = make_float2((float)vr, (float)vi);
+        if (lane == 0) tw[c] = w;
+    }
+    __syncthreads();
+    // rows of 32 consecutive kx: contiguous in the volume
+    for (int z = wid; z < 32; z += 8) {
+        const size_t o = ((size_t)(iz0 + z) * N + iy) * N + ix0 + lane;
+        vol[o] = tv[z][lane];
+        if (wgt) wgt[o] = tw[lane];
+    }
+}
+
 }  // namespace cpra
