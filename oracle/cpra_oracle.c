@@ -954,6 +954,60 @@ int oracle_merge_finish(oracle_plan_t p, int n_ref, double* out, int* shifts, in
     return ORACLE_OK;
 }
 
+/* Consistency of the projections of ONE episode before Step D (reading A28 -- an addition of this build, not the
+ * paper's: the paper relies on the carousel coupling alone).  Two freedoms of an unconstrained complex
+ * iterate survive the loop projection by projection, and both are fixed by facts of the forward model:
+ *  (1) global phase: every projection of one object has the same total, sum_px P_n = sum_voxels O (line
+ *      integrals), so each PO is multiplied by the unit factor that makes its total real and positive
+ *      (conj(s_n)/|s_n|, s_n = sum_px O_n; left alone if s_n = 0);
+ *  (2) twin: neighbouring projections are similar, so, walking away from projection n_ref in both directions,
+ *      PO n is replaced by its twin conj(O_n(-r)) iff that is closer to the already decided neighbour:
+ *      Re<a, T O_n> > Re<a, O_n>.  (The twin keeps a real positive total, so (1) stays satisfied.)
+ * ep: interleaved complex double [Np][N][N], in place.  flips (optional): int [Np]. */
+int oracle_align_episode(double* ep, int N, int Np, int n_ref, int* flips)
+{
+    if (!ep || N < 1 || Np < 1 || n_ref < 0 || n_ref >= Np) return ORACLE_ERR_INVALID_ARG;
+    const size_t px = (size_t)N * N;
+    for (int n = 0; n < Np; ++n) {
+        double* o = ep + 2 * (size_t)n * px;
+        double sr = 0.0, si = 0.0;
+        for (size_t i = 0; i < px; ++i) { sr += o[2 * i]; si += o[2 * i + 1]; }
+        const double m = sqrt(sr * sr + si * si);
+        if (m > 0.0) {
+            const double ur = sr / m, ui = -si / m;
+            for (size_t i = 0; i < px; ++i) {
+                const double a = o[2 * i], b = o[2 * i + 1];
+                o[2 * i] = ur * a - ui * b; o[2 * i + 1] = ur * b + ui * a;
+            }
+        }
+    }
+    double* tmp = (double*)malloc(sizeof(double) * 2 * px);
+    if (flips) for (int n = 0; n < Np; ++n) flips[n] = 0;
+    for (int dir = 1; dir >= -1; dir -= 2)
+        for (int n = n_ref + dir; n >= 0 && n < Np; n += dir) {
+            const double* a = ep + 2 * (size_t)(n - dir) * px;      /* the decided neighbour */
+            double* o = ep + 2 * (size_t)n * px;
+            double pp = 0.0, qq = 0.0;
+            for (int y = 0; y < N; ++y)
+                for (int x = 0; x < N; ++x) {
+                    const size_t i = (size_t)y * N + x, j = (size_t)((N - y) % N) * N + (size_t)((N - x) % N);
+                    pp += a[2 * i] * o[2 * i] + a[2 * i + 1] * o[2 * i + 1];          /* Re conj(a) o      */
+                    qq += a[2 * i] * o[2 * j] - a[2 * i + 1] * o[2 * j + 1];          /* Re conj(a) conj(o(-r)) */
+                }
+            if (qq > pp) {
+                memcpy(tmp, o, sizeof(double) * 2 * px);
+                for (int y = 0; y < N; ++y)
+                    for (int x = 0; x < N; ++x) {
+                        const size_t i = (size_t)y * N + x, j = (size_t)((N - y) % N) * N + (size_t)((N - x) % N);
+                        o[2 * i] = tmp[2 * j]; o[2 * i + 1] = -tmp[2 * j + 1];
+                    }
+                if (flips) flips[n] = 1;
+            }
+        }
+    free(tmp);
+    return ORACLE_OK;
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* the 3D transform of Step D ("3D FTs as a set of 2D FTs")     */
 /* ------------------------------------------------------------------------------------------ */

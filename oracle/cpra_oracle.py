@@ -67,6 +67,7 @@ def _lib(precision: str = "f64"):
         lib.oracle_merge_errors.argtypes = [vp, vp, vp]
         lib.oracle_merge_finish.argtypes = [vp, ci, vp, vp, vp]
         lib.oracle_fft3.argtypes = [vp, vp, ci, ci]
+        lib.oracle_align_episode.argtypes = [vp, ci, ci, ci, vp]
         lib.oracle_refine_3d.argtypes = [vp, vp, vp, ci, ci, vp, vp]
         lib.oracle_fsc.argtypes = [vp, vp, ci, vp]
         lib.oracle_prtf.argtypes = [vp, vp, vp]
@@ -177,6 +178,15 @@ def refine_3d(E, W, S3, k):
     _chk(_lib().oracle_refine_3d(e.ctypes.data, w.ctypes.data, s3.ctypes.data, e.shape[-1], int(k), obj.ctypes.data, err.ctypes.data),
          "oracle_refine_3d")
     return obj, err
+
+
+def align_episode(episode, n_ref=0):
+    """Phase gauge and twin chain of one episode (reading A28): returns (aligned copy, flips int32[Np])."""
+    e = _c128(episode).copy()
+    Np, N = e.shape[0], e.shape[-1]
+    fl = np.zeros(Np, dtype=np.int32)
+    _chk(_lib().oracle_align_episode(e.ctypes.data, N, Np, int(n_ref), fl.ctypes.data), "oracle_align_episode")
+    return e, fl
 
 
 def fsc(F1, F2):

@@ -1,0 +1,139 @@
+"""CPRA as the paper composes it (Fig. 2), on top of the C-ABI calls: orchestration only.
+
+    Step A  pre-reconstruct projection 0 from a random start -- for ALL N_r restarts at once: the
+            N_r random starts of that one projection are a stack of their own (a plan with N_r images of the same
+            data, coupling off), so the N_i^pre conventional iterations run batched instead of one image at a time
+    Step B  per restart: N_e episodes of N_ei iterations of the coupled loop (cpra_iterate with n_ei = N_ei)
+    Step C  the bank keeps the N_l lowest-error episodes (cpra_merge_offer, decided on the device); centre of mass,
+            twin selection, average (cpra_merge_finish)
+    Step D  Fourier-slice assembly of the merged episode (cpra_assemble_3d), then optionally the inverse 3D
+            transform / the iterations against a 3D support (cpra_fft3 / cpra_refine_3d; power-of-two N)
+
+Every arithmetic step runs in the library's kernels; this module only allocates torch tensors, draws the random
+starting phases (torch's generator on the device: input generation, not part of the method) and calls the binding."""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass
+from typing import Optional
+
+
+from . import binding
+
+
+@dataclass
+class CpraResult:
+    episode: "object"            # merged episode, complex64 [Np, N, N] (device)
+    errors: "object"             # float64 [N_l] errors of the kept restarts (device)
+    shifts: "object"             # int32 [N_l, Np, 2]
+    twins: "object"              # int32 [N_l]
+    spectrum: "object" = None    # complex64 [N, N, N], the assembled E(q) (device) if assemble=True
+    weight: "object" = None      # float32 [N, N, N]
+    obj: "object" = None         # complex64 [N, N, N], O(r) if a 3D step was asked for (power-of-two N)
+    refine_error: "object" = None
+    seconds: dict = None
+
+
+def random_phase_starts(plan, intensity, mask, seed: int):
+    """Random-phase starts g0 = F^-1[M sqrt(I) e^{i phi}], phi ~ U[0, 2 pi) per pixel (reading A15; "random
+    initial guess") for a stack: intensity fp32 [n, N, N] detector-centred, mask u8 [n, N, N] or None, n = plan.Np.
+    The phases come from torch's generator on the device (input generation); the transform is the library's own
+    cpra_fft2.  Returns complex64 [n, N, N]."""
+    import torch
+    gen = torch.Generator(device=intensity.device)
+    gen.manual_seed(int(seed))
+    N = intensity.shape[-1]
+    A = torch.sqrt(torch.clamp(intensity.to(torch.float32), min=0.0))
+    if mask is not None:
+        A = A * mask.to(torch.float32)
+    A = torch.roll(A, shifts=(-(N // 2), -(N // 2)), dims=(-2, -1))          # detector-centred -> native order
+    phi = torch.rand(A.shape, generator=gen, device=intensity.device, dtype=torch.float32) * (2.0 * math.pi)
+    return plan.fft2(torch.polar(A, phi).to(torch.complex64).contiguous(), +1)
+
+
+def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, n_pre: int, n_episodes: int, n_ei: int,
+                beta: float = 0.9, alpha=(0.6, 0.2), update: str = "hio", seam_flip: bool = False, seed: int = 0,
+                shrinkwrap: Optional[tuple] = None, assemble: bool = True, support3d=None, refine_iters: int = 0,
+                n_ref: int = 0) -> CpraResult:
+    """Steps A-D.  intensity fp32 [Np, N, N], mask u8 [Np, N, N] or None, support u8 [Np, N, N]: CUDA tensors;
+    angles: Np radians (host).  shrinkwrap = (sigma, threshold): one support update at the end of every episode
+    (power-of-two N).  support3d u8 [N, N, N] + refine_iters > 0: Step D's iterations; refine_iters == 0
+    with assemble: only E(q) (and O(r) = F3^-1[E] when N is a power of two)."""
+    import torch
+    Np, N = int(intensity.shape[0]), int(intensity.shape[-1])
+    dev = intensity.device
+    sec = {}
+
+    def timed(name, t0):
+        t1 = torch.cuda.Event(enable_timing=True)
+        t1.record()
+        torch.cuda.synchronize(dev)
+        sec[name] = t0.elapsed_time(t1) * 1e-3
+
+    def start():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
+
+    # ---- Step A, batched over the restarts: N_r starts of projection 0, no coupling -------------------------------
+    t0 = start()
+    pre = None
+    if n_pre > 0:
+        pa = binding.Plan(N, n_restarts)
+        pa.set_data(intensity[:1].expand(n_restarts, N, N).contiguous(),
+                    None if mask is None else mask[:1].expand(n_restarts, N, N).contiguous(), None)
+        pa.set_support(support[:1].expand(n_restarts, N, N).contiguous())
+        pa.set_carousel((1.0,), 1)
+        pa.set_update(update)
+        I0 = intensity[:1].expand(n_restarts, N, N).contiguous()
+        M0 = None if mask is None else mask[:1].expand(n_restarts, N, N).contiguous()
+        pa.set_estimate(random_phase_starts(pa, I0, M0, seed))
+        pa.iterate(n_pre, beta)
+        pre = pa.get_projections(binding.ITERATE)
+        pa.close()
+    timed("step_a", t0)
+
+    # ---- Steps B and C ----------------------------------------------------------------------------------------------
+    t0 = start()
+    plan = binding.Plan(N, Np)
+    plan.set_data(intensity, mask, angles)
+    plan.set_carousel(alpha, n_ei)
+    plan.set_update(update)
+    plan.set_seam(seam_flip)
+    plan.merge_begin(n_keep)
+    for r in range(n_restarts):
+        plan.set_support(support)
+        g0 = random_phase_starts(plan, intensity, mask, seed + 7919 * (r + 1))
+        if pre is not None:
+            g0[0] = pre[r]
+        plan.set_estimate(g0)
+        for _ in range(n_episodes):
+            plan.iterate(n_ei, beta)
+            if shrinkwrap is not None:
+                plan.shrinkwrap(float(shrinkwrap[0]), float(shrinkwrap[1]))
+        plan.merge_offer()
+    episode, shifts, twins = plan.merge_finish(n_ref)
+    errors, count = plan.merge_errors()
+    timed("steps_b_c", t0)
+    res = CpraResult(episode=episode, errors=errors[:int(count.cpu()[0])], shifts=shifts, twins=twins, seconds=sec)
+
+    # ---- Step D -----------------------------------------------------------------------------------------------------
+    if assemble:
+        t0 = start()
+        # the merged episode is already restricted to (shifted) supports: assemble it as it is
+        plan.set_support(torch.ones((Np, N, N), dtype=torch.uint8, device=dev))
+        plan.set_estimate(episode)
+        res.spectrum, res.weight = plan.assemble_3d()
+        timed("assemble", t0)
+        if N & (N - 1) == 0:
+            t0 = start()
+            plan.close()
+            p3 = binding.Plan(N, N)
+            if refine_iters > 0 and support3d is not None:
+                res.obj, res.refine_error = p3.refine_3d(res.spectrum, res.weight, support3d, refine_iters)
+            else:
+                res.obj = p3.fft3(res.spectrum, +1)
+            p3.close()
+            timed("step_d_3d", t0)
+    plan.close()
+    return res

@@ -5,7 +5,7 @@ routine (numpy)."""
 import numpy as np
 
 import cpra_inputs
-from oracle import Oracle, blur, center_of_mass, fft3, fsc, mix, mix_seam, refine_3d
+from oracle import Oracle, align_episode, blur, center_of_mass, fft3, fsc, mix, mix_seam, refine_3d
 
 
 def _stack(Np, N, seed):
@@ -426,3 +426,36 @@ def test_positivity_closed_form():
             assert np.abs(out[keep] - g[keep]).max() < 1e-14, (rule, pos)
             assert np.abs(out[~keep] - outside * g[~keep]).max() < 1e-14, (rule, pos)
     assert (inside & neg).sum() > 5 and (inside & ~neg).sum() > 5
+
+
+# ---------------------------------------------------------------- consistency of one episode before Step D (A28)
+def test_align_episode_restores_phases_and_twins_of_true_projections():
+    """The projections of one object all have the same total (line integrals), and neighbours are
+    similar.  A stack of true projections whose members were multiplied by arbitrary unit phases, and
+    some replaced by their twins conj(P(-r)), comes back exactly."""
+    p = cpra_inputs.make_problem(1, Np=12, noise=False)
+    P = p.projections
+    tot = P.sum(axis=(1, 2))
+    assert np.abs(tot - tot[0]).max() < 2e-3 * abs(tot[0]) and tot[0].real > 0      # the identity itself (bilinear rotation: to 1e-3)
+    rng = np.random.default_rng(3)
+    N = p.N
+    i = (N - np.arange(N)) % N
+    tw = lambda a: np.conj(a[..., i, :][..., :, i])
+    for n_ref, twinned in ((0, [3, 4, 5, 9]), (6, [0, 1, 11]), (2, [])):
+        ep = P * np.exp(1j * rng.uniform(0, 2 * np.pi, size=p.Np))[:, None, None]
+        for n in twinned:
+            ep[n] = tw(ep[n])
+        out, fl = align_episode(ep, n_ref)
+        assert np.abs(out - P).max() < 1e-10 * np.abs(P).max(), (n_ref, twinned)
+        assert sorted(np.flatnonzero(fl)) == sorted(twinned)
+    # if the reference projection itself is a twin the whole stack comes out as the twin object: consistent again
+    ep = P.copy()
+    ep[0] = tw(ep[0])
+    out, fl = align_episode(ep, 0)
+    assert np.abs(out - tw(P)).max() < 1e-10 * np.abs(P).max() and fl.sum() == p.Np - 1
+    # invariants on arbitrary data: totals real and positive, Fourier moduli untouched
+    g = _stack(5, 8, 77)
+    out, _ = align_episode(g, 2)
+    s = out.sum(axis=(1, 2))
+    assert np.abs(s.imag).max() < 1e-12 and s.real.min() > 0
+    assert np.abs(np.abs(np.fft.fft2(out)) - np.abs(np.fft.fft2(g))).max() < 1e-11
