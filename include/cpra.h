@@ -270,6 +270,20 @@ int cpra_merge_get(cpra_plan_t plan, int slot, float* d_episode);
 int cpra_merge_finish(cpra_plan_t plan, int n_ref, float* d_out, int* d_shifts, int* d_twins);
 
 /*
+ * Consistency of the projections of ONE episode before Step D (reading A28 -- an addition of this
+ * library, not a step the paper states: the paper relies on the carousel coupling alone).  An iterate
+ * without reality constraint keeps, projection by projection, a free global phase and the twin ambiguity; both are
+ * fixed from facts of the forward model, in place on d_episode (complex fp32 [Np][N][N], e.g. cpra_merge_finish's
+ * output):
+ *   1. every projection of one object has the same total (line integrals), so each PO is multiplied by the
+ *      unit phase that makes its total real and positive;
+ *   2. neighbouring projections are similar, so, walking away from projection n_ref in both directions, PO n
+ *      is replaced by its twin conj(O_n(-r)) iff the twin is closer to its already decided neighbour.
+ * d_flips: optional int [Np], 1 where the twin was taken.  Errors: INVALID_ARG, WORKSPACE, CUDA.
+ */
+int cpra_align_episode(cpra_plan_t plan, float* d_episode, int n_ref, int* d_flips);
+
+/*
  * Step D ("performing 3D FTs as a set of 2D FTs"): the 3D transform of a cube, on a plan created
  * with Np == N.  d_in, d_out: complex fp32 [N][N][N] (z, y, x), natural order, may not alias; sign = -1
  * forward (unnormalised), +1 inverse (/ N^3).  The (y, x) transforms of the N slices run through the loop's

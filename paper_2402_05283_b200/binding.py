@@ -58,6 +58,7 @@ SIGNATURES = {
     "cpra_merge_errors": (_ci, [_vp, _vp, _vp]),
     "cpra_merge_get": (_ci, [_vp, _ci, _vp]),
     "cpra_merge_finish": (_ci, [_vp, _ci, _vp, _vp, _vp]),
+    "cpra_align_episode": (_ci, [_vp, _vp, _ci, _vp]),
     "cpra_fft3": (_ci, [_vp, _vp, _vp, _ci]),
     "cpra_refine_3d": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp, _vp]),
     "cpra_fsc": (_ci, [_vp, _vp, _vp, _vp]),
@@ -298,6 +299,13 @@ class Plan:
         tw = torch.zeros(self._n_keep, dtype=torch.int32, device=self.device)
         _chk(self._l.cpra_merge_finish(self._h, int(n_ref), out.data_ptr(), sh.data_ptr(), tw.data_ptr()), "cpra_merge_finish")
         return out, sh, tw
+
+    def align_episode(self, episode, n_ref: int = 0):
+        """Phase gauge and twin chain of one episode, in place; returns the flips (int32 [Np], device)."""
+        import torch
+        fl = torch.zeros(self.Np, dtype=torch.int32, device=self.device)
+        _chk(self._l.cpra_align_episode(self._h, _dptr(episode, torch.complex64, self._px), int(n_ref), fl.data_ptr()), "cpra_align_episode")
+        return fl
 
     def fft3(self, vol, sign: int = -1):
         import torch

@@ -159,6 +159,7 @@ int cpra_bind_workspace(cpra_plan_t p, void* d_ws, size_t bytes)
     p->rays = (int*)(w + L.rays);
     p->mx = (float*)(w + L.mx);
     p->shell = (double*)(w + L.shell);
+    p->align = (double*)(w + L.align);
     p->cur = 0;
     p->have_data = p->have_support = p->have_estimate = p->have_error = false;
     if (!p->attrs_set) {
@@ -633,6 +634,22 @@ int cpra_merge_finish(cpra_plan_t p, int n_ref, float* d_out, int* d_shifts, int
     if (int rc = check_launch(p)) return rc;
     if (d_shifts && cudaMemcpyAsync(d_shifts, b.shift, sizeof(int) * 2 * (size_t)p->Np * p->bank_NL, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
     if (d_twins && cudaMemcpyAsync(d_twins, b.twin, sizeof(int) * p->bank_NL, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    return CPRA_OK;
+}
+
+int cpra_align_episode(cpra_plan_t p, float* d_episode, int n_ref, int* d_flips)
+{
+    if (!p || !d_episode || n_ref < 0 || n_ref >= p->Np) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    int* flags = (int*)(p->align + (size_t)8 * p->Np);
+    k_align_sums<<<p->Np, 256, 0, p->stream>>>((const float2*)d_episode, p->align, p->N);
+    if (int rc = check_launch(p)) return rc;
+    k_align_decide<<<1, 32, 0, p->stream>>>(p->align, flags, p->Np, n_ref);
+    if (int rc = check_launch(p)) return rc;
+    k_align_apply<<<blocks_for(total, 256), 256, 0, p->stream>>>((float2*)d_episode, p->align, flags, p->N, total);
+    if (int rc = check_launch(p)) return rc;
+    if (d_flips && cudaMemcpyAsync(d_flips, flags, sizeof(int) * p->Np, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
     return CPRA_OK;
 }
 

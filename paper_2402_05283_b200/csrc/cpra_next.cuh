@@ -375,4 +375,79 @@ __global__ void k_prtf_finalize(const double* __restrict__ acc, float* __restric
     if (s < ns) out[s] = acc[ns + s] > 0.0 ? (float)(acc[s] / acc[ns + s]) : 0.f;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Consistency of one episode before Step D (reading A28): phase gauge (every projection of one
+// object has the same total) and twin chain (neighbouring projections are similar), on a natural
+// [n][y][x] complex fp32 stack, in place.  scratch: double [Np][8] = (s_re, s_im, c_re, c_im, d_re, d_im, -, -),
+// c_n = <O_{n-1}, O_n>, d_n = <O_{n-1}, T O_n> on the raw data; flags: int [Np].
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_align_sums(const float2* __restrict__ ep, double* __restrict__ scratch, int N)
+{
+    __shared__ double red[32];
+    const int n = blockIdx.x;
+    const size_t px = (size_t)N * N;
+    const float2* __restrict__ o = ep + (size_t)n * px;
+    const float2* __restrict__ a = n > 0 ? ep + (size_t)(n - 1) * px : nullptr;
+    double sr = 0.0, si = 0.0, cr = 0.0, ci = 0.0, dr = 0.0, di = 0.0;
+    for (int i = threadIdx.x; i < N * N; i += blockDim.x) {
+        const float2 v = o[i];
+        sr += v.x; si += v.y;
+        if (a) {
+            const int y = i / N, x = i % N;
+            const float2 w = o[(size_t)((N - y) % N) * N + (N - x) % N];    // T O = conj of this
+            const float2 u = a[i];
+            cr += (double)u.x * v.x + (double)u.y * v.y;  ci += (double)u.x * v.y - (double)u.y * v.x;      // conj(u) v
+            dr += (double)u.x * w.x - (double)u.y * w.y;  di += -(double)u.x * w.y - (double)u.y * w.x;     // conj(u) conj(w)
+        }
+    }
+    sr = block_sum(sr, red); si = block_sum(si, red); cr = block_sum(cr, red); ci = block_sum(ci, red);
+    dr = block_sum(dr, red); di = block_sum(di, red);
+    if (threadIdx.x == 0) {
+        double* s = scratch + (size_t)n * 8;
+        s[0] = sr; s[1] = si; s[2] = cr; s[3] = ci; s[4] = dr; s[5] = di;
+    }
+}
+// unit phases u_n = conj(s_n)/|s_n| (into scratch[n][6..7]); relative twin flags from
+// Re<O'_{n-1}, O'_n> = Re(conj(u_{n-1}) u_n c_n)  and  Re<O'_{n-1}, T O'_n> = Re(conj(u_{n-1}) conj(u_n) d_n);
+// absolute flags by walking away from n_ref
+__global__ void k_align_decide(double* __restrict__ scratch, int* __restrict__ flags, int Np, int n_ref)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    for (int n = 0; n < Np; ++n) {
+        double* s = scratch + (size_t)n * 8;
+        const double m = sqrt(s[0] * s[0] + s[1] * s[1]);
+        s[6] = m > 0.0 ? s[0] / m : 1.0;
+        s[7] = m > 0.0 ? -s[1] / m : 0.0;
+    }
+    auto rel = [&](int n) -> int {   // does projection n flip relative to n - 1?
+        const double* a = scratch + (size_t)(n - 1) * 8;
+        const double* b = scratch + (size_t)n * 8;
+        // conj(u_a) u_b and conj(u_a) conj(u_b)
+        const double pr = a[6] * b[6] + a[7] * b[7], pi = a[6] * b[7] - a[7] * b[6];
+        const double qr = a[6] * b[6] - a[7] * b[7], qi = -a[6] * b[7] - a[7] * b[6];
+        const double pp = pr * b[2] - pi * b[3];
+        const double qq = qr * b[4] - qi * b[5];
+        return qq > pp;
+    };
+    flags[n_ref] = 0;
+    for (int n = n_ref + 1; n < Np; ++n) flags[n] = flags[n - 1] ^ rel(n);
+    for (int n = n_ref - 1; n >= 0; --n) flags[n] = flags[n + 1] ^ rel(n + 1);
+}
+// O_n <- u_n O_n, then its twin where flagged; every thread owns a pixel and its mirror partner
+__global__ void k_align_apply(float2* __restrict__ ep, const double* __restrict__ scratch, const int* __restrict__ flags, int N, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const size_t px = (size_t)N * N;
+    const int n = (int)(i / px), y = (int)((i % px) / N), x = (int)(i % N);
+    const size_t j = (size_t)n * px + (size_t)((N - y) % N) * N + (N - x) % N;
+    if (j < i) return;                                  // the partner's thread does both
+    const double ur = scratch[(size_t)n * 8 + 6], ui = scratch[(size_t)n * 8 + 7];
+    auto rot = [&](float2 v) { return make_float2((float)(ur * v.x - ui * v.y), (float)(ur * v.y + ui * v.x)); };
+    float2 a = rot(ep[i]), b = rot(ep[j]);
+    if (flags[n]) { const float2 t = a; a = make_float2(b.x, -b.y); b = make_float2(t.x, -t.y); }
+    ep[i] = a;
+    if (j != i) ep[j] = b;
+}
+
 }  // namespace cpra

@@ -41,6 +41,7 @@ struct cpra_plan_s {
     int* rays = nullptr;
     float* mx = nullptr;      // per-image maxima of the shrink-wrap update
     double* shell = nullptr;  // shell sums of cpra_fsc / cpra_prtf
+    double* align = nullptr;  // scratch of cpra_align_episode
     int cur = 0;
     // parameters / state
     int K = 1;
@@ -89,7 +90,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t tw, A, S16, S8, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, mx, shell, total;
+    size_t tw, A, S16, S8, st0, st1, scr, scr2, partial, den, uphi, ustart, rays, mx, shell, align, total;
 };
 
 inline Layout layout_of(int N, int Np, bool generic = false)
@@ -112,6 +113,7 @@ inline Layout layout_of(int N, int Np, bool generic = false)
     L.rays = c.take(sizeof(int) * 2 * (size_t)Np);
     L.mx = c.take(sizeof(float) * (size_t)Np);
     L.shell = c.take(sizeof(double) * 3 * (size_t)(N / 2 + 1));   // shell sums of cpra_fsc / cpra_prtf
+    L.align = c.take(sizeof(double) * 9 * (size_t)Np);   // cpra_align_episode: sums, inner products, phases, flags
     L.total = c.off;
     return L;
 }

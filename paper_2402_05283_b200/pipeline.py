@@ -6,6 +6,8 @@
     Step B  per restart: N_e episodes of N_ei iterations of the coupled loop (cpra_iterate with n_ei = N_ei)
     Step C  the bank keeps the N_l lowest-error episodes (cpra_merge_offer, decided on the device); centre of mass,
             twin selection, average (cpra_merge_finish)
+            then cpra_align_episode: the projections of the merged episode are given one common phase gauge and one
+            twin choice (reading A28) -- without it the slices of an unconstrained complex iterate do not fit together
     Step D  Fourier-slice assembly of the merged episode (cpra_assemble_3d), then optionally the inverse 3D
             transform / the iterations against a 3D support (cpra_fft3 / cpra_refine_3d; power-of-two N)
 
@@ -54,7 +56,7 @@ def random_phase_starts(plan, intensity, mask, seed: int):
 def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, n_pre: int, n_episodes: int, n_ei: int,
                 beta: float = 0.9, alpha=(0.6, 0.2), update: str = "hio", seam_flip: bool = False, seed: int = 0,
                 shrinkwrap: Optional[tuple] = None, assemble: bool = True, support3d=None, refine_iters: int = 0,
-                n_ref: int = 0) -> CpraResult:
+                n_ref: int = 0, align: bool = True) -> CpraResult:
     """Steps A-D.  intensity fp32 [Np, N, N], mask u8 [Np, N, N] or None, support u8 [Np, N, N]: CUDA tensors;
     angles: Np radians (host).  shrinkwrap = (sigma, threshold): one support update at the end of every episode
     (power-of-two N).  support3d u8 [N, N, N] + refine_iters > 0: Step D's iterations; refine_iters == 0
@@ -113,6 +115,8 @@ def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, 
                 plan.shrinkwrap(float(shrinkwrap[0]), float(shrinkwrap[1]))
         plan.merge_offer()
     episode, shifts, twins = plan.merge_finish(n_ref)
+    if align:
+        plan.align_episode(episode, n_ref)          # one phase gauge and one twin choice for the whole stack (reading A28)
     errors, count = plan.merge_errors()
     timed("steps_b_c", t0)
     res = CpraResult(episode=episode, errors=errors[:int(count.cpu()[0])], shifts=shifts, twins=twins, seconds=sec)

@@ -448,3 +448,54 @@ def test_positivity(torch_cuda, N, Np, rule, flags):
     o.iterate(1, 0.9)
     g.iterate(1, 0.9)
     assert rel_l2(_get(g), o.get_projections(0)) <= 2e-3
+
+
+@pytest.mark.parametrize("N,Np,n_ref", [(64, 12, 0), (128, 7, 3), (160, 5, 4)])
+def test_align_episode(torch_cuda, N, Np, n_ref):
+    """cpra_align_episode against the oracle on a stack of true projections with scrambled phases and twins, and on
+    a reconstructed episode."""
+    import paper_2402_05283_b200 as cpra
+    from oracle import align_episode
+    p = cpra_inputs.make_problem(1, Np=Np, N=N, noise=False)
+    rng = np.random.default_rng(N)
+    i = (N - np.arange(N)) % N
+    ep = (p.projections * np.exp(1j * rng.uniform(0, 6.28, size=Np))[:, None, None]).astype(np.complex64)
+    for n in (1, Np - 2):
+        ep[n] = np.conj(ep[n][i][:, i])
+    plan = cpra.Plan(N, Np)
+    d = torch_cuda.from_numpy(ep.copy()).cuda()
+    fl = plan.align_episode(d, n_ref).cpu().numpy()
+    ref, flo = align_episode(ep, n_ref)
+    assert np.array_equal(fl, flo)
+    assert rel_l2(d.cpu().numpy(), ref) <= 1e-6
+    g = _gpu(p)
+    g.iterate(5, p.beta)
+    e2 = g.get_projections(1)
+    ref2, fl2 = align_episode(e2.cpu().numpy(), n_ref)
+    flg = g.align_episode(e2, n_ref).cpu().numpy()
+    assert np.array_equal(flg, fl2) and rel_l2(e2.cpu().numpy(), ref2) <= 1e-6
+
+
+def test_pipeline_steps_a_to_d(torch_cuda):
+    """paper_2402_05283_b200.pipeline.reconstruct on config 1 (noise-free, 32 angles): N_r = 6 restarts, N_l = 3 kept,
+    Step A batched over the restarts, Step D to O(r).  The merged projections correlate with the true ones and the
+    3D object with the true object (up to the twin of the whole object)."""
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.make_problem(1, keep_object=True)
+    dev = "cuda"
+    I, M, S = (torch_cuda.from_numpy(a).to(dev) for a in (p.intensity, p.mask, p.support))
+    res = cpra.pipeline.reconstruct(I, M, S, p.angles, n_restarts=6, n_keep=3, n_pre=200, n_episodes=25, n_ei=2, seam_flip=True)
+    N = p.N
+    ep = res.episode.cpu().numpy()
+    corr = lambda a, b: abs(np.vdot(a, b)) / (np.linalg.norm(a) * np.linalg.norm(b))
+    c2 = np.mean([max(corr(np.abs(ep[n]), np.abs(p.projections[n])), corr(np.abs(ep[n][::-1, ::-1]), np.abs(p.projections[n]))) for n in range(p.Np)])
+    assert c2 > 0.9, c2
+    pad = np.zeros((N, N, N))
+    off = (N - p.obj.shape[0]) // 2
+    pad[off:off + p.obj.shape[0], off:off + p.obj.shape[0], off:off + p.obj.shape[0]] = p.obj
+    rec = res.obj.cpu().numpy()
+    i = (N - np.arange(N)) % N
+    c3 = max(corr(np.abs(rec), pad), corr(np.abs(rec[i][:, i][:, :, i]), pad))
+    print(f"\npipeline: corr2d={c2:.3f} corr3d={c3:.3f} errors={res.errors.cpu().numpy()} seconds={res.seconds}")
+    assert c3 > 0.8, c3
+    assert len(res.errors) == 3 and float(res.errors.max()) < 0.2
