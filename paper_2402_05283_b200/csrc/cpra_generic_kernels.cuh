@@ -19,20 +19,35 @@ __device__ __forceinline__ void gen_small_dft(c2 (&v)[R], const float2* __restri
     if constexpr (R == 2 || R == 4 || R == 8) {
         dft<R, INV>(v);
     } else {
-        c2 o[R];
+        // odd prime R: X[p], X[R-p] = t -+ i u (forward) with t = v0 + sum_q cos(2 pi p q / R) (v_q + v_{R-q}),
+        // u = sum_q sin(2 pi p q / R) (v_q - v_{R-q}), q = 1 .. (R-1)/2: real coefficients only
+        constexpr int H = (R - 1) / 2;
+        c2 A[H], B[H];
+        c2 sum = v[0];
 #pragma unroll
-        for (int p = 0; p < R; ++p) {
-            c2 acc = v[0];
-#pragma unroll
-            for (int q = 1; q < R; ++q) {
-                const float2 t = tw[((p * q) % R) * rstep];
-                const c2 y = INV ? cmulc(v[q], bc(t.x), bc(t.y)) : cmul(v[q], bc(t.x), bc(t.y));
-                acc = cadd(acc, y);
-            }
-            o[p] = acc;
+        for (int q = 1; q <= H; ++q) {
+            A[q - 1] = cadd(v[q], v[R - q]);
+            B[q - 1] = csub(v[q], v[R - q]);
+            sum = cadd(sum, A[q - 1]);
         }
+        const c2 v0 = v[0];
+        v[0] = sum;
 #pragma unroll
-        for (int p = 0; p < R; ++p) v[p] = o[p];
+        for (int p = 1; p <= H; ++p) {
+            c2 t = v0, u{make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+#pragma unroll
+            for (int q = 1; q <= H; ++q) {
+                const float2 w = tw[((p * q) % R) * rstep];          // (cos, -sin) of 2 pi p q / R
+                const float2 c = bc(w.x), sn = bc(-w.y);
+                t = c2{pfma(c, A[q - 1].re, t.re), pfma(c, A[q - 1].im, t.im)};
+                u = c2{pfma(sn, B[q - 1].re, u.re), pfma(sn, B[q - 1].im, u.im)};
+            }
+            // -i u = (u.im, -u.re)
+            const c2 lo{padd(t.re, u.im), psub(t.im, u.re)};     // t - i u
+            const c2 hi{psub(t.re, u.im), padd(t.im, u.re)};     // t + i u
+            v[p] = INV ? hi : lo;
+            v[R - p] = INV ? lo : hi;
+        }
     }
 }
 
@@ -42,8 +57,11 @@ __device__ __forceinline__ void gen_stage(const float2* __restrict__ a, float2* 
                                           int N, int W, int Ns)
 {
     const int Wp = gen_wp(W), W2 = W / 2, m = N / R, tstep = N / (Ns * R), rstep = N / R;
+    const int w2shift = 31 - __clz(W2);                      // W / 2 is a power of two
+    const float invNs = 1.0f / (float)Ns;                    // j / Ns by reciprocal: (j + 0.5) / Ns is never within rounding of an integer
     for (int i = threadIdx.x; i < m * W2; i += blockDim.x) {
-        const int w = 2 * (i % W2), j = i / W2, k = j % Ns;
+        const int w = 2 * (i & (W2 - 1)), j = i >> w2shift;
+        const int jb = (int)(((float)j + 0.5f) * invNs), k = j - jb * Ns;
         c2 v[R];
 #pragma unroll
         for (int q = 0; q < R; ++q) {
@@ -54,7 +72,7 @@ __device__ __forceinline__ void gen_stage(const float2* __restrict__ a, float2* 
             }
         }
         gen_small_dft<R, INV>(v, tw, rstep);
-        const int j0 = (j / Ns) * Ns * R + k;
+        const int j0 = jb * Ns * R + k;
 #pragma unroll
         for (int p = 0; p < R; ++p) gen_st2(b + (j0 + p * Ns) * Wp + w, v[p]);
     }
