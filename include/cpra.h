@@ -326,6 +326,27 @@ int cpra_fsc(cpra_plan_t plan, const float* d_F1, const float* d_F2, float* d_ou
 int cpra_prtf(cpra_plan_t plan, const float* d_avg, float* d_out);
 
 /*
+ * cpra_fsc for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same Fourier shell correlation (same kernels' arithmetic, same
+ * result up to the order of the double atomics), but with no plan and no workspace.  The shell accumulators live in
+ * a file-scope __device__ array of CPRA_FSC_STATIC_SCRATCH_BYTES inside libcpra.so, which every GPU that loads the
+ * library holds until the process exits; the call allocates nothing (no cudaMalloc / cudaFree, no allocating
+ * library routine; the array's device address is looked up once per device, on the first call made with that device
+ * current).
+ *   N        grid size, even, 2 <= N <= CPRA_FSC_STATIC_MAX_N; a larger N is refused with UNSUPPORTED_SIZE
+ *   d_F1/2   DEVICE complex fp32 [N][N][N], native order (caller-owned, read only)
+ *   d_out    DEVICE fp32 [N/2 + 1] (caller-owned)
+ *   stream   a cudaStream_t of the current device (NULL = default stream); the call is asynchronous on it
+ * All calls share the one array, which keeps the sums of the last call: every call clears it first, on its stream.
+ * Two calls that overlap on the GPU (different streams without a dependency, or two host threads on two streams)
+ * race on it and both results are undefined; calls on one stream, or otherwise ordered, are safe.
+ * Errors: INVALID_ARG (NULL, N odd or < 2), UNSUPPORTED_SIZE (N > CPRA_FSC_STATIC_MAX_N), CUDA.
+ */
+#define CPRA_FSC_STATIC_MAX_N 1024
+#define CPRA_FSC_STATIC_SCRATCH_BYTES 12312 /* 3 * (CPRA_FSC_STATIC_MAX_N / 2 + 1) doubles */
+int cpra_fsc_static(int N, const float* d_F1, const float* d_F2, float* d_out, void* stream);
+
+/*
  * End-to-end convenience with HOST buffers (pinned memory recommended): uploads the inputs,
  * runs k iterations, downloads the result and synchronises the plan's stream.
  *   h_I [Np][N][N] fp32, h_mask [Np][N][N] u8 or NULL, h_angles [Np] or NULL, h_S [Np][N][N] u8,

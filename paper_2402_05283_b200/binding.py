@@ -17,6 +17,7 @@ ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_READY, ERR_WORKSPACE, ERR_CUDA, E
 ITERATE, SUPPORTED = 0, 1
 FLAG_DEFAULT, FLAG_FORCE_MULTIPASS, FLAG_NO_CHUNKING, FLAG_NO_WALK = 0, 1, 2, 4
 MAX_K = 8
+FSC_STATIC_MAX_N = 1024
 PROFILE_CLASSES = 5
 PROFILE_NAMES = ("row_fwd", "col", "row_inv", "image", "walk")
 
@@ -63,6 +64,7 @@ SIGNATURES = {
     "cpra_refine_3d": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp, _vp]),
     "cpra_fsc": (_ci, [_vp, _vp, _vp, _vp]),
     "cpra_prtf": (_ci, [_vp, _vp, _vp]),
+    "cpra_fsc_static": (_ci, [_ci, _vp, _vp, _vp, _vp]),
     "cpra_destroy": (_ci, [_vp]),
     "cpra_status_string": (ctypes.c_char_p, [_ci]),
 }
@@ -113,6 +115,24 @@ def _dptr(t, dtype, nelem=None):
     if nelem is not None and t.numel() != nelem:
         raise ValueError(f"expected {nelem} elements, got {t.numel()}")
     return t.data_ptr()
+
+
+def fsc_static(F1, F2, out=None):
+    """cpra_fsc_static: the Fourier shell correlation of two complex64 [N, N, N] CUDA tensors with no plan, no
+    workspace and no device allocation inside the call (its scratch is a fixed __device__ array in libcpra.so;
+    N even, N <= FSC_STATIC_MAX_N; calls that overlap on the GPU race on that array).  `out`: float32 [N/2 + 1]
+    CUDA tensor to write into -- pass one where nothing may be allocated; otherwise torch allocates it here."""
+    import torch
+    N = int(F1.shape[-1])
+    if out is None:
+        out = torch.empty(N // 2 + 1, dtype=torch.float32, device=F1.device)
+    with torch.cuda.device(F1.device):      # the array's address is looked up for the CURRENT device
+        rc = lib().cpra_fsc_static(N, _dptr(F1, torch.complex64, N ** 3), _dptr(F2, torch.complex64, N ** 3),
+                                   _dptr(out, torch.float32, N // 2 + 1), torch.cuda.current_stream(F1.device).cuda_stream)
+    if rc == ERR_UNSUPPORTED_SIZE:
+        raise CpraError(rc, f"cpra_fsc_static (N = {N} exceeds the static scratch, N <= {FSC_STATIC_MAX_N})")
+    _chk(rc, "cpra_fsc_static")
+    return out
 
 
 class Plan:

@@ -19,7 +19,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcpra.so")
 SIZES = (16, 32, 64, 128, 256, 512, 1024)
 HEADERS = ["cpra_generic.cuh", "cpra_generic_kernels.cuh", "cpra_fft.cuh", "cpra_kernels.cuh", "cpra_layout.cuh", "cpra_image.cuh", "cpra_walk.cuh", "cpra_plan.cuh", "cpra_next.cuh", "cpra_cluster.cuh"]
-DEPENDS = [os.path.join(CSRC, f) for f in ["cpra_api.cu", "cpra_inst.cu", "cpra_generic.cu"] + HEADERS] + [
+DEPENDS = [os.path.join(CSRC, f) for f in ["cpra_api.cu", "cpra_inst.cu", "cpra_generic.cu", "cpra_static.cu"] + HEADERS] + [
     os.path.join(os.path.dirname(HERE), "include", "cpra.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "static"]
@@ -38,7 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "nvcc")
     os.makedirs(OBJ, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
-    units = [("cpra_api.o", "cpra_api.cu", []), ("cpra_generic.o", "cpra_generic.cu", [])] + [(f"cpra_inst_{n}.o", "cpra_inst.cu", [f"-DCPRA_INST_N={n}"]) for n in SIZES]
+    units = [("cpra_api.o", "cpra_api.cu", []), ("cpra_generic.o", "cpra_generic.cu", []), ("cpra_static.o", "cpra_static.cu", [])] + [(f"cpra_inst_{n}.o", "cpra_inst.cu", [f"-DCPRA_INST_N={n}"]) for n in SIZES]
     procs = []
     for obj, src, defs in units:
         cmd = [nvcc] + NVCC_FLAGS + extra + defs + ["-c", "-o", os.path.join(OBJ, obj), os.path.join(CSRC, src)]
