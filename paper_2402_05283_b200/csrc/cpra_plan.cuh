@@ -372,13 +372,13 @@ inline bool encode_scratch_tmap(CUtensorMap* tm, void* base, int N, int Np, int 
                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// K3 of one iteration fused with K1 of the next (cpra_walk.cuh): 2 CTAs per SM, each a run of tiles
+// K3 of one iteration fused with K1 of the next (cpra_walk.cuh): walk_ctas_per_sm CTAs per SM, each a run of tiles
 template <int N>
 int Launch<N>::walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta, bool fires)
 {
     if constexpr (walk_ok<N>()) {
         const int total = (N / tile_batch<N>()) * p->Np;
-        const int per_sm = p->walk_ctas > 0 ? p->walk_ctas : (N >= 512 ? 2 : 4);   // what the kernel's registers / shared memory allow
+        const int per_sm = p->walk_ctas > 0 ? p->walk_ctas : walk_ctas_per_sm<N>();   // what the kernel's registers / shared memory allow
         const int ctas = std::min(total, per_sm * p->sms);
         const int per = (total + ctas - 1) / ctas;
         const dim3 grid((unsigned)((total + per - 1) / per));

@@ -1,5 +1,5 @@
 // cpra_walk.cuh -- K3 of iteration t fused with K1 of iteration t + 1 in a CTA that WALKS along n
-// (sm_100a; plans with 8-row tiles: a tile is N x 64 B = 32 KiB at N = 512).
+// (sm_100a; plans with 8-row tiles: a tile is N x 64 B = 16 / 32 / 64 KiB at N = 256 / 512 / 1024).
 //
 // The carousel mix (Eq. (4)) needs the NEW states of projections n-1, n, n+1.  A CTA
 // that owns a run of consecutive n for one row tile rt keeps the last three new tiles in shared
@@ -25,7 +25,9 @@
 
 namespace cpra {
 
-template <int N> __host__ __device__ constexpr bool walk_ok() { return tile_batch<N>() == 8 && Radix<N>::S == 3 && N <= 512; }
+template <int N> __host__ __device__ constexpr bool walk_ok() { return tile_batch<N>() == 8 && Radix<N>::S == 3 && N <= 1024; }
+// CTAs per SM that the three slots allow (N = 1024: 3 x 64 KiB, one CTA of 512 threads)
+template <int N> __host__ __device__ constexpr int walk_ctas_per_sm() { return N >= 1024 ? 1 : (N >= 512 ? 2 : 4); }
 constexpr int WALK_SLOTS = 3;
 // slots + twiddles + 3 mbarriers + support words of the 3 slots
 template <int N> __host__ __device__ constexpr int walk_smem_bytes()
@@ -34,8 +36,31 @@ template <int N> __host__ __device__ constexpr int walk_smem_bytes()
 }
 template <int N> __host__ __device__ constexpr int walk_threads() { return tile_pairs<N>() * (N / last_radix<N>()); }
 
+// N = 1024: the two threads (lanes l, l ^ 8) that share a radix-16 first-stage butterfly
+__device__ __forceinline__ c2 walk_xchg(c2 a)   // the partner's value
+{
+    return c2{make_float2(__shfl_xor_sync(0xffffffffu, a.re.x, 8), __shfl_xor_sync(0xffffffffu, a.re.y, 8)),
+              make_float2(__shfl_xor_sync(0xffffffffu, a.im.x, 8), __shfl_xor_sync(0xffffffffu, a.im.y, 8))};
+}
+__device__ __forceinline__ c2 walk_sel(int c, c2 a, c2 b)
+{
+    return c2{make_float2(c ? a.re.x : b.re.x, c ? a.re.y : b.re.y), make_float2(c ? a.im.x : b.im.x, c ? a.im.y : b.im.y)};
+}
+// the outputs 8 h0 + m of dft<16> from its two radix-8 halves: a = the half this thread computed (inputs of parity h0)
+template <bool INV>
+__device__ __forceinline__ void walk_combine(c2 (&a)[8], int h0)
+{
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        const c2 o = walk_xchg(a[m]);
+        c2 lo, hi;
+        tw_addsub<INV>(walk_sel(h0, o, a[m]), walk_sel(h0, a[m], o), m, lo, hi);
+        a[m] = walk_sel(h0, hi, lo);
+    }
+}
+
 template <int N>
-__global__ void __launch_bounds__(walk_threads<N>(), N >= 512 ? 2 : 4)
+__global__ void __launch_bounds__(walk_threads<N>(), walk_ctas_per_sm<N>())
 k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out, const float4* __restrict__ gh_old,
            float4* __restrict__ gh_new, const float2* __restrict__ twg, const uint16_t* __restrict__ S16,
            MixParams mp, float beta, int Np, int per_cta)
@@ -44,9 +69,18 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>(), NT = walk_threads<N>();
     constexpr int NRT = N / TBN, NCT = N / TBN, R0 = RX::R0, R1 = RX::R1, RL = RX::R2, M0 = N / R0;
     // every thread owns E0 = 8 elements of the tile in the first-stage arrangement: B0 butterflies of radix R0
-    // (N = 512: one of radix 8; N = 256: two of radix 4), and one radix-8 butterfly in each inner stage
-    constexpr int QN = NT / NP, B0 = NP * M0 / NT, E0 = B0 * R0;
-    static_assert(B0 * NT == NP * M0 && E0 == 8 && NP * (N / R1) == NT && RL == 8, "8 first-stage elements and one inner butterfly per thread");
+    // (N = 512: one of radix 8; N = 256: two of radix 4), and one radix-8 butterfly in each inner stage.
+    // N = 1024 (R0 = 16, SPLIT = 2): a first-stage butterfly belongs to TWO threads of a warp (lanes l, l ^ 8).  The
+    // radix-16 DFT of cpra_fft.cuh is two radix-8 DFTs over the inputs of even / odd index followed by 8 twiddled
+    // add/subs that give outputs k and k + 8: thread h0 does the radix-8 DFT of the inputs of parity h0, the two
+    // exchange their 8 results by shuffles, and each does the add/subs keeping the outputs of half h0 (8 h0 + k).
+    // Every operation is the one dft<16> does on the same operands: the results are bit-identical to the tile kernels'.
+    // On the object side (g_new, ghat, the mix, the support) a thread therefore owns the elements r = 8 h0 + e, on
+    // the spectrum side of the inverse the elements r = 2 e + h0; the forward transform regroups by parity first.
+    constexpr int SPLIT = R0 == 16 ? 2 : 1;
+    constexpr int QN = NT / NP, B0 = SPLIT == 2 ? 1 : NP * M0 / NT, E0 = SPLIT == 2 ? R0 / 2 : B0 * R0;
+    static_assert((SPLIT == 2 ? 2 * NP * M0 == NT : B0 * NT == NP * M0) && E0 == 8 && NP * (N / R1) == NT && RL == 8,
+                  "8 first-stage elements and one inner butterfly per thread");
     static_assert(NP == 4 && R1 == 8, "the two inner stages of a 64-position block must belong to one warp");
     extern __shared__ __align__(128) float4 sm[];
     float4* const slots = sm;
@@ -75,32 +109,72 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     //   stage 0 (stride M0):    p = q + QN b + M0 r     ppos(p) = ppos(q) + QN b + M0 r   (element e = R0 b + r)
     //   stage 1 (stride 8):     p = 64 b + n2 + 8 r     ppos(p) = p ^ (r & 1)
     //   last    (contiguous):   p = 8 q + r             ppos(p) = 8 q + (r ^ (q & 1))
-    const int o0 = ppos<N>(q) * NP + j;
+    // first stage: SPLIT == 1: the thread's inner indices (q, j).  SPLIT == 2: lane bits [1:0] = pair, [2] = low bit
+    // of the butterfly index q0 (a quarter-warp reads two neighbouring positions: conflict-free), [3] = half h0
+    const int j0 = SPLIT == 2 ? (int)(threadIdx.x & 3) : j;
+    const int q0 = SPLIT == 2 ? (int)(((threadIdx.x >> 4) << 1) | ((threadIdx.x >> 2) & 1)) : q;
+    const int h0 = SPLIT == 2 ? (int)((threadIdx.x >> 3) & 1) : 0;
+    const int o0 = ppos<N>(q0) * NP + j0;
     const int o1e = ((q / 8) * 64 + (q % 8)) * NP + j, o1o = ((q / 8) * 64 + ((q % 8) ^ 1)) * NP + j;
     const int oLe = (8 * q + (q & 1)) * NP + j, oLo = (8 * q + 1 - (q & 1)) * NP + j;
-    auto p0 = [&](int e) -> int { return q + QN * (e / R0) + M0 * (e % R0); };   // position of first-stage element e
-    auto i0 = [&](int e) -> int { return o0 + (e / R0) * (QN * NP) + (e % R0) * (M0 * NP); };
+    // object side: position and quad of first-stage element e (SPLIT == 2: r = 8 h0 + e)
+    auto p0 = [&](int e) -> int { return SPLIT == 2 ? q0 + M0 * (E0 * h0 + e) : q + QN * (e / R0) + M0 * (e % R0); };
+    auto i0 = [&](int e) -> int { return SPLIT == 2 ? o0 + (E0 * h0 + e) * (M0 * NP) : o0 + (e / R0) * (QN * NP) + (e % R0) * (M0 * NP); };
+    // spectrum side of the inverse first stage: where its inputs are read (SPLIT == 2: r = 2 e + h0)
+    auto iS = [&](int e) -> int { return SPLIT == 2 ? o0 + (2 * e + h0) * (M0 * NP) : i0(e); };
     auto i1 = [&](int r) -> int { return ((r & 1) ? o1o : o1e) + r * (8 * NP); };
     auto iL = [&](int r) -> int { return ((r & 1) ? oLo : oLe) + (r & ~1) * NP; };
     // the quad of the stage-0 element r of this thread MIRRORED in x (position p -> (N - p) mod N): read for a
     // halo tile that lies across the seam of a [0, 180) scan (cpra_set_seam, reading A5b)
-    auto i0m = [&](int e) -> int { return ppos<N>((N - p0(e)) & (N - 1)) * NP + j; };
+    auto i0m = [&](int e) -> int { return ppos<N>((N - p0(e)) & (N - 1)) * NP + j0; };
     static_assert(N / R0 == 64 && QN % 16 == 0, "offsets above assume inner radices 8 x 8 (64-position blocks)");
-    // the B0 first-stage butterflies of this thread (twiddle index n2 = q + QN b)
+    // the B0 first-stage butterflies of this thread (twiddle index n2 = q + QN b); SPLIT == 2: its half of one
     auto stage0_inv = [&](c2 (&a)[E0]) {
+        if constexpr (SPLIT == 2) {
+            const float2* __restrict__ t = tw0 + q0 * (R0 - 1);   // a[e] = input r = 2 e + h0, times conj w_r (r >= 1)
 #pragma unroll
-        for (int b = 0; b < B0; ++b) {
-            c2(&u)[R0] = *reinterpret_cast<c2(*)[R0]>(&a[b * R0]);
-            twiddle<R0, true>(u, tw0, q + QN * b);
-            dft<R0, true>(u);
+            for (int e = 0; e < E0; ++e) {
+                const float2 w = t[e == 0 ? 0 : 2 * e + h0 - 1];
+                const c2 x = cmulc(a[e], bc(w.x), bc(w.y));
+                a[e] = e == 0 ? walk_sel(h0, x, a[e]) : x;
+            }
+            dft<E0, true>(a);
+            walk_combine<true>(a, h0);
+        } else {
+#pragma unroll
+            for (int b = 0; b < B0; ++b) {
+                c2(&u)[R0] = *reinterpret_cast<c2(*)[R0]>(&a[b * R0]);
+                twiddle<R0, true>(u, tw0, q + QN * b);
+                dft<R0, true>(u);
+            }
         }
     };
     auto stage0_fwd = [&](c2 (&a)[E0]) {
+        if constexpr (SPLIT == 2) {
+            // a[e] = element r = 8 h0 + e; the radix-8 DFT of parity h0 needs r = 2 e' + h0: half of them are the partner's
+            c2 n[E0];
 #pragma unroll
-        for (int b = 0; b < B0; ++b) {
-            c2(&u)[R0] = *reinterpret_cast<c2(*)[R0]>(&a[b * R0]);
-            dft<R0, false>(u);
-            twiddle<R0, false>(u, tw0, q + QN * b);
+            for (int i = 0; i < E0 / 2; ++i) {
+                const c2 recv = walk_xchg(walk_sel(h0, a[2 * i], a[2 * i + 1]));
+                n[i] = walk_sel(h0, recv, a[2 * i]);
+                n[E0 / 2 + i] = walk_sel(h0, a[2 * i + 1], recv);
+            }
+            dft<E0, false>(n);
+            walk_combine<false>(n, h0);
+            const float2* __restrict__ t = tw0 + q0 * (R0 - 1);   // output r = 8 h0 + m, times w_r (r >= 1)
+#pragma unroll
+            for (int m = 0; m < E0; ++m) {
+                const float2 w = t[m == 0 ? (E0 - 1) * h0 : E0 * h0 + m - 1];
+                const c2 x = cmul(n[m], bc(w.x), bc(w.y));
+                a[m] = m == 0 ? walk_sel(h0, x, n[m]) : x;
+            }
+        } else {
+#pragma unroll
+            for (int b = 0; b < B0; ++b) {
+                c2(&u)[R0] = *reinterpret_cast<c2(*)[R0]>(&a[b * R0]);
+                dft<R0, false>(u);
+                twiddle<R0, false>(u, tw0, q + QN * b);
+            }
         }
     };
     const float2 a0 = bc(mp.a[0]), a1 = bc(mp.a[1]);
@@ -163,12 +237,12 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             }
             pend_tile = -1;
 #pragma unroll
-            for (int r = 0; r < E0; ++r) v[r] = from_quad(tile[i0(r)]);
+            for (int r = 0; r < E0; ++r) v[r] = from_quad(tile[iS(r)]);
             stage0_inv(v);
             const uint16_t* __restrict__ sp = sup + s * N;
 #pragma unroll
             for (int r = 0; r < E0; ++r) {
-                const unsigned bits = inside_bits(mp, (unsigned)sp[p0(r)] >> (sshift + 2 * j), v[r].re);
+                const unsigned bits = inside_bits(mp, (unsigned)sp[p0(r)] >> (sshift + 2 * j0), v[r].re);
                 const float2 ore = update_outside(mp, v[r].re, g0[r].re), oim = update_outside(mp, v[r].im, g0[r].im);
                 v[r].re = make_float2((bits & 1) ? v[r].re.x : ore.x, (bits & 2) ? v[r].re.y : ore.y);
                 v[r].im = make_float2((bits & 1) ? v[r].im.x : oim.x, (bits & 2) ? v[r].im.y : oim.y);
