@@ -46,16 +46,48 @@ __device__ __forceinline__ c2 walk_sel(int c, c2 a, c2 b)
 {
     return c2{make_float2(c ? a.re.x : b.re.x, c ? a.re.y : b.re.y), make_float2(c ? a.im.x : b.im.x, c ? a.im.y : b.im.y)};
 }
-// the outputs 8 h0 + m of dft<16> from its two radix-8 halves: a = the half this thread computed (inputs of parity h0)
+// tw_addsub<INV>(e, o, k, lo, hi) of cpra_fft.cuh for k = m + 4 h0 with h0 known only at run time: the same operations
+// on the same operands as the compile-time version (k and k + 4 share a code shape; constants and operand roles are selected)
+template <bool INV>
+__device__ __forceinline__ void walk_tw_addsub(c2 e, c2 o, int m, int h0, c2& lo, c2& hi)
+{
+    constexpr float H = 0.70710678118654752440f;
+    constexpr float C1 = 0.92387953251128675613f, S1 = 0.38268343236508977173f;
+    if (m == 0) {
+        // k = 0: W o = o;  k = 4: W o = (o.im, -o.re) forward, (-o.im, o.re) inverse
+        const float2 x = h0 ? (INV ? neg2(o.im) : o.im) : o.re, y = h0 ? (INV ? o.re : neg2(o.re)) : o.im;
+        lo = c2{padd(e.re, x), padd(e.im, y)};
+        hi = c2{psub(e.re, x), psub(e.im, y)};
+    } else if (m == 2) {
+        const float2 s = padd(o.re, o.im), d = psub(o.im, o.re);
+        const float2 tr = h0 ? (INV ? neg2(s) : d) : (INV ? neg2(d) : s);
+        const float2 ti = h0 ? (INV ? neg2(d) : neg2(s)) : (INV ? s : d);
+        lo = c2{pfma(tr, bc(H), e.re), pfma(ti, bc(H), e.im)};
+        hi = c2{pfma(tr, bc(-H), e.re), pfma(ti, bc(-H), e.im)};
+    } else {
+        // m = 1: k = 1 | 5;  m = 3: k = 3 | 7
+        const float c = (m == 1) ? (h0 ? -S1 : C1) : (h0 ? -C1 : S1);
+        const float s0 = (m == 1) ? (h0 ? C1 : S1) : (h0 ? S1 : C1);
+        const float s = INV ? -s0 : s0;
+        const float2 tr = pfma(o.re, bc(c), pmul(o.im, bc(s)));
+        const float2 ti = pfma(o.im, bc(c), neg2(pmul(o.re, bc(s))));
+        lo = c2{padd(e.re, tr), padd(e.im, ti)};
+        hi = c2{psub(e.re, tr), psub(e.im, ti)};
+    }
+}
+// The second half of dft<16>: a = the radix-8 DFT this thread computed over the inputs of parity h0 (E if h0 = 0, O if
+// h0 = 1).  Thread h0 takes k = 4 h0 + m, m = 0 .. 3: it gets the four values of the other parity it needs, and ends with
+// output k in a[m] and output k + 8 in a[4 + m].
 template <bool INV>
 __device__ __forceinline__ void walk_combine(c2 (&a)[8], int h0)
 {
 #pragma unroll
-    for (int m = 0; m < 8; ++m) {
-        const c2 o = walk_xchg(a[m]);
+    for (int m = 0; m < 4; ++m) {
+        const c2 recv = walk_xchg(walk_sel(h0, a[m], a[4 + m]));   // h0 = 0 sends E[4 + m] and gets O[m]; h0 = 1 the reverse
         c2 lo, hi;
-        tw_addsub<INV>(walk_sel(h0, o, a[m]), walk_sel(h0, a[m], o), m, lo, hi);
-        a[m] = walk_sel(h0, hi, lo);
+        walk_tw_addsub<INV>(walk_sel(h0, recv, a[m]), walk_sel(h0, a[4 + m], recv), m, h0, lo, hi);
+        a[m] = lo;
+        a[4 + m] = hi;
     }
 }
 
@@ -73,10 +105,11 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     // N = 1024 (R0 = 16, SPLIT = 2): a first-stage butterfly belongs to TWO threads of a warp (lanes l, l ^ 8).  The
     // radix-16 DFT of cpra_fft.cuh is two radix-8 DFTs over the inputs of even / odd index followed by 8 twiddled
     // add/subs that give outputs k and k + 8: thread h0 does the radix-8 DFT of the inputs of parity h0, the two
-    // exchange their 8 results by shuffles, and each does the add/subs keeping the outputs of half h0 (8 h0 + k).
+    // exchange 4 results each by shuffles, and thread h0 does the add/subs k = 4 h0 + m, m = 0 .. 3 (outputs k, k + 8).
     // Every operation is the one dft<16> does on the same operands: the results are bit-identical to the tile kernels'.
-    // On the object side (g_new, ghat, the mix, the support) a thread therefore owns the elements r = 8 h0 + e, on
-    // the spectrum side of the inverse the elements r = 2 e + h0; the forward transform regroups by parity first.
+    // On the object side (g_new, ghat, the mix, the support) a thread therefore owns the elements
+    // r(e) = 4 h0 + (e & 3) + 8 (e >> 2), on the spectrum side of the inverse the elements r = 2 e + h0; the forward
+    // transform regroups by parity first (4 more exchanges).
     constexpr int SPLIT = R0 == 16 ? 2 : 1;
     constexpr int QN = NT / NP, B0 = SPLIT == 2 ? 1 : NP * M0 / NT, E0 = SPLIT == 2 ? R0 / 2 : B0 * R0;
     static_assert((SPLIT == 2 ? 2 * NP * M0 == NT : B0 * NT == NP * M0) && E0 == 8 && NP * (N / R1) == NT && RL == 8,
@@ -117,9 +150,10 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     const int o0 = ppos<N>(q0) * NP + j0;
     const int o1e = ((q / 8) * 64 + (q % 8)) * NP + j, o1o = ((q / 8) * 64 + ((q % 8) ^ 1)) * NP + j;
     const int oLe = (8 * q + (q & 1)) * NP + j, oLo = (8 * q + 1 - (q & 1)) * NP + j;
-    // object side: position and quad of first-stage element e (SPLIT == 2: r = 8 h0 + e)
-    auto p0 = [&](int e) -> int { return SPLIT == 2 ? q0 + M0 * (E0 * h0 + e) : q + QN * (e / R0) + M0 * (e % R0); };
-    auto i0 = [&](int e) -> int { return SPLIT == 2 ? o0 + (E0 * h0 + e) * (M0 * NP) : o0 + (e / R0) * (QN * NP) + (e % R0) * (M0 * NP); };
+    // object side: position and quad of first-stage element e (SPLIT == 2: r = 4 h0 + (e & 3) + 8 (e >> 2))
+    auto r0s = [&](int e) -> int { return 4 * h0 + (e & 3) + 8 * (e >> 2); };
+    auto p0 = [&](int e) -> int { return SPLIT == 2 ? q0 + M0 * r0s(e) : q + QN * (e / R0) + M0 * (e % R0); };
+    auto i0 = [&](int e) -> int { return SPLIT == 2 ? o0 + r0s(e) * (M0 * NP) : o0 + (e / R0) * (QN * NP) + (e % R0) * (M0 * NP); };
     // spectrum side of the inverse first stage: where its inputs are read (SPLIT == 2: r = 2 e + h0)
     auto iS = [&](int e) -> int { return SPLIT == 2 ? o0 + (2 * e + h0) * (M0 * NP) : i0(e); };
     auto i1 = [&](int r) -> int { return ((r & 1) ? o1o : o1e) + r * (8 * NP); };
@@ -151,20 +185,22 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     };
     auto stage0_fwd = [&](c2 (&a)[E0]) {
         if constexpr (SPLIT == 2) {
-            // a[e] = element r = 8 h0 + e; the radix-8 DFT of parity h0 needs r = 2 e' + h0: half of them are the partner's
+            // a[e] = element r(e); the radix-8 DFT of parity h0 needs r = 2 e' + h0: half of them are the partner's.
+            // h0 = 0 owns r = 0 1 2 3 8 9 10 11 and sends the odd ones, h0 = 1 owns 4 5 6 7 12 13 14 15 and sends the even ones
             c2 n[E0];
 #pragma unroll
             for (int i = 0; i < E0 / 2; ++i) {
                 const c2 recv = walk_xchg(walk_sel(h0, a[2 * i], a[2 * i + 1]));
-                n[i] = walk_sel(h0, recv, a[2 * i]);
-                n[E0 / 2 + i] = walk_sel(h0, a[2 * i + 1], recv);
+                const int lo_i = 4 * (i / 2) + (i % 2);   // r = 2 e' + h0 < 4 + 8 (i / 2): h0 = 0 has it, h0 = 1 receives it
+                n[lo_i] = walk_sel(h0, recv, a[2 * i]);
+                n[lo_i + 2] = walk_sel(h0, a[2 * i + 1], recv);
             }
             dft<E0, false>(n);
             walk_combine<false>(n, h0);
-            const float2* __restrict__ t = tw0 + q0 * (R0 - 1);   // output r = 8 h0 + m, times w_r (r >= 1)
+            const float2* __restrict__ t = tw0 + q0 * (R0 - 1);   // output r(m), times w_r (r >= 1)
 #pragma unroll
             for (int m = 0; m < E0; ++m) {
-                const float2 w = t[m == 0 ? (E0 - 1) * h0 : E0 * h0 + m - 1];
+                const float2 w = t[m == 0 ? 3 * h0 : r0s(m) - 1];
                 const c2 x = cmul(n[m], bc(w.x), bc(w.y));
                 a[m] = m == 0 ? walk_sel(h0, x, n[m]) : x;
             }
