@@ -117,6 +117,22 @@ struct GenSmem {
     }
 };
 
+// The W x N elements of a row tile are handed out in chunks of 32 consecutive x of one line: a warp takes chunks
+// wid, wid + nw, ... (coalesced; every warp has work whatever W is).  GEN_U chunks are in flight per warp at a time:
+// all their global loads are issued before the first value is used.
+constexpr int GEN_U = 4;
+struct GenChunks {
+    int cpl, total;   // chunks per line, chunks per tile
+    __device__ __forceinline__ GenChunks(int N, int W) : cpl((N + 31) >> 5), total(((N + 31) >> 5) * W) {}
+};
+__device__ __forceinline__ void gen_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void gen_cp_async8(void* smem_dst, const void* gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void gen_cp_async_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // Eq. (4) at pixel (y, x) of projection n on natural arrays, with the mirrored wrap of cpra_set_seam
 __device__ __forceinline__ float2 gen_mix(const float2* __restrict__ g, const GenGeo& gg, const MixParams& mp, int n, int y, int x, bool fires)
 {
@@ -149,18 +165,66 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
               MixParams mp, GenGeo gg, int n0, int fires, int mask_mode, float2* __restrict__ ghat_out)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
-    const int N = gg.N, W = gg.W, Wp = gen_wp(W);
+    const int N = gg.N, W = gg.W, Wp = gen_wp(W), Np = gg.Np;
     GenSmem s(smraw, N, W);
     const int tiles = (N + W - 1) / W;
     const int n = n0 + (int)(blockIdx.x / tiles), y0 = (int)(blockIdx.x % tiles) * W;
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
-    // a warp takes whole lines (x over the lanes: coalesced); unrolled so that several loads are in flight per thread
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int w = wid; w < W; w += nw) {
-        const int y = y0 + w;
-#pragma unroll 8
-        for (int x = lane; x < N; x += 32) {
+    const GenChunks ch(N, W);
+    const size_t tbase = (size_t)n * px + (size_t)y0 * N;       // element (w, x) of the tile at tbase + w N + x
+    const bool mixes = fires != 0 && !(mp.K == 0 && mp.a[0] == 1.0f);
+    if (!mixes && !mask_mode && !ghat_out) {
+        // a plain copy: asynchronous, every element of the tile in flight at once
+        for (int c = wid; c < ch.total; c += nw) {
+            const int w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            if (x >= N) continue;
+            if (y0 + w < N) gen_cp_async8(s.a + x * Wp + w, cur + tbase + (size_t)w * N + x);
+            else s.a[x * Wp + w] = make_float2(0.f, 0.f);
+        }
+        gen_cp_async_wait();
+    } else if (mixes && mp.K == 1) {
+        // Eq. (4) with the default coupling: own + the two neighbours, the loads of GEN_U chunks issued before any is used
+        int mm = n - 1, mp1 = n + 1;
+        const bool wm = mm < 0, wp = mp1 >= Np;
+        if (wm) mm += Np;
+        if (wp) mp1 -= Np;
+        const bool fm = wm && mp.flip_seam, fp = wp && mp.flip_seam;
+        const float2* __restrict__ gm = cur + (size_t)mm * px + (size_t)y0 * N;
+        const float2* __restrict__ gq = cur + (size_t)mp1 * px + (size_t)y0 * N;
+        for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
+            float2 o[GEN_U], a[GEN_U], b[GEN_U];
+#pragma unroll
+            for (int u = 0; u < GEN_U; ++u) {
+                const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+                o[u] = a[u] = b[u] = make_float2(0.f, 0.f);
+                if (c < ch.total && x < N && y0 + w < N) {
+                    const int xm = N - x == N ? 0 : N - x;
+                    o[u] = cur[tbase + (size_t)w * N + x];
+                    a[u] = gm[(size_t)w * N + (fm ? xm : x)];
+                    b[u] = gq[(size_t)w * N + (fp ? xm : x)];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < GEN_U; ++u) {
+                const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+                if (c >= ch.total || x >= N) continue;
+                float2 v = make_float2(0.f, 0.f);
+                if (y0 + w < N) {
+                    const float sx = (0.f + a[u].x) + b[u].x, sy = (0.f + a[u].y) + b[u].y;
+                    v = make_float2(fmaf(mp.a[1], sx, mp.a[0] * o[u].x), fmaf(mp.a[1], sy, mp.a[0] * o[u].y));
+                    const size_t g = tbase + (size_t)w * N + x;
+                    if (mask_mode && !S[g]) v = make_float2(0.f, 0.f);
+                    if (ghat_out) ghat_out[g] = v;
+                }
+                s.a[x * Wp + w] = v;
+            }
+        }
+    } else {
+        for (int c = wid; c < ch.total; c += nw) {
+            const int w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane, y = y0 + w;
+            if (x >= N) continue;
             float2 v = make_float2(0.f, 0.f);
             if (y < N) {
                 v = gen_mix(cur, gg, mp, n, y, x, fires != 0);
@@ -172,11 +236,18 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
     }
     __syncthreads();
     const float2* r = gen_fft(s.a, s.b, s.tw, gg, false);
-    for (int w = wid; w < W; w += nw) {
-        const int y = y0 + w;
-        if (y >= N) continue;
-#pragma unroll 8
-        for (int x = lane; x < N; x += 32) scr[(size_t)n * px + (size_t)y * N + x] = r[x * Wp + w];
+    for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
+        float2 v[GEN_U];
+#pragma unroll
+        for (int u = 0; u < GEN_U; ++u) {
+            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            if (c < ch.total && x < N && y0 + w < N) v[u] = r[x * Wp + w];
+        }
+#pragma unroll
+        for (int u = 0; u < GEN_U; ++u) {
+            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            if (c < ch.total && x < N && y0 + w < N) scr[tbase + (size_t)w * N + x] = v[u];
+        }
     }
 }
 
@@ -214,27 +285,36 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     if (mode != 2) { r = gen_fft(s.a, s.b, s.tw, gg, false); other = (r == s.a) ? s.b : s.a; }
     if (mode == 0) {
         double acc = 0.0;
-#pragma unroll 8
-        for (int ky = r0; ky < N; ky += rstep) {
-            const int w = cw, x = cx;
-            if (x >= N) continue;
-            float2 G = r[ky * Wp + w];
-            const float a = __ldg(A + (size_t)n * px + (size_t)ky * N + x);
-            float f = scale;
-            if (a >= 0.f) {
-                const float m2 = G.x * G.x + G.y * G.y;
-                if (m2 >= 1.17549435e-38f) {
-                    const float mag = sqrtf(m2);
-                    const float d = mag - a;
-                    acc += (double)d * (double)d;
-                    f = a / mag * scale;
-                } else {
-                    acc += (double)a * (double)a;
-                    G = make_float2(1.f, 0.f);
-                    f = a * scale;
-                }
+        constexpr int UA = 8;   // sqrt(I) of UA rows requested before the first is used
+        for (int kb = r0; kb < N && cx < N; kb += UA * rstep) {
+            float av[UA];
+#pragma unroll
+            for (int u = 0; u < UA; ++u) {
+                const int ky = kb + u * rstep;
+                av[u] = ky < N ? __ldg(A + (size_t)n * px + (size_t)ky * N + cx) : -1.f;
             }
-            r[ky * Wp + w] = make_float2(G.x * f, G.y * f);
+#pragma unroll
+            for (int u = 0; u < UA; ++u) {
+                const int ky = kb + u * rstep;
+                if (ky >= N) break;
+                float2 G = r[ky * Wp + cw];
+                const float a = av[u];
+                float f = scale;
+                if (a >= 0.f) {
+                    const float m2 = G.x * G.x + G.y * G.y;
+                    if (m2 >= 1.17549435e-38f) {
+                        const float mag = sqrtf(m2);
+                        const float d = mag - a;
+                        acc += (double)d * (double)d;
+                        f = a / mag * scale;
+                    } else {
+                        acc += (double)a * (double)a;
+                        G = make_float2(1.f, 0.f);
+                        f = a * scale;
+                    }
+                }
+                r[ky * Wp + cw] = make_float2(G.x * f, G.y * f);
+            }
         }
         // fixed-order block reduction of the error numerator
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -268,28 +348,53 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int w = wid; w < W; w += nw) {
-        const int y = y0 + w;
-#pragma unroll 8
-        for (int x = lane; x < N; x += 32)
-            s.a[x * Wp + w] = y < N ? __ldg(scr + (size_t)n * px + (size_t)y * N + x) : make_float2(0.f, 0.f);
+    const GenChunks ch(N, W);
+    const size_t tbase = (size_t)n * px + (size_t)y0 * N;       // element (w, x) of the tile at tbase + w N + x
+    // the spectrum rows arrive by asynchronous copies, all in flight at once
+    for (int c = wid; c < ch.total; c += nw) {
+        const int w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+        if (x >= N) continue;
+        if (y0 + w < N) gen_cp_async8(s.a + x * Wp + w, scr + tbase + (size_t)w * N + x);
+        else s.a[x * Wp + w] = make_float2(0.f, 0.f);
     }
+    if (hio) {
+        // what the update will read after the transform (support bytes, stored ghat) is requested into L2 meanwhile
+        const int rows = min(W, N - y0), el = rows * N;
+        for (int i = threadIdx.x * 128; i < el; i += blockDim.x * 128) gen_prefetch_l2(S + tbase + i);
+        if (ghat) for (int i = threadIdx.x * 16; i < el; i += blockDim.x * 16) gen_prefetch_l2(ghat + tbase + i);
+    }
+    gen_cp_async_wait();
     __syncthreads();
     const float2* r = gen_fft(s.a, s.b, s.tw, gg, true);
-    for (int w = wid; w < W; w += nw) {
-      const int y = y0 + w;
-      if (y >= N) continue;
-#pragma unroll 8
-      for (int x = lane; x < N; x += 32) {
-        const size_t o = (size_t)n * px + (size_t)y * N + x;
-        float2 gp = r[x * Wp + w];
-        gp.x *= scale; gp.y *= scale;
-        if (hio && (!S[o] || (mp.positivity && gp.x < 0.f))) {
-            const float2 gh = ghat ? ghat[o] : gen_mix(cur, gg, mp, n, y, x, fires != 0);
-            gp = make_float2(fmaf(mp.c_gp, gp.x, mp.c_ghat * gh.x), fmaf(mp.c_gp, gp.y, mp.c_ghat * gh.y));
+    for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
+        float2 gp[GEN_U], gh[GEN_U];
+        unsigned char sv[GEN_U];
+#pragma unroll
+        for (int u = 0; u < GEN_U; ++u) {
+            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            gh[u] = make_float2(0.f, 0.f);
+            sv[u] = 1;
+            if (c < ch.total && x < N && y0 + w < N) {
+                const size_t o = tbase + (size_t)w * N + x;
+                gp[u] = r[x * Wp + w];
+                if (hio) {
+                    sv[u] = S[o];
+                    if (ghat) gh[u] = ghat[o];
+                }
+            }
         }
-        nxt[o] = gp;
-      }
+#pragma unroll
+        for (int u = 0; u < GEN_U; ++u) {
+            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            if (c >= ch.total || x >= N || y0 + w >= N) continue;
+            const size_t o = tbase + (size_t)w * N + x;
+            float2 g = make_float2(gp[u].x * scale, gp[u].y * scale);
+            if (hio && (!sv[u] || (mp.positivity && g.x < 0.f))) {
+                const float2 h = ghat ? gh[u] : gen_mix(cur, gg, mp, n, y0 + w, x, fires != 0);
+                g = make_float2(fmaf(mp.c_gp, g.x, mp.c_ghat * h.x), fmaf(mp.c_gp, g.y, mp.c_ghat * h.y));
+            }
+            nxt[o] = g;
+        }
     }
 }
 
