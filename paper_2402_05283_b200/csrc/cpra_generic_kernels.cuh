@@ -22,6 +22,13 @@ __device__ __forceinline__ void gen_small_dft(c2 (&v)[R], const float2* __restri
         // odd prime R: X[p], X[R-p] = t -+ i u (forward) with t = v0 + sum_q cos(2 pi p q / R) (v_q + v_{R-q}),
         // u = sum_q sin(2 pi p q / R) (v_q - v_{R-q}), q = 1 .. (R-1)/2: real coefficients only
         constexpr int H = (R - 1) / 2;
+        float2 cs[H], sn[H];          // cos, sin of 2 pi k / R, k = 1 .. H (the other roots by symmetry)
+#pragma unroll
+        for (int k = 1; k <= H; ++k) {
+            const float2 w = tw[k * rstep];
+            cs[k - 1] = bc(w.x);
+            sn[k - 1] = bc(-w.y);
+        }
         c2 A[H], B[H];
         c2 sum = v[0];
 #pragma unroll
@@ -37,10 +44,11 @@ __device__ __forceinline__ void gen_small_dft(c2 (&v)[R], const float2* __restri
             c2 t = v0, u{make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
             for (int q = 1; q <= H; ++q) {
-                const float2 w = tw[((p * q) % R) * rstep];          // (cos, -sin) of 2 pi p q / R
-                const float2 c = bc(w.x), sn = bc(-w.y);
+                // cos, sin of 2 pi (p q mod R) / R: k > H is the mirror of R - k (same cosine, opposite sine)
+                const int k = (p * q) % R, km = k <= H ? k : R - k;
+                const float2 c = cs[km - 1], sg = k <= H ? sn[km - 1] : neg2(sn[km - 1]);
                 t = c2{pfma(c, A[q - 1].re, t.re), pfma(c, A[q - 1].im, t.im)};
-                u = c2{pfma(sn, B[q - 1].re, u.re), pfma(sn, B[q - 1].im, u.im)};
+                u = c2{pfma(sg, B[q - 1].re, u.re), pfma(sg, B[q - 1].im, u.im)};
             }
             // -i u = (u.im, -u.re)
             const c2 lo{padd(t.re, u.im), psub(t.im, u.re)};     // t - i u
@@ -123,7 +131,10 @@ struct GenSmem {
 constexpr int GEN_U = 4;
 struct GenChunks {
     int cpl, total;   // chunks per line, chunks per tile
-    __device__ __forceinline__ GenChunks(int N, int W) : cpl((N + 31) >> 5), total(((N + 31) >> 5) * W) {}
+    float inv;
+    __device__ __forceinline__ GenChunks(int N, int W) : cpl((N + 31) >> 5), total(((N + 31) >> 5) * W), inv(1.0f / (float)((N + 31) >> 5)) {}
+    // line of chunk c = c / cpl by reciprocal: (c + 0.5) / cpl is never within rounding of an integer (c < 2^15)
+    __device__ __forceinline__ int line(int c) const { return (int)(((float)c + 0.5f) * inv); }
 };
 __device__ __forceinline__ void gen_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void gen_cp_async8(void* smem_dst, const void* gsrc)
@@ -178,7 +189,7 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
     if (!mixes && !mask_mode && !ghat_out) {
         // a plain copy: asynchronous, every element of the tile in flight at once
         for (int c = wid; c < ch.total; c += nw) {
-            const int w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
             if (x >= N) continue;
             if (y0 + w < N) gen_cp_async8(s.a + x * Wp + w, cur + tbase + (size_t)w * N + x);
             else s.a[x * Wp + w] = make_float2(0.f, 0.f);
@@ -197,7 +208,7 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
             float2 o[GEN_U], a[GEN_U], b[GEN_U];
 #pragma unroll
             for (int u = 0; u < GEN_U; ++u) {
-                const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+                const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
                 o[u] = a[u] = b[u] = make_float2(0.f, 0.f);
                 if (c < ch.total && x < N && y0 + w < N) {
                     const int xm = N - x == N ? 0 : N - x;
@@ -208,7 +219,7 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
             }
 #pragma unroll
             for (int u = 0; u < GEN_U; ++u) {
-                const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+                const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
                 if (c >= ch.total || x >= N) continue;
                 float2 v = make_float2(0.f, 0.f);
                 if (y0 + w < N) {
@@ -223,7 +234,7 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
         }
     } else {
         for (int c = wid; c < ch.total; c += nw) {
-            const int w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane, y = y0 + w;
+            const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane, y = y0 + w;
             if (x >= N) continue;
             float2 v = make_float2(0.f, 0.f);
             if (y < N) {
@@ -240,12 +251,12 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
         float2 v[GEN_U];
 #pragma unroll
         for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
             if (c < ch.total && x < N && y0 + w < N) v[u] = r[x * Wp + w];
         }
 #pragma unroll
         for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
             if (c < ch.total && x < N && y0 + w < N) scr[tbase + (size_t)w * N + x] = v[u];
         }
     }
@@ -352,7 +363,7 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     const size_t tbase = (size_t)n * px + (size_t)y0 * N;       // element (w, x) of the tile at tbase + w N + x
     // the spectrum rows arrive by asynchronous copies, all in flight at once
     for (int c = wid; c < ch.total; c += nw) {
-        const int w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+        const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
         if (x >= N) continue;
         if (y0 + w < N) gen_cp_async8(s.a + x * Wp + w, scr + tbase + (size_t)w * N + x);
         else s.a[x * Wp + w] = make_float2(0.f, 0.f);
@@ -371,7 +382,7 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
         unsigned char sv[GEN_U];
 #pragma unroll
         for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
             gh[u] = make_float2(0.f, 0.f);
             sv[u] = 1;
             if (c < ch.total && x < N && y0 + w < N) {
@@ -385,7 +396,7 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
         }
 #pragma unroll
         for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = c / ch.cpl, x = (c - w * ch.cpl) * 32 + lane;
+            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
             if (c >= ch.total || x >= N || y0 + w >= N) continue;
             const size_t o = tbase + (size_t)w * N + x;
             float2 g = make_float2(gp[u].x * scale, gp[u].y * scale);
