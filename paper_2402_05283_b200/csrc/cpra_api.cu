@@ -102,7 +102,7 @@ int cpra_plan(cpra_plan_t* out, int N, int Np, unsigned flags, void* cuda_stream
     p->generic = generic;
     int R0 = 1, R1 = 1, R2 = 1, RL = 1, TBN = 16;
     if (!generic) { auto f = [&]() -> int { CPRA_DISPATCH_N(N, R0 = Radix<NN>::R0; R1 = Radix<NN>::R1; R2 = Radix<NN>::R2; RL = last_radix<NN>(); TBN = tile_batch<NN>()); return 0; }; f(); }
-    p->geo = Geo{N, Np, R0, R1, R2, RL, generic ? (N <= 256 ? 16 : (N <= 512 ? 8 : 4)) : TBN};   // (generic: TB = lines per tile, for the error partials only)
+    p->geo = Geo{N, Np, R0, R1, R2, RL, generic ? gen_lines_per_tile(N) : TBN};   // (generic: TB = lines per tile, for the error partials only)
     // reading A2: the paper's example weights
     if (Np >= 3) { p->K = 1; p->alpha[0] = 0.6f; p->alpha[1] = 0.2f; }
     else { p->K = 0; p->alpha[0] = 1.0f; }

@@ -12,10 +12,11 @@ bool gen_supported(int N)
     return n == 1;
 }
 
-// stages: 8s, then 4 / 2, then 3s, 5s, 7s; W = lines per tile; tw[m] = e^{-2 pi i m / N}
+// stages: 8s, then 4 / 2, then 3s, 5s, 7s (an odd radix last: the stage with contiguous positions is then free of
+// bank conflicts); W = lines per tile; tw[m] = e^{-2 pi i m / N}
 void gen_make_geo(int N, int Np, GenGeo& g, std::vector<float2>& tw)
 {
-    g.N = N; g.Np = Np; g.W = N <= 256 ? 16 : (N <= 512 ? 8 : 4); g.nf = 0;   // lines per tile: 3-4 CTAs of 256 threads per SM
+    g.N = N; g.Np = Np; g.W = gen_lines_per_tile(N); g.nf = 0;
     int n = N;
     while (n % 8 == 0) { g.radix[g.nf++] = 8; n /= 8; }
     if (n % 4 == 0) { g.radix[g.nf++] = 4; n /= 4; }
@@ -73,7 +74,7 @@ int row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, int n0, int nimg, bo
 
 int gen_set_data(cpra_plan_s* p, const float* d_I, const unsigned char* d_mask)
 {
-    k_gen_set_data<<<p->Np, 256, 0, p->stream>>>(d_I, d_mask, p->A, p->den, p->N);
+    k_gen_set_data<<<p->Np, 256, 0, p->stream>>>(d_I, d_mask, p->A, p->den, p->gg);
     return check_launch(p);
 }
 int gen_set_support(cpra_plan_s* p, const unsigned char* d_S)
@@ -144,9 +145,11 @@ int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign)
     if (sign < 0) {
         if ((rc = row_fwd(p, (const float2*)d_in, 0, p->Np, false, false, nullptr))) return rc;
         if ((rc = col(p, 0, p->Np, 1, 1.0f))) return rc;
-        return cudaMemcpyAsync(d_out, p->scr, sizeof(float2) * total, cudaMemcpyDeviceToDevice, p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+        k_gen_permute<<<gblocks(total, 256), 256, 0, p->stream>>>((const float2*)p->scr, (float2*)d_out, p->gg, total, 0);
+        return check_launch(p);
     }
-    if (cudaMemcpyAsync(p->scr, d_in, sizeof(float2) * total, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    k_gen_permute<<<gblocks(total, 256), 256, 0, p->stream>>>((const float2*)d_in, (float2*)p->scr, p->gg, total, 1);
+    if ((rc = check_launch(p))) return rc;
     if ((rc = col(p, 0, p->Np, 2, 1.0f))) return rc;
     if ((rc = row_inv(p, tmp, tmp, 0, p->Np, false, false, 0.f, 1.0f / ((float)p->N * (float)p->N), nullptr))) return rc;
     return cudaMemcpyAsync(d_out, tmp, sizeof(float2) * total, cudaMemcpyDeviceToDevice, p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
@@ -158,7 +161,7 @@ int gen_slices(cpra_plan_s* p, float2* Et)
     int rc = row_fwd(p, (const float2*)p->st[p->cur], 0, p->Np, false, true, nullptr);
     if (rc == CPRA_OK) rc = col(p, 0, p->Np, 1, 1.0f);
     if (rc) return rc;
-    k_gen_transpose<<<gblocks(total, 256), 256, 0, p->stream>>>((const float2*)p->scr, Et, p->N, total);
+    k_gen_transpose<<<gblocks(total, 256), 256, 0, p->stream>>>((const float2*)p->scr, Et, p->gg, total);
     return check_launch(p);
 }
 

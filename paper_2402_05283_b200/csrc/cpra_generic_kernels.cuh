@@ -59,68 +59,90 @@ __device__ __forceinline__ void gen_small_dft(c2 (&v)[R], const float2* __restri
     }
 }
 
-// one Stockham stage of radix R over W lines (W / 2 packed pairs per position): a -> b
+// ---- the tile in shared memory --------------------------------------------------------------------------------
+// float2 index of line w at position x: the W / 2 pairs of a position are XOR-ed with key(x) (see cpra_generic.cuh)
+struct GenTile {
+    int W, W2m, ksh;
+    __device__ __forceinline__ explicit GenTile(int W_) : W(W_), W2m(W_ / 2 - 1), ksh(W_ >= 16 ? 0 : (W_ == 8 ? 1 : 2)) {}
+    __device__ __forceinline__ int pair(int x, int w2) const { return x * W + 2 * (w2 ^ ((x >> ksh) & W2m)); }      // 16-byte aligned
+    __device__ __forceinline__ int line(int x, int w) const { return pair(x, w >> 1) + (w & 1); }
+};
+
+// one in-place stage of radix R on sub-transforms of length L (M = L / R): butterfly (blk, n2) of a pair of lines
+// touches positions blk L + n2 + M q.  Forward: DFT, then output p times w_L^{n2 p}; inverse: input q times the
+// conjugate first.  w_L^{m} = tw[m N / L].
 template <int R, bool INV>
-__device__ __forceinline__ void gen_stage(const float2* __restrict__ a, float2* __restrict__ b, const float2* __restrict__ tw,
-                                          int N, int W, int Ns)
+__device__ __forceinline__ void gen_stage(float2* __restrict__ a, const float2* __restrict__ tw, int N, int W, int L)
 {
-    const int Wp = gen_wp(W), W2 = W / 2, m = N / R, tstep = N / (Ns * R), rstep = N / R;
+    const GenTile t(W);
+    const int W2 = W / 2, M = L / R, ts = N / L, nb = N / R;
     const int w2shift = 31 - __clz(W2);                      // W / 2 is a power of two
-    const float invNs = 1.0f / (float)Ns;                    // j / Ns by reciprocal: (j + 0.5) / Ns is never within rounding of an integer
-    for (int i = threadIdx.x; i < m * W2; i += blockDim.x) {
-        const int w = 2 * (i & (W2 - 1)), j = i >> w2shift;
-        const int jb = (int)(((float)j + 0.5f) * invNs), k = j - jb * Ns;
+    const float invM = 1.0f / (float)M;                      // b / M by reciprocal: (b + 0.5) / M is never within rounding of an integer
+    for (int i = threadIdx.x; i < nb * W2; i += blockDim.x) {
+        const int w2 = i & (W2 - 1), b = i >> w2shift;
+        const int blk = (int)(((float)b + 0.5f) * invM), n2 = b - blk * M;
+        const int base = blk * L + n2;
+        int off[R];
         c2 v[R];
 #pragma unroll
         for (int q = 0; q < R; ++q) {
-            v[q] = gen_ld2(a + (j + q * m) * Wp + w);
-            if (q > 0 && Ns > 1) {
-                const float2 t = tw[q * k * tstep];          // q k tstep < N: no reduction needed
-                v[q] = INV ? cmulc(v[q], bc(t.x), bc(t.y)) : cmul(v[q], bc(t.x), bc(t.y));
+            off[q] = t.pair(base + q * M, w2);
+            v[q] = gen_ld2(a + off[q]);
+            if (INV && q > 0 && M > 1) {
+                const float2 w = tw[q * n2 * ts];             // q n2 < L: the index stays below N
+                v[q] = cmulc(v[q], bc(w.x), bc(w.y));
             }
         }
-        gen_small_dft<R, INV>(v, tw, rstep);
-        const int j0 = jb * Ns * R + k;
+        gen_small_dft<R, INV>(v, tw, N / R);
 #pragma unroll
-        for (int p = 0; p < R; ++p) gen_st2(b + (j0 + p * Ns) * Wp + w, v[p]);
-    }
-}
-
-// W lines of length N in a (element x of line w at x * gen_wp(W) + w), result in the returned buffer;
-// tw[m] = e^{-2 pi i m / N} in shared memory
-template <bool INV>
-__device__ float2* gen_fft_t(float2* a, float2* b, const float2* __restrict__ tw, const GenGeo& g)
-{
-    int Ns = 1;
-    for (int f = 0; f < g.nf; ++f) {
-        const int r = g.radix[f];
-        switch (r) {
-            case 8: gen_stage<8, INV>(a, b, tw, g.N, g.W, Ns); break;
-            case 4: gen_stage<4, INV>(a, b, tw, g.N, g.W, Ns); break;
-            case 2: gen_stage<2, INV>(a, b, tw, g.N, g.W, Ns); break;
-            case 3: gen_stage<3, INV>(a, b, tw, g.N, g.W, Ns); break;
-            case 5: gen_stage<5, INV>(a, b, tw, g.N, g.W, Ns); break;
-            default: gen_stage<7, INV>(a, b, tw, g.N, g.W, Ns); break;
+        for (int q = 0; q < R; ++q) {
+            if (!INV && q > 0 && M > 1) {
+                const float2 w = tw[q * n2 * ts];
+                v[q] = cmul(v[q], bc(w.x), bc(w.y));
+            }
+            gen_st2(a + off[q], v[q]);
         }
-        __syncthreads();
-        float2* t = a; a = b; b = t;
-        Ns *= r;
     }
-    return a;
 }
-__device__ __forceinline__ float2* gen_fft(float2* a, float2* b, const float2* __restrict__ tw, const GenGeo& g, bool inverse)
+template <bool INV>
+__device__ __forceinline__ void gen_stage_any(int r, float2* a, const float2* __restrict__ tw, int N, int W, int L)
 {
-    return inverse ? gen_fft_t<true>(a, b, tw, g) : gen_fft_t<false>(a, b, tw, g);
+    switch (r) {
+        case 8: gen_stage<8, INV>(a, tw, N, W, L); break;
+        case 4: gen_stage<4, INV>(a, tw, N, W, L); break;
+        case 2: gen_stage<2, INV>(a, tw, N, W, L); break;
+        case 3: gen_stage<3, INV>(a, tw, N, W, L); break;
+        case 5: gen_stage<5, INV>(a, tw, N, W, L); break;
+        default: gen_stage<7, INV>(a, tw, N, W, L); break;
+    }
+}
+// W lines of length N in the tile a, in place (a block barrier after every stage); tw[m] = e^{-2 pi i m / N} in shared memory
+__device__ void gen_fft_fwd(float2* a, const float2* __restrict__ tw, const GenGeo& g)
+{
+    int L = g.N;
+    for (int f = 0; f < g.nf; ++f) {
+        gen_stage_any<false>(g.radix[f], a, tw, g.N, g.W, L);
+        __syncthreads();
+        L /= g.radix[f];
+    }
+}
+__device__ void gen_fft_inv(float2* a, const float2* __restrict__ tw, const GenGeo& g)
+{
+    int L = 1;
+    for (int f = g.nf - 1; f >= 0; --f) {
+        L *= g.radix[f];
+        gen_stage_any<true>(g.radix[f], a, tw, g.N, g.W, L);
+        __syncthreads();
+    }
 }
 
 struct GenSmem {
-    float2 *a, *b, *tw;
+    float2 *a, *tw;
     double* red;
     __device__ __forceinline__ GenSmem(unsigned char* sm, int N, int W)
     {
         a = reinterpret_cast<float2*>(sm);
-        b = a + (size_t)N * gen_wp(W);
-        tw = b + (size_t)N * gen_wp(W);
+        tw = a + (size_t)N * W;
         red = reinterpret_cast<double*>(tw + N);
     }
 };
@@ -171,13 +193,14 @@ __device__ __forceinline__ float2 gen_mix(const float2* __restrict__ g, const Ge
 
 // K1: mix + forward FFT along x of W rows; spectrum rows to scr (natural [n][y][kx]).  mask_mode: multiply by the
 // support first (the slices of the assembly); ghat_out: also store the mixed input (for the update of K3).
-__global__ void __launch_bounds__(GEN_NT, 3)
+__global__ void __launch_bounds__(GEN_NT, 4)
 k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const float2* __restrict__ twg, const unsigned char* __restrict__ S,
               MixParams mp, GenGeo gg, int n0, int fires, int mask_mode, float2* __restrict__ ghat_out)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
-    const int N = gg.N, W = gg.W, Wp = gen_wp(W), Np = gg.Np;
+    const int N = gg.N, W = gg.W, Np = gg.Np;
     GenSmem s(smraw, N, W);
+    const GenTile t(W);
     const int tiles = (N + W - 1) / W;
     const int n = n0 + (int)(blockIdx.x / tiles), y0 = (int)(blockIdx.x % tiles) * W;
     const size_t px = (size_t)N * N;
@@ -191,8 +214,8 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
         for (int c = wid; c < ch.total; c += nw) {
             const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
             if (x >= N) continue;
-            if (y0 + w < N) gen_cp_async8(s.a + x * Wp + w, cur + tbase + (size_t)w * N + x);
-            else s.a[x * Wp + w] = make_float2(0.f, 0.f);
+            if (y0 + w < N) gen_cp_async8(s.a + t.line(x, w), cur + tbase + (size_t)w * N + x);
+            else s.a[t.line(x, w)] = make_float2(0.f, 0.f);
         }
         gen_cp_async_wait();
     } else if (mixes && mp.K == 1) {
@@ -229,7 +252,7 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
                     if (mask_mode && !S[g]) v = make_float2(0.f, 0.f);
                     if (ghat_out) ghat_out[g] = v;
                 }
-                s.a[x * Wp + w] = v;
+                s.a[t.line(x, w)] = v;
             }
         }
     } else {
@@ -242,17 +265,19 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
                 if (mask_mode && !S[(size_t)n * px + (size_t)y * N + x]) v = make_float2(0.f, 0.f);
                 if (ghat_out) ghat_out[(size_t)n * px + (size_t)y * N + x] = v;
             }
-            s.a[x * Wp + w] = v;
+            s.a[t.line(x, w)] = v;
         }
     }
     __syncthreads();
-    const float2* r = gen_fft(s.a, s.b, s.tw, gg, false);
+    gen_fft_fwd(s.a, s.tw, gg);
+    // position p of the transform goes to column p of the scratch row (position order, see cpra_generic.cuh)
+    const float2* r = s.a;
     for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
         float2 v[GEN_U];
 #pragma unroll
         for (int u = 0; u < GEN_U; ++u) {
             const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-            if (c < ch.total && x < N && y0 + w < N) v[u] = r[x * Wp + w];
+            if (c < ch.total && x < N && y0 + w < N) v[u] = r[t.line(x, w)];
         }
 #pragma unroll
         for (int u = 0; u < GEN_U; ++u) {
@@ -263,14 +288,17 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
 }
 
 // K2: W columns: forward FFT along y, error metric + Fourier-modulus constraint, inverse FFT along y (unnormalised);
-// mode 0 = all three, 1 = forward only, 2 = inverse only.  A: natural native order, A < 0 = unmeasured.
-__global__ void __launch_bounds__(GEN_NT, 3)
+// mode 0 = all three, 1 = forward only (rows left in position order), 2 = inverse only (rows expected in position
+// order).  The columns of scr are in position order (K1).  A: sqrt(I) in position order on both axes
+// (A[pos(ky)][pos(kx)], k_gen_set_data), A < 0 = unmeasured.
+__global__ void __launch_bounds__(GEN_NT, 4)
 k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* __restrict__ twg, double* __restrict__ partial,
           GenGeo gg, int n0, int mode, float scale)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
-    const int N = gg.N, W = gg.W, Wp = gen_wp(W);
+    const int N = gg.N, W = gg.W;
     GenSmem s(smraw, N, W);
+    const GenTile t(W);
     const int tiles = (N + W - 1) / W;
     const int n = n0 + (int)(blockIdx.x / tiles), tile = (int)(blockIdx.x % tiles), x0 = tile * W;
     const size_t px = (size_t)N * N;
@@ -281,19 +309,18 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     // requested into L2 meanwhile
     if (cx < N) {
         for (int y = r0; y < N; y += rstep) {
-            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + y * Wp + cw);
+            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + t.line(y, cw));
             asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(scr + (size_t)n * px + (size_t)y * N + cx) : "memory");
         }
         if (mode == 0 && (cw & 7) == 0)
             for (int y = r0; y < N; y += rstep) asm volatile("prefetch.global.L2 [%0];" ::"l"(A + (size_t)n * px + (size_t)y * N + cx));
     } else {
-        for (int y = r0; y < N; y += rstep) s.a[y * Wp + cw] = make_float2(0.f, 0.f);
+        for (int y = r0; y < N; y += rstep) s.a[t.line(y, cw)] = make_float2(0.f, 0.f);
     }
     asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();
-    float2* r = s.a;
-    float2* other = s.b;
-    if (mode != 2) { r = gen_fft(s.a, s.b, s.tw, gg, false); other = (r == s.a) ? s.b : s.a; }
+    float2* const r = s.a;
+    if (mode != 2) gen_fft_fwd(s.a, s.tw, gg);
     if (mode == 0) {
         double acc = 0.0;
         constexpr int UA = 8;   // sqrt(I) of UA rows requested before the first is used
@@ -308,7 +335,7 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
             for (int u = 0; u < UA; ++u) {
                 const int ky = kb + u * rstep;
                 if (ky >= N) break;
-                float2 G = r[ky * Wp + cw];
+                float2 G = r[t.line(ky, cw)];
                 const float a = av[u];
                 float f = scale;
                 if (a >= 0.f) {
@@ -324,7 +351,7 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
                         f = a * scale;
                     }
                 }
-                r[ky * Wp + cw] = make_float2(G.x * f, G.y * f);
+                r[t.line(ky, cw)] = make_float2(G.x * f, G.y * f);
             }
         }
         // fixed-order block reduction of the error numerator
@@ -332,28 +359,29 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
         if ((threadIdx.x & 31) == 0) s.red[threadIdx.x >> 5] = acc;
         __syncthreads();
         if (threadIdx.x == 0) {
-            double t = 0.0;
-            for (int w = 0; w < (int)blockDim.x / 32; ++w) t += s.red[w];
-            partial[(size_t)n * tiles + tile] = t;
+            double sum = 0.0;
+            for (int w = 0; w < (int)blockDim.x / 32; ++w) sum += s.red[w];
+            partial[(size_t)n * tiles + tile] = sum;
         }
     }
-    if (mode != 1) r = gen_fft(r, other, s.tw, gg, true);
+    if (mode != 1) gen_fft_inv(s.a, s.tw, gg);
     if (cx < N) {
 #pragma unroll 8
-        for (int y = r0; y < N; y += rstep) scr[(size_t)n * px + (size_t)y * N + cx] = r[y * Wp + cw];
+        for (int y = r0; y < N; y += rstep) scr[(size_t)n * px + (size_t)y * N + cx] = r[t.line(y, cw)];
     }
 }
 
 // K3: inverse FFT along x of W rows (times `scale`) + support / update (cpra_set_update); hio = 0: plain
 // scaled inverse transform.  ghat: the mixed input stored by K1, or NULL = re-mix from the previous state.
-__global__ void __launch_bounds__(GEN_NT, 3)
+__global__ void __launch_bounds__(GEN_NT, 4)
 k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, float2* __restrict__ nxt, const float2* __restrict__ twg,
               const unsigned char* __restrict__ S, MixParams mp, GenGeo gg, int n0, int fires, int hio, float scale,
               const float2* __restrict__ ghat)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
-    const int N = gg.N, W = gg.W, Wp = gen_wp(W);
+    const int N = gg.N, W = gg.W;
     GenSmem s(smraw, N, W);
+    const GenTile t(W);
     const int tiles = (N + W - 1) / W;
     const int n = n0 + (int)(blockIdx.x / tiles), y0 = (int)(blockIdx.x % tiles) * W;
     const size_t px = (size_t)N * N;
@@ -361,12 +389,12 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const GenChunks ch(N, W);
     const size_t tbase = (size_t)n * px + (size_t)y0 * N;       // element (w, x) of the tile at tbase + w N + x
-    // the spectrum rows arrive by asynchronous copies, all in flight at once
+    // the spectrum rows (columns in position order, as K1 stored them) arrive by asynchronous copies, all in flight at once
     for (int c = wid; c < ch.total; c += nw) {
         const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
         if (x >= N) continue;
-        if (y0 + w < N) gen_cp_async8(s.a + x * Wp + w, scr + tbase + (size_t)w * N + x);
-        else s.a[x * Wp + w] = make_float2(0.f, 0.f);
+        if (y0 + w < N) gen_cp_async8(s.a + t.line(x, w), scr + tbase + (size_t)w * N + x);
+        else s.a[t.line(x, w)] = make_float2(0.f, 0.f);
     }
     if (hio) {
         // what the update will read after the transform (support bytes, stored ghat) is requested into L2 meanwhile
@@ -376,7 +404,8 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     }
     gen_cp_async_wait();
     __syncthreads();
-    const float2* r = gen_fft(s.a, s.b, s.tw, gg, true);
+    gen_fft_inv(s.a, s.tw, gg);
+    const float2* r = s.a;
     for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
         float2 gp[GEN_U], gh[GEN_U];
         unsigned char sv[GEN_U];
@@ -387,7 +416,7 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
             sv[u] = 1;
             if (c < ch.total && x < N && y0 + w < N) {
                 const size_t o = tbase + (size_t)w * N + x;
-                gp[u] = r[x * Wp + w];
+                gp[u] = r[t.line(x, w)];
                 if (hio) {
                     sv[u] = S[o];
                     if (ghat) gh[u] = ghat[o];
@@ -409,17 +438,18 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     }
 }
 
-// A0 on natural arrays: A = sqrt(max(I, 0)), mask folded in as A = -1, detector-centred -> native (ifftshift); den_n
-__global__ void k_gen_set_data(const float* __restrict__ I, const unsigned char* __restrict__ mask, float* __restrict__ A, double* __restrict__ den, int N)
+// A0: A = sqrt(max(I, 0)), mask folded in as A = -1, detector-centred -> native (ifftshift) -> position order on both
+// axes (where the transforms of the loop leave frequency (ky, kx)); den_n
+__global__ void k_gen_set_data(const float* __restrict__ I, const unsigned char* __restrict__ mask, float* __restrict__ A, double* __restrict__ den, GenGeo gg)
 {
-    const int n = blockIdx.x, h = N / 2;
+    const int N = gg.N, n = blockIdx.x, h = N / 2;
     double acc = 0.0;
     for (int i = threadIdx.x; i < N * N; i += blockDim.x) {
         const int yc = i / N, xc = i % N;
         const size_t src = (size_t)n * N * N + i;
         const float v = fmaxf(I[src], 0.f);
         const bool m = mask ? (mask[src] != 0) : true;
-        A[(size_t)n * N * N + (size_t)((yc + h) % N) * N + (xc + h) % N] = m ? sqrtf(v) : -1.f;
+        A[(size_t)n * N * N + (size_t)gen_pos((yc + h) % N, gg) * N + gen_pos((xc + h) % N, gg)] = m ? sqrtf(v) : -1.f;
         if (m) acc += (double)v;
     }
     __shared__ double red[32];
@@ -443,14 +473,24 @@ __global__ void k_gen_get(const float2* __restrict__ st, const unsigned char* __
     if (i >= total) return;
     out[i] = (masked && !S[i]) ? make_float2(0.f, 0.f) : st[i];
 }
-// natural spectrum [n][kz][ku] -> [n][ku][kz] (what k_assemble reads)
-__global__ void k_gen_transpose(const float2* __restrict__ in, float2* __restrict__ out, int N, size_t total)
+// spectrum in position order [n][pos(kz)][pos(ku)] -> natural and transposed [n][ku][kz] (what k_assemble reads)
+__global__ void k_gen_transpose(const float2* __restrict__ in, float2* __restrict__ out, GenGeo gg, size_t total)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
-    const int kz = (int)(i % N), ku = (int)((i / N) % N);
+    const int N = gg.N, kz = (int)(i % N), ku = (int)((i / N) % N);
     const size_t n = i / ((size_t)N * N);
-    out[i] = in[(n * N + kz) * N + ku];
+    out[i] = in[(n * N + gen_pos(kz, gg)) * N + gen_pos(ku, gg)];
+}
+// natural [n][ky][kx] <-> position order [n][pos(ky)][pos(kx)]  (to_pos: scatter into position order; else gather from it)
+__global__ void k_gen_permute(const float2* __restrict__ in, float2* __restrict__ out, GenGeo gg, size_t total, int to_pos)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = gg.N, kx = (int)(i % N), ky = (int)((i / N) % N);
+    const size_t n = i / ((size_t)N * N);
+    const size_t j = (n * N + gen_pos(ky, gg)) * N + gen_pos(kx, gg);
+    if (to_pos) out[j] = in[i]; else out[i] = in[j];
 }
 
 }  // namespace cpra
