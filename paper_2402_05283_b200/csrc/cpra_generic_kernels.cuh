@@ -147,17 +147,9 @@ struct GenSmem {
     }
 };
 
-// The W x N elements of a row tile are handed out in chunks of 32 consecutive x of one line: a warp takes chunks
-// wid, wid + nw, ... (coalesced; every warp has work whatever W is).  GEN_U chunks are in flight per warp at a time:
-// all their global loads are issued before the first value is used.
+// Row tiles: a warp takes whole lines (w = warp, warp + nw, ...: W >= the number of warps), the lanes run along x
+// (coalesced), GEN_U steps of 32 at a time: all their global loads are issued before the first value is used.
 constexpr int GEN_U = 4;
-struct GenChunks {
-    int cpl, total;   // chunks per line, chunks per tile
-    float inv;
-    __device__ __forceinline__ GenChunks(int N, int W) : cpl((N + 31) >> 5), total(((N + 31) >> 5) * W), inv(1.0f / (float)((N + 31) >> 5)) {}
-    // line of chunk c = c / cpl by reciprocal: (c + 0.5) / cpl is never within rounding of an integer (c < 2^15)
-    __device__ __forceinline__ int line(int c) const { return (int)(((float)c + 0.5f) * inv); }
-};
 __device__ __forceinline__ void gen_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void gen_cp_async8(void* smem_dst, const void* gsrc)
 {
@@ -191,8 +183,8 @@ __device__ __forceinline__ float2 gen_mix(const float2* __restrict__ g, const Ge
     return acc;
 }
 
-// K1: mix + forward FFT along x of W rows; spectrum rows to scr (natural [n][y][kx]).  mask_mode: multiply by the
-// support first (the slices of the assembly); ghat_out: also store the mixed input (for the update of K3).
+// K1: mix + forward FFT along x of W rows; spectrum rows to scr ([n][y][position], see cpra_generic.cuh).  mask_mode:
+// multiply by the support first (the slices of the assembly); ghat_out: also store the mixed input (for the update of K3).
 __global__ void __launch_bounds__(GEN_NT, 4)
 k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const float2* __restrict__ twg, const unsigned char* __restrict__ S,
               MixParams mp, GenGeo gg, int n0, int fires, int mask_mode, float2* __restrict__ ghat_out)
@@ -206,83 +198,74 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    const GenChunks ch(N, W);
-    const size_t tbase = (size_t)n * px + (size_t)y0 * N;       // element (w, x) of the tile at tbase + w N + x
     const bool mixes = fires != 0 && !(mp.K == 0 && mp.a[0] == 1.0f);
-    if (!mixes && !mask_mode && !ghat_out) {
-        // a plain copy: asynchronous, every element of the tile in flight at once
-        for (int c = wid; c < ch.total; c += nw) {
-            const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-            if (x >= N) continue;
-            if (y0 + w < N) gen_cp_async8(s.a + t.line(x, w), cur + tbase + (size_t)w * N + x);
-            else s.a[t.line(x, w)] = make_float2(0.f, 0.f);
+    int mm = n - 1, mq = n + 1;                                  // the neighbours of the default coupling (K = 1)
+    const bool wm = mm < 0, wq = mq >= Np;
+    if (wm) mm += Np;
+    if (wq) mq -= Np;
+    const bool fm = wm && mp.flip_seam, fq = wq && mp.flip_seam;
+    for (int w = wid; w < W; w += nw) {
+        const int y = y0 + w;
+        if (y >= N) {
+            for (int x = lane; x < N; x += 32) s.a[t.line(x, w)] = make_float2(0.f, 0.f);
+            continue;
         }
-        gen_cp_async_wait();
-    } else if (mixes && mp.K == 1) {
-        // Eq. (4) with the default coupling: own + the two neighbours, the loads of GEN_U chunks issued before any is used
-        int mm = n - 1, mp1 = n + 1;
-        const bool wm = mm < 0, wp = mp1 >= Np;
-        if (wm) mm += Np;
-        if (wp) mp1 -= Np;
-        const bool fm = wm && mp.flip_seam, fp = wp && mp.flip_seam;
-        const float2* __restrict__ gm = cur + (size_t)mm * px + (size_t)y0 * N;
-        const float2* __restrict__ gq = cur + (size_t)mp1 * px + (size_t)y0 * N;
-        for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
-            float2 o[GEN_U], a[GEN_U], b[GEN_U];
+        const size_t row = (size_t)n * px + (size_t)y * N;
+        if (!mixes && !mask_mode && !ghat_out) {
+            // a plain copy: asynchronous, the whole line in flight at once
+            for (int x = lane; x < N; x += 32) gen_cp_async8(s.a + t.line(x, w), cur + row + x);
+        } else if (mixes && mp.K == 1) {
+            // Eq. (4) with the default coupling: own + the two neighbours
+            const float2* __restrict__ go = cur + row;
+            const float2* __restrict__ gm = cur + (size_t)mm * px + (size_t)y * N;
+            const float2* __restrict__ gq = cur + (size_t)mq * px + (size_t)y * N;
+            for (int x0 = lane; x0 < N; x0 += 32 * GEN_U) {
+                float2 o[GEN_U], a[GEN_U], b[GEN_U];
 #pragma unroll
-            for (int u = 0; u < GEN_U; ++u) {
-                const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-                o[u] = a[u] = b[u] = make_float2(0.f, 0.f);
-                if (c < ch.total && x < N && y0 + w < N) {
-                    const int xm = N - x == N ? 0 : N - x;
-                    o[u] = cur[tbase + (size_t)w * N + x];
-                    a[u] = gm[(size_t)w * N + (fm ? xm : x)];
-                    b[u] = gq[(size_t)w * N + (fp ? xm : x)];
+                for (int u = 0; u < GEN_U; ++u) {
+                    const int x = x0 + 32 * u;
+                    if (x < N) {
+                        const int xm = x == 0 ? 0 : N - x;
+                        o[u] = go[x];
+                        a[u] = gm[fm ? xm : x];
+                        b[u] = gq[fq ? xm : x];
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < GEN_U; ++u) {
+                    const int x = x0 + 32 * u;
+                    if (x < N) {
+                        const float sx = (0.f + a[u].x) + b[u].x, sy = (0.f + a[u].y) + b[u].y;
+                        float2 v = make_float2(fmaf(mp.a[1], sx, mp.a[0] * o[u].x), fmaf(mp.a[1], sy, mp.a[0] * o[u].y));
+                        if (mask_mode && !S[row + x]) v = make_float2(0.f, 0.f);
+                        if (ghat_out) ghat_out[row + x] = v;
+                        s.a[t.line(x, w)] = v;
+                    }
                 }
             }
-#pragma unroll
-            for (int u = 0; u < GEN_U; ++u) {
-                const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-                if (c >= ch.total || x >= N) continue;
-                float2 v = make_float2(0.f, 0.f);
-                if (y0 + w < N) {
-                    const float sx = (0.f + a[u].x) + b[u].x, sy = (0.f + a[u].y) + b[u].y;
-                    v = make_float2(fmaf(mp.a[1], sx, mp.a[0] * o[u].x), fmaf(mp.a[1], sy, mp.a[0] * o[u].y));
-                    const size_t g = tbase + (size_t)w * N + x;
-                    if (mask_mode && !S[g]) v = make_float2(0.f, 0.f);
-                    if (ghat_out) ghat_out[g] = v;
-                }
+        } else {
+            for (int x = lane; x < N; x += 32) {
+                float2 v = gen_mix(cur, gg, mp, n, y, x, fires != 0);
+                if (mask_mode && !S[row + x]) v = make_float2(0.f, 0.f);
+                if (ghat_out) ghat_out[row + x] = v;
                 s.a[t.line(x, w)] = v;
             }
         }
-    } else {
-        for (int c = wid; c < ch.total; c += nw) {
-            const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane, y = y0 + w;
-            if (x >= N) continue;
-            float2 v = make_float2(0.f, 0.f);
-            if (y < N) {
-                v = gen_mix(cur, gg, mp, n, y, x, fires != 0);
-                if (mask_mode && !S[(size_t)n * px + (size_t)y * N + x]) v = make_float2(0.f, 0.f);
-                if (ghat_out) ghat_out[(size_t)n * px + (size_t)y * N + x] = v;
-            }
-            s.a[t.line(x, w)] = v;
-        }
     }
+    gen_cp_async_wait();
     __syncthreads();
     gen_fft_fwd(s.a, s.tw, gg);
-    // position p of the transform goes to column p of the scratch row (position order, see cpra_generic.cuh)
-    const float2* r = s.a;
-    for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
-        float2 v[GEN_U];
+    // position p of the transform goes to column p of the scratch row (position order)
+    for (int w = wid; w < W; w += nw) {
+        const int y = y0 + w;
+        if (y >= N) continue;
+        float2* __restrict__ out = scr + (size_t)n * px + (size_t)y * N;
+        for (int x0 = lane; x0 < N; x0 += 32 * GEN_U) {
+            float2 v[GEN_U];
 #pragma unroll
-        for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-            if (c < ch.total && x < N && y0 + w < N) v[u] = r[t.line(x, w)];
-        }
+            for (int u = 0; u < GEN_U; ++u) if (x0 + 32 * u < N) v[u] = s.a[t.line(x0 + 32 * u, w)];
 #pragma unroll
-        for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-            if (c < ch.total && x < N && y0 + w < N) scr[tbase + (size_t)w * N + x] = v[u];
+            for (int u = 0; u < GEN_U; ++u) if (x0 + 32 * u < N) out[x0 + 32 * u] = v[u];
         }
     }
 }
@@ -387,14 +370,15 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    const GenChunks ch(N, W);
     const size_t tbase = (size_t)n * px + (size_t)y0 * N;       // element (w, x) of the tile at tbase + w N + x
     // the spectrum rows (columns in position order, as K1 stored them) arrive by asynchronous copies, all in flight at once
-    for (int c = wid; c < ch.total; c += nw) {
-        const int w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-        if (x >= N) continue;
-        if (y0 + w < N) gen_cp_async8(s.a + t.line(x, w), scr + tbase + (size_t)w * N + x);
-        else s.a[t.line(x, w)] = make_float2(0.f, 0.f);
+    for (int w = wid; w < W; w += nw) {
+        if (y0 + w < N) {
+            const float2* __restrict__ in = scr + tbase + (size_t)w * N;
+            for (int x = lane; x < N; x += 32) gen_cp_async8(s.a + t.line(x, w), in + x);
+        } else {
+            for (int x = lane; x < N; x += 32) s.a[t.line(x, w)] = make_float2(0.f, 0.f);
+        }
     }
     if (hio) {
         // what the update will read after the transform (support bytes, stored ghat) is requested into L2 meanwhile
@@ -405,35 +389,37 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     gen_cp_async_wait();
     __syncthreads();
     gen_fft_inv(s.a, s.tw, gg);
-    const float2* r = s.a;
-    for (int c0 = wid; c0 < ch.total; c0 += nw * GEN_U) {
-        float2 gp[GEN_U], gh[GEN_U];
-        unsigned char sv[GEN_U];
+    for (int w = wid; w < W; w += nw) {
+        const int y = y0 + w;
+        if (y >= N) continue;
+        const size_t row = tbase + (size_t)w * N;
+        for (int x0 = lane; x0 < N; x0 += 32 * GEN_U) {
+            float2 gp[GEN_U], gh[GEN_U];
+            unsigned char sv[GEN_U];
 #pragma unroll
-        for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-            gh[u] = make_float2(0.f, 0.f);
-            sv[u] = 1;
-            if (c < ch.total && x < N && y0 + w < N) {
-                const size_t o = tbase + (size_t)w * N + x;
-                gp[u] = r[t.line(x, w)];
-                if (hio) {
-                    sv[u] = S[o];
-                    if (ghat) gh[u] = ghat[o];
+            for (int u = 0; u < GEN_U; ++u) {
+                const int x = x0 + 32 * u;
+                gh[u] = make_float2(0.f, 0.f);
+                sv[u] = 1;
+                if (x < N) {
+                    gp[u] = s.a[t.line(x, w)];
+                    if (hio) {
+                        sv[u] = S[row + x];
+                        if (ghat) gh[u] = ghat[row + x];
+                    }
                 }
             }
-        }
 #pragma unroll
-        for (int u = 0; u < GEN_U; ++u) {
-            const int c = c0 + u * nw, w = ch.line(c), x = (c - w * ch.cpl) * 32 + lane;
-            if (c >= ch.total || x >= N || y0 + w >= N) continue;
-            const size_t o = tbase + (size_t)w * N + x;
-            float2 g = make_float2(gp[u].x * scale, gp[u].y * scale);
-            if (hio && (!sv[u] || (mp.positivity && g.x < 0.f))) {
-                const float2 h = ghat ? gh[u] : gen_mix(cur, gg, mp, n, y0 + w, x, fires != 0);
-                g = make_float2(fmaf(mp.c_gp, g.x, mp.c_ghat * h.x), fmaf(mp.c_gp, g.y, mp.c_ghat * h.y));
+            for (int u = 0; u < GEN_U; ++u) {
+                const int x = x0 + 32 * u;
+                if (x >= N) continue;
+                float2 g = make_float2(gp[u].x * scale, gp[u].y * scale);
+                if (hio && (!sv[u] || (mp.positivity && g.x < 0.f))) {
+                    const float2 h = ghat ? gh[u] : gen_mix(cur, gg, mp, n, y, x, fires != 0);
+                    g = make_float2(fmaf(mp.c_gp, g.x, mp.c_ghat * h.x), fmaf(mp.c_gp, g.y, mp.c_ghat * h.y));
+                }
+                nxt[row + x] = g;
             }
-            nxt[o] = g;
         }
     }
 }
