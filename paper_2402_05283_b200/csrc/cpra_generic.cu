@@ -22,6 +22,10 @@ void gen_make_geo(int N, int Np, GenGeo& g, std::vector<float2>& tw)
     if (n % 4 == 0) { g.radix[g.nf++] = 4; n /= 4; }
     if (n % 2 == 0) { g.radix[g.nf++] = 2; n /= 2; }
     for (int f : {3, 5, 7}) while (n % f == 0) { g.radix[g.nf++] = f; n /= f; }
+    for (int s = 0, L = N; s < g.nf; ++s) {
+        g.L[s] = L; g.M[s] = L / g.radix[s]; g.ts[s] = N / L; g.nb[s] = N / g.radix[s]; g.invM[s] = 1.0f / (float)g.M[s];
+        L /= g.radix[s];
+    }
     const double PI = 3.14159265358979323846264338327950288;
     tw.assign(1024, make_float2(0.f, 0.f));
     for (int m = 0; m < N; ++m) {

@@ -26,6 +26,10 @@ constexpr int GEN_MAXF = 12;
 struct GenGeo {
     int N, Np, W, nf;          // image size, projections, lines per tile, number of stages
     int radix[GEN_MAXF];
+    // per stage s (sub-transform length L_s = N / (r_0 ... r_{s-1})), filled by gen_make_geo so that no thread divides:
+    int L[GEN_MAXF], M[GEN_MAXF], ts[GEN_MAXF];   // L_s, M_s = L_s / r_s, twiddle step N / L_s
+    int nb[GEN_MAXF];                              // butterflies per line N / r_s (= the table step of the r_s-th roots of unity)
+    float invM[GEN_MAXF];                          // 1 / M_s
 };
 constexpr int GEN_NT = 256;
 // lines per tile: as many as leave four CTAs per SM their shared memory (N W 8 bytes each + the table)

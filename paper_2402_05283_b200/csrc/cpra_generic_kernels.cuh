@@ -72,12 +72,12 @@ struct GenTile {
 // touches positions blk L + n2 + M q.  Forward: DFT, then output p times w_L^{n2 p}; inverse: input q times the
 // conjugate first.  w_L^{m} = tw[m N / L].
 template <int R, bool INV>
-__device__ __forceinline__ void gen_stage(float2* __restrict__ a, const float2* __restrict__ tw, int N, int W, int L)
+__device__ __forceinline__ void gen_stage(float2* __restrict__ a, const float2* __restrict__ tw, const GenGeo& g, int st)
 {
+    const int W = g.W, L = g.L[st], M = g.M[st], ts = g.ts[st], nb = g.nb[st];
     const GenTile t(W);
-    const int W2 = W / 2, M = L / R, ts = N / L, nb = N / R;
-    const int w2shift = 31 - __clz(W2);                      // W / 2 is a power of two
-    const float invM = 1.0f / (float)M;                      // b / M by reciprocal: (b + 0.5) / M is never within rounding of an integer
+    const int W2 = W / 2, w2shift = 31 - __clz(W2);          // W / 2 is a power of two
+    const float invM = g.invM[st];                           // b / M by reciprocal: (b + 0.5) / M is never within rounding of an integer
     for (int i = threadIdx.x; i < nb * W2; i += blockDim.x) {
         const int w2 = i & (W2 - 1), b = i >> w2shift;
         const int blk = (int)(((float)b + 0.5f) * invM), n2 = b - blk * M;
@@ -93,7 +93,7 @@ __device__ __forceinline__ void gen_stage(float2* __restrict__ a, const float2* 
                 v[q] = cmulc(v[q], bc(w.x), bc(w.y));
             }
         }
-        gen_small_dft<R, INV>(v, tw, N / R);
+        gen_small_dft<R, INV>(v, tw, nb);
 #pragma unroll
         for (int q = 0; q < R; ++q) {
             if (!INV && q > 0 && M > 1) {
@@ -105,33 +105,29 @@ __device__ __forceinline__ void gen_stage(float2* __restrict__ a, const float2* 
     }
 }
 template <bool INV>
-__device__ __forceinline__ void gen_stage_any(int r, float2* a, const float2* __restrict__ tw, int N, int W, int L)
+__device__ __forceinline__ void gen_stage_any(float2* a, const float2* __restrict__ tw, const GenGeo& g, int st)
 {
-    switch (r) {
-        case 8: gen_stage<8, INV>(a, tw, N, W, L); break;
-        case 4: gen_stage<4, INV>(a, tw, N, W, L); break;
-        case 2: gen_stage<2, INV>(a, tw, N, W, L); break;
-        case 3: gen_stage<3, INV>(a, tw, N, W, L); break;
-        case 5: gen_stage<5, INV>(a, tw, N, W, L); break;
-        default: gen_stage<7, INV>(a, tw, N, W, L); break;
+    switch (g.radix[st]) {
+        case 8: gen_stage<8, INV>(a, tw, g, st); break;
+        case 4: gen_stage<4, INV>(a, tw, g, st); break;
+        case 2: gen_stage<2, INV>(a, tw, g, st); break;
+        case 3: gen_stage<3, INV>(a, tw, g, st); break;
+        case 5: gen_stage<5, INV>(a, tw, g, st); break;
+        default: gen_stage<7, INV>(a, tw, g, st); break;
     }
 }
 // W lines of length N in the tile a, in place (a block barrier after every stage); tw[m] = e^{-2 pi i m / N} in shared memory
 __device__ void gen_fft_fwd(float2* a, const float2* __restrict__ tw, const GenGeo& g)
 {
-    int L = g.N;
     for (int f = 0; f < g.nf; ++f) {
-        gen_stage_any<false>(g.radix[f], a, tw, g.N, g.W, L);
+        gen_stage_any<false>(a, tw, g, f);
         __syncthreads();
-        L /= g.radix[f];
     }
 }
 __device__ void gen_fft_inv(float2* a, const float2* __restrict__ tw, const GenGeo& g)
 {
-    int L = 1;
     for (int f = g.nf - 1; f >= 0; --f) {
-        L *= g.radix[f];
-        gen_stage_any<true>(g.radix[f], a, tw, g.N, g.W, L);
+        gen_stage_any<true>(a, tw, g, f);
         __syncthreads();
     }
 }
@@ -286,60 +282,51 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     const int n = n0 + (int)(blockIdx.x / tiles), tile = (int)(blockIdx.x % tiles), x0 = tile * W;
     const size_t px = (size_t)N * N;
     for (int i = threadIdx.x; i < N; i += blockDim.x) s.tw[i] = twg[i];
-    // thread -> (column w of the tile, rows r0, r0 + rstep, ...): a row segment of W complex numbers is contiguous
-    const int cw = threadIdx.x % W, r0 = threadIdx.x / W, rstep = blockDim.x / W, cx = x0 + cw;
-    // the tile arrives by asynchronous 8-byte copies (all of a thread's rows in flight at once); sqrt(I) of the tile is
+    // thread -> (pair of columns w2 of the tile, rows r0, r0 + rstep, ...): a row segment of W complex numbers is
+    // contiguous, a pair of columns is 16 aligned bytes both in the scratch row and in the tile (N and W are even)
+    const int W2 = W / 2, w2 = threadIdx.x & (W2 - 1), r0 = threadIdx.x / W2, rstep = blockDim.x / W2, cx = x0 + 2 * w2;
+    float2* __restrict__ col0 = scr + (size_t)n * px + cx;
+    const float* __restrict__ A0 = A + (size_t)n * px + cx;
+    // the tile arrives by asynchronous 16-byte copies (all of a thread's rows in flight at once); sqrt(I) of the tile is
     // requested into L2 meanwhile
     if (cx < N) {
         for (int y = r0; y < N; y += rstep) {
-            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + t.line(y, cw));
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(scr + (size_t)n * px + (size_t)y * N + cx) : "memory");
+            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + t.pair(y, w2));
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(col0 + (size_t)y * N) : "memory");
         }
-        if (mode == 0 && (cw & 7) == 0)
-            for (int y = r0; y < N; y += rstep) asm volatile("prefetch.global.L2 [%0];" ::"l"(A + (size_t)n * px + (size_t)y * N + cx));
+        if (mode == 0 && (w2 & 3) == 0)
+            for (int y = r0; y < N; y += rstep) gen_prefetch_l2(A0 + (size_t)y * N);
     } else {
-        for (int y = r0; y < N; y += rstep) s.a[t.line(y, cw)] = make_float2(0.f, 0.f);
+        for (int y = r0; y < N; y += rstep) *reinterpret_cast<float4*>(s.a + t.pair(y, w2)) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    asm volatile("cp.async.wait_all;" ::: "memory");
+    gen_cp_async_wait();
     __syncthreads();
-    float2* const r = s.a;
     if (mode != 2) gen_fft_fwd(s.a, s.tw, gg);
     if (mode == 0) {
-        double acc = 0.0;
-        constexpr int UA = 8;   // sqrt(I) of UA rows requested before the first is used
+        // the modulus step of the power-of-two path (cpra_kernels.cuh) on the two columns of the pair
+        float2 acc2 = make_float2(0.f, 0.f);
+        constexpr int UA = 4;   // sqrt(I) of UA rows requested before the first is used
         for (int kb = r0; kb < N && cx < N; kb += UA * rstep) {
-            float av[UA];
+            float2 av[UA];
 #pragma unroll
             for (int u = 0; u < UA; ++u) {
                 const int ky = kb + u * rstep;
-                av[u] = ky < N ? __ldg(A + (size_t)n * px + (size_t)ky * N + cx) : -1.f;
+                av[u] = ky < N ? __ldg(reinterpret_cast<const float2*>(A0 + (size_t)ky * N)) : make_float2(-1.f, -1.f);
             }
 #pragma unroll
             for (int u = 0; u < UA; ++u) {
                 const int ky = kb + u * rstep;
                 if (ky >= N) break;
-                float2 G = r[t.line(ky, cw)];
-                const float a = av[u];
-                float f = scale;
-                if (a >= 0.f) {
-                    const float m2 = G.x * G.x + G.y * G.y;
-                    if (m2 >= 1.17549435e-38f) {
-                        const float mag = sqrtf(m2);
-                        const float d = mag - a;
-                        acc += (double)d * (double)d;
-                        f = a / mag * scale;
-                    } else {
-                        acc += (double)a * (double)a;
-                        G = make_float2(1.f, 0.f);
-                        f = a * scale;
-                    }
-                }
-                r[t.line(ky, cw)] = make_float2(G.x * f, G.y * f);
+                float2* q = s.a + t.pair(ky, w2);
+                c2 v = gen_ld2(q);
+                modulus_pair(v, av[u], scale, acc2);
+                gen_st2(q, v);
             }
         }
         // fixed-order block reduction of the error numerator
+        float acc = acc2.x + acc2.y;
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if ((threadIdx.x & 31) == 0) s.red[threadIdx.x >> 5] = acc;
+        if ((threadIdx.x & 31) == 0) s.red[threadIdx.x >> 5] = (double)acc;
         __syncthreads();
         if (threadIdx.x == 0) {
             double sum = 0.0;
@@ -349,8 +336,9 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     }
     if (mode != 1) gen_fft_inv(s.a, s.tw, gg);
     if (cx < N) {
-#pragma unroll 8
-        for (int y = r0; y < N; y += rstep) scr[(size_t)n * px + (size_t)y * N + cx] = r[t.line(y, cw)];
+#pragma unroll 4
+        for (int y = r0; y < N; y += rstep)
+            *reinterpret_cast<float4*>(col0 + (size_t)y * N) = *reinterpret_cast<const float4*>(s.a + t.pair(y, w2));
     }
 }
 
