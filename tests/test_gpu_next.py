@@ -355,7 +355,7 @@ def test_prtf(torch_cuda, cfg, Np, N):
 # ------------------------------------------------------------------------------------------------
 # f4: sizes that are not powers of two (PAPER.md:82 N = 160, :98 N = 700): the mixed-radix path
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("N", [20, 48, 100, 160, 224, 700])
+@pytest.mark.parametrize("N", [20, 48, 100, 160, 224, 360, 420, 700, 1008])
 def test_fft2_mixed_radix(torch_cuda, N):
     import paper_2402_05283_b200 as cpra
     Np = 2
@@ -375,7 +375,8 @@ def test_fft2_mixed_radix(torch_cuda, N):
 
 @pytest.mark.parametrize("N,Np,alpha,n_ei,seam,rule", [
     (160, 6, (0.6, 0.2), 1, 0, "hio"), (160, 5, (0.5, 0.2, 0.05), 2, 1, "raar"), (48, 7, (0.6, 0.2), 1, 1, "hio"),
-    (100, 3, (0.6, 0.2), 3, 0, "er"), (700, 3, (0.6, 0.2), 1, 0, "hio"), (20, 1, (1.0,), 1, 0, "hio")])
+    (100, 3, (0.6, 0.2), 3, 0, "er"), (700, 3, (0.6, 0.2), 1, 0, "hio"), (20, 1, (1.0,), 1, 0, "hio"),
+    (420, 3, (0.6, 0.2), 1, 1, "hio")])
 def test_loop_mixed_radix(torch_cuda, N, Np, alpha, n_ei, seam, rule):
     """The loop at the paper's own detector sizes (160, 700) and other 2^a 3^b 5^c 7^d sizes against the oracle,
     whose transform for these N is the O(N^2)-per-line definition."""
@@ -383,7 +384,7 @@ def test_loop_mixed_radix(torch_cuda, N, Np, alpha, n_ei, seam, rule):
     o, g = _oracle(p, alpha, n_ei), _gpu(p, alpha, n_ei)
     o.set_seam(seam); g.set_seam(bool(seam))
     o.set_update(rule); g.set_update(rule)
-    k = 2 if N == 700 else 4
+    k = 2 if N >= 420 else 4
     o.iterate(k, 0.9)
     g.iterate(k, 0.9)
     assert rel_l2(_get(g), o.get_projections(0)) <= k * TOL_1
