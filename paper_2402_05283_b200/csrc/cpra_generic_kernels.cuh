@@ -213,6 +213,8 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
         } else if (mixes && mp.K == 1) {
             // Eq. (4) with the default coupling: own + the two neighbours
             const float2* __restrict__ go = cur + row;
+            const unsigned char* __restrict__ Sr = S + row;
+            float2* __restrict__ ghr = ghat_out ? ghat_out + row : nullptr;
             const float2* __restrict__ gm = cur + (size_t)mm * px + (size_t)y * N;
             const float2* __restrict__ gq = cur + (size_t)mq * px + (size_t)y * N;
             for (int x0 = lane; x0 < N; x0 += 32 * GEN_U) {
@@ -233,8 +235,8 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
                     if (x < N) {
                         const float sx = (0.f + a[u].x) + b[u].x, sy = (0.f + a[u].y) + b[u].y;
                         float2 v = make_float2(fmaf(mp.a[1], sx, mp.a[0] * o[u].x), fmaf(mp.a[1], sy, mp.a[0] * o[u].y));
-                        if (mask_mode && !S[row + x]) v = make_float2(0.f, 0.f);
-                        if (ghat_out) ghat_out[row + x] = v;
+                        if (mask_mode && !Sr[x]) v = make_float2(0.f, 0.f);
+                        if (ghr) ghr[x] = v;
                         s.a[t.line(x, w)] = v;
                     }
                 }
@@ -380,7 +382,12 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
     for (int w = wid; w < W; w += nw) {
         const int y = y0 + w;
         if (y >= N) continue;
+        // the line's rows of the global arrays as pointers of their own: the loop below adds only x
         const size_t row = tbase + (size_t)w * N;
+        const unsigned char* __restrict__ Sr = S + row;
+        const float2* __restrict__ ghr = ghat ? ghat + row : nullptr;
+        float2* __restrict__ outr = nxt + row;
+        const bool use_gh = hio && ghat != nullptr;
         for (int x0 = lane; x0 < N; x0 += 32 * GEN_U) {
             float2 gp[GEN_U], gh[GEN_U];
             unsigned char sv[GEN_U];
@@ -391,10 +398,8 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
                 sv[u] = 1;
                 if (x < N) {
                     gp[u] = s.a[t.line(x, w)];
-                    if (hio) {
-                        sv[u] = S[row + x];
-                        if (ghat) gh[u] = ghat[row + x];
-                    }
+                    if (hio) sv[u] = Sr[x];
+                    if (use_gh) gh[u] = ghr[x];
                 }
             }
 #pragma unroll
@@ -406,7 +411,7 @@ k_gen_row_inv(const float2* __restrict__ scr, const float2* __restrict__ cur, fl
                     const float2 h = ghat ? gh[u] : gen_mix(cur, gg, mp, n, y, x, fires != 0);
                     g = make_float2(fmaf(mp.c_gp, g.x, mp.c_ghat * h.x), fmaf(mp.c_gp, g.y, mp.c_ghat * h.y));
                 }
-                nxt[row + x] = g;
+                outr[x] = g;
             }
         }
     }
