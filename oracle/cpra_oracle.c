@@ -716,7 +716,7 @@ static void blur_image(const real* a, real* b, int N, double sigma)
 
 int oracle_blur(const double* in, double* out, int N, double sigma)
 {
-    if (!in || !out || !is_pow2(N) || !(sigma >= 0.0)) return ORACLE_ERR_INVALID_ARG;
+    if (!in || !out || N < 2 || (N & 1) || !(sigma >= 0.0)) return ORACLE_ERR_INVALID_ARG;   /* any even N (fft2d: reading A20) */
     const size_t px = (size_t)N * N;
     real* a = (real*)malloc(sizeof(real) * px); real* b = (real*)malloc(sizeof(real) * px);
     for (size_t i = 0; i < px; ++i) a[i] = (real)in[i];
@@ -1015,32 +1015,39 @@ int oracle_align_episode(double* ep, int N, int Np, int n_ref, int* flips)
  * all z lines with the textbook fft1d.  sign = -1 forward, unnormalised; +1 inverse, / N^3. */
 int oracle_fft3(const double* in, double* out, int N, int sign)
 {
-    if (!in || !out || !is_pow2(N) || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    if (!in || !out || N < 2 || (N & 1) || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
     const size_t n3 = (size_t)N * N * N;
     cplx* v = (cplx*)malloc(sizeof(cplx) * n3);
     for (size_t i = 0; i < n3; ++i) { v[i].re = (real)in[2 * i]; v[i].im = (real)in[2 * i + 1]; }
-    cplx* tw = twiddle_table(N, sign);
+    /* the 1D transform of a line: the radix-2 FFT for a power of two, the O(N^2) definition otherwise (reading A20,
+     * as in fft2d) */
+    const int p2 = is_pow2(N);
+    cplx* tw = p2 ? twiddle_table(N, sign) : root_table(N, sign);
     #pragma omp parallel
     {
         cplx* line = (cplx*)malloc(sizeof(cplx) * (size_t)N);
+        cplx* tmp = (cplx*)malloc(sizeof(cplx) * (size_t)N);
         #pragma omp for schedule(static)
         for (int z = 0; z < N; ++z)
-            for (int y = 0; y < N; ++y) fft1d(v + ((size_t)z * N + y) * N, N, tw);
+            for (int y = 0; y < N; ++y) {
+                cplx* l = v + ((size_t)z * N + y) * N;
+                if (p2) fft1d(l, N, tw); else dft1d_direct(l, N, tw, tmp);
+            }
         #pragma omp for schedule(static)
         for (int z = 0; z < N; ++z)
             for (int x = 0; x < N; ++x) {
                 for (int y = 0; y < N; ++y) line[y] = v[((size_t)z * N + y) * N + x];
-                fft1d(line, N, tw);
+                if (p2) fft1d(line, N, tw); else dft1d_direct(line, N, tw, tmp);
                 for (int y = 0; y < N; ++y) v[((size_t)z * N + y) * N + x] = line[y];
             }
         #pragma omp for schedule(static)
         for (int y = 0; y < N; ++y)
             for (int x = 0; x < N; ++x) {
                 for (int z = 0; z < N; ++z) line[z] = v[((size_t)z * N + y) * N + x];
-                fft1d(line, N, tw);
+                if (p2) fft1d(line, N, tw); else dft1d_direct(line, N, tw, tmp);
                 for (int z = 0; z < N; ++z) v[((size_t)z * N + y) * N + x] = line[z];
             }
-        free(line);
+        free(line); free(tmp);
     }
     free(tw);
     const double sc = sign > 0 ? 1.0 / ((double)N * N * N) : 1.0;
@@ -1061,7 +1068,7 @@ int oracle_fft3(const double* in, double* out, int N, int sign)
  * S3: u8 [N][N][N]; obj (out): the object after the last support step; err (optional): k doubles. */
 int oracle_refine_3d(const double* E, const double* W, const unsigned char* S3, int N, int k, double* obj, double* err)
 {
-    if (!E || !W || !S3 || !obj || !is_pow2(N) || k < 1) return ORACLE_ERR_INVALID_ARG;
+    if (!E || !W || !S3 || !obj || N < 2 || (N & 1) || k < 1) return ORACLE_ERR_INVALID_ARG;
     const size_t n3 = (size_t)N * N * N;
     double* F = (double*)malloc(sizeof(double) * 2 * n3);
     double* T = (double*)malloc(sizeof(double) * 2 * n3);

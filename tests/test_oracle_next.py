@@ -80,6 +80,17 @@ def test_blur_of_a_delta_is_the_periodic_gaussian():
     H = np.exp(-2 * np.pi ** 2 * sig ** 2 * (k[:, None] ** 2 + k[None, :] ** 2) / N ** 2)
     r = np.random.default_rng(2).uniform(size=(N, N))
     assert np.abs(blur(r, sig) - np.fft.ifft2(np.fft.fft2(r) * H).real).max() < 1e-12
+    # a size that is not a power of two (reading A20): the same closed form and library route
+    N = 24
+    a = np.zeros((N, N))
+    a[20, 3] = 1.5
+    d = N * np.arange(-4, 5)
+    g1 = lambda c: np.array([np.exp(-0.5 * ((i - c + d) / sig) ** 2).sum() for i in range(N)]) / (sig * np.sqrt(2 * np.pi))
+    assert np.abs(blur(a, sig) - 1.5 * g1(20)[:, None] * g1(3)[None, :]).max() < 1e-12
+    k = np.fft.fftfreq(N, 1.0 / N)
+    H = np.exp(-2 * np.pi ** 2 * sig ** 2 * (k[:, None] ** 2 + k[None, :] ** 2) / N ** 2)
+    r = np.random.default_rng(3).uniform(size=(N, N))
+    assert np.abs(blur(r, sig) - np.fft.ifft2(np.fft.fft2(r) * H).real).max() < 1e-12
 
 
 def _sw_plan(g, S):
@@ -273,7 +284,7 @@ def test_merge_offer_from_the_plan_takes_the_supported_estimate_and_its_error():
 
 # ---------------------------------------------------------------- f3: 3D transform
 def test_fft3_against_numpy_and_round_trip():
-    for N in (4, 8, 16):
+    for N in (4, 8, 16, 12, 20):       # 12, 20: not powers of two (reading A20: the definition, line by line)
         rng = np.random.default_rng(N)
         v = rng.normal(size=(N, N, N)) + 1j * rng.normal(size=(N, N, N))
         F = fft3(v, -1)
@@ -336,6 +347,20 @@ def test_refine_3d_closed_forms():
     # second iteration: the unknown voxels carry F' of the first, the known ones E again
     o2, _ = refine_3d(E, W, S3, 2)
     assert np.abs(o2 - np.fft.ifftn(np.where(W > 0, E, Fp)) * S3).max() < 1e-13
+
+
+def test_refine_3d_at_a_size_that_is_not_a_power_of_two():
+    """Reading A20 carried to Step D: N = 12, two iterations by hand with numpy's FFT."""
+    obj, S3, E, rng = _cube_case(N=12, seed=5)
+    W = (rng.uniform(size=(12, 12, 12)) < 0.6).astype(float)
+    o2, e2 = refine_3d(E, W, S3, 2)
+    o1 = np.fft.ifftn(E * (W > 0)) * S3
+    F1 = np.fft.fftn(o1)
+    want = np.fft.ifftn(np.where(W > 0, E, F1)) * S3
+    assert np.abs(o2 - want).max() < 1e-13
+    den = (np.abs(E)[W > 0] ** 2).sum()
+    assert abs(e2[0] - np.sqrt((np.abs(F1 - E)[W > 0] ** 2).sum() / den)) < 1e-13
+    assert abs(e2[1] - np.sqrt((np.abs(np.fft.fftn(want) - E)[W > 0] ** 2).sum() / den)) < 1e-13
 
 
 def test_refine_3d_error_never_increases_and_recovers_the_object():
