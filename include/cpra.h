@@ -12,7 +12,8 @@
  *
  * Conventions
  *   - n = 0..Np-1 projections (the paper counts from 1); pixel (y, x), row-major, x fastest;
- *     complex = interleaved (re, im) fp32; N a power of two in [16, 1024].
+ *     complex = interleaved (re, im) fp32; N a power of two in [16, 1024], or any even N in [16, 1024] whose
+ *     prime factors are 2, 3, 5, 7 (the paper's detectors: 160; 700): every call serves both kinds.
  *   - Pointer names: d_* = DEVICE pointers (the caller's allocator, e.g. torch data_ptr());
  *     h_* = HOST pointers.  The library never allocates device memory: every internal buffer lives
  *     in the workspace the caller binds (cpra_workspace_bytes / cpra_bind_workspace).
@@ -39,7 +40,7 @@ typedef struct cpra_plan_s* cpra_plan_t; /* opaque */
 enum {
     CPRA_OK = 0,
     CPRA_ERR_INVALID_ARG = -1,      /* NULL pointer, k < 0, bad K / n_ei / beta, bad `which` */
-    CPRA_ERR_UNSUPPORTED_SIZE = -2, /* N not a power of two in [16, 1024], or Np < 1 */
+    CPRA_ERR_UNSUPPORTED_SIZE = -2, /* N outside [16, 1024], odd, or with a prime factor above 7; or Np < 1 */
     CPRA_ERR_NOT_READY = -3,        /* call made before the state it needs exists */
     CPRA_ERR_WORKSPACE = -4,        /* workspace missing, too small or misaligned */
     CPRA_ERR_CUDA = -5,             /* a CUDA runtime call or an earlier kernel failed */
@@ -319,8 +320,7 @@ int cpra_refine_3d(cpra_plan_t plan, const float* d_E, const float* d_W, const u
  *              PRTF(s) = mean over n and the measured pixels with A > 0 of ring s of |F2[avg_n]| / A_n.
  *   d_out: fp32 [N/2 + 1].  Shell sums are double atomics: reproducible to ~1e-15, not bit for bit.
  * cpra_prtf uses the FFT scratch and the spare state buffer; the loop state is untouched.
- * Errors: INVALID_ARG (cpra_fsc: Np != N), NOT_READY (cpra_prtf without data), UNSUPPORTED_SIZE (N not a power of
- * two), CUDA.
+ * Errors: INVALID_ARG (cpra_fsc: Np != N), NOT_READY (cpra_prtf without data), CUDA.
  */
 int cpra_fsc(cpra_plan_t plan, const float* d_F1, const float* d_F2, float* d_out);
 int cpra_prtf(cpra_plan_t plan, const float* d_avg, float* d_out);

@@ -483,7 +483,7 @@ int cpra_shrinkwrap(cpra_plan_t p, float sigma, float threshold, float* d_blurre
     if (!p || !(sigma >= 0.f) || !(threshold >= 0.f) || !std::isfinite(sigma) || !std::isfinite(threshold)) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
-    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
+    if (p->generic) return gen_shrinkwrap(p, sigma, threshold, d_blurred);
     const size_t total = (size_t)p->Np * p->N * p->N, nquads = total / 2;
     float4* tmp = p->st[p->cur ^ 1];
     // |S g| -> forward 2D FT -> Gaussian transfer function -> inverse 2D FT -> per-image maximum -> threshold
@@ -657,9 +657,9 @@ int cpra_fft3(cpra_plan_t p, const float* d_in, float* d_out, int sign)
 {
     if (!p || !d_in || !d_out || (sign != 1 && sign != -1)) return CPRA_ERR_INVALID_ARG;
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;   // a cube is a stack of N slices of N x N
-    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
     int rc = cpra_fft2(p, d_in, d_out, sign);          // the (y, x) transforms of all z slices
     if (rc) return rc;
+    if (p->generic) return gen_fftz(p, (float2*)d_out, sign);
     { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, rc = Launch<NN>::fftz(p, (float2*)d_out, sign)); return 0; }; f(); }
     return rc;
 }
@@ -668,7 +668,6 @@ int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsi
 {
     if (!p || !d_E || !d_W || !d_S3 || !d_obj || k < 1) return CPRA_ERR_INVALID_ARG;
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
-    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
     if (int rc = ready(p)) return rc;
     const size_t n3 = (size_t)p->N * p->N * p->N;
     const int nblk = (int)std::min<size_t>(512, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
@@ -714,9 +713,13 @@ int cpra_prtf(cpra_plan_t p, const float* d_avg, float* d_out)
     if (!p || !d_avg || !d_out) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->have_data) return CPRA_ERR_NOT_READY;
-    if (p->generic) return CPRA_ERR_UNSUPPORTED_SIZE;
     const size_t total = (size_t)p->Np * p->N * p->N;
     const int ns = p->N / 2 + 1;
+    if (p->generic) {
+        if (int rc = gen_prtf_sums(p, d_avg, p->shell)) return rc;
+        k_prtf_finalize<<<blocks_for(ns, 128), 128, 0, p->stream>>>(p->shell, d_out, ns);
+        return check_launch(p);
+    }
     float4* tmp = p->st[p->cur ^ 1];
     k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_avg, (float*)tmp, p->geo, total);
     int rc = check_launch(p);

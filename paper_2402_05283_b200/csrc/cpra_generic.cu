@@ -64,7 +64,8 @@ int row_fwd(cpra_plan_s* p, const float2* cur, int n0, int nimg, bool fires, boo
 int col(cpra_plan_s* p, int n0, int nimg, int mode, float scale)
 {
     ProfScope prof(p, CPRA_PROFILE_COL);
-    k_gen_col<<<(unsigned)(nimg * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, mode, scale);
+    k_gen_col<<<(unsigned)(nimg * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, mode, scale,
+                                                                                  (size_t)p->N * p->N, (size_t)p->N);
     return check_launch(p);
 }
 int row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, int n0, int nimg, bool fires, bool hio, float beta, float scale, const float2* ghat)
@@ -157,6 +158,49 @@ int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign)
     if ((rc = col(p, 0, p->Np, 2, 1.0f))) return rc;
     if ((rc = row_inv(p, tmp, tmp, 0, p->Np, false, false, 0.f, 1.0f / ((float)p->N * (float)p->N), nullptr))) return rc;
     return cudaMemcpyAsync(d_out, tmp, sizeof(float2) * total, cudaMemcpyDeviceToDevice, p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
+}
+
+// the z pass of cpra_fft3 on a natural [z][y][x] volume, in place: for every y, the W-column tiles of the [z][x] slice
+// (rows N^2 apart) through the column kernel's natural-order modes; inverse: times 1 / N
+int gen_fftz(cpra_plan_s* p, float2* vol, int sign)
+{
+    const size_t N = (size_t)p->N;
+    k_gen_col<<<(unsigned)(p->N * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>(vol, nullptr, p->tw, nullptr, p->gg, 0, sign < 0 ? 3 : 4,
+                                                                                  sign < 0 ? 1.0f : 1.0f / (float)p->N, N, N * N);
+    return check_launch(p);
+}
+
+// shrink-wrap (cpra_shrinkwrap): b_n = G_sigma * |S_n g_n| through this path's own transforms, S_n <- [b_n >= threshold max b_n]
+int gen_shrinkwrap(cpra_plan_s* p, float sigma, float threshold, float* d_blurred)
+{
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    float2* tmp = (float2*)p->st[p->cur ^ 1];
+    k_gen_abs_supported<<<gblocks(total, 256), 256, 0, p->stream>>>((const float2*)p->st[p->cur], p->S8, tmp, total);
+    int rc = check_launch(p);
+    if (rc == CPRA_OK) rc = row_fwd(p, tmp, 0, p->Np, false, false, nullptr);
+    if (rc == CPRA_OK) rc = col(p, 0, p->Np, 1, 1.0f);
+    if (rc) return rc;
+    k_gen_gauss_filter<<<gblocks(total, 256), 256, 0, p->stream>>>((float2*)p->scr, p->gg, total, sigma);
+    if ((rc = check_launch(p))) return rc;
+    if ((rc = col(p, 0, p->Np, 2, 1.0f))) return rc;
+    if ((rc = row_inv(p, tmp, tmp, 0, p->Np, false, false, 0.f, 1.0f / ((float)p->N * (float)p->N), nullptr))) return rc;
+    k_gen_image_max<<<p->Np, 256, 0, p->stream>>>(tmp, p->mx, p->N);
+    if ((rc = check_launch(p))) return rc;
+    k_gen_threshold<<<gblocks(total, 256), 256, 0, p->stream>>>(tmp, p->mx, p->S8, d_blurred, p->N, total, threshold);
+    return check_launch(p);
+}
+
+// the shell sums of cpra_prtf into acc (2 (N / 2 + 1) doubles, cleared here)
+int gen_prtf_sums(cpra_plan_s* p, const float* d_avg, double* acc)
+{
+    const size_t total = (size_t)p->Np * p->N * p->N;
+    const int ns = p->N / 2 + 1;
+    int rc = row_fwd(p, (const float2*)d_avg, 0, p->Np, false, false, nullptr);
+    if (rc == CPRA_OK) rc = col(p, 0, p->Np, 1, 1.0f);
+    if (rc) return rc;
+    if (cudaMemsetAsync(acc, 0, sizeof(double) * 2 * ns, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    k_gen_prtf_accumulate<<<4 * p->sms, 256, sizeof(double) * 2 * ns, p->stream>>>((const float2*)p->scr, p->A, acc, p->gg, total);
+    return check_launch(p);
 }
 
 int gen_slices(cpra_plan_s* p, float2* Et)

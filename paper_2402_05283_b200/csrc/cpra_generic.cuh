@@ -34,7 +34,8 @@ struct GenGeo {
 constexpr int GEN_NT = 256;
 // lines per tile: as many as leave four CTAs per SM their shared memory (N W 8 bytes each + the table)
 __host__ __device__ __forceinline__ int gen_lines_per_tile(int N) { return N <= 360 ? 16 : 8; }
-__host__ __device__ __forceinline__ size_t gen_smem_bytes(int N, int W) { return (size_t)N * W * 8 + (size_t)N * 8 + 32 * 8 + 16; }
+// the tile, the table of roots, 32 doubles of reduction scratch, the position table of the natural-order column modes
+__host__ __device__ __forceinline__ size_t gen_smem_bytes(int N, int W) { return (size_t)N * W * 8 + (size_t)N * 8 + 32 * 8 + (size_t)N * 4 + 16; }
 // position of frequency k after the forward transform
 __host__ __device__ __forceinline__ int gen_pos(int k, const GenGeo& g)
 {

@@ -135,11 +135,13 @@ __device__ void gen_fft_inv(float2* a, const float2* __restrict__ tw, const GenG
 struct GenSmem {
     float2 *a, *tw;
     double* red;
+    int* perm;   // pos(k), filled by the kernels that need it
     __device__ __forceinline__ GenSmem(unsigned char* sm, int N, int W)
     {
         a = reinterpret_cast<float2*>(sm);
         tw = a + (size_t)N * W;
         red = reinterpret_cast<double*>(tw + N);
+        perm = reinterpret_cast<int*>(red + 32);
     }
 };
 
@@ -272,9 +274,11 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
 // mode 0 = all three, 1 = forward only (rows left in position order), 2 = inverse only (rows expected in position
 // order).  The columns of scr are in position order (K1).  A: sqrt(I) in position order on both axes
 // (A[pos(ky)][pos(kx)], k_gen_set_data), A < 0 = unmeasured.
+// Modes 3 and 4 are the plain 1D transform along the slow axis with NATURAL order on both sides (the z pass of
+// cpra_fft3): 3 = forward, 4 = inverse times `scale`.  "Image" n starts at scr + n istride, its rows are `pitch` apart.
 __global__ void __launch_bounds__(GEN_NT, 4)
 k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* __restrict__ twg, double* __restrict__ partial,
-          GenGeo gg, int n0, int mode, float scale)
+          GenGeo gg, int n0, int mode, float scale, size_t istride, size_t pitch)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int N = gg.N, W = gg.W;
@@ -287,14 +291,18 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     // thread -> (pair of columns w2 of the tile, rows r0, r0 + rstep, ...): a row segment of W complex numbers is
     // contiguous, a pair of columns is 16 aligned bytes both in the scratch row and in the tile (N and W are even)
     const int W2 = W / 2, w2 = threadIdx.x & (W2 - 1), r0 = threadIdx.x / W2, rstep = blockDim.x / W2, cx = x0 + 2 * w2;
-    float2* __restrict__ col0 = scr + (size_t)n * px + cx;
+    float2* __restrict__ col0 = scr + (size_t)n * istride + cx;
     const float* __restrict__ A0 = A + (size_t)n * px + cx;
+    if (mode >= 3) {
+        for (int i = threadIdx.x; i < N; i += blockDim.x) s.perm[i] = gen_pos(i, gg);
+        __syncthreads();
+    }
     // the tile arrives by asynchronous 16-byte copies (all of a thread's rows in flight at once); sqrt(I) of the tile is
     // requested into L2 meanwhile
     if (cx < N) {
         for (int y = r0; y < N; y += rstep) {
-            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + t.pair(y, w2));
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(col0 + (size_t)y * N) : "memory");
+            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + t.pair(mode == 4 ? s.perm[y] : y, w2));
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(col0 + (size_t)y * pitch) : "memory");
         }
         if (mode == 0 && (w2 & 3) == 0)
             for (int y = r0; y < N; y += rstep) gen_prefetch_l2(A0 + (size_t)y * N);
@@ -303,7 +311,7 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     }
     gen_cp_async_wait();
     __syncthreads();
-    if (mode != 2) gen_fft_fwd(s.a, s.tw, gg);
+    if (mode != 2 && mode != 4) gen_fft_fwd(s.a, s.tw, gg);
     if (mode == 0) {
         // the modulus step of the power-of-two path (cpra_kernels.cuh) on the two columns of the pair
         float2 acc2 = make_float2(0.f, 0.f);
@@ -336,11 +344,19 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
             partial[(size_t)n * tiles + tile] = sum;
         }
     }
-    if (mode != 1) gen_fft_inv(s.a, s.tw, gg);
+    if (mode != 1 && mode != 3) gen_fft_inv(s.a, s.tw, gg);
     if (cx < N) {
+        if (mode >= 3) {
+            const float f = mode == 4 ? scale : 1.0f;
+            for (int y = r0; y < N; y += rstep) {
+                const float4 q = *reinterpret_cast<const float4*>(s.a + t.pair(mode == 3 ? s.perm[y] : y, w2));
+                *reinterpret_cast<float4*>(col0 + (size_t)y * pitch) = make_float4(q.x * f, q.y * f, q.z * f, q.w * f);
+            }
+        } else {
 #pragma unroll 4
-        for (int y = r0; y < N; y += rstep)
-            *reinterpret_cast<float4*>(col0 + (size_t)y * N) = *reinterpret_cast<const float4*>(s.a + t.pair(y, w2));
+            for (int y = r0; y < N; y += rstep)
+                *reinterpret_cast<float4*>(col0 + (size_t)y * pitch) = *reinterpret_cast<const float4*>(s.a + t.pair(y, w2));
+        }
     }
 }
 
@@ -470,6 +486,82 @@ __global__ void k_gen_permute(const float2* __restrict__ in, float2* __restrict_
     const size_t n = i / ((size_t)N * N);
     const size_t j = (n * N + gen_pos(ky, gg)) * N + gen_pos(kx, gg);
     if (to_pos) out[j] = in[i]; else out[i] = in[j];
+}
+
+// ---- shrink-wrap (reading A23) on natural arrays ------------------------------------
+// (|S g|, 0)
+__global__ void k_gen_abs_supported(const float2* __restrict__ st, const unsigned char* __restrict__ S, float2* __restrict__ out, size_t total)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const float2 v = st[i];
+    out[i] = make_float2(S[i] ? sqrtf(v.x * v.x + v.y * v.y) : 0.f, 0.f);
+}
+// spectrum in position order *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2); one thread per natural (n, ky, kx)
+__global__ void k_gen_gauss_filter(float2* __restrict__ scr, GenGeo gg, size_t total, float sigma)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int N = gg.N;
+    const int ix = (int)(i % N), iy = (int)((i / N) % N);
+    const size_t n = i / ((size_t)N * N);
+    const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N;
+    const double sg = (double)sigma;
+    const float f = (float)exp(-2.0 * 9.86960440108935861883 * sg * sg * ((double)ky * ky + (double)kx * kx) / ((double)N * N));
+    const size_t o = (n * N + gen_pos(iy, gg)) * N + gen_pos(ix, gg);
+    scr[o].x *= f;
+    scr[o].y *= f;
+}
+// per-image maximum of the real part (one block per image)
+__global__ void k_gen_image_max(const float2* __restrict__ st, float* __restrict__ mx, int N)
+{
+    const size_t px = (size_t)N * N;
+    const float2* __restrict__ p = st + (size_t)blockIdx.x * px;
+    float m = -3.402823466e38f;
+    for (size_t i = threadIdx.x; i < px; i += blockDim.x) m = fmaxf(m, p[i].x);
+    __shared__ float red[32];
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, red[w]);
+        mx[blockIdx.x] = m;
+    }
+}
+// S <- [ b >= threshold max_n b ], max_n > 0; blurred (optional): b as natural floats
+__global__ void k_gen_threshold(const float2* __restrict__ b, const float* __restrict__ mx, unsigned char* __restrict__ S,
+                                float* __restrict__ blurred, int N, size_t total, float threshold)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const float m = mx[i / ((size_t)N * N)];
+    const float v = b[i].x;
+    S[i] = (m > 0.f && v >= threshold * m) ? 1 : 0;
+    if (blurred) blurred[i] = v;
+}
+// PRTF sums: scr = F2[avg_n] and A = sqrt(I), both in position order; acc[0..ns): sum of |G| / A over
+// the measured pixels with A > 0 of ring s = round(|k|), acc[ns..2ns): their number
+__global__ void k_gen_prtf_accumulate(const float2* __restrict__ scr, const float* __restrict__ A, double* __restrict__ acc, GenGeo gg, size_t total)
+{
+    extern __shared__ double sh[];   // 2 ns
+    const int N = gg.N, ns = N / 2 + 1;
+    for (int i = threadIdx.x; i < 2 * ns; i += blockDim.x) sh[i] = 0.0;
+    __syncthreads();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % N), iy = (int)((i / N) % N);
+        const size_t n = i / ((size_t)N * N);
+        const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N;
+        const int sh_i = (int)floor(sqrt((double)kx * kx + (double)ky * ky) + 0.5);
+        if (sh_i >= ns) continue;
+        const size_t o = (n * N + gen_pos(iy, gg)) * N + gen_pos(ix, gg);
+        const float a = A[o];
+        if (!(a > 0.f)) continue;
+        const float2 G = scr[o];
+        atomicAdd(&sh[sh_i], sqrt((double)G.x * G.x + (double)G.y * G.y) / (double)a);
+        atomicAdd(&sh[ns + sh_i], 1.0);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 2 * ns; i += blockDim.x) if (sh[i] != 0.0) atomicAdd(&acc[i], sh[i]);
 }
 
 }  // namespace cpra

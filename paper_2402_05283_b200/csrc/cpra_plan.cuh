@@ -513,7 +513,10 @@ int gen_iterate(cpra_plan_s* p, int k, float beta);
 int gen_prereconstruct(cpra_plan_s* p, int n, int k, float beta);
 int gen_get_projections(cpra_plan_s* p, int which, float* d_out);
 int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign);
-int gen_slices(cpra_plan_s* p, float2* Et);   // E_n = F[S_n g_n], natural, transposed to [n][ku][kz]
+int gen_slices(cpra_plan_s* p, float2* Et);
+int gen_fftz(cpra_plan_s* p, float2* vol, int sign);                        // natural [z][y][x], in place
+int gen_shrinkwrap(cpra_plan_s* p, float sigma, float threshold, float* d_blurred);
+int gen_prtf_sums(cpra_plan_s* p, const float* d_avg, double* acc);   // E_n = F[S_n g_n], natural, transposed to [n][ku][kz]
 
 #define CPRA_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
 #ifndef CPRA_INST_N

@@ -9,7 +9,7 @@
             then cpra_align_episode: the projections of the merged episode are given one common phase gauge and one
             twin choice (reading A28) -- without it the slices of an unconstrained complex iterate do not fit together
     Step D  Fourier-slice assembly of the merged episode (cpra_assemble_3d), then optionally the inverse 3D
-            transform / the iterations against a 3D support (cpra_fft3 / cpra_refine_3d; power-of-two N)
+            transform / the iterations against a 3D support (cpra_fft3 / cpra_refine_3d)
 
 Every arithmetic step runs in the library's kernels; this module only allocates torch tensors, draws the random
 starting phases (torch's generator on the device: input generation, not part of the method) and calls the binding."""
@@ -31,7 +31,7 @@ class CpraResult:
     twins: "object"              # int32 [N_l]
     spectrum: "object" = None    # complex64 [N, N, N], the assembled E(q) (device) if assemble=True
     weight: "object" = None      # float32 [N, N, N]
-    obj: "object" = None         # complex64 [N, N, N], O(r) if a 3D step was asked for (power-of-two N)
+    obj: "object" = None         # complex64 [N, N, N], O(r) if a 3D step was asked for
     refine_error: "object" = None
     seconds: dict = None
 
@@ -56,11 +56,11 @@ def random_phase_starts(plan, intensity, mask, seed: int):
 def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, n_pre: int, n_episodes: int, n_ei: int,
                 beta: float = 0.9, alpha=(0.6, 0.2), update: str = "hio", seam_flip: bool = False, seed: int = 0,
                 shrinkwrap: Optional[tuple] = None, assemble: bool = True, support3d=None, refine_iters: int = 0,
-                n_ref: int = 0, align: bool = True) -> CpraResult:
+                n_ref: int = 0, align: bool = True, step3d: bool = True) -> CpraResult:
     """Steps A-D.  intensity fp32 [Np, N, N], mask u8 [Np, N, N] or None, support u8 [Np, N, N]: CUDA tensors;
     angles: Np radians (host).  shrinkwrap = (sigma, threshold): one support update at the end of every episode
-    (power-of-two N).  support3d u8 [N, N, N] + refine_iters > 0: Step D's iterations; refine_iters == 0
-    with assemble: only E(q) (and O(r) = F3^-1[E] when N is a power of two)."""
+    (PAPER.md:104).  support3d u8 [N, N, N] + refine_iters > 0: Step D's iterations; refine_iters == 0 with assemble:
+    E(q) and O(r) = F3^-1[E] (step3d=False: E(q) only)."""
     import torch
     Np, N = int(intensity.shape[0]), int(intensity.shape[-1])
     dev = intensity.device
@@ -129,7 +129,7 @@ def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, 
         plan.set_estimate(episode)
         res.spectrum, res.weight = plan.assemble_3d()
         timed("assemble", t0)
-        if N & (N - 1) == 0:
+        if step3d:
             t0 = start()
             plan.close()
             p3 = binding.Plan(N, N)

@@ -82,7 +82,7 @@ def test_seam_flip_on_config_2_and_3(torch_cuda):
 # ------------------------------------------------------------------------------------------------
 # f2: shrink-wrap
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("cfg,Np,N", [(1, 8, None), (2, 12, None), (3, 6, None), (4, 4, None), (5, 3, None)])
+@pytest.mark.parametrize("cfg,Np,N", [(1, 8, None), (2, 12, None), (3, 6, None), (4, 4, None), (5, 3, None), (1, 5, 160), (1, 4, 48)])
 def test_shrinkwrap(torch_cuda, cfg, Np, N):
     p = cpra_inputs.make_problem(cfg, Np=Np, N=N)
     o, g = _oracle(p), _gpu(p)
@@ -249,7 +249,7 @@ def test_merge_of_restarts_from_the_plan(torch_cuda):
 # ------------------------------------------------------------------------------------------------
 # f3: the 3D transform of Step D
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("N", [16, 32, 64, 128, 256])
+@pytest.mark.parametrize("N", [16, 32, 64, 128, 256, 20, 48, 160])
 def test_fft3(torch_cuda, N):
     import paper_2402_05283_b200 as cpra
     rng = np.random.default_rng(N)
@@ -299,7 +299,7 @@ def test_step_d_assemble_then_inverse_3d(torch_cuda):
     assert abs(np.vdot(pad, rec)) / (np.linalg.norm(pad) * np.linalg.norm(rec)) > 0.97
 
 
-@pytest.mark.parametrize("N", [16, 64, 128])
+@pytest.mark.parametrize("N", [16, 64, 128, 48])
 def test_refine_3d(torch_cuda, N):
     """Step D's iterations on the device against the oracle: half of the spectrum known, a box support."""
     import paper_2402_05283_b200 as cpra
@@ -337,7 +337,7 @@ def test_fsc(torch_cuda, N):
     assert np.abs(plan.fsc(torch_cuda.from_numpy(F).cuda(), torch_cuda.from_numpy(F).cuda()).cpu().numpy() - 1.0).max() <= 2e-6
 
 
-@pytest.mark.parametrize("cfg,Np,N", [(1, 8, None), (2, 12, None), (3, 6, None), (4, 4, None)])
+@pytest.mark.parametrize("cfg,Np,N", [(1, 8, None), (2, 12, None), (3, 6, None), (4, 4, None), (1, 5, 160)])
 def test_prtf(torch_cuda, cfg, Np, N):
     """PRTF of the supported estimate after a few iterations against the measured amplitudes (beamstop pixels
     and zero-count pixels left out), device vs oracle."""
