@@ -1096,6 +1096,97 @@ int oracle_refine_3d(const double* E, const double* W, const unsigned char* S3, 
     return ORACLE_OK;
 }
 
+/* Step D with the support update of P:104 ("We shrink the 3D space constraint every 5 iterations, leading to a tighter
+ * 3D space constraint close to the shape of the object at the end"; reading A30): oracle_refine_3d's iteration, and after
+ * every `every`-th iteration that is not the last the 3D analogue of the 2D shrink-wrap (reading A23):
+ *     b = G_sigma * |O|   (Gaussian of standard deviation sigma voxels, as a product with exp(-2 pi^2 sigma^2 |k|^2 / N^2)
+ *                          between a forward and an inverse 3D transform; the real part is kept)
+ *     S3 <- [ b >= threshold . max b ]      (all zero if the maximum is not positive)
+ * S3 is updated in place; blurred (optional, N^3 doubles) receives the b of the LAST update, so that a comparison can
+ * set aside the voxels within rounding of the threshold.  every < 1: never (= oracle_refine_3d). */
+int oracle_refine_3d_sw(const double* E, const double* W, unsigned char* S3, int N, int k, int every, double sigma, double threshold,
+                        double* obj, double* err, double* blurred)
+{
+    if (!E || !W || !S3 || !obj || N < 2 || (N & 1) || k < 1 || !(sigma >= 0.0) || !(threshold >= 0.0)) return ORACLE_ERR_INVALID_ARG;
+    const size_t n3 = (size_t)N * N * N;
+    double* F = (double*)malloc(sizeof(double) * 2 * n3);
+    double* T = (double*)malloc(sizeof(double) * 2 * n3);
+    double den = 0.0;
+    for (size_t i = 0; i < n3; ++i) {
+        const int known = W[i] > 0.0;
+        F[2 * i] = known ? E[2 * i] : 0.0; F[2 * i + 1] = known ? E[2 * i + 1] : 0.0;
+        if (known) den += E[2 * i] * E[2 * i] + E[2 * i + 1] * E[2 * i + 1];
+    }
+    for (int it = 0; it < k; ++it) {
+        oracle_fft3(F, obj, N, +1);
+        for (size_t i = 0; i < n3; ++i) if (!S3[i]) { obj[2 * i] = 0.0; obj[2 * i + 1] = 0.0; }
+        oracle_fft3(obj, T, N, -1);
+        double num = 0.0;
+        for (size_t i = 0; i < n3; ++i) {
+            if (W[i] > 0.0) {
+                const double dr = T[2 * i] - E[2 * i], di = T[2 * i + 1] - E[2 * i + 1];
+                num += dr * dr + di * di;
+                F[2 * i] = E[2 * i]; F[2 * i + 1] = E[2 * i + 1];
+            } else { F[2 * i] = T[2 * i]; F[2 * i + 1] = T[2 * i + 1]; }
+        }
+        if (err) err[it] = den > 0.0 ? sqrt(num / den) : 0.0;
+        if (every >= 1 && (it + 1) % every == 0 && it + 1 < k) {
+            for (size_t i = 0; i < n3; ++i) { T[2 * i] = sqrt(obj[2 * i] * obj[2 * i] + obj[2 * i + 1] * obj[2 * i + 1]); T[2 * i + 1] = 0.0; }
+            oracle_fft3(T, T, N, -1);
+            for (int iz = 0; iz < N; ++iz) {
+                const int kz = iz < N / 2 ? iz : iz - N;
+                for (int iy = 0; iy < N; ++iy) {
+                    const int ky = iy < N / 2 ? iy : iy - N;
+                    for (int ix = 0; ix < N; ++ix) {
+                        const int kx = ix < N / 2 ? ix : ix - N;
+                        const double f = exp(-2.0 * PI * PI * sigma * sigma * ((double)kz * kz + (double)ky * ky + (double)kx * kx) / ((double)N * N));
+                        const size_t i = ((size_t)iz * N + iy) * N + ix;
+                        T[2 * i] *= f; T[2 * i + 1] *= f;
+                    }
+                }
+            }
+            oracle_fft3(T, T, N, +1);
+            double m = T[0];
+            for (size_t i = 1; i < n3; ++i) if (T[2 * i] > m) m = T[2 * i];
+            for (size_t i = 0; i < n3; ++i) {
+                S3[i] = (m > 0.0 && T[2 * i] >= threshold * m) ? 1 : 0;
+                if (blurred) blurred[i] = T[2 * i];
+            }
+        }
+    }
+    free(F); free(T);
+    return ORACLE_OK;
+}
+
+/* The 3D support of Step D from the 2D supports ("We project the 2D space constrains back to the 3D space to
+ * form a relatively tight 3D space constraint"; reading A29).  The projections are line integrals along the direction
+ * perpendicular to the rotation axis z: voxel (z, y, x) falls on detector row z at column
+ *     u_n = c + (x - c) cos theta_n + (y - c) sin theta_n,        c = N / 2,
+ * and it stays in the 3D support iff in EVERY projection n its footprint touches the 2D support:
+ * S_n[z][floor(u_n)] or S_n[z][floor(u_n) + 1] is set (columns outside the detector count as outside).
+ * S3: u8 [N][N][N] (z, y, x) out. */
+int oracle_backproject_support(oracle_plan_t p, unsigned char* S3)
+{
+    if (!p || !S3) return ORACLE_ERR_INVALID_ARG;
+    if (!p->have_support) return ORACLE_ERR_NOT_READY;
+    const int N = p->N, c = N / 2;
+    #pragma omp parallel for schedule(static)
+    for (int z = 0; z < N; ++z)
+        for (int y = 0; y < N; ++y)
+            for (int x = 0; x < N; ++x) {
+                int in = 1;
+                for (int n = 0; n < p->Np && in; ++n) {
+                    const double u = (double)c + (double)(x - c) * cos(p->angles[n]) + (double)(y - c) * sin(p->angles[n]);
+                    const long u0 = (long)floor(u);
+                    const unsigned char* row = p->S + (size_t)n * p->px + (size_t)z * N;
+                    const int a = (u0 >= 0 && u0 < N) ? row[u0] : 0, b = (u0 + 1 >= 0 && u0 + 1 < N) ? row[u0 + 1] : 0;
+                    in = a || b;
+                }
+                S3[((size_t)z * N + y) * N + x] = (unsigned char)in;
+            }
+    return ORACLE_OK;
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* the paper's quality metrics (PRTF, FSC, cut-off at 0.5)   */
 /* ------------------------------------------------------------------------------------------ */

@@ -69,6 +69,8 @@ def _lib(precision: str = "f64"):
         lib.oracle_fft3.argtypes = [vp, vp, ci, ci]
         lib.oracle_align_episode.argtypes = [vp, ci, ci, ci, vp]
         lib.oracle_refine_3d.argtypes = [vp, vp, vp, ci, ci, vp, vp]
+        lib.oracle_refine_3d_sw.argtypes = [vp, vp, vp, ci, ci, ci, cd, cd, vp, vp, vp]
+        lib.oracle_backproject_support.argtypes = [vp, vp]
         lib.oracle_fsc.argtypes = [vp, vp, ci, vp]
         lib.oracle_prtf.argtypes = [vp, vp, vp]
         _LIBS[precision] = lib
@@ -180,6 +182,21 @@ def refine_3d(E, W, S3, k):
     return obj, err
 
 
+def refine_3d_sw(E, W, S3, k, every, sigma, threshold, want_blurred=False):
+    """Step D's iterations with the 3D support re-thresholded every `every` iterations (readings A26, A30): returns
+    (object [N,N,N] complex128, err[k], final support u8 [N,N,N][, the blurred |O| of the last update])."""
+    e = _c128(E)
+    w = np.ascontiguousarray(W, dtype=np.float64)
+    s3 = np.ascontiguousarray(S3, dtype=np.uint8).copy()
+    obj = np.empty_like(e)
+    err = np.empty(int(k), dtype=np.float64)
+    bl = np.zeros(s3.shape, dtype=np.float64) if want_blurred else None
+    _chk(_lib().oracle_refine_3d_sw(e.ctypes.data, w.ctypes.data, s3.ctypes.data, e.shape[-1], int(k), int(every), float(sigma),
+                                    float(threshold), obj.ctypes.data, err.ctypes.data, None if bl is None else bl.ctypes.data),
+         "oracle_refine_3d_sw")
+    return (obj, err, s3, bl) if want_blurred else (obj, err, s3)
+
+
 def align_episode(episode, n_ref=0):
     """Phase gauge and twin chain of one episode (reading A28): returns (aligned copy, flips int32[Np])."""
     e = _c128(episode).copy()
@@ -286,6 +303,12 @@ class Oracle:
         S = np.empty((self.Np, self.N, self.N), dtype=np.uint8)
         _chk(self._l.oracle_get_support(self._h, S.ctypes.data), "oracle_get_support")
         return S
+
+    def backproject_support(self):
+        """The 3D support from the 2D supports and the angles (reading A29): u8 [N, N, N] (z, y, x)."""
+        S3 = np.empty((self.N, self.N, self.N), dtype=np.uint8)
+        _chk(self._l.oracle_backproject_support(self._h, S3.ctypes.data), "oracle_backproject_support")
+        return S3
 
     def prereconstruct(self, n, k, beta=0.9):
         _chk(self._l.oracle_prereconstruct(self._h, int(n), int(k), float(beta)), "oracle_prereconstruct")

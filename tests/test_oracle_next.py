@@ -5,7 +5,7 @@ routine (numpy)."""
 import numpy as np
 
 import cpra_inputs
-from oracle import Oracle, align_episode, blur, center_of_mass, fft3, fsc, mix, mix_seam, refine_3d
+from oracle import Oracle, align_episode, blur, center_of_mass, fft3, fsc, mix, mix_seam, refine_3d, refine_3d_sw
 
 
 def _stack(Np, N, seed):
@@ -361,6 +361,95 @@ def test_refine_3d_at_a_size_that_is_not_a_power_of_two():
     den = (np.abs(E)[W > 0] ** 2).sum()
     assert abs(e2[0] - np.sqrt((np.abs(F1 - E)[W > 0] ** 2).sum() / den)) < 1e-13
     assert abs(e2[1] - np.sqrt((np.abs(np.fft.fftn(want) - E)[W > 0] ** 2).sum() / den)) < 1e-13
+
+
+def test_refine_3d_sw_closed_forms():
+    """Reading A30: the 3D support update inside Step D's iterations, by hand with numpy's FFT."""
+    obj, S3, E, rng = _cube_case()
+    N = obj.shape[0]
+    W = (rng.uniform(size=(N, N, N)) < 0.6).astype(float)
+    # never updating = refine_3d, support untouched
+    o0, e0 = refine_3d(E, W, S3, 4)
+    o1, e1, s1 = refine_3d_sw(E, W, S3, 4, 0, 1.0, 0.1)
+    assert np.array_equal(o0, o1) and np.array_equal(e0, e1) and np.array_equal(s1, S3)
+    o1, e1, s1 = refine_3d_sw(E, W, S3, 4, 4, 1.0, 0.1)          # the only multiple of 4 is the last iteration: no update
+    assert np.array_equal(o0, o1) and np.array_equal(s1, S3)
+    # one update after iteration 2 of 3, sigma = 0: the new support is the threshold of |O_2| itself
+    o2, _ = refine_3d(E, W, S3, 2)
+    thr = 0.2
+    want_s = (np.abs(o2) >= thr * np.abs(o2).max()).astype(np.uint8)
+    o3, e3, s3, b3 = refine_3d_sw(E, W, S3, 3, 2, 0.0, thr, want_blurred=True)
+    clear = np.abs(np.abs(o2) - thr * np.abs(o2).max()) > 1e-12
+    assert np.abs(b3 - np.abs(o2)).max() < 1e-13
+    assert np.array_equal(s3[clear], want_s[clear]) and 0 < s3.sum() < S3.sum()
+    # ... and iteration 3 ran against it: by hand
+    F2 = np.fft.fftn(o2)
+    F = np.where(W > 0, E, F2)
+    want_o = np.fft.ifftn(F) * s3
+    assert np.abs(o3 - want_o).max() < 1e-13
+    assert abs(e3[2] - np.sqrt((np.abs(np.fft.fftn(want_o) - E)[W > 0] ** 2).sum() / (np.abs(E)[W > 0] ** 2).sum())) < 1e-13
+    # sigma > 0: the blur is the 3D Gaussian transfer function (numpy route), real part
+    sig = 1.5
+    _, _, s4, b4 = refine_3d_sw(E, W, S3, 3, 2, sig, thr, want_blurred=True)
+    k = np.fft.fftfreq(N, 1.0 / N)
+    H = np.exp(-2 * np.pi ** 2 * sig ** 2 * (k[:, None, None] ** 2 + k[None, :, None] ** 2 + k[None, None, :] ** 2) / N ** 2)
+    wb = np.fft.ifftn(np.fft.fftn(np.abs(o2)) * H).real
+    assert np.abs(b4 - wb).max() < 1e-13
+    clear = np.abs(wb - thr * wb.max()) > 1e-12
+    assert np.array_equal(s4[clear], (wb >= thr * wb.max()).astype(np.uint8)[clear])
+    assert abs(wb.sum() - np.abs(o2).sum()) < 1e-10               # the blur conserves the mass
+    # nothing left: an all-zero estimate empties the support
+    _, _, s5 = refine_3d_sw(np.zeros_like(E), W, S3, 3, 1, 1.0, 0.1)
+    assert s5.sum() == 0
+
+
+def test_backproject_support_closed_forms(tiny_problem):
+    """Reading A29: the visual hull of the 2D supports."""
+    N = 32
+    c = N // 2
+    def plan(S, angles):
+        o = Oracle(N, len(angles))
+        o.set_data(np.ones((len(angles), N, N)), None, np.asarray(angles, float))
+        o.set_support(S)
+        return o
+    yy, xx = np.meshgrid(np.arange(N) - c, np.arange(N) - c, indexing="ij")
+    rad = np.hypot(yy, xx)
+    # full supports: everything whose footprint stays on the detector at every angle (the inscribed cylinder) stays
+    full = plan(np.ones((3, N, N), np.uint8), [0.0, 0.7, 2.0]).backproject_support()
+    assert full[:, rad <= c - 1].all() and np.array_equal(full[0], full[N - 1])
+    assert plan(np.ones((1, N, N), np.uint8), [0.0]).backproject_support()[:, :, :N - 1].all()
+    # one projection at 0 degrees: S3[z][y][x] = S[z][x] or S[z][x + 1] for every y (u = x exactly: the footprint rule
+    # looks at columns u and u + 1); at 90 degrees u = y
+    rng = np.random.default_rng(4)
+    S = (rng.uniform(size=(1, N, N)) < 0.3).astype(np.uint8)
+    dil = S[0] | np.concatenate([S[0][:, 1:], np.zeros((N, 1), np.uint8)], axis=1)
+    s3 = plan(S, [0.0]).backproject_support()
+    assert np.array_equal(s3, np.broadcast_to(dil[:, None, :], (N, N, N)))
+    s3 = plan(S, [np.pi / 2]).backproject_support()
+    # cos(pi/2) = 6e-17: u = y up to rounding, so columns y and y + 1 (or y - 1 and y) are looked at: the hull contains S[z][y]
+    assert np.all(s3[:, :, :][np.broadcast_to(S[0][:, :, None].astype(bool), (N, N, N))])
+    # a strip |u - c| <= r at many angles: the hull is the cylinder of radius r (up to the one-pixel footprint)
+    r = 6
+    strip = np.zeros((N, N), np.uint8)
+    strip[:, c - r:c + r + 1] = 1
+    angles = np.linspace(0, np.pi, 36, endpoint=False)
+    s3 = plan(np.broadcast_to(strip, (36, N, N)).copy(), angles).backproject_support()
+    assert s3[:, rad <= r - 0.5].all() and not s3[:, rad >= r + 1.5].any()
+    # an empty row z in one projection empties the slab z
+    S2 = np.ones((4, N, N), np.uint8)
+    S2[2, 5, :] = 0
+    s3 = plan(S2, [0.0, 0.5, 1.0, 1.5]).backproject_support()
+    assert not s3[5].any() and s3[4][rad <= c - 1].all() and s3[6][rad <= c - 1].all()
+    # physics: the supports of an object's true projections contain the object
+    p = tiny_problem
+    o = Oracle(p.N, p.Np)
+    o.set_data(np.ones((p.Np, p.N, p.N)), None, p.angles)
+    o.set_support((np.abs(p.projections) > 0).astype(np.uint8))
+    hull = o.backproject_support()
+    pad = np.zeros((p.N,) * 3)
+    off = (p.N - p.obj.shape[0]) // 2
+    pad[off:off + p.obj.shape[0], off:off + p.obj.shape[0], off:off + p.obj.shape[0]] = np.abs(p.obj)
+    assert hull[pad > 0].all() and hull.sum() < 0.5 * p.N ** 3          # (every voxel adds a positive amount to its footprint)
 
 
 def test_refine_3d_error_never_increases_and_recovers_the_object():
