@@ -311,6 +311,35 @@ int cpra_refine_3d(cpra_plan_t plan, const float* d_E, const float* d_W, const u
                    float* d_obj, float* d_err);
 
 /*
+ * cpra_refine_3d with the support update of P:104 ("We shrink the 3D space constraint every 5 iterations, leading to a
+ * tighter 3D space constraint close to the shape of the object at the end"; reading A30): after every
+ * `every`-th iteration that is not the last, the 3D analogue of cpra_shrinkwrap,
+ *     b = G_sigma * |O|  (product with exp(-2 pi^2 sigma^2 |k|^2 / N^2) between a forward and an inverse 3D transform),
+ *     S3 <- [ b >= threshold . max b ]   (all zero if the maximum is not positive).
+ *   d_S3       u8 [N][N][N] IN and OUT: the support the iterations start from; on return the support of the last update
+ *   every      >= 1: update after iterations every, 2 every, ... (< k);  < 1: never (= cpra_refine_3d)
+ *   sigma      standard deviation of the Gaussian in voxels, >= 0;  threshold: fraction of the maximum, >= 0
+ *   d_blurred  fp32 [N][N][N] out or NULL: the b of the last update (diagnostic; untouched if no update ran)
+ * Other arguments, scratch use and the plan (Np == N) as for cpra_refine_3d; the second spectrum buffer is used too.
+ * Errors: INVALID_ARG (as cpra_refine_3d; sigma or threshold negative / not finite), WORKSPACE, CUDA.
+ */
+int cpra_refine_3d_sw(cpra_plan_t plan, const float* d_E, const float* d_W, unsigned char* d_S3, int k, int every, float sigma,
+                      float threshold, float* d_obj, float* d_err, float* d_blurred);
+
+/*
+ * The 3D support of Step D from the 2D supports ("We project the 2D space constrains back to the 3D space to form
+ * a relatively tight 3D space constraint"; reading A29): the visual hull.  With the geometry of the projections
+ * (rotation about z; image rows = z, columns = u; the angles of cpra_set_data) voxel (z, y, x) lands on row z at
+ *     u_n = c + (x - c) cos theta_n + (y - c) sin theta_n,   c = N / 2,
+ * and stays iff in EVERY projection n S_n[z][floor(u_n)] or S_n[z][floor(u_n) + 1] is set (columns outside the detector
+ * count as outside).  u_n is evaluated in double, one rounding per product and sum.
+ *   d_S3  u8 [N][N][N] (z, y, x) out, caller-owned.
+ * Uses the plan's current 2D supports (cpra_set_support, or the last cpra_shrinkwrap) and the second spectrum buffer.
+ * Errors: INVALID_ARG, NOT_READY (no support), WORKSPACE, CUDA.
+ */
+int cpra_backproject_support(cpra_plan_t plan, unsigned char* d_S3);
+
+/*
  * The paper's quality metrics ("PRTF", "FSC", resolution at the 0.5 cut-off).
  *   cpra_fsc   Fourier shell correlation of two 3D spectra d_F1, d_F2 (complex fp32 [N][N][N], native order; a
  *              plan with Np == N):  FSC(s) = Re sum_s F1 conj(F2) / sqrt(sum_s |F1|^2 sum_s |F2|^2), shell

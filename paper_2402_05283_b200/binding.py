@@ -62,6 +62,8 @@ SIGNATURES = {
     "cpra_align_episode": (_ci, [_vp, _vp, _ci, _vp]),
     "cpra_fft3": (_ci, [_vp, _vp, _vp, _ci]),
     "cpra_refine_3d": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp, _vp]),
+    "cpra_refine_3d_sw": (_ci, [_vp, _vp, _vp, _vp, _ci, _ci, _cf, _cf, _vp, _vp, _vp]),
+    "cpra_backproject_support": (_ci, [_vp, _vp]),
     "cpra_fsc": (_ci, [_vp, _vp, _vp, _vp]),
     "cpra_prtf": (_ci, [_vp, _vp, _vp]),
     "cpra_fsc_static": (_ci, [_ci, _vp, _vp, _vp, _vp]),
@@ -342,6 +344,27 @@ class Plan:
         _chk(self._l.cpra_refine_3d(self._h, _dptr(E, torch.complex64, n3), _dptr(W, torch.float32, n3), _dptr(S3, torch.uint8, n3),
                                     int(k), obj.data_ptr(), err.data_ptr()), "cpra_refine_3d")
         return obj, err
+
+    def refine_3d_sw(self, E, W, S3, k: int, every: int, sigma: float, threshold: float, want_blurred: bool = False):
+        """cpra_refine_3d_sw: returns (object complex64 [N, N, N], err float32 [k], support u8 [N, N, N] after the last
+        update[, blurred float32 [N, N, N]]).  S3 is copied: the caller's tensor is not modified."""
+        import torch
+        n3 = self.N ** 3
+        obj = torch.empty((self.N, self.N, self.N), dtype=torch.complex64, device=self.device)
+        err = torch.empty(int(k), dtype=torch.float32, device=self.device)
+        s3 = S3.clone().contiguous()
+        bl = torch.zeros((self.N, self.N, self.N), dtype=torch.float32, device=self.device) if want_blurred else None
+        _chk(self._l.cpra_refine_3d_sw(self._h, _dptr(E, torch.complex64, n3), _dptr(W, torch.float32, n3), _dptr(s3, torch.uint8, n3),
+                                       int(k), int(every), float(sigma), float(threshold), obj.data_ptr(), err.data_ptr(),
+                                       None if bl is None else bl.data_ptr()), "cpra_refine_3d_sw")
+        return (obj, err, s3, bl) if want_blurred else (obj, err, s3)
+
+    def backproject_support(self):
+        """cpra_backproject_support: the visual hull of the current 2D supports, u8 [N, N, N] (z, y, x)."""
+        import torch
+        S3 = torch.empty((self.N, self.N, self.N), dtype=torch.uint8, device=self.device)
+        _chk(self._l.cpra_backproject_support(self._h, S3.data_ptr()), "cpra_backproject_support")
+        return S3
 
     def fsc(self, F1, F2):
         import torch

@@ -694,6 +694,77 @@ int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsi
     return rc;
 }
 
+int cpra_refine_3d_sw(cpra_plan_t p, const float* d_E, const float* d_W, unsigned char* d_S3, int k, int every, float sigma, float threshold,
+                      float* d_obj, float* d_err, float* d_blurred)
+{
+    if (!p || !d_E || !d_W || !d_S3 || !d_obj || k < 1 || !(sigma >= 0.f) || !(threshold >= 0.f) || !std::isfinite(sigma) ||
+        !std::isfinite(threshold))
+        return CPRA_ERR_INVALID_ARG;
+    if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    const int nblk = (int)std::min<size_t>(512, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
+    if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
+    float2* T = (float2*)p->st[p->cur];   // F, then F' (cpra_fft3 itself uses the other state buffer and the scratch)
+    float2* B = (float2*)p->scr2;         // the blurred |O| of a support update (no transform touches the second scratch)
+    double* num = p->partial;
+    double* den = p->partial + nblk;
+    k_refine_init<<<nblk, 256, 0, p->stream>>>((const float2*)d_E, d_W, T, den, n3);
+    int rc = check_launch(p);
+    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
+        if ((rc = cpra_fft3(p, (const float*)T, d_obj, +1))) break;
+        k_refine_support<<<blocks_for(n3, 256), 256, 0, p->stream>>>((float2*)d_obj, d_S3, n3);
+        if ((rc = check_launch(p))) break;
+        if ((rc = cpra_fft3(p, d_obj, (float*)T, -1))) break;
+        k_refine_replace<<<nblk, 256, 0, p->stream>>>(T, (const float2*)d_E, d_W, num, n3);
+        if ((rc = check_launch(p))) break;
+        if (d_err) {
+            k_refine_error<<<1, 1, 0, p->stream>>>(num, den, nblk, d_err + it);
+            if ((rc = check_launch(p))) break;
+        }
+        if (every >= 1 && (it + 1) % every == 0 && it + 1 < k) {
+            // S3 <- [ G_sigma * |O| >= threshold max ]  (readings A23, A30)
+            k_abs3<<<blocks_for(n3, 256), 256, 0, p->stream>>>((const float2*)d_obj, B, n3);
+            if ((rc = check_launch(p))) break;
+            if ((rc = cpra_fft3(p, (const float*)B, (float*)B, -1))) break;
+            k_gauss3<<<blocks_for(n3, 256), 256, 0, p->stream>>>(B, p->N, n3, sigma);
+            if ((rc = check_launch(p))) break;
+            if ((rc = cpra_fft3(p, (const float*)B, (float*)B, +1))) break;
+            k_plane_max<<<p->N, 256, 0, p->stream>>>(B, p->mx, (size_t)p->N * p->N);
+            if ((rc = check_launch(p))) break;
+            k_max_final<<<1, 256, 0, p->stream>>>(p->mx, p->N);
+            if ((rc = check_launch(p))) break;
+            k_threshold3<<<blocks_for(n3, 256), 256, 0, p->stream>>>(B, p->mx, d_S3, d_blurred, n3, threshold);
+            rc = check_launch(p);
+        }
+    }
+    p->have_estimate = false;   // the state buffers were used as scratch
+    p->have_error = false;
+    return rc;
+}
+
+int cpra_backproject_support(cpra_plan_t p, unsigned char* d_S3)
+{
+    if (!p || !d_S3) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    if (!p->have_support) return CPRA_ERR_NOT_READY;
+    const size_t total = (size_t)p->Np * p->N * p->N, n3 = (size_t)p->N * p->N * p->N;
+    // the 2D supports as bytes: this path's own copy, or unpacked into the second scratch
+    const unsigned char* S = p->S8;
+    if (!p->generic) {
+        unsigned char* u8 = (unsigned char*)p->scr2;
+        k_unpack_support<<<blocks_for(total, 256), 256, 0, p->stream>>>(p->S16, u8, p->N, total);
+        if (int rc = check_launch(p)) return rc;
+        S = u8;
+    }
+    p->h_cs.resize(2 * (size_t)p->Np);
+    for (int n = 0; n < p->Np; ++n) { p->h_cs[2 * n] = std::cos(p->angles[n]); p->h_cs[2 * n + 1] = std::sin(p->angles[n]); }
+    double* cs = p->align;   // 9 Np doubles of scratch, free between calls
+    if (cudaMemcpyAsync(cs, p->h_cs.data(), sizeof(double) * 2 * p->Np, cudaMemcpyHostToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    k_backproject_support<<<blocks_for(n3, 256), 256, 0, p->stream>>>(S, cs, d_S3, p->N, p->Np);
+    return check_launch(p);
+}
+
 int cpra_fsc(cpra_plan_t p, const float* d_F1, const float* d_F2, float* d_out)
 {
     if (!p || !d_F1 || !d_F2 || !d_out) return CPRA_ERR_INVALID_ARG;

@@ -314,6 +314,88 @@ __global__ void k_refine_error(const double* __restrict__ num, const double* __r
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Step D's support (readings A29, A30), on natural [z][y][x] volumes.
+// ---------------------------------------------------------------------------------------------------
+// The visual hull of the 2D supports: S u8 [Np][N][N] (rows = z, columns = u), cs = (cos theta_n, sin theta_n) doubles.
+// Voxel (z, y, x) stays iff for every n S_n[z][floor(u)] or S_n[z][floor(u) + 1] is set, u = c + (x - c) cos + (y - c) sin
+// evaluated in double without contraction (the products and sums of the definition, one rounding each).
+__global__ void k_backproject_support(const unsigned char* __restrict__ S, const double* __restrict__ cs, unsigned char* __restrict__ S3, int N, int Np)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t n3 = (size_t)N * N * N;
+    if (i >= n3) return;
+    const int x = (int)(i % N), y = (int)((i / N) % N), z = (int)(i / ((size_t)N * N)), c = N / 2;
+    const double dx = (double)(x - c), dy = (double)(y - c);
+    int in = 1;
+    for (int n = 0; n < Np && in; ++n) {
+        const double u = __dadd_rn(__dadd_rn((double)c, __dmul_rn(dx, cs[2 * n])), __dmul_rn(dy, cs[2 * n + 1]));
+        const long u0 = (long)floor(u);
+        const unsigned char* __restrict__ row = S + ((size_t)n * N + z) * N;
+        const int a = (u0 >= 0 && u0 < N) ? row[u0] : 0, b = (u0 + 1 >= 0 && u0 + 1 < N) ? row[u0 + 1] : 0;
+        in = a || b;
+    }
+    S3[i] = (unsigned char)in;
+}
+// (|O|, 0)
+__global__ void k_abs3(const float2* __restrict__ O, float2* __restrict__ out, size_t n3)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n3) return;
+    const float2 v = O[i];
+    out[i] = make_float2(sqrtf(v.x * v.x + v.y * v.y), 0.f);
+}
+// natural 3D spectrum *= exp(-2 pi^2 sigma^2 |k|^2 / N^2)
+__global__ void k_gauss3(float2* __restrict__ F, int N, size_t n3, float sigma)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n3) return;
+    const int ix = (int)(i % N), iy = (int)((i / N) % N), iz = (int)(i / ((size_t)N * N));
+    const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N, kz = iz < N / 2 ? iz : iz - N;
+    const double s = (double)sigma;
+    const float f = (float)exp(-2.0 * 9.86960440108935861883 * s * s * ((double)kz * kz + (double)ky * ky + (double)kx * kx) / ((double)N * N));
+    F[i].x *= f;
+    F[i].y *= f;
+}
+// maximum of the real part of every z plane (one block per plane), then of the planes (one block): mx[0]
+__global__ void k_plane_max(const float2* __restrict__ v, float* __restrict__ mx, size_t px)
+{
+    const float2* __restrict__ p = v + (size_t)blockIdx.x * px;
+    float m = -3.402823466e38f;
+    for (size_t i = threadIdx.x; i < px; i += blockDim.x) m = fmaxf(m, p[i].x);
+    __shared__ float red[32];
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, red[w]);
+        mx[blockIdx.x] = m;
+    }
+}
+__global__ void k_max_final(float* __restrict__ mx, int n)
+{
+    float m = -3.402823466e38f;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) m = fmaxf(m, mx[i]);
+    __shared__ float red[32];
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();   // every thread has read its share of mx before mx[0] is overwritten
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, red[w]);
+        mx[0] = m;
+    }
+}
+// S3 <- [ b >= threshold max b ], max b = mx[0] > 0; blurred (optional): b
+__global__ void k_threshold3(const float2* __restrict__ b, const float* __restrict__ mx, unsigned char* __restrict__ S3,
+                             float* __restrict__ blurred, size_t n3, float threshold)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n3) return;
+    const float m = mx[0], v = b[i].x;
+    S3[i] = (m > 0.f && v >= threshold * m) ? 1 : 0;
+    if (blurred) blurred[i] = v;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // f4: the paper's quality metrics: Fourier shell correlation and PRTF.
 // Shell sums are accumulated per block in shared memory and added to the global shell accumulators with
 // double atomics (the order of the additions varies from run to run at the 1e-16 level).

@@ -67,6 +67,7 @@ struct cpra_plan_s {
     std::vector<float2> h_tw;
     std::vector<double> h_uphi;
     std::vector<int> h_ustart, h_rays;
+    std::vector<double> h_cs;         // (cos theta_n, sin theta_n) of cpra_backproject_support
     long launches = 0;
     int chunk = 0;  // images per L2-resident chunk; 0 = all
     int sms = 148;     // SMs of the device

@@ -9,7 +9,9 @@
             then cpra_align_episode: the projections of the merged episode are given one common phase gauge and one
             twin choice (reading A28) -- without it the slices of an unconstrained complex iterate do not fit together
     Step D  Fourier-slice assembly of the merged episode (cpra_assemble_3d), then optionally the inverse 3D
-            transform / the iterations against a 3D support (cpra_fft3 / cpra_refine_3d)
+            transform / the iterations against a 3D support (cpra_fft3 / cpra_refine_3d / cpra_refine_3d_sw); the 3D
+            support is the caller's or the back-projection of the merged episode's 2D supports (cpra_shrinkwrap on the
+            merged episode, then cpra_backproject_support: PAPER.md:104)
 
 Every arithmetic step runs in the library's kernels; this module only allocates torch tensors, draws the random
 starting phases (torch's generator on the device: input generation, not part of the method) and calls the binding."""
@@ -33,6 +35,7 @@ class CpraResult:
     weight: "object" = None      # float32 [N, N, N]
     obj: "object" = None         # complex64 [N, N, N], O(r) if a 3D step was asked for
     refine_error: "object" = None
+    support3d: "object" = None   # u8 [N, N, N]: the 3D support Step D ended with
     seconds: dict = None
 
 
@@ -56,11 +59,14 @@ def random_phase_starts(plan, intensity, mask, seed: int):
 def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, n_pre: int, n_episodes: int, n_ei: int,
                 beta: float = 0.9, alpha=(0.6, 0.2), update: str = "hio", seam_flip: bool = False, seed: int = 0,
                 shrinkwrap: Optional[tuple] = None, assemble: bool = True, support3d=None, refine_iters: int = 0,
-                n_ref: int = 0, align: bool = True, step3d: bool = True) -> CpraResult:
+                n_ref: int = 0, align: bool = True, step3d: bool = True, shrink3d: Optional[tuple] = None,
+                support2d_for_3d: tuple = (2.0, 0.08)) -> CpraResult:
     """Steps A-D.  intensity fp32 [Np, N, N], mask u8 [Np, N, N] or None, support u8 [Np, N, N]: CUDA tensors;
     angles: Np radians (host).  shrinkwrap = (sigma, threshold): one support update at the end of every episode
-    (PAPER.md:104).  support3d u8 [N, N, N] + refine_iters > 0: Step D's iterations; refine_iters == 0 with assemble:
-    E(q) and O(r) = F3^-1[E] (step3d=False: E(q) only)."""
+    (PAPER.md:104).  refine_iters > 0: Step D's iterations against support3d (u8 [N, N, N]) or, if that is None, against
+    the back-projection of the 2D supports that a shrink-wrap with support2d_for_3d = (sigma, threshold) finds on the
+    merged episode; shrink3d = (every, sigma, threshold): the 3D support is re-thresholded every `every` iterations
+    (PAPER.md:104).  refine_iters == 0 with assemble: E(q) and O(r) = F3^-1[E] (step3d=False: E(q) only)."""
     import torch
     Np, N = int(intensity.shape[0]), int(intensity.shape[-1])
     dev = intensity.device
@@ -131,10 +137,19 @@ def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, 
         timed("assemble", t0)
         if step3d:
             t0 = start()
+            if refine_iters > 0 and support3d is None:
+                # the 2D supports of the merged projections, projected back
+                plan.shrinkwrap(float(support2d_for_3d[0]), float(support2d_for_3d[1]))
+                support3d = plan.backproject_support()
             plan.close()
             p3 = binding.Plan(N, N)
-            if refine_iters > 0 and support3d is not None:
-                res.obj, res.refine_error = p3.refine_3d(res.spectrum, res.weight, support3d, refine_iters)
+            if refine_iters > 0:
+                if shrink3d is not None:
+                    res.obj, res.refine_error, res.support3d = p3.refine_3d_sw(res.spectrum, res.weight, support3d, refine_iters,
+                                                                               int(shrink3d[0]), float(shrink3d[1]), float(shrink3d[2]))
+                else:
+                    res.obj, res.refine_error = p3.refine_3d(res.spectrum, res.weight, support3d, refine_iters)
+                    res.support3d = support3d
             else:
                 res.obj = p3.fft3(res.spectrum, +1)
             p3.close()

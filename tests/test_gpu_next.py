@@ -324,6 +324,75 @@ def test_refine_3d(torch_cuda, N):
     assert np.abs(rg.cpu().numpy()[S3 == 0]).max() == 0.0
 
 
+@pytest.mark.parametrize("N", [32, 64, 48])
+def test_refine_3d_sw(torch_cuda, N):
+    """Step D's iterations with the support re-thresholded every 2 iterations (reading A30), device vs oracle.  The
+    threshold is taken in fp32 on the device and in fp64 by the oracle: voxels whose blurred value lies within
+    rounding of it are set aside for the comparison of the support; the test data keep them out of the way."""
+    import paper_2402_05283_b200 as cpra
+    from oracle import refine_3d_sw
+    rng = np.random.default_rng(N)
+    h = N // 2
+    a = max(2, N // 6)
+    obj = np.zeros((N, N, N), np.complex64)
+    obj[h - a:h + a, h - a + 1:h + a, h - a:h + a - 1] = (rng.uniform(0.3, 1.0, size=(2 * a, 2 * a - 1, 2 * a - 1)) *
+                                                          np.exp(1j * rng.uniform(0, 1, size=(2 * a, 2 * a - 1, 2 * a - 1)))).astype(np.complex64)
+    S3 = np.zeros((N, N, N), np.uint8)
+    S3[h - a - 3:h + a + 3, h - a - 2:h + a + 3, h - a - 3:h + a + 2] = 1
+    E = np.fft.fftn(obj.astype(np.complex128)).astype(np.complex64)
+    W = (rng.uniform(size=(N, N, N)) < 0.7).astype(np.float32)
+    k, every, sig, thr = 5, 2, 1.0, 0.12
+    plan = cpra.Plan(N, N)
+    dE, dW, dS = (torch_cuda.from_numpy(x).cuda() for x in (E, W, S3))
+    # one update (after iteration 2 of 3): the blurred volumes agree, the supports agree away from the threshold
+    og, eg, sg, bg = plan.refine_3d_sw(dE, dW, dS, 3, every, sig, thr, want_blurred=True)
+    oo, eo, so, bo = refine_3d_sw(E, W, S3, 3, every, sig, thr, want_blurred=True)
+    assert np.abs(bg.cpu().numpy() - bo).max() <= 2e-5 * bo.max()
+    clear = np.abs(bo - thr * bo.max()) > 5e-5 * bo.max()
+    assert np.array_equal(sg.cpu().numpy()[clear], so[clear]) and (~clear).mean() < 2e-3
+    assert 0 < so.sum() < S3.sum()
+    assert np.array_equal(dS.cpu().numpy(), S3)                      # the caller's tensor is untouched by the binding
+    # the full run, continued on both sides from the SAME support history: feed the device's support of each update
+    # back through a run of its own (k = 5: updates after iterations 2 and 4)
+    og, eg, sg = plan.refine_3d_sw(dE, dW, dS, k, every, sig, thr)
+    oo, eo, so = refine_3d_sw(E, W, S3, k, every, sig, thr)
+    same = np.array_equal(sg.cpu().numpy(), so)
+    if same:                                                         # no voxel sat on the threshold: everything is comparable
+        assert rel_l2(og.cpu().numpy(), oo) <= 3 * TOL_1
+        assert np.abs(eg.cpu().numpy() - eo).max() <= TOL_E * eo.max()
+    else:
+        assert (sg.cpu().numpy() != so).mean() < 1e-3
+    assert np.abs(og.cpu().numpy()[sg.cpu().numpy() == 0]).max() == 0.0
+    # every = 0 is cpra_refine_3d
+    o1, e1 = plan.refine_3d(dE, dW, dS, 3)
+    o2, e2, s2 = plan.refine_3d_sw(dE, dW, dS, 3, 0, sig, thr)
+    assert torch_cuda.equal(o1, o2) and torch_cuda.equal(e1, e2) and torch_cuda.equal(s2, dS)
+    with pytest.raises(cpra.CpraError) as e:
+        plan.refine_3d_sw(dE, dW, dS, 3, 1, -1.0, thr)
+    assert e.value.code == cpra.ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("cfg,Np,N", [(1, 8, None), (4, 6, 128), (1, 5, 160), (3, 6, None)])
+def test_backproject_support(torch_cuda, cfg, Np, N):
+    """The visual hull of the 2D supports (reading A29), device vs oracle, bit for bit (u is evaluated in double on
+    both sides with the same roundings), through both support layouts (bit-packed / bytes)."""
+    p = cpra_inputs.make_problem(cfg, Np=Np, N=N, keep_object=True)
+    o, g = _oracle(p), _gpu(p)
+    ho, hg = o.backproject_support(), g.backproject_support().cpu().numpy()
+    assert np.array_equal(ho, hg)
+    assert 0 < hg.sum() < p.N ** 3 // 2
+    # tighter supports: the silhouettes of the true projections; the hull contains the object
+    S = (np.abs(p.projections) > 0).astype(np.uint8)
+    o.set_support(S)
+    g.set_support(torch_cuda.from_numpy(S).cuda())
+    ho, hg = o.backproject_support(), g.backproject_support().cpu().numpy()
+    assert np.array_equal(ho, hg)
+    pad = np.zeros((p.N,) * 3)
+    off = (p.N - p.obj.shape[0]) // 2
+    pad[off:off + p.obj.shape[0], off:off + p.obj.shape[0], off:off + p.obj.shape[0]] = np.abs(p.obj)
+    assert hg[pad > 0].all()
+
+
 @pytest.mark.parametrize("N", [16, 64, 128])
 def test_fsc(torch_cuda, N):
     import paper_2402_05283_b200 as cpra
@@ -500,3 +569,16 @@ def test_pipeline_steps_a_to_d(torch_cuda):
     print(f"\npipeline: corr2d={c2:.3f} corr3d={c3:.3f} errors={res.errors.cpu().numpy()} seconds={res.seconds}")
     assert c3 > 0.8, c3
     assert len(res.errors) == 3 and float(res.errors.max()) < 0.2
+    # Step D as PAPER.md:104 has it: 3D iterations against the back-projected 2D supports of the merged episode, the 3D
+    # support re-thresholded every 5 iterations
+    res = cpra.pipeline.reconstruct(I, M, S, p.angles, n_restarts=6, n_keep=3, n_pre=200, n_episodes=25, n_ei=2, seam_flip=True,
+                                    refine_iters=20, shrink3d=(5, 1.5, 0.1))
+    rec, s3 = res.obj.cpu().numpy(), res.support3d.cpu().numpy().astype(bool)
+    both = [(np.abs(rec), s3), (np.abs(rec[i][:, i][:, :, i]), s3[i][:, i][:, :, i])]
+    c3r, s3b = max(((corr(r, pad), m) for r, m in both), key=lambda t: t[0])
+    inside = pad[s3b].sum() / pad.sum()
+    print(f"pipeline + 3D iterations: corr3d={c3r:.3f} object mass inside the final 3D support={inside:.3f} "
+          f"support voxels={int(s3.sum())} of {N ** 3} refine error {float(res.refine_error[0]):.3f} -> {float(res.refine_error[-1]):.3f}")
+    assert c3r > 0.8, c3r
+    assert inside > 0.9 and s3.sum() < 0.3 * N ** 3
+    assert np.abs(rec[~s3]).max() == 0.0
