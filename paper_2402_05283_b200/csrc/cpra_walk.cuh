@@ -350,11 +350,15 @@ k_row_walk(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             if (i == 0) {   // the first halo tile is only needed in registers: its slot takes the tile of m_3 at once
 #pragma unroll
                 for (int r = 0; r < E0; ++r) gm[r] = v[r];
+                // A(0) wrote the halo's new state into slot 0 with ordinary stores: they must be ordered before the
+                // asynchronous-proxy writes of the copy that refills the slot (a barrier alone does not order the two proxies)
+                fence_async_smem();
                 __syncthreads();   // every thread is done with slot 0
                 if (io && 3 <= len + 1) load_tile(proj(3), rt, 0);
             }
             if (i >= 2) stepB(i - 1);
         }
+        fence_async_smem();   // the ordinary stores of the last A (the halo's new state) before the next run's copies into the slots
         if (io) bulk_wait_read0();
         __syncthreads();   // the last store has been read out (warp 0 waited) before the next run reloads the slots
         u += len;

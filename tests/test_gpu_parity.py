@@ -422,6 +422,32 @@ def test_walk_and_tile_kernel_paths_agree(torch_cuda, N, n_ei):
     assert abs(Ega - Egb) <= 1e-5 * Egb
 
 
+@pytest.mark.parametrize("N,Np,ctas", [(256, 180, 0), (256, 90, 6), (512, 60, 8), (1024, 20, 1)])
+def test_walk_short_runs_repeat_exactly(torch_cuda, N, Np, ctas):
+    """Many short runs per launch (every run start refills a slot that ordinary stores have just written: the order of
+    the two memory proxies there needs a fence, and without it one launch in a few went wrong).  The same two iterations
+    twenty times over, with the allocator churned in between: every repetition equals the first bit for bit, and the
+    first agrees with the three tile kernels."""
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(N, Np, seed=N + Np, beamstop=3)
+
+    def run(flags=0):
+        plan = cpra.Plan(N, Np, flags=flags).load(p)
+        if ctas:
+            plan.set_walk_ctas(ctas)
+        plan.iterate(2, 0.9)
+        out = plan.get_projections(0)
+        plan.close()
+        return out
+    ref = run(cpra.FLAG_NO_WALK)
+    first = run()
+    assert rel_l2(first.cpu().numpy(), ref.cpu().numpy()) <= 2e-6
+    for rep in range(20):
+        junk = torch_cuda.empty(int(5e8), dtype=torch_cuda.uint8, device="cuda").random_()
+        del junk
+        assert torch_cuda.equal(run(), first), rep
+
+
 @pytest.mark.parametrize("N,Np", [(16, 1), (16, 2), (32, 3), (64, 1), (128, 5), (256, 2), (512, 1), (1024, 1)])
 def test_small_and_ragged_stacks(torch_cuda, N, Np):
     """Np = 1 and 2 (no room for K = 1: default falls back to no coupling), Np = 3 (every image is
