@@ -60,7 +60,7 @@ def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, 
                 beta: float = 0.9, alpha=(0.6, 0.2), update: str = "hio", seam_flip: bool = False, seed: int = 0,
                 shrinkwrap: Optional[tuple] = None, assemble: bool = True, support3d=None, refine_iters: int = 0,
                 n_ref: int = 0, align: bool = True, step3d: bool = True, shrink3d: Optional[tuple] = None,
-                support2d_for_3d: tuple = (2.0, 0.08)) -> CpraResult:
+                support2d_for_3d: tuple = (3.0, 0.03)) -> CpraResult:
     """Steps A-D.  intensity fp32 [Np, N, N], mask u8 [Np, N, N] or None, support u8 [Np, N, N]: CUDA tensors;
     angles: Np radians (host).  shrinkwrap = (sigma, threshold): one support update at the end of every episode
     (PAPER.md:104).  refine_iters > 0: Step D's iterations against support3d (u8 [N, N, N]) or, if that is None, against

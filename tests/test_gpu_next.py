@@ -572,7 +572,7 @@ def test_pipeline_steps_a_to_d(torch_cuda):
     # Step D as PAPER.md:104 has it: 3D iterations against the back-projected 2D supports of the merged episode, the 3D
     # support re-thresholded every 5 iterations
     res = cpra.pipeline.reconstruct(I, M, S, p.angles, n_restarts=6, n_keep=3, n_pre=200, n_episodes=25, n_ei=2, seam_flip=True,
-                                    refine_iters=20, shrink3d=(5, 1.5, 0.1))
+                                    refine_iters=20, shrink3d=(5, 2.0, 0.05))
     rec, s3 = res.obj.cpu().numpy(), res.support3d.cpu().numpy().astype(bool)
     both = [(np.abs(rec), s3), (np.abs(rec[i][:, i][:, :, i]), s3[i][:, i][:, :, i])]
     c3r, s3b = max(((corr(r, pad), m) for r, m in both), key=lambda t: t[0])
