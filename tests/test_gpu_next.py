@@ -442,6 +442,34 @@ def test_fft2_mixed_radix(torch_cuda, N):
     assert np.abs(Fd[1] - np.exp(-2j * np.pi * (3 * ky + 5 * kx) / N)).max() < 2e-5
 
 
+def test_fft2_every_supported_mixed_radix_size(torch_cuda):
+    """Every even N in [16, 1024] with prime factors 2, 3, 5, 7 that is not a power of two (every combination of stage
+    radices, ragged last tiles on both tile widths): forward transform of one random image against numpy, round trip."""
+    import paper_2402_05283_b200 as cpra
+    sizes = []
+    for N in range(16, 1025, 2):
+        n = N
+        for f in (2, 3, 5, 7):
+            while n % f == 0:
+                n //= f
+        if n == 1 and N & (N - 1):
+            sizes.append(N)
+    assert len(sizes) > 60 and 160 in sizes and 700 in sizes
+    rng = np.random.default_rng(9)
+    worst = 0.0
+    for N in sizes:
+        x = (rng.normal(size=(1, N, N)) + 1j * rng.normal(size=(1, N, N))).astype(np.complex64)
+        plan = cpra.Plan(N, 1)
+        d = torch_cuda.from_numpy(x).cuda()
+        F = plan.fft2(d, -1)
+        e = rel_l2(F.cpu().numpy(), np.fft.fft2(x.astype(np.complex128)))
+        b = rel_l2(plan.fft2(F, +1).cpu().numpy(), x)
+        plan.close()
+        worst = max(worst, e, b)
+        assert e < 3e-6 and b < 4e-6, (N, e, b)
+    print(f"\n{len(sizes)} mixed-radix sizes, worst relL2 {worst:.2e}")
+
+
 @pytest.mark.parametrize("N,Np,alpha,n_ei,seam,rule", [
     (160, 6, (0.6, 0.2), 1, 0, "hio"), (160, 5, (0.5, 0.2, 0.05), 2, 1, "raar"), (48, 7, (0.6, 0.2), 1, 1, "hio"),
     (100, 3, (0.6, 0.2), 3, 0, "er"), (700, 3, (0.6, 0.2), 1, 0, "hio"), (20, 1, (1.0,), 1, 0, "hio"),
