@@ -40,11 +40,13 @@ int gen_set_attrs()
     auto acc = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     const int SM = 200 * 1024;
     acc(allow_smem(k_gen_row_fwd, SM));
-    acc(allow_smem(k_gen_col, SM));
+    acc(allow_smem(k_gen_col<false>, SM));
+    acc(allow_smem(k_gen_col<true>, SM));
     acc(allow_smem(k_gen_row_inv, SM));
     // as much shared memory as the SM has, whatever one block asks for (the default carveout fits fewer blocks)
     acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_row_fwd), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<false>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<true>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_row_inv), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
 }
@@ -64,7 +66,7 @@ int row_fwd(cpra_plan_s* p, const float2* cur, int n0, int nimg, bool fires, boo
 int col(cpra_plan_s* p, int n0, int nimg, int mode, float scale)
 {
     ProfScope prof(p, CPRA_PROFILE_COL);
-    k_gen_col<<<(unsigned)(nimg * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, mode, scale,
+    k_gen_col<false><<<(unsigned)(nimg * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, mode, scale,
                                                                                   (size_t)p->N * p->N, (size_t)p->N);
     return check_launch(p);
 }
@@ -165,7 +167,7 @@ int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign)
 int gen_fftz(cpra_plan_s* p, float2* vol, int sign)
 {
     const size_t N = (size_t)p->N;
-    k_gen_col<<<(unsigned)(p->N * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>(vol, nullptr, p->tw, nullptr, p->gg, 0, sign < 0 ? 3 : 4,
+    k_gen_col<true><<<(unsigned)(p->N * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>(vol, nullptr, p->tw, nullptr, p->gg, 0, sign < 0 ? 3 : 4,
                                                                                   sign < 0 ? 1.0f : 1.0f / (float)p->N, N, N * N);
     return check_launch(p);
 }

@@ -276,6 +276,8 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
 // (A[pos(ky)][pos(kx)], k_gen_set_data), A < 0 = unmeasured.
 // Modes 3 and 4 are the plain 1D transform along the slow axis with NATURAL order on both sides (the z pass of
 // cpra_fft3): 3 = forward, 4 = inverse times `scale`.  "Image" n starts at scr + n istride, its rows are `pitch` apart.
+// ZM: the instantiation that also serves modes 3 and 4 (kept apart so that the loop's kernel carries none of it).
+template <bool ZM>
 __global__ void __launch_bounds__(GEN_NT, 4)
 k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* __restrict__ twg, double* __restrict__ partial,
           GenGeo gg, int n0, int mode, float scale, size_t istride, size_t pitch)
@@ -293,7 +295,7 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     const int W2 = W / 2, w2 = threadIdx.x & (W2 - 1), r0 = threadIdx.x / W2, rstep = blockDim.x / W2, cx = x0 + 2 * w2;
     float2* __restrict__ col0 = scr + (size_t)n * istride + cx;
     const float* __restrict__ A0 = A + (size_t)n * px + cx;
-    if (mode >= 3) {
+    if constexpr (ZM) {
         for (int i = threadIdx.x; i < N; i += blockDim.x) s.perm[i] = gen_pos(i, gg);
         __syncthreads();
     }
@@ -301,7 +303,7 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     // requested into L2 meanwhile
     if (cx < N) {
         for (int y = r0; y < N; y += rstep) {
-            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + t.pair(mode == 4 ? s.perm[y] : y, w2));
+            const unsigned d = (unsigned)__cvta_generic_to_shared(s.a + t.pair(ZM && mode == 4 ? s.perm[y] : y, w2));
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(col0 + (size_t)y * pitch) : "memory");
         }
         if (mode == 0 && (w2 & 3) == 0)
@@ -346,7 +348,7 @@ k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* _
     }
     if (mode != 1 && mode != 3) gen_fft_inv(s.a, s.tw, gg);
     if (cx < N) {
-        if (mode >= 3) {
+        if (ZM && mode >= 3) {
             const float f = mode == 4 ? scale : 1.0f;
             for (int y = r0; y < N; y += rstep) {
                 const float4 q = *reinterpret_cast<const float4*>(s.a + t.pair(mode == 3 ? s.perm[y] : y, w2));
