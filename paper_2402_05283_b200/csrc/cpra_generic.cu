@@ -40,13 +40,19 @@ int gen_set_attrs()
     auto acc = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     const int SM = 200 * 1024;
     acc(allow_smem(k_gen_row_fwd, SM));
-    acc(allow_smem(k_gen_col<false>, SM));
-    acc(allow_smem(k_gen_col<true>, SM));
+    acc(allow_smem(k_gen_col<0>, SM));
+    acc(allow_smem(k_gen_col<1>, SM));
+    acc(allow_smem(k_gen_col<2>, SM));
+    acc(allow_smem(k_gen_col<3>, SM));
+    acc(allow_smem(k_gen_col<4>, SM));
     acc(allow_smem(k_gen_row_inv, SM));
     // as much shared memory as the SM has, whatever one block asks for (the default carveout fits fewer blocks)
     acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_row_fwd), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<false>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<true>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<0>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<1>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<2>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<3>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_col<4>), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     acc(cudaFuncSetAttribute(reinterpret_cast<const void*>(k_gen_row_inv), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     return e == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
 }
@@ -66,8 +72,11 @@ int row_fwd(cpra_plan_s* p, const float2* cur, int n0, int nimg, bool fires, boo
 int col(cpra_plan_s* p, int n0, int nimg, int mode, float scale)
 {
     ProfScope prof(p, CPRA_PROFILE_COL);
-    k_gen_col<false><<<(unsigned)(nimg * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, mode, scale,
-                                                                                  (size_t)p->N * p->N, (size_t)p->N);
+    const unsigned grid = (unsigned)(nimg * tiles_of(p));
+    const size_t px = (size_t)p->N * p->N, N = (size_t)p->N;
+    if (mode == 0) k_gen_col<0><<<grid, GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, scale, px, N);
+    else if (mode == 1) k_gen_col<1><<<grid, GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, scale, px, N);
+    else k_gen_col<2><<<grid, GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, scale, px, N);
     return check_launch(p);
 }
 int row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, int n0, int nimg, bool fires, bool hio, float beta, float scale, const float2* ghat)
@@ -167,8 +176,9 @@ int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign)
 int gen_fftz(cpra_plan_s* p, float2* vol, int sign)
 {
     const size_t N = (size_t)p->N;
-    k_gen_col<true><<<(unsigned)(p->N * tiles_of(p)), GEN_NT, smem_of(p), p->stream>>>(vol, nullptr, p->tw, nullptr, p->gg, 0, sign < 0 ? 3 : 4,
-                                                                                  sign < 0 ? 1.0f : 1.0f / (float)p->N, N, N * N);
+    const unsigned grid = (unsigned)(p->N * tiles_of(p));
+    if (sign < 0) k_gen_col<3><<<grid, GEN_NT, smem_of(p), p->stream>>>(vol, nullptr, p->tw, nullptr, p->gg, 0, 1.0f, N, N * N);
+    else k_gen_col<4><<<grid, GEN_NT, smem_of(p), p->stream>>>(vol, nullptr, p->tw, nullptr, p->gg, 0, 1.0f / (float)p->N, N, N * N);
     return check_launch(p);
 }
 

@@ -276,12 +276,14 @@ k_gen_row_fwd(const float2* __restrict__ cur, float2* __restrict__ scr, const fl
 // (A[pos(ky)][pos(kx)], k_gen_set_data), A < 0 = unmeasured.
 // Modes 3 and 4 are the plain 1D transform along the slow axis with NATURAL order on both sides (the z pass of
 // cpra_fft3): 3 = forward, 4 = inverse times `scale`.  "Image" n starts at scr + n istride, its rows are `pitch` apart.
-// ZM: the instantiation that also serves modes 3 and 4 (kept apart so that the loop's kernel carries none of it).
-template <bool ZM>
+// The mode is a template parameter: the loop's kernel (mode 0) carries nothing of the others.
+template <int MODE>
 __global__ void __launch_bounds__(GEN_NT, 4)
 k_gen_col(float2* __restrict__ scr, const float* __restrict__ A, const float2* __restrict__ twg, double* __restrict__ partial,
-          GenGeo gg, int n0, int mode, float scale, size_t istride, size_t pitch)
+          GenGeo gg, int n0, float scale, size_t istride, size_t pitch)
 {
+    constexpr int mode = MODE;
+    constexpr bool ZM = MODE >= 3;
     extern __shared__ __align__(16) unsigned char smraw[];
     const int N = gg.N, W = gg.W;
     GenSmem s(smraw, N, W);
