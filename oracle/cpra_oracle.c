@@ -34,6 +34,12 @@
  * duplicate rays in the assembly (slices with different constant spectra on a 360 degree scan).
  * Full multi-iteration trajectories have no external pin: PARITY UNPINNED beyond those invariants.
  *
+ * Around the loop (each function below cites its passage and is pinned in tests/test_oracle_next.py):
+ * seam flip, blur / shrink-wrap, Step A, centre of mass / bank / merge (Step C), phase gauge and twin chain of an
+ * episode, the 3D transform and Step D's iterations, the 3D support as the back-projection of the 2D supports and its
+ * re-thresholding, FSC / PRTF, positivity.  Sizes that are not powers of two use the O(N^2)
+ * definition of the 1D transform, in 2D and in 3D.
+ *
  * Layout: images row-major [n][y][x], x fastest; complex = interleaved (re, im).  All I/O arrays of
  * this library are double / interleaved double regardless of `real`.
  */
