@@ -499,6 +499,23 @@ def test_loop_mixed_radix(torch_cuda, N, Np, alpha, n_ei, seam, rule):
     assert rel_l2(_get(g), o.get_projections(0)) <= (k + 2) * TOL_1
 
 
+def test_full_size_paper_simulation_detector(torch_cuda):
+    """The paper's simulated case at its own size (N = 160 with N_p = 90 projections): config 1's object
+    scaled to N = 160, every projection after two iterations of the coupled loop against the oracle (whose transform at
+    this N is the O(N^2) definition), and the per-projection errors."""
+    p = cpra_inputs.make_problem(1, Np=90, N=160)
+    o, g = _oracle(p), _gpu(p)
+    o.set_seam(1); g.set_seam(True)
+    o.iterate(2, p.beta)
+    g.iterate(2, p.beta)
+    out, ref = _get(g), o.get_projections(0)
+    pn = np.sqrt((np.abs(out - ref) ** 2).sum(axis=(1, 2)) / (np.abs(ref) ** 2).sum(axis=(1, 2)))
+    assert pn.max() <= 3 * TOL_1 and np.median(pn) <= TOL_1, (pn.max(), np.median(pn))
+    E, Eg = g.get_error()
+    Eo, Ego = o.get_error()
+    assert np.abs(E.cpu().numpy() - Eo).max() <= TOL_E * Eo.max() and abs(float(Eg.cpu()[0]) - Ego) <= TOL_E * Ego
+
+
 def test_assembly_and_merge_mixed_radix(torch_cuda):
     """Config 1 scaled to N = 160 (the paper's oxide-particle detector size): three iterations, the
     Fourier-slice assembly and a merge from the plan, against the oracle."""
