@@ -236,7 +236,7 @@ int cpra_set_estimate(cpra_plan_t p, const float* d_g0)
     const size_t total = (size_t)p->Np * p->N * p->N;
     if (p->generic) { if (int rc = gen_set_estimate(p, d_g0)) return rc; }
     else {
-        k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_g0, (float*)p->st[p->cur], p->geo, total);
+        k_pack_state<<<blocks_for(total / (p->geo.TB), 256), 256, 0, p->stream>>>((const float2*)d_g0, (float*)p->st[p->cur], p->geo, total / p->geo.TB);
         if (int rc = check_launch(p)) return rc;
     }
     p->t = 0;
@@ -350,7 +350,8 @@ int cpra_get_projections(cpra_plan_t p, int which, float* d_out)
     if (!p->have_estimate || (which == CPRA_SUPPORTED && !p->have_support)) return CPRA_ERR_NOT_READY;
     if (p->generic) return gen_get_projections(p, which, d_out);
     const size_t total = (size_t)p->Np * p->N * p->N;
-    k_unpack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float*)p->st[p->cur], p->S16, (float2*)d_out, p->geo, total, which == CPRA_SUPPORTED);
+    k_unpack_state<<<blocks_for(total / p->geo.TB, 256), 256, 0, p->stream>>>((const float*)p->st[p->cur], p->S16, (float2*)d_out, p->geo, total / p->geo.TB,
+                                                                           which == CPRA_SUPPORTED);
     return check_launch(p);
 }
 
@@ -361,10 +362,12 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
     if (p->generic) return gen_fft2(p, d_in, d_out, sign);
     const size_t total = (size_t)p->Np * p->N * p->N;
     float4* tmp = p->st[p->cur ^ 1];
-    const unsigned nb = blocks_for(total, 256);
+    const size_t units = total / p->geo.TB;                              // (n, row tile, x) of the state conversions
+    const unsigned rows = (unsigned)((size_t)p->Np * p->N);              // one block per natural spectrum row
+    const int rowt = std::min(256, std::max(32, p->N / 2)), rowsm = (int)sizeof(float2) * p->N;
     int rc = CPRA_OK;
     if (sign < 0) {
-        k_pack_state<<<nb, 256, 0, p->stream>>>((const float2*)d_in, (float*)tmp, p->geo, total);
+        k_pack_state<<<blocks_for(units, 256), 256, 0, p->stream>>>((const float2*)d_in, (float*)tmp, p->geo, units);
         if ((rc = check_launch(p))) return rc;
         { auto f = [&]() -> int {
             CPRA_DISPATCH_N(p->N,
@@ -372,10 +375,10 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
                 if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
             return 0; }; f(); }
         if (rc) return rc;
-        k_unpack_spectrum<<<nb, 256, 0, p->stream>>>((const float*)p->scr, (float2*)d_out, p->geo, total);
+        k_unpack_spectrum<<<rows, rowt, rowsm, p->stream>>>((const float*)p->scr, (float2*)d_out, p->geo);
         return check_launch(p);
     }
-    k_pack_spectrum<<<nb, 256, 0, p->stream>>>((const float2*)d_in, (float*)p->scr, p->geo, total);
+    k_pack_spectrum<<<rows, rowt, rowsm, p->stream>>>((const float2*)d_in, (float*)p->scr, p->geo);
     if ((rc = check_launch(p))) return rc;
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     { auto f = [&]() -> int {
@@ -384,7 +387,7 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
             if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, tmp, tmp, false, MIX_NONE, 0.f, scale, 0, p->Np));
         return 0; }; f(); }
     if (rc) return rc;
-    k_unpack_state<<<nb, 256, 0, p->stream>>>((const float*)tmp, p->S16, (float2*)d_out, p->geo, total, 0);
+    k_unpack_state<<<blocks_for(units, 256), 256, 0, p->stream>>>((const float*)tmp, p->S16, (float2*)d_out, p->geo, units, 0);
     return check_launch(p);
 }
 
@@ -792,7 +795,7 @@ int cpra_prtf(cpra_plan_t p, const float* d_avg, float* d_out)
         return check_launch(p);
     }
     float4* tmp = p->st[p->cur ^ 1];
-    k_pack_state<<<blocks_for(total, 256), 256, 0, p->stream>>>((const float2*)d_avg, (float*)tmp, p->geo, total);
+    k_pack_state<<<blocks_for(total / p->geo.TB, 256), 256, 0, p->stream>>>((const float2*)d_avg, (float*)tmp, p->geo, total / p->geo.TB);
     int rc = check_launch(p);
     if (rc) return rc;
     { auto f = [&]() -> int {

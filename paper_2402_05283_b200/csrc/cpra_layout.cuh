@@ -69,35 +69,95 @@ __global__ void k_pack_support(const unsigned char* __restrict__ S, uint16_t* __
     S16[i] = (uint16_t)bits;
 }
 
-// natural [n][y][x] <-> row-tiled state; `masked` multiplies by the support.  One thread per
-// element, indexed in natural order.
-__global__ void k_pack_state(const float2* __restrict__ in, float* __restrict__ st, Geo g, size_t total)
+// position -> frequency (the inverse of fft_pos)
+__host__ __device__ __forceinline__ int fft_unpos(int pos, int R0, int R1, int R2)
+{
+    const int k2 = pos % R2, k1 = (pos / R2) % R1, k0 = pos / (R2 * R1);
+    return k0 + R0 * (k1 + R1 * k2);
+}
+
+// natural [n][y][x] <-> row-tiled state; `masked` multiplies by the support.  One thread per (n, row tile, x): it
+// moves the TB rows of the tile at column x, i.e. TB coalesced 8-byte accesses on the natural side (the lanes run
+// along x) and the TB / 2 quads of one position = 64 or 128 contiguous bytes on the tiled side.  units = Np (N / TB) N.
+__global__ void k_pack_state(const float2* __restrict__ in, float* __restrict__ st, Geo g, size_t units)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= total) return;
-    const int N = g.N;
-    const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    st_c(st, st_idx(g, n, y, x), in[i]);
+    if (i >= units) return;
+    const int N = g.N, tb = g.TB, np = tb / 2;
+    const int x = (int)(i % N);
+    const size_t nrt = i / N;                        // n (N / TB) + rt
+    const int rt = (int)(nrt % (N / tb));
+    const size_t n = nrt / (N / tb);
+    const float2* __restrict__ src = in + (n * N + (size_t)rt * tb) * N + x;
+    float4* __restrict__ dst = reinterpret_cast<float4*>(st) + (nrt * N + ppos(x, tb)) * np;
+#pragma unroll
+    for (int j = 0; j < NPAIR; ++j) {
+        if (j >= np) break;
+        const float2 a = src[(size_t)(2 * j) * N], b = src[(size_t)(2 * j + 1) * N];
+        dst[j] = make_float4(a.x, b.x, a.y, b.y);
+    }
 }
 __global__ void k_unpack_state(const float* __restrict__ st, const uint16_t* __restrict__ S16,
-                               float2* __restrict__ out, Geo g, size_t total, int masked)
+                               float2* __restrict__ out, Geo g, size_t units, int masked)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= total) return;
-    const int N = g.N;
-    const int x = (int)(i % N), y = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    float2 v = ld_c(st, st_idx(g, n, y, x));
-    if (masked && !((S16[((size_t)n * (N / 16) + y / 16) * N + x] >> (y % 16)) & 1)) v = make_float2(0.f, 0.f);
-    out[i] = v;
+    if (i >= units) return;
+    const int N = g.N, tb = g.TB, np = tb / 2;
+    const int x = (int)(i % N);
+    const size_t nrt = i / N;
+    const int rt = (int)(nrt % (N / tb));
+    const size_t n = nrt / (N / tb);
+    const float4* __restrict__ src = reinterpret_cast<const float4*>(st) + (nrt * N + ppos(x, tb)) * np;
+    float2* __restrict__ dst = out + (n * N + (size_t)rt * tb) * N + x;
+    const int y0 = rt * tb;
+    const unsigned bits = masked ? ((unsigned)S16[(n * (N / 16) + y0 / 16) * N + x] >> (y0 % 16)) : 0xffffu;
+#pragma unroll
+    for (int j = 0; j < NPAIR; ++j) {
+        if (j >= np) break;
+        const float4 q = src[j];
+        dst[(size_t)(2 * j) * N] = ((bits >> (2 * j)) & 1) ? make_float2(q.x, q.z) : make_float2(0.f, 0.f);
+        dst[(size_t)(2 * j + 1) * N] = ((bits >> (2 * j + 1)) & 1) ? make_float2(q.y, q.w) : make_float2(0.f, 0.f);
+    }
 }
-// natural-order spectrum [n][ky][kx] <-> column-tiled permuted scratch
-__global__ void k_unpack_spectrum(const float* __restrict__ scr, float2* __restrict__ out, Geo g, size_t total)
+// natural-order spectrum [n][ky][kx] <-> column-tiled permuted scratch.  One block per natural row (n, ky): the scratch
+// row py = pos(ky) is N / TB pieces of TB / 2 quads (64 or 128 contiguous bytes each, one quad per thread); the
+// permutation along x happens in shared memory (N complex numbers), so the natural row moves coalesced.
+__global__ void k_unpack_spectrum(const float* __restrict__ scr, float2* __restrict__ out, Geo g)
 {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= total) return;
-    const int N = g.N;
-    const int kx = (int)(i % N), ky = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    out[i] = ld_c(scr, sc_idx(g, n, fft_pos(ky, g.R0, g.R1, g.R2), fft_pos(kx, g.R0, g.R1, g.R2)));
+    extern __shared__ __align__(16) float2 rowbuf[];
+    const int N = g.N, tb = g.TB, np = tb / 2;
+    const int ky = (int)(blockIdx.x % N);
+    const size_t n = blockIdx.x / N;
+    const int py = fft_pos(ky, g.R0, g.R1, g.R2);
+    const float4* __restrict__ src = reinterpret_cast<const float4*>(scr);
+    for (int q = threadIdx.x; q < N / 2; q += blockDim.x) {
+        const int ct = q / np, slot = q % np, j = sw(slot, py, np);          // slot = j ^ s is its own inverse
+        const float4 v = src[((n * (N / tb) + ct) * N + ppos(py, tb, ct & 1)) * np + slot];
+        const int px = ct * tb + 2 * j;
+        rowbuf[fft_unpos(px, g.R0, g.R1, g.R2)] = make_float2(v.x, v.z);
+        rowbuf[fft_unpos(px + 1, g.R0, g.R1, g.R2)] = make_float2(v.y, v.w);
+    }
+    __syncthreads();
+    float2* __restrict__ dst = out + (n * N + ky) * N;
+    for (int x = threadIdx.x; x < N; x += blockDim.x) dst[x] = rowbuf[x];
+}
+__global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict__ scr, Geo g)
+{
+    extern __shared__ __align__(16) float2 rowbuf[];
+    const int N = g.N, tb = g.TB, np = tb / 2;
+    const int ky = (int)(blockIdx.x % N);
+    const size_t n = blockIdx.x / N;
+    const int py = fft_pos(ky, g.R0, g.R1, g.R2);
+    const float2* __restrict__ src = in + (n * N + ky) * N;
+    for (int x = threadIdx.x; x < N; x += blockDim.x) rowbuf[x] = src[x];
+    __syncthreads();
+    float4* __restrict__ dst = reinterpret_cast<float4*>(scr);
+    for (int q = threadIdx.x; q < N / 2; q += blockDim.x) {
+        const int ct = q / np, slot = q % np, j = sw(slot, py, np);
+        const int px = ct * tb + 2 * j;
+        const float2 a = rowbuf[fft_unpos(px, g.R0, g.R1, g.R2)], b = rowbuf[fft_unpos(px + 1, g.R0, g.R1, g.R2)];
+        dst[((n * (N / tb) + ct) * N + ppos(py, tb, ct & 1)) * np + slot] = make_float4(a.x, b.x, a.y, b.y);
+    }
 }
 // spectrum of the assembly: column-tiled permuted scratch -> natural order, TRANSPOSED: Et[n][ku][kz],
 // kz fastest, so that the gather kernel, which walks kz for fixed (n, ku), streams contiguous memory
@@ -278,12 +338,6 @@ __global__ void k_assemble_geo(AsmGeo* __restrict__ geo, const double* __restric
     geo[i] = g;
 }
 
-// position -> frequency (the inverse of fft_pos)
-__host__ __device__ __forceinline__ int fft_unpos(int pos, int R0, int R1, int R2)
-{
-    const int k2 = pos % R2, k1 = (pos / R2) % R1, k0 = pos / (R2 * R1);
-    return k0 + R0 * (k1 + R1 * k2);
-}
 // one block per scratch column tile (n, ct): TB columns x N positions, contiguous in HBM
 __global__ void k_unpack_tile_T(const float4* __restrict__ scr, float2* __restrict__ Et, Geo g)
 {
