@@ -363,8 +363,9 @@ int cpra_fft2(cpra_plan_t p, const float* d_in, float* d_out, int sign)
     const size_t total = (size_t)p->Np * p->N * p->N;
     float4* tmp = p->st[p->cur ^ 1];
     const size_t units = total / p->geo.TB;                              // (n, row tile, x) of the state conversions
-    const unsigned rows = (unsigned)((size_t)p->Np * p->N);              // one block per natural spectrum row
-    const int rowt = std::min(256, std::max(32, p->N / 2)), rowsm = (int)sizeof(float2) * p->N;
+    const int PB = spectrum_rows_per_block(p->N);                        // scratch rows per block of the spectrum conversions
+    const unsigned rows = (unsigned)((size_t)p->Np * (p->N / PB));
+    const int rowt = 256, rowsm = (int)sizeof(float2) * p->N * PB;
     int rc = CPRA_OK;
     if (sign < 0) {
         k_pack_state<<<blocks_for(units, 256), 256, 0, p->stream>>>((const float2*)d_in, (float*)tmp, p->geo, units);

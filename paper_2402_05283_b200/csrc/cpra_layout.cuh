@@ -119,44 +119,69 @@ __global__ void k_unpack_state(const float* __restrict__ st, const uint16_t* __r
         dst[(size_t)(2 * j + 1) * N] = ((bits >> (2 * j + 1)) & 1) ? make_float2(q.y, q.w) : make_float2(0.f, 0.f);
     }
 }
-// natural-order spectrum [n][ky][kx] <-> column-tiled permuted scratch.  One block per natural row (n, ky): the scratch
-// row py = pos(ky) is N / TB pieces of TB / 2 quads (64 or 128 contiguous bytes each, one quad per thread); the
-// permutation along x happens in shared memory (N complex numbers), so the natural row moves coalesced.
+// natural-order spectrum [n][ky][kx] <-> column-tiled permuted scratch.  One block per (n, group of PB consecutive
+// scratch rows py): in every column tile those rows are PB x TB/2 quads = one contiguous piece (512 B at PB = TB = 8),
+// read / written with the lanes along it; the permutation along x happens in shared memory (PB rows of N complex
+// numbers), and each of the PB natural rows ky = unpos(py) moves coalesced.  PB divides 8.
+__host__ __device__ __forceinline__ int spectrum_rows_per_block(int N) { return N <= 512 ? 8 : 4; }   // PB N 8 bytes <= 32 KiB
+// fft_unpos with the radices (powers of two on this path) given as shifts: no division per element
+__host__ __device__ __forceinline__ int ilog2_of(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+struct Unpos {
+    int l1, l2, l0s;   // log2 R1, log2 R2, log2 (R2 R1)... and the shift of k2 in the result
+    int R0, m1, m2;
+    __device__ __forceinline__ explicit Unpos(const Geo& g)
+        : l1(ilog2_of(g.R1)), l2(ilog2_of(g.R2)), l0s(0), R0(g.R0), m1(g.R1 - 1), m2(g.R2 - 1) {}
+    __device__ __forceinline__ int operator()(int pos) const
+    {
+        const int k2 = pos & m2, k1 = (pos >> l2) & m1, k0 = pos >> (l2 + l1);
+        return k0 + R0 * (k1 + (k2 << l1));
+    }
+};
 __global__ void k_unpack_spectrum(const float* __restrict__ scr, float2* __restrict__ out, Geo g)
 {
     extern __shared__ __align__(16) float2 rowbuf[];
-    const int N = g.N, tb = g.TB, np = tb / 2;
-    const int ky = (int)(blockIdx.x % N);
-    const size_t n = blockIdx.x / N;
-    const int py = fft_pos(ky, g.R0, g.R1, g.R2);
+    const int N = g.N, tb = g.TB, np = tb / 2, nct = N / tb, PB = spectrum_rows_per_block(N);
+    const int py0 = (int)(blockIdx.x % (N / PB)) * PB;
+    const size_t n = blockIdx.x / (N / PB);
     const float4* __restrict__ src = reinterpret_cast<const float4*>(scr);
-    for (int q = threadIdx.x; q < N / 2; q += blockDim.x) {
-        const int ct = q / np, slot = q % np, j = sw(slot, py, np);          // slot = j ^ s is its own inverse
-        const float4 v = src[((n * (N / tb) + ct) * N + ppos(py, tb, ct & 1)) * np + slot];
-        const int px = ct * tb + 2 * j;
-        rowbuf[fft_unpos(px, g.R0, g.R1, g.R2)] = make_float2(v.x, v.z);
-        rowbuf[fft_unpos(px + 1, g.R0, g.R1, g.R2)] = make_float2(v.y, v.w);
+    const Unpos unpos(g);
+    const int lnp = ilog2_of(np), lpb = ilog2_of(PB);
+    for (int t = threadIdx.x; t < PB * np * nct; t += blockDim.x) {
+        const int slot = t & (np - 1), pp = (t >> lnp) & (PB - 1), ct = t >> (lnp + lpb);
+        const int py = ppos(py0 + pp, tb, ct & 1);                  // the row stored at physical row py0 + pp (ppos is an involution)
+        const float4 v = src[((n * nct + ct) * N + py0 + pp) * np + slot];
+        const int px = ct * tb + 2 * sw(slot, py, np);               // slot = j ^ s is its own inverse
+        float2* __restrict__ row = rowbuf + (py - py0) * N;
+        row[unpos(px)] = make_float2(v.x, v.z);
+        row[unpos(px + 1)] = make_float2(v.y, v.w);
     }
     __syncthreads();
-    float2* __restrict__ dst = out + (n * N + ky) * N;
-    for (int x = threadIdx.x; x < N; x += blockDim.x) dst[x] = rowbuf[x];
+    for (int r = 0; r < PB; ++r) {
+        float2* __restrict__ dst = out + (n * N + fft_unpos(py0 + r, g.R0, g.R1, g.R2)) * N;
+        for (int x = threadIdx.x; x < N; x += blockDim.x) dst[x] = rowbuf[r * N + x];
+    }
 }
 __global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict__ scr, Geo g)
 {
     extern __shared__ __align__(16) float2 rowbuf[];
-    const int N = g.N, tb = g.TB, np = tb / 2;
-    const int ky = (int)(blockIdx.x % N);
-    const size_t n = blockIdx.x / N;
-    const int py = fft_pos(ky, g.R0, g.R1, g.R2);
-    const float2* __restrict__ src = in + (n * N + ky) * N;
-    for (int x = threadIdx.x; x < N; x += blockDim.x) rowbuf[x] = src[x];
+    const int N = g.N, tb = g.TB, np = tb / 2, nct = N / tb, PB = spectrum_rows_per_block(N);
+    const int py0 = (int)(blockIdx.x % (N / PB)) * PB;
+    const size_t n = blockIdx.x / (N / PB);
+    for (int r = 0; r < PB; ++r) {
+        const float2* __restrict__ src = in + (n * N + fft_unpos(py0 + r, g.R0, g.R1, g.R2)) * N;
+        for (int x = threadIdx.x; x < N; x += blockDim.x) rowbuf[r * N + x] = src[x];
+    }
     __syncthreads();
     float4* __restrict__ dst = reinterpret_cast<float4*>(scr);
-    for (int q = threadIdx.x; q < N / 2; q += blockDim.x) {
-        const int ct = q / np, slot = q % np, j = sw(slot, py, np);
-        const int px = ct * tb + 2 * j;
-        const float2 a = rowbuf[fft_unpos(px, g.R0, g.R1, g.R2)], b = rowbuf[fft_unpos(px + 1, g.R0, g.R1, g.R2)];
-        dst[((n * (N / tb) + ct) * N + ppos(py, tb, ct & 1)) * np + slot] = make_float4(a.x, b.x, a.y, b.y);
+    const Unpos unpos(g);
+    const int lnp = ilog2_of(np), lpb = ilog2_of(PB);
+    for (int t = threadIdx.x; t < PB * np * nct; t += blockDim.x) {
+        const int slot = t & (np - 1), pp = (t >> lnp) & (PB - 1), ct = t >> (lnp + lpb);
+        const int py = ppos(py0 + pp, tb, ct & 1);
+        const int px = ct * tb + 2 * sw(slot, py, np);
+        const float2* __restrict__ row = rowbuf + (py - py0) * N;
+        const float2 a = row[unpos(px)], b = row[unpos(px + 1)];
+        dst[((n * nct + ct) * N + py0 + pp) * np + slot] = make_float4(a.x, b.x, a.y, b.y);
     }
 }
 // spectrum of the assembly: column-tiled permuted scratch -> natural order, TRANSPOSED: Et[n][ku][kz],
