@@ -79,6 +79,13 @@ int col(cpra_plan_s* p, int n0, int nimg, int mode, float scale)
     else k_gen_col<2><<<grid, GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, scale, px, N);
     return check_launch(p);
 }
+int permute(cpra_plan_s* p, const float2* in, float2* out, int to_pos)
+{
+    const int N = p->N, nb = (N + GEN_PB - 1) / GEN_PB;
+    const size_t sm = sizeof(float2) * GEN_PB * N + sizeof(int) * 2 * N;
+    k_gen_permute<<<(unsigned)(p->Np * nb), 256, sm, p->stream>>>(in, out, p->gg, to_pos);
+    return check_launch(p);
+}
 int row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, int n0, int nimg, bool fires, bool hio, float beta, float scale, const float2* ghat)
 {
     ProfScope prof(p, CPRA_PROFILE_ROW_INV);
@@ -161,11 +168,9 @@ int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign)
     if (sign < 0) {
         if ((rc = row_fwd(p, (const float2*)d_in, 0, p->Np, false, false, nullptr))) return rc;
         if ((rc = col(p, 0, p->Np, 1, 1.0f))) return rc;
-        k_gen_permute<<<gblocks(total, 256), 256, 0, p->stream>>>((const float2*)p->scr, (float2*)d_out, p->gg, total, 0);
-        return check_launch(p);
+        return permute(p, (const float2*)p->scr, (float2*)d_out, 0);
     }
-    k_gen_permute<<<gblocks(total, 256), 256, 0, p->stream>>>((const float2*)d_in, (float2*)p->scr, p->gg, total, 1);
-    if ((rc = check_launch(p))) return rc;
+    if ((rc = permute(p, (const float2*)d_in, (float2*)p->scr, 1))) return rc;
     if ((rc = col(p, 0, p->Np, 2, 1.0f))) return rc;
     if ((rc = row_inv(p, tmp, tmp, 0, p->Np, false, false, 0.f, 1.0f / ((float)p->N * (float)p->N), nullptr))) return rc;
     return cudaMemcpyAsync(d_out, tmp, sizeof(float2) * total, cudaMemcpyDeviceToDevice, p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;

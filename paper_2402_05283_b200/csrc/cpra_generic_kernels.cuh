@@ -481,17 +481,47 @@ __global__ void k_gen_transpose(const float2* __restrict__ in, float2* __restric
     const size_t n = i / ((size_t)N * N);
     out[i] = in[(n * N + gen_pos(kz, gg)) * N + gen_pos(ku, gg)];
 }
-// natural [n][ky][kx] <-> position order [n][pos(ky)][pos(kx)]  (to_pos: scatter into position order; else gather from it)
-__global__ void k_gen_permute(const float2* __restrict__ in, float2* __restrict__ out, GenGeo gg, size_t total, int to_pos)
+// natural [n][ky][kx] <-> position order [n][pos(ky)][pos(kx)]  (to_pos: into position order; else out of it).  One
+// block per (n, GEN_PB consecutive rows of the position-order array): those rows and the natural rows they map to
+// both move coalesced; the permutation along x goes through shared memory with the tables pos / its inverse built
+// once per block.  Dynamic shared memory: GEN_PB N float2 + 2 N int.
+constexpr int GEN_PB = 4;
+__global__ void k_gen_permute(const float2* __restrict__ in, float2* __restrict__ out, GenGeo gg, int to_pos)
 {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= total) return;
-    const int N = gg.N, kx = (int)(i % N), ky = (int)((i / N) % N);
-    const size_t n = i / ((size_t)N * N);
-    const size_t j = (n * N + gen_pos(ky, gg)) * N + gen_pos(kx, gg);
-    if (to_pos) out[j] = in[i]; else out[i] = in[j];
+    extern __shared__ __align__(16) unsigned char pm[];
+    const int N = gg.N;
+    float2* rows = reinterpret_cast<float2*>(pm);
+    int* pos = reinterpret_cast<int*>(rows + (size_t)GEN_PB * N);
+    int* inv = pos + N;
+    const int nb = (N + GEN_PB - 1) / GEN_PB;
+    const int py0 = (int)(blockIdx.x % nb) * GEN_PB, nr = min(GEN_PB, N - py0);
+    const size_t n = blockIdx.x / nb;
+    for (int k = threadIdx.x; k < N; k += blockDim.x) {
+        const int p = gen_pos(k, gg);
+        pos[k] = p;
+        inv[p] = k;
+    }
+    __syncthreads();
+    if (to_pos) {
+        for (int r = 0; r < nr; ++r) {
+            const float2* __restrict__ src = in + (n * N + inv[py0 + r]) * N;
+            for (int x = threadIdx.x; x < N; x += blockDim.x) rows[r * N + x] = src[x];
+        }
+        __syncthreads();
+        for (int r = 0; r < nr; ++r) {
+            float2* __restrict__ dst = out + (n * N + py0 + r) * N;
+            for (int q = threadIdx.x; q < N; q += blockDim.x) dst[q] = rows[r * N + inv[q]];
+        }
+    } else {
+        const float2* __restrict__ src = in + (n * N + py0) * N;          // nr rows, contiguous
+        for (int i = threadIdx.x; i < nr * N; i += blockDim.x) rows[i] = src[i];
+        __syncthreads();
+        for (int r = 0; r < nr; ++r) {
+            float2* __restrict__ dst = out + (n * N + inv[py0 + r]) * N;
+            for (int x = threadIdx.x; x < N; x += blockDim.x) dst[x] = rows[r * N + pos[x]];
+        }
+    }
 }
-
 // ---- shrink-wrap (reading A23) on natural arrays ------------------------------------
 // (|S g|, 0)
 __global__ void k_gen_abs_supported(const float2* __restrict__ st, const unsigned char* __restrict__ S, float2* __restrict__ out, size_t total)
