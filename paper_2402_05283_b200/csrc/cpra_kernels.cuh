@@ -783,10 +783,21 @@ k_fft_z(float2* __restrict__ vol, const float2* __restrict__ twg, float scale)
     const int y = blockIdx.y, x0 = blockIdx.x * TBN;
     float4* __restrict__ v4 = reinterpret_cast<float4*>(vol);   // two complex numbers (re_a, im_a, re_b, im_b)
     for (int i = threadIdx.x; i < tw_count<N>(); i += NT) tw0[i] = twg[i];
-    for (int i = threadIdx.x; i < N * NP; i += NT) {
-        const int z = i / NP, j = i % NP;
-        const float4 a = v4[(((size_t)z * N + y) * N + x0) / 2 + j];
-        tile[(INV ? fft_pos(z, RX::R0, RX::R1, RX::R2) : z) * NP + j] = make_float4(a.x, a.z, a.y, a.w);
+    // all of a thread's loads are issued before the first is used (N NP / NT = 16 at N = 512: two batches of 8)
+    constexpr int PER = N * NP / NT, UB = PER % 8 == 0 ? 8 : (PER % 4 == 0 ? 4 : 1);
+    static_assert(PER * NT == N * NP, "whole loads per thread");
+    for (int b = 0; b < PER; b += UB) {
+        float4 a[UB];
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int i = (int)threadIdx.x + (b + u) * NT, z = i / NP, j = i % NP;
+            a[u] = v4[(((size_t)z * N + y) * N + x0) / 2 + j];
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int i = (int)threadIdx.x + (b + u) * NT, z = i / NP, j = i % NP;
+            tile[(INV ? fft_pos(z, RX::R0, RX::R1, RX::R2) : z) * NP + j] = make_float4(a[u].x, a[u].z, a[u].y, a[u].w);
+        }
     }
     __syncthreads();
     auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NP + j]); };
