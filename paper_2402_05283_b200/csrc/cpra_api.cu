@@ -500,7 +500,7 @@ int cpra_shrinkwrap(cpra_plan_t p, float sigma, float threshold, float* d_blurre
             if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
         return 0; }; f(); }
     if (rc) return rc;
-    k_gauss_filter<<<blocks_for(total, 256), 256, 0, p->stream>>>((float*)p->scr, p->geo, total, sigma);
+    k_gauss_filter<<<8 * p->sms, 256, sizeof(float) * p->N, p->stream>>>(p->scr, p->geo, nquads, sigma);
     if ((rc = check_launch(p))) return rc;
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     { auto f = [&]() -> int {

@@ -197,7 +197,7 @@ int gen_shrinkwrap(cpra_plan_s* p, float sigma, float threshold, float* d_blurre
     if (rc == CPRA_OK) rc = row_fwd(p, tmp, 0, p->Np, false, false, nullptr);
     if (rc == CPRA_OK) rc = col(p, 0, p->Np, 1, 1.0f);
     if (rc) return rc;
-    k_gen_gauss_filter<<<gblocks(total, 256), 256, 0, p->stream>>>((float2*)p->scr, p->gg, total, sigma);
+    k_gen_gauss_filter<<<8 * p->sms, 256, sizeof(float) * p->N, p->stream>>>((float2*)p->scr, p->gg, total, sigma);
     if ((rc = check_launch(p))) return rc;
     if ((rc = col(p, 0, p->Np, 2, 1.0f))) return rc;
     if ((rc = row_inv(p, tmp, tmp, 0, p->Np, false, false, 0.f, 1.0f / ((float)p->N * (float)p->N), nullptr))) return rc;

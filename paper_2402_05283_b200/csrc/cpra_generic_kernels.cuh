@@ -531,20 +531,26 @@ __global__ void k_gen_abs_supported(const float2* __restrict__ st, const unsigne
     const float2 v = st[i];
     out[i] = make_float2(S[i] ? sqrtf(v.x * v.x + v.y * v.y) : 0.f, 0.f);
 }
-// spectrum in position order *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2); one thread per natural (n, ky, kx)
+// spectrum in position order *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2): the product of two entries of a table over the
+// positions (tab[pos(k)] = exp(-2 pi^2 sigma^2 k^2 / N^2), k signed; built per block in shared memory), so the array is
+// walked in its own order.  Dynamic shared memory: N floats.
 __global__ void k_gen_gauss_filter(float2* __restrict__ scr, GenGeo gg, size_t total, float sigma)
 {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= total) return;
+    extern __shared__ float gtab[];
     const int N = gg.N;
-    const int ix = (int)(i % N), iy = (int)((i / N) % N);
-    const size_t n = i / ((size_t)N * N);
-    const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N;
-    const double sg = (double)sigma;
-    const float f = (float)exp(-2.0 * 9.86960440108935861883 * sg * sg * ((double)ky * ky + (double)kx * kx) / ((double)N * N));
-    const size_t o = (n * N + gen_pos(iy, gg)) * N + gen_pos(ix, gg);
-    scr[o].x *= f;
-    scr[o].y *= f;
+    const double c = -2.0 * 9.86960440108935861883 * (double)sigma * (double)sigma / ((double)N * N);
+    for (int k = threadIdx.x; k < N; k += blockDim.x) {
+        const int ks = k < N / 2 ? k : k - N;
+        gtab[gen_pos(k, gg)] = (float)exp(c * (double)ks * (double)ks);
+    }
+    __syncthreads();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int px = (int)(i % N), py = (int)((i / N) % N);
+        const float f = gtab[py] * gtab[px];
+        float2 v = scr[i];
+        v.x *= f; v.y *= f;
+        scr[i] = v;
+    }
 }
 // per-image maximum of the real part (one block per image)
 __global__ void k_gen_image_max(const float2* __restrict__ st, float* __restrict__ mx, int N)

@@ -30,19 +30,30 @@ __global__ void k_abs_supported(const float4* __restrict__ st, const uint16_t* _
     const float4 v = st[i];
     out[i] = make_float4((bits & 1) ? sqrtf(v.x * v.x + v.z * v.z) : 0.f, (bits & 2) ? sqrtf(v.y * v.y + v.w * v.w) : 0.f, 0.f, 0.f);
 }
-// spectrum (scratch layout) *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2); one thread per natural (n, ky, kx)
-__global__ void k_gauss_filter(float* __restrict__ scr, Geo g, size_t total, float sigma)
+// spectrum (scratch layout) *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2).  The factor is the product of two entries of a
+// table over the scratch POSITIONS (tab[pos(k)] = exp(-2 pi^2 sigma^2 k^2 / N^2), k signed; built per block in shared
+// memory, N floats), so the kernel walks the scratch quad by quad, coalesced.  Dynamic shared memory: N floats.
+__global__ void k_gauss_filter(float4* __restrict__ scr, Geo g, size_t nquads, float sigma)
 {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= total) return;
-    const int N = g.N;
-    const int ix = (int)(i % N), iy = (int)((i / N) % N), n = (int)(i / ((size_t)N * N));
-    const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N;
-    const double s = (double)sigma;
-    const float f = (float)exp(-2.0 * 9.86960440108935861883 * s * s * ((double)ky * ky + (double)kx * kx) / ((double)N * N));
-    const size_t o = sc_idx(g, n, fft_pos(iy, g.R0, g.R1, g.R2), fft_pos(ix, g.R0, g.R1, g.R2));
-    scr[o] *= f;
-    scr[o + 2] *= f;
+    extern __shared__ float gtab[];
+    const int N = g.N, tb = g.TB, np = tb / 2;
+    const double c = -2.0 * 9.86960440108935861883 * (double)sigma * (double)sigma / ((double)N * N);
+    for (int k = threadIdx.x; k < N; k += blockDim.x) {
+        const int ks = k < N / 2 ? k : k - N;
+        gtab[fft_pos(k, g.R0, g.R1, g.R2)] = (float)exp(c * (double)ks * (double)ks);
+    }
+    __syncthreads();
+    const size_t per_image = (size_t)N * N / 2;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < nquads; q += (size_t)gridDim.x * blockDim.x) {
+        const int qi = (int)(q % per_image);
+        const int slot = qi % np, phys = (qi / np) % N, ct = qi / (np * N);
+        const int py = ppos(phys, tb, ct & 1);                       // the scratch row stored at this physical row
+        const int px = ct * tb + 2 * sw(slot, py, np);
+        const float f = gtab[py], fa = f * gtab[px], fb = f * gtab[px + 1];
+        float4 v = scr[q];
+        v.x *= fa; v.y *= fb; v.z *= fa; v.w *= fb;
+        scr[q] = v;
+    }
 }
 // per-image maximum of the real part of a state-layout stack (one block per image)
 __global__ void k_image_max(const float4* __restrict__ st, float* __restrict__ mx, Geo g)

@@ -39,21 +39,30 @@ class CpraResult:
     seconds: dict = None
 
 
-def random_phase_starts(plan, intensity, mask, seed: int):
-    """Random-phase starts g0 = F^-1[M sqrt(I) e^{i phi}], phi ~ U[0, 2 pi) per pixel (reading A15; PAPER.md:56 "random
-    initial guess") for a stack: intensity fp32 [n, N, N] detector-centred, mask u8 [n, N, N] or None, n = plan.Np.
-    The phases come from torch's generator on the device (input generation); the transform is the library's own
-    cpra_fft2.  Returns complex64 [n, N, N]."""
+def native_amplitudes(intensity, mask):
+    """M sqrt(max(I, 0)) in native order (zero frequency at index 0) from detector-centred intensities: the modulus of
+    every random-phase start (the same for all restarts: computed once)."""
     import torch
-    gen = torch.Generator(device=intensity.device)
-    gen.manual_seed(int(seed))
     N = intensity.shape[-1]
     A = torch.sqrt(torch.clamp(intensity.to(torch.float32), min=0.0))
     if mask is not None:
         A = A * mask.to(torch.float32)
-    A = torch.roll(A, shifts=(-(N // 2), -(N // 2)), dims=(-2, -1))          # detector-centred -> native order
-    phi = torch.rand(A.shape, generator=gen, device=intensity.device, dtype=torch.float32) * (2.0 * math.pi)
-    return plan.fft2(torch.polar(A, phi).to(torch.complex64).contiguous(), +1)
+    return torch.roll(A, shifts=(-(N // 2), -(N // 2)), dims=(-2, -1)).contiguous()
+
+
+def random_phase_starts(plan, intensity, mask, seed: int, amplitudes=None):
+    """Random-phase starts g0 = F^-1[M sqrt(I) e^{i phi}], phi ~ U[0, 2 pi) per pixel (reading A15; PAPER.md:56 "random
+    initial guess") for a stack: intensity fp32 [n, N, N] detector-centred, mask u8 [n, N, N] or None, n = plan.Np
+    (or amplitudes = native_amplitudes(intensity, mask), computed once for many restarts).  The phases come from
+    torch's generator on the device (input generation); the transform is the library's own cpra_fft2.
+    Returns complex64 [n, N, N]."""
+    import torch
+    A = native_amplitudes(intensity, mask) if amplitudes is None else amplitudes
+    gen = torch.Generator(device=A.device)
+    gen.manual_seed(int(seed))
+    phi = torch.rand(A.shape, generator=gen, device=A.device, dtype=torch.float32)
+    phi.mul_(2.0 * math.pi)
+    return plan.fft2(torch.polar(A, phi), +1)
 
 
 def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, n_pre: int, n_episodes: int, n_ei: int,
@@ -109,9 +118,10 @@ def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, 
     plan.set_update(update)
     plan.set_seam(seam_flip)
     plan.merge_begin(n_keep)
+    amplitudes = native_amplitudes(intensity, mask)
     for r in range(n_restarts):
         plan.set_support(support)
-        g0 = random_phase_starts(plan, intensity, mask, seed + 7919 * (r + 1))
+        g0 = random_phase_starts(plan, intensity, mask, seed + 7919 * (r + 1), amplitudes)
         if pre is not None:
             g0[0] = pre[r]
         plan.set_estimate(g0)
