@@ -120,6 +120,15 @@ int cpra_set_carousel(cpra_plan_t plan, int K, const double* h_alpha, int n_ei);
  */
 int cpra_set_estimate(cpra_plan_t plan, const float* d_g0);
 
+/*
+ * The starting estimate given as its spectrum: g0 = F^-1[G0] (inverse 2D FT of every projection, e^{+2 pi i ...} / N^2),
+ * d_G0 interleaved complex fp32 [Np][N][N] in native frequency order (zero frequency at index (0, 0)).  What a random
+ * start is made of ("random initial guess"; A15: G0 = M sqrt(I) e^{i phi}, phi uniform): the same result as
+ * cpra_fft2(+1) followed by cpra_set_estimate, without the natural-order copy in between.  Resets t to 0.
+ * Uses the FFT scratch.  Errors: INVALID_ARG, WORKSPACE, CUDA.
+ */
+int cpra_set_estimate_spectrum(cpra_plan_t plan, const float* d_G0);
+
 /* Iteration counter t (iterations since cpra_set_estimate); settable for exact resume with n_ei > 1. */
 int cpra_get_iteration(cpra_plan_t plan, long* t);
 int cpra_set_iteration(cpra_plan_t plan, long t);

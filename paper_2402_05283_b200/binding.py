@@ -32,6 +32,7 @@ SIGNATURES = {
     "cpra_set_support": (_ci, [_vp, _vp]),
     "cpra_set_carousel": (_ci, [_vp, _ci, _vp, _ci]),
     "cpra_set_estimate": (_ci, [_vp, _vp]),
+    "cpra_set_estimate_spectrum": (_ci, [_vp, _vp]),
     "cpra_get_iteration": (_ci, [_vp, ctypes.POINTER(_cl)]),
     "cpra_set_iteration": (_ci, [_vp, _cl]),
     "cpra_iterate": (_ci, [_vp, _ci, _cf]),
@@ -204,6 +205,11 @@ class Plan:
     def set_estimate(self, g0):
         import torch
         _chk(self._l.cpra_set_estimate(self._h, _dptr(g0, torch.complex64, self._px)), "cpra_set_estimate")
+
+    def set_estimate_spectrum(self, G0):
+        """cpra_set_estimate_spectrum: the starting estimate as F^-1 of a natural-order spectrum complex64 [Np, N, N]."""
+        import torch
+        _chk(self._l.cpra_set_estimate_spectrum(self._h, _dptr(G0, torch.complex64, self._px)), "cpra_set_estimate_spectrum")
 
     @property
     def iteration(self) -> int:

@@ -245,6 +245,33 @@ int cpra_set_estimate(cpra_plan_t p, const float* d_g0)
     return CPRA_OK;
 }
 
+int cpra_set_estimate_spectrum(cpra_plan_t p, const float* d_G0)
+{
+    if (!p || !d_G0) return CPRA_ERR_INVALID_ARG;
+    if (int rc = ready(p)) return rc;
+    int rc = CPRA_OK;
+    const float scale = 1.0f / ((float)p->N * (float)p->N);
+    if (p->generic) {
+        if ((rc = gen_set_estimate_spectrum(p, d_G0))) return rc;
+    } else {
+        // cpra_fft2's inverse path with the state buffer as its destination: no natural-order copy in between
+        const int PB = spectrum_rows_per_block(p->N);
+        k_pack_spectrum<<<(unsigned)((size_t)p->Np * (p->N / PB)), 256, sizeof(float2) * p->N * PB, p->stream>>>((const float2*)d_G0, (float*)p->scr, p->geo);
+        if ((rc = check_launch(p))) return rc;
+        float4* g = p->st[p->cur];
+        { auto f = [&]() -> int {
+            CPRA_DISPATCH_N(p->N,
+                rc = Launch<NN>::col(p, COL_INV, 0, p->Np, 1.0f);
+                if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, g, g, false, MIX_NONE, 0.f, scale, 0, p->Np));
+            return 0; }; f(); }
+        if (rc) return rc;
+    }
+    p->t = 0;
+    p->have_estimate = true;
+    p->have_error = false;
+    return CPRA_OK;
+}
+
 int cpra_get_iteration(cpra_plan_t p, long* t)
 {
     if (!p || !t) return CPRA_ERR_INVALID_ARG;

@@ -111,6 +111,15 @@ int gen_set_estimate(cpra_plan_s* p, const float* d_g0)
     const size_t total = (size_t)p->Np * p->N * p->N;
     return cudaMemcpyAsync(p->st[p->cur], d_g0, sizeof(float2) * total, cudaMemcpyDeviceToDevice, p->stream) == cudaSuccess ? CPRA_OK : CPRA_ERR_CUDA;
 }
+// g0 = F^-1[G0], G0 natural, straight into the state buffer
+int gen_set_estimate_spectrum(cpra_plan_s* p, const float* d_G0)
+{
+    int rc = permute(p, (const float2*)d_G0, (float2*)p->scr, 1);
+    if (rc == CPRA_OK) rc = col(p, 0, p->Np, 2, 1.0f);
+    float2* g = (float2*)p->st[p->cur];
+    if (rc == CPRA_OK) rc = row_inv(p, g, g, 0, p->Np, false, false, 0.f, 1.0f / ((float)p->N * (float)p->N), nullptr);
+    return rc;
+}
 int gen_get_projections(cpra_plan_s* p, int which, float* d_out)
 {
     const size_t total = (size_t)p->Np * p->N * p->N;

@@ -510,6 +510,7 @@ int gen_set_attrs();
 int gen_set_data(cpra_plan_s* p, const float* d_I, const unsigned char* d_mask);
 int gen_set_support(cpra_plan_s* p, const unsigned char* d_S);
 int gen_set_estimate(cpra_plan_s* p, const float* d_g0);
+int gen_set_estimate_spectrum(cpra_plan_s* p, const float* d_G0);
 int gen_iterate(cpra_plan_s* p, int k, float beta);
 int gen_prereconstruct(cpra_plan_s* p, int n, int k, float beta);
 int gen_get_projections(cpra_plan_s* p, int which, float* d_out);

@@ -50,19 +50,22 @@ def native_amplitudes(intensity, mask):
     return torch.roll(A, shifts=(-(N // 2), -(N // 2)), dims=(-2, -1)).contiguous()
 
 
-def random_phase_starts(plan, intensity, mask, seed: int, amplitudes=None):
-    """Random-phase starts g0 = F^-1[M sqrt(I) e^{i phi}], phi ~ U[0, 2 pi) per pixel (reading A15; "random
-    initial guess") for a stack: intensity fp32 [n, N, N] detector-centred, mask u8 [n, N, N] or None, n = plan.Np
-    (or amplitudes = native_amplitudes(intensity, mask), computed once for many restarts).  The phases come from
-    torch's generator on the device (input generation); the transform is the library's own cpra_fft2.
-    Returns complex64 [n, N, N]."""
+def random_phase_spectra(intensity, mask, seed: int, amplitudes=None):
+    """G0 = M sqrt(I) e^{i phi}, phi ~ U[0, 2 pi) per pixel (reading A15; "random initial guess"), native
+    order, complex64 [n, N, N]: the spectrum of a random start (input generation: torch's generator on the device).
+    amplitudes = native_amplitudes(intensity, mask), computed once for many restarts."""
     import torch
     A = native_amplitudes(intensity, mask) if amplitudes is None else amplitudes
     gen = torch.Generator(device=A.device)
     gen.manual_seed(int(seed))
     phi = torch.rand(A.shape, generator=gen, device=A.device, dtype=torch.float32)
     phi.mul_(2.0 * math.pi)
-    return plan.fft2(torch.polar(A, phi), +1)
+    return torch.polar(A, phi)
+
+
+def random_phase_starts(plan, intensity, mask, seed: int, amplitudes=None):
+    """Random-phase starts g0 = F^-1[G0] of random_phase_spectra, through the library's own cpra_fft2; complex64 [n, N, N]."""
+    return plan.fft2(random_phase_spectra(intensity, mask, seed, amplitudes), +1)
 
 
 def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, n_pre: int, n_episodes: int, n_ei: int,
@@ -104,9 +107,10 @@ def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, 
         pa.set_update(update)
         I0 = intensity[:1].expand(n_restarts, N, N).contiguous()
         M0 = None if mask is None else mask[:1].expand(n_restarts, N, N).contiguous()
-        pa.set_estimate(random_phase_starts(pa, I0, M0, seed))
+        pa.set_estimate_spectrum(random_phase_spectra(I0, M0, seed))
         pa.iterate(n_pre, beta)
-        pre = pa.get_projections(binding.ITERATE)
+        # the restarts take their projection 0 from here: as spectra, which is how the starts are handed over
+        pre = pa.fft2(pa.get_projections(binding.ITERATE), -1)
         pa.close()
     timed("step_a", t0)
 
@@ -121,10 +125,10 @@ def reconstruct(intensity, mask, support, angles, n_restarts: int, n_keep: int, 
     amplitudes = native_amplitudes(intensity, mask)
     for r in range(n_restarts):
         plan.set_support(support)
-        g0 = random_phase_starts(plan, intensity, mask, seed + 7919 * (r + 1), amplitudes)
+        G0 = random_phase_spectra(intensity, mask, seed + 7919 * (r + 1), amplitudes)
         if pre is not None:
-            g0[0] = pre[r]
-        plan.set_estimate(g0)
+            G0[0] = pre[r]
+        plan.set_estimate_spectrum(G0)
         for _ in range(n_episodes):
             plan.iterate(n_ei, beta)
             if shrinkwrap is not None:

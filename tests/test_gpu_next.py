@@ -442,6 +442,26 @@ def test_fft2_mixed_radix(torch_cuda, N):
     assert np.abs(Fd[1] - np.exp(-2j * np.pi * (3 * ky + 5 * kx) / N)).max() < 2e-5
 
 
+@pytest.mark.parametrize("N,Np", [(64, 5), (256, 4), (512, 3), (1024, 2), (160, 3), (700, 2)])
+def test_set_estimate_spectrum(torch_cuda, N, Np):
+    """cpra_set_estimate_spectrum: the start given as its spectrum equals the inverse transform handed to
+    cpra_set_estimate, and the loop runs on from it like the oracle's."""
+    p = cpra_inputs.random_stack(N, Np, seed=40 + N, beamstop=3)
+    rng = np.random.default_rng(N)
+    G0 = (rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))).astype(np.complex64)
+    g0 = np.fft.ifft2(G0.astype(np.complex128))
+    alpha = (0.6, 0.2) if Np >= 3 else (1.0,)
+    g = _gpu(p, alpha)
+    g.set_estimate_spectrum(torch_cuda.from_numpy(G0).cuda())
+    assert g.iteration == 0
+    assert rel_l2(_get(g), g0) <= 4e-6 if N < 700 else 6e-6
+    p.estimate = g0.astype(np.complex64)
+    o = _oracle(p, alpha)
+    o.iterate(2, 0.9)
+    g.iterate(2, 0.9)
+    assert rel_l2(_get(g), o.get_projections(0)) <= 3 * TOL_1
+
+
 def test_fft2_every_supported_mixed_radix_size(torch_cuda):
     """Every even N in [16, 1024] with prime factors 2, 3, 5, 7 that is not a power of two (every combination of stage
     radices, ragged last tiles on both tile widths): forward transform of one random image against numpy, round trip."""
