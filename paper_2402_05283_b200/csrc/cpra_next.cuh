@@ -305,12 +305,23 @@ __global__ void k_refine_replace(float2* __restrict__ T, const float2* __restric
     __shared__ double red[32];
     const size_t per = (n3 + gridDim.x - 1) / gridDim.x, i0 = (size_t)blockIdx.x * per, i1 = min(n3, i0 + per);
     double acc = 0.0;
-    for (size_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
-        if (W[i] > 0.f) {
-            const float2 e = E[i], t = T[i];
-            const double dr = (double)t.x - (double)e.x, di = (double)t.y - (double)e.y;
-            acc += dr * dr + di * di;
-            T[i] = e;
+    // four elements per pass, their loads issued together (the order of the additions is the element order, as before)
+    for (size_t i = i0 + threadIdx.x; i < i1; i += (size_t)4 * blockDim.x) {
+        float w[4];
+        float2 e[4], t[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const size_t k = i + (size_t)u * blockDim.x;
+            w[u] = 0.f;
+            if (k < i1) { w[u] = W[k]; e[u] = E[k]; t[u] = T[k]; }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (w[u] > 0.f) {
+                const double dr = (double)t[u].x - (double)e[u].x, di = (double)t[u].y - (double)e[u].y;
+                acc += dr * dr + di * di;
+                T[i + (size_t)u * blockDim.x] = e[u];
+            }
         }
     }
     acc = block_sum(acc, red);
