@@ -5,8 +5,6 @@
 
 namespace cpra {
 
-__device__ __forceinline__ float2 cm(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-
 // two lines (w, w + 1) as one packed value: the 16 bytes (re_w, im_w, re_w1, im_w1) of shared memory <-> c2
 __device__ __forceinline__ c2 gen_ld2(const float2* p) { const float4 q = *reinterpret_cast<const float4*>(p); return c2{make_float2(q.x, q.z), make_float2(q.y, q.w)}; }
 __device__ __forceinline__ void gen_st2(float2* p, c2 v) { *reinterpret_cast<float4*>(p) = make_float4(v.re.x, v.im.x, v.re.y, v.im.y); }
