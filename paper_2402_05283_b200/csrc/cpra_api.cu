@@ -301,8 +301,10 @@ int cpra_iterate(cpra_plan_t p, int k, float beta)
     if (p->generic) return gen_iterate(p, k, beta);
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     const int chunk = (p->chunk > 0 && !(p->flags & CPRA_FLAG_NO_CHUNKING)) ? std::min(p->chunk, p->Np) : p->Np;
-    // the walking kernel serves the default carousel (K = 1 every iteration) on plans with 8-row tiles
-    if (k > 0 && p->walk && p->cluster <= 0 && p->have_tmap && chunk == p->Np && p->K == 1 && p->Np >= 3) {
+    // the walking kernel serves the default carousel (K = 1) and the uncoupled loop (K = 0 with alpha_0 = 1: the batched
+    // pre-reconstructions of Step A) on plans with 8-row tiles
+    const bool uncoupled = p->K == 0 && p->alpha[0] == 1.0f;
+    if (k > 0 && p->walk && p->cluster <= 0 && p->have_tmap && chunk == p->Np && (p->K == 1 || uncoupled) && p->Np >= 3) {
         int rc = CPRA_ERR_UNSUPPORTED_SIZE;
         { auto f = [&]() -> int { CPRA_DISPATCH_N(p->N, if constexpr (walk_ok<NN>()) rc = Launch<NN>::iterate_walk(p, k, beta, scale)); return 0; }; f(); }
         if (rc != CPRA_ERR_UNSUPPORTED_SIZE) return rc;

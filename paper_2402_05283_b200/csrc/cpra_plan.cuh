@@ -402,7 +402,8 @@ int Launch<N>::iterate_walk(cpra_plan_s* p, int k, float beta, float scale)
 {
     float4* g = p->st[p->cur];
     float4* other = p->st[p->cur ^ 1];
-    auto fires = [&](long t) { return (t % p->n_ei) == 0; };   // does the carousel mix open iteration t (reading A3)
+    // does the carousel mix open iteration t (reading A3); never for the uncoupled loop (K = 0, alpha_0 = 1)
+    auto fires = [&](long t) { return p->K == 1 && (t % p->n_ei) == 0; };
     int rc = row_fwd(p, g, fires(p->t) ? MIX_K1 : MIX_NONE, 0, p->Np, other);
     float4 *sin = p->scr, *sout = p->scr2, *gh_old = other, *gh_new = g;
     for (int it = 0; it < k && rc == CPRA_OK; ++it) {

@@ -422,6 +422,26 @@ def test_walk_and_tile_kernel_paths_agree(torch_cuda, N, n_ei):
     assert abs(Ega - Egb) <= 1e-5 * Egb
 
 
+@pytest.mark.parametrize("N", [256, 512, 1024])
+def test_uncoupled_loop_through_the_fused_row_kernel(torch_cuda, N):
+    """K = 0, alpha_0 = 1 (the batched pre-reconstructions of Step A): the fused inverse-row / forward-row kernel runs
+    with weights (1, 0); against the oracle and against the three tile kernels."""
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(N, 4, seed=900 + N, beamstop=3)
+    o = _oracle(p, (1.0,))
+    a = _gpu(p, (1.0,))
+    b = _gpu(p, (1.0,), flags=cpra.FLAG_NO_WALK)
+    for plan in (o, a, b):
+        plan.iterate(3, 0.9)
+    ref = o.get_projections(0)
+    assert rel_l2(_get(a), ref) <= 3 * TOL_1
+    assert rel_l2(_get(a), _get(b)) <= 2e-6
+    assert a.launch_count < b.launch_count                       # two launches per steady-state iteration instead of three
+    Eo, Ego = o.get_error()
+    E, Eg = _errors(a)
+    assert np.abs(E - Eo).max() <= TOL_E * Eo.max() and abs(Eg - Ego) <= TOL_E * Ego
+
+
 @pytest.mark.parametrize("N,Np,ctas", [(256, 180, 0), (256, 90, 6), (512, 60, 8), (1024, 20, 1)])
 def test_walk_short_runs_repeat_exactly(torch_cuda, N, Np, ctas):
     """Many short runs per launch (every run start refills a slot that ordinary stores have just written: the order of
