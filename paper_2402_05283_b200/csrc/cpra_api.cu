@@ -189,7 +189,11 @@ int cpra_set_data(cpra_plan_t p, const float* d_I, const unsigned char* d_mask, 
     for (int n = 0; n < p->Np; ++n) p->angles[n] = h_angles ? h_angles[n] : 0.0;
     if (p->generic) { if (int rc = gen_set_data(p, d_I, d_mask)) return rc; }
     else {
-        k_set_data<<<p->Np, 256, 0, p->stream>>>(d_I, d_mask, p->A, p->den, p->geo);
+        static_assert(SET_DATA_SPLIT <= 8, "the band sums use the error scratch: Np max(N / 4 + 1, 8) doubles (layout_of)");
+        double* part = p->partial;
+        k_set_data<<<p->Np * SET_DATA_SPLIT, 256, 0, p->stream>>>(d_I, d_mask, p->A, part, p->geo);
+        if (int rc = check_launch(p)) return rc;
+        k_set_data_den<<<blocks_for(p->Np, 128), 128, 0, p->stream>>>(part, p->den, p->Np);
         if (int rc = check_launch(p)) return rc;
     }
     p->have_data = true;

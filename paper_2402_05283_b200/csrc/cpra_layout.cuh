@@ -29,12 +29,16 @@ __device__ __forceinline__ void st_c(float* __restrict__ a, size_t i, float2 v) 
 
 // A0: A = sqrt(max(I, 0)) (A14), mask folded in as A = -1, detector-centred ->
 // native (ifftshift, A11) -> the permuted order of the FFT kernels; den_n = sum_{M=1} max(I, 0).
+// SET_DATA_SPLIT blocks per image, each a band of rows; the band sums go to part[n][band] and k_set_data_den adds
+// them in band order (fixed order: deterministic).
+constexpr int SET_DATA_SPLIT = 8;
 __global__ void k_set_data(const float* __restrict__ I, const unsigned char* __restrict__ mask,
-                           float* __restrict__ Aperm, double* __restrict__ den, Geo g)
+                           float* __restrict__ Aperm, double* __restrict__ part, Geo g)
 {
-    const int n = blockIdx.x, N = g.N, h = N / 2;
+    const int n = blockIdx.x / SET_DATA_SPLIT, band = blockIdx.x % SET_DATA_SPLIT, N = g.N, h = N / 2;
+    const int rows = (N + SET_DATA_SPLIT - 1) / SET_DATA_SPLIT, y0 = band * rows, y1 = min(N, y0 + rows);
     double acc = 0.0;
-    for (int i = threadIdx.x; i < N * N; i += blockDim.x) {
+    for (int i = y0 * N + threadIdx.x; i < y1 * N; i += blockDim.x) {
         const int yc = i / N, xc = i % N;
         const size_t src = (size_t)n * N * N + i;
         const float v = fmaxf(I[src], 0.f);
@@ -50,8 +54,16 @@ __global__ void k_set_data(const float* __restrict__ I, const unsigned char* __r
     if (threadIdx.x == 0) {
         double s = 0.0;
         for (int w = 0; w < (int)blockDim.x / 32; ++w) s += red[w];
-        den[n] = s;
+        part[blockIdx.x] = s;
     }
+}
+__global__ void k_set_data_den(const double* __restrict__ part, double* __restrict__ den, int Np)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= Np) return;
+    double s = 0.0;
+    for (int b = 0; b < SET_DATA_SPLIT; ++b) s += part[n * SET_DATA_SPLIT + b];
+    den[n] = s;
 }
 
 // support u8 [n][y][x] -> bit-packed [n][rt][x] u16

@@ -107,7 +107,7 @@ inline Layout layout_of(int N, int Np, bool generic = false)
     L.st1 = c.take(sizeof(float2) * px);
     L.scr = c.take(sizeof(float2) * px);
     L.scr2 = c.take(sizeof(float2) * px);
-    L.partial = c.take(sizeof(double) * (size_t)Np * (N / 4 + 1));   // >= N / Radix<N>::TB (or ceil(N / W)) tiles per image
+    L.partial = c.take(sizeof(double) * (size_t)Np * std::max(N / 4 + 1, 8));   // >= N / Radix<N>::TB (or ceil(N / W)) tiles per image, >= SET_DATA_SPLIT
     L.den = c.take(sizeof(double) * Np);
     L.uphi = c.take(sizeof(double) * 2 * Np);
     L.ustart = c.take(sizeof(int) * (2 * (size_t)Np + 1));
