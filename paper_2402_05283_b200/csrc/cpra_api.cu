@@ -707,7 +707,7 @@ int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsi
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     const size_t n3 = (size_t)p->N * p->N * p->N;
-    const int nblk = (int)std::min<size_t>(512, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
+    const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
     if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
     float2* T = (float2*)p->st[p->cur];   // F, then F' (cpra_fft3 itself uses the other state buffer and the scratch)
     double* num = p->partial;
@@ -740,7 +740,7 @@ int cpra_refine_3d_sw(cpra_plan_t p, const float* d_E, const float* d_W, unsigne
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     const size_t n3 = (size_t)p->N * p->N * p->N;
-    const int nblk = (int)std::min<size_t>(512, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
+    const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
     if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
     float2* T = (float2*)p->st[p->cur];   // F, then F' (cpra_fft3 itself uses the other state buffer and the scratch)
     float2* B = (float2*)p->scr2;         // the blurred |O| of a support update (no transform touches the second scratch)
