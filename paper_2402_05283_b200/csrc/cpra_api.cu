@@ -690,6 +690,123 @@ int cpra_align_episode(cpra_plan_t p, float* d_episode, int n_ref, int* d_flips)
     return CPRA_OK;
 }
 
+}  // extern "C"
+
+namespace {
+// Step D's iterations for a power-of-two N with the cube kept in the loop's own layouts: O in the row-tiled state, the
+// spectra F (scratch), E (second scratch) and the weights (spare state buffer) quad by quad in the scratch layout with the
+// planes in position order.  An iteration is z pass (inverse) -> column pass -> row pass with the support as an ER update
+// (outside the support 0) -> row pass -> column pass -> z pass -> replace: no natural-order copy in between.
+// every >= 1: the support update of cpra_refine_3d_sw, with the blur run through the same kernels (F is parked in d_obj).
+int refine_3d_tiled(cpra_plan_s* p, const float* d_E, const float* d_W, const unsigned char* d_S3_in, unsigned char* d_S3_out, int k, int every,
+                    float sigma, float threshold, float* d_obj, float* d_err, float* d_blurred)
+{
+    const int N = p->N;
+    const size_t n3 = (size_t)N * N * N, nq = n3 / 2, total16 = n3 / 16, units = n3 / p->geo.TB;
+    const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (N / 8) / 2);
+    if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
+    float4* O = p->st[p->cur];                       // the object, row-tiled
+    float2* Wq = (float2*)p->st[p->cur ^ 1];         // (w_a, w_b) per quad
+    float4* F = p->scr;                              // the spectrum the transforms work on
+    float4* Eq = p->scr2;                            // the assembled spectrum
+    double* num = p->partial;
+    double* den = p->partial + nblk;
+    const int PB = spectrum_rows_per_block(N);
+    const unsigned rows = (unsigned)((size_t)N * (N / PB));
+    const int saved_update = p->update;
+    int rc = CPRA_OK;
+    auto launch = [&]() { return (rc = check_launch(p)) == CPRA_OK; };
+    auto run = [&](auto&& f) { f(); return rc == CPRA_OK; };
+    auto dispatch = [&](auto&& body) { auto f = [&]() -> int { CPRA_DISPATCH_N(N, body(std::integral_constant<int, NN>{})); return 0; }; f(); };
+    (void)run;
+    // layouts: support bits, E and W quad by quad with the planes in position order; O starts as zeros (it is only ever
+    // multiplied by 0 before the first row pass overwrites it)
+    k_pack_support<<<blocks_for(total16, 256), 256, 0, p->stream>>>(d_S3_in, p->S16, N, total16);
+    if (!launch()) return rc;
+    k_pack_spectrum<<<rows, 256, sizeof(float2) * N * PB, p->stream>>>((const float2*)d_E, (float*)Eq, p->geo, 1);
+    if (!launch()) return rc;
+    // (the row pass reads the weights' buffer as the "previous state" it multiplies by 0: all of it must be finite)
+    if (cudaMemsetAsync(Wq, 0, sizeof(float2) * n3, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    k_pack_weight<<<rows, 256, sizeof(float) * N * PB, p->stream>>>(d_W, Wq, p->geo);
+    if (!launch()) return rc;
+    if (cudaMemsetAsync(O, 0, sizeof(float2) * n3, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    k_refine_init_q<<<nblk, 256, 0, p->stream>>>(Eq, Wq, F, den, nq);
+    if (!launch()) return rc;
+    const float inv3 = 1.0f / ((float)N * (float)N * (float)N);
+    p->update = CPRA_UPDATE_ER;                      // the support step: inside g', outside 0
+    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
+        // O = S3 . F3^-1[F]
+        dispatch([&](auto nn) {
+            constexpr int NN = decltype(nn)::value;
+            rc = Launch<NN>::fftz_scr(p, F, +1, inv3);
+            if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_INV, 0, N, 1.0f);
+            if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, (const float4*)Wq, O, true, MIX_NONE, 0.f, 1.0f, 0, N, nullptr, (const float4*)Wq);
+            // F' = F3[O]
+            if (rc == CPRA_OK) rc = Launch<NN>::row_fwd(p, O, MIX_NONE, 0, N);
+            if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, N, 1.0f);
+            if (rc == CPRA_OK) rc = Launch<NN>::fftz_scr(p, F, -1, 1.0f);
+        });
+        if (rc) break;
+        k_refine_replace_q<<<nblk, 256, 0, p->stream>>>(F, Eq, Wq, num, nq);
+        if (!launch()) break;
+        if (d_err) {
+            k_refine_error<<<1, 1, 0, p->stream>>>(num, den, nblk, d_err + it);
+            if (!launch()) break;
+        }
+        if (every >= 1 && (it + 1) % every == 0 && it + 1 < k) {
+            // S3 <- [ G_sigma * |O| >= threshold max ] (readings A23, A30) through the same kernels; F waits in d_obj
+            if (cudaMemcpyAsync(d_obj, F, sizeof(float2) * n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) { rc = CPRA_ERR_CUDA; break; }
+            k_abs_supported<<<blocks_for(nq, 256), 256, 0, p->stream>>>(O, p->S16, O, p->geo, nq);
+            if (!launch()) break;
+            dispatch([&](auto nn) {
+                constexpr int NN = decltype(nn)::value;
+                rc = Launch<NN>::row_fwd(p, O, MIX_NONE, 0, N);
+                if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, N, 1.0f);
+                if (rc == CPRA_OK) rc = Launch<NN>::fftz_scr(p, F, -1, 1.0f);
+            });
+            if (rc) break;
+            k_gauss3_q<<<8 * p->sms, 256, sizeof(float) * N, p->stream>>>(F, p->geo, nq, sigma);
+            if (!launch()) break;
+            dispatch([&](auto nn) {
+                constexpr int NN = decltype(nn)::value;
+                rc = Launch<NN>::fftz_scr(p, F, +1, inv3);
+                if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_INV, 0, N, 1.0f);
+                if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, O, O, false, MIX_NONE, 0.f, 1.0f, 0, N);
+            });
+            if (rc) break;
+            k_image_max<<<N, 256, 0, p->stream>>>(O, p->mx, p->geo);
+            if (!launch()) break;
+            k_max_final<<<1, 256, 0, p->stream>>>(p->mx, N);
+            if (!launch()) break;
+            k_max_broadcast<<<1, 256, 0, p->stream>>>(p->mx, N);
+            if (!launch()) break;
+            if (d_blurred) {
+                k_unpack_real<<<blocks_for(n3, 256), 256, 0, p->stream>>>((const float*)O, d_blurred, p->geo, n3);
+                if (!launch()) break;
+            }
+            k_threshold_pack<<<blocks_for(total16, 256), 256, 0, p->stream>>>((const float*)O, p->mx, p->S16, p->geo, total16, threshold);
+            if (!launch()) break;
+            if (d_S3_out) {
+                k_unpack_support<<<blocks_for(n3, 256), 256, 0, p->stream>>>(p->S16, d_S3_out, N, n3);
+                if (!launch()) break;
+            }
+            if (cudaMemcpyAsync(F, d_obj, sizeof(float2) * n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) { rc = CPRA_ERR_CUDA; break; }
+        }
+    }
+    p->update = saved_update;
+    if (rc == CPRA_OK) {
+        k_unpack_state<<<blocks_for(units, 256), 256, 0, p->stream>>>((const float*)O, p->S16, (float2*)d_obj, p->geo, units, 0);
+        rc = check_launch(p);
+    }
+    p->have_estimate = false;   // the state buffers, the scratch and the packed support were used
+    p->have_support = false;
+    p->have_error = false;
+    return rc;
+}
+}  // namespace
+
+extern "C" {
+
 int cpra_fft3(cpra_plan_t p, const float* d_in, float* d_out, int sign)
 {
     if (!p || !d_in || !d_out || (sign != 1 && sign != -1)) return CPRA_ERR_INVALID_ARG;
@@ -706,6 +823,7 @@ int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsi
     if (!p || !d_E || !d_W || !d_S3 || !d_obj || k < 1) return CPRA_ERR_INVALID_ARG;
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
+    if (!p->generic) return refine_3d_tiled(p, d_E, d_W, d_S3, nullptr, k, 0, 0.f, 0.f, d_obj, d_err, nullptr);
     const size_t n3 = (size_t)p->N * p->N * p->N;
     const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
     if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
@@ -739,6 +857,7 @@ int cpra_refine_3d_sw(cpra_plan_t p, const float* d_E, const float* d_W, unsigne
         return CPRA_ERR_INVALID_ARG;
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
+    if (!p->generic) return refine_3d_tiled(p, d_E, d_W, d_S3, d_S3, k, every, sigma, threshold, d_obj, d_err, d_blurred);
     const size_t n3 = (size_t)p->N * p->N * p->N;
     const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
     if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;

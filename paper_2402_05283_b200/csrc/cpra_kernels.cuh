@@ -821,4 +821,55 @@ k_fft_z(float2* __restrict__ vol, const float2* __restrict__ twg, float scale)
     }
 }
 
+// The same z pass on a cube kept in the loop's own layouts (Step D's iterations, cpra_refine_3d): plane z of the cube is
+// image z of the column-tiled scratch, so the z line of (column tile ct, scratch row `row`, pair j) is the quad
+// scr[((z NCT + ct) N + row) NP + j], z = 0 .. N-1: the tile [z][NP] arrives as quads already.  The forward pass leaves
+// frequency kz in plane pos(kz) and the inverse pass expects it there: the cube's planes stay in position order between
+// the two, so nothing is permuted.  grid = (N rows, N / TB column tiles).
+template <int N, bool INV>
+__global__ void __launch_bounds__(Radix<N>::NT)
+k_fft_z_scr(float4* __restrict__ scr, const float2* __restrict__ twg, float scale)
+{
+    using RX = Radix<N>;
+    constexpr int TBN = tile_batch<N>(), NP = tile_pairs<N>(), NT = RX::NT, RL = last_radix<N>(), NCT = N / TBN;
+    extern __shared__ __align__(128) float4 sm[];
+    float4* __restrict__ tile = sm;
+    float2* tw0 = reinterpret_cast<float2*>(sm + tile_quads<N>());
+    const float2* tw1 = tw0 + tw_count_stage0<N>();
+    const size_t plane = (size_t)NCT * N * NP;                                  // quads per plane
+    float4* __restrict__ line = scr + ((size_t)blockIdx.y * N + blockIdx.x) * NP;   // (ct = blockIdx.y, row = blockIdx.x), plane 0
+    for (int i = threadIdx.x; i < tw_count<N>(); i += NT) tw0[i] = twg[i];
+    constexpr int PER = N * NP / NT, UB = PER % 8 == 0 ? 8 : (PER % 4 == 0 ? 4 : 1);
+    static_assert(PER * NT == N * NP, "whole loads per thread");
+    for (int b = 0; b < PER; b += UB) {
+        float4 a[UB];
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int i = (int)threadIdx.x + (b + u) * NT;
+            a[u] = line[(size_t)(i / NP) * plane + i % NP];
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) tile[(int)threadIdx.x + (b + u) * NT] = a[u];
+    }
+    __syncthreads();
+    auto ld_s = [&](int p, int j) -> c2 { return from_quad(tile[p * NP + j]); };
+    auto st_s = [&](int p, int j, c2 v) { st_quad(tile + p * NP + j, v); };
+    if constexpr (!INV) {
+        fft_stage<N, RX::R0, N, false, NT, 1>(tw0, ld_s, st_s);
+        __syncthreads();
+        if constexpr (RX::S == 3) { fft_stage<N, RX::R1, N / RX::R0, false, NT, 1>(tw1, ld_s, st_s); __syncthreads(); }
+        fft_stage<N, RL, RL, false, NT, 1>(tw0, ld_s, st_s);
+    } else {
+        fft_stage<N, RL, RL, true, NT, 1>(tw0, ld_s, st_s);
+        __syncthreads();
+        if constexpr (RX::S == 3) { fft_stage<N, RX::R1, N / RX::R0, true, NT, 1>(tw1, ld_s, st_s); __syncthreads(); }
+        fft_stage<N, RX::R0, N, true, NT, 1>(tw0, ld_s, st_s);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < N * NP; i += NT) {
+        const float4 q = tile[i];
+        line[(size_t)(i / NP) * plane + i % NP] = make_float4(q.x * scale, q.y * scale, q.z * scale, q.w * scale);
+    }
+}
+
 }  // namespace cpra

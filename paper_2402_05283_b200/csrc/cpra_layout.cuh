@@ -173,12 +173,14 @@ __global__ void k_unpack_spectrum(const float* __restrict__ scr, float2* __restr
         for (int x = threadIdx.x; x < N; x += blockDim.x) dst[x] = rowbuf[r * N + x];
     }
 }
-__global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict__ scr, Geo g)
+// zperm (a cube of N planes, Step D): plane n of the natural array goes to plane pos(n) of the scratch
+__global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict__ scr, Geo g, int zperm = 0)
 {
     extern __shared__ __align__(16) float2 rowbuf[];
     const int N = g.N, tb = g.TB, np = tb / 2, nct = N / tb, PB = spectrum_rows_per_block(N);
     const int py0 = (int)(blockIdx.x % (N / PB)) * PB;
     const size_t n = blockIdx.x / (N / PB);
+    const size_t nd = zperm ? (size_t)fft_pos((int)n, g.R0, g.R1, g.R2) : n;
     for (int r = 0; r < PB; ++r) {
         const float2* __restrict__ src = in + (n * N + fft_unpos(py0 + r, g.R0, g.R1, g.R2)) * N;
         for (int x = threadIdx.x; x < N; x += blockDim.x) rowbuf[r * N + x] = src[x];
@@ -193,7 +195,31 @@ __global__ void k_pack_spectrum(const float2* __restrict__ in, float* __restrict
         const int px = ct * tb + 2 * sw(slot, py, np);
         const float2* __restrict__ row = rowbuf + (py - py0) * N;
         const float2 a = row[unpos(px)], b = row[unpos(px + 1)];
-        dst[((n * nct + ct) * N + py0 + pp) * np + slot] = make_float4(a.x, b.x, a.y, b.y);
+        dst[((nd * nct + ct) * N + py0 + pp) * np + slot] = make_float4(a.x, b.x, a.y, b.y);
+    }
+}
+// the weights of Step D, float [kz][ky][kx] natural -> one float2 (w_a, w_b) per quad of the scratch layout, planes in
+// position order: what k_pack_spectrum(zperm) does to the spectrum they belong to
+__global__ void k_pack_weight(const float* __restrict__ in, float2* __restrict__ wq, Geo g)
+{
+    extern __shared__ __align__(16) float wrow[];
+    const int N = g.N, tb = g.TB, np = tb / 2, nct = N / tb, PB = spectrum_rows_per_block(N);
+    const int py0 = (int)(blockIdx.x % (N / PB)) * PB;
+    const size_t n = blockIdx.x / (N / PB);
+    const size_t nd = (size_t)fft_pos((int)n, g.R0, g.R1, g.R2);
+    for (int r = 0; r < PB; ++r) {
+        const float* __restrict__ src = in + (n * N + fft_unpos(py0 + r, g.R0, g.R1, g.R2)) * N;
+        for (int x = threadIdx.x; x < N; x += blockDim.x) wrow[r * N + x] = src[x];
+    }
+    __syncthreads();
+    const Unpos unpos(g);
+    const int lnp = ilog2_of(np), lpb = ilog2_of(PB);
+    for (int t = threadIdx.x; t < PB * np * nct; t += blockDim.x) {
+        const int slot = t & (np - 1), pp = (t >> lnp) & (PB - 1), ct = t >> (lnp + lpb);
+        const int py = ppos(py0 + pp, tb, ct & 1);
+        const int px = ct * tb + 2 * sw(slot, py, np);
+        const float* __restrict__ row = wrow + (py - py0) * N;
+        wq[((nd * nct + ct) * N + py0 + pp) * np + slot] = make_float2(row[unpos(px)], row[unpos(px + 1)]);
     }
 }
 // spectrum of the assembly: column-tiled permuted scratch -> natural order, TRANSPOSED: Et[n][ku][kz],

@@ -417,6 +417,87 @@ __global__ void k_threshold3(const float2* __restrict__ b, const float* __restri
     if (blurred) blurred[i] = v;
 }
 
+// Step D's iterations with the cube kept in the loop's own layouts (power-of-two N): the spectrum F, the assembled
+// spectrum E and the weights W live quad by quad in the scratch layout with the planes in position order (k_pack_spectrum
+// / k_pack_weight with zperm), so these run over quads: a = (x, z), b = (y, w) are the two complex numbers of a quad.
+// F = E on the known voxels (W > 0), 0 elsewhere; part[block] = sum over the block's known voxels of |E|^2
+__global__ void k_refine_init_q(const float4* __restrict__ E, const float2* __restrict__ W, float4* __restrict__ F,
+                                double* __restrict__ part, size_t nq)
+{
+    __shared__ double red[32];
+    const size_t per = (nq + gridDim.x - 1) / gridDim.x, i0 = (size_t)blockIdx.x * per, i1 = min(nq, i0 + per);
+    double acc = 0.0;
+    for (size_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+        const float2 w = W[i];
+        const float4 e = E[i];
+        const bool ka = w.x > 0.f, kb = w.y > 0.f;
+        if (ka) acc += (double)e.x * e.x + (double)e.z * e.z;
+        if (kb) acc += (double)e.y * e.y + (double)e.w * e.w;
+        F[i] = make_float4(ka ? e.x : 0.f, kb ? e.y : 0.f, ka ? e.z : 0.f, kb ? e.w : 0.f);
+    }
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = acc;
+}
+// F holds F'; on the known voxels the residual |F' - E|^2 is accumulated and E is put back
+__global__ void k_refine_replace_q(float4* __restrict__ F, const float4* __restrict__ E, const float2* __restrict__ W,
+                                   double* __restrict__ part, size_t nq)
+{
+    __shared__ double red[32];
+    const size_t per = (nq + gridDim.x - 1) / gridDim.x, i0 = (size_t)blockIdx.x * per, i1 = min(nq, i0 + per);
+    double acc = 0.0;
+    for (size_t i = i0 + threadIdx.x; i < i1; i += (size_t)2 * blockDim.x) {
+        float2 w[2];
+        float4 e[2], t[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const size_t k = i + (size_t)u * blockDim.x;
+            w[u] = make_float2(0.f, 0.f);
+            if (k < i1) { w[u] = W[k]; e[u] = E[k]; t[u] = F[k]; }
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const bool ka = w[u].x > 0.f, kb = w[u].y > 0.f;
+            if (!(ka || kb)) continue;
+            if (ka) { const double dr = (double)t[u].x - (double)e[u].x, di = (double)t[u].z - (double)e[u].z; acc += dr * dr + di * di; }
+            if (kb) { const double dr = (double)t[u].y - (double)e[u].y, di = (double)t[u].w - (double)e[u].w; acc += dr * dr + di * di; }
+            F[i + (size_t)u * blockDim.x] = make_float4(ka ? e[u].x : t[u].x, kb ? e[u].y : t[u].y, ka ? e[u].z : t[u].z, kb ? e[u].w : t[u].w);
+        }
+    }
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = acc;
+}
+// the cube's spectrum in the scratch layout, planes in position order, *= exp(-2 pi^2 sigma^2 |k|^2 / N^2): three entries of
+// the table over positions (see k_gauss_filter) per quad
+__global__ void k_gauss3_q(float4* __restrict__ scr, Geo g, size_t nquads, float sigma)
+{
+    extern __shared__ float gtab[];
+    const int N = g.N, tb = g.TB, np = tb / 2;
+    const double c = -2.0 * 9.86960440108935861883 * (double)sigma * (double)sigma / ((double)N * N);
+    for (int k = threadIdx.x; k < N; k += blockDim.x) {
+        const int ks = k < N / 2 ? k : k - N;
+        gtab[fft_pos(k, g.R0, g.R1, g.R2)] = (float)exp(c * (double)ks * (double)ks);
+    }
+    __syncthreads();
+    const size_t per_image = (size_t)N * N / 2;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < nquads; q += (size_t)gridDim.x * blockDim.x) {
+        const int qi = (int)(q % per_image), pz = (int)(q / per_image);
+        const int slot = qi % np, phys = (qi / np) % N, ct = qi / (np * N);
+        const int py = ppos(phys, tb, ct & 1);
+        const int px = ct * tb + 2 * sw(slot, py, np);
+        const float f = gtab[pz] * gtab[py], fa = f * gtab[px], fb = f * gtab[px + 1];
+        float4 v = scr[q];
+        v.x *= fa; v.y *= fb; v.z *= fa; v.w *= fb;
+        scr[q] = v;
+    }
+}
+// mx[i] = mx[0] for all i < n (after k_max_final): the per-image thresholds of k_threshold_pack become one
+__global__ void k_max_broadcast(float* __restrict__ mx, int n)
+{
+    const float m = mx[0];
+    __syncthreads();
+    for (int i = 1 + threadIdx.x; i < n; i += blockDim.x) mx[i] = m;
+}
+
 // ---------------------------------------------------------------------------------------------------
 // f4: the paper's quality metrics: Fourier shell correlation and PRTF.
 // Shell sums are accumulated per block in shared memory and added to the global shell accumulators with

@@ -157,6 +157,7 @@ struct Launch {
     static int iterate_walk(cpra_plan_s* p, int k, float beta, float scale);
     static int image(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale);
     static int fftz(cpra_plan_s* p, float2* vol, int sign);
+    static int fftz_scr(cpra_plan_s* p, float4* scr, int sign, float scale);   // the cube in the scratch layout (Np == N)
     static int image_cl(cpra_plan_s* p, const float4* cur, float4* nxt, int mode, float beta, float scale, int C);
     static bool image_cl_ok(int C);
     static bool has_image() { return image_ok<N>(); }
@@ -222,6 +223,8 @@ int Launch<N>::set_attrs()
     set_attrs_cl<N, 1>(acc); set_attrs_cl<N, 2>(acc); set_attrs_cl<N, 4>(acc); set_attrs_cl<N, 8>(acc); set_attrs_cl<N, 16>(acc);
     acc(allow_smem(k_fft_z<N, false>, SM));
     acc(allow_smem(k_fft_z<N, true>, SM));
+    acc(allow_smem(k_fft_z_scr<N, false>, SM));
+    acc(allow_smem(k_fft_z_scr<N, true>, SM));
     if constexpr (image_ok<N>()) {
         constexpr int ISM = image_smem_bytes<N>();
         acc(allow_smem(k_image<N, MIX_NONE>, ISM));
@@ -451,6 +454,15 @@ int Launch<N>::fftz(cpra_plan_s* p, float2* vol, int sign)
     const dim3 grid((unsigned)(N / tile_batch<N>()), (unsigned)N);
     if (sign < 0) k_fft_z<N, false><<<grid, Radix<N>::NT, smem_bytes<N>(), p->stream>>>(vol, p->tw, 1.0f);
     else k_fft_z<N, true><<<grid, Radix<N>::NT, smem_bytes<N>(), p->stream>>>(vol, p->tw, 1.0f / (float)N);
+    return check_launch(p);
+}
+
+template <int N>
+int Launch<N>::fftz_scr(cpra_plan_s* p, float4* scr, int sign, float scale)
+{
+    const dim3 grid((unsigned)N, (unsigned)(N / tile_batch<N>()));
+    if (sign < 0) k_fft_z_scr<N, false><<<grid, Radix<N>::NT, smem_bytes<N>(), p->stream>>>(scr, p->tw, scale);
+    else k_fft_z_scr<N, true><<<grid, Radix<N>::NT, smem_bytes<N>(), p->stream>>>(scr, p->tw, scale);
     return check_launch(p);
 }
 
