@@ -313,7 +313,9 @@ int cpra_fft3(cpra_plan_t plan, const float* d_in, float* d_out, int sign);
  *   d_S3  u8 [N][N][N], the 3D support (1 = inside), in the object's frame (centre at (N/2, N/2, N/2))
  *   d_obj complex fp32 [N][N][N] out: the object after the last support step
  *   d_err fp32 [k] out or NULL
- * Uses the plan's state buffers as scratch: a loop state held by this plan is lost (Step D runs on its own plan).
+ * Uses the plan's state buffers, both spectrum buffers and its packed support as scratch: a loop state and a support
+ * held by this plan are lost (Step D runs on its own plan).  The cube stays in the library's internal layouts between
+ * the transforms of an iteration; only d_E, d_W, d_S3 and d_obj are natural-order arrays.
  * Errors: INVALID_ARG (Np != N, k < 1, NULL), WORKSPACE, CUDA.
  */
 int cpra_refine_3d(cpra_plan_t plan, const float* d_E, const float* d_W, const unsigned char* d_S3, int k,

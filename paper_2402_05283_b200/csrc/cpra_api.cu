@@ -803,6 +803,69 @@ int refine_3d_tiled(cpra_plan_s* p, const float* d_E, const float* d_W, const un
     p->have_error = false;
     return rc;
 }
+
+// The same for the sizes that are not powers of two: the cube's spectrum, the assembled spectrum and the weights in position
+// order on all three axes (scratch, second scratch, spare state buffer), the object natural in the state buffer.  An
+// iteration is z pass -> column pass -> row pass with the support as an ER update -> row pass -> column pass -> z pass ->
+// replace; the natural-order path needed two conversions and a copy more per iteration.
+int refine_3d_pos(cpra_plan_s* p, const float* d_E, const float* d_W, const unsigned char* d_S3_in, unsigned char* d_S3_out, int k, int every,
+                  float sigma, float threshold, float* d_obj, float* d_err, float* d_blurred)
+{
+    const int N = p->N;
+    const size_t n3 = (size_t)N * N * N;
+    const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (N / 8) / 2);
+    if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
+    float2* O = (float2*)p->st[p->cur];
+    float* Wp = (float*)p->st[p->cur ^ 1];
+    float2* F = (float2*)p->scr;
+    float2* Ep = (float2*)p->scr2;
+    double* num = p->partial;
+    double* den = p->partial + nblk;
+    const int saved_update = p->update;
+    int rc = CPRA_OK;
+    auto launch = [&]() { return (rc = check_launch(p)) == CPRA_OK; };
+    if (cudaMemcpyAsync(p->S8, d_S3_in, n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    // (the weights' buffer doubles as the finite "previous state" that the ER update multiplies by 0: clear all of it)
+    if (cudaMemsetAsync(Wp, 0, sizeof(float2) * n3, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
+    if ((rc = gen_cube_to_pos(p, (const float2*)d_E, Ep))) return rc;
+    if ((rc = gen_cube_to_pos_f(p, d_W, Wp))) return rc;
+    k_refine_init<<<nblk, 256, 0, p->stream>>>(Ep, Wp, F, den, n3);
+    if (!launch()) return rc;
+    p->update = CPRA_UPDATE_ER;
+    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
+        if ((rc = gen_cube_inverse(p, O, true, (const float2*)Wp))) break;       // O = S3 . F3^-1[F]
+        if ((rc = gen_cube_forward(p, O))) break;                                 // F' = F3[O]
+        k_refine_replace<<<nblk, 256, 0, p->stream>>>(F, Ep, Wp, num, n3);
+        if (!launch()) break;
+        if (d_err) {
+            k_refine_error<<<1, 1, 0, p->stream>>>(num, den, nblk, d_err + it);
+            if (!launch()) break;
+        }
+        if (every >= 1 && (it + 1) % every == 0 && it + 1 < k) {
+            // S3 <- [ G_sigma * |O| >= threshold max ] through the same transforms; F waits in d_obj
+            if (cudaMemcpyAsync(d_obj, F, sizeof(float2) * n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) { rc = CPRA_ERR_CUDA; break; }
+            k_abs3<<<blocks_for(n3, 256), 256, 0, p->stream>>>(O, O, n3);
+            if (!launch()) break;
+            if ((rc = gen_cube_forward(p, O))) break;
+            if ((rc = gen_cube_gauss(p, sigma))) break;
+            if ((rc = gen_cube_inverse(p, O, false, nullptr))) break;
+            k_plane_max<<<N, 256, 0, p->stream>>>(O, p->mx, (size_t)N * N);
+            if (!launch()) break;
+            k_max_final<<<1, 256, 0, p->stream>>>(p->mx, N);
+            if (!launch()) break;
+            k_threshold3<<<blocks_for(n3, 256), 256, 0, p->stream>>>(O, p->mx, p->S8, d_blurred, n3, threshold);
+            if (!launch()) break;
+            if (d_S3_out && cudaMemcpyAsync(d_S3_out, p->S8, n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) { rc = CPRA_ERR_CUDA; break; }
+            if (cudaMemcpyAsync(F, d_obj, sizeof(float2) * n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) { rc = CPRA_ERR_CUDA; break; }
+        }
+    }
+    p->update = saved_update;
+    if (rc == CPRA_OK && cudaMemcpyAsync(d_obj, O, sizeof(float2) * n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) rc = CPRA_ERR_CUDA;
+    p->have_estimate = false;
+    p->have_support = false;
+    p->have_error = false;
+    return rc;
+}
 }  // namespace
 
 extern "C" {
@@ -824,29 +887,7 @@ int cpra_refine_3d(cpra_plan_t p, const float* d_E, const float* d_W, const unsi
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->generic) return refine_3d_tiled(p, d_E, d_W, d_S3, nullptr, k, 0, 0.f, 0.f, d_obj, d_err, nullptr);
-    const size_t n3 = (size_t)p->N * p->N * p->N;
-    const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
-    if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
-    float2* T = (float2*)p->st[p->cur];   // F, then F' (cpra_fft3 itself uses the other state buffer and the scratch)
-    double* num = p->partial;
-    double* den = p->partial + nblk;
-    k_refine_init<<<nblk, 256, 0, p->stream>>>((const float2*)d_E, d_W, T, den, n3);
-    int rc = check_launch(p);
-    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
-        if ((rc = cpra_fft3(p, (const float*)T, d_obj, +1))) break;
-        k_refine_support<<<blocks_for(n3, 256), 256, 0, p->stream>>>((float2*)d_obj, d_S3, n3);
-        if ((rc = check_launch(p))) break;
-        if ((rc = cpra_fft3(p, d_obj, (float*)T, -1))) break;
-        k_refine_replace<<<nblk, 256, 0, p->stream>>>(T, (const float2*)d_E, d_W, num, n3);
-        if ((rc = check_launch(p))) break;
-        if (d_err) {
-            k_refine_error<<<1, 1, 0, p->stream>>>(num, den, nblk, d_err + it);
-            rc = check_launch(p);
-        }
-    }
-    p->have_estimate = false;   // the state buffers were used as scratch
-    p->have_error = false;
-    return rc;
+    return refine_3d_pos(p, d_E, d_W, d_S3, nullptr, k, 0, 0.f, 0.f, d_obj, d_err, nullptr);
 }
 
 int cpra_refine_3d_sw(cpra_plan_t p, const float* d_E, const float* d_W, unsigned char* d_S3, int k, int every, float sigma, float threshold,
@@ -858,45 +899,7 @@ int cpra_refine_3d_sw(cpra_plan_t p, const float* d_E, const float* d_W, unsigne
     if (p->Np != p->N) return CPRA_ERR_INVALID_ARG;
     if (int rc = ready(p)) return rc;
     if (!p->generic) return refine_3d_tiled(p, d_E, d_W, d_S3, d_S3, k, every, sigma, threshold, d_obj, d_err, d_blurred);
-    const size_t n3 = (size_t)p->N * p->N * p->N;
-    const int nblk = (int)std::min<size_t>(2048, (size_t)p->Np * (p->N / 8) / 2);   // two rows of partial sums fit the error scratch
-    if (nblk < 1) return CPRA_ERR_UNSUPPORTED_SIZE;
-    float2* T = (float2*)p->st[p->cur];   // F, then F' (cpra_fft3 itself uses the other state buffer and the scratch)
-    float2* B = (float2*)p->scr2;         // the blurred |O| of a support update (no transform touches the second scratch)
-    double* num = p->partial;
-    double* den = p->partial + nblk;
-    k_refine_init<<<nblk, 256, 0, p->stream>>>((const float2*)d_E, d_W, T, den, n3);
-    int rc = check_launch(p);
-    for (int it = 0; it < k && rc == CPRA_OK; ++it) {
-        if ((rc = cpra_fft3(p, (const float*)T, d_obj, +1))) break;
-        k_refine_support<<<blocks_for(n3, 256), 256, 0, p->stream>>>((float2*)d_obj, d_S3, n3);
-        if ((rc = check_launch(p))) break;
-        if ((rc = cpra_fft3(p, d_obj, (float*)T, -1))) break;
-        k_refine_replace<<<nblk, 256, 0, p->stream>>>(T, (const float2*)d_E, d_W, num, n3);
-        if ((rc = check_launch(p))) break;
-        if (d_err) {
-            k_refine_error<<<1, 1, 0, p->stream>>>(num, den, nblk, d_err + it);
-            if ((rc = check_launch(p))) break;
-        }
-        if (every >= 1 && (it + 1) % every == 0 && it + 1 < k) {
-            // S3 <- [ G_sigma * |O| >= threshold max ]  (readings A23, A30)
-            k_abs3<<<blocks_for(n3, 256), 256, 0, p->stream>>>((const float2*)d_obj, B, n3);
-            if ((rc = check_launch(p))) break;
-            if ((rc = cpra_fft3(p, (const float*)B, (float*)B, -1))) break;
-            k_gauss3<<<blocks_for(n3, 256), 256, 0, p->stream>>>(B, p->N, n3, sigma);
-            if ((rc = check_launch(p))) break;
-            if ((rc = cpra_fft3(p, (const float*)B, (float*)B, +1))) break;
-            k_plane_max<<<p->N, 256, 0, p->stream>>>(B, p->mx, (size_t)p->N * p->N);
-            if ((rc = check_launch(p))) break;
-            k_max_final<<<1, 256, 0, p->stream>>>(p->mx, p->N);
-            if ((rc = check_launch(p))) break;
-            k_threshold3<<<blocks_for(n3, 256), 256, 0, p->stream>>>(B, p->mx, d_S3, d_blurred, n3, threshold);
-            rc = check_launch(p);
-        }
-    }
-    p->have_estimate = false;   // the state buffers were used as scratch
-    p->have_error = false;
-    return rc;
+    return refine_3d_pos(p, d_E, d_W, d_S3, d_S3, k, every, sigma, threshold, d_obj, d_err, d_blurred);
 }
 
 int cpra_backproject_support(cpra_plan_t p, unsigned char* d_S3)

@@ -79,11 +79,21 @@ int col(cpra_plan_s* p, int n0, int nimg, int mode, float scale)
     else k_gen_col<2><<<grid, GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, p->A, p->tw, p->partial, p->gg, n0, scale, px, N);
     return check_launch(p);
 }
-int permute(cpra_plan_s* p, const float2* in, float2* out, int to_pos)
+int permute(cpra_plan_s* p, const float2* in, float2* out, int to_pos, int zperm = 0)
 {
     const int N = p->N, nb = (N + GEN_PB - 1) / GEN_PB;
     const size_t sm = sizeof(float2) * GEN_PB * N + sizeof(int) * 2 * N;
-    k_gen_permute<<<(unsigned)(p->Np * nb), 256, sm, p->stream>>>(in, out, p->gg, to_pos);
+    k_gen_permute<float2><<<(unsigned)(p->Np * nb), 256, sm, p->stream>>>(in, out, p->gg, to_pos, zperm);
+    return check_launch(p);
+}
+// the z pass on the cube held in p->scr with its planes in position order (modes 1 / 2 of the column kernel with rows one
+// plane apart): forward natural z -> position order, inverse position order -> natural z
+int zpass_pos(cpra_plan_s* p, int sign)
+{
+    const size_t N = (size_t)p->N;
+    const unsigned grid = (unsigned)(p->N * tiles_of(p));
+    if (sign < 0) k_gen_col<1><<<grid, GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, nullptr, p->tw, nullptr, p->gg, 0, 1.0f, N, N * N);
+    else k_gen_col<2><<<grid, GEN_NT, smem_of(p), p->stream>>>((float2*)p->scr, nullptr, p->tw, nullptr, p->gg, 0, 1.0f, N, N * N);
     return check_launch(p);
 }
 int row_inv(cpra_plan_s* p, const float2* cur, float2* nxt, int n0, int nimg, bool fires, bool hio, float beta, float scale, const float2* ghat)
@@ -226,6 +236,42 @@ int gen_prtf_sums(cpra_plan_s* p, const float* d_avg, double* acc)
     if (rc) return rc;
     if (cudaMemsetAsync(acc, 0, sizeof(double) * 2 * ns, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
     k_gen_prtf_accumulate<<<4 * p->sms, 256, sizeof(double) * 2 * ns, p->stream>>>((const float2*)p->scr, p->A, acc, p->gg, total);
+    return check_launch(p);
+}
+
+// ---- Step D's iterations with the cube in position order on all three axes (cpra_refine_3d on this path; Np == N) ----
+// natural cube -> position order (complex / float)
+int gen_cube_to_pos(cpra_plan_s* p, const float2* in, float2* out) { return permute(p, in, out, 1, 1); }
+int gen_cube_to_pos_f(cpra_plan_s* p, const float* in, float* out)
+{
+    const int N = p->N, nb = (N + GEN_PB - 1) / GEN_PB;
+    const size_t sm = sizeof(float) * GEN_PB * N + sizeof(int) * 2 * N;
+    k_gen_permute<float><<<(unsigned)(N * nb), 256, sm, p->stream>>>(in, out, p->gg, 1, 1);
+    return check_launch(p);
+}
+// O = [support .] F3^-1[spectrum in p->scr] / N^3, natural order: z pass, column pass, row pass; with_support: the row pass
+// applies the plan's support bytes as an ER update (outside 0), `finite` = any buffer of N^3 finite complex numbers (it is
+// read as the previous state and multiplied by 0)
+int gen_cube_inverse(cpra_plan_s* p, float2* O, bool with_support, const float2* finite)
+{
+    const float inv3 = 1.0f / ((float)p->N * (float)p->N * (float)p->N);
+    int rc = zpass_pos(p, +1);
+    if (rc == CPRA_OK) rc = col(p, 0, p->N, 2, 1.0f);
+    if (rc == CPRA_OK) rc = row_inv(p, finite, O, 0, p->N, false, with_support, 0.f, inv3, with_support ? finite : nullptr);
+    return rc;
+}
+// spectrum of the natural cube O into p->scr, position order
+int gen_cube_forward(cpra_plan_s* p, const float2* O)
+{
+    int rc = row_fwd(p, O, 0, p->N, false, false, nullptr);
+    if (rc == CPRA_OK) rc = col(p, 0, p->N, 1, 1.0f);
+    if (rc == CPRA_OK) rc = zpass_pos(p, -1);
+    return rc;
+}
+int gen_cube_gauss(cpra_plan_s* p, float sigma)
+{
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    k_gen_gauss3<<<8 * p->sms, 256, sizeof(float) * p->N, p->stream>>>((float2*)p->scr, p->gg, n3, sigma);
     return check_launch(p);
 }
 

@@ -483,39 +483,43 @@ __global__ void k_gen_transpose(const float2* __restrict__ in, float2* __restric
 // block per (n, GEN_PB consecutive rows of the position-order array): those rows and the natural rows they map to
 // both move coalesced; the permutation along x goes through shared memory with the tables pos / its inverse built
 // once per block.  Dynamic shared memory: GEN_PB N float2 + 2 N int.
+// zperm (a cube of N planes, Step D): the planes are permuted too, natural plane n <-> plane pos(n) of the position-order array.
 constexpr int GEN_PB = 4;
-__global__ void k_gen_permute(const float2* __restrict__ in, float2* __restrict__ out, GenGeo gg, int to_pos)
+template <class T>
+__global__ void k_gen_permute(const T* __restrict__ in, T* __restrict__ out, GenGeo gg, int to_pos, int zperm)
 {
     extern __shared__ __align__(16) unsigned char pm[];
     const int N = gg.N;
-    float2* rows = reinterpret_cast<float2*>(pm);
+    T* rows = reinterpret_cast<T*>(pm);
     int* pos = reinterpret_cast<int*>(rows + (size_t)GEN_PB * N);
     int* inv = pos + N;
     const int nb = (N + GEN_PB - 1) / GEN_PB;
     const int py0 = (int)(blockIdx.x % nb) * GEN_PB, nr = min(GEN_PB, N - py0);
-    const size_t n = blockIdx.x / nb;
+    const size_t n = blockIdx.x / nb;                                  // plane of the position-order array
+    const size_t nn = zperm ? (size_t)-1 : n;                          // plane of the natural array (zperm: inv[n], below)
     for (int k = threadIdx.x; k < N; k += blockDim.x) {
         const int p = gen_pos(k, gg);
         pos[k] = p;
         inv[p] = k;
     }
     __syncthreads();
+    const size_t nnat = zperm ? (size_t)inv[n] : nn;
     if (to_pos) {
         for (int r = 0; r < nr; ++r) {
-            const float2* __restrict__ src = in + (n * N + inv[py0 + r]) * N;
+            const T* __restrict__ src = in + (nnat * N + inv[py0 + r]) * N;
             for (int x = threadIdx.x; x < N; x += blockDim.x) rows[r * N + x] = src[x];
         }
         __syncthreads();
         for (int r = 0; r < nr; ++r) {
-            float2* __restrict__ dst = out + (n * N + py0 + r) * N;
+            T* __restrict__ dst = out + (n * N + py0 + r) * N;
             for (int q = threadIdx.x; q < N; q += blockDim.x) dst[q] = rows[r * N + inv[q]];
         }
     } else {
-        const float2* __restrict__ src = in + (n * N + py0) * N;          // nr rows, contiguous
+        const T* __restrict__ src = in + (n * N + py0) * N;               // nr rows, contiguous
         for (int i = threadIdx.x; i < nr * N; i += blockDim.x) rows[i] = src[i];
         __syncthreads();
         for (int r = 0; r < nr; ++r) {
-            float2* __restrict__ dst = out + (n * N + inv[py0 + r]) * N;
+            T* __restrict__ dst = out + (nnat * N + inv[py0 + r]) * N;
             for (int x = threadIdx.x; x < N; x += blockDim.x) dst[x] = rows[r * N + pos[x]];
         }
     }
@@ -545,6 +549,25 @@ __global__ void k_gen_gauss_filter(float2* __restrict__ scr, GenGeo gg, size_t t
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int px = (int)(i % N), py = (int)((i / N) % N);
         const float f = gtab[py] * gtab[px];
+        float2 v = scr[i];
+        v.x *= f; v.y *= f;
+        scr[i] = v;
+    }
+}
+// the cube's spectrum in position order on all three axes *= exp(-2 pi^2 sigma^2 |k|^2 / N^2)
+__global__ void k_gen_gauss3(float2* __restrict__ scr, GenGeo gg, size_t n3, float sigma)
+{
+    extern __shared__ float gtab[];
+    const int N = gg.N;
+    const double c = -2.0 * 9.86960440108935861883 * (double)sigma * (double)sigma / ((double)N * N);
+    for (int k = threadIdx.x; k < N; k += blockDim.x) {
+        const int ks = k < N / 2 ? k : k - N;
+        gtab[gen_pos(k, gg)] = (float)exp(c * (double)ks * (double)ks);
+    }
+    __syncthreads();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += (size_t)gridDim.x * blockDim.x) {
+        const int px = (int)(i % N), py = (int)((i / N) % N), pz = (int)(i / ((size_t)N * N));
+        const float f = gtab[pz] * gtab[py] * gtab[px];
         float2 v = scr[i];
         v.x *= f; v.y *= f;
         scr[i] = v;

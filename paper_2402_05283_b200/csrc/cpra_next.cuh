@@ -293,11 +293,6 @@ __global__ void k_refine_init(const float2* __restrict__ E, const float* __restr
     acc = block_sum(acc, red);
     if (threadIdx.x == 0) part[blockIdx.x] = acc;
 }
-__global__ void k_refine_support(float2* __restrict__ O, const unsigned char* __restrict__ S3, size_t n3)
-{
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n3 && !S3[i]) O[i] = make_float2(0.f, 0.f);
-}
 // T holds F'; on the known voxels the residual is accumulated and E is put back
 __global__ void k_refine_replace(float2* __restrict__ T, const float2* __restrict__ E, const float* __restrict__ W,
                                  double* __restrict__ part, size_t n3)
@@ -365,18 +360,6 @@ __global__ void k_abs3(const float2* __restrict__ O, float2* __restrict__ out, s
     if (i >= n3) return;
     const float2 v = O[i];
     out[i] = make_float2(sqrtf(v.x * v.x + v.y * v.y), 0.f);
-}
-// natural 3D spectrum *= exp(-2 pi^2 sigma^2 |k|^2 / N^2)
-__global__ void k_gauss3(float2* __restrict__ F, int N, size_t n3, float sigma)
-{
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n3) return;
-    const int ix = (int)(i % N), iy = (int)((i / N) % N), iz = (int)(i / ((size_t)N * N));
-    const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N, kz = iz < N / 2 ? iz : iz - N;
-    const double s = (double)sigma;
-    const float f = (float)exp(-2.0 * 9.86960440108935861883 * s * s * ((double)kz * kz + (double)ky * ky + (double)kx * kx) / ((double)N * N));
-    F[i].x *= f;
-    F[i].y *= f;
 }
 // maximum of the real part of every z plane (one block per plane), then of the planes (one block): mx[0]
 __global__ void k_plane_max(const float2* __restrict__ v, float* __restrict__ mx, size_t px)

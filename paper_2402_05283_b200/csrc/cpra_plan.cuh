@@ -531,7 +531,12 @@ int gen_fft2(cpra_plan_s* p, const float* d_in, float* d_out, int sign);
 int gen_slices(cpra_plan_s* p, float2* Et);
 int gen_fftz(cpra_plan_s* p, float2* vol, int sign);                        // natural [z][y][x], in place
 int gen_shrinkwrap(cpra_plan_s* p, float sigma, float threshold, float* d_blurred);
-int gen_prtf_sums(cpra_plan_s* p, const float* d_avg, double* acc);   // E_n = F[S_n g_n], natural, transposed to [n][ku][kz]
+int gen_prtf_sums(cpra_plan_s* p, const float* d_avg, double* acc);
+int gen_cube_to_pos(cpra_plan_s* p, const float2* in, float2* out);          // Step D in position order (cpra_generic.cu)
+int gen_cube_to_pos_f(cpra_plan_s* p, const float* in, float* out);
+int gen_cube_inverse(cpra_plan_s* p, float2* O, bool with_support, const float2* finite);
+int gen_cube_forward(cpra_plan_s* p, const float2* O);
+int gen_cube_gauss(cpra_plan_s* p, float sigma);   // E_n = F[S_n g_n], natural, transposed to [n][ku][kz]
 
 #define CPRA_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024)
 #ifndef CPRA_INST_N
