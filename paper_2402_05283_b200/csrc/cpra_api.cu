@@ -714,6 +714,7 @@ int refine_3d_tiled(cpra_plan_s* p, const float* d_E, const float* d_W, const un
     const int PB = spectrum_rows_per_block(N);
     const unsigned rows = (unsigned)((size_t)N * (N / PB));
     const int saved_update = p->update;
+    const auto saved_positivity = p->positivity;
     int rc = CPRA_OK;
     auto launch = [&]() { return (rc = check_launch(p)) == CPRA_OK; };
     auto run = [&](auto&& f) { f(); return rc == CPRA_OK; };
@@ -734,6 +735,7 @@ int refine_3d_tiled(cpra_plan_s* p, const float* d_E, const float* d_W, const un
     if (!launch()) return rc;
     const float inv3 = 1.0f / ((float)N * (float)N * (float)N);
     p->update = CPRA_UPDATE_ER;                      // the support step: inside g', outside 0
+    p->positivity = 0;                               // (Step D has no positivity step: reading A26)
     for (int it = 0; it < k && rc == CPRA_OK; ++it) {
         // O = S3 . F3^-1[F]
         dispatch([&](auto nn) {
@@ -794,6 +796,7 @@ int refine_3d_tiled(cpra_plan_s* p, const float* d_E, const float* d_W, const un
         }
     }
     p->update = saved_update;
+    p->positivity = saved_positivity;
     if (rc == CPRA_OK) {
         k_unpack_state<<<blocks_for(units, 256), 256, 0, p->stream>>>((const float*)O, p->S16, (float2*)d_obj, p->geo, units, 0);
         rc = check_launch(p);
@@ -822,6 +825,7 @@ int refine_3d_pos(cpra_plan_s* p, const float* d_E, const float* d_W, const unsi
     double* num = p->partial;
     double* den = p->partial + nblk;
     const int saved_update = p->update;
+    const auto saved_positivity = p->positivity;
     int rc = CPRA_OK;
     auto launch = [&]() { return (rc = check_launch(p)) == CPRA_OK; };
     if (cudaMemcpyAsync(p->S8, d_S3_in, n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) return CPRA_ERR_CUDA;
@@ -832,6 +836,7 @@ int refine_3d_pos(cpra_plan_s* p, const float* d_E, const float* d_W, const unsi
     k_refine_init<<<nblk, 256, 0, p->stream>>>(Ep, Wp, F, den, n3);
     if (!launch()) return rc;
     p->update = CPRA_UPDATE_ER;
+    p->positivity = 0;                               // (Step D has no positivity step: reading A26)
     for (int it = 0; it < k && rc == CPRA_OK; ++it) {
         if ((rc = gen_cube_inverse(p, O, true, (const float2*)Wp))) break;       // O = S3 . F3^-1[F]
         if ((rc = gen_cube_forward(p, O))) break;                                 // F' = F3[O]
@@ -860,6 +865,7 @@ int refine_3d_pos(cpra_plan_s* p, const float* d_E, const float* d_W, const unsi
         }
     }
     p->update = saved_update;
+    p->positivity = saved_positivity;
     if (rc == CPRA_OK && cudaMemcpyAsync(d_obj, O, sizeof(float2) * n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) rc = CPRA_ERR_CUDA;
     p->have_estimate = false;
     p->have_support = false;
