@@ -527,18 +527,16 @@ int cpra_shrinkwrap(cpra_plan_t p, float sigma, float threshold, float* d_blurre
     k_abs_supported<<<blocks_for(nquads, 256), 256, 0, p->stream>>>(p->st[p->cur], p->S16, tmp, p->geo, nquads);
     int rc = check_launch(p);
     if (rc) return rc;
-    { auto f = [&]() -> int {
-        CPRA_DISPATCH_N(p->N,
-            rc = Launch<NN>::row_fwd(p, tmp, MIX_NONE, 0, p->Np);
-            if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, p->Np, 1.0f));
-        return 0; }; f(); }
-    if (rc) return rc;
-    k_gauss_filter<<<8 * p->sms, 256, sizeof(float) * p->N, p->stream>>>(p->scr, p->geo, nquads, sigma);
+    // the transfer function as a table over the scratch positions (the shell scratch: 12 N bytes are there), applied between
+    // the forward and the inverse column pass inside one kernel
+    float* tab = (float*)p->shell;
+    k_gauss_table<<<blocks_for(p->N, 128), 128, 0, p->stream>>>(tab, p->geo, sigma);
     if ((rc = check_launch(p))) return rc;
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     { auto f = [&]() -> int {
         CPRA_DISPATCH_N(p->N,
-            rc = Launch<NN>::col(p, COL_INV, 0, p->Np, 1.0f);
+            rc = Launch<NN>::row_fwd(p, tmp, MIX_NONE, 0, p->Np);
+            if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_GAUSS, 0, p->Np, 1.0f, nullptr, tab);
             if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, tmp, tmp, false, MIX_NONE, 0.f, scale, 0, p->Np));
         return 0; }; f(); }
     if (rc) return rc;

@@ -58,7 +58,7 @@ __device__ __forceinline__ unsigned inside_bits(const MixParams& mp, unsigned bi
 }
 
 enum { MIX_NONE = 0, MIX_K1 = 1, MIX_GEN = 2, MIX_MASK = 3 };
-enum { COL_FULL = 0, COL_FWD = 1, COL_INV = 2 };
+enum { COL_FULL = 0, COL_FWD = 1, COL_INV = 2, COL_GAUSS = 3 };   // COL_GAUSS: forward, times a separable table, inverse (shrink-wrap's blur)
 enum { ROWINV_HIO = 0, ROWINV_PLAIN = 1 };
 
 template <int N> __host__ __device__ constexpr int tile_quads() { return N * tile_pairs<N>(); }
@@ -568,7 +568,7 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
     auto st_s = [&](int p, int j, c2 v) { st_quad(tile + ppos(p, TBN, par) * NP + sw(j, p, NP), v); };
 
     constexpr bool FAST = inner_stages_warp_local<N>();   // 8-wide, inner radices 8 x 8: affine offsets
-    if constexpr (MODE == COL_FULL || MODE == COL_FWD) {
+    if constexpr (MODE == COL_FULL || MODE == COL_FWD || MODE == COL_GAUSS) {
         if constexpr (FAST) stage0_8<N, false, true, NT>(tile, s.tw0, par);
         else fft_stage<N, RX::R0, N, false, NT, 1>(s.tw0, ld_s, st_s);
         __syncthreads();
@@ -618,6 +618,39 @@ k_col(float4* __restrict__ scr, const float* __restrict__ Aperm, const float2* _
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
         if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    }
+    if constexpr (MODE == COL_GAUSS) {
+        // the pointwise step of the blur: Aperm is a table of N floats over the scratch POSITIONS here, the factor of
+        // element (row position py, column position px) is tab[py] tab[px] (cpra_shrinkwrap; reading A23)
+        const float* __restrict__ tab = Aperm;
+        auto pw = [&](c2 (&v)[RL], int q, int j) {
+            const float2 fx = __ldg(reinterpret_cast<const float2*>(tab + ct * TBN + 2 * j));
+#pragma unroll
+            for (int r = 0; r < RL; ++r) {
+                const float fy = __ldg(tab + q * RL + r);
+                const float2 f = make_float2(fy * fx.x, fy * fx.y);
+                v[r].re = pmul(v[r].re, f);
+                v[r].im = pmul(v[r].im, f);
+            }
+        };
+        if constexpr (FAST) {
+            constexpr int NBF = NP * (N / RL), ITERS = (NBF + NT - 1) / NT;
+#pragma unroll 1
+            for (int it = 0; it < ITERS; ++it) {
+                const int bf = (int)threadIdx.x + it * NT, j = bf % NP, q = bf / NP;
+                const Last8<true> at(tile, q, j, par);
+                c2 v[RL];
+#pragma unroll
+                for (int r = 0; r < RL; ++r) v[r] = from_quad(*at(r));
+                dft<RL, false>(v);
+                pw(v, q, j);
+                dft<RL, true>(v);
+#pragma unroll
+                for (int r = 0; r < RL; ++r) st_quad(at(r), v[r]);
+            }
+        } else {
+            fft_stage_mid<N, RL, NT, 1>(ld_s, pw, st_s);
+        }
     }
     if constexpr (MODE == COL_INV) fft_stage<N, RL, RL, true, NT, 1>(s.tw0, ld_s, st_s);
     if constexpr (MODE != COL_FWD) {

@@ -30,30 +30,16 @@ __global__ void k_abs_supported(const float4* __restrict__ st, const uint16_t* _
     const float4 v = st[i];
     out[i] = make_float4((bits & 1) ? sqrtf(v.x * v.x + v.z * v.z) : 0.f, (bits & 2) ? sqrtf(v.y * v.y + v.w * v.w) : 0.f, 0.f, 0.f);
 }
-// spectrum (scratch layout) *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2).  The factor is the product of two entries of a
-// table over the scratch POSITIONS (tab[pos(k)] = exp(-2 pi^2 sigma^2 k^2 / N^2), k signed; built per block in shared
-// memory, N floats), so the kernel walks the scratch quad by quad, coalesced.  Dynamic shared memory: N floats.
-__global__ void k_gauss_filter(float4* __restrict__ scr, Geo g, size_t nquads, float sigma)
+// spectrum (scratch layout) *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2): the factor is the product of two entries of a table
+// over the scratch POSITIONS, tab[pos(k)] = exp(-2 pi^2 sigma^2 k^2 / N^2), k signed, applied by k_col<COL_GAUSS> between its
+// forward and inverse stages
+__global__ void k_gauss_table(float* __restrict__ tab, Geo g, float sigma)
 {
-    extern __shared__ float gtab[];
-    const int N = g.N, tb = g.TB, np = tb / 2;
+    const int N = g.N, k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
     const double c = -2.0 * 9.86960440108935861883 * (double)sigma * (double)sigma / ((double)N * N);
-    for (int k = threadIdx.x; k < N; k += blockDim.x) {
-        const int ks = k < N / 2 ? k : k - N;
-        gtab[fft_pos(k, g.R0, g.R1, g.R2)] = (float)exp(c * (double)ks * (double)ks);
-    }
-    __syncthreads();
-    const size_t per_image = (size_t)N * N / 2;
-    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < nquads; q += (size_t)gridDim.x * blockDim.x) {
-        const int qi = (int)(q % per_image);
-        const int slot = qi % np, phys = (qi / np) % N, ct = qi / (np * N);
-        const int py = ppos(phys, tb, ct & 1);                       // the scratch row stored at this physical row
-        const int px = ct * tb + 2 * sw(slot, py, np);
-        const float f = gtab[py], fa = f * gtab[px], fb = f * gtab[px + 1];
-        float4 v = scr[q];
-        v.x *= fa; v.y *= fb; v.z *= fa; v.w *= fb;
-        scr[q] = v;
-    }
+    const int ks = k < N / 2 ? k : k - N;
+    tab[fft_pos(k, g.R0, g.R1, g.R2)] = (float)exp(c * (double)ks * (double)ks);
 }
 // per-image maximum of the real part of a state-layout stack (one block per image)
 __global__ void k_image_max(const float4* __restrict__ st, float* __restrict__ mx, Geo g)
@@ -450,7 +436,7 @@ __global__ void k_refine_replace_q(float4* __restrict__ F, const float4* __restr
     if (threadIdx.x == 0) part[blockIdx.x] = acc;
 }
 // the cube's spectrum in the scratch layout, planes in position order, *= exp(-2 pi^2 sigma^2 |k|^2 / N^2): three entries of
-// the table over positions (see k_gauss_filter) per quad
+// the table over positions (see k_gauss_table) per quad
 __global__ void k_gauss3_q(float4* __restrict__ scr, Geo g, size_t nquads, float sigma)
 {
     extern __shared__ float gtab[];

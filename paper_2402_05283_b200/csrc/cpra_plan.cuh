@@ -150,7 +150,7 @@ template <int N>
 struct Launch {
     static int set_attrs();
     static int row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int nimg, float4* ghat_out = nullptr);
-    static int col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, float4* scr = nullptr);
+    static int col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, float4* scr = nullptr, const float* table = nullptr);
     static int row_inv(cpra_plan_s* p, const float4* cur, float4* nxt, bool hio, int mode, float beta, float scale, int n0, int nimg,
                        const float4* scr = nullptr, const float4* ghat_in = nullptr);
     static int walk(cpra_plan_s* p, const float4* scr_in, float4* scr_out, const float4* gh_old, float4* gh_new, float beta, bool fires);
@@ -215,6 +215,7 @@ int Launch<N>::set_attrs()
     acc(allow_smem(k_col<N, COL_FULL>, SM));
     acc(allow_smem(k_col<N, COL_FWD>, SM));
     acc(allow_smem(k_col<N, COL_INV>, SM));
+    acc(allow_smem(k_col<N, COL_GAUSS>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_PLAIN, MIX_NONE>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_NONE>, SM));
     acc(allow_smem(k_row_inv<N, ROWINV_HIO, MIX_K1>, SM));
@@ -318,7 +319,7 @@ int Launch<N>::row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int 
 }
 
 template <int N>
-int Launch<N>::col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, float4* scr)
+int Launch<N>::col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, float4* scr, const float* table)
 {
     constexpr int NT = Radix<N>::NT;
     const dim3 grid((unsigned)nimg * (N / tile_batch<N>()));
@@ -328,6 +329,7 @@ int Launch<N>::col(cpra_plan_s* p, int mode, int n0, int nimg, float scale, floa
     switch (mode) {
         case COL_FULL: k_col<N, COL_FULL><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
         case COL_FWD: k_col<N, COL_FWD><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
+        case COL_GAUSS: k_col<N, COL_GAUSS><<<grid, NT, smem, p->stream>>>(scr, table, p->tw, p->partial, n0, scale); break;
         default: k_col<N, COL_INV><<<grid, NT, smem, p->stream>>>(scr, p->A, p->tw, p->partial, n0, scale); break;
     }
     return check_launch(p);
