@@ -521,12 +521,11 @@ int cpra_shrinkwrap(cpra_plan_t p, float sigma, float threshold, float* d_blurre
     if (int rc = ready(p)) return rc;
     if (!p->have_support || !p->have_estimate) return CPRA_ERR_NOT_READY;
     if (p->generic) return gen_shrinkwrap(p, sigma, threshold, d_blurred);
-    const size_t total = (size_t)p->Np * p->N * p->N, nquads = total / 2;
+    const size_t total = (size_t)p->Np * p->N * p->N;
     float4* tmp = p->st[p->cur ^ 1];
-    // |S g| -> forward 2D FT -> Gaussian transfer function -> inverse 2D FT -> per-image maximum -> threshold
-    k_abs_supported<<<blocks_for(nquads, 256), 256, 0, p->stream>>>(p->st[p->cur], p->S16, tmp, p->geo, nquads);
-    int rc = check_launch(p);
-    if (rc) return rc;
+    // |S g| (formed by the row pass as it loads the state) -> forward 2D FT -> Gaussian transfer function -> inverse 2D FT ->
+    // per-image maximum -> threshold
+    int rc = CPRA_OK;
     // the transfer function as a table over the scratch positions (the shell scratch: 12 N bytes are there), applied between
     // the forward and the inverse column pass inside one kernel
     float* tab = (float*)p->shell;
@@ -535,7 +534,7 @@ int cpra_shrinkwrap(cpra_plan_t p, float sigma, float threshold, float* d_blurre
     const float scale = 1.0f / ((float)p->N * (float)p->N);
     { auto f = [&]() -> int {
         CPRA_DISPATCH_N(p->N,
-            rc = Launch<NN>::row_fwd(p, tmp, MIX_NONE, 0, p->Np);
+            rc = Launch<NN>::row_fwd(p, p->st[p->cur], MIX_ABS, 0, p->Np);
             if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_GAUSS, 0, p->Np, 1.0f, nullptr, tab);
             if (rc == CPRA_OK) rc = Launch<NN>::row_inv(p, tmp, tmp, false, MIX_NONE, 0.f, scale, 0, p->Np));
         return 0; }; f(); }
@@ -756,11 +755,9 @@ int refine_3d_tiled(cpra_plan_s* p, const float* d_E, const float* d_W, const un
         if (every >= 1 && (it + 1) % every == 0 && it + 1 < k) {
             // S3 <- [ G_sigma * |O| >= threshold max ] (readings A23, A30) through the same kernels; F waits in d_obj
             if (cudaMemcpyAsync(d_obj, F, sizeof(float2) * n3, cudaMemcpyDeviceToDevice, p->stream) != cudaSuccess) { rc = CPRA_ERR_CUDA; break; }
-            k_abs_supported<<<blocks_for(nq, 256), 256, 0, p->stream>>>(O, p->S16, O, p->geo, nq);
-            if (!launch()) break;
             dispatch([&](auto nn) {
                 constexpr int NN = decltype(nn)::value;
-                rc = Launch<NN>::row_fwd(p, O, MIX_NONE, 0, N);
+                rc = Launch<NN>::row_fwd(p, O, MIX_ABS, 0, N);                      // |S3 O| formed as the row pass loads O
                 if (rc == CPRA_OK) rc = Launch<NN>::col(p, COL_FWD, 0, N, 1.0f);
                 if (rc == CPRA_OK) rc = Launch<NN>::fftz_scr(p, F, -1, 1.0f);
             });

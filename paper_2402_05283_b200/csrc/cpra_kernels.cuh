@@ -57,7 +57,14 @@ __device__ __forceinline__ unsigned inside_bits(const MixParams& mp, unsigned bi
     return bits;
 }
 
-enum { MIX_NONE = 0, MIX_K1 = 1, MIX_GEN = 2, MIX_MASK = 3 };
+enum { MIX_NONE = 0, MIX_K1 = 1, MIX_GEN = 2, MIX_MASK = 3, MIX_ABS = 4 };   // MIX_MASK: S g (assembly); MIX_ABS: (|S g|, 0) (shrink-wrap)
+// (|a|, 0), (|b|, 0) of a pair: sqrt(re^2 + im^2) with one rounding of the sum of squares' product term (fma), as the
+// scalar expression sqrtf(x * x + y * y) compiles
+__device__ __forceinline__ c2 abs_pair(c2 v)
+{
+    const float2 m2 = pfma(v.re, v.re, pmul(v.im, v.im));
+    return c2{make_float2(sqrtf(m2.x), sqrtf(m2.y)), make_float2(0.f, 0.f)};
+}
 enum { COL_FULL = 0, COL_FWD = 1, COL_INV = 2, COL_GAUSS = 3 };   // COL_GAUSS: forward, times a separable table, inverse (shrink-wrap's blur)
 enum { ROWINV_HIO = 0, ROWINV_PLAIN = 1 };
 
@@ -157,7 +164,7 @@ struct MixLoader {
     }
     __device__ __forceinline__ c2 operator()(c2 own, size_t q) const
     {
-        if constexpr (MODE == MIX_NONE || MODE == MIX_MASK) {
+        if constexpr (MODE == MIX_NONE || MODE == MIX_MASK || MODE == MIX_ABS) {
             return own;
         } else if constexpr (MODE == MIX_K1) {
             const c2 m = ldm(q), p = ldp(q);
@@ -382,11 +389,12 @@ k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm
 
     auto ld_first = [&](int x, int j) -> c2 {
         c2 v = mix(from_quad(tile[tq(x, j)]), toff + (size_t)tq(x, j));
-        if constexpr (MODE == MIX_MASK) {
+        if constexpr (MODE == MIX_MASK || MODE == MIX_ABS) {
             const unsigned bits = (unsigned)Srow[x] >> (sshift + 2 * j);
             if (!(bits & 1)) { v.re.x = 0.f; v.im.x = 0.f; }
             if (!(bits & 2)) { v.re.y = 0.f; v.im.y = 0.f; }
         }
+        if constexpr (MODE == MIX_ABS) v = abs_pair(v);
         if (ghat_out) ghat_out[(size_t)n * istride + toff + (size_t)tq(x, j)] = to_quad(v);
         return v;
     };
@@ -436,11 +444,12 @@ k_row_fwd(const float4* __restrict__ cur, const __grid_constant__ CUtensorMap tm
             for (int r = 0; r < R0; ++r) {
                 const int idx = o + r * (M0 * NP);
                 v[r] = mix(from_quad(tile[idx]), toff + (size_t)idx);
-                if constexpr (MODE == MIX_MASK) {
+                if constexpr (MODE == MIX_MASK || MODE == MIX_ABS) {
                     const unsigned bits = (unsigned)Srow[n2 + M0 * r] >> (sshift + 2 * j);
                     if (!(bits & 1)) { v[r].re.x = 0.f; v[r].im.x = 0.f; }
                     if (!(bits & 2)) { v[r].re.y = 0.f; v[r].im.y = 0.f; }
                 }
+                if constexpr (MODE == MIX_ABS) v[r] = abs_pair(v[r]);
                 if (ghat_out) ghat_out[(size_t)n * istride + toff + (size_t)idx] = to_quad(v[r]);
             }
             dft<R0, false>(v);

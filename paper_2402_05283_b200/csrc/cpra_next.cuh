@@ -10,26 +10,9 @@ namespace cpra {
 // ---------------------------------------------------------------------------------------------------
 // f2: shrink-wrap (PAPER.md:82 "2D CSWA" ref [35], :104; reading A23)
 //     b_n = G_sigma * |S_n g_n|,   S_n <- [ b_n >= threshold max b_n ]
-// The blur is a product in Fourier space between the loop's own forward and inverse FFT kernels.
+// The blur is a product in Fourier space between the loop's own forward and inverse FFT kernels: |S g| is formed by the
+// forward row pass as it loads the state (k_row_fwd<MIX_ABS>), the transfer function sits inside the column kernel.
 // ---------------------------------------------------------------------------------------------------
-// state -> (|S g|, 0) in the state layout (one thread per quad)
-__global__ void k_abs_supported(const float4* __restrict__ st, const uint16_t* __restrict__ S16, float4* __restrict__ out,
-                                Geo g, size_t nquads)
-{
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nquads) return;
-    const int np = g.TB / 2;
-    const size_t pos = i / np;                 // (n * NRT + rt) * N + physical position
-    const int j = (int)(i % np);
-    const int x = ppos((int)(pos % g.N), g.TB);
-    const size_t nrt = pos / g.N;              // n * (N / TB) + rt
-    const int rt = (int)(nrt % (g.N / g.TB));
-    const size_t n = nrt / (g.N / g.TB);
-    const int y0 = rt * g.TB + 2 * j;
-    const unsigned bits = (unsigned)S16[(n * (g.N / 16) + y0 / 16) * g.N + x] >> (y0 % 16);
-    const float4 v = st[i];
-    out[i] = make_float4((bits & 1) ? sqrtf(v.x * v.x + v.z * v.z) : 0.f, (bits & 2) ? sqrtf(v.y * v.y + v.w * v.w) : 0.f, 0.f, 0.f);
-}
 // spectrum (scratch layout) *= exp(-2 pi^2 sigma^2 (ky^2 + kx^2) / N^2): the factor is the product of two entries of a table
 // over the scratch POSITIONS, tab[pos(k)] = exp(-2 pi^2 sigma^2 k^2 / N^2), k signed, applied by k_col<COL_GAUSS> between its
 // forward and inverse stages

@@ -212,6 +212,7 @@ int Launch<N>::set_attrs()
     acc(allow_smem(k_row_fwd<N, MIX_K1>, SM));
     acc(allow_smem(k_row_fwd<N, MIX_GEN>, SM));
     acc(allow_smem(k_row_fwd<N, MIX_MASK>, SM));
+    acc(allow_smem(k_row_fwd<N, MIX_ABS>, SM));
     acc(allow_smem(k_col<N, COL_FULL>, SM));
     acc(allow_smem(k_col<N, COL_FWD>, SM));
     acc(allow_smem(k_col<N, COL_INV>, SM));
@@ -312,6 +313,7 @@ int Launch<N>::row_fwd(cpra_plan_s* p, const float4* cur, int mode, int n0, int 
         case MIX_NONE: ROWFWD(MIX_NONE); break;
         case MIX_K1: ROWFWD(MIX_K1); break;
         case MIX_GEN: ROWFWD(MIX_GEN); break;
+        case MIX_ABS: ROWFWD(MIX_ABS); break;
         default: ROWFWD(MIX_MASK); break;
     }
 #undef ROWFWD
