@@ -422,6 +422,31 @@ def test_walk_and_tile_kernel_paths_agree(torch_cuda, N, n_ei):
     assert abs(Ega - Egb) <= 1e-5 * Egb
 
 
+@pytest.mark.parametrize("N,Np,cluster", [(64, 32, 0), (64, 180, 0), (64, 40, 4), (128, 24, 2), (128, 90, 0)])
+def test_whole_image_kernels_repeat_exactly(torch_cuda, N, Np, cluster):
+    """The clustered whole-image kernel (distributed shared memory between the CTAs of an image, programmatic dependent
+    launch from one iteration to the next) and the one-CTA kernel: thirty back-to-back iterations, repeated ten times with
+    the allocator churned in between, give the same bits every time and agree with the three tile kernels."""
+    import paper_2402_05283_b200 as cpra
+    p = cpra_inputs.random_stack(N, Np, seed=N + Np, beamstop=3)
+
+    def run(flags=0):
+        plan = cpra.Plan(N, Np, flags=flags).load(p)
+        if cluster:
+            plan.set_cluster(cluster)
+        plan.iterate(30, 0.9)
+        out = plan.get_projections(0)
+        plan.close()
+        return out
+    first = run()
+    for rep in range(10):
+        junk = torch_cuda.empty(int(3e8), dtype=torch_cuda.uint8, device="cuda").random_()
+        del junk
+        assert torch_cuda.equal(run(), first), rep
+    ref = run(cpra.FLAG_FORCE_MULTIPASS)
+    assert rel_l2(first.cpu().numpy(), ref.cpu().numpy()) <= 1e-3      # 30 iterations of a chaotic map: rounding-level agreement only
+
+
 @pytest.mark.parametrize("N", [256, 512, 1024])
 def test_uncoupled_loop_through_the_fused_row_kernel(torch_cuda, N):
     """K = 0, alpha_0 = 1 (the batched pre-reconstructions of Step A): the fused inverse-row / forward-row kernel runs
