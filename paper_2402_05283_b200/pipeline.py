@@ -58,8 +58,7 @@ def random_phase_spectra(intensity, mask, seed: int, amplitudes=None):
     A = native_amplitudes(intensity, mask) if amplitudes is None else amplitudes
     gen = torch.Generator(device=A.device)
     gen.manual_seed(int(seed))
-    phi = torch.rand(A.shape, generator=gen, device=A.device, dtype=torch.float32)
-    phi.mul_(2.0 * math.pi)
+    phi = torch.empty(A.shape, device=A.device, dtype=torch.float32).uniform_(0.0, 2.0 * math.pi, generator=gen)
     return torch.polar(A, phi)
 
 
