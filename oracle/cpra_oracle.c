@@ -23,8 +23,10 @@
  *                                        S=1: g_n <- g'_n ;  S=0: g_n <- ghat_n - beta g'_n
  *   7. t <- t + 1
  * plus the one-shot Fourier-slice assembly of Step D's first sentence; the
- * interpolation scheme is the polar bilinear gather of DESIGN.md (the paper only says
- * "interpolate"): PARITY UNPINNED for the interpolation error itself.
+ * interpolation scheme is the polar bilinear gather of DESIGN.md (reading A17: the paper only says
+ * "interpolate").  Its steps are pinned (geometry, centring, duplicate rays, and the weights: exact on a
+ * spectrum bilinear in angle and radius); how close the scheme comes to the continuous transform is a
+ * property of the method, measured on an analytic Gaussian, not a parity matter.
  *
  * Pins (tests/test_oracle_*.py): brute-force O(N^4) DFT below (separate code path), numpy.fft,
  * Parseval, shift theorem, Fourier-slice identity, idempotence of the two projections, closed-form
@@ -32,7 +34,8 @@
  * the feedback operand of step 6 under coupling (one-hot stack, nothing measured: (1 - beta) alpha
  * outside the support), the clamp of negative intensities (|F[g']| = 0 there), and the averaging of
  * duplicate rays in the assembly (slices with different constant spectra on a 360 degree scan).
- * Full multi-iteration trajectories have no external pin: PARITY UNPINNED beyond those invariants.
+ * A multi-iteration trajectory is the composition of these pinned steps; the composition itself is pinned by the
+ * closed-form decay over k iterations, the fixed points and the split-call identity, not by an external trajectory.
  *
  * Around the loop (each function below cites its passage and is pinned in tests/test_oracle_next.py):
  * seam flip, blur / shrink-wrap, Step A, centre of mass / bank / merge (Step C), phase gauge and twin chain of an
