@@ -668,3 +668,38 @@ def test_assembly_exact_grid_lines(torch_cuda):
         for k in (1, 2, 7, h - 1):
             for idx in ((kz, 0, k), (kz, 0, N - k), (kz, k, 0), (kz, N - k, 0)):
                 assert abs(vol[idx] - F3[idx]) <= 2e-5 * np.abs(F3).max(), idx
+
+
+@pytest.mark.parametrize("N,Np", [(32, 12), (64, 20), (48, 10), (256, 6)])
+def test_assembly_is_exact_on_a_bilinear_field(torch_cuda, N, Np):
+    """The device assembly against mathematics, not against the oracle: a spectrum that is bilinear in the ray angle and
+    the radius, a + rho (b phi + c) + d kz, must come back exactly (fp32) wherever the bracketing rays do not straddle the
+    0 / 2 pi cut: the interpolation weights, the bracketing, the centring factors and the layout conversions of the tiled
+    gather (N a multiple of 32), of the one-thread-per-(ky, kx) gather (N = 48) and of the mixed-radix path (N = 48)."""
+    import paper_2402_05283_b200 as cpra
+    a, b, c, d = 0.7, 0.31, -0.45, 0.05
+    ang = np.pi * np.arange(Np) / Np
+    k = np.fft.fftfreq(N, 1.0 / N).astype(int)
+    KZ, KU = np.meshgrid(k, k, indexing="ij")
+    G = np.empty((Np, N, N), np.complex64)
+    for n, th in enumerate(ang):
+        phi = np.where(KU >= 0, th, th + np.pi)
+        C = a + np.abs(KU) * (b * phi + c) + d * KZ + 1j * (0.2 + 0.1 * np.abs(KU) * phi)
+        G[n] = np.fft.ifft2(C * (-1.0) ** ((KZ + KU) % 2)).astype(np.complex64)
+    plan = cpra.Plan(N, Np)
+    plan.set_data(torch_cuda.ones((Np, N, N), dtype=torch_cuda.float32, device="cuda"), None, ang)
+    plan.set_support(torch_cuda.ones((Np, N, N), dtype=torch_cuda.uint8, device="cuda"))
+    plan.set_estimate(torch_cuda.from_numpy(G).cuda())
+    vol, w = plan.assemble_3d()
+    vol, w = vol.cpu().numpy(), w.cpu().numpy()
+    Z, Y, X = np.meshgrid(k, k, k, indexing="ij")
+    rho = np.hypot(X, Y)
+    phi = np.mod(np.arctan2(Y, X), 2 * np.pi)
+    want = (a + rho * (b * phi + c) + d * Z + 1j * (0.2 + 0.1 * rho * phi)) * (-1.0) ** ((X + Y + Z) % 2)
+    ok = (rho > 0) & (rho <= N // 2 - 1) & (phi <= ang[-1] + np.pi)
+    assert ok.mean() > 0.6
+    scale = np.abs(want[ok]).max()
+    assert np.abs(vol[ok] - want[ok]).max() <= 3e-5 * scale, np.abs(vol[ok] - want[ok]).max() / scale
+    assert np.all(w[ok] == 1.0) and np.all(w[rho > N // 2 - 1] == 0.0) and np.all(vol[rho > N // 2 - 1] == 0.0)
+    axis = (X == 0) & (Y == 0)
+    assert np.abs(vol[axis] - want[axis]).max() <= 3e-5 * scale
