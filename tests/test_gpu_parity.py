@@ -703,3 +703,87 @@ def test_assembly_is_exact_on_a_bilinear_field(torch_cuda, N, Np):
     assert np.all(w[ok] == 1.0) and np.all(w[rho > N // 2 - 1] == 0.0) and np.all(vol[rho > N // 2 - 1] == 0.0)
     axis = (X == 0) & (Y == 0)
     assert np.abs(vol[axis] - want[axis]).max() <= 3e-5 * scale
+
+
+@pytest.mark.parametrize("N,Np", [(64, 6), (128, 5), (256, 6), (512, 5), (1024, 4), (160, 5)])
+def test_loop_closed_forms_on_the_device(torch_cuda, N, Np):
+    """The device loop against mathematics (every kernel family: whole-image / cluster, tile + fused row, mixed radix).
+    With nothing measured (mask = 0 everywhere) the modulus step is the identity, so one iteration is
+    g <- S ? ghat : ghat - beta ghat:
+      (a) S = 1, stack = cos(2 pi m n / Np) x image: an eigenvector of the carousel, after k iterations
+          (alpha_0 + 2 alpha_1 cos(2 pi m / Np))^k times the start (Eq. (4), PAPER.md:58-62);
+      (b) K = 0: inside the support nothing changes, outside the start decays as (1 - beta)^k (HIO)."""
+    import paper_2402_05283_b200 as cpra
+    rng = np.random.default_rng(N + Np)
+    img = (rng.normal(size=(N, N)) + 1j * rng.normal(size=(N, N))).astype(np.complex64)
+    I = torch_cuda.ones((Np, N, N), dtype=torch_cuda.float32, device="cuda")
+    M0 = torch_cuda.zeros((Np, N, N), dtype=torch_cuda.uint8, device="cuda")
+    k, beta, a0, a1, m = 4, 0.9, 0.6, 0.2, 1
+    # (a)
+    plan = cpra.Plan(N, Np)
+    plan.set_data(I, M0, None)
+    plan.set_support(torch_cuda.ones((Np, N, N), dtype=torch_cuda.uint8, device="cuda"))
+    plan.set_carousel((a0, a1), 1)
+    c = np.cos(2 * np.pi * m * np.arange(Np) / Np).astype(np.float32)
+    g0 = (c[:, None, None] * img[None]).astype(np.complex64)
+    plan.set_estimate(torch_cuda.from_numpy(g0).cuda())
+    plan.iterate(k, beta)
+    lam = a0 + 2 * a1 * np.cos(2 * np.pi * m / Np)
+    assert rel_l2(_get(plan), lam ** k * g0.astype(np.complex128)) <= k * TOL_1
+    E, Eg = _errors(plan)
+    assert Eg == 0.0 and np.all(E == 0.0)                           # nothing measured: den = 0 => E = 0 (reading A9)
+    # (b)
+    S = (rng.uniform(size=(Np, N, N)) < 0.4).astype(np.uint8)
+    g0 = (rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))).astype(np.complex64)
+    plan = cpra.Plan(N, Np)
+    plan.set_data(I, M0, None)
+    plan.set_support(torch_cuda.from_numpy(S).cuda())
+    plan.set_carousel((1.0,), 1)
+    plan.set_estimate(torch_cuda.from_numpy(g0).cuda())
+    plan.iterate(k, beta)
+    want = np.where(S == 1, g0, (1 - beta) ** k * g0.astype(np.complex128))
+    out = _get(plan)
+    assert rel_l2(out[S == 1], want[S == 1]) <= k * TOL_1
+    assert np.linalg.norm(out[S == 0] - want[S == 0]) <= k * TOL_1 * np.linalg.norm(g0[S == 0])
+
+
+@pytest.mark.parametrize("N,Np", [(64, 4), (128, 3), (256, 4), (512, 3), (160, 3)])
+def test_modulus_and_error_closed_forms_on_the_device(torch_cuda, N, Np):
+    """The Fourier-modulus step and the error metric of the device loop against mathematics (numpy's FFT as the judge):
+    with S = 1 and K = 0 one iteration is g <- F^-1[A G / |G|], so |F[g_new]| = A on the measured pixels and F[g_new] = G
+    on the unmeasured ones; and for g = c x (an image whose spectrum has modulus A), E = ||c| - 1|
+    on every projection (reading A9)."""
+    import paper_2402_05283_b200 as cpra
+    rng = np.random.default_rng(3 * N + Np)
+    truth = (rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))).astype(np.complex64)
+    A = np.abs(np.fft.fft2(truth.astype(np.complex128)))                      # native order
+    I_c = np.fft.fftshift(A ** 2, axes=(-2, -1)).astype(np.float32)           # detector-centred intensities
+    mask = np.ones((Np, N, N), np.uint8)
+    mask[:, N // 2 - 2:N // 2 + 3, N // 2 - 2:N // 2 + 3] = 0                  # a 5 x 5 beamstop
+    g0 = (rng.normal(size=(Np, N, N)) + 1j * rng.normal(size=(Np, N, N))).astype(np.complex64)
+    plan = cpra.Plan(N, Np)
+    plan.set_data(torch_cuda.from_numpy(I_c).cuda(), torch_cuda.from_numpy(mask).cuda(), None)
+    plan.set_support(torch_cuda.ones((Np, N, N), dtype=torch_cuda.uint8, device="cuda"))
+    plan.set_carousel((1.0,), 1)
+    plan.set_estimate(torch_cuda.from_numpy(g0).cuda())
+    plan.iterate(1, 0.9)
+    Gn = np.fft.fft2(_get(plan).astype(np.complex128))
+    G0 = np.fft.fft2(g0.astype(np.complex128))
+    meas = np.fft.ifftshift(mask, axes=(-2, -1)).astype(bool)                 # native order
+    An = np.sqrt(np.maximum(np.fft.ifftshift(I_c.astype(np.float64), axes=(-2, -1)), 0.0))
+    assert np.abs(np.abs(Gn)[meas] - An[meas]).max() <= 2e-5 * An.max()
+    big = meas & (np.abs(G0) > 1e-2 * np.abs(G0).max())                        # phases kept (where |G| is not tiny)
+    assert np.abs(np.angle(Gn[big] * np.conj(G0[big]))).max() <= 1e-3
+    assert np.abs(Gn[~meas] - G0[~meas]).max() <= 2e-5 * np.abs(G0).max()
+    # the error metric of that iteration (taken on its input g0), by hand
+    E, Eg = _errors(plan)
+    num = (((np.abs(G0) - An) ** 2) * meas).sum(axis=(1, 2))
+    den = ((An ** 2) * meas).sum(axis=(1, 2))
+    assert np.abs(E - np.sqrt(num / den)).max() <= 1e-4 * np.sqrt(num / den).max()
+    assert abs(Eg - np.sqrt(num.sum() / den.sum())) <= 1e-4 * np.sqrt(num.sum() / den.sum())
+    # g = c x truth: E_n = ||c| - 1|
+    c = 0.8 - 0.3j
+    plan.set_estimate(torch_cuda.from_numpy((c * truth).astype(np.complex64)).cuda())
+    plan.iterate(1, 0.9)
+    E, Eg = _errors(plan)
+    assert np.abs(E - abs(abs(c) - 1)).max() <= 1e-4 and abs(Eg - abs(abs(c) - 1)) <= 1e-4
